@@ -1,0 +1,860 @@
+/*
+ * pd_oracle.c -- fp64 single-threaded CPU ORACLE (test infrastructure, see pd_oracle.h).
+ *
+ * Written from SURVEY.md 8c.2 (steps O0..O7) and the readings A1..A32 of DESIGN.md; the steps it
+ * follows are the ones the paper names in P:L46 / P:L81 / P:L653-657.  Plain C99, one thread, no
+ * blocking, fusion or reordering: every step is the formula of the reading, written out.
+ * Build: gcc -O2 -ffp-contract=off -std=c99 -shared -fPIC (oracle/build.py).
+ */
+#include "pd_oracle.h"
+
+#include <ctype.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define PDO_MAX_EFF_ROWS 32
+#define PDO_PI 3.14159265358979323846
+#define PDO_TWO_PI 6.28318530717958647692
+#define PDO_REL_TOL 1e-6 /* near-edge band of BASELINE.json north_star / SURVEY 8c.4 */
+
+struct pdo_card {
+  char name[64];
+  double bz, radius, half_length, kappa; /* tesla, metres, metres, GeV/(T m)  (reading A1, A2) */
+  int grid_coord;                        /* 0: eta edges, 1: theta edges      (reading A15)    */
+  int n_bins;
+  double *edges;   /* [n_bins+1], ascending */
+  int32_t *nphi;   /* [n_bins]              */
+  int32_t *offset; /* [n_bins] exclusive prefix sum of nphi */
+  int n_towers;
+  int n_eff;
+  double eff[PDO_MAX_EFF_ROWS][5]; /* pt_lo, pt_hi, aeta_lo, aeta_hi, eps   (reading A8)      */
+  int has_cos;
+  double abs_costheta_max; /* reading A9 */
+  double trk_a, trk_b;     /* sigma_rel = sqrt(a^2 + (b pT)^2) */
+  double ecal[3], hcal[3]; /* (C, S, N): sigma = sqrt(C^2 E^2 + S^2 E + N^2)  (reading A20)   */
+  double thr_ecal, thr_hcal;
+};
+
+/* reading A28: every card number is rounded to fp32 at load; the oracle uses the promoted value */
+static double f32(double x) { return (double)(float)x; }
+
+const char *pdo_strerror(int code) {
+  switch (code) {
+    case PDO_OK: return "ok";
+    case PDO_EINVAL: return "invalid argument";
+    case PDO_ECARD: return "unknown card name or malformed card file";
+    case PDO_ECAPACITY: return "output capacity too small";
+    case PDO_EOVERRIDE: return "override outside the near-edge tolerance";
+    default: return "unknown error";
+  }
+}
+
+/* ------------------------------------------------------------------ cards ----------------- */
+
+static int card_alloc_grid(pdo_card *c, int n_bins) {
+  c->n_bins = n_bins;
+  c->edges = (double *)calloc((size_t)n_bins + 1, sizeof(double));
+  c->nphi = (int32_t *)calloc((size_t)n_bins, sizeof(int32_t));
+  c->offset = (int32_t *)calloc((size_t)n_bins, sizeof(int32_t));
+  return (c->edges && c->nphi && c->offset) ? 0 : -1;
+}
+
+static void card_finish(pdo_card *c) {
+  int i, acc = 0;
+  for (i = 0; i <= c->n_bins; ++i) c->edges[i] = f32(c->edges[i]);
+  for (i = 0; i < c->n_bins; ++i) {
+    c->offset[i] = acc;
+    acc += c->nphi[i];
+  }
+  c->n_towers = acc;
+  c->bz = f32(c->bz);
+  c->radius = f32(c->radius);
+  c->half_length = f32(c->half_length);
+  c->kappa = f32(c->kappa);
+  for (i = 0; i < c->n_eff; ++i) {
+    int k;
+    for (k = 0; k < 5; ++k) c->eff[i][k] = f32(c->eff[i][k]);
+  }
+  c->abs_costheta_max = f32(c->abs_costheta_max);
+  c->trk_a = f32(c->trk_a);
+  c->trk_b = f32(c->trk_b);
+  for (i = 0; i < 3; ++i) {
+    c->ecal[i] = f32(c->ecal[i]);
+    c->hcal[i] = f32(c->hcal[i]);
+  }
+  c->thr_ecal = f32(c->thr_ecal);
+  c->thr_hcal = f32(c->thr_hcal);
+}
+
+/* the three efficiency rows of BASELINE.json configs[0] in reading A8 */
+static void card_default_eff(pdo_card *c) {
+  static const double rows[3][5] = {{1.0, INFINITY, 0.0, 1.5, 0.97},
+                                    {1.0, INFINITY, 1.5, 2.5, 0.85},
+                                    {0.1, 1.0, 0.0, 2.5, 0.70}};
+  memcpy(c->eff, rows, sizeof(rows));
+  c->n_eff = 3;
+  c->trk_a = 0.01;
+  c->trk_b = 1.5e-4;
+  c->thr_ecal = 0.5;
+  c->thr_hcal = 1.0;
+  c->kappa = 0.299792458;
+}
+
+static int card_builtin_cms(pdo_card *c) {
+  /* configs[0]: d_eta 0.087, 72 phi bins for |eta|<3; 0.175, 36 phi bins for 3<|eta|<5 (A15) */
+  double pos[48];
+  int n = 0, k, i;
+  for (k = 0; k <= 34; ++k) pos[n++] = (double)k * 0.087;
+  pos[n++] = 3.0;
+  for (k = 1; k <= 11; ++k) pos[n++] = 3.0 + (double)k * 0.175;
+  pos[n++] = 5.0; /* n == 48: 0 plus 47 positive edges */
+  if (card_alloc_grid(c, 94)) return -1;
+  for (i = 0; i < 47; ++i) c->edges[i] = -pos[47 - i];
+  for (i = 0; i <= 47; ++i) c->edges[47 + i] = pos[i];
+  for (i = 0; i < 94; ++i) c->nphi[i] = (i < 12 || i >= 82) ? 36 : 72;
+  c->bz = 3.8;
+  c->radius = 1.29;
+  c->half_length = 3.0;
+  card_default_eff(c);
+  c->ecal[0] = 0.007, c->ecal[1] = 0.07, c->ecal[2] = 0.35;
+  c->hcal[0] = 0.05, c->hcal[1] = 1.5, c->hcal[2] = 0.0;
+  return 0;
+}
+
+static int card_builtin_atlas(pdo_card *c) {
+  /* configs[3]: uniform d_eta 0.1 x 64 phi bins for |eta| < 3.2; unspecified fields inherit cfg0 (A9) */
+  int i;
+  if (card_alloc_grid(c, 64)) return -1;
+  for (i = 0; i <= 64; ++i) c->edges[i] = (double)(i - 32) * 0.1;
+  for (i = 0; i < 64; ++i) c->nphi[i] = 64;
+  c->bz = 2.0;
+  c->radius = 1.15;
+  c->half_length = 3.5;
+  card_default_eff(c);
+  c->ecal[0] = 0.0017, c->ecal[1] = 0.101, c->ecal[2] = 0.0;
+  c->hcal[0] = 0.0302, c->hcal[1] = 0.5205, c->hcal[2] = 0.0;
+  return 0;
+}
+
+static int card_builtin_aleph(pdo_card *c) {
+  /* configs[4]: towers 0.03 rad in theta x 0.03 rad in phi, |cos theta| < 0.98 (A15) */
+  int i;
+  if (card_alloc_grid(c, 92)) return -1;
+  c->grid_coord = 1;
+  c->edges[0] = acos(0.98);
+  for (i = 0; i <= 90; ++i) c->edges[1 + i] = PDO_PI / 2.0 + (double)(i - 45) * 0.03;
+  c->edges[92] = acos(-0.98);
+  for (i = 0; i < 92; ++i) c->nphi[i] = 210;
+  c->bz = 1.5;
+  c->radius = 1.8;
+  c->half_length = 2.5;
+  card_default_eff(c);
+  c->has_cos = 1;
+  c->abs_costheta_max = 0.98;
+  c->ecal[0] = 0.009, c->ecal[1] = 0.18, c->ecal[2] = 0.0;
+  c->hcal[0] = 0.0, c->hcal[1] = 0.85, c->hcal[2] = 0.0;
+  return 0;
+}
+
+/* card text file: "key = v v v ..." lines, '#' comments; keys: name bz radius half_length kappa
+ * grid(eta|theta) edges(+, may repeat) nphi(+, may repeat) eff(5 numbers, repeat per row)
+ * abs_costheta_max track_res(a b) ecal_res(C S N) hcal_res(C S N) ecal_thr hcal_thr */
+static int card_from_file(pdo_card *c, const char *path) {
+  FILE *f = fopen(path, "r");
+  char *line = NULL;
+  size_t cap = 1 << 16;
+  double *edges = NULL, *nphi = NULL;
+  int n_edges = 0, n_nphi = 0, cap_e = 0, cap_n = 0, ok = 1, i;
+  if (!f) return -1;
+  line = (char *)malloc(cap);
+  card_default_eff(c);
+  c->n_eff = 0;
+  while (ok && fgets(line, (int)cap, f)) {
+    char *hash = strchr(line, '#'), *eq, *key, *val, *end;
+    double v[64];
+    int nv = 0;
+    if (hash) *hash = 0;
+    eq = strchr(line, '=');
+    if (!eq) continue;
+    *eq = 0;
+    key = line;
+    while (isspace((unsigned char)*key)) ++key;
+    end = key + strlen(key);
+    while (end > key && isspace((unsigned char)end[-1])) *--end = 0;
+    val = eq + 1;
+    if (!strcmp(key, "name")) {
+      while (isspace((unsigned char)*val)) ++val;
+      strncpy(c->name, val, sizeof(c->name) - 1);
+      end = c->name + strlen(c->name);
+      while (end > c->name && isspace((unsigned char)end[-1])) *--end = 0;
+      continue;
+    }
+    if (!strcmp(key, "grid")) {
+      while (isspace((unsigned char)*val)) ++val;
+      c->grid_coord = !strncmp(val, "theta", 5) ? 1 : 0;
+      continue;
+    }
+    if (!strcmp(key, "edges") || !strcmp(key, "nphi")) {
+      double **arr = !strcmp(key, "edges") ? &edges : &nphi;
+      int *n = !strcmp(key, "edges") ? &n_edges : &n_nphi;
+      int *cp = !strcmp(key, "edges") ? &cap_e : &cap_n;
+      for (;;) {
+        double x = strtod(val, &end);
+        if (end == val) break;
+        if (*n == *cp) {
+          *cp = *cp ? 2 * *cp : 256;
+          *arr = (double *)realloc(*arr, (size_t)*cp * sizeof(double));
+        }
+        (*arr)[(*n)++] = x;
+        val = end;
+      }
+      continue;
+    }
+    for (nv = 0; nv < 64; ++nv) {
+      v[nv] = strtod(val, &end);
+      if (end == val) break;
+      val = end;
+    }
+    if (!strcmp(key, "bz") && nv == 1) c->bz = v[0];
+    else if (!strcmp(key, "radius") && nv == 1) c->radius = v[0];
+    else if (!strcmp(key, "half_length") && nv == 1) c->half_length = v[0];
+    else if (!strcmp(key, "kappa") && nv == 1) c->kappa = v[0];
+    else if (!strcmp(key, "abs_costheta_max") && nv == 1) c->has_cos = 1, c->abs_costheta_max = v[0];
+    else if (!strcmp(key, "track_res") && nv == 2) c->trk_a = v[0], c->trk_b = v[1];
+    else if (!strcmp(key, "ecal_res") && nv == 3) memcpy(c->ecal, v, 3 * sizeof(double));
+    else if (!strcmp(key, "hcal_res") && nv == 3) memcpy(c->hcal, v, 3 * sizeof(double));
+    else if (!strcmp(key, "ecal_thr") && nv == 1) c->thr_ecal = v[0];
+    else if (!strcmp(key, "hcal_thr") && nv == 1) c->thr_hcal = v[0];
+    else if (!strcmp(key, "eff") && nv == 5 && c->n_eff < PDO_MAX_EFF_ROWS)
+      memcpy(c->eff[c->n_eff++], v, 5 * sizeof(double));
+    else ok = 0;
+  }
+  fclose(f);
+  free(line);
+  if (ok && (n_edges < 2 || n_nphi != n_edges - 1)) ok = 0;
+  if (ok && !(c->radius > 0 && c->half_length > 0 && c->kappa > 0)) ok = 0;
+  if (ok && card_alloc_grid(c, n_edges - 1)) ok = 0;
+  if (ok) {
+    for (i = 0; i < n_edges; ++i) c->edges[i] = edges[i];
+    for (i = 0; i < n_nphi; ++i) {
+      c->nphi[i] = (int32_t)nphi[i];
+      if (c->nphi[i] < 1) ok = 0;
+    }
+    for (i = 1; i < n_edges; ++i)
+      if (!((float)edges[i] > (float)edges[i - 1])) ok = 0;
+  }
+  free(edges);
+  free(nphi);
+  return ok ? 0 : -1;
+}
+
+int pdo_load_card(const char *name_or_path, pdo_card **out) {
+  pdo_card *c;
+  int rc;
+  if (!name_or_path || !out) return PDO_EINVAL;
+  c = (pdo_card *)calloc(1, sizeof(pdo_card));
+  if (!c) return PDO_EINVAL;
+  strncpy(c->name, name_or_path, sizeof(c->name) - 1);
+  if (!strcmp(name_or_path, "cms_like")) rc = card_builtin_cms(c);
+  else if (!strcmp(name_or_path, "atlas_like")) rc = card_builtin_atlas(c);
+  else if (!strcmp(name_or_path, "aleph_like")) rc = card_builtin_aleph(c);
+  else rc = card_from_file(c, name_or_path);
+  if (rc) {
+    pdo_free_card(c);
+    return PDO_ECARD;
+  }
+  card_finish(c);
+  *out = c;
+  return PDO_OK;
+}
+
+void pdo_free_card(pdo_card *c) {
+  if (!c) return;
+  free(c->edges);
+  free(c->nphi);
+  free(c->offset);
+  free(c);
+}
+
+int pdo_card_info(const pdo_card *c, pdo_card_info_t *out) {
+  if (!c || !out) return PDO_EINVAL;
+  out->n_towers = c->n_towers;
+  out->n_eta_bins = c->n_bins;
+  out->grid_coord = c->grid_coord;
+  out->bz = (float)c->bz;
+  out->radius = (float)c->radius;
+  out->half_length = (float)c->half_length;
+  out->n_eff_rows = c->n_eff;
+  return PDO_OK;
+}
+
+int pdo_card_grid(const pdo_card *c, double *edges, int32_t *nphi, int32_t *offset) {
+  int i;
+  if (!c) return PDO_EINVAL;
+  for (i = 0; i <= c->n_bins && edges; ++i) edges[i] = c->edges[i];
+  for (i = 0; i < c->n_bins; ++i) {
+    if (nphi) nphi[i] = c->nphi[i];
+    if (offset) offset[i] = c->offset[i];
+  }
+  return PDO_OK;
+}
+
+/* ------------------------------------------------------------------ O0: RNG ---------------- */
+/* Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), as restated in SURVEY 8c.2 O0. */
+
+void pdo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+  int r;
+  for (r = 0; r < 10; ++r) {
+    uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;
+    uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    uint32_t n1 = (uint32_t)p1;
+    uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    uint32_t n3 = (uint32_t)p0;
+    c0 = n0, c1 = n1, c2 = n2, c3 = n3;
+    k0 += W0, k1 += W1;
+  }
+  out[0] = c0, out[1] = c1, out[2] = c2, out[3] = c3;
+}
+
+/* reading A26/A27: key = (seed lo, seed hi); counter = (object, event lo, event hi, stream<<16 | block),
+ * block = 0.  stream 0: object = particle index within its event; stream 1: object = tower id. */
+void pdo_rng_block(uint64_t seed, int64_t event, uint32_t object, uint32_t stream, uint32_t out[4]) {
+  uint32_t ctr[4], key[2];
+  uint64_t ev = (uint64_t)event;
+  ctr[0] = object;
+  ctr[1] = (uint32_t)ev;
+  ctr[2] = (uint32_t)(ev >> 32);
+  ctr[3] = stream << 16;
+  key[0] = (uint32_t)seed;
+  key[1] = (uint32_t)(seed >> 32);
+  pdo_philox4x32_10(ctr, key, out);
+}
+
+double pdo_uniform(uint32_t x) { return (double)(x >> 8) * (1.0 / 16777216.0); }
+double pdo_uniform_pos(uint32_t x) { return ((double)(x >> 8) + 1.0) * (1.0 / 16777216.0); }
+
+/* z = sqrt(-2 ln u+(xa)) cos(2 pi u(xb)) */
+double pdo_normal(uint32_t xa, uint32_t xb) {
+  return sqrt(-2.0 * log(pdo_uniform_pos(xa))) * cos(PDO_TWO_PI * pdo_uniform(xb));
+}
+
+/* reading A21: log-normal with mean m and standard deviation s driven by a standard normal z */
+double pdo_lognormal(double m, double s, double z) {
+  double b2;
+  if (!(m > 0.0)) return 0.0;
+  if (!(s > 0.0)) return m;
+  b2 = log(1.0 + (s * s) / (m * m));
+  return exp(log(m) - 0.5 * b2 + sqrt(b2) * z);
+}
+
+static double resolution(const double csn[3], double E) {
+  return sqrt(csn[0] * csn[0] * E * E + csn[1] * csn[1] * E + csn[2] * csn[2]);
+}
+
+/* ------------------------------------------------------------------ grid ------------------- */
+
+static double tol_angle(double edge) { return PDO_REL_TOL * fmax(1.0, fabs(edge)); }
+
+/* bin i with edges[i] <= coord < edges[i+1]; -1 if outside (reading A16) */
+static int grid_bin(const pdo_card *c, double coord) {
+  int i;
+  if (!(coord >= c->edges[0]) || !(coord < c->edges[c->n_bins])) return -1;
+  for (i = 0; i < c->n_bins; ++i)
+    if (coord < c->edges[i + 1]) return i;
+  return -1;
+}
+
+static int phi_bin(int n, double phi_pos) {
+  int j = (int)floor((phi_pos + PDO_PI) / (PDO_TWO_PI / (double)n));
+  if (j < 0) j = 0;
+  if (j > n - 1) j = n - 1;
+  return j;
+}
+
+int32_t pdo_tower_index(const pdo_card *c, double coord, double phi_pos) {
+  int i = grid_bin(c, coord);
+  if (i < 0) return -1;
+  return c->offset[i] + phi_bin(c->nphi[i], phi_pos);
+}
+
+/* is `tower` an outcome the position (coord, phi) may legitimately take within the tolerance? */
+static int tower_allowed(const pdo_card *c, double coord, double phi_pos, int32_t tower) {
+  int i, j, n;
+  double lo, hi, w, plo, phi_edge_lo, phi_edge_hi, d;
+  if (tower < 0) {
+    if (!(coord == coord)) return 1;
+    return coord < c->edges[0] + tol_angle(c->edges[0]) ||
+           coord >= c->edges[c->n_bins] - tol_angle(c->edges[c->n_bins]);
+  }
+  if (tower >= c->n_towers) return 0;
+  for (i = c->n_bins - 1; i > 0; --i)
+    if (c->offset[i] <= tower) break;
+  j = tower - c->offset[i];
+  n = c->nphi[i];
+  lo = c->edges[i], hi = c->edges[i + 1];
+  if (!(coord >= lo - tol_angle(lo) && coord < hi + tol_angle(hi))) return 0;
+  w = PDO_TWO_PI / (double)n;
+  phi_edge_lo = -PDO_PI + (double)j * w;
+  phi_edge_hi = -PDO_PI + (double)(j + 1) * w;
+  if (phi_pos >= phi_edge_lo - tol_angle(phi_edge_lo) && phi_pos < phi_edge_hi + tol_angle(phi_edge_hi))
+    return 1;
+  /* wrap-around: phi = +pi and phi = -pi are the same direction */
+  plo = phi_pos + PDO_TWO_PI;
+  d = tol_angle(PDO_PI);
+  if (plo >= phi_edge_lo - d && plo < phi_edge_hi + d) return 1;
+  plo = phi_pos - PDO_TWO_PI;
+  if (plo >= phi_edge_lo - d && plo < phi_edge_hi + d) return 1;
+  return 0;
+}
+
+/* near-edge bits of the tower decision (D5) */
+static uint32_t tower_near(const pdo_card *c, double coord, double phi_pos) {
+  uint32_t near = 0;
+  int i = grid_bin(c, coord), k, n;
+  double x, fr, w, e;
+  if (!(coord == coord) || isinf(coord)) return 0;
+  for (k = 0; k <= c->n_bins; ++k)
+    if (fabs(coord - c->edges[k]) <= tol_angle(c->edges[k])) near |= PDO_NEAR_ETA;
+  if (i < 0) {
+    /* outside: the phi bin matters only if the eta decision may flip into the grid */
+    if (!near) return 0;
+    i = coord < c->edges[0] ? 0 : c->n_bins - 1;
+  }
+  for (k = (i > 0 ? i - 1 : 0); k <= (i + 1 < c->n_bins ? i + 1 : c->n_bins - 1); ++k) {
+    if (k != i && !near) continue;
+    n = c->nphi[k];
+    w = PDO_TWO_PI / (double)n;
+    x = (phi_pos + PDO_PI) / w;
+    fr = x - floor(x + 0.5); /* signed distance to the nearest boundary, in bins */
+    e = -PDO_PI + floor(x + 0.5) * w;
+    if (fabs(fr) * w <= tol_angle(e)) near |= PDO_NEAR_PHI;
+  }
+  return near;
+}
+
+int pdo_tower_centre(const pdo_card *c, int32_t tower, double *eta_c, double *phi_c) {
+  int i, j;
+  double mid;
+  if (!c || tower < 0 || tower >= c->n_towers) return PDO_EINVAL;
+  for (i = c->n_bins - 1; i > 0; --i)
+    if (c->offset[i] <= tower) break;
+  j = tower - c->offset[i];
+  mid = 0.5 * (c->edges[i] + c->edges[i + 1]);
+  if (eta_c) *eta_c = c->grid_coord ? -log(tan(0.5 * mid)) : mid;
+  if (phi_c) *phi_c = -PDO_PI + ((double)j + 0.5) * (PDO_TWO_PI / (double)c->nphi[i]);
+  return PDO_OK;
+}
+
+/* ------------------------------------------------------------------ O3: efficiency --------- */
+
+/* mode 0: exact; +1: loose (conditions widened by the tolerance); -1: strict (narrowed) */
+static int eff_row_match(const pdo_card *c, int r, double pt, double aeta, int mode) {
+  const double *row = c->eff[r];
+  double m = (double)mode;
+  double t0 = m * PDO_REL_TOL * fabs(row[0]), t1 = isinf(row[1]) ? 0.0 : m * PDO_REL_TOL * fabs(row[1]);
+  double t2 = m * tol_angle(row[2]), t3 = isinf(row[3]) ? 0.0 : m * tol_angle(row[3]);
+  if (!(pt > row[0] - t0)) return 0;
+  if (!(pt <= row[1] + t1)) return 0;
+  if (row[2] > 0.0 ? !(aeta >= row[2] - t2) : 0) return 0;
+  if (!(aeta < row[3] + t3)) return 0;
+  return 1;
+}
+
+double pdo_efficiency(const pdo_card *c, double pt, double eta_mom, double abs_costheta, int *row) {
+  int r;
+  double aeta = fabs(eta_mom);
+  if (row) *row = -1;
+  if (c->has_cos && abs_costheta >= c->abs_costheta_max) return 0.0;
+  for (r = 0; r < c->n_eff; ++r)
+    if (eff_row_match(c, r, pt, aeta, 0)) {
+      if (row) *row = r;
+      return c->eff[r][4];
+    }
+  return 0.0;
+}
+
+static int eff_row_allowed(const pdo_card *c, double pt, double aeta, double abs_costheta, int row) {
+  int r;
+  if (row >= c->n_eff) return 0;
+  if (c->has_cos) {
+    double t = tol_angle(c->abs_costheta_max);
+    if (row >= 0 && abs_costheta >= c->abs_costheta_max + t) return 0;
+    if (row < 0 && abs_costheta >= c->abs_costheta_max - t) return 1;
+  }
+  for (r = 0; r < (row < 0 ? c->n_eff : row); ++r)
+    if (eff_row_match(c, r, pt, aeta, -1)) return 0;
+  return row < 0 ? 1 : eff_row_match(c, row, pt, aeta, +1);
+}
+
+static uint32_t eff_near(const pdo_card *c, double pt, double aeta, double abs_costheta) {
+  int r;
+  if (c->has_cos && fabs(abs_costheta - c->abs_costheta_max) <= tol_angle(c->abs_costheta_max))
+    return PDO_NEAR_EFF;
+  for (r = 0; r < c->n_eff; ++r) {
+    const double *row = c->eff[r];
+    if (fabs(pt - row[0]) <= PDO_REL_TOL * fabs(row[0])) return PDO_NEAR_EFF;
+    if (!isinf(row[1]) && fabs(pt - row[1]) <= PDO_REL_TOL * fabs(row[1])) return PDO_NEAR_EFF;
+    if (row[2] > 0.0 && fabs(aeta - row[2]) <= tol_angle(row[2])) return PDO_NEAR_EFF;
+    if (!isinf(row[3]) && fabs(aeta - row[3]) <= tol_angle(row[3])) return PDO_NEAR_EFF;
+  }
+  return 0;
+}
+
+/* ------------------------------------------------------------------ O2: propagation -------- */
+
+typedef struct {
+  int status;           /* face | PDO_LOOPER */
+  double x, y, z;       /* hit position, metres */
+  double alpha;         /* turning angle (0 for straight lines) */
+  double eta_pos, phi_pos, coord; /* coord = eta_pos or theta_pos per the card's grid */
+  uint32_t near;        /* PDO_NEAR_VERTEX | PDO_NEAR_FACE | PDO_NEAR_LOWPT */
+  int face_ov_bad;      /* a face override was requested outside the tolerance */
+} pdo_hit;
+
+static double sgn(double x) { return x > 0.0 ? 1.0 : (x < 0.0 ? -1.0 : 0.0); }
+
+/* ov_face: -1 none, PDO_BARREL / PDO_ENDCAP to force the D2 decision (honoured only when near) */
+static void propagate(const pdo_card *c, int q, double px, double py, double pz, double vx,
+                      double vy, double vz, int ov_face, pdo_hit *h) {
+  const double R = c->radius, L = c->half_length, B = c->bz;
+  double pt2 = px * px + py * py, pt = hypot(px, py), r0 = hypot(vx, vy);
+  double x = 0, y = 0, z = 0, alpha = 0;
+  int face = PDO_DROPPED, looper = 0;
+  memset(h, 0, sizeof(*h));
+  /* near-edge bookkeeping of D1 and D7 */
+  if (fabs(r0 - R) <= PDO_REL_TOL * R || fabs(fabs(vz) - L) <= PDO_REL_TOL * L) h->near |= PDO_NEAR_VERTEX;
+  if (fabs(pt2 - 1e-9) <= PDO_REL_TOL * 1e-9) h->near |= PDO_NEAR_LOWPT;
+  /* readings A4, A5: born on/outside the cylinder, or (almost) no transverse momentum: dropped */
+  if (r0 >= R || fabs(vz) >= L || pt2 < 1e-9) {
+    h->status = PDO_DROPPED;
+    h->eta_pos = h->phi_pos = h->coord = NAN;
+    return;
+  }
+  if (q == 0 || B == 0.0) {
+    /* straight line: |v + t p|_perp = R  or  z = sgn(pz) L, whichever comes first */
+    double a = pt2, b = vx * px + vy * py, cc = r0 * r0 - R * R;
+    double tR = (-b + sqrt(b * b - a * cc)) / a;
+    double tZ = pz != 0.0 ? (sgn(pz) * L - vz) / pz : INFINITY;
+    int endcap = tZ < tR;
+    if (isfinite(tZ) && fabs(tR - tZ) <= PDO_REL_TOL * fmax(tR, tZ)) {
+      h->near |= PDO_NEAR_FACE;
+      if (ov_face == PDO_BARREL) endcap = 0;
+      if (ov_face == PDO_ENDCAP) endcap = 1;
+    } else if (ov_face >= 0 && ov_face != (endcap ? PDO_ENDCAP : PDO_BARREL)) {
+      h->face_ov_bad = 1;
+    }
+    if (endcap) {
+      x = vx + tZ * px, y = vy + tZ * py, z = sgn(pz) * L;
+      face = PDO_ENDCAP;
+    } else {
+      x = vx + tR * px, y = vy + tR * py, z = vz + tR * pz;
+      face = PDO_BARREL;
+    }
+  } else {
+    /* helix: radius rho, rotation sense s (reading A3: q > 0 in +z field turns clockwise) */
+    double aq = fabs((double)q);
+    double rho = pt / (c->kappa * aq * fabs(B));
+    double s = -sgn((double)q * B);
+    double phi0 = atan2(py, px);
+    double cx = vx - s * rho * sin(phi0), cy = vy + s * rho * cos(phi0);
+    double rc = hypot(cx, cy), dx = vx - cx, dy = vy - cy;
+    double aR = INFINITY, aZ = INFINITY, Cs = 2.0, h2;
+    int endcap, near_loop = 0, near_corner = 0, reach;
+    if (rc > 0.0) Cs = (R * R - rc * rc - rho * rho) / (2.0 * rc * rho);
+    reach = rc > 0.0 && Cs <= 1.0;
+    if (fabs(rc + rho - R) <= PDO_REL_TOL * R) near_loop = 1;
+    if (near_loop && ov_face == PDO_BARREL) reach = rc > 0.0;
+    if (near_loop && ov_face == PDO_ENDCAP) reach = 0;
+    if (reach) {
+      double psis = acos(fmax(fmin(Cs, 1.0), -1.0));
+      double psi0 = atan2(cx * dy - cy * dx, cx * dx + cy * dy);
+      if (psi0 < 0.0) psi0 += PDO_TWO_PI;
+      aR = s > 0.0 ? (PDO_TWO_PI - psis - psi0) : (psi0 - psis);
+      if (aR < 0.0) aR = 0.0;
+    } else {
+      looper = PDO_LOOPER;
+    }
+    if (pz != 0.0) aZ = (sgn(pz) * L - vz) * pt / (rho * pz);
+    if (near_loop) h->near |= PDO_NEAR_FACE;
+    if (isinf(aR) && isinf(aZ)) {
+      /* trapped: never leaves the tracker volume (reading A6) */
+      h->status = PDO_DROPPED | looper;
+      h->eta_pos = h->phi_pos = h->coord = NAN;
+      if (ov_face >= 0 && !near_loop) h->face_ov_bad = 1;
+      return;
+    }
+    endcap = aZ < aR;
+    if (isfinite(aR) && isfinite(aZ) && fabs(aR - aZ) <= PDO_REL_TOL * fmax(aR, aZ)) near_corner = 1;
+    if (near_corner) {
+      h->near |= PDO_NEAR_FACE;
+      if (ov_face == PDO_BARREL) endcap = 0;
+      if (ov_face == PDO_ENDCAP) endcap = 1;
+    }
+    if (ov_face >= 0 && !near_corner && !near_loop && ov_face != (endcap ? PDO_ENDCAP : PDO_BARREL))
+      h->face_ov_bad = 1;
+    alpha = endcap ? aZ : aR;
+    /* chord form: vertex + 2 rho sin(alpha/2) (cos, sin)(phi0 + s alpha/2) */
+    h2 = 0.5 * alpha;
+    x = vx + 2.0 * rho * sin(h2) * cos(phi0 + s * h2);
+    y = vy + 2.0 * rho * sin(h2) * sin(phi0 + s * h2);
+    z = endcap ? sgn(pz) * L : vz + rho * alpha * pz / pt;
+    face = endcap ? PDO_ENDCAP : PDO_BARREL;
+  }
+  h->status = face | looper;
+  h->x = x, h->y = y, h->z = z, h->alpha = alpha;
+  {
+    double r = hypot(x, y);
+    h->eta_pos = r > 0.0 ? asinh(z / r) : (z > 0 ? INFINITY : -INFINITY);
+    h->phi_pos = atan2(y, x);
+    h->coord = c->grid_coord ? atan2(r, z) : h->eta_pos;
+  }
+}
+
+int pdo_propagate(const pdo_card *c, int charge, double px, double py, double pz, double vx,
+                  double vy, double vz, double *x, double *y, double *z, double *alpha,
+                  double *eta_pos, double *phi_pos) {
+  pdo_hit h;
+  propagate(c, charge, px, py, pz, vx, vy, vz, -1, &h);
+  if (x) *x = h.x;
+  if (y) *y = h.y;
+  if (z) *z = h.z;
+  if (alpha) *alpha = h.alpha;
+  if (eta_pos) *eta_pos = h.eta_pos;
+  if (phi_pos) *phi_pos = h.phi_pos;
+  return h.status;
+}
+
+/* ------------------------------------------------------------------ O1..O7: the chain ------ */
+
+static int cmp_i32(const void *a, const void *b) {
+  int32_t x = *(const int32_t *)a, y = *(const int32_t *)b;
+  return x < y ? -1 : (x > y ? 1 : 0);
+}
+
+/* decide "value > thr" with an optional forced outcome; *near receives whether it was near */
+static int above_thr(double value, double thr, double scale, int forced, int *near) {
+  int res = value > thr;
+  *near = fabs(value - thr) <= 1e-5 * scale; /* D6 band: the float tolerance of north_star */
+  if (forced >= 0 && *near) res = forced;
+  return res;
+}
+
+int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t event_base,
+                 pdo_tracks *trk, pdo_towers *tow, pdo_eflow *efl, pdo_debug *dbg,
+                 const pdo_overrides *ov) {
+  double *Eem, *Ehad, *Tem, *Thad, *ph_E, *nh_E;
+  uint8_t *touched;
+  int32_t *list, *ph_id, *nh_id;
+  int64_t e, n_trk = 0, n_tow = 0, n_efl = 0, n_dbg_tw = 0, rejected = 0;
+  int rc = PDO_OK;
+  if (!c || !ev || !trk || !tow || !efl || ev->n_events < 0 || ev->n_particles < 0) return PDO_EINVAL;
+  if (ev->n_events > 0 && !ev->offsets) return PDO_EINVAL;
+  Eem = (double *)calloc((size_t)c->n_towers * 4, sizeof(double));
+  touched = (uint8_t *)calloc((size_t)c->n_towers, 1);
+  list = (int32_t *)malloc((size_t)c->n_towers * 3 * sizeof(int32_t));
+  ph_E = (double *)malloc((size_t)c->n_towers * 2 * sizeof(double));
+  if (!Eem || !touched || !list || !ph_E) {
+    free(Eem), free(touched), free(list), free(ph_E);
+    return PDO_EINVAL;
+  }
+  Ehad = Eem + c->n_towers, Tem = Ehad + c->n_towers, Thad = Tem + c->n_towers;
+  ph_id = list + c->n_towers, nh_id = ph_id + c->n_towers;
+  nh_E = ph_E + c->n_towers;
+  trk->offsets[0] = tow->offsets[0] = efl->offsets[0] = 0;
+  if (dbg && dbg->tw_offsets) dbg->tw_offsets[0] = 0;
+
+  for (e = 0; e < ev->n_events && rc == PDO_OK; ++e) {
+    int64_t i0 = ev->offsets[e], i1 = ev->offsets[e + 1], i, trk_begin = n_trk;
+    int n_list = 0, n_ph = 0, n_nh = 0, t;
+    int64_t event = event_base + e; /* reading A27 */
+    for (i = i0; i < i1; ++i) {
+      /* O1 classify (reading A18) */
+      int apid = ev->pid[i] < 0 ? -ev->pid[i] : ev->pid[i], q = ev->charge[i];
+      int cls = apid == 11 ? PDO_CLS_ELECTRON : (apid == 13 ? PDO_CLS_MUON : PDO_CLS_CHHAD);
+      double fe = (apid == 11 || apid == 22) ? 1.0 : 0.0;
+      double fh = (apid == 11 || apid == 22 || apid == 13 || apid == 12 || apid == 14 || apid == 16) ? 0.0 : 1.0;
+      double px = ev->px[i], py = ev->py[i], pz = ev->pz[i], E = ev->E[i];
+      double pt = hypot(px, py), pt_smeared = 0.0, Etrk = 0.0;
+      int accepted = 0, row = -1;
+      int32_t tower;
+      uint32_t near;
+      pdo_hit h;
+      /* O2 propagate */
+      propagate(c, q, px, py, pz, ev->vx[i], ev->vy[i], ev->vz[i], (ov && ov->face) ? ov->face[i] : -1, &h);
+      if (h.face_ov_bad) ++rejected;
+      near = h.near;
+      tower = -1;
+      if ((h.status & PDO_FACE_MASK) != PDO_DROPPED) {
+        /* O3 track: efficiency at the true vertex momentum (A7), accept iff u < eps (A11) */
+        if (q != 0) {
+          double eta_mom = asinh(pz / pt), p = sqrt(pt * pt + pz * pz), act = fabs(pz) / p;
+          double eps = pdo_efficiency(c, pt, eta_mom, act, &row);
+          uint32_t r[4];
+          near |= eff_near(c, pt, fabs(eta_mom), act);
+          if (ov && ov->eps_row && ov->eps_row[i] != -2 && ov->eps_row[i] != row) {
+            if ((near & PDO_NEAR_EFF) && eff_row_allowed(c, pt, fabs(eta_mom), act, ov->eps_row[i])) {
+              row = ov->eps_row[i];
+              eps = row < 0 ? 0.0 : c->eff[row][4];
+            } else {
+              ++rejected;
+            }
+          }
+          pdo_rng_block(seed, event, (uint32_t)(i - i0), 0u, r);
+          accepted = pdo_uniform(r[0]) < eps;
+          if (accepted) {
+            /* track smearing (A12, A13): log-normal, mean pT, std sigma_rel pT; eta, phi unchanged */
+            double srel = sqrt(c->trk_a * c->trk_a + (c->trk_b * pt) * (c->trk_b * pt));
+            pt_smeared = pdo_lognormal(pt, srel * pt, pdo_normal(r[1], r[2]));
+            Etrk = pt_smeared * cosh(eta_mom);
+            if (n_trk >= trk->capacity || n_efl >= efl->capacity) {
+              rc = PDO_ECAPACITY;
+              break;
+            }
+            trk->src[n_trk] = (int32_t)i;
+            trk->pid[n_trk] = ev->pid[i];
+            trk->charge[n_trk] = (int8_t)q;
+            trk->pt[n_trk] = pt_smeared;
+            trk->eta[n_trk] = eta_mom;
+            trk->phi[n_trk] = atan2(py, px);
+            trk->E[n_trk] = Etrk;
+            trk->eta_out[n_trk] = h.eta_pos;
+            trk->phi_out[n_trk] = h.phi_pos;
+            /* O7: the event's EFlow list starts with its accepted tracks, in particle order */
+            efl->cls[n_efl] = (int8_t)cls;
+            efl->src[n_efl] = (int32_t)i;
+            efl->pt[n_efl] = pt_smeared;
+            efl->eta[n_efl] = eta_mom;
+            efl->phi[n_efl] = trk->phi[n_trk];
+            efl->E[n_efl] = Etrk;
+            ++n_trk, ++n_efl;
+          }
+        }
+        /* O4 deposit: tower of the hit position; sums in particle order (A17, A19) */
+        tower = pdo_tower_index(c, h.coord, h.phi_pos);
+        near |= tower_near(c, h.coord, h.phi_pos);
+        if (ov && ov->tower && ov->tower[i] != -2 && ov->tower[i] != tower) {
+          if (tower_allowed(c, h.coord, h.phi_pos, ov->tower[i])) tower = ov->tower[i];
+          else ++rejected;
+        }
+        if (tower >= 0 && (fe != 0.0 || fh != 0.0)) {
+          if (!touched[tower]) touched[tower] = 1, list[n_list++] = tower;
+          Eem[tower] += fe * E;
+          Ehad[tower] += fh * E;
+          if (accepted) Tem[tower] += fe * Etrk, Thad[tower] += fh * Etrk;
+        }
+      }
+      if (dbg) {
+        if (dbg->status) dbg->status[i] = (uint8_t)h.status;
+        if (dbg->x) dbg->x[i] = h.x;
+        if (dbg->y) dbg->y[i] = h.y;
+        if (dbg->z) dbg->z[i] = h.z;
+        if (dbg->eta_pos) dbg->eta_pos[i] = h.eta_pos;
+        if (dbg->phi_pos) dbg->phi_pos[i] = h.phi_pos;
+        if (dbg->tower) dbg->tower[i] = tower;
+        if (dbg->accepted) dbg->accepted[i] = (uint8_t)accepted;
+        if (dbg->eps_row) dbg->eps_row[i] = (int8_t)row;
+        if (dbg->pt_smeared) dbg->pt_smeared[i] = pt_smeared;
+        if (dbg->near) dbg->near[i] = near;
+      }
+    }
+    if (rc != PDO_OK) break;
+    trk->offsets[e + 1] = n_trk;
+    (void)trk_begin;
+
+    /* O5 towers, ascending id; O6 EFlow neutrals */
+    qsort(list, (size_t)n_list, sizeof(int32_t), cmp_i32);
+    for (t = 0; t < n_list; ++t) {
+      int32_t id = list[t];
+      uint32_t r[4];
+      double em_s, had_s, em_f, had_f, n_em, n_had, eta_c, phi_c;
+      int forced[4] = {-1, -1, -1, -1}, nr[4], k, is_ph, is_nh;
+      uint8_t tw_near = 0;
+      if (ov && ov->n_tower_ov > 0) {
+        int64_t j;
+        for (j = 0; j < ov->n_tower_ov; ++j)
+          if (ov->tw_event[j] == e && ov->tw_id[j] == id)
+            for (k = 0; k < 4; ++k)
+              if (ov->tw_mask[j] & (1 << k)) forced[k] = (ov->tw_value[j] >> k) & 1;
+      }
+      pdo_rng_block(seed, event, (uint32_t)id, 1u, r);
+      em_s = pdo_lognormal(Eem[id], resolution(c->ecal, Eem[id]), pdo_normal(r[0], r[1]));
+      had_s = pdo_lognormal(Ehad[id], resolution(c->hcal, Ehad[id]), pdo_normal(r[2], r[3]));
+      /* reading A22: the threshold is applied twice, strictly, per component */
+      em_f = above_thr(em_s, c->thr_ecal, fmax(c->thr_ecal, em_s), forced[0], &nr[0]) ? em_s : 0.0;
+      had_f = above_thr(had_s, c->thr_hcal, fmax(c->thr_hcal, had_s), forced[1], &nr[1]) ? had_s : 0.0;
+      n_em = em_f - Tem[id];
+      n_had = had_f - Thad[id];
+      is_ph = above_thr(n_em, c->thr_ecal, fmax(c->thr_ecal, fmax(em_f, Tem[id])), forced[2], &nr[2]);
+      is_nh = above_thr(n_had, c->thr_hcal, fmax(c->thr_hcal, fmax(had_f, Thad[id])), forced[3], &nr[3]);
+      for (k = 0; k < 4; ++k) {
+        if (nr[k]) tw_near |= (uint8_t)(1 << k);
+        else if (forced[k] >= 0) ++rejected;
+      }
+      if (dbg && dbg->tw_offsets) {
+        if (n_dbg_tw >= dbg->tw_capacity) {
+          rc = PDO_ECAPACITY;
+          break;
+        }
+        if (dbg->tw_id) dbg->tw_id[n_dbg_tw] = id;
+        if (dbg->Eem_true) dbg->Eem_true[n_dbg_tw] = Eem[id];
+        if (dbg->Ehad_true) dbg->Ehad_true[n_dbg_tw] = Ehad[id];
+        if (dbg->Tem) dbg->Tem[n_dbg_tw] = Tem[id];
+        if (dbg->Thad) dbg->Thad[n_dbg_tw] = Thad[id];
+        if (dbg->Eem_smeared) dbg->Eem_smeared[n_dbg_tw] = em_s;
+        if (dbg->Ehad_smeared) dbg->Ehad_smeared[n_dbg_tw] = had_s;
+        if (dbg->tw_near) dbg->tw_near[n_dbg_tw] = tw_near;
+        ++n_dbg_tw;
+      }
+      pdo_tower_centre(c, id, &eta_c, &phi_c);
+      if (em_f + had_f > 0.0) {
+        if (n_tow >= tow->capacity) {
+          rc = PDO_ECAPACITY;
+          break;
+        }
+        tow->tower[n_tow] = id;
+        tow->eta[n_tow] = eta_c;
+        tow->phi[n_tow] = phi_c;
+        tow->E[n_tow] = em_f + had_f;
+        tow->Eem[n_tow] = em_f;
+        tow->Ehad[n_tow] = had_f;
+        tow->ET[n_tow] = (em_f + had_f) / cosh(eta_c);
+        ++n_tow;
+      }
+      if (is_ph) ph_id[n_ph] = id, ph_E[n_ph] = n_em, ++n_ph;
+      if (is_nh) nh_id[n_nh] = id, nh_E[n_nh] = n_had, ++n_nh;
+      /* reset the dense accumulators for the next event */
+      Eem[id] = Ehad[id] = Tem[id] = Thad[id] = 0.0;
+      touched[id] = 0;
+    }
+    if (rc != PDO_OK) break;
+    tow->offsets[e + 1] = n_tow;
+    if (dbg && dbg->tw_offsets) dbg->tw_offsets[e + 1] = n_dbg_tw;
+    /* O7: EFlow = tracks (already written) ++ photons ascending id ++ neutral hadrons ascending id */
+    if (n_efl + n_ph + n_nh > efl->capacity) {
+      rc = PDO_ECAPACITY;
+      break;
+    }
+    for (t = 0; t < n_ph + n_nh; ++t) {
+      int is_photon = t < n_ph;
+      int32_t id = is_photon ? ph_id[t] : nh_id[t - n_ph];
+      double En = is_photon ? ph_E[t] : nh_E[t - n_ph], eta_c, phi_c;
+      pdo_tower_centre(c, id, &eta_c, &phi_c);
+      efl->cls[n_efl] = (int8_t)(is_photon ? PDO_CLS_PHOTON : PDO_CLS_NEUHAD);
+      efl->src[n_efl] = id;
+      efl->pt[n_efl] = En / cosh(eta_c);
+      efl->eta[n_efl] = eta_c;
+      efl->phi[n_efl] = phi_c;
+      efl->E[n_efl] = En;
+      ++n_efl;
+    }
+    efl->offsets[e + 1] = n_efl;
+  }
+  free(Eem), free(touched), free(list), free(ph_E);
+  if (ov && ov->n_rejected) *ov->n_rejected = rejected;
+  if (rc == PDO_OK && rejected > 0) rc = PDO_EOVERRIDE;
+  return rc;
+}

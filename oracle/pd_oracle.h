@@ -1,0 +1,163 @@
+/*
+ * pd_oracle.h -- fp64, single-threaded CPU ORACLE of the Delphes-style detector response.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing under oracle/ is part of the product path: only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build, link or
+ * call it.  It shares no code, header, table or constant generator with the CUDA path
+ * (paper_2606_26089_b200/csrc, include/pd.h); both were written separately from SURVEY.md section 8c.
+ *
+ * What it computes (citations: P:Lnnn = /root/reference/PAPER.md line nnn):
+ *   the TorchDelphes chain named in P:L46 and P:L81 -- "particle propagation through the magnetic
+ *   field, tracking efficiency, momentum smearing, calorimeter response, and energy-flow merging,
+ *   with per-module parameters loaded from the selected detector card" -- up to "the generation of
+ *   calorimeter tower hits (Towers) and reconstructed photons, neutral hadrons, and charged tracks
+ *   (EFlowObjects)".  The paper prints no formula for any step; the formulas are the
+ *   readings A1..A32 listed in DESIGN.md (from SURVEY.md 8c.2 / 8c.3 and BASELINE.json configs).
+ *
+ * Parity status: every function below is pinned by tests/test_oracle_*.py (Philox known-answer
+ * vectors, RK4 integration of the Lorentz force, closed forms, the worked values of
+ * the text fixtures under tests/golden, invariants, a brute-force tiny event).  What stays UNPINNED is the choice of
+ * readings versus the paper's own software (not in the container): "parity with the paper's
+ * software: unpinned" -- see DESIGN.md.
+ *
+ * All pointers are HOST pointers owned by the caller.  Nothing is allocated for outputs.
+ */
+#ifndef PD_ORACLE_H
+#define PD_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pdo_card pdo_card;
+
+/* status byte: low two bits = face, bit 2 = looper (charged, cannot reach r = R) */
+enum { PDO_DROPPED = 0, PDO_BARREL = 1, PDO_ENDCAP = 2, PDO_FACE_MASK = 3, PDO_LOOPER = 4 };
+
+/* EFlow / particle classes (charged hadron, electron, muon, neutral hadron, photon) */
+enum { PDO_CLS_CHHAD = 0, PDO_CLS_ELECTRON = 1, PDO_CLS_MUON = 2, PDO_CLS_NEUHAD = 3, PDO_CLS_PHOTON = 4 };
+
+/* near-edge bits, per particle (SURVEY 8c.4 decisions D1, D2, D3, D5, D7) */
+enum {
+  PDO_NEAR_VERTEX = 1,   /* D1: r0 vs R or |vz| vs L                         */
+  PDO_NEAR_FACE   = 2,   /* D2: looper threshold or barrel/endcap corner     */
+  PDO_NEAR_EFF    = 4,   /* D3: a pT / |eta| / |cos theta| edge of the table */
+  PDO_NEAR_ETA    = 8,   /* D5: eta (theta) bin edge or grid coverage        */
+  PDO_NEAR_PHI    = 16,  /* D5: phi bin edge                                 */
+  PDO_NEAR_LOWPT  = 32   /* D7: pT^2 vs 1e-9                                 */
+};
+/* near-threshold bits, per deposited tower (decision D6) */
+enum { PDO_NEAR_EEM = 1, PDO_NEAR_EHAD = 2, PDO_NEAR_NEM = 4, PDO_NEAR_NHAD = 8 };
+
+/* error codes */
+enum { PDO_OK = 0, PDO_EINVAL = -1, PDO_ECARD = -2, PDO_ECAPACITY = -3, PDO_EOVERRIDE = -4 };
+
+typedef struct {
+  int32_t n_towers, n_eta_bins, grid_coord; /* grid_coord: 0 = eta, 1 = theta */
+  float bz, radius, half_length;
+  int32_t n_eff_rows;
+} pdo_card_info_t;
+
+typedef struct {
+  int64_t n_events;
+  int64_t n_particles;
+  const int64_t *offsets; /* [n_events+1] */
+  const int32_t *pid;
+  const int8_t *charge;
+  const float *px, *py, *pz, *E, *vx, *vy, *vz;
+} pdo_events;
+
+typedef struct {
+  int64_t capacity;
+  int64_t *offsets; /* [n_events+1] */
+  int32_t *src, *pid;
+  int8_t *charge;
+  double *pt, *eta, *phi, *E, *eta_out, *phi_out;
+} pdo_tracks;
+
+typedef struct {
+  int64_t capacity;
+  int64_t *offsets;
+  int32_t *tower;
+  double *eta, *phi, *E, *Eem, *Ehad, *ET;
+} pdo_towers;
+
+typedef struct {
+  int64_t capacity;
+  int64_t *offsets;
+  int8_t *cls;
+  int32_t *src;
+  double *pt, *eta, *phi, *E;
+} pdo_eflow;
+
+/* optional (NULL allowed as a whole; individual arrays may be NULL too) */
+typedef struct {
+  /* per particle */
+  uint8_t *status;
+  double *x, *y, *z, *eta_pos, *phi_pos;
+  int32_t *tower;       /* geometric tower id of the hit, -1 if none */
+  uint8_t *accepted;
+  int8_t *eps_row;      /* row of the efficiency table used, -1 none */
+  double *pt_smeared;   /* 0 if not an accepted track */
+  uint32_t *near;       /* PDO_NEAR_* bits */
+  /* per deposited tower (emitted or not), CSR over events */
+  int64_t tw_capacity;
+  int64_t *tw_offsets;  /* [n_events+1] */
+  int32_t *tw_id;
+  double *Eem_true, *Ehad_true, *Tem, *Thad, *Eem_smeared, *Ehad_smeared;
+  uint8_t *tw_near;     /* PDO_NEAR_E* bits */
+} pdo_debug;
+
+/* optional overrides.  An override is honoured only if the oracle itself finds the
+ * requested outcome within the near-edge tolerance; otherwise pdo_simulate returns PDO_EOVERRIDE
+ * and *n_rejected counts the offenders. */
+typedef struct {
+  const int8_t *face;     /* per particle: -1 none, PDO_BARREL or PDO_ENDCAP */
+  const int32_t *tower;   /* per particle: -2 none, else tower id or -1 (no tower) */
+  const int8_t *eps_row;  /* per particle: -2 none, else row index or -1 (no row) */
+  int64_t n_tower_ov;     /* tower-level overrides of threshold decisions */
+  const int64_t *tw_event;/* event index within the call */
+  const int32_t *tw_id;
+  const uint8_t *tw_mask; /* which PDO_NEAR_E* decisions to force */
+  const uint8_t *tw_value;/* forced outcome bits (1 = "above threshold") */
+  int64_t *n_rejected;    /* out, may be NULL */
+} pdo_overrides;
+
+int pdo_load_card(const char *name_or_path, pdo_card **out);
+void pdo_free_card(pdo_card *card);
+int pdo_card_info(const pdo_card *card, pdo_card_info_t *out);
+/* copy of the card tables for tests: edges[n_eta_bins+1], nphi[n_eta_bins], offset[n_eta_bins] */
+int pdo_card_grid(const pdo_card *card, double *edges, int32_t *nphi, int32_t *offset);
+/* tower centre (eta_c, phi_c) of a tower id; returns PDO_EINVAL if out of range */
+int pdo_tower_centre(const pdo_card *card, int32_t tower, double *eta_c, double *phi_c);
+
+int pdo_simulate(const pdo_card *card, const pdo_events *ev, uint64_t seed, int64_t event_base,
+                 pdo_tracks *tracks, pdo_towers *towers, pdo_eflow *eflow, pdo_debug *debug,
+                 const pdo_overrides *ov);
+
+const char *pdo_strerror(int code);
+
+/* ---- building blocks exposed so that tests can pin them one by one ---- */
+void pdo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* the RNG layout of reading A26: stream 0 = particle stream, 1 = tower stream */
+void pdo_rng_block(uint64_t seed, int64_t event, uint32_t object, uint32_t stream, uint32_t out[4]);
+double pdo_uniform(uint32_t x);       /* (x >> 8) * 2^-24          in [0,1) */
+double pdo_uniform_pos(uint32_t x);   /* ((x >> 8) + 1) * 2^-24    in (0,1] */
+double pdo_normal(uint32_t xa, uint32_t xb); /* Box-Muller, cosine branch */
+double pdo_lognormal(double mean, double sigma, double z);
+/* one particle through O2; returns the status byte. alpha = turning angle (0 for neutrals) */
+int pdo_propagate(const pdo_card *card, int charge, double px, double py, double pz, double vx,
+                  double vy, double vz, double *x, double *y, double *z, double *alpha,
+                  double *eta_pos, double *phi_pos);
+/* tower id (or -1) of a position given as (eta_pos or theta_pos per the card's grid, phi_pos) */
+int32_t pdo_tower_index(const pdo_card *card, double coord, double phi_pos);
+/* efficiency of O3 for true (pt, eta_mom, |cos theta|); *row receives the row index or -1 */
+double pdo_efficiency(const pdo_card *card, double pt, double eta_mom, double abs_costheta,
+                      int *row);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PD_ORACLE_H */
