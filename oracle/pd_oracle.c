@@ -630,6 +630,15 @@ int pdo_propagate(const pdo_card *c, int charge, double px, double py, double pz
 
 /* ------------------------------------------------------------------ O1..O7: the chain ------ */
 
+/* order of the tower overrides by (event, tower id) */
+static const pdo_overrides *g_sort_ov;
+static int cmp_ov(const void *a, const void *b) {
+  int64_t i = *(const int64_t *)a, j = *(const int64_t *)b;
+  if (g_sort_ov->tw_event[i] != g_sort_ov->tw_event[j]) return g_sort_ov->tw_event[i] < g_sort_ov->tw_event[j] ? -1 : 1;
+  if (g_sort_ov->tw_id[i] != g_sort_ov->tw_id[j]) return g_sort_ov->tw_id[i] < g_sort_ov->tw_id[j] ? -1 : 1;
+  return i < j ? -1 : (i > j ? 1 : 0);
+}
+
 static int cmp_i32(const void *a, const void *b) {
   int32_t x = *(const int32_t *)a, y = *(const int32_t *)b;
   return x < y ? -1 : (x > y ? 1 : 0);
@@ -650,6 +659,7 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
   uint8_t *touched;
   int32_t *list, *ph_id, *nh_id;
   int64_t e, n_trk = 0, n_tow = 0, n_efl = 0, n_dbg_tw = 0, rejected = 0;
+  int64_t *ov_order = NULL, ov_pos = 0;
   int rc = PDO_OK;
   if (!c || !ev || !trk || !tow || !efl || ev->n_events < 0 || ev->n_particles < 0) return PDO_EINVAL;
   if (ev->n_events > 0 && !ev->offsets) return PDO_EINVAL;
@@ -660,6 +670,17 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
   if (!Eem || !touched || !list || !ph_E) {
     free(Eem), free(touched), free(list), free(ph_E);
     return PDO_EINVAL;
+  }
+  if (ov && ov->n_tower_ov > 0) {
+    int64_t j;
+    ov_order = (int64_t *)malloc((size_t)ov->n_tower_ov * sizeof(int64_t));
+    if (!ov_order) {
+      free(Eem), free(touched), free(list), free(ph_E);
+      return PDO_EINVAL;
+    }
+    for (j = 0; j < ov->n_tower_ov; ++j) ov_order[j] = j;
+    g_sort_ov = ov;
+    qsort(ov_order, (size_t)ov->n_tower_ov, sizeof(int64_t), cmp_ov);
   }
   Ehad = Eem + c->n_towers, Tem = Ehad + c->n_towers, Thad = Tem + c->n_towers;
   ph_id = list + c->n_towers, nh_id = ph_id + c->n_towers;
@@ -773,12 +794,20 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
       double em_s, had_s, em_f, had_f, n_em, n_had, eta_c, phi_c;
       int forced[4] = {-1, -1, -1, -1}, nr[4], k, is_ph, is_nh;
       uint8_t tw_near = 0;
-      if (ov && ov->n_tower_ov > 0) {
-        int64_t j;
-        for (j = 0; j < ov->n_tower_ov; ++j)
-          if (ov->tw_event[j] == e && ov->tw_id[j] == id)
-            for (k = 0; k < 4; ++k)
-              if (ov->tw_mask[j] & (1 << k)) forced[k] = (ov->tw_value[j] >> k) & 1;
+      if (ov_order) {
+        /* tower overrides, visited in (event, id) order alongside the ascending tower loop */
+        while (ov_pos < ov->n_tower_ov &&
+               (ov->tw_event[ov_order[ov_pos]] < e ||
+                (ov->tw_event[ov_order[ov_pos]] == e && ov->tw_id[ov_order[ov_pos]] < id))) {
+          ++rejected; /* names a tower that received no deposit */
+          ++ov_pos;
+        }
+        while (ov_pos < ov->n_tower_ov && ov->tw_event[ov_order[ov_pos]] == e &&
+               ov->tw_id[ov_order[ov_pos]] == id) {
+          int64_t j = ov_order[ov_pos++];
+          for (k = 0; k < 4; ++k)
+            if (ov->tw_mask[j] & (1 << k)) forced[k] = (ov->tw_value[j] >> k) & 1;
+        }
       }
       pdo_rng_block(seed, event, (uint32_t)id, 1u, r);
       em_s = pdo_lognormal(Eem[id], resolution(c->ecal, Eem[id]), pdo_normal(r[0], r[1]));
@@ -853,7 +882,8 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
     }
     efl->offsets[e + 1] = n_efl;
   }
-  free(Eem), free(touched), free(list), free(ph_E);
+  if (rc == PDO_OK && ov_order) rejected += ov->n_tower_ov - ov_pos; /* overrides never reached */
+  free(Eem), free(touched), free(list), free(ph_E), free(ov_order);
   if (ov && ov->n_rejected) *ov->n_rejected = rejected;
   if (rc == PDO_OK && rejected > 0) rc = PDO_EOVERRIDE;
   return rc;

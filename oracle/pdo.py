@@ -1,0 +1,254 @@
+"""ctypes binding of the fp64 CPU oracle (oracle/libpd_oracle.so).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  It shares nothing with the CUDA path (paper_2606_26089_b200/).
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+PDO_DROPPED, PDO_BARREL, PDO_ENDCAP, PDO_FACE_MASK, PDO_LOOPER = 0, 1, 2, 3, 4
+NEAR_VERTEX, NEAR_FACE, NEAR_EFF, NEAR_ETA, NEAR_PHI, NEAR_LOWPT = 1, 2, 4, 8, 16, 32
+NEAR_EEM, NEAR_EHAD, NEAR_NEM, NEAR_NHAD = 1, 2, 4, 8
+PDO_OK, PDO_EINVAL, PDO_ECARD, PDO_ECAPACITY, PDO_EOVERRIDE = 0, -1, -2, -3, -4
+
+_p = C.c_void_p
+
+
+class _CardInfo(C.Structure):
+    _fields_ = [("n_towers", C.c_int32), ("n_eta_bins", C.c_int32), ("grid_coord", C.c_int32),
+                ("bz", C.c_float), ("radius", C.c_float), ("half_length", C.c_float),
+                ("n_eff_rows", C.c_int32)]
+
+
+class _Events(C.Structure):
+    _fields_ = [("n_events", C.c_int64), ("n_particles", C.c_int64), ("offsets", _p), ("pid", _p),
+                ("charge", _p), ("px", _p), ("py", _p), ("pz", _p), ("E", _p), ("vx", _p), ("vy", _p),
+                ("vz", _p)]
+
+
+class _Tracks(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("offsets", _p), ("src", _p), ("pid", _p), ("charge", _p),
+                ("pt", _p), ("eta", _p), ("phi", _p), ("E", _p), ("eta_out", _p), ("phi_out", _p)]
+
+
+class _Towers(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("offsets", _p), ("tower", _p), ("eta", _p), ("phi", _p),
+                ("E", _p), ("Eem", _p), ("Ehad", _p), ("ET", _p)]
+
+
+class _EFlow(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("offsets", _p), ("cls", _p), ("src", _p), ("pt", _p),
+                ("eta", _p), ("phi", _p), ("E", _p)]
+
+
+class _Debug(C.Structure):
+    _fields_ = [("status", _p), ("x", _p), ("y", _p), ("z", _p), ("eta_pos", _p), ("phi_pos", _p),
+                ("tower", _p), ("accepted", _p), ("eps_row", _p), ("pt_smeared", _p), ("near", _p),
+                ("tw_capacity", C.c_int64), ("tw_offsets", _p), ("tw_id", _p), ("Eem_true", _p),
+                ("Ehad_true", _p), ("Tem", _p), ("Thad", _p), ("Eem_smeared", _p), ("Ehad_smeared", _p),
+                ("tw_near", _p)]
+
+
+class _Overrides(C.Structure):
+    _fields_ = [("face", _p), ("tower", _p), ("eps_row", _p), ("n_tower_ov", C.c_int64),
+                ("tw_event", _p), ("tw_id", _p), ("tw_mask", _p), ("tw_value", _p), ("n_rejected", _p)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        L.pdo_load_card.argtypes = [C.c_char_p, C.POINTER(_p)]
+        L.pdo_free_card.argtypes = [_p]
+        L.pdo_free_card.restype = None
+        L.pdo_card_info.argtypes = [_p, C.POINTER(_CardInfo)]
+        L.pdo_card_grid.argtypes = [_p, _p, _p, _p]
+        L.pdo_tower_centre.argtypes = [_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.pdo_simulate.argtypes = [_p, C.POINTER(_Events), C.c_uint64, C.c_int64, C.POINTER(_Tracks),
+                                   C.POINTER(_Towers), C.POINTER(_EFlow), C.POINTER(_Debug),
+                                   C.POINTER(_Overrides)]
+        L.pdo_strerror.argtypes = [C.c_int]
+        L.pdo_strerror.restype = C.c_char_p
+        L.pdo_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
+        L.pdo_philox4x32_10.restype = None
+        L.pdo_rng_block.argtypes = [C.c_uint64, C.c_int64, C.c_uint32, C.c_uint32, C.POINTER(C.c_uint32)]
+        L.pdo_rng_block.restype = None
+        for name in ("pdo_uniform", "pdo_uniform_pos"):
+            getattr(L, name).argtypes = [C.c_uint32]
+            getattr(L, name).restype = C.c_double
+        L.pdo_normal.argtypes = [C.c_uint32, C.c_uint32]
+        L.pdo_normal.restype = C.c_double
+        L.pdo_lognormal.argtypes = [C.c_double] * 3
+        L.pdo_lognormal.restype = C.c_double
+        L.pdo_propagate.argtypes = [_p, C.c_int] + [C.c_double] * 6 + [C.POINTER(C.c_double)] * 6
+        L.pdo_tower_index.argtypes = [_p, C.c_double, C.c_double]
+        L.pdo_tower_index.restype = C.c_int32
+        L.pdo_efficiency.argtypes = [_p, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int)]
+        L.pdo_efficiency.restype = C.c_double
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(_p)
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code, n_rejected=0):
+        super().__init__("oracle: %s (code %d, rejected overrides %d)"
+                         % (lib().pdo_strerror(code).decode(), code, n_rejected))
+        self.code = code
+        self.n_rejected = n_rejected
+
+
+class Card:
+    """A detector card: "cms_like" | "atlas_like" | "aleph_like" | path of a card text file."""
+
+    def __init__(self, name_or_path: str):
+        self._h = _p()
+        rc = lib().pdo_load_card(str(name_or_path).encode(), C.byref(self._h))
+        if rc != PDO_OK:
+            raise OracleError(rc)
+        info = _CardInfo()
+        lib().pdo_card_info(self._h, C.byref(info))
+        self.n_towers, self.n_bins, self.grid_coord = info.n_towers, info.n_eta_bins, info.grid_coord
+        self.bz, self.radius, self.half_length = info.bz, info.radius, info.half_length
+        self.n_eff_rows = info.n_eff_rows
+        self.edges = np.zeros(self.n_bins + 1)
+        self.nphi = np.zeros(self.n_bins, dtype=np.int32)
+        self.offset = np.zeros(self.n_bins, dtype=np.int32)
+        lib().pdo_card_grid(self._h, _ptr(self.edges), _ptr(self.nphi), _ptr(self.offset))
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().pdo_free_card(self._h)
+            self._h = None
+
+    def tower_centre(self, tower: int):
+        e, p = C.c_double(), C.c_double()
+        if lib().pdo_tower_centre(self._h, int(tower), C.byref(e), C.byref(p)) != PDO_OK:
+            raise OracleError(PDO_EINVAL)
+        return e.value, p.value
+
+    def tower_index(self, coord: float, phi: float) -> int:
+        return int(lib().pdo_tower_index(self._h, float(coord), float(phi)))
+
+    def efficiency(self, pt, eta_mom, abs_costheta=0.0):
+        row = C.c_int(-1)
+        eps = lib().pdo_efficiency(self._h, float(pt), float(eta_mom), float(abs_costheta), C.byref(row))
+        return eps, row.value
+
+    def propagate(self, q, px, py, pz, vx=0.0, vy=0.0, vz=0.0):
+        out = [C.c_double() for _ in range(6)]
+        st = lib().pdo_propagate(self._h, int(q), float(px), float(py), float(pz), float(vx), float(vy),
+                                 float(vz), *[C.byref(o) for o in out])
+        x, y, z, alpha, eta_pos, phi_pos = [o.value for o in out]
+        return dict(status=st, x=x, y=y, z=z, alpha=alpha, eta_pos=eta_pos, phi_pos=phi_pos)
+
+
+def philox(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr)
+    k = (C.c_uint32 * 2)(*key)
+    o = (C.c_uint32 * 4)()
+    lib().pdo_philox4x32_10(c, k, o)
+    return tuple(int(x) for x in o)
+
+
+def rng_block(seed, event, obj, stream):
+    o = (C.c_uint32 * 4)()
+    lib().pdo_rng_block(int(seed), int(event), int(obj), int(stream), o)
+    return tuple(int(x) for x in o)
+
+
+def uniform(x):
+    return lib().pdo_uniform(int(x))
+
+
+def uniform_pos(x):
+    return lib().pdo_uniform_pos(int(x))
+
+
+def normal(xa, xb):
+    return lib().pdo_normal(int(xa), int(xb))
+
+
+def lognormal(m, s, z):
+    return lib().pdo_lognormal(float(m), float(s), float(z))
+
+
+def simulate(card: Card, ev, seed: int, event_base: int = 0, overrides: dict | None = None,
+             debug: bool = True) -> dict:
+    """Run the oracle on an `Events`-like record (attributes offsets, pid, charge, px..vz).
+
+    Returns a dict of numpy arrays: trk_*, tow_*, efl_* (CSR, trimmed to their totals) and, with
+    debug=True, per-particle dbg_* and per-deposited-tower dtw_* arrays.
+    overrides: dict with optional keys face (int8[n], -1 none), tower (int32[n], -2 none),
+    eps_row (int8[n], -2 none), tw_event (int64[m]), tw_id (int32[m]), tw_mask (uint8[m]), tw_value (uint8[m]).
+    """
+    L = lib()
+    ne, n = int(ev.offsets.shape[0] - 1), int(ev.offsets[-1])
+    keep = [np.ascontiguousarray(getattr(ev, k)) for k in
+            ("offsets", "pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")]
+    cevt = _Events(ne, n, *[_ptr(a) for a in keep])
+    cap = max(n, 1)
+    i64, i32, i8, u8, f8 = np.int64, np.int32, np.int8, np.uint8, np.float64
+    z = lambda m, t: np.zeros(m, dtype=t)  # noqa: E731
+    T = dict(offsets=z(ne + 1, i64), src=z(cap, i32), pid=z(cap, i32), charge=z(cap, i8), pt=z(cap, f8),
+             eta=z(cap, f8), phi=z(cap, f8), E=z(cap, f8), eta_out=z(cap, f8), phi_out=z(cap, f8))
+    W = dict(offsets=z(ne + 1, i64), tower=z(cap, i32), eta=z(cap, f8), phi=z(cap, f8), E=z(cap, f8),
+             Eem=z(cap, f8), Ehad=z(cap, f8), ET=z(cap, f8))
+    F = dict(offsets=z(ne + 1, i64), cls=z(2 * cap, i8), src=z(2 * cap, i32), pt=z(2 * cap, f8),
+             eta=z(2 * cap, f8), phi=z(2 * cap, f8), E=z(2 * cap, f8))
+    ct = _Tracks(cap, *[_ptr(T[k]) for k in ("offsets", "src", "pid", "charge", "pt", "eta", "phi", "E", "eta_out", "phi_out")])
+    cw = _Towers(cap, *[_ptr(W[k]) for k in ("offsets", "tower", "eta", "phi", "E", "Eem", "Ehad", "ET")])
+    cf = _EFlow(2 * cap, *[_ptr(F[k]) for k in ("offsets", "cls", "src", "pt", "eta", "phi", "E")])
+    D = None
+    cd = None
+    if debug:
+        D = dict(status=z(cap, u8), x=z(cap, f8), y=z(cap, f8), z=z(cap, f8), eta_pos=z(cap, f8),
+                 phi_pos=z(cap, f8), tower=z(cap, i32), accepted=z(cap, u8), eps_row=z(cap, i8),
+                 pt_smeared=z(cap, f8), near=z(cap, np.uint32))
+        DT = dict(tw_offsets=z(ne + 1, i64), tw_id=z(cap, i32), Eem_true=z(cap, f8), Ehad_true=z(cap, f8),
+                  Tem=z(cap, f8), Thad=z(cap, f8), Eem_smeared=z(cap, f8), Ehad_smeared=z(cap, f8),
+                  tw_near=z(cap, u8))
+        cd = _Debug(*[_ptr(D[k]) for k in ("status", "x", "y", "z", "eta_pos", "phi_pos", "tower",
+                                           "accepted", "eps_row", "pt_smeared", "near")],
+                    cap, *[_ptr(DT[k]) for k in ("tw_offsets", "tw_id", "Eem_true", "Ehad_true", "Tem",
+                                                 "Thad", "Eem_smeared", "Ehad_smeared", "tw_near")])
+    co = None
+    n_rej = np.zeros(1, dtype=i64)
+    if overrides:
+        ov = {}
+        for k, t in (("face", i8), ("tower", i32), ("eps_row", i8)):
+            ov[k] = None if overrides.get(k) is None else np.ascontiguousarray(overrides[k], dtype=t)
+        m = 0
+        for k, t in (("tw_event", i64), ("tw_id", i32), ("tw_mask", u8), ("tw_value", u8)):
+            ov[k] = None if overrides.get(k) is None else np.ascontiguousarray(overrides[k], dtype=t)
+            if ov[k] is not None:
+                m = int(ov[k].shape[0])
+        co = _Overrides(_ptr(ov["face"]), _ptr(ov["tower"]), _ptr(ov["eps_row"]), m, _ptr(ov["tw_event"]),
+                        _ptr(ov["tw_id"]), _ptr(ov["tw_mask"]), _ptr(ov["tw_value"]), _ptr(n_rej))
+    rc = L.pdo_simulate(card._h, C.byref(cevt), int(seed) & (2**64 - 1), int(event_base), C.byref(ct),
+                        C.byref(cw), C.byref(cf), C.byref(cd) if cd is not None else None,
+                        C.byref(co) if co is not None else None)
+    if rc != PDO_OK:
+        raise OracleError(rc, int(n_rej[0]))
+    out = {}
+    for prefix, d in (("trk", T), ("tow", W), ("efl", F)):
+        tot = int(d["offsets"][-1])
+        for k, a in d.items():
+            out["%s_%s" % (prefix, k)] = a if k == "offsets" else a[:tot]
+    if debug:
+        for k, a in D.items():
+            out["dbg_" + k] = a[:n]
+        tot = int(DT["tw_offsets"][-1])
+        for k, a in DT.items():
+            out["dtw_" + k.replace("tw_", "")] = a if k == "tw_offsets" else a[:tot]
+    return out

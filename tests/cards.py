@@ -1,0 +1,52 @@
+"""Helper: write detector-card text files (the `pd_load_card` / `pdo_load_card` file format) for tests.
+
+Format ("key = values", '#' comments): name, bz, radius, half_length, kappa, grid (eta|theta),
+edges (may repeat), nphi (may repeat), eff (pt_lo pt_hi aeta_lo aeta_hi eps; one line per row),
+abs_costheta_max, track_res (a b), ecal_res (C S N), hcal_res (C S N), ecal_thr, hcal_thr.
+"""
+import numpy as np
+
+BASE = {
+    "cms_like": dict(bz=3.8, radius=1.29, half_length=3.0, ecal=(0.007, 0.07, 0.35), hcal=(0.05, 1.5, 0.0)),
+    "atlas_like": dict(bz=2.0, radius=1.15, half_length=3.5, ecal=(0.0017, 0.101, 0.0), hcal=(0.0302, 0.5205, 0.0)),
+    "aleph_like": dict(bz=1.5, radius=1.8, half_length=2.5, ecal=(0.009, 0.18, 0.0), hcal=(0.0, 0.85, 0.0),
+                       abs_costheta_max=0.98),
+}
+DEFAULT_EFF = [(1.0, "inf", 0.0, 1.5, 0.97), (1.0, "inf", 1.5, 2.5, 0.85), (0.1, 1.0, 0.0, 2.5, 0.70)]
+
+
+def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kappa=0.299792458,
+              eff=DEFAULT_EFF, abs_costheta_max=None, track_res=(0.01, 1.5e-4), ecal=(0.007, 0.07, 0.35),
+              hcal=(0.05, 1.5, 0.0), ecal_thr=0.5, hcal_thr=1.0, name="custom"):
+    lines = ["name = %s" % name, "bz = %r" % bz, "radius = %r" % radius, "half_length = %r" % half_length,
+             "kappa = %r" % kappa, "grid = %s" % grid]
+    edges = [float(x) for x in edges]
+    for i in range(0, len(edges), 8):
+        lines.append("edges = " + " ".join(repr(x) for x in edges[i:i + 8]))
+    nphi = [int(x) for x in nphi]
+    for i in range(0, len(nphi), 16):
+        lines.append("nphi = " + " ".join(str(x) for x in nphi[i:i + 16]))
+    for row in eff:
+        lines.append("eff = " + " ".join(str(x) for x in row))
+    if abs_costheta_max is not None:
+        lines.append("abs_costheta_max = %r" % abs_costheta_max)
+    lines.append("track_res = %r %r" % tuple(track_res))
+    lines.append("ecal_res = %r %r %r" % tuple(ecal))
+    lines.append("hcal_res = %r %r %r" % tuple(hcal))
+    lines.append("ecal_thr = %r" % ecal_thr)
+    lines.append("hcal_thr = %r" % hcal_thr)
+    return "\n".join(lines) + "\n"
+
+
+def variant(path, base_edges, base_nphi, base="cms_like", **kw):
+    """Write a card file that is `base` with fields replaced by kw; returns str(path).
+    base_edges / base_nphi: the grid of the base card (taken from a loaded card by the caller)."""
+    b = dict(BASE[base])
+    args = dict(bz=b["bz"], radius=b["radius"], half_length=b["half_length"], ecal=b["ecal"], hcal=b["hcal"],
+                grid="theta" if base == "aleph_like" else "eta")
+    if "abs_costheta_max" in b:
+        args["abs_costheta_max"] = b["abs_costheta_max"]
+    args.update(kw)
+    with open(path, "w") as f:
+        f.write(card_text(np.asarray(base_edges, dtype=np.float64), base_nphi, **args))
+    return str(path)
