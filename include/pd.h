@@ -1,0 +1,165 @@
+/*
+ * pd.h -- C ABI of the B200-native Delphes-style detector-response hot path ("pd").
+ *
+ * What the library computes: the TorchDelphes chain of the Parnassus paper (arxiv/paper_2606_26089),
+ *   "particle propagation through the magnetic field, tracking efficiency, momentum smearing,
+ *    calorimeter response, and energy-flow merging, with per-module parameters loaded from the
+ *    selected detector card"                                   (section 1, L81 section 2.2)
+ * up to "calorimeter tower hits (Towers) and reconstructed photons, neutral hadrons, and charged
+ * tracks (EFlowObjects)" (App. D.1), for a batch of variable-length truth events
+ * ("no fixed model limit", Table 1).  The paper prints no formula for any step; the
+ * formulas are the readings A1..A32 of DESIGN.md (SURVEY.md section 8c.2/8c.3 + BASELINE.json configs).
+ *
+ * Conventions
+ *   - Plain C.  No exception crosses the boundary.  Every entry point returns 0 (PD_OK) or a negative
+ *     pd_status; pd_strerror() turns it into text.
+ *   - Units: GeV, metres, tesla (reading A1).  Pseudorapidity / azimuth in radians, phi in [-pi, pi].
+ *   - `pd_simulate` takes DEVICE pointers (memory of the current CUDA device, owned by the caller,
+ *     typically torch tensors) and a CUDA stream handle; it allocates nothing, launches its kernels
+ *     on that stream and returns without synchronising.  `pd_simulate_host` takes HOST pointers and
+ *     performs the host<->device copies itself (stream-ordered allocations), returning after the
+ *     results are in host memory.
+ *   - There is no CPU fallback: with no CUDA device both simulate calls fail with PD_ECUDA.
+ */
+#ifndef PD_H
+#define PD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  PD_OK = 0,
+  PD_EINVAL = -1,     /* null pointer, negative size, inconsistent arguments                 */
+  PD_ECARD = -2,      /* unknown card name or malformed card file                             */
+  PD_ECAPACITY = -3,  /* an output capacity is below the sufficient bound (see pd_simulate)    */
+  PD_EWORKSPACE = -4, /* workspace null or smaller than pd_workspace_bytes()                  */
+  PD_ECUDA = -5,      /* a CUDA runtime call failed (no device, launch error, ...)            */
+  PD_EEVENTSIZE = -6  /* device-side: a tile of events exceeded the on-chip capacity           */
+} pd_status;
+
+/* status byte of a propagated particle ("PropagatedParticle"): low two bits = face */
+enum { PD_DROPPED = 0, PD_BARREL = 1, PD_ENDCAP = 2, PD_FACE_MASK = 3, PD_LOOPER = 4 };
+/* object classes (charged hadron, electron, muon, neutral hadron, photon) */
+enum { PD_CLS_CHHAD = 0, PD_CLS_ELECTRON = 1, PD_CLS_MUON = 2, PD_CLS_NEUHAD = 3, PD_CLS_PHOTON = 4 };
+/* bits of pd_debug.tw_decisions (threshold decisions of steps S6/S7) */
+enum { PD_DEC_EEM = 1, PD_DEC_EHAD = 2, PD_DEC_NEM = 4, PD_DEC_NHAD = 8 };
+
+typedef struct pd_card pd_card; /* opaque, owned by the library; immutable after pd_load_card */
+
+typedef struct {
+  int32_t n_towers, n_eta_bins, grid_coord; /* grid_coord: 0 = eta edges, 1 = theta edges */
+  float bz, radius, half_length;            /* tesla, metres, metres                      */
+  int32_t n_eff_rows;
+} pd_card_info_t;
+
+/* Input: truth events in CSR form (BASELINE.json north_star: "events CSR: offsets, pid, charge, px,
+ * py, pz, E, vx, vy, vz").  Particle i of event e has index offsets[e] + i.  Non-finite values are
+ * undefined behaviour (reading A31). */
+typedef struct {
+  int64_t n_events;       /* >= 0                                                        */
+  int64_t n_particles;    /* == offsets[n_events]; < 2^31                                */
+  const int64_t *offsets; /* [n_events+1], offsets[0] == 0, non-decreasing               */
+  const int32_t *pid;     /* PDG id                                                      */
+  const int8_t *charge;   /* units of e; authoritative for charged/neutral               */
+  const float *px, *py, *pz, *E; /* GeV                                                  */
+  const float *vx, *vy, *vz;     /* production vertex, metres                            */
+} pd_events;
+
+/* Output collections (PAPER.md L329-342 Table A.6: Track, Tower, PFlow), CSR over the call's events.
+ * offsets[e] .. offsets[e+1] delimit event e; offsets[n_events] is the total.
+ * Order (reading A25): tracks in particle order; towers by ascending tower id; eflow = the event's
+ * tracks (particle order), then photons (ascending tower id), then neutral hadrons (ascending id). */
+typedef struct {
+  int64_t capacity;  /* elements available in every array below; must be >= n_particles   */
+  int64_t *offsets;  /* [n_events+1]                                                      */
+  int32_t *src;      /* index of the truth particle within the call                       */
+  int32_t *pid;
+  int8_t *charge;
+  float *pt, *eta, *phi, *E; /* smeared pT; direction of the vertex momentum; E = pT cosh(eta) */
+  float *eta_out, *phi_out;  /* position on the calorimeter face                          */
+} pd_tracks;
+
+typedef struct {
+  int64_t capacity; /* >= n_particles */
+  int64_t *offsets;
+  int32_t *tower;   /* tower id in the card's grid */
+  float *eta, *phi; /* tower centre */
+  float *E, *Eem, *Ehad, *ET;
+} pd_towers;
+
+typedef struct {
+  int64_t capacity; /* >= 2 * n_particles */
+  int64_t *offsets;
+  int8_t *cls;      /* PD_CLS_* */
+  int32_t *src;     /* tracks: truth particle index; neutrals: tower id */
+  float *pt, *eta, *phi, *E;
+} pd_eflow;
+
+/* Optional intermediate products (the paper's `debug` option, PAPER.md L589 / L669).  All arrays have
+ * n_particles elements; any pointer may be NULL.  The per-tower fields describe every tower that
+ * received a deposit (emitted or not) and are stored at the index of the FIRST particle (in particle
+ * order) that deposited into that (event, tower); tw_first marks those indices. */
+typedef struct {
+  uint8_t *status;   /* PD_DROPPED / PD_BARREL / PD_ENDCAP | PD_LOOPER                     */
+  float *eta_pos, *phi_pos; /* hit position on the calorimeter surface (NaN if dropped)    */
+  int32_t *tower;    /* geometric tower id of the hit, -1 if none                          */
+  uint8_t *accepted; /* 1 if the particle became a track                                   */
+  int8_t *eps_row;   /* row of the efficiency table used, -1 none                          */
+  float *pt_smeared; /* 0 if not an accepted track                                         */
+  uint8_t *tw_first;
+  float *tw_Eem_true, *tw_Ehad_true, *tw_Tem, *tw_Thad, *tw_Eem_smeared, *tw_Ehad_smeared;
+  uint8_t *tw_decisions; /* PD_DEC_* bits: 1 = "above threshold"                           */
+} pd_debug;
+
+/* Load a detector card: a built-in name ("cms_like" | "atlas_like" | "aleph_like", the parameter
+ * sets of BASELINE.json configs[0], [3], [4]) or the path of a card text file ("key = values" lines,
+ * '#' comments; keys name, bz, radius, half_length, kappa, grid (eta|theta), edges, nphi, eff,
+ * abs_costheta_max, track_res, ecal_res, hcal_res, ecal_thr, hcal_thr).  Pure host work: no CUDA
+ * call is made until the card is first used by a simulate call.  Every card number is rounded to
+ * fp32 at load (reading A28).  *out is owned by the library until pd_free_card. */
+int pd_load_card(const char *name_or_path, pd_card **out);
+void pd_free_card(pd_card *card);
+int pd_card_info(const pd_card *card, pd_card_info_t *out);
+
+/* Bytes of DEVICE workspace pd_simulate needs for a call of this size (look-back chains, tile
+ * counter, status word).  Negative pd_status on invalid arguments. */
+int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles);
+
+/* One pass of the whole chain S0..S8 over a batch of events.
+ *   events, tracks, towers, eflow, debug (nullable): structs in HOST memory whose pointer members
+ *     are DEVICE pointers.  Outputs are fully overwritten up to their totals.
+ *   seed, event_base: the Philox4x32-10 key is (seed lo, seed hi); the counter is (object, event lo,
+ *     event hi, stream << 16) with event = event_base + index in the call (readings A26, A27), so a
+ *     batch split over several calls / GPUs reproduces the single-call result bit for bit.
+ *   workspace: >= pd_workspace_bytes() bytes, 16-byte aligned, device memory; contents are scratch.
+ *   cuda_stream: a cudaStream_t (NULL = default stream).  Asynchronous: results are valid after the
+ *     caller synchronises the stream; pd_last_status() then reports device-side conditions.
+ * Errors are detected synchronously (PD_EINVAL, PD_ECAPACITY, PD_EWORKSPACE, PD_ECUDA); there is no
+ * device-side overflow path for the outputs because the capacities above are sufficient bounds. */
+int pd_simulate(const pd_card *card, const pd_events *events, uint64_t seed, int64_t event_base,
+                pd_tracks *tracks, pd_towers *towers, pd_eflow *eflow, pd_debug *debug,
+                void *workspace, int64_t workspace_bytes, void *cuda_stream);
+
+/* Reads back (synchronising the stream) the device-side status word a pd_simulate call left in its
+ * workspace: PD_OK, or PD_EEVENTSIZE if some tile of events did not fit on chip (its events then
+ * produced no objects). */
+int pd_last_status(const void *workspace, void *cuda_stream);
+
+/* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
+int pd_last_launch_count(void);
+
+/* Same computation with HOST pointers everywhere (inputs and outputs in host memory, pinned or
+ * pageable).  Copies inputs to the device, runs pd_simulate, copies the three collections back and
+ * synchronises.  Output capacities as for pd_simulate; totals are offsets[n_events]. */
+int pd_simulate_host(const pd_card *card, const pd_events *events, uint64_t seed, int64_t event_base,
+                     pd_tracks *tracks, pd_towers *towers, pd_eflow *eflow, void *cuda_stream);
+
+const char *pd_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PD_H */

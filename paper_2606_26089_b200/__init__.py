@@ -1,0 +1,7 @@
+"""pd: B200-native (sm_100a) Delphes-style detector-response hot path behind a C ABI (include/pd.h).
+
+`binding` marshals torch tensors into libpd.so; every step of the chain runs in its CUDA kernels.
+There is no CPU fallback."""
+from . import binding  # noqa: F401
+from .binding import (Card, DeviceEvents, DeviceOutputs, HostBuffers, PdError, last_launch_count, last_status,  # noqa: F401
+                      simulate, simulate_host, workspace_bytes)

@@ -1,0 +1,275 @@
+"""Thin ctypes binding of libpd.so (include/pd.h).  Argument marshalling only: every step of the chain
+runs in the CUDA kernels of the library.  torch is used for device memory and streams.
+
+There is no CPU fallback: if libpd.so cannot be built/loaded, importing `lib()` raises; if no CUDA
+device is present `simulate` raises PdError(PD_ECUDA)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+PD_OK, PD_EINVAL, PD_ECARD, PD_ECAPACITY, PD_EWORKSPACE, PD_ECUDA, PD_EEVENTSIZE = 0, -1, -2, -3, -4, -5, -6
+PD_DROPPED, PD_BARREL, PD_ENDCAP, PD_FACE_MASK, PD_LOOPER = 0, 1, 2, 3, 4
+PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
+
+# every symbol include/pd.h declares
+SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
+           "pd_last_launch_count", "pd_simulate_host", "pd_strerror")
+
+_p = C.c_void_p
+_lib = None
+
+
+class CardInfo(C.Structure):
+    _fields_ = [("n_towers", C.c_int32), ("n_eta_bins", C.c_int32), ("grid_coord", C.c_int32), ("bz", C.c_float),
+                ("radius", C.c_float), ("half_length", C.c_float), ("n_eff_rows", C.c_int32)]
+
+
+class Events(C.Structure):
+    _fields_ = [("n_events", C.c_int64), ("n_particles", C.c_int64), ("offsets", _p), ("pid", _p), ("charge", _p),
+                ("px", _p), ("py", _p), ("pz", _p), ("E", _p), ("vx", _p), ("vy", _p), ("vz", _p)]
+
+
+class Tracks(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("offsets", _p), ("src", _p), ("pid", _p), ("charge", _p), ("pt", _p),
+                ("eta", _p), ("phi", _p), ("E", _p), ("eta_out", _p), ("phi_out", _p)]
+
+
+class Towers(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("offsets", _p), ("tower", _p), ("eta", _p), ("phi", _p), ("E", _p),
+                ("Eem", _p), ("Ehad", _p), ("ET", _p)]
+
+
+class EFlow(C.Structure):
+    _fields_ = [("capacity", C.c_int64), ("offsets", _p), ("cls", _p), ("src", _p), ("pt", _p), ("eta", _p),
+                ("phi", _p), ("E", _p)]
+
+
+class Debug(C.Structure):
+    _fields_ = [("status", _p), ("eta_pos", _p), ("phi_pos", _p), ("tower", _p), ("accepted", _p), ("eps_row", _p),
+                ("pt_smeared", _p), ("tw_first", _p), ("tw_Eem_true", _p), ("tw_Ehad_true", _p), ("tw_Tem", _p),
+                ("tw_Thad", _p), ("tw_Eem_smeared", _p), ("tw_Ehad_smeared", _p), ("tw_decisions", _p)]
+
+
+TRACK_FIELDS = (("src", "int32"), ("pid", "int32"), ("charge", "int8"), ("pt", "float32"), ("eta", "float32"),
+                ("phi", "float32"), ("E", "float32"), ("eta_out", "float32"), ("phi_out", "float32"))
+TOWER_FIELDS = (("tower", "int32"), ("eta", "float32"), ("phi", "float32"), ("E", "float32"), ("Eem", "float32"),
+                ("Ehad", "float32"), ("ET", "float32"))
+EFLOW_FIELDS = (("cls", "int8"), ("src", "int32"), ("pt", "float32"), ("eta", "float32"), ("phi", "float32"),
+                ("E", "float32"))
+DEBUG_FIELDS = (("status", "uint8"), ("eta_pos", "float32"), ("phi_pos", "float32"), ("tower", "int32"),
+                ("accepted", "uint8"), ("eps_row", "int8"), ("pt_smeared", "float32"), ("tw_first", "uint8"),
+                ("tw_Eem_true", "float32"), ("tw_Ehad_true", "float32"), ("tw_Tem", "float32"), ("tw_Thad", "float32"),
+                ("tw_Eem_smeared", "float32"), ("tw_Ehad_smeared", "float32"), ("tw_decisions", "uint8"))
+EVENT_FIELDS = (("offsets", "int64"), ("pid", "int32"), ("charge", "int8"), ("px", "float32"), ("py", "float32"),
+                ("pz", "float32"), ("E", "float32"), ("vx", "float32"), ("vy", "float32"), ("vz", "float32"))
+
+
+def lib():
+    """Load libpd.so (building it in-tree if stale).  Raises if that is impossible: no fallback."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path) or os.environ.get("PD_REBUILD"):
+            path = _build.build()
+        L = C.CDLL(path)
+        L.pd_load_card.argtypes = [C.c_char_p, C.POINTER(_p)]
+        L.pd_free_card.argtypes = [_p]
+        L.pd_free_card.restype = None
+        L.pd_card_info.argtypes = [_p, C.POINTER(CardInfo)]
+        L.pd_workspace_bytes.argtypes = [_p, C.c_int64, C.c_int64]
+        L.pd_workspace_bytes.restype = C.c_int64
+        L.pd_simulate.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks), C.POINTER(Towers),
+                                  C.POINTER(EFlow), C.POINTER(Debug), _p, C.c_int64, _p]
+        L.pd_last_status.argtypes = [_p, _p]
+        L.pd_last_launch_count.argtypes = []
+        L.pd_simulate_host.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks),
+                                       C.POINTER(Towers), C.POINTER(EFlow), _p]
+        L.pd_strerror.argtypes = [C.c_int]
+        L.pd_strerror.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+class PdError(RuntimeError):
+    def __init__(self, code):
+        super().__init__("pd: %s (code %d)" % (lib().pd_strerror(int(code)).decode(), int(code)))
+        self.code = int(code)
+
+
+def _check(rc):
+    if rc != PD_OK:
+        raise PdError(rc)
+
+
+class Card:
+    """pd_load_card / pd_card_info / pd_free_card."""
+
+    def __init__(self, name_or_path: str):
+        self._h = _p()
+        _check(lib().pd_load_card(str(name_or_path).encode(), C.byref(self._h)))
+        info = CardInfo()
+        _check(lib().pd_card_info(self._h, C.byref(info)))
+        self.n_towers, self.n_bins, self.grid_coord = info.n_towers, info.n_eta_bins, info.grid_coord
+        self.bz, self.radius, self.half_length, self.n_eff_rows = info.bz, info.radius, info.half_length, info.n_eff_rows
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            try:
+                lib().pd_free_card(self._h)
+            except Exception:
+                pass
+            self._h = None
+
+
+def workspace_bytes(card: Card, n_events: int, n_particles: int) -> int:
+    n = lib().pd_workspace_bytes(card._h, int(n_events), int(n_particles))
+    if n < 0:
+        raise PdError(n)
+    return int(n)
+
+
+def last_launch_count() -> int:
+    return int(lib().pd_last_launch_count())
+
+
+def _torch():
+    import torch
+
+    return torch
+
+
+def _tptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class DeviceEvents:
+    """Truth events resident in device memory (torch tensors), CSR."""
+
+    def __init__(self, ev, device="cuda"):
+        torch = _torch()
+        self.n_events = int(ev.offsets.shape[0] - 1)
+        self.n_particles = int(ev.offsets[-1])
+        self.t = {}
+        for name, dt in EVENT_FIELDS:
+            a = np.ascontiguousarray(getattr(ev, name), dtype=dt)
+            self.t[name] = torch.from_numpy(a).to(device)
+        self.c = Events(self.n_events, self.n_particles, *[_tptr(self.t[k]) for k, _ in EVENT_FIELDS])
+
+    def nbytes(self):
+        return sum(t.numel() * t.element_size() for t in self.t.values())
+
+
+class DeviceOutputs:
+    """Output buffers (torch tensors) sized to the sufficient bounds of pd.h, plus the workspace."""
+
+    def __init__(self, card: Card, n_events: int, n_particles: int, debug: bool = False, device="cuda"):
+        torch = _torch()
+        n = max(int(n_particles), 1)
+        self.n_events, self.n_particles = int(n_events), int(n_particles)
+        mk = lambda m, dt: torch.empty(m, dtype=getattr(torch, dt), device=device)  # noqa: E731
+        self.trk = {"offsets": mk(n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TRACK_FIELDS}}
+        self.tow = {"offsets": mk(n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TOWER_FIELDS}}
+        self.efl = {"offsets": mk(n_events + 1, "int64"), **{k: mk(2 * n, dt) for k, dt in EFLOW_FIELDS}}
+        self.dbg = {k: mk(n, dt) for k, dt in DEBUG_FIELDS} if debug else None
+        self.ws_bytes = workspace_bytes(card, n_events, n_particles)
+        self.ws = torch.empty(self.ws_bytes + 16, dtype=torch.uint8, device=device)
+        self.c_trk = Tracks(n, _tptr(self.trk["offsets"]), *[_tptr(self.trk[k]) for k, _ in TRACK_FIELDS])
+        self.c_tow = Towers(n, _tptr(self.tow["offsets"]), *[_tptr(self.tow[k]) for k, _ in TOWER_FIELDS])
+        self.c_efl = EFlow(2 * n, _tptr(self.efl["offsets"]), *[_tptr(self.efl[k]) for k, _ in EFLOW_FIELDS])
+        self.c_dbg = Debug(*[_tptr(self.dbg[k]) for k, _ in DEBUG_FIELDS]) if debug else None
+
+    def to_numpy(self) -> dict:
+        """Synchronise and return trimmed numpy arrays: trk_*, tow_*, efl_*, dbg_*."""
+        torch = _torch()
+        torch.cuda.synchronize()
+        out = {}
+        for prefix, d in (("trk", self.trk), ("tow", self.tow), ("efl", self.efl)):
+            off = d["offsets"].cpu().numpy()
+            tot = int(off[-1])
+            out[prefix + "_offsets"] = off
+            for k, t in d.items():
+                if k != "offsets":
+                    out["%s_%s" % (prefix, k)] = t[:tot].cpu().numpy()
+        if self.dbg is not None:
+            for k, t in self.dbg.items():
+                out["dbg_" + k] = t[: self.n_particles].cpu().numpy()
+        return out
+
+
+def simulate(card: Card, dev_events: DeviceEvents, out: DeviceOutputs, seed: int, event_base: int = 0, stream=None):
+    """pd_simulate on torch's current stream (or `stream`).  Asynchronous."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    rc = lib().pd_simulate(card._h, C.byref(dev_events.c), int(seed) & (2**64 - 1), int(event_base), C.byref(out.c_trk),
+                           C.byref(out.c_tow), C.byref(out.c_efl), C.byref(out.c_dbg) if out.c_dbg is not None else None,
+                           _tptr(out.ws), out.ws_bytes, C.c_void_p(st.cuda_stream))
+    _check(rc)
+
+
+def last_status(out: DeviceOutputs, stream=None) -> int:
+    torch = _torch()
+    st = torch.cuda.current_stream() if stream is None else stream
+    return int(lib().pd_last_status(_tptr(out.ws), C.c_void_p(st.cuda_stream)))
+
+
+class HostBuffers:
+    """Pinned host buffers for pd_simulate_host (the end-to-end path)."""
+
+    def __init__(self, ev, pin=True):
+        torch = _torch()
+        self.n_events = int(ev.offsets.shape[0] - 1)
+        self.n_particles = int(ev.offsets[-1])
+        n = max(self.n_particles, 1)
+        pin = bool(pin and torch.cuda.is_available())
+
+        def host(a):
+            t = torch.from_numpy(np.ascontiguousarray(a))
+            return t.pin_memory() if pin else t
+
+        self.ev = {name: host(np.ascontiguousarray(getattr(ev, name), dtype=dt)) for name, dt in EVENT_FIELDS}
+        mk = lambda m, dt: torch.empty(m, dtype=getattr(torch, dt), pin_memory=pin)  # noqa: E731
+        self.trk = {"offsets": mk(self.n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TRACK_FIELDS}}
+        self.tow = {"offsets": mk(self.n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TOWER_FIELDS}}
+        self.efl = {"offsets": mk(self.n_events + 1, "int64"), **{k: mk(2 * n, dt) for k, dt in EFLOW_FIELDS}}
+        self.c_ev = Events(self.n_events, self.n_particles, *[_tptr(self.ev[k]) for k, _ in EVENT_FIELDS])
+        self.c_trk = Tracks(n, _tptr(self.trk["offsets"]), *[_tptr(self.trk[k]) for k, _ in TRACK_FIELDS])
+        self.c_tow = Towers(n, _tptr(self.tow["offsets"]), *[_tptr(self.tow[k]) for k, _ in TOWER_FIELDS])
+        self.c_efl = EFlow(2 * n, _tptr(self.efl["offsets"]), *[_tptr(self.efl[k]) for k, _ in EFLOW_FIELDS])
+
+    def h2d_bytes(self):
+        return sum(t.numel() * t.element_size() for t in self.ev.values())
+
+    def d2h_bytes(self):
+        b = 3 * 8 * (self.n_events + 1)
+        for d, fields in ((self.trk, TRACK_FIELDS), (self.tow, TOWER_FIELDS), (self.efl, EFLOW_FIELDS)):
+            tot = int(d["offsets"][-1])
+            b += tot * sum(np.dtype(dt).itemsize for _, dt in fields)
+        return b
+
+    def to_numpy(self) -> dict:
+        out = {}
+        for prefix, d in (("trk", self.trk), ("tow", self.tow), ("efl", self.efl)):
+            off = d["offsets"].numpy()
+            tot = int(off[-1])
+            out[prefix + "_offsets"] = off.copy()
+            for k, t in d.items():
+                if k != "offsets":
+                    out["%s_%s" % (prefix, k)] = t[:tot].numpy().copy()
+        return out
+
+
+def simulate_host(card: Card, hb: HostBuffers, seed: int, event_base: int = 0, stream=None):
+    """pd_simulate_host: host buffers in, host buffers out, copies inside the call.  Synchronous."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().pd_simulate_host(card._h, C.byref(hb.c_ev), int(seed) & (2**64 - 1), int(event_base), C.byref(hb.c_trk),
+                                  C.byref(hb.c_tow), C.byref(hb.c_efl), C.c_void_p(st.cuda_stream)))

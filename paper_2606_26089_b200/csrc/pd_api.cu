@@ -1,0 +1,317 @@
+// pd_api.cu -- the C ABI of libpd (include/pd.h): argument checking, card upload, workspace layout,
+// kernel launch, and the host-pointer convenience entry point.  No torch types, no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+
+#include "pd_internal.h"
+
+namespace {
+
+thread_local int t_launches = 0;
+thread_local char t_cuda_msg[256] = "";
+std::mutex g_card_mutex;
+
+constexpr size_t kWsHeader = 16;  // tile counter (u32), status word (i32), padding
+
+int cuda_fail(cudaError_t e, const char *what) {
+  std::snprintf(t_cuda_msg, sizeof(t_cuda_msg), "CUDA error in %s: %s", what, cudaGetErrorString(e));
+  return PD_ECUDA;
+}
+
+#define PD_CUDA(call)                                   \
+  do {                                                  \
+    cudaError_t e__ = (call);                           \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+  } while (0)
+
+}  // namespace
+
+extern "C" {
+
+const char *pd_strerror(int code) {
+  switch (code) {
+    case PD_OK: return "ok";
+    case PD_EINVAL: return "invalid argument";
+    case PD_ECARD: return "unknown card name or malformed card file";
+    case PD_ECAPACITY: return "output capacity below the sufficient bound";
+    case PD_EWORKSPACE: return "workspace missing or too small";
+    case PD_ECUDA: return t_cuda_msg[0] ? t_cuda_msg : "CUDA runtime error";
+    case PD_EEVENTSIZE: return "a tile of events exceeded the on-chip capacity";
+    default: return "unknown error";
+  }
+}
+
+int pd_load_card(const char *name_or_path, pd_card **out) {
+  if (!name_or_path || !out) return PD_EINVAL;
+  pd_card *c = new (std::nothrow) pd_card();
+  if (!c) return PD_EINVAL;
+  const int rc = pd_card_parse(name_or_path, c);
+  if (rc != PD_OK) {
+    delete c;
+    return rc;
+  }
+  *out = c;
+  return PD_OK;
+}
+
+void pd_free_card(pd_card *card) {
+  if (!card) return;
+  if (card->dev_blob) cudaFree(card->dev_blob);
+  delete card;
+}
+
+int pd_card_info(const pd_card *card, pd_card_info_t *out) {
+  if (!card || !out) return PD_EINVAL;
+  out->n_towers = card->sc.n_towers;
+  out->n_eta_bins = card->sc.n_bins;
+  out->grid_coord = card->sc.grid_theta;
+  out->bz = card->bz;
+  out->radius = card->sc.R;
+  out->half_length = card->sc.L;
+  out->n_eff_rows = card->sc.n_eff;
+  return PD_OK;
+}
+
+int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles) {
+  if (!card || n_events < 0 || n_particles < 0) return PD_EINVAL;
+  PdLaunchPlan plan;
+  pd_plan(card, n_events, n_particles, &plan);
+  return (int64_t)(kWsHeader + 3 * sizeof(unsigned long long) * (size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1));
+}
+
+int pd_last_launch_count(void) { return t_launches; }
+
+}  // extern "C"
+
+// Upload the per-bin tables of a card to the current device (once).
+int pd_card_to_device(const pd_card *c) {
+  std::lock_guard<std::mutex> lock(g_card_mutex);
+  int dev = 0;
+  PD_CUDA(cudaGetDevice(&dev));
+  if (c->dev_blob && c->dev_id == dev) return PD_OK;
+  if (c->dev_blob) {
+    cudaFree(c->dev_blob);
+    c->dev_blob = nullptr;
+  }
+  const size_t nb = (size_t)c->sc.n_bins;
+  const size_t words = (nb + 1) + nb + (nb + 1) + 5 * nb;
+  std::vector<uint32_t> blob(words);
+  size_t o = 0;
+  auto put = [&](const void *src, size_t n) {
+    std::memcpy(blob.data() + o, src, 4 * n);
+    size_t at = o;
+    o += n;
+    return at;
+  };
+  const size_t o_tb = put(c->tb.data(), nb + 1), o_nphi = put(c->nphi.data(), nb), o_off = put(c->offset.data(), nb + 1);
+  const size_t o_iw = put(c->inv_w.data(), nb), o_half = put(c->half.data(), nb), o_w = put(c->w.data(), nb);
+  const size_t o_eta = put(c->eta_c.data(), nb), o_ic = put(c->inv_cosh.data(), nb);
+  void *d = nullptr;
+  PD_CUDA(cudaMalloc(&d, 4 * words));
+  cudaError_t e = cudaMemcpy(d, blob.data(), 4 * words, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(d);
+    return cuda_fail(e, "cudaMemcpy(card)");
+  }
+  const uint32_t *base = (const uint32_t *)d;
+  c->dev_tab.tb = (const float *)(base + o_tb);
+  c->dev_tab.nphi = (const int *)(base + o_nphi);
+  c->dev_tab.offset = (const int *)(base + o_off);
+  c->dev_tab.inv_w = (const float *)(base + o_iw);
+  c->dev_tab.half = (const float *)(base + o_half);
+  c->dev_tab.w = (const float *)(base + o_w);
+  c->dev_tab.eta_c = (const float *)(base + o_eta);
+  c->dev_tab.inv_cosh = (const float *)(base + o_ic);
+  c->dev_blob = d;
+  c->dev_id = dev;
+  return PD_OK;
+}
+
+extern "C" {
+
+int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                pd_towers *tow, pd_eflow *efl, pd_debug *dbg, void *workspace, int64_t workspace_bytes,
+                void *cuda_stream) {
+  t_launches = 0;
+  if (!card || !ev || !trk || !tow || !efl) return PD_EINVAL;
+  if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 31)) return PD_EINVAL;
+  if (!ev->offsets || !trk->offsets || !tow->offsets || !efl->offsets) return PD_EINVAL;
+  const int64_t n = ev->n_particles;
+  if (n > 0) {
+    if (!ev->pid || !ev->charge || !ev->px || !ev->py || !ev->pz || !ev->E || !ev->vx || !ev->vy || !ev->vz) return PD_EINVAL;
+    if (!trk->src || !trk->pid || !trk->charge || !trk->pt || !trk->eta || !trk->phi || !trk->E || !trk->eta_out || !trk->phi_out) return PD_EINVAL;
+    if (!tow->tower || !tow->eta || !tow->phi || !tow->E || !tow->Eem || !tow->Ehad || !tow->ET) return PD_EINVAL;
+    if (!efl->cls || !efl->src || !efl->pt || !efl->eta || !efl->phi || !efl->E) return PD_EINVAL;
+  }
+  if (trk->capacity < n || tow->capacity < n || efl->capacity < 2 * n) return PD_ECAPACITY;
+  const int64_t need = pd_workspace_bytes(card, ev->n_events, n);
+  if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15u)) return PD_EWORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+
+  PD_CUDA(cudaMemsetAsync(workspace, 0, (size_t)need, st));
+  if (ev->n_events == 0) {
+    PD_CUDA(cudaMemsetAsync(trk->offsets, 0, sizeof(int64_t), st));
+    PD_CUDA(cudaMemsetAsync(tow->offsets, 0, sizeof(int64_t), st));
+    PD_CUDA(cudaMemsetAsync(efl->offsets, 0, sizeof(int64_t), st));
+    return PD_OK;
+  }
+  int rc = pd_card_to_device(card);
+  if (rc != PD_OK) return rc;
+
+  PdLaunchPlan plan;
+  pd_plan(card, ev->n_events, n, &plan);
+
+  PdParams p;
+  std::memset(&p, 0, sizeof(p));
+  p.sc = card->sc;
+  p.tab = card->dev_tab;
+  p.n_events = ev->n_events, p.n_particles = n;
+  p.offsets = (const long long *)ev->offsets;
+  p.pid = ev->pid, p.charge = ev->charge;
+  p.px = ev->px, p.py = ev->py, p.pz = ev->pz, p.E = ev->E, p.vx = ev->vx, p.vy = ev->vy, p.vz = ev->vz;
+  p.seed = seed, p.event_base = event_base;
+  p.trk_offsets = (long long *)trk->offsets;
+  p.trk_src = trk->src, p.trk_pid = trk->pid, p.trk_charge = trk->charge;
+  p.trk_pt = trk->pt, p.trk_eta = trk->eta, p.trk_phi = trk->phi, p.trk_E = trk->E;
+  p.trk_eta_out = trk->eta_out, p.trk_phi_out = trk->phi_out;
+  p.tow_offsets = (long long *)tow->offsets;
+  p.tow_tower = tow->tower, p.tow_eta = tow->eta, p.tow_phi = tow->phi, p.tow_E = tow->E;
+  p.tow_Eem = tow->Eem, p.tow_Ehad = tow->Ehad, p.tow_ET = tow->ET;
+  p.efl_offsets = (long long *)efl->offsets;
+  p.efl_cls = efl->cls, p.efl_src = efl->src, p.efl_pt = efl->pt, p.efl_eta = efl->eta, p.efl_phi = efl->phi, p.efl_E = efl->E;
+  if (dbg) {
+    p.dbg_status = dbg->status, p.dbg_eta_pos = dbg->eta_pos, p.dbg_phi_pos = dbg->phi_pos, p.dbg_tower = dbg->tower;
+    p.dbg_accepted = dbg->accepted, p.dbg_eps_row = dbg->eps_row, p.dbg_pt_smeared = dbg->pt_smeared;
+    p.dbg_tw_first = dbg->tw_first;
+    p.dbg_tw[0] = dbg->tw_Eem_true, p.dbg_tw[1] = dbg->tw_Ehad_true, p.dbg_tw[2] = dbg->tw_Tem, p.dbg_tw[3] = dbg->tw_Thad;
+    p.dbg_tw[4] = dbg->tw_Eem_smeared, p.dbg_tw[5] = dbg->tw_Ehad_smeared;
+    p.dbg_tw_dec = dbg->tw_decisions;
+  }
+  p.events_per_tile = plan.events_per_tile;
+  p.n_tiles = plan.n_tiles;
+  p.capacity = plan.capacity;
+  p.event_bits = plan.event_bits;
+  unsigned char *ws = (unsigned char *)workspace;
+  p.tile_counter = (unsigned int *)ws;
+  p.status_word = (int *)(ws + 4);
+  p.chain = (unsigned long long *)(ws + kWsHeader);
+
+  rc = pd_launch_chain(p, plan, dbg != nullptr, cuda_stream);
+  if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "kernel launch");
+  t_launches = 1;
+  return PD_OK;
+}
+
+int pd_last_status(const void *workspace, void *cuda_stream) {
+  if (!workspace) return PD_EINVAL;
+  int word = 0;
+  PD_CUDA(cudaMemcpyAsync(&word, (const unsigned char *)workspace + 4, sizeof(int), cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
+  PD_CUDA(cudaStreamSynchronize((cudaStream_t)cuda_stream));
+  return word;
+}
+
+int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                     pd_towers *tow, pd_eflow *efl, void *cuda_stream) {
+  t_launches = 0;
+  if (!card || !ev || !trk || !tow || !efl) return PD_EINVAL;
+  if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 31)) return PD_EINVAL;
+  if (!ev->offsets || !trk->offsets || !tow->offsets || !efl->offsets) return PD_EINVAL;
+  const int64_t n = ev->n_particles, ne = ev->n_events;
+  if (trk->capacity < n || tow->capacity < n || efl->capacity < 2 * n) return PD_ECAPACITY;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t np = (size_t)(n > 0 ? n : 1);
+  const int64_t ws_bytes = pd_workspace_bytes(card, ne, n);
+  // one stream-ordered allocation, carved up (256-byte aligned pieces)
+  auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  const size_t b_off = up(8 * (size_t)(ne + 1));
+  const size_t in_bytes = b_off + up(4 * np) + up(np) + 7 * up(4 * np);
+  const size_t trk_bytes = b_off + 2 * up(4 * np) + up(np) + 6 * up(4 * np);
+  const size_t tow_bytes = b_off + up(4 * np) + 6 * up(4 * np);
+  const size_t efl_bytes = b_off + up(2 * np) + up(8 * np) + 4 * up(8 * np);
+  const size_t total = in_bytes + trk_bytes + tow_bytes + efl_bytes + up((size_t)ws_bytes);
+  unsigned char *base = nullptr;
+  PD_CUDA(cudaMallocAsync((void **)&base, total, st));
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    unsigned char *ptr = base + o;
+    o += up(bytes);
+    return ptr;
+  };
+  int rc = PD_OK;
+  pd_events d_ev = *ev;
+  pd_tracks d_trk = *trk;
+  pd_towers d_tow = *tow;
+  pd_eflow d_efl = *efl;
+  cudaError_t ce = cudaSuccess;
+  auto h2d = [&](const void *src, size_t bytes) {
+    unsigned char *dst = take(bytes);
+    if (ce == cudaSuccess && bytes > 0 && src) ce = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
+    return dst;
+  };
+  d_ev.offsets = (const int64_t *)h2d(ev->offsets, 8 * (size_t)(ne + 1));
+  d_ev.pid = (const int32_t *)h2d(ev->pid, 4 * (size_t)n);
+  d_ev.charge = (const int8_t *)h2d(ev->charge, (size_t)n);
+  d_ev.px = (const float *)h2d(ev->px, 4 * (size_t)n);
+  d_ev.py = (const float *)h2d(ev->py, 4 * (size_t)n);
+  d_ev.pz = (const float *)h2d(ev->pz, 4 * (size_t)n);
+  d_ev.E = (const float *)h2d(ev->E, 4 * (size_t)n);
+  d_ev.vx = (const float *)h2d(ev->vx, 4 * (size_t)n);
+  d_ev.vy = (const float *)h2d(ev->vy, 4 * (size_t)n);
+  d_ev.vz = (const float *)h2d(ev->vz, 4 * (size_t)n);
+  d_trk.offsets = (int64_t *)take(8 * (size_t)(ne + 1));
+  d_trk.src = (int32_t *)take(4 * np), d_trk.pid = (int32_t *)take(4 * np), d_trk.charge = (int8_t *)take(np);
+  d_trk.pt = (float *)take(4 * np), d_trk.eta = (float *)take(4 * np), d_trk.phi = (float *)take(4 * np);
+  d_trk.E = (float *)take(4 * np), d_trk.eta_out = (float *)take(4 * np), d_trk.phi_out = (float *)take(4 * np);
+  d_tow.offsets = (int64_t *)take(8 * (size_t)(ne + 1));
+  d_tow.tower = (int32_t *)take(4 * np);
+  d_tow.eta = (float *)take(4 * np), d_tow.phi = (float *)take(4 * np), d_tow.E = (float *)take(4 * np);
+  d_tow.Eem = (float *)take(4 * np), d_tow.Ehad = (float *)take(4 * np), d_tow.ET = (float *)take(4 * np);
+  d_efl.offsets = (int64_t *)take(8 * (size_t)(ne + 1));
+  d_efl.cls = (int8_t *)take(2 * np), d_efl.src = (int32_t *)take(8 * np);
+  d_efl.pt = (float *)take(8 * np), d_efl.eta = (float *)take(8 * np), d_efl.phi = (float *)take(8 * np), d_efl.E = (float *)take(8 * np);
+  void *ws = take((size_t)ws_bytes);
+  if (ce != cudaSuccess) rc = cuda_fail(ce, "cudaMemcpyAsync(H2D)");
+  if (rc == PD_OK) rc = pd_simulate(card, &d_ev, seed, event_base, &d_trk, &d_tow, &d_efl, nullptr, ws, ws_bytes, cuda_stream);
+  const int launches = t_launches;
+  int64_t tot[3] = {0, 0, 0};
+  if (rc == PD_OK) {
+    // totals first (three 8-byte reads), then exactly the produced elements
+    ce = cudaMemcpyAsync(&tot[0], d_trk.offsets + ne, 8, cudaMemcpyDeviceToHost, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(&tot[1], d_tow.offsets + ne, 8, cudaMemcpyDeviceToHost, st);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(&tot[2], d_efl.offsets + ne, 8, cudaMemcpyDeviceToHost, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) rc = cuda_fail(ce, "read totals");
+  }
+  if (rc == PD_OK) {
+    auto d2h = [&](void *dst, const void *src, size_t bytes) {
+      if (ce == cudaSuccess && bytes > 0 && dst) ce = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
+    };
+    const size_t nt = (size_t)tot[0], nw = (size_t)tot[1], nf = (size_t)tot[2], nofs = 8 * (size_t)(ne + 1);
+    d2h(trk->offsets, d_trk.offsets, nofs);
+    d2h(trk->src, d_trk.src, 4 * nt), d2h(trk->pid, d_trk.pid, 4 * nt), d2h(trk->charge, d_trk.charge, nt);
+    d2h(trk->pt, d_trk.pt, 4 * nt), d2h(trk->eta, d_trk.eta, 4 * nt), d2h(trk->phi, d_trk.phi, 4 * nt);
+    d2h(trk->E, d_trk.E, 4 * nt), d2h(trk->eta_out, d_trk.eta_out, 4 * nt), d2h(trk->phi_out, d_trk.phi_out, 4 * nt);
+    d2h(tow->offsets, d_tow.offsets, nofs);
+    d2h(tow->tower, d_tow.tower, 4 * nw), d2h(tow->eta, d_tow.eta, 4 * nw), d2h(tow->phi, d_tow.phi, 4 * nw);
+    d2h(tow->E, d_tow.E, 4 * nw), d2h(tow->Eem, d_tow.Eem, 4 * nw), d2h(tow->Ehad, d_tow.Ehad, 4 * nw), d2h(tow->ET, d_tow.ET, 4 * nw);
+    d2h(efl->offsets, d_efl.offsets, nofs);
+    d2h(efl->cls, d_efl.cls, nf), d2h(efl->src, d_efl.src, 4 * nf), d2h(efl->pt, d_efl.pt, 4 * nf);
+    d2h(efl->eta, d_efl.eta, 4 * nf), d2h(efl->phi, d_efl.phi, 4 * nf), d2h(efl->E, d_efl.E, 4 * nf);
+    int word = 0;
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(&word, (unsigned char *)ws + 4, 4, cudaMemcpyDeviceToHost, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    if (ce != cudaSuccess) rc = cuda_fail(ce, "cudaMemcpyAsync(D2H)");
+    else if (word != 0) rc = word;
+  }
+  cudaFreeAsync(base, st);
+  cudaStreamSynchronize(st);
+  t_launches = launches;
+  return rc;
+}
+
+}  // extern "C"

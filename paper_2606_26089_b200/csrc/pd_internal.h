@@ -1,0 +1,116 @@
+// pd_internal.h -- types shared by the host side (card loader, API) and the kernels of libpd.
+// Product code: shares nothing with oracle/ (see DESIGN.md "Independence").
+#pragma once
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "pd.h"
+
+constexpr int PD_MAX_BINS = 1024;  // eta/theta bins of a card's grid
+constexpr int PD_MAX_EFF = 32;     // rows of the efficiency table
+constexpr int PD_MAX_TOWER_BITS = 15;
+
+// Scalars of a card as the kernels want them (all derived in double at load, stored as fp32).
+struct PdCardScalars {
+  float R, L, R2;        // calorimeter radius, half length, R^2
+  float kB;              // kappa * |B|   [GeV / m]
+  double kB_d;           // same in double (only used for the endcap turning angle)
+  float sB;              // sign of B (0 if B == 0)
+  int grid_theta;        // 0: bins in eta, 1: bins in theta
+  int n_bins, n_towers, tower_bits;
+  int n_eff, has_cos;
+  float t_cos;           // |pz|/pT threshold equivalent to |cos theta| >= abs_costheta_max
+  float trk_a2, trk_b;   // sigma_rel^2 = a^2 + (b pT)^2
+  float ecal2[3], hcal2[3];  // C^2, S^2, N^2 of sigma^2 = C^2 E^2 + S^2 E + N^2
+  float thr_ecal, thr_hcal;
+  float eff[PD_MAX_EFF][5];  // pt_lo, pt_hi, sinh(|eta|_lo) (<= 0: no lower cut), sinh(|eta|_hi), eps
+};
+
+// Per-bin tables, each n_bins (+1 for tb / offset) long, contiguous in one device allocation.
+struct PdCardTables {
+  const float *tb;        // [n_bins+1] bin thresholds in u = z/r (eta grid) or -z/r (theta grid)
+  const int *nphi;        // [n_bins]
+  const int *offset;      // [n_bins+1] exclusive prefix sum of nphi
+  const float *inv_w;     // [n_bins] nphi / (2 pi)
+  const float *half;      // [n_bins] 0.5 if nphi odd else 0
+  const float *w;         // [n_bins] 2 pi / nphi
+  const float *eta_c;     // [n_bins] tower-centre pseudorapidity
+  const float *inv_cosh;  // [n_bins] 1 / cosh(eta_c)
+};
+
+struct pd_card {
+  std::string name;
+  // host copy (rounded to fp32 where the kernels use fp32)
+  PdCardScalars sc{};
+  std::vector<float> edges;  // [n_bins+1] the card's edges (eta or theta), fp32
+  std::vector<float> tb, inv_w, half, w, eta_c, inv_cosh;
+  std::vector<int> nphi, offset;
+  float bz = 0.f;
+  // device copy, created lazily by the first simulate call
+  mutable void *dev_blob = nullptr;
+  mutable int dev_id = -1;
+  mutable PdCardTables dev_tab{};
+};
+
+// Kernel parameters (passed by value).
+struct PdParams {
+  PdCardScalars sc;
+  PdCardTables tab;
+  // inputs
+  long long n_events, n_particles;
+  const long long *offsets;
+  const int *pid;
+  const signed char *charge;
+  const float *px, *py, *pz, *E, *vx, *vy, *vz;
+  unsigned long long seed;
+  long long event_base;
+  // outputs
+  long long *trk_offsets;
+  int *trk_src, *trk_pid;
+  signed char *trk_charge;
+  float *trk_pt, *trk_eta, *trk_phi, *trk_E, *trk_eta_out, *trk_phi_out;
+  long long *tow_offsets;
+  int *tow_tower;
+  float *tow_eta, *tow_phi, *tow_E, *tow_Eem, *tow_Ehad, *tow_ET;
+  long long *efl_offsets;
+  signed char *efl_cls;
+  int *efl_src;
+  float *efl_pt, *efl_eta, *efl_phi, *efl_E;
+  // debug (all nullable)
+  unsigned char *dbg_status;
+  float *dbg_eta_pos, *dbg_phi_pos;
+  int *dbg_tower;
+  unsigned char *dbg_accepted;
+  signed char *dbg_eps_row;
+  float *dbg_pt_smeared;
+  unsigned char *dbg_tw_first;
+  float *dbg_tw[6];
+  unsigned char *dbg_tw_dec;
+  // tiling / workspace
+  int events_per_tile;   // G
+  int n_tiles;
+  int capacity;          // C: particles a tile may hold on chip
+  int event_bits;        // bits needed for a local event index
+  unsigned long long *chain;  // [3][n_tiles] look-back words: tracks, towers, eflow
+  unsigned int *tile_counter;
+  int *status_word;
+};
+
+// pd_card.cpp
+int pd_card_parse(const char *name_or_path, pd_card *c);
+// pd_api.cu
+int pd_card_to_device(const pd_card *c);
+// pd_kernels.cu
+struct PdLaunchPlan {
+  int threads;       // 256 or 512
+  int capacity;      // C
+  int events_per_tile;
+  int n_tiles;
+  int event_bits;
+  size_t smem_bytes;
+  int grid;
+};
+int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);
+int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, void *stream);

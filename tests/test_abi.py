@@ -1,0 +1,76 @@
+"""CPU tests of the boundary: libpd.so builds, loads and exports every symbol include/pd.h declares;
+card loading (pure host work) agrees with the oracle's independent loader; argument checking works
+without a GPU.  No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2606_26089_b200 import binding as B
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "pd.h")).read()
+    declared = set(re.findall(r"\b(pd_[a-z_]+)\s*\(", hdr))
+    assert declared == set(B.SYMBOLS), declared ^ set(B.SYMBOLS)
+    L = B.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+@pytest.mark.parametrize("name,towers,bins,coord", [("cms_like", 5904, 94, 0), ("atlas_like", 4096, 64, 0), ("aleph_like", 19320, 92, 1)])
+def test_builtin_cards_match_oracle_loader(name, towers, bins, coord):
+    from oracle import pdo
+
+    c = B.Card(name)
+    o = pdo.Card(name)
+    assert (c.n_towers, c.n_bins, c.grid_coord) == (towers, bins, coord) == (o.n_towers, o.n_bins, o.grid_coord)
+    assert (c.bz, c.radius, c.half_length, c.n_eff_rows) == (o.bz, o.radius, o.half_length, o.n_eff_rows)
+
+
+def test_card_file_and_errors(tmp_path):
+    from oracle import pdo
+    from tests import cards
+
+    o = pdo.Card("cms_like")
+    path = cards.variant(tmp_path / "v.card", o.edges, o.nphi, bz=-2.5, ecal_thr=0.0)
+    c = B.Card(path)
+    assert c.n_towers == 5904 and abs(c.bz + 2.5) < 1e-6
+    with pytest.raises(B.PdError) as e:
+        B.Card("no_such_card")
+    assert e.value.code == B.PD_ECARD
+    bad = tmp_path / "bad.card"
+    bad.write_text("bz = 1\nradius = 1\nhalf_length = 1\nedges = 0 1 0.5\nnphi = 4 4\n")
+    with pytest.raises(B.PdError):
+        B.Card(str(bad))
+
+
+def test_argument_checking_without_gpu():
+    L = B.lib()
+    c = B.Card("cms_like")
+    assert B.workspace_bytes(c, 1000, 60000) >= 16 + 24
+    assert L.pd_workspace_bytes(c._h, -1, 0) == B.PD_EINVAL
+    ev = B.Events(1, 10, None, None, None, None, None, None, None, None, None, None)
+    trk, tow, efl = B.Tracks(), B.Towers(), B.EFlow()
+    assert L.pd_simulate(c._h, C.byref(ev), 1, 0, C.byref(trk), C.byref(tow), C.byref(efl), None, None, 0, None) == B.PD_EINVAL
+    assert L.pd_simulate(None, C.byref(ev), 1, 0, C.byref(trk), C.byref(tow), C.byref(efl), None, None, 0, None) == B.PD_EINVAL
+    assert L.pd_strerror(B.PD_ECAPACITY).decode().startswith("output capacity")
+
+
+def test_no_cpu_fallback():
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    import importlib
+
+    wl = importlib.import_module("workloads.generate")
+
+    ev = wl.generate(0, 2)
+    with pytest.raises((B.PdError, RuntimeError, AssertionError)):
+        dev = B.DeviceEvents(ev, device="cuda")
+        out = B.DeviceOutputs(B.Card("cms_like"), dev.n_events, dev.n_particles)
+        B.simulate(B.Card("cms_like"), dev, out, 1)

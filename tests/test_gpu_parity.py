@@ -1,0 +1,116 @@
+"""-m gpu: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on seeded
+synthetic inputs of the five BASELINE.json configs at sizes the oracle finishes in seconds, plus edge
+cases.  Tolerances: integers exact (near-edge overrides counted), floats 1e-5 rel / 1e-6 abs
+(BASELINE.json north_star); see tests/parity.py."""
+import numpy as np
+import pytest
+
+import importlib
+
+wl = importlib.import_module("workloads.generate")
+
+pytestmark = pytest.mark.gpu
+
+SMALL = {0: 1000, 1: 400, 2: 24, 3: 3000, 4: 3000}
+
+
+def _check(rep, max_override_frac=2e-3):
+    assert rep["unexcused"] == 0, rep["problems"][:10]
+    assert rep["overridden_particles"] <= max(2, max_override_frac * rep["n_particles"]), rep
+    return rep
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_config_parity(cfg):
+    from tests.gpu_util import run_gpu
+    from tests.parity import compare
+
+    ev = wl.generate(cfg, SMALL[cfg])
+    seed = wl.CONFIGS[cfg]["seed"]
+    card = wl.config_card(cfg)
+    gpu = run_gpu(card, ev, seed)
+    assert gpu["status_word"] == 0
+    assert gpu["launches"] >= 1
+    rep = _check(compare(card, ev, seed, gpu))
+    print("cfg%d parity: %s" % (cfg, {k: v for k, v in rep.items() if k != "problems"}))
+
+
+def test_edge_cases_empty_and_ragged():
+    from tests.gpu_util import run_gpu
+    from tests.parity import compare
+
+    base = wl.generate(0, 40)
+    empty = wl.from_lists([[] for _ in range(5)])
+    one = wl.from_lists([[wl.particle(211, 1, 10.0, 0.5, 0.3, 0.13957039)]])
+    ragged = wl.concat_events([empty, wl.slice_events(base, 0, 7), empty, one, wl.slice_events(base, 7, 40), empty])
+    for ev in (empty, one, ragged):
+        gpu = run_gpu("cms_like", ev, 11)
+        assert gpu["status_word"] == 0
+        _check(compare("cms_like", ev, 11, gpu))
+    # zero events at all
+    gpu = run_gpu("cms_like", wl.from_lists([]), 3)
+    assert gpu["trk_offsets"].tolist() == [0] and gpu["tow_offsets"].tolist() == [0] and gpu["efl_offsets"].tolist() == [0]
+
+
+def test_degenerate_particles():
+    """Dropped vertices, pz = 0 loopers, neutrinos/muons, huge turning angles, all into one tower."""
+    from tests.gpu_util import run_gpu
+    from tests.parity import compare
+
+    P = wl.particle
+    evs = [[
+        P(211, 1, 0.3, 0.0, 0.1, 0.13957039),            # trapped looper (pz = 0): dropped
+        P(211, 1, 0.3, 1e-4, 0.1, 0.13957039),           # ~1e5 rad of turning before the endcap
+        P(-211, -1, 0.2, -2e-3, 2.0, 0.13957039, vz=0.1),
+        P(22, 0, 5.0, 0.0, -3.0, 0.0),                   # pz = 0 neutral: barrel
+        P(12, 0, 5.0, 0.3, 1.0, 0.0), P(13, -1, 20.0, 0.3, 1.0, 0.1056584),   # no deposit
+        P(211, 1, 5.0, 0.5, 1.0, 0.13957039, vx=2.0),    # born outside the cylinder
+        P(211, 1, 5.0, 0.5, 1.0, 0.13957039, vz=3.5),
+        P(130, 0, 50.0, 4.999, 0.0, 0.497611), P(130, 0, 50.0, 5.2, 0.0, 0.497611),  # grid edge / outside
+        P(211, 1, 300.0, 0.1, -0.5, 0.13957039, vx=0.3, vy=-0.4, vz=0.2),
+        P(-11, 1, 0.74, 0.2, 0.5, 0.000511), P(-11, 1, 0.73, 0.2, 0.5, 0.000511),  # around the looper threshold
+    ], [P(22, 0, 2.0 + 0.01 * k, 0.02, 0.01, 0.0) for k in range(300)]]            # 300 deposits in one tower
+    ev = wl.from_lists(evs)
+    for card in ("cms_like", "atlas_like", "aleph_like"):
+        gpu = run_gpu(card, ev, 5)
+        assert gpu["status_word"] == 0
+        _check(compare(card, ev, 5, gpu), max_override_frac=1.0)
+
+
+def test_bitwise_reproducible_and_event_base():
+    from tests.gpu_util import run_gpu
+
+    ev = wl.generate(1, 64)
+    a = run_gpu("cms_like", ev, 77, debug=False)
+    b = run_gpu("cms_like", ev, 77, debug=False)
+    for k in a:
+        if isinstance(a[k], np.ndarray):
+            assert a[k].tobytes() == b[k].tobytes(), k
+    # one call versus two half-calls with event_base (P9-v): the concatenation is identical
+    h1, h2 = wl.slice_events(ev, 0, 30), wl.slice_events(ev, 30, 64)
+    r1 = run_gpu("cms_like", h1, 77, event_base=0, debug=False)
+    r2 = run_gpu("cms_like", h2, 77, event_base=30, debug=False)
+    for prefix in ("trk", "tow", "efl"):
+        for k in a:
+            if not k.startswith(prefix + "_") or k.endswith("offsets"):
+                continue
+            cat = np.concatenate([r1[k], r2[k]])
+            if k == "trk_src" or (k == "efl_src"):
+                continue  # particle indices are per call
+            assert cat.tobytes() == a[k].tobytes(), k
+        off = np.concatenate([r1[prefix + "_offsets"], r2[prefix + "_offsets"][1:] + r1[prefix + "_offsets"][-1]])
+        assert np.array_equal(off, a[prefix + "_offsets"])
+
+
+def test_host_pointer_entry_matches_device_entry():
+    import paper_2606_26089_b200 as pd
+    from tests.gpu_util import run_gpu
+
+    ev = wl.generate(0, 200)
+    ref = run_gpu("cms_like", ev, 9, debug=False)
+    card = pd.Card("cms_like")
+    hb = pd.HostBuffers(ev)
+    pd.simulate_host(card, hb, 9)
+    got = hb.to_numpy()
+    for k, v in got.items():
+        assert v.tobytes() == ref[k].tobytes(), k
