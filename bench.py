@@ -1,0 +1,279 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole Delphes-chain hot path.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one pd_simulate call over one batch: every event of the workload, inputs resident in
+HBM.  Default workload: BASELINE.json configs[2] (CMS-like PU200-like pile-up, 10,000 events x ~4,060
+particles), the largest config, on which north_star states the bandwidth target.  Prints ONE JSON line.
+
+  value      truth particles/s, whole job (all ranks), device-timed with CUDA events, max over ranks
+  e2e        same metric through pd_simulate_host: pinned HOST buffers in and out, copies timed
+  roofline   algorithmic HBM bytes of one launch / its CUDA-event duration, against the measured
+             copy bandwidth in MEASURED_PEAKS.json
+  cpu_baseline  the fp64 oracle (oracle/, as it stands) on a bounded sample of the same workload,
+             one host core
+
+N > 1 (torchrun): events are independent, so every rank runs the same-size batch with its own
+event_base (weak scaling, no data-path collective); rank 0 prints.
+--impl reference: the oracle on the host cores, bounded sample per step (rank 0 only).
+"""
+import argparse
+import importlib
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+wl = importlib.import_module("workloads.generate")
+
+METRIC = "truth particles/sec through Delphes chain"
+UNIT = "particles/s"
+SAMPLE_PARTICLES = 8_000_000  # cpu_baseline sample: ~10-15 s of one core
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def _traffic(cfg):
+    """DRAM bytes per launch from the committed ncu --set full capture, if one exists for this config."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "dram_traffic.json")) as f:
+            return json.load(f).get("cfg%d" % cfg)
+    except Exception:
+        return None
+
+
+def _sample_events(ev, max_particles):
+    """Leading events of the workload holding at most max_particles particles."""
+    k = int(np.searchsorted(ev.offsets, max_particles, side="right") - 1)
+    k = max(1, min(k, ev.n_events))
+    return wl.slice_events(ev, 0, k), k
+
+
+def _oracle_rate(cfg, ev, seed, steps=1, warmup=0):
+    from oracle import pdo
+
+    card = pdo.Card(wl.config_card(cfg))
+    sample, k = _sample_events(ev, SAMPLE_PARTICLES)
+    for _ in range(warmup):
+        pdo.simulate(card, wl.slice_events(sample, 0, max(1, k // 50)), seed, debug=False)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        pdo.simulate(card, sample, seed, debug=False)
+    dt = (time.perf_counter() - t0) / steps
+    what = "first %d events (%d particles) of %s" % (k, sample.n_particles, wl.CONFIGS[cfg]["name"])
+    return sample.n_particles / dt, dt, what
+
+
+class _Clocks:
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.QUERY,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for line in self.f:
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])), mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+        return out
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    cfg = args.config
+    seed = wl.CONFIGS[cfg]["seed"]
+    # the oracle only sees a bounded sample: generate just enough events
+    avg = {0: 60, 1: 250, 2: 4060, 3: 40, 4: 30}[cfg]
+    ne = min(wl.CONFIGS[cfg]["n_events"], max(1, int(1.05 * SAMPLE_PARTICLES / avg) + 2))
+    ev = wl.generate(cfg, ne)
+    rate, dt, what = _oracle_rate(cfg, ev, seed, steps=max(1, args.steps), warmup=min(args.warmup, 1))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": wl.CONFIGS[cfg]["name"], "card": wl.config_card(cfg), "sample": what},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": what},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    import paper_2606_26089_b200 as pd
+
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    cfg = args.config
+    seed = wl.CONFIGS[cfg]["seed"]
+    ev = wl.generate(cfg, args.events)
+    n, ne = ev.n_particles, ev.n_events
+    event_base = rank * ne  # shard r of a world x ne event job (weak scaling)
+    card = pd.Card(wl.config_card(cfg))
+    dev = pd.DeviceEvents(ev)
+    out = pd.DeviceOutputs(card, ne, n, debug=False)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    launches = 0
+    for _ in range(args.warmup):
+        pd.simulate(card, dev, out, seed, event_base)
+    torch.cuda.synchronize()
+    status = pd.last_status(out)
+    if status != 0:
+        raise SystemExit("bench.py: device-side status %d" % status)
+    totals = [int(out.trk["offsets"][-1]), int(out.tow["offsets"][-1]), int(out.efl["offsets"][-1])]
+
+    # ---- device-timed region: K steps, per-launch events on the launching stream
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    clocks = _Clocks(local_rank) if rank == 0 else None
+    time.sleep(0.25 if clocks else 0.0)
+    barrier()
+    evs[0].record(stream)
+    for k in range(args.steps):
+        pd.simulate(card, dev, out, seed, event_base)
+        launches += pd.last_launch_count()
+        evs[k + 1].record(stream)
+    barrier()
+    clk = clocks.stop() if clocks else None
+    per_launch_ms = [evs[k].elapsed_time(evs[k + 1]) for k in range(args.steps)]
+    total_ms = evs[0].elapsed_time(evs[args.steps])
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    value = world * n * args.steps / (total_ms_max * 1e-3)
+
+    # ---- end-to-end: pinned host buffers through pd_simulate_host, copies inside the timed region
+    hb = pd.HostBuffers(ev)
+    pd.simulate_host(card, hb, seed, event_base)
+    e2e_steps = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        pd.simulate_host(card, hb, seed, event_base)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * n / float(t.item())
+    h2d, d2h = hb.h2d_bytes(), hb.d2h_bytes()
+
+    if dist is not None:
+        # CSR rebasing of shard outputs: one all-gather of three int64 per rank, outside the data path
+        mine = torch.tensor(totals, dtype=torch.int64, device="cuda")
+        allt = [torch.zeros_like(mine) for _ in range(world)]
+        dist.all_gather(allt, mine)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the (single) kernel: algorithmic bytes / launch
+    alg_bytes = 33 * n + 8 * (ne + 1) + 33 * totals[0] + 28 * totals[1] + 21 * totals[2] + 3 * 8 * (ne + 1)
+    kern_ms = float(np.mean(per_launch_ms))
+    peak, peak_src = _peaks()
+    achieved = alg_bytes / (kern_ms * 1e-3) / 1e9
+    cpu_rate, cpu_dt, cpu_what = _oracle_rate(cfg, ev, seed)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": wl.CONFIGS[cfg]["name"], "card": wl.config_card(cfg), "events_per_gpu": ne, "particles_per_gpu": n,
+                   "tracks": totals[0], "towers": totals[1], "eflow": totals[2], "events_per_s": world * ne * args.steps / (total_ms_max * 1e-3),
+                   "l2": "inputs+outputs (%.2f GB) larger than L2, no flush" % (alg_bytes / 1e9), "parallelism": "event sharding x%d" % world,
+                   "input_sha256": ev.sha256()[:16], "numpy": np.__version__},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": _traffic(cfg), "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                     "bytes_per_particle": alg_bytes / max(n, 1), "kernel_ms": kern_ms, "kernel": "pd_chain_kernel",
+                     "frac_of_8TBs_nominal": achieved / 8000.0},
+        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": cpu_what},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
+        "gpu_launches": launches, "clocks": clk,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--events", type=int, default=None, help="override the config's event count (debugging)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

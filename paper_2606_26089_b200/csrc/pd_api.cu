@@ -235,6 +235,19 @@ int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, in
   const size_t efl_bytes = b_off + up(2 * np) + up(8 * np) + 4 * up(8 * np);
   const size_t total = in_bytes + trk_bytes + tow_bytes + efl_bytes + up((size_t)ws_bytes);
   unsigned char *base = nullptr;
+  {
+    // keep freed blocks in the stream-ordered pool between calls (default threshold releases them at every sync)
+    static thread_local int pool_dev = -1;
+    int dev = 0;
+    PD_CUDA(cudaGetDevice(&dev));
+    if (pool_dev != dev) {
+      cudaMemPool_t pool;
+      PD_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
+      unsigned long long keep = ~0ull;
+      PD_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+      pool_dev = dev;
+    }
+  }
   PD_CUDA(cudaMallocAsync((void **)&base, total, st));
   size_t o = 0;
   auto take = [&](size_t bytes) {

@@ -148,15 +148,40 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
     const float P = 2.f * rho * a_;
     const float Q = fmaf(4.f * rho, rho + b_, -D);
     const float disc = fmaf(P, P, Q * D);
-    const bool reach = disc >= 0.f;
+    const float scale = fmaf(P, P, 4.f * rho * rho * D);
+    bool reach;
+    float cc = 1.f, ss = 0.f;
+    if (disc >= 0.f ? disc < 0.08f * scale : -disc < 1e-3f * scale) {
+      // grazing the barrel (within a few % of the looper threshold): the crossing angle amplifies the
+      // rounding of rho by 1/sqrt(distance to tangency), so this rare case is redone in double
+      const double pxd = px, pyd = py, vxd = vx, vyd = vy, Rd = sc.R;
+      const double ptd = sqrt(pxd * pxd + pyd * pyd);
+      const double rhod = ptd / (sc.kB_d * (double)aq);
+      const double ipt = 1.0 / ptd;
+      const double ad = (vxd * pxd + vyd * pyd) * ipt;
+      const double bd = (double)s * (vyd * pxd - vxd * pyd) * ipt;
+      const double Dd = Rd * Rd - (vxd * vxd + vyd * vyd);
+      const double Pd = 2.0 * rhod * ad;
+      const double Qd = 4.0 * rhod * (rhod + bd) - Dd;
+      const double dd = Pd * Pd + Qd * Dd;
+      reach = dd >= 0.0;
+      if (reach) {
+        const double Sd = sqrt(dd);
+        if (Pd >= 0.0) cc = (float)(Pd + Sd), ss = (float)Dd;
+        else cc = (float)Qd, ss = (float)(Sd - Pd);
+      }
+    } else {
+      reach = disc >= 0.f;
+      if (reach) {
+        const float S = sqrtf(disc);
+        // first crossing: (cos h, sin h) proportional to (P + S, D) if P >= 0 else (Q, S - P)
+        if (P >= 0.f) cc = P + S, ss = D;
+        else cc = Q, ss = S - P;
+      }
+    }
     float sh = 0.f, ch = 1.f, hR = 0.f;
     float aR = __int_as_float(0x7f800000), aZ = aR;
     if (reach) {
-      const float S = sqrtf(disc);
-      // first crossing: (cos h, sin h) proportional to (P + S, D) if P >= 0 else (Q, S - P)
-      float cc, ss;
-      if (P >= 0.f) cc = P + S, ss = D;
-      else cc = Q, ss = S - P;
       const float inv = 1.0f / sqrtf(fmaf(cc, cc, ss * ss));
       ch = cc * inv, sh = ss * inv;
       hR = atan2f(ss, cc);
@@ -203,7 +228,16 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
     int row = -1;
     if (!(sc.has_cos && T >= sc.t_cos)) {
       for (int k = 0; k < sc.n_eff; ++k) {
-        if (pt > sc.eff[k][0] && pt <= sc.eff[k][1] && (sc.eff[k][2] <= 0.f || T >= sc.eff[k][2]) && T < sc.eff[k][3]) {
+        const float lo = sc.eff[k][0], hi = sc.eff[k][1];
+        bool above_lo = pt > lo, below_hi = pt <= hi;
+        if (fabsf(pt - lo) <= 2e-6f * lo || fabsf(pt - hi) <= 2e-6f * hi) {
+          // pT within rounding of a table edge (e.g. a generator floor at exactly 0.1 GeV): decide on
+          // pT^2 in double, where px^2 + py^2 is (almost) exact
+          const double p2 = (double)px * (double)px + (double)py * (double)py;
+          above_lo = p2 > (double)lo * (double)lo;
+          below_hi = p2 <= (double)hi * (double)hi;
+        }
+        if (above_lo && below_hi && (sc.eff[k][2] <= 0.f || T >= sc.eff[k][2]) && T < sc.eff[k][3]) {
           row = k;
           eps = sc.eff[k][4];
           break;

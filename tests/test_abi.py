@@ -33,7 +33,7 @@ def test_builtin_cards_match_oracle_loader(name, towers, bins, coord):
 
 def test_card_file_and_errors(tmp_path):
     from oracle import pdo
-    from tests import cards
+    import cards
 
     o = pdo.Card("cms_like")
     path = cards.variant(tmp_path / "v.card", o.edges, o.nphi, bz=-2.5, ecal_thr=0.0)

@@ -22,8 +22,8 @@ def _check(rep, max_override_frac=2e-3):
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
 def test_config_parity(cfg):
-    from tests.gpu_util import run_gpu
-    from tests.parity import compare
+    from gpu_util import run_gpu
+    from parity import compare
 
     ev = wl.generate(cfg, SMALL[cfg])
     seed = wl.CONFIGS[cfg]["seed"]
@@ -36,8 +36,8 @@ def test_config_parity(cfg):
 
 
 def test_edge_cases_empty_and_ragged():
-    from tests.gpu_util import run_gpu
-    from tests.parity import compare
+    from gpu_util import run_gpu
+    from parity import compare
 
     base = wl.generate(0, 40)
     empty = wl.from_lists([[] for _ in range(5)])
@@ -54,8 +54,8 @@ def test_edge_cases_empty_and_ragged():
 
 def test_degenerate_particles():
     """Dropped vertices, pz = 0 loopers, neutrinos/muons, huge turning angles, all into one tower."""
-    from tests.gpu_util import run_gpu
-    from tests.parity import compare
+    from gpu_util import run_gpu
+    from parity import compare
 
     P = wl.particle
     evs = [[
@@ -78,7 +78,7 @@ def test_degenerate_particles():
 
 
 def test_bitwise_reproducible_and_event_base():
-    from tests.gpu_util import run_gpu
+    from gpu_util import run_gpu
 
     ev = wl.generate(1, 64)
     a = run_gpu("cms_like", ev, 77, debug=False)
@@ -104,7 +104,7 @@ def test_bitwise_reproducible_and_event_base():
 
 def test_host_pointer_entry_matches_device_entry():
     import paper_2606_26089_b200 as pd
-    from tests.gpu_util import run_gpu
+    from gpu_util import run_gpu
 
     ev = wl.generate(0, 200)
     ref = run_gpu("cms_like", ev, 9, debug=False)
