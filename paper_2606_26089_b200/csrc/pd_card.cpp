@@ -163,7 +163,6 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     if (n < 1) return PD_ECARD;
     total += n;
   }
-  if (total >= (1L << PD_MAX_TOWER_BITS)) return PD_ECARD;
 
   c->name = r.name;
   c->bz = float(r.bz);
@@ -176,8 +175,17 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
   s.grid_theta = r.theta ? 1 : 0;
   s.n_bins = int(nb);
   s.n_towers = int(total);
-  s.tower_bits = 1;
-  while ((1 << s.tower_bits) < s.n_towers) ++s.tower_bits;
+  {
+    long max_n = 1;
+    for (long n : r.nphi) max_n = std::max(max_n, n);
+    s.j_bits = 0;
+    while ((1L << s.j_bits) < max_n) ++s.j_bits;
+    int bin_bits = 0;
+    while ((size_t(1) << bin_bits) < nb) ++bin_bits;
+    s.code_bits = bin_bits + s.j_bits;
+    if (s.code_bits < 1) s.code_bits = 1;
+    if (s.code_bits > PD_MAX_CODE_BITS) return PD_ECARD;
+  }
   s.n_eff = int(r.eff.size());
   s.has_cos = r.has_cos ? 1 : 0;
   {

@@ -10,7 +10,7 @@
 
 constexpr int PD_MAX_BINS = 1024;  // eta/theta bins of a card's grid
 constexpr int PD_MAX_EFF = 32;     // rows of the efficiency table
-constexpr int PD_MAX_TOWER_BITS = 15;
+constexpr int PD_MAX_CODE_BITS = 20;  // packed (eta bin, phi bin) tower code
 
 // Scalars of a card as the kernels want them (all derived in double at load, stored as fp32).
 struct PdCardScalars {
@@ -19,7 +19,8 @@ struct PdCardScalars {
   double kB_d;           // same in double (only used for the endcap turning angle)
   float sB;              // sign of B (0 if B == 0)
   int grid_theta;        // 0: bins in eta, 1: bins in theta
-  int n_bins, n_towers, tower_bits;
+  int n_bins, n_towers;
+  int j_bits, code_bits;  // packed tower code = bin << j_bits | phi bin (ordered like the tower id)
   int n_eff, has_cos;
   float t_cos;           // |pz|/pT threshold equivalent to |cos theta| >= abs_costheta_max
   float trk_a2, trk_b;   // sigma_rel^2 = a^2 + (b pT)^2

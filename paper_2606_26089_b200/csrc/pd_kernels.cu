@@ -15,7 +15,9 @@
 // stable, the per-tower sum is sequential, and the only atomics are integer counters.
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdint>
+#include <cstdlib>
 
 #include "pd_internal.h"
 #include "pd_math.cuh"
@@ -23,8 +25,8 @@
 namespace pdk {
 
 constexpr int G_MAX = 256;     // events per tile (8 event bits)
-constexpr int R_MAX = 12;      // radix-sort rounds per warp: C <= THREADS * R_MAX
-// deposit key = hcal << 31 | local event << tower_bits | tower
+constexpr int r_max(int threads) { return threads >= 1024 ? 6 : 12; }  // radix-sort rounds per warp: C <= THREADS * r_max
+// deposit key = hcal << 31 | local event << code_bits | tower code (eta bin << j_bits | phi bin)
 constexpr uint32_t KEY_MASK = 0x7fffffffu;
 constexpr unsigned long long FLAG_A = 1ull << 62, FLAG_P = 2ull << 62, VAL_MASK = (1ull << 62) - 1;
 
@@ -62,13 +64,13 @@ __host__ __device__ inline Layout make_layout(int n_bins, int threads, int C) {
   l.ntow = take(4 * (G_MAX + 1));
   l.nph = take(4 * (G_MAX + 1));
   l.nnh = take(4 * (G_MAX + 1));
-  l.misc = take(8 * 64);
+  l.misc = take(8 * 96);
   l.cnt = take(2 * 256 * (threads / 32));
   l.dep_key = take(4 * (size_t)C);
   l.dep_E = take(4 * (size_t)C);
   l.dep_T = take(4 * (size_t)C);
   l.dep_idx = take(2 * (size_t)C);
-  l.uni = take(26 * (size_t)C + 16);
+  l.uni = take(20 * (size_t)C + 16);
   l.total = o;
   return l;
 }
@@ -171,25 +173,23 @@ __device__ __forceinline__ int find_bin(const int *offset, int nb, int id) {
   return lo;
 }
 
-// Block-wide exclusive prefix of a packed per-thread value given per-warp totals in wtot[W].
-// Returns the exclusive prefix of this thread's WARP and the block total.
+// Block-wide exclusive prefix of packed per-warp totals wtot[W] (REDUX adds): returns the exclusive
+// prefix of this thread's WARP and the block total.  Fields of the packed word must not overflow.
 template <int W>
 __device__ __forceinline__ void warp_totals_scan(const unsigned *wtot, unsigned &excl_warp, unsigned &total) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned v = lane < W ? wtot[lane] : 0u;
-  unsigned incl = v;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const unsigned t = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += t;
-  }
-  total = __shfl_sync(0xffffffffu, incl, 31);
-  excl_warp = __shfl_sync(0xffffffffu, incl - v, wid);
+  total = __reduce_add_sync(0xffffffffu, v);
+  excl_warp = __reduce_add_sync(0xffffffffu, lane < wid ? v : 0u);
 }
 
-template <int THREADS, bool DEBUG>
-__global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_kernel(const __grid_constant__ PdParams prm) {
+// bits of the per-particle result word written by pass P1
+constexpr uint32_t RES_DEP = 1u << 21, RES_HCAL = 1u << 22, RES_ACC = 1u << 23;
+
+template <int THREADS, int CTAS, bool DEBUG>
+__global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_constant__ PdParams prm) {
   constexpr int W = THREADS / 32;
+  constexpr int R_MAX = r_max(THREADS);
   extern __shared__ __align__(16) unsigned char smem[];
   const PdCardScalars &sc = prm.sc;
   const int nb = sc.n_bins;
@@ -209,17 +209,18 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
   int *s_nph = (int *)(smem + L.nph);
   int *s_nnh = (int *)(smem + L.nnh);
   unsigned long long *s_misc = (unsigned long long *)(smem + L.misc);
-  unsigned *s_wtot = (unsigned *)(s_misc + 8);  // [2][32]
+  int *s_ctr = (int *)(s_misc + 4);             // [0] charged count, [1] neutral count
+  unsigned *s_wtot = (unsigned *)(s_misc + 8);  // [5][32]
   uint16_t *s_cnt = (uint16_t *)(smem + L.cnt);
   uint32_t *dep_key = (uint32_t *)(smem + L.dep_key);
   float *dep_E = (float *)(smem + L.dep_E);
   float *dep_T = (float *)(smem + L.dep_T);
   uint16_t *dep_idx = (uint16_t *)(smem + L.dep_idx);
-  // union region, view 1: track staging
-  float *tk_pt = (float *)(smem + L.uni);
-  float *tk_eta = tk_pt + C, *tk_phi = tk_eta + C, *tk_E = tk_phi + C, *tk_eo = tk_E + C, *tk_po = tk_eo + C;
-  uint16_t *tk_i = (uint16_t *)(tk_po + C);
-  // union region, view 2: per deposited tower
+  // union region, view A (passes P0..P2): per-particle scratch
+  uint32_t *p_res = (uint32_t *)(smem + L.uni);
+  float *p_u = (float *)(p_res + C), *p_phi = p_u + C;
+  uint16_t *p_perm = (uint16_t *)(p_phi + C), *tk_i = p_perm + C;
+  // union region, view B (phase 2b on): per deposited tower
   uint32_t *st_key = (uint32_t *)(smem + L.uni);
   float *st_em = (float *)(st_key + C), *st_had = st_em + C, *st_nem = st_had + C, *st_nhad = st_nem + C;
 
@@ -240,12 +241,16 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
   }
   SmCard cd{s_tb, s_nphi, s_offset, s_inv_w, s_half, s_w, s_eta_c, s_inv_cosh};
   const int G = prm.events_per_tile;
-  const int EV_SHIFT = sc.tower_bits;
-  const uint32_t tower_mask = (1u << EV_SHIFT) - 1u;
+  const int EV_SHIFT = sc.code_bits;
+  const int JB = sc.j_bits;
+  const uint32_t code_mask = (1u << EV_SHIFT) - 1u, j_mask = (1u << JB) - 1u;
 
   for (;;) {
     __syncthreads();  // previous tile fully done with shared memory (and card tables staged)
-    if (tid == 0) s_misc[0] = atomicAdd(prm.tile_counter, 1u);
+    if (tid == 0) {
+      s_misc[0] = atomicAdd(prm.tile_counter, 1u);
+      s_ctr[0] = 0, s_ctr[1] = 0;
+    }
     __syncthreads();
     const int tile = (int)s_misc[0];
     if (tile >= prm.n_tiles) break;
@@ -263,63 +268,80 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
       s_off32[e] = overflow ? 0 : (int)(prm.offsets[e0 + e] - p0);
       s_ntrk[e] = 0, s_ntow[e] = 0, s_nph[e] = 0, s_nnh[e] = 0;
     }
+
+    // ------------------------------------------------------------------ P0: charged-first permutation
+    // (the per-particle math is order-independent; grouping by kind keeps its warps converged)
+    for (int it = 0; it * THREADS < n; ++it) {
+      const int i = it * THREADS + tid;
+      const bool valid = i < n;
+      const int q = valid ? (int)__ldg(prm.charge + p0 + i) : 0;
+      const bool chg = valid && q != 0, neu = valid && q == 0;
+      const unsigned cm = __ballot_sync(0xffffffffu, chg), nm = __ballot_sync(0xffffffffu, neu);
+      int cb = 0, nbs = 0;
+      if (lane == 0) {
+        if (cm) cb = atomicAdd(&s_ctr[0], __popc(cm));
+        if (nm) nbs = atomicAdd(&s_ctr[1], __popc(nm));
+      }
+      cb = __shfl_sync(0xffffffffu, cb, 0), nbs = __shfl_sync(0xffffffffu, nbs, 0);
+      if (chg) p_perm[cb + __popc(cm & lt_mask)] = (uint16_t)i;
+      if (neu) p_perm[n - 1 - (nbs + __popc(nm & lt_mask))] = (uint16_t)i;
+    }
     __syncthreads();
 
-    // ------------------------------------------------------------------ phase 1: particles
+    // ------------------------------------------------------------------ P1: S0-S2, S4 per particle (no barriers)
+    for (int k = tid; k < n; k += THREADS) {
+      const int i = p_perm[k];
+      const long long g = p0 + i;
+      const int pid = __ldg(prm.pid + g);
+      const int q = (int)__ldg(prm.charge + g);
+      const float px = __ldg(prm.px + g), py = __ldg(prm.py + g), pz = __ldg(prm.pz + g);
+      const float vx = __ldg(prm.vx + g), vy = __ldg(prm.vy + g), vz = __ldg(prm.vz + g);
+      const int e = find_event(s_off32, ne, i);
+      ParticleOut o;
+      particle_chain(sc, cd, pid, q, px, py, pz, vx, vy, vz, prm.seed, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), o);
+      const int apid = pid < 0 ? -pid : pid;
+      const bool to_ecal = apid == 11 || apid == 22;
+      const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
+      uint32_t res = 0;
+      if (o.bin >= 0) res = ((uint32_t)o.bin << JB) | (uint32_t)o.j | (to_none ? 0u : RES_DEP) | (to_ecal ? 0u : RES_HCAL);
+      if (o.accepted) {
+        res |= RES_ACC;
+        p_u[i] = o.u, p_phi[i] = o.phi_pos;
+        atomicAdd(&s_ntrk[e], 1);
+      }
+      p_res[i] = res;
+      if (DEBUG) {
+        if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)o.status;
+        if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = (o.status & PD_FACE_MASK) ? eta_from_u(sc, o.u) : o.u;
+        if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = o.phi_pos;
+        if (prm.dbg_tower) prm.dbg_tower[g] = o.bin >= 0 ? s_offset[o.bin] + o.j : -1;
+        if (prm.dbg_accepted) prm.dbg_accepted[g] = o.accepted ? 1 : 0;
+        if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)o.eps_row;
+        if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = 0.f;
+        if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 0;
+      }
+    }
+    __syncthreads();
+
+    // ------------------------------------------------------------------ P1b: ordered compaction (particle order)
     int trk_base = 0, dep_base = 0;
     for (int it = 0; it * THREADS < n; ++it) {
       const int i = it * THREADS + tid;
-      bool acc = false, dep = false;
-      uint32_t key = 0;
-      int e = 0;
-      ParticleOut o;
-      float Ein = 0.f, eta_out = 0.f;
-      if (i < n) {
-        const long long g = p0 + i;
-        const int pid = __ldg(prm.pid + g);
-        const int q = (int)__ldg(prm.charge + g);
-        const float px = __ldg(prm.px + g), py = __ldg(prm.py + g), pz = __ldg(prm.pz + g);
-        Ein = __ldg(prm.E + g);
-        const float vx = __ldg(prm.vx + g), vy = __ldg(prm.vy + g), vz = __ldg(prm.vz + g);
-        e = find_event(s_off32, ne, i);
-        particle_chain(sc, cd, pid, q, px, py, pz, vx, vy, vz, prm.seed, prm.event_base + e0 + e,
-                       (uint32_t)(i - s_off32[e]), o);
-        acc = o.accepted;
-        const int apid = pid < 0 ? -pid : pid;
-        const bool to_ecal = apid == 11 || apid == 22;
-        const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
-        dep = o.tower >= 0 && !to_none;
-        key = (to_ecal ? 0u : 0x80000000u) | ((uint32_t)e << EV_SHIFT) | (uint32_t)(o.tower & (int)tower_mask);
-        if (acc || DEBUG) eta_out = (o.status & PD_FACE_MASK) ? eta_from_u(sc, o.u) : o.u;
-        if (DEBUG) {
-          if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)o.status;
-          if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = eta_out;
-          if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = o.phi_pos;
-          if (prm.dbg_tower) prm.dbg_tower[g] = o.tower;
-          if (prm.dbg_accepted) prm.dbg_accepted[g] = acc ? 1 : 0;
-          if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)o.eps_row;
-          if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = o.pt_s;
-          if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 0;
-        }
-      }
+      const uint32_t res = i < n ? p_res[i] : 0u;
+      const bool acc = (res & RES_ACC) != 0, dep = (res & RES_DEP) != 0;
       const unsigned am = __ballot_sync(0xffffffffu, acc), dm = __ballot_sync(0xffffffffu, dep);
       if (lane == 0) s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(am) | ((unsigned)__popc(dm) << 16);
       __syncthreads();
       unsigned excl_w, tot;
       warp_totals_scan<W>(s_wtot + (it & 1) * 32, excl_w, tot);
-      if (acc) {
-        const int s = trk_base + (int)(excl_w & 0xffffu) + __popc(am & lt_mask);
-        tk_pt[s] = o.pt_s, tk_eta[s] = o.eta_mom, tk_phi[s] = o.phi0, tk_E[s] = o.E_trk;
-        tk_eo[s] = eta_out, tk_po[s] = o.phi_pos;
-        tk_i[s] = (uint16_t)i;
-        atomicAdd(&s_ntrk[e], 1);
-      }
+      if (acc) tk_i[trk_base + (int)(excl_w & 0xffffu) + __popc(am & lt_mask)] = (uint16_t)i;
       if (dep) {
         const int s = dep_base + (int)(excl_w >> 16) + __popc(dm & lt_mask);
-        dep_key[s] = key;
+        const int e = find_event(s_off32, ne, i);
+        dep_key[s] = ((res & RES_HCAL) ? 0x80000000u : 0u) | ((uint32_t)e << EV_SHIFT) | (res & code_mask);
         dep_idx[s] = (uint16_t)i;
-        dep_E[i] = Ein;
-        dep_T[i] = acc ? o.E_trk : 0.f;
+        dep_E[i] = __ldg(prm.E + p0 + i);
+        dep_T[i] = 0.f;
       }
       trk_base += (int)(tot & 0xffffu);
       dep_base += (int)(tot >> 16);
@@ -404,7 +426,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
         __syncthreads();
       }
     }
-    // ------------------------------------------------------------------ chain T + track flush
+
+    // ------------------------------------------------------------------ chain T (tracks)
     if (wid == 0) {
       const unsigned long long ex = chain_lookback(prm.chain, tile, (unsigned long long)n_trk);
       if (lane == 0) s_misc[1] = ex;
@@ -413,95 +436,103 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
     }
     __syncthreads();
     const long long base_trk = (long long)s_misc[1];
+
+    // ------------------------------------------------------------------ P2: S3 on the accepted tracks (converged),
+    // written straight to the track collection
     for (int s = tid; s < n_trk; s += THREADS) {
-      const long long g = base_trk + s;
-      const long long src = p0 + tk_i[s];
+      const int i = tk_i[s];
+      const long long src = p0 + i, g = base_trk + s;
+      const int pid = __ldg(prm.pid + src);
+      const float px = __ldg(prm.px + src), py = __ldg(prm.py + src), pz = __ldg(prm.pz + src);
+      const int e = find_event(s_off32, ne, i);
+      TrackOut t;
+      track_smear(sc, px, py, pz, prm.seed, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), t);
+      dep_T[i] = t.E_trk;
       prm.trk_src[g] = (int)src;
-      prm.trk_pid[g] = __ldg(prm.pid + src);
+      prm.trk_pid[g] = pid;
       prm.trk_charge[g] = __ldg(prm.charge + src);
-      prm.trk_pt[g] = tk_pt[s];
-      prm.trk_eta[g] = tk_eta[s];
-      prm.trk_phi[g] = tk_phi[s];
-      prm.trk_E[g] = tk_E[s];
-      prm.trk_eta_out[g] = tk_eo[s];
-      prm.trk_phi_out[g] = tk_po[s];
+      prm.trk_pt[g] = t.pt_s;
+      prm.trk_eta[g] = t.eta_mom;
+      prm.trk_phi[g] = t.phi0;
+      prm.trk_E[g] = t.E_trk;
+      prm.trk_eta_out[g] = eta_from_u(sc, p_u[i]);
+      prm.trk_phi_out[g] = p_phi[i];
+      if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[src] = t.pt_s;
     }
     for (int e = tid; e < ne; e += THREADS) prm.trk_offsets[e0 + e + 1] = base_trk + s_ntrk[e + 1];
     if (tile == 0 && tid == 0) prm.trk_offsets[0] = 0, prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
+    __syncthreads();  // view A of the union region is dead from here on
 
-    __syncthreads();  // track staging fully flushed by every thread before the union region is reused
-
-    // ------------------------------------------------------------------ phase 2b: towers + EFlow
+    // ------------------------------------------------------------------ phase 2b-1: run heads, in order
     int dt_base = 0;
     for (int it = 0; it * THREADS < m; ++it) {
       const int pos = it * THREADS + tid;
       bool head = false;
-      uint32_t kk = 0;
-      float em_f = 0.f, had_f = 0.f, n_em_out = 0.f, n_had_out = 0.f;
       if (pos < m) {
-        kk = dep_key[pos] & KEY_MASK;
+        const uint32_t kk = dep_key[pos] & KEY_MASK;
         const uint32_t prev = pos > 0 ? (dep_key[pos - 1] & KEY_MASK) : 0xffffffffu;
         head = kk != prev;
-      }
-      if (head) {
-        float Eem = 0.f, Ehad = 0.f, Tem = 0.f, Thad = 0.f;
-        int qpos = pos;
-        do {
-          const uint32_t kq = dep_key[qpos];
-          if ((kq & KEY_MASK) != kk) break;
-          const int pi = dep_idx[qpos];
-          const float Ev = dep_E[pi], Tv = dep_T[pi];
-          if (kq >> 31) Ehad += Ev, Thad += Tv;
-          else Eem += Ev, Tem += Tv;
-          ++qpos;
-        } while (qpos < m);
-        const int tower = (int)(kk & tower_mask);
-        const int e = (int)(kk >> EV_SHIFT);
-        uint32_t rn[4];
-        rng_block(prm.seed, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
-        const float em_s = smear_component(Eem, sc.ecal2, rn[0], rn[1]);
-        const float had_s = smear_component(Ehad, sc.hcal2, rn[2], rn[3]);
-        // reading A22: the threshold is applied twice, strictly, per component
-        const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
-        em_f = k_em ? em_s : 0.f;
-        had_f = k_had ? had_s : 0.f;
-        const float n_em = em_f - Tem, n_had = had_f - Thad;
-        const bool is_ph = n_em > sc.thr_ecal, is_nh = n_had > sc.thr_hcal;
-        n_em_out = is_ph ? n_em : 0.f;
-        n_had_out = is_nh ? n_had : 0.f;
-        if (em_f + had_f > 0.f) atomicAdd(&s_ntow[e], 1);
-        if (is_ph) atomicAdd(&s_nph[e], 1);
-        if (is_nh) atomicAdd(&s_nnh[e], 1);
-        if (DEBUG) {
-          const long long g = p0 + dep_idx[pos];
-          if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 1;
-          if (prm.dbg_tw[0]) prm.dbg_tw[0][g] = Eem;
-          if (prm.dbg_tw[1]) prm.dbg_tw[1][g] = Ehad;
-          if (prm.dbg_tw[2]) prm.dbg_tw[2][g] = Tem;
-          if (prm.dbg_tw[3]) prm.dbg_tw[3][g] = Thad;
-          if (prm.dbg_tw[4]) prm.dbg_tw[4][g] = em_s;
-          if (prm.dbg_tw[5]) prm.dbg_tw[5][g] = had_s;
-          if (prm.dbg_tw_dec)
-            prm.dbg_tw_dec[g] = (unsigned char)((k_em ? PD_DEC_EEM : 0) | (k_had ? PD_DEC_EHAD : 0) |
-                                                (is_ph ? PD_DEC_NEM : 0) | (is_nh ? PD_DEC_NHAD : 0));
-        }
       }
       const unsigned hm = __ballot_sync(0xffffffffu, head);
       if (lane == 0) s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(hm);
       __syncthreads();
       unsigned excl_w, tot;
       warp_totals_scan<W>(s_wtot + (it & 1) * 32, excl_w, tot);
-      if (head) {
-        const int s = dt_base + (int)excl_w + __popc(hm & lt_mask);
-        st_key[s] = kk;
-        st_em[s] = em_f, st_had[s] = had_f, st_nem[s] = n_em_out, st_nhad[s] = n_had_out;
-      }
+      if (head) st_key[dt_base + (int)excl_w + __popc(hm & lt_mask)] = (uint32_t)pos;
       dt_base += (int)tot;
     }
     const int n_dt = dt_base;
     __syncthreads();
 
-    // ------------------------------------------------------------------ chain W
+    // ------------------------------------------------------------------ phase 2b-2: S5-S7, one thread per tower
+    for (int d = tid; d < n_dt; d += THREADS) {
+      const int pos = (int)st_key[d];
+      const uint32_t kk = dep_key[pos] & KEY_MASK;
+      float Eem = 0.f, Ehad = 0.f, Tem = 0.f, Thad = 0.f;
+      int qpos = pos;
+      do {  // sequential sum in particle order (the sort is stable)
+        const uint32_t kq = dep_key[qpos];
+        if ((kq & KEY_MASK) != kk) break;
+        const int pi = dep_idx[qpos];
+        const float Ev = dep_E[pi], Tv = dep_T[pi];
+        if (kq >> 31) Ehad += Ev, Thad += Tv;
+        else Eem += Ev, Tem += Tv;
+        ++qpos;
+      } while (qpos < m);
+      const uint32_t code = kk & code_mask;
+      const int e = (int)(kk >> EV_SHIFT);
+      const int tower = s_offset[code >> JB] + (int)(code & j_mask);
+      uint32_t rn[4];
+      rng_block(prm.seed, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
+      float em_s, had_s;
+      tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
+      // reading A22: the threshold is applied twice, strictly, per component
+      const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
+      const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
+      const float n_em = em_f - Tem, n_had = had_f - Thad;
+      const bool is_ph = n_em > sc.thr_ecal, is_nh = n_had > sc.thr_hcal;
+      if (em_f + had_f > 0.f) atomicAdd(&s_ntow[e], 1);
+      if (is_ph) atomicAdd(&s_nph[e], 1);
+      if (is_nh) atomicAdd(&s_nnh[e], 1);
+      st_key[d] = kk;
+      st_em[d] = em_f, st_had[d] = had_f, st_nem[d] = is_ph ? n_em : 0.f, st_nhad[d] = is_nh ? n_had : 0.f;
+      if (DEBUG) {
+        const long long g = p0 + dep_idx[pos];
+        if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 1;
+        if (prm.dbg_tw[0]) prm.dbg_tw[0][g] = Eem;
+        if (prm.dbg_tw[1]) prm.dbg_tw[1][g] = Ehad;
+        if (prm.dbg_tw[2]) prm.dbg_tw[2][g] = Tem;
+        if (prm.dbg_tw[3]) prm.dbg_tw[3][g] = Thad;
+        if (prm.dbg_tw[4]) prm.dbg_tw[4][g] = em_s;
+        if (prm.dbg_tw[5]) prm.dbg_tw[5][g] = had_s;
+        if (prm.dbg_tw_dec)
+          prm.dbg_tw_dec[g] = (unsigned char)((k_em ? PD_DEC_EEM : 0) | (k_had ? PD_DEC_EHAD : 0) |
+                                              (is_ph ? PD_DEC_NEM : 0) | (is_nh ? PD_DEC_NHAD : 0));
+      }
+    }
+    __syncthreads();
+
+    // ------------------------------------------------------------------ chain W (towers, eflow)
     if (wid == 0) event_scan(s_ntow, ne);
     else if (wid == 1) event_scan(s_nph, ne);
     else if (wid == 2) event_scan(s_nnh, ne);
@@ -552,21 +583,24 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
       }
       const unsigned m_tw = __ballot_sync(0xffffffffu, f_tw), m_ph = __ballot_sync(0xffffffffu, f_ph),
                      m_nh = __ballot_sync(0xffffffffu, f_nh);
-      if (lane == 0)
-        s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 10) | ((unsigned)__popc(m_nh) << 20);
+      if (lane == 0) {
+        s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 16);
+        s_wtot[96 + (it & 1) * 32 + wid] = (unsigned)__popc(m_nh);
+      }
       __syncthreads();
-      unsigned excl_w, tot;
+      unsigned excl_w, tot, excl_n, tot_n;
       warp_totals_scan<W>(s_wtot + (it & 1) * 32, excl_w, tot);
+      warp_totals_scan<W>(s_wtot + 96 + (it & 1) * 32, excl_n, tot_n);
       if (f_tw || f_ph || f_nh) {
-        const int tower = (int)(kk & tower_mask);
+        const uint32_t code = kk & code_mask;
         const int e = (int)(kk >> EV_SHIFT);
-        const int b = find_bin(s_offset, nb, tower);
-        const int j = tower - s_offset[b];
+        const int b = (int)(code >> JB), j = (int)(code & j_mask);
+        const int tower = s_offset[b] + j;
         const float eta_c = s_eta_c[b];
         const float phi_c = fmaf((float)j + 0.5f, s_w[b], -kPiF);
         const float ic = s_inv_cosh[b];
         if (f_tw) {
-          const long long at = base_tow + tw_run + (int)(excl_w & 1023u) + __popc(m_tw & lt_mask);
+          const long long at = base_tow + tw_run + (int)(excl_w & 0xffffu) + __popc(m_tw & lt_mask);
           prm.tow_tower[at] = tower;
           prm.tow_eta[at] = eta_c;
           prm.tow_phi[at] = phi_c;
@@ -576,7 +610,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
           prm.tow_ET[at] = (em + had) * ic;
         }
         if (f_ph) {
-          const int slot = ph_run + (int)((excl_w >> 10) & 1023u) + __popc(m_ph & lt_mask);
+          const int slot = ph_run + (int)(excl_w >> 16) + __popc(m_ph & lt_mask);
           const long long at = base_efl + s_ntrk[e + 1] + s_nnh[e] + slot;
           prm.efl_cls[at] = (signed char)PD_CLS_PHOTON;
           prm.efl_src[at] = tower;
@@ -586,7 +620,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
           prm.efl_E[at] = nem;
         }
         if (f_nh) {
-          const int slot = nh_run + (int)((excl_w >> 20) & 1023u) + __popc(m_nh & lt_mask);
+          const int slot = nh_run + (int)excl_n + __popc(m_nh & lt_mask);
           const long long at = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + slot;
           prm.efl_cls[at] = (signed char)PD_CLS_NEUHAD;
           prm.efl_src[at] = tower;
@@ -596,9 +630,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == 256 ? 2 : 1)) pd_chain_ke
           prm.efl_E[at] = nhad;
         }
       }
-      tw_run += (int)(tot & 1023u);
-      ph_run += (int)((tot >> 10) & 1023u);
-      nh_run += (int)((tot >> 20) & 1023u);
+      tw_run += (int)(tot & 0xffffu);
+      ph_run += (int)(tot >> 16);
+      nh_run += (int)tot_n;
     }
   }
 }
@@ -628,15 +662,16 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   const double avg = n_events > 0 ? double(n_particles) / double(n_events) : 0.0;
   auto cap_for = [&](int threads, size_t budget) {
     const size_t fixed = pdk::make_layout(nb, threads, 0).total;
-    long cap = budget > fixed + 64 ? long((budget - fixed - 64) / 40) : 0;
-    cap = cap > long(threads) * pdk::R_MAX ? long(threads) * pdk::R_MAX : cap;
+    long cap = budget > fixed + 64 ? long((budget - fixed - 64) / 34) : 0;
+    cap = cap > long(threads) * pdk::r_max(threads) ? long(threads) * pdk::r_max(threads) : cap;
     cap = cap > 65535 ? 65535 : cap;
     return int(cap);
   };
   const int c_small = cap_for(256, (228 * 1024 - 2 * 1024) / 2);
-  const int c_large = cap_for(512, smem_sm);
+  static const int large_threads = std::getenv("PD_LARGE_THREADS") ? std::atoi(std::getenv("PD_LARGE_THREADS")) : 1024;
+  const int c_large = cap_for(large_threads, smem_sm);
   const bool small = avg * 1.3 + 64.0 <= double(c_small) * 0.5;
-  plan->threads = small ? 256 : 512;
+  plan->threads = small ? 256 : large_threads;
   plan->capacity = small ? c_small : c_large;
   long g = 1;
   if (avg > 0.0) {
@@ -659,7 +694,7 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
 
 template <int THREADS, bool DEBUG>
 static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
-  auto kern = pdk::pd_chain_kernel<THREADS, DEBUG>;
+  auto kern = pdk::pd_chain_kernel<THREADS, (THREADS == 256 ? 2 : 1), DEBUG>;
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g_max_smem_optin) != cudaSuccess) return PD_ECUDA;
@@ -678,5 +713,6 @@ int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, v
   if (plan.smem_bytes > (size_t)g_max_smem_optin) return PD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
   if (plan.threads == 256) return debug ? launch_variant<256, true>(prm, plan, st) : launch_variant<256, false>(prm, plan, st);
+  if (plan.threads == 1024) return debug ? launch_variant<1024, true>(prm, plan, st) : launch_variant<1024, false>(prm, plan, st);
   return debug ? launch_variant<512, true>(prm, plan, st) : launch_variant<512, false>(prm, plan, st);
 }

@@ -71,11 +71,15 @@ __device__ __forceinline__ float smear_component(float E, const float (&csn2)[3]
 // ---- S1..S4 for one particle -------------------------------------------------------------------
 struct ParticleOut {
   uint32_t status;  // PD_DROPPED / PD_BARREL / PD_ENDCAP | PD_LOOPER
-  int tower;        // geometric tower id, -1 none
+  int bin, j;       // eta/theta bin and phi bin of the hit; bin = -1: outside the grid
   int eps_row;      // -1 none
   bool accepted;
   float u, phi_pos;  // hit: u = z/r (or -z/r for a theta grid), azimuth
-  float pt_s, eta_mom, phi0, E_trk;  // valid if accepted
+};
+
+// smeared track quantities (S3), computed in a separate, converged pass over the accepted tracks
+struct TrackOut {
+  float pt_s, eta_mom, phi0, E_trk;
 };
 
 // bin i with tb[i] <= u < tb[i+1], -1 if outside or NaN
@@ -102,12 +106,11 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
                                                unsigned long long seed, long long event, uint32_t pidx,
                                                ParticleOut &o) {
   o.status = PD_DROPPED;
-  o.tower = -1;
+  o.bin = -1, o.j = 0;
   o.eps_row = -1;
   o.accepted = false;
   o.u = __int_as_float(0x7fc00000);
   o.phi_pos = o.u;
-  o.pt_s = 0.f, o.eta_mom = 0.f, o.phi0 = 0.f, o.E_trk = 0.f;
 
   const float pt2 = fmaf(px, px, py * py);
   const float r02 = fmaf(vx, vx, vy * vy);
@@ -248,22 +251,49 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
     if (eps > 0.f) {
       uint32_t rn[4];
       rng_block(seed, event, pidx, 0u, rn);
-      if (uniform24(rn[0]) < eps) {
-        o.accepted = true;
-        // A12/A13: log-normal with mean pT and std sigma_rel pT; eta, phi unchanged; E = pT' cosh(eta)
-        const float bp = sc.trk_b * pt;
-        const float rel2 = fmaf(bp, bp, sc.trk_a2);
-        o.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(rn[1], rn[2])) : pt;
-        o.E_trk = o.pt_s * (sqrtf(fmaf(pz, pz, pt2)) / pt);
-        o.eta_mom = asinhf(pz / pt);
-        o.phi0 = atan2f(py, px);
-      }
+      o.accepted = uniform24(rn[0]) < eps;
     }
   }
 
   // S4 tower of the hit
   const int i = grid_bin(cd, sc.n_bins, u);
-  if (i >= 0) o.tower = cd.offset[i] + phi_bin(cd, i, phi_pos);
+  o.bin = i;
+  if (i >= 0) o.j = phi_bin(cd, i, phi_pos);
+}
+
+// S3 for one accepted track (A12/A13): log-normal with mean pT and std sigma_rel pT, driven by words
+// 1 and 2 of the particle's Philox block; eta, phi unchanged; E = pT' cosh(eta) = pT' |p| / pT.
+__device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, float py, float pz,
+                                            unsigned long long seed, long long event, uint32_t pidx, TrackOut &t) {
+  const float pt2 = fmaf(px, px, py * py);
+  const float pt = sqrtf(pt2);
+  uint32_t rn[4];
+  rng_block(seed, event, pidx, 0u, rn);
+  const float bp = sc.trk_b * pt;
+  const float rel2 = fmaf(bp, bp, sc.trk_a2);
+  t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(rn[1], rn[2])) : pt;
+  t.E_trk = t.pt_s * (sqrtf(fmaf(pz, pz, pt2)) / pt);
+  t.eta_mom = asinhf(pz / pt);
+  t.phi0 = atan2f(py, px);
+}
+
+// per-tower smear of both components (S6): the common case of a single non-zero component runs one
+// branch-free log-normal; only towers holding both ECAL and HCAL energy take the second
+__device__ __forceinline__ void tower_smear(const PdCardScalars &sc, float Eem, float Ehad, const uint32_t (&rn)[4],
+                                            float &em_s, float &had_s) {
+  const bool prim_em = Eem > 0.f;
+  const float Ep = prim_em ? Eem : Ehad;
+  const float c2 = prim_em ? sc.ecal2[0] : sc.hcal2[0], s2c = prim_em ? sc.ecal2[1] : sc.hcal2[1],
+              n2 = prim_em ? sc.ecal2[2] : sc.hcal2[2];
+  const uint32_t xa = prim_em ? rn[0] : rn[2], xb = prim_em ? rn[1] : rn[3];
+  float sp = 0.f;
+  if (Ep > 0.f) {
+    const float v = fmaf(c2 * Ep, Ep, fmaf(s2c, Ep, n2));
+    sp = v > 0.f ? lognormal_rel(Ep, v / (Ep * Ep), normal_bm(xa, xb)) : Ep;
+  }
+  em_s = prim_em ? sp : 0.f;
+  had_s = prim_em ? 0.f : sp;
+  if (prim_em && Ehad > 0.f) had_s = smear_component(Ehad, sc.hcal2, rn[2], rn[3]);
 }
 
 // eta of a hit from u (only tracks and debug need it as a number)
