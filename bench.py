@@ -49,12 +49,18 @@ def _peaks():
 
 
 def _traffic(cfg):
-    """DRAM bytes per launch from the committed ncu --set full capture, if one exists for this config."""
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed ncu --set full
+    capture of this config, if one exists: last matching row of profiles/dram_traffic.csv."""
+    val = None
     try:
-        with open(os.path.join(ROOT, "profiles", "dram_traffic.json")) as f:
-            return json.load(f).get("cfg%d" % cfg)
+        with open(os.path.join(ROOT, "profiles", "dram_traffic.csv")) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 2 and c[0] == "cfg%d" % cfg:
+                    val = float(c[1])
     except Exception:
         return None
+    return val
 
 
 def _sample_events(ev, max_particles):
@@ -221,9 +227,9 @@ def run_ours(args, rank, world, local_rank):
 
     if dist is not None:
         # CSR rebasing of shard outputs: one all-gather of three int64 per rank, outside the data path
-        mine = torch.tensor(totals, dtype=torch.int64, device="cuda")
-        allt = [torch.zeros_like(mine) for _ in range(world)]
-        dist.all_gather(allt, mine)
+        from paper_2606_26089_b200 import shard
+
+        shard.exchange_totals(totals, rank, world, dist, device="cuda")
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
