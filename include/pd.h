@@ -60,7 +60,7 @@ typedef struct {
  * undefined behaviour (reading A31). */
 typedef struct {
   int64_t n_events;       /* >= 0                                                        */
-  int64_t n_particles;    /* == offsets[n_events]; < 2^31                                */
+  int64_t n_particles;    /* == offsets[n_events]; < 2^30                                */
   const int64_t *offsets; /* [n_events+1], offsets[0] == 0, non-decreasing               */
   const int32_t *pid;     /* PDG id                                                      */
   const int8_t *charge;   /* units of e; authoritative for charged/neutral               */

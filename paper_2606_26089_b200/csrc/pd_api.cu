@@ -73,7 +73,7 @@ int pd_card_info(const pd_card *card, pd_card_info_t *out) {
   out->bz = card->bz;
   out->radius = card->sc.R;
   out->half_length = card->sc.L;
-  out->n_eff_rows = card->sc.n_eff;
+  out->n_eff_rows = card->n_eff_rows;
   return PD_OK;
 }
 
@@ -81,7 +81,7 @@ int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_part
   if (!card || n_events < 0 || n_particles < 0) return PD_EINVAL;
   PdLaunchPlan plan;
   pd_plan(card, n_events, n_particles, &plan);
-  return (int64_t)(kWsHeader + 3 * sizeof(unsigned long long) * (size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1));
+  return (int64_t)(kWsHeader + 2 * sizeof(unsigned long long) * (size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1));
 }
 
 int pd_last_launch_count(void) { return t_launches; }
@@ -99,7 +99,8 @@ int pd_card_to_device(const pd_card *c) {
     c->dev_blob = nullptr;
   }
   const size_t nb = (size_t)c->sc.n_bins;
-  const size_t words = (nb + 1) + nb + (nb + 1) + 5 * nb;
+  const size_t lut_words = (c->lut.size() + 1) / 2;
+  const size_t words = (nb + 1) + nb + (nb + 1) + 5 * nb + lut_words;
   std::vector<uint32_t> blob(words);
   size_t o = 0;
   auto put = [&](const void *src, size_t n) {
@@ -111,6 +112,9 @@ int pd_card_to_device(const pd_card *c) {
   const size_t o_tb = put(c->tb.data(), nb + 1), o_nphi = put(c->nphi.data(), nb), o_off = put(c->offset.data(), nb + 1);
   const size_t o_iw = put(c->inv_w.data(), nb), o_half = put(c->half.data(), nb), o_w = put(c->w.data(), nb);
   const size_t o_eta = put(c->eta_c.data(), nb), o_ic = put(c->inv_cosh.data(), nb);
+  const size_t o_lut = o;
+  std::memcpy(blob.data() + o, c->lut.data(), 2 * c->lut.size());
+  o += lut_words;
   void *d = nullptr;
   PD_CUDA(cudaMalloc(&d, 4 * words));
   cudaError_t e = cudaMemcpy(d, blob.data(), 4 * words, cudaMemcpyHostToDevice);
@@ -127,6 +131,7 @@ int pd_card_to_device(const pd_card *c) {
   c->dev_tab.w = (const float *)(base + o_w);
   c->dev_tab.eta_c = (const float *)(base + o_eta);
   c->dev_tab.inv_cosh = (const float *)(base + o_ic);
+  c->dev_tab.lut = (const unsigned short *)(base + o_lut);
   c->dev_blob = d;
   c->dev_id = dev;
   return PD_OK;
@@ -139,7 +144,7 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
                 void *cuda_stream) {
   t_launches = 0;
   if (!card || !ev || !trk || !tow || !efl) return PD_EINVAL;
-  if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 31)) return PD_EINVAL;
+  if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 30)) return PD_EINVAL;
   if (!ev->offsets || !trk->offsets || !tow->offsets || !efl->offsets) return PD_EINVAL;
   const int64_t n = ev->n_particles;
   if (n > 0) {
@@ -195,7 +200,6 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
   p.events_per_tile = plan.events_per_tile;
   p.n_tiles = plan.n_tiles;
   p.capacity = plan.capacity;
-  p.event_bits = plan.event_bits;
   unsigned char *ws = (unsigned char *)workspace;
   p.tile_counter = (unsigned int *)ws;
   p.status_word = (int *)(ws + 4);
@@ -219,7 +223,7 @@ int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, in
                      pd_towers *tow, pd_eflow *efl, void *cuda_stream) {
   t_launches = 0;
   if (!card || !ev || !trk || !tow || !efl) return PD_EINVAL;
-  if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 31)) return PD_EINVAL;
+  if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 30)) return PD_EINVAL;
   if (!ev->offsets || !trk->offsets || !tow->offsets || !efl->offsets) return PD_EINVAL;
   const int64_t n = ev->n_particles, ne = ev->n_events;
   if (trk->capacity < n || tow->capacity < n || efl->capacity < 2 * n) return PD_ECAPACITY;

@@ -164,35 +164,22 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     total += n;
   }
 
+  if (total > long(PD_MAX_TOWERS)) return PD_ECARD;
+
   c->name = r.name;
   c->bz = float(r.bz);
+  c->n_eff_rows = int(r.eff.size());
   PdCardScalars &s = c->sc;
   const double R = f32(r.radius), L = f32(r.half_length), B = f32(r.bz), kappa = f32(r.kappa);
-  s.R = float(R), s.L = float(L), s.R2 = float(R * R);
+  s.R = float(R), s.L = float(L), s.R2 = float(R * R), s.inv_R = float(1.0 / R);
   s.kB_d = kappa * std::fabs(B);
   s.kB = float(s.kB_d);
+  s.inv_kB = s.kB_d > 0 ? float(1.0 / s.kB_d) : 0.f;
   s.sB = B > 0 ? 1.f : (B < 0 ? -1.f : 0.f);
   s.grid_theta = r.theta ? 1 : 0;
   s.n_bins = int(nb);
   s.n_towers = int(total);
-  {
-    long max_n = 1;
-    for (long n : r.nphi) max_n = std::max(max_n, n);
-    s.j_bits = 0;
-    while ((1L << s.j_bits) < max_n) ++s.j_bits;
-    int bin_bits = 0;
-    while ((size_t(1) << bin_bits) < nb) ++bin_bits;
-    s.code_bits = bin_bits + s.j_bits;
-    if (s.code_bits < 1) s.code_bits = 1;
-    if (s.code_bits > PD_MAX_CODE_BITS) return PD_ECARD;
-  }
-  s.n_eff = int(r.eff.size());
-  s.has_cos = r.has_cos ? 1 : 0;
-  {
-    // |cos theta| >= cmax  <=>  |pz|/pT >= cmax / sqrt(1 - cmax^2)
-    const double cm = f32(r.cos_max);
-    s.t_cos = r.has_cos ? (cm < 1.0 ? float(cm / std::sqrt(1.0 - cm * cm)) : std::numeric_limits<float>::infinity()) : 0.f;
-  }
+  s.words_per_event = int((total + 127) / 128) * 4;
   {
     const double a = f32(r.trk_a);
     s.trk_a2 = float(a * a);
@@ -204,14 +191,67 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     s.hcal2[k] = float(h * h);
   }
   s.thr_ecal = float(r.thr_ecal), s.thr_hcal = float(r.thr_hcal);
-  for (int i = 0; i < s.n_eff; ++i) {
-    const auto &row = r.eff[size_t(i)];
-    s.eff[i][0] = float(row[0]);
-    s.eff[i][1] = float(row[1]);
-    const double lo = f32(row[2]), hi = f32(row[3]);
-    s.eff[i][2] = lo > 0 ? float(std::sinh(lo)) : -1.f;
-    s.eff[i][3] = std::isinf(hi) ? std::numeric_limits<float>::infinity() : float(std::sinh(hi));
-    s.eff[i][4] = float(row[4]);
+
+  // ---- efficiency table -> grid of cells (reading A8: rows are pt_lo < pT <= pt_hi and
+  // |eta|_lo <= |eta| < |eta|_hi, first match wins; A9: eps = 0 for |cos theta| >= cmax).  Every pT
+  // edge therefore splits "pT > e", every |eta| edge splits "|eta| >= e", i.e. T = |pz|/pT >= sinh e.
+  {
+    std::vector<double> pte, te;  // distinct finite edges, ascending (fp32 values)
+    auto add = [](std::vector<double> &v, double x) {
+      if (!std::isfinite(x)) return;
+      for (double y : v)
+        if (float(y) == float(x)) return;
+      v.push_back(x);
+    };
+    const double cm = f32(r.cos_max);
+    // |cos theta| >= cmax  <=>  |pz|/pT >= cmax / sqrt(1 - cmax^2)
+    const double t_cos = r.has_cos ? (cm < 1.0 ? double(float(cm / std::sqrt(1.0 - cm * cm))) : kInf) : kInf;
+    struct Row { double lo, hi, tlo, thi, eps; };
+    std::vector<Row> rows;
+    for (const auto &row : r.eff) {
+      Row w;
+      w.lo = f32(row[0]), w.hi = std::isinf(row[1]) ? kInf : f32(row[1]);
+      const double elo = f32(row[2]), ehi = std::isinf(row[3]) ? kInf : f32(row[3]);
+      w.tlo = elo > 0 ? double(float(std::sinh(elo))) : -1.0;
+      w.thi = std::isinf(ehi) ? kInf : double(float(std::sinh(ehi)));
+      w.eps = f32(row[4]);
+      rows.push_back(w);
+      if (w.lo > 0) add(pte, w.lo);
+      add(pte, w.hi);
+      if (w.tlo > 0) add(te, w.tlo);
+      add(te, w.thi);
+    }
+    if (r.has_cos) add(te, t_cos);
+    std::sort(pte.begin(), pte.end());
+    std::sort(te.begin(), te.end());
+    if (pte.size() > size_t(PD_MAX_EFF_EDGES) || te.size() > size_t(PD_MAX_EFF_EDGES)) return PD_ECARD;
+    s.n_pt = int(pte.size()), s.n_T = int(te.size());
+    for (int k = 0; k < s.n_pt; ++k) {
+      s.pt_edge2_d[k] = pte[size_t(k)] * pte[size_t(k)];
+      s.pt_edge2[k] = float(s.pt_edge2_d[k]);
+    }
+    for (int k = 0; k < s.n_T; ++k) s.T_edge[k] = float(te[size_t(k)]);
+    for (int ip = 0; ip <= s.n_pt; ++ip) {
+      // representative pT of the interval (e[ip-1], e[ip]]: its closed upper end, or beyond the last edge
+      const double pt_rep = ip < s.n_pt ? pte[size_t(ip)] : (s.n_pt ? 2.0 * pte.back() + 1.0 : 1.0);
+      for (int it = 0; it <= s.n_T; ++it) {
+        // representative T of [t[it-1], t[it]): its closed lower end, or 0
+        const double T_rep = it > 0 ? te[size_t(it - 1)] : 0.0;
+        float eps = 0.f;
+        int rowi = -1;
+        if (!(r.has_cos && T_rep >= t_cos)) {
+          for (size_t k = 0; k < rows.size(); ++k) {
+            const Row &w = rows[k];
+            if (pt_rep > w.lo && pt_rep <= w.hi && (w.tlo <= 0 || T_rep >= w.tlo) && T_rep < w.thi) {
+              rowi = int(k), eps = float(w.eps);
+              break;
+            }
+          }
+        }
+        s.cell_eps[ip * (s.n_T + 1) + it] = eps;
+        s.cell_row[ip * (s.n_T + 1) + it] = (signed char)rowi;
+      }
+    }
   }
 
   c->edges.resize(nb + 1);
@@ -246,5 +286,42 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     c->inv_cosh[i] = float(1.0 / std::cosh(eta));
   }
   c->offset[nb] = acc;
+
+  // ---- eta-bin lookup: cells of |u| by float bits (2^(23 - PD_LUT_SHIFT) cells per octave, |u| < 2^MIN_EXP in
+  // one cell), mirrored for u < 0.  lut[cell] = the bin holding the cell's LOWER bound (clamped to the grid);
+  // the kernel then steps forward while u >= tb[bin + 1], so any monotone edge list is handled exactly.
+  {
+    float umax = 1.f;
+    for (float t : c->tb)
+      if (std::isfinite(t)) umax = std::max(umax, std::fabs(t));
+    auto bits = [](float x) {
+      uint32_t b;
+      std::memcpy(&b, &x, 4);
+      return int(b >> PD_LUT_SHIFT);
+    };
+    s.lut_base = bits(std::ldexp(1.f, PD_LUT_MIN_EXP));
+    s.lut_side = bits(umax) - s.lut_base + 2;
+    const int side = s.lut_side;
+    c->lut.assign(size_t(2 * side), 0);
+    auto cell_lo_abs = [&](int ca) {  // smallest |u| of cell ca on one side
+      if (ca <= 0) return 0.f;
+      const uint32_t b = uint32_t(ca + s.lut_base) << PD_LUT_SHIFT;
+      float x;
+      std::memcpy(&x, &b, 4);
+      return x;
+    };
+    auto bin_of = [&](double u) {  // largest b with tb[b] <= u, clamped to [0, nb-1]
+      int b = 0;
+      while (b + 1 < int(nb) && double(c->tb[size_t(b + 1)]) <= u) ++b;
+      return b;
+    };
+    for (int ca = 0; ca < side; ++ca) {
+      // positive side: u in [lo(ca), lo(ca+1)); cell index side + ca
+      c->lut[size_t(side + ca)] = (unsigned short)bin_of(double(cell_lo_abs(ca)));
+      // negative side: u in (-lo(ca+1), -lo(ca)]; lower bound -lo(ca+1) (-inf for the last cell)
+      const double lo = ca + 1 < side ? -double(cell_lo_abs(ca + 1)) : -kInf;
+      c->lut[size_t(side - 1 - ca)] = (unsigned short)bin_of(lo);
+    }
+  }
   return PD_OK;
 }

@@ -8,28 +8,39 @@
 
 #include "pd.h"
 
-constexpr int PD_MAX_BINS = 1024;  // eta/theta bins of a card's grid
-constexpr int PD_MAX_EFF = 32;     // rows of the efficiency table
-constexpr int PD_MAX_CODE_BITS = 20;  // packed (eta bin, phi bin) tower code
+constexpr int PD_MAX_BINS = 1024;      // eta/theta bins of a card's grid
+constexpr int PD_MAX_EFF = 32;         // rows of the efficiency table in a card
+constexpr int PD_MAX_EFF_EDGES = 8;    // distinct pT edges / distinct |eta| edges of the table
+constexpr int PD_MAX_EFF_CELLS = (PD_MAX_EFF_EDGES + 1) * (PD_MAX_EFF_EDGES + 1);
+constexpr int PD_MAX_TOWERS = 1 << 15;  // tower ids are packed into 15 bits on chip
+constexpr int PD_LUT_SHIFT = 19;       // eta-bin lookup: 16 cells per octave of |u|
+constexpr int PD_LUT_MIN_EXP = -8;     // |u| < 2^-8 shares one cell per side
 
 // Scalars of a card as the kernels want them (all derived in double at load, stored as fp32).
 struct PdCardScalars {
-  float R, L, R2;        // calorimeter radius, half length, R^2
-  float kB;              // kappa * |B|   [GeV / m]
-  double kB_d;           // same in double (only used for the endcap turning angle)
-  float sB;              // sign of B (0 if B == 0)
-  int grid_theta;        // 0: bins in eta, 1: bins in theta
+  float R, L, R2, inv_R;  // calorimeter radius, half length, R^2, 1/R
+  float kB, inv_kB;       // kappa * |B|  [GeV / m] and its inverse
+  double kB_d;            // same in double (only used for the endcap turning angle)
+  float sB;               // sign of B (0 if B == 0)
+  int grid_theta;         // 0: bins in eta, 1: bins in theta
   int n_bins, n_towers;
-  int j_bits, code_bits;  // packed tower code = bin << j_bits | phi bin (ordered like the tower id)
-  int n_eff, has_cos;
-  float t_cos;           // |pz|/pT threshold equivalent to |cos theta| >= abs_costheta_max
-  float trk_a2, trk_b;   // sigma_rel^2 = a^2 + (b pT)^2
+  int words_per_event;    // tower bitmap: ceil(n_towers / 128) * 4 words of 32 tower bits
+  // eta-bin lookup table over the float bits of |u| (see pd_card.cpp): cells per side, bias
+  int lut_side, lut_base;
+  // efficiency table resolved into a grid at load (reading A8: first matching row wins):
+  // cell = (#pT edges with pT > e) * (n_T + 1) + (#T edges with |pz|/pT >= t)
+  int n_pt, n_T;
+  float pt_edge2[PD_MAX_EFF_EDGES];   // e^2 (fp32) for the fast test
+  double pt_edge2_d[PD_MAX_EFF_EDGES];  // e^2 in double for pT within rounding of an edge
+  float T_edge[PD_MAX_EFF_EDGES];     // sinh |eta| edges (incl. the |cos theta| cut)
+  float cell_eps[PD_MAX_EFF_CELLS];
+  signed char cell_row[PD_MAX_EFF_CELLS];  // row of the card's table, -1 none
+  float trk_a2, trk_b;       // sigma_rel^2 = a^2 + (b pT)^2
   float ecal2[3], hcal2[3];  // C^2, S^2, N^2 of sigma^2 = C^2 E^2 + S^2 E + N^2
   float thr_ecal, thr_hcal;
-  float eff[PD_MAX_EFF][5];  // pt_lo, pt_hi, sinh(|eta|_lo) (<= 0: no lower cut), sinh(|eta|_hi), eps
 };
 
-// Per-bin tables, each n_bins (+1 for tb / offset) long, contiguous in one device allocation.
+// Per-bin tables, contiguous in one device allocation.
 struct PdCardTables {
   const float *tb;        // [n_bins+1] bin thresholds in u = z/r (eta grid) or -z/r (theta grid)
   const int *nphi;        // [n_bins]
@@ -39,6 +50,7 @@ struct PdCardTables {
   const float *w;         // [n_bins] 2 pi / nphi
   const float *eta_c;     // [n_bins] tower-centre pseudorapidity
   const float *inv_cosh;  // [n_bins] 1 / cosh(eta_c)
+  const unsigned short *lut;  // [2 * lut_side] first candidate bin of a cell
 };
 
 struct pd_card {
@@ -48,7 +60,9 @@ struct pd_card {
   std::vector<float> edges;  // [n_bins+1] the card's edges (eta or theta), fp32
   std::vector<float> tb, inv_w, half, w, eta_c, inv_cosh;
   std::vector<int> nphi, offset;
+  std::vector<unsigned short> lut;
   float bz = 0.f;
+  int n_eff_rows = 0;
   // device copy, created lazily by the first simulate call
   mutable void *dev_blob = nullptr;
   mutable int dev_id = -1;
@@ -93,8 +107,7 @@ struct PdParams {
   int events_per_tile;   // G
   int n_tiles;
   int capacity;          // C: particles a tile may hold on chip
-  int event_bits;        // bits needed for a local event index
-  unsigned long long *chain;  // [3][n_tiles] look-back words: tracks, towers, eflow
+  unsigned long long *chain;  // [2][n_tiles] look-back words: tracks; towers | neutrals
   unsigned int *tile_counter;
   int *status_word;
 };
@@ -105,13 +118,11 @@ int pd_card_parse(const char *name_or_path, pd_card *c);
 int pd_card_to_device(const pd_card *c);
 // pd_kernels.cu
 struct PdLaunchPlan {
-  int threads;       // 256 or 512
+  int threads;       // 512 (two CTAs per SM) or 1024 (one)
   int capacity;      // C
   int events_per_tile;
   int n_tiles;
-  int event_bits;
   size_t smem_bytes;
-  int grid;
 };
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);
 int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, void *stream);

@@ -1,18 +1,23 @@
-// pd_kernels.cu -- the fused Delphes-chain kernel for sm_100a (steps S0..S8 of SURVEY.md section 8a).
+// pd_kernels.cu -- the fused Delphes-chain kernel for sm_100a (steps S0..S8 of SURVEY.md section 8a), v3.
 //
-// One persistent CTA per SM slot; a CTA repeatedly claims a TILE (a run of G whole events, <= C
-// particles) from an atomic counter and takes it through
-//   phase 1   S0-S4  one thread per particle: classify, propagate, efficiency, pT smear, tower key;
-//                    accepted tracks and deposits are compacted IN PARTICLE ORDER into shared memory
-//   chain T          decoupled look-back over tiles -> global track offset; tracks + track CSR written
-//   phase 2a  S5     stable LSD radix sort of the deposits by (local event, tower) in shared memory
-//   phase 2b  S5-S7  one thread per distinct (event, tower): sequential sum in particle order,
-//                    Philox tower stream, log-normal smear, thresholds, EFlow subtraction
-//   chain W          look-back for the tower and eflow offsets
-//   phase 3   S8     ordered compaction of towers / photons / neutral hadrons, EFlow track entries,
-//                    CSR offsets
-// Nothing but the inputs and the final collections touches HBM.  Sums are order-stable: the sort is
-// stable, the per-tower sum is sequential, and the only atomics are integer counters.
+// Persistent CTAs (two 512-thread CTAs per SM, or one 1024-thread CTA for large events); a CTA repeatedly
+// claims a TILE (a run of G whole events, <= C particles) from an atomic counter and takes it through
+//   pass A   S0-S2, S4  one thread per particle, particle order, inputs prefetched one iteration ahead:
+//                       classify, propagate, efficiency, tower id; marks the tower in the event's BITMAP
+//   scan 1              one block scan for two things: the ordered list of accepted tracks, and the
+//                       popcount prefix of the bitmaps = the rank ("slot") of every occupied tower in
+//                       (event, tower id) order -- this replaces a sort of the deposits
+//   pass B   S5         every deposit pushes itself on its slot's list (one integer atomicExch)
+//   chain T             decoupled look-back over tiles -> global track offset (overlaps pass B)
+//   pass T   S3         one thread per accepted track: pT smear, track record written to HBM
+//   pass W   S5-S7      one thread per occupied tower: sum of its list IN PARTICLE ORDER (fp32, sequential),
+//                       Philox tower stream, log-normal smear, thresholds, EFlow subtraction
+//   chain W             look-back for the tower and neutral offsets (one packed 64-bit word)
+//   pass O   S8         ordered compaction of towers / photons / neutral hadrons, EFlow track entries,
+//                       CSR offsets
+// Nothing but the inputs and the final collections touches HBM.  Sums are order-stable: each tower's
+// deposits are added sequentially in ascending particle index whatever order the list was built in, and
+// the only atomics are integer (bitmap OR, list exchange, counters).
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -24,26 +29,29 @@
 
 namespace pdk {
 
-constexpr int G_MAX = 256;     // events per tile (8 event bits)
-constexpr int r_max(int threads) { return threads >= 1024 ? 6 : 12; }  // radix-sort rounds per warp: C <= THREADS * r_max
-// deposit key = hcal << 31 | local event << code_bits | tower code (eta bin << j_bits | phi bin)
-constexpr uint32_t KEY_MASK = 0x7fffffffu;
+constexpr int G_MAX = 256;         // events per tile (event index of a particle is kept in 8 bits)
+constexpr int C_MAX = 8191;        // particles per tile: list links are 13 bits, 0x1fff = end of list
+constexpr uint32_t LINK_END = 0x1fffu;
+// per-particle result word: tower id (15 bits, 0x7fff none) | flags | link to the next deposit of the tower
+constexpr uint32_t RES_TOWER = 0x7fffu, RES_DEP = 1u << 15, RES_HCAL = 1u << 16, RES_ACC = 1u << 17;
+constexpr int RES_LINK_SHIFT = 18;
 constexpr unsigned long long FLAG_A = 1ull << 62, FLAG_P = 2ull << 62, VAL_MASK = (1ull << 62) - 1;
+constexpr unsigned long long FIELD_MASK = (1ull << 31) - 1;  // chain W packs towers | neutrals << 31
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~size_t(15); }
 
 // Shared-memory carve-up, identical on host (size) and device (pointers).
 struct Layout {
-  size_t tb, nphi, offset, inv_w, half, w, eta_c, inv_cosh;  // card tables
-  size_t off32, ntrk, ntow, nph, nnh;                        // per-event arrays [G_MAX+1]
-  size_t misc;                                               // 64 x u64 scratch
-  size_t cnt;                                                // radix counters u16 [256 * W]
-  size_t dep_key, dep_E, dep_T, dep_idx;                     // deposits
-  size_t uni;                                                // union: track staging | tower staging
+  size_t tb, nphi, offset, inv_w, half, w, eta_c, inv_cosh, lut, binlut;  // card tables
+  size_t off32, ntrk, ntow, nph, nnh;                                     // per-event arrays [G+1]
+  size_t misc;                                                            // scratch words
+  size_t bitmap, gprefix;                                                 // per event: tower bits, group prefix
+  size_t res, uT, phi, Ev, head, stg, ev;                                 // per particle / per slot
   size_t total;
 };
 
-__host__ __device__ inline Layout make_layout(int n_bins, int threads, int C) {
+__host__ __device__ inline Layout make_layout(int n_bins, int lut_cells, int n_towers, int words_per_event, int G,
+                                              int C) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) {
@@ -59,18 +67,23 @@ __host__ __device__ inline Layout make_layout(int n_bins, int threads, int C) {
   l.w = take(4 * n_bins);
   l.eta_c = take(4 * n_bins);
   l.inv_cosh = take(4 * n_bins);
-  l.off32 = take(4 * (G_MAX + 1));
-  l.ntrk = take(4 * (G_MAX + 1));
-  l.ntow = take(4 * (G_MAX + 1));
-  l.nph = take(4 * (G_MAX + 1));
-  l.nnh = take(4 * (G_MAX + 1));
-  l.misc = take(8 * 96);
-  l.cnt = take(2 * 256 * (threads / 32));
-  l.dep_key = take(4 * (size_t)C);
-  l.dep_E = take(4 * (size_t)C);
-  l.dep_T = take(4 * (size_t)C);
-  l.dep_idx = take(2 * (size_t)C);
-  l.uni = take(20 * (size_t)C + 16);
+  l.lut = take(2 * (size_t)lut_cells);
+  l.binlut = take(2 * (size_t)((n_towers >> 5) + 2));
+  l.off32 = take(4 * (G + 1));
+  l.ntrk = take(4 * (G + 1));
+  l.ntow = take(4 * (G + 1));
+  l.nph = take(4 * (G + 1));
+  l.nnh = take(4 * (G + 1));
+  l.misc = take(8 * 64);
+  l.bitmap = take(4 * (size_t)G * words_per_event);
+  l.gprefix = take(2 * ((size_t)G * (words_per_event / 4) + 1));
+  l.res = take(4 * (size_t)C);
+  l.uT = take(4 * (size_t)C);
+  l.phi = take(4 * (size_t)C);
+  l.Ev = take(4 * (size_t)C);
+  l.head = take(2 * (size_t)C);
+  l.stg = take(4 * (size_t)C);
+  l.ev = take(G > 1 ? (size_t)C : 0);
   l.total = o;
   return l;
 }
@@ -92,7 +105,7 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
 }
 
 // Called by one full warp.  Publishes this tile's aggregate, returns the exclusive prefix over all
-// earlier tiles to every lane, then publishes the inclusive prefix.
+// earlier tiles to every lane, then publishes the inclusive prefix.  (Packed fields add independently.)
 __device__ unsigned long long chain_lookback(unsigned long long *st, int tile, unsigned long long agg) {
   const int lane = threadIdx.x & 31;
   if (tile == 0) {
@@ -151,28 +164,6 @@ __device__ __forceinline__ void event_scan(int *a, int ne) {
   if (lane == 0) a[ne] = total;
 }
 
-// largest e in [0, ne) with off[e] <= i
-__device__ __forceinline__ int find_event(const int *off, int ne, int i) {
-  int lo = 0, hi = ne;
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (off[mid] <= i) lo = mid;
-    else hi = mid;
-  }
-  return lo;
-}
-
-// largest b in [0, nb) with offset[b] <= id
-__device__ __forceinline__ int find_bin(const int *offset, int nb, int id) {
-  int lo = 0, hi = nb;
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (offset[mid] <= id) lo = mid;
-    else hi = mid;
-  }
-  return lo;
-}
-
 // Block-wide exclusive prefix of packed per-warp totals wtot[W] (REDUX adds): returns the exclusive
 // prefix of this thread's WARP and the block total.  Fields of the packed word must not overflow.
 template <int W>
@@ -183,18 +174,54 @@ __device__ __forceinline__ void warp_totals_scan(const unsigned *wtot, unsigned 
   excl_warp = __reduce_add_sync(0xffffffffu, lane < wid ? v : 0u);
 }
 
-// bits of the per-particle result word written by pass P1
-constexpr uint32_t RES_DEP = 1u << 21, RES_HCAL = 1u << 22, RES_ACC = 1u << 23;
+__device__ __forceinline__ unsigned warp_incl_scan(unsigned v) {
+  const int lane = threadIdx.x & 31;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned t = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= o) v += t;
+  }
+  return v;
+}
+
+struct ParticleIn {
+  int pid, q;
+  float px, py, pz, E, vx, vy, vz;
+};
+
+__device__ __forceinline__ ParticleIn load_particle(const PdParams &prm, long long g) {
+  ParticleIn p;
+  p.pid = __ldg(prm.pid + g);
+  p.q = (int)__ldg(prm.charge + g);
+  p.px = __ldg(prm.px + g), p.py = __ldg(prm.py + g), p.pz = __ldg(prm.pz + g);
+  p.E = __ldg(prm.E + g);
+  p.vx = __ldg(prm.vx + g), p.vy = __ldg(prm.vy + g), p.vz = __ldg(prm.vz + g);
+  return p;
+}
+
+__device__ __forceinline__ int popc4(const uint4 &v) { return __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w); }
+
+// number of set bits of the 128-bit group below bit position pos (0..127)
+__device__ __forceinline__ int popc_below(const uint4 &v, int pos) {
+  const int w = pos >> 5;
+  const uint32_t m = (1u << (pos & 31)) - 1u;
+  const uint32_t cur = w == 0 ? v.x : (w == 1 ? v.y : (w == 2 ? v.z : v.w));
+  int c = __popc(cur & m);
+  c += w > 0 ? __popc(v.x) : 0;
+  c += w > 1 ? __popc(v.y) : 0;
+  c += w > 2 ? __popc(v.z) : 0;
+  return c;
+}
 
 template <int THREADS, int CTAS, bool DEBUG>
 __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_constant__ PdParams prm) {
   constexpr int W = THREADS / 32;
-  constexpr int R_MAX = r_max(THREADS);
   extern __shared__ __align__(16) unsigned char smem[];
   const PdCardScalars &sc = prm.sc;
   const int nb = sc.n_bins;
-  const int C = prm.capacity;
-  const Layout L = make_layout(nb, THREADS, C);
+  const int C = prm.capacity, G = prm.events_per_tile;
+  const int wpe = sc.words_per_event, gpe = wpe >> 2;
+  const Layout L = make_layout(nb, 2 * sc.lut_side, sc.n_towers, wpe, G, C);
   float *s_tb = (float *)(smem + L.tb);
   int *s_nphi = (int *)(smem + L.nphi);
   int *s_offset = (int *)(smem + L.offset);
@@ -203,26 +230,25 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
   float *s_w = (float *)(smem + L.w);
   float *s_eta_c = (float *)(smem + L.eta_c);
   float *s_inv_cosh = (float *)(smem + L.inv_cosh);
+  unsigned short *s_lut = (unsigned short *)(smem + L.lut);
+  unsigned short *s_binlut = (unsigned short *)(smem + L.binlut);
   int *s_off32 = (int *)(smem + L.off32);
   int *s_ntrk = (int *)(smem + L.ntrk);
   int *s_ntow = (int *)(smem + L.ntow);
   int *s_nph = (int *)(smem + L.nph);
   int *s_nnh = (int *)(smem + L.nnh);
   unsigned long long *s_misc = (unsigned long long *)(smem + L.misc);
-  int *s_ctr = (int *)(s_misc + 4);             // [0] charged count, [1] neutral count
-  unsigned *s_wtot = (unsigned *)(s_misc + 8);  // [5][32]
-  uint16_t *s_cnt = (uint16_t *)(smem + L.cnt);
-  uint32_t *dep_key = (uint32_t *)(smem + L.dep_key);
-  float *dep_E = (float *)(smem + L.dep_E);
-  float *dep_T = (float *)(smem + L.dep_T);
-  uint16_t *dep_idx = (uint16_t *)(smem + L.dep_idx);
-  // union region, view A (passes P0..P2): per-particle scratch
-  uint32_t *p_res = (uint32_t *)(smem + L.uni);
-  float *p_u = (float *)(p_res + C), *p_phi = p_u + C;
-  uint16_t *p_perm = (uint16_t *)(p_phi + C), *tk_i = p_perm + C;
-  // union region, view B (phase 2b on): per deposited tower
-  uint32_t *st_key = (uint32_t *)(smem + L.uni);
-  float *st_em = (float *)(st_key + C), *st_had = st_em + C, *st_nem = st_had + C, *st_nhad = st_nem + C;
+  unsigned *s_tot = (unsigned *)(s_misc + 4);    // [0] towers | photons << 16, [1] neutral hadrons
+  unsigned *s_wtot = (unsigned *)(s_misc + 8);   // [3][32] per-warp totals
+  uint32_t *s_bitmap = (uint32_t *)(smem + L.bitmap);
+  unsigned short *s_gp = (unsigned short *)(smem + L.gprefix);
+  uint32_t *s_res = (uint32_t *)(smem + L.res);
+  float *s_uT = (float *)(smem + L.uT);    // hit u of accepted tracks, then E_trk, then staged photon energy
+  float *s_phi = (float *)(smem + L.phi);  // hit phi of accepted tracks, then staged Eem''
+  float *s_Ev = (float *)(smem + L.Ev);    // deposit energy, then staged Ehad''
+  unsigned *s_head = (unsigned *)(smem + L.stg);         // per slot: last pusher, then head | tower id << 13
+  unsigned short *s_tk = (unsigned short *)(smem + L.head);  // accepted tracks in particle order
+  unsigned char *s_ev = smem + L.ev;
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
@@ -239,23 +265,33 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
     s_eta_c[i] = prm.tab.eta_c[i];
     s_inv_cosh[i] = prm.tab.inv_cosh[i];
   }
-  SmCard cd{s_tb, s_nphi, s_offset, s_inv_w, s_half, s_w, s_eta_c, s_inv_cosh};
-  const int G = prm.events_per_tile;
-  const int EV_SHIFT = sc.code_bits;
-  const int JB = sc.j_bits;
-  const uint32_t code_mask = (1u << EV_SHIFT) - 1u, j_mask = (1u << JB) - 1u;
+  for (int i = tid; i < 2 * sc.lut_side; i += THREADS) s_lut[i] = prm.tab.lut[i];
+  __syncthreads();
+  // eta bin of tower ids 0, 32, 64, ...: start of the short forward search of pass O
+  for (int c = tid; c <= (sc.n_towers >> 5); c += THREADS) {
+    const int id = c << 5;
+    int lo = 0, hi = nb;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (s_offset[mid] <= id) lo = mid;
+      else hi = mid;
+    }
+    s_binlut[c] = (unsigned short)lo;
+  }
+  SmCard cd{s_tb, s_nphi, s_offset, s_inv_w, s_half, s_w, s_eta_c, s_inv_cosh, s_lut};
 
   for (;;) {
     __syncthreads();  // previous tile fully done with shared memory (and card tables staged)
     if (tid == 0) {
       s_misc[0] = atomicAdd(prm.tile_counter, 1u);
-      s_ctr[0] = 0, s_ctr[1] = 0;
+      s_tot[0] = 0u, s_tot[1] = 0u;
     }
     __syncthreads();
     const int tile = (int)s_misc[0];
     if (tile >= prm.n_tiles) break;
     const long long e0 = (long long)tile * G;
     const int ne = (int)min((long long)G, prm.n_events - e0);
+    const bool multi = G > 1;
     const long long p0 = prm.offsets[e0];
     const long long p1 = prm.offsets[e0 + ne];
     int n = (int)min(p1 - p0, (long long)0x7fffffff);
@@ -268,186 +304,126 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       s_off32[e] = overflow ? 0 : (int)(prm.offsets[e0 + e] - p0);
       s_ntrk[e] = 0, s_ntow[e] = 0, s_nph[e] = 0, s_nnh[e] = 0;
     }
+    const int NG = ne * gpe;  // 128-tower bitmap groups of the tile
+    for (int k = tid; k < NG; k += THREADS) ((uint4 *)s_bitmap)[k] = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
+    if (multi) {
+      // event index of every particle of the tile: warp per event, lanes over its particles
+      for (int e = wid; e < ne; e += W)
+        for (int i = s_off32[e] + lane; i < s_off32[e + 1]; i += 32) s_ev[i] = (unsigned char)e;
+      __syncthreads();
+    }
 
-    // ------------------------------------------------------------------ P0: charged-first permutation
-    // (the per-particle math is order-independent; grouping by kind keeps its warps converged)
-    for (int it = 0; it * THREADS < n; ++it) {
-      const int i = it * THREADS + tid;
-      const bool valid = i < n;
-      const int q = valid ? (int)__ldg(prm.charge + p0 + i) : 0;
-      const bool chg = valid && q != 0, neu = valid && q == 0;
-      const unsigned cm = __ballot_sync(0xffffffffu, chg), nm = __ballot_sync(0xffffffffu, neu);
-      int cb = 0, nbs = 0;
-      if (lane == 0) {
-        if (cm) cb = atomicAdd(&s_ctr[0], __popc(cm));
-        if (nm) nbs = atomicAdd(&s_ctr[1], __popc(nm));
+    // ------------------------------------------------------------------ pass A: S0-S2, S4 per particle
+    {
+      ParticleIn nxt;
+      if (tid < n) nxt = load_particle(prm, p0 + tid);
+      for (int i = tid; i < n; i += THREADS) {
+        const ParticleIn c = nxt;
+        if (i + THREADS < n) nxt = load_particle(prm, p0 + i + THREADS);
+        const int e = multi ? (int)s_ev[i] : 0;
+        ParticleOut o;
+        particle_chain(sc, cd, c.q, c.px, c.py, c.pz, c.vx, c.vy, c.vz, prm.seed, prm.event_base + e0 + e,
+                       (uint32_t)(i - s_off32[e]), o);
+        const int apid = c.pid < 0 ? -c.pid : c.pid;
+        const bool to_ecal = apid == 11 || apid == 22;                             // reading A18
+        const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
+        uint32_t res = RES_TOWER | (LINK_END << RES_LINK_SHIFT);
+        if (o.tower >= 0) {
+          res = (uint32_t)o.tower | (LINK_END << RES_LINK_SHIFT);
+          if (!to_none) {
+            res |= RES_DEP | (to_ecal ? 0u : RES_HCAL);
+            atomicOr(&s_bitmap[e * wpe + (o.tower >> 5)], 1u << (o.tower & 31));
+            s_Ev[i] = c.E;
+          }
+        }
+        if (o.accepted) {
+          res |= RES_ACC;
+          s_uT[i] = o.u, s_phi[i] = o.phi_pos;
+          if (multi) atomicAdd(&s_ntrk[e], 1);
+        }
+        s_res[i] = res;
+        s_head[i] = 0xffffffffu;
+        if (DEBUG) {
+          const long long g = p0 + i;
+          if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)o.status;
+          if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = (o.status & PD_FACE_MASK) ? eta_from_u(sc, o.u) : o.u;
+          if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = o.phi_pos;
+          if (prm.dbg_tower) prm.dbg_tower[g] = o.tower;
+          if (prm.dbg_accepted) prm.dbg_accepted[g] = o.accepted ? 1 : 0;
+          if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)o.eps_row;
+          if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = 0.f;
+          if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 0;
+        }
       }
-      cb = __shfl_sync(0xffffffffu, cb, 0), nbs = __shfl_sync(0xffffffffu, nbs, 0);
-      if (chg) p_perm[cb + __popc(cm & lt_mask)] = (uint16_t)i;
-      if (neu) p_perm[n - 1 - (nbs + __popc(nm & lt_mask))] = (uint16_t)i;
     }
     __syncthreads();
 
-    // ------------------------------------------------------------------ P1: S0-S2, S4 per particle (no barriers)
-    for (int k = tid; k < n; k += THREADS) {
-      const int i = p_perm[k];
-      const long long g = p0 + i;
-      const int pid = __ldg(prm.pid + g);
-      const int q = (int)__ldg(prm.charge + g);
-      const float px = __ldg(prm.px + g), py = __ldg(prm.py + g), pz = __ldg(prm.pz + g);
-      const float vx = __ldg(prm.vx + g), vy = __ldg(prm.vy + g), vz = __ldg(prm.vz + g);
-      const int e = find_event(s_off32, ne, i);
-      ParticleOut o;
-      particle_chain(sc, cd, pid, q, px, py, pz, vx, vy, vz, prm.seed, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), o);
-      const int apid = pid < 0 ? -pid : pid;
-      const bool to_ecal = apid == 11 || apid == 22;
-      const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
-      uint32_t res = 0;
-      if (o.bin >= 0) res = ((uint32_t)o.bin << JB) | (uint32_t)o.j | (to_none ? 0u : RES_DEP) | (to_ecal ? 0u : RES_HCAL);
-      if (o.accepted) {
-        res |= RES_ACC;
-        p_u[i] = o.u, p_phi[i] = o.phi_pos;
-        atomicAdd(&s_ntrk[e], 1);
-      }
-      p_res[i] = res;
-      if (DEBUG) {
-        if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)o.status;
-        if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = (o.status & PD_FACE_MASK) ? eta_from_u(sc, o.u) : o.u;
-        if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = o.phi_pos;
-        if (prm.dbg_tower) prm.dbg_tower[g] = o.bin >= 0 ? s_offset[o.bin] + o.j : -1;
-        if (prm.dbg_accepted) prm.dbg_accepted[g] = o.accepted ? 1 : 0;
-        if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)o.eps_row;
-        if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = 0.f;
-        if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 0;
-      }
-    }
-    __syncthreads();
-
-    // ------------------------------------------------------------------ P1b: ordered compaction (particle order)
-    int trk_base = 0, dep_base = 0;
-    for (int it = 0; it * THREADS < n; ++it) {
-      const int i = it * THREADS + tid;
-      const uint32_t res = i < n ? p_res[i] : 0u;
-      const bool acc = (res & RES_ACC) != 0, dep = (res & RES_DEP) != 0;
-      const unsigned am = __ballot_sync(0xffffffffu, acc), dm = __ballot_sync(0xffffffffu, dep);
-      if (lane == 0) s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(am) | ((unsigned)__popc(dm) << 16);
+    // ------------------------------------------------------------------ scan 1: tracks in order + tower slots
+    // Each thread owns a contiguous chunk of particles and of bitmap groups (odd chunk lengths keep the
+    // shared-memory accesses of a warp on distinct banks); one packed block scan serves both.
+    int n_trk, n_slots;
+    {
+      const int ka = ((n + THREADS - 1) / THREADS) | 1;
+      const int a0 = min(n, tid * ka), a1 = min(n, a0 + ka);
+      unsigned cnt_a = 0;
+      for (int i = a0; i < a1; ++i) cnt_a += (s_res[i] >> 17) & 1u;
+      const int kg = ((NG + THREADS - 1) / THREADS) | 1;
+      const int g0 = min(NG, tid * kg), g1 = min(NG, g0 + kg);
+      unsigned cnt_g = 0;
+      for (int g = g0; g < g1; ++g) cnt_g += (unsigned)popc4(((const uint4 *)s_bitmap)[g]);
+      const unsigned packed = cnt_a | (cnt_g << 16);
+      const unsigned incl = warp_incl_scan(packed);
+      if (lane == 31) s_wtot[wid] = incl;
       __syncthreads();
       unsigned excl_w, tot;
-      warp_totals_scan<W>(s_wtot + (it & 1) * 32, excl_w, tot);
-      if (acc) tk_i[trk_base + (int)(excl_w & 0xffffu) + __popc(am & lt_mask)] = (uint16_t)i;
-      if (dep) {
-        const int s = dep_base + (int)(excl_w >> 16) + __popc(dm & lt_mask);
-        const int e = find_event(s_off32, ne, i);
-        dep_key[s] = ((res & RES_HCAL) ? 0x80000000u : 0u) | ((uint32_t)e << EV_SHIFT) | (res & code_mask);
-        dep_idx[s] = (uint16_t)i;
-        dep_E[i] = __ldg(prm.E + p0 + i);
-        dep_T[i] = 0.f;
+      warp_totals_scan<W>(s_wtot, excl_w, tot);
+      const unsigned excl = excl_w + incl - packed;
+      int ra = (int)(excl & 0xffffu), rg = (int)(excl >> 16);
+      for (int i = a0; i < a1; ++i)
+        if (s_res[i] & RES_ACC) s_tk[ra++] = (unsigned short)i;
+      for (int g = g0; g < g1; ++g) {
+        s_gp[g] = (unsigned short)rg;
+        rg += popc4(((const uint4 *)s_bitmap)[g]);
       }
-      trk_base += (int)(tot & 0xffffu);
-      dep_base += (int)(tot >> 16);
+      n_trk = (int)(tot & 0xffffu), n_slots = (int)(tot >> 16);
     }
-    const int n_trk = trk_base, m = dep_base;
     __syncthreads();
 
-    // ------------------------------------------------------------------ phase 2a: stable radix sort
-    {
-      const int nbits = EV_SHIFT + prm.event_bits;
-      int n_pass = (nbits + 7) / 8;
-      int bits_per = (nbits + n_pass - 1) / n_pass;
-      if (bits_per < 5) bits_per = 5;
-      const int bins = 1 << bits_per;
-      const int ipw = 32 * ((m + 32 * W - 1) / (32 * W));  // items per warp, multiple of 32
-      for (int pass = 0; pass < n_pass; ++pass) {
-        const int shift = pass * bits_per;
-        const uint32_t dmask = (uint32_t)bins - 1u;
-        for (int k = tid; k < bins * W / 2; k += THREADS) ((uint32_t *)s_cnt)[k] = 0u;
-        __syncthreads();
-        uint32_t kreg[R_MAX], ireg[R_MAX];
-#pragma unroll
-        for (int r = 0; r < R_MAX; ++r) {
-          kreg[r] = 0, ireg[r] = 0;
-          if (r * 32 < ipw) {  // warp-uniform
-            const int pos = wid * ipw + r * 32 + lane;
-            const bool valid = pos < m;
-            const uint32_t k = valid ? dep_key[pos] : 0u;
-            const uint32_t ix = valid ? (uint32_t)dep_idx[pos] : 0u;
-            const uint32_t d = valid ? ((k >> shift) & dmask) : 0xffffffffu;
-            const unsigned peers = __match_any_sync(0xffffffffu, d);
-            const unsigned lower = peers & lt_mask;
-            const uint32_t c = valid ? (uint32_t)s_cnt[d * W + wid] : 0u;
-            __syncwarp();
-            if (valid && lower == 0u) s_cnt[d * W + wid] = (uint16_t)(c + (uint32_t)__popc(peers));
-            __syncwarp();
-            kreg[r] = k;
-            ireg[r] = ix | ((c + (uint32_t)__popc(lower)) << 16);
-          }
-        }
-        __syncthreads();
-        // exclusive scan of the bins*W counters (digit-major, warp-minor); bins*W/THREADS = bins/32 per thread
-        {
-          const int per = bins / 32;
-          const int at = tid * per;
-          uint32_t loc[8], sum = 0;
-#pragma unroll
-          for (int k = 0; k < 8; ++k) {
-            loc[k] = k < per ? (uint32_t)s_cnt[at + k] : 0u;
-            sum += loc[k];
-          }
-          uint32_t incl = sum;
-#pragma unroll
-          for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += t;
-          }
-          if (lane == 31) s_wtot[64 + wid] = incl;
-          __syncthreads();
-          unsigned excl_w, tot;
-          warp_totals_scan<W>(s_wtot + 64, excl_w, tot);
-          uint32_t run = excl_w + incl - sum;
-#pragma unroll
-          for (int k = 0; k < 8; ++k) {
-            if (k < per) s_cnt[at + k] = (uint16_t)run;
-            run += loc[k];
-          }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int r = 0; r < R_MAX; ++r) {
-          if (r * 32 < ipw) {
-            const int pos = wid * ipw + r * 32 + lane;
-            if (pos < m) {
-              const uint32_t d = (kreg[r] >> shift) & dmask;
-              const uint32_t rank = (uint32_t)s_cnt[d * W + wid] + (ireg[r] >> 16);
-              dep_key[rank] = kreg[r];
-              dep_idx[rank] = (uint16_t)(ireg[r] & 0xffffu);
-            }
-          }
-        }
-        __syncthreads();
-      }
-    }
-
-    // ------------------------------------------------------------------ chain T (tracks)
+    // ------------------------------------------------------------------ chain T (one warp) beside pass B
     if (wid == 0) {
       const unsigned long long ex = chain_lookback(prm.chain, tile, (unsigned long long)n_trk);
       if (lane == 0) s_misc[1] = ex;
     } else if (wid == 1) {
-      event_scan(s_ntrk, ne);
+      if (multi) event_scan(s_ntrk, ne);
+      else if (lane == 0) s_ntrk[0] = 0, s_ntrk[1] = n_trk;
+    }
+    // pass B (S5): every deposit finds its tower's slot and pushes itself on the slot's list
+    for (int i = tid; i < n; i += THREADS) {
+      const uint32_t r = s_res[i];
+      if (r & RES_DEP) {
+        const int id = (int)(r & RES_TOWER);
+        const int g = (multi ? (int)s_ev[i] * gpe : 0) + (id >> 7);
+        const int slot = (int)s_gp[g] + popc_below(((const uint4 *)s_bitmap)[g], id & 127);
+        const unsigned prev = atomicExch(&s_head[slot], (unsigned)i);
+        s_res[i] = (r & ~(LINK_END << RES_LINK_SHIFT)) | ((prev & LINK_END) << RES_LINK_SHIFT);
+      }
     }
     __syncthreads();
     const long long base_trk = (long long)s_misc[1];
 
-    // ------------------------------------------------------------------ P2: S3 on the accepted tracks (converged),
-    // written straight to the track collection
+    // ------------------------------------------------------------------ pass T: S3 on the accepted tracks
+    // (converged: one thread per track), written straight to the track collection
     for (int s = tid; s < n_trk; s += THREADS) {
-      const int i = tk_i[s];
+      const int i = s_tk[s];
       const long long src = p0 + i, g = base_trk + s;
       const int pid = __ldg(prm.pid + src);
       const float px = __ldg(prm.px + src), py = __ldg(prm.py + src), pz = __ldg(prm.pz + src);
-      const int e = find_event(s_off32, ne, i);
+      const int e = multi ? (int)s_ev[i] : 0;
       TrackOut t;
       track_smear(sc, px, py, pz, prm.seed, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), t);
-      dep_T[i] = t.E_trk;
+      const float u = s_uT[i];
+      s_uT[i] = t.E_trk;  // from here on: the track energy that pass W subtracts
       prm.trk_src[g] = (int)src;
       prm.trk_pid[g] = pid;
       prm.trk_charge[g] = __ldg(prm.charge + src);
@@ -455,100 +431,109 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       prm.trk_eta[g] = t.eta_mom;
       prm.trk_phi[g] = t.phi0;
       prm.trk_E[g] = t.E_trk;
-      prm.trk_eta_out[g] = eta_from_u(sc, p_u[i]);
-      prm.trk_phi_out[g] = p_phi[i];
+      prm.trk_eta_out[g] = eta_from_u(sc, u);
+      prm.trk_phi_out[g] = s_phi[i];
       if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[src] = t.pt_s;
     }
     for (int e = tid; e < ne; e += THREADS) prm.trk_offsets[e0 + e + 1] = base_trk + s_ntrk[e + 1];
     if (tile == 0 && tid == 0) prm.trk_offsets[0] = 0, prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
-    __syncthreads();  // view A of the union region is dead from here on
+    __syncthreads();
 
-    // ------------------------------------------------------------------ phase 2b-1: run heads, in order
-    int dt_base = 0;
-    for (int it = 0; it * THREADS < m; ++it) {
-      const int pos = it * THREADS + tid;
-      bool head = false;
-      if (pos < m) {
-        const uint32_t kk = dep_key[pos] & KEY_MASK;
-        const uint32_t prev = pos > 0 ? (dep_key[pos - 1] & KEY_MASK) : 0xffffffffu;
-        head = kk != prev;
+    // ------------------------------------------------------------------ pass W: S5-S7, one thread per tower
+    for (int it = 0; it * THREADS < n_slots; ++it) {
+      const int d = it * THREADS + tid;
+      bool f_tw = false, f_ph = false, f_nh = false;
+      if (d < n_slots) {
+        const int h = (int)(s_head[d] & LINK_END);
+        const uint32_t rh = s_res[h];
+        const int tower = (int)(rh & RES_TOWER);
+        const int e = multi ? (int)s_ev[h] : 0;
+        float Eem = 0.f, Ehad = 0.f, Tem = 0.f, Thad = 0.f;
+        int first = h;
+        if ((rh >> RES_LINK_SHIFT) == LINK_END) {
+          const float Ev = s_Ev[h], Tv = (rh & RES_ACC) ? s_uT[h] : 0.f;
+          if (rh & RES_HCAL) Ehad = Ev, Thad = Tv;
+          else Eem = Ev, Tem = Tv;
+        } else {
+          // several deposits: add them in ascending particle index (the list is in arrival order)
+          int last = -1;
+          first = -1;
+          for (;;) {
+            int best = 0x7fffffff;
+            uint32_t rbest = 0;
+            for (int c = h; c != (int)LINK_END;) {
+              const uint32_t rc = s_res[c];
+              if (c > last && c < best) best = c, rbest = rc;
+              c = (int)(rc >> RES_LINK_SHIFT);
+            }
+            if (best == 0x7fffffff) break;
+            if (first < 0) first = best;
+            const float Ev = s_Ev[best], Tv = (rbest & RES_ACC) ? s_uT[best] : 0.f;
+            if (rbest & RES_HCAL) Ehad += Ev, Thad += Tv;
+            else Eem += Ev, Tem += Tv;
+            last = best;
+          }
+        }
+        uint32_t rn[4];
+        rng_block(prm.seed, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
+        float em_s, had_s;
+        tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
+        // reading A22: the threshold is applied twice, strictly, per component
+        const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
+        const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
+        const float n_em = em_f - Tem, n_had = had_f - Thad;
+        f_ph = n_em > sc.thr_ecal, f_nh = n_had > sc.thr_hcal;
+        f_tw = em_f + had_f > 0.f;
+        if (multi) {
+          if (f_tw) atomicAdd(&s_ntow[e], 1);
+          if (f_ph) atomicAdd(&s_nph[e], 1);
+          if (f_nh) atomicAdd(&s_nnh[e], 1);
+        }
+        // stage the tower at its head particle's index (only this thread ever touches that particle again)
+        s_phi[h] = em_f, s_Ev[h] = had_f, s_uT[h] = f_ph ? n_em : 0.f;
+        s_res[h] = __float_as_uint(f_nh ? n_had : 0.f);
+        s_head[d] = (unsigned)h | ((unsigned)tower << 13);
+        if (DEBUG) {
+          const long long g = p0 + first;
+          if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 1;
+          if (prm.dbg_tw[0]) prm.dbg_tw[0][g] = Eem;
+          if (prm.dbg_tw[1]) prm.dbg_tw[1][g] = Ehad;
+          if (prm.dbg_tw[2]) prm.dbg_tw[2][g] = Tem;
+          if (prm.dbg_tw[3]) prm.dbg_tw[3][g] = Thad;
+          if (prm.dbg_tw[4]) prm.dbg_tw[4][g] = em_s;
+          if (prm.dbg_tw[5]) prm.dbg_tw[5][g] = had_s;
+          if (prm.dbg_tw_dec)
+            prm.dbg_tw_dec[g] = (unsigned char)((k_em ? PD_DEC_EEM : 0) | (k_had ? PD_DEC_EHAD : 0) |
+                                                (f_ph ? PD_DEC_NEM : 0) | (f_nh ? PD_DEC_NHAD : 0));
+        }
       }
-      const unsigned hm = __ballot_sync(0xffffffffu, head);
-      if (lane == 0) s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(hm);
-      __syncthreads();
-      unsigned excl_w, tot;
-      warp_totals_scan<W>(s_wtot + (it & 1) * 32, excl_w, tot);
-      if (head) st_key[dt_base + (int)excl_w + __popc(hm & lt_mask)] = (uint32_t)pos;
-      dt_base += (int)tot;
-    }
-    const int n_dt = dt_base;
-    __syncthreads();
-
-    // ------------------------------------------------------------------ phase 2b-2: S5-S7, one thread per tower
-    for (int d = tid; d < n_dt; d += THREADS) {
-      const int pos = (int)st_key[d];
-      const uint32_t kk = dep_key[pos] & KEY_MASK;
-      float Eem = 0.f, Ehad = 0.f, Tem = 0.f, Thad = 0.f;
-      int qpos = pos;
-      do {  // sequential sum in particle order (the sort is stable)
-        const uint32_t kq = dep_key[qpos];
-        if ((kq & KEY_MASK) != kk) break;
-        const int pi = dep_idx[qpos];
-        const float Ev = dep_E[pi], Tv = dep_T[pi];
-        if (kq >> 31) Ehad += Ev, Thad += Tv;
-        else Eem += Ev, Tem += Tv;
-        ++qpos;
-      } while (qpos < m);
-      const uint32_t code = kk & code_mask;
-      const int e = (int)(kk >> EV_SHIFT);
-      const int tower = s_offset[code >> JB] + (int)(code & j_mask);
-      uint32_t rn[4];
-      rng_block(prm.seed, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
-      float em_s, had_s;
-      tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
-      // reading A22: the threshold is applied twice, strictly, per component
-      const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
-      const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
-      const float n_em = em_f - Tem, n_had = had_f - Thad;
-      const bool is_ph = n_em > sc.thr_ecal, is_nh = n_had > sc.thr_hcal;
-      if (em_f + had_f > 0.f) atomicAdd(&s_ntow[e], 1);
-      if (is_ph) atomicAdd(&s_nph[e], 1);
-      if (is_nh) atomicAdd(&s_nnh[e], 1);
-      st_key[d] = kk;
-      st_em[d] = em_f, st_had[d] = had_f, st_nem[d] = is_ph ? n_em : 0.f, st_nhad[d] = is_nh ? n_had : 0.f;
-      if (DEBUG) {
-        const long long g = p0 + dep_idx[pos];
-        if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 1;
-        if (prm.dbg_tw[0]) prm.dbg_tw[0][g] = Eem;
-        if (prm.dbg_tw[1]) prm.dbg_tw[1][g] = Ehad;
-        if (prm.dbg_tw[2]) prm.dbg_tw[2][g] = Tem;
-        if (prm.dbg_tw[3]) prm.dbg_tw[3][g] = Thad;
-        if (prm.dbg_tw[4]) prm.dbg_tw[4][g] = em_s;
-        if (prm.dbg_tw[5]) prm.dbg_tw[5][g] = had_s;
-        if (prm.dbg_tw_dec)
-          prm.dbg_tw_dec[g] = (unsigned char)((k_em ? PD_DEC_EEM : 0) | (k_had ? PD_DEC_EHAD : 0) |
-                                              (is_ph ? PD_DEC_NEM : 0) | (is_nh ? PD_DEC_NHAD : 0));
+      const unsigned m_tw = __ballot_sync(0xffffffffu, f_tw), m_ph = __ballot_sync(0xffffffffu, f_ph),
+                     m_nh = __ballot_sync(0xffffffffu, f_nh);
+      if (lane == 0) {
+        if (m_tw | m_ph) atomicAdd(&s_tot[0], (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 16));
+        if (m_nh) atomicAdd(&s_tot[1], (unsigned)__popc(m_nh));
       }
     }
     __syncthreads();
 
-    // ------------------------------------------------------------------ chain W (towers, eflow)
-    if (wid == 0) event_scan(s_ntow, ne);
-    else if (wid == 1) event_scan(s_nph, ne);
-    else if (wid == 2) event_scan(s_nnh, ne);
-    __syncthreads();
+    // ------------------------------------------------------------------ chain W (towers | neutrals)
+    const int n_tow = (int)(s_tot[0] & 0xffffu), n_ph = (int)(s_tot[0] >> 16), n_nh = (int)s_tot[1];
     if (wid == 0) {
-      const unsigned long long ex = chain_lookback(prm.chain + prm.n_tiles, tile, (unsigned long long)s_ntow[ne]);
+      const unsigned long long agg = (unsigned long long)n_tow | ((unsigned long long)(n_ph + n_nh) << 31);
+      const unsigned long long ex = chain_lookback(prm.chain + prm.n_tiles, tile, agg);
       if (lane == 0) s_misc[2] = ex;
-    } else if (wid == 1) {
-      const unsigned long long agg = (unsigned long long)n_trk + (unsigned long long)s_nph[ne] + (unsigned long long)s_nnh[ne];
-      const unsigned long long ex = chain_lookback(prm.chain + 2 * (size_t)prm.n_tiles, tile, agg);
-      if (lane == 0) s_misc[3] = ex;
+    } else if (multi) {
+      if (wid == 1) event_scan(s_ntow, ne);
+      else if (wid == 2) event_scan(s_nph, ne);
+      else if (wid == 3) event_scan(s_nnh, ne);
+    } else if (tid == 32) {
+      s_ntow[0] = 0, s_ntow[1] = n_tow, s_nph[0] = 0, s_nph[1] = n_ph, s_nnh[0] = 0, s_nnh[1] = n_nh;
     }
     __syncthreads();
-    const long long base_tow = (long long)s_misc[2], base_efl = (long long)s_misc[3];
+    const long long base_tow = (long long)(s_misc[2] & FIELD_MASK);
+    const long long base_efl = base_trk + (long long)((s_misc[2] >> 31) & FIELD_MASK);
 
-    // ------------------------------------------------------------------ phase 3: ordered outputs
+    // ------------------------------------------------------------------ pass O: ordered outputs
     for (int e = tid; e < ne; e += THREADS) {
       prm.tow_offsets[e0 + e + 1] = base_tow + s_ntow[e + 1];
       prm.efl_offsets[e0 + e + 1] = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + s_nnh[e + 1];
@@ -557,7 +542,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
     for (int s = tid; s < n_trk; s += THREADS) {
       const long long g = base_trk + s;
       const int src = __ldcg(prm.trk_src + g);
-      const int e = find_event(s_off32, ne, (int)(src - p0));
+      const int e = multi ? (int)s_ev[(int)((long long)src - p0)] : 0;
       const long long at = base_efl + s + s_nph[e] + s_nnh[e];
       const int pid = __ldcg(prm.trk_pid + g);
       const int apid = pid < 0 ? -pid : pid;
@@ -569,14 +554,15 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       prm.efl_E[at] = __ldcg(prm.trk_E + g);
     }
     int tw_run = 0, ph_run = 0, nh_run = 0;
-    for (int it = 0; it * THREADS < n_dt; ++it) {
+    for (int it = 0; it * THREADS < n_slots; ++it) {
       const int d = it * THREADS + tid;
       bool f_tw = false, f_ph = false, f_nh = false;
-      uint32_t kk = 0;
+      int h = 0, tower = 0;
       float em = 0.f, had = 0.f, nem = 0.f, nhad = 0.f;
-      if (d < n_dt) {
-        kk = st_key[d];
-        em = st_em[d], had = st_had[d], nem = st_nem[d], nhad = st_nhad[d];
+      if (d < n_slots) {
+        const unsigned hv = s_head[d];
+        h = (int)(hv & LINK_END), tower = (int)(hv >> 13);
+        em = s_phi[h], had = s_Ev[h], nem = s_uT[h], nhad = __uint_as_float(s_res[h]);
         f_tw = em + had > 0.f;
         f_ph = nem > 0.f;
         f_nh = nhad > 0.f;
@@ -585,17 +571,17 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
                      m_nh = __ballot_sync(0xffffffffu, f_nh);
       if (lane == 0) {
         s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 16);
-        s_wtot[96 + (it & 1) * 32 + wid] = (unsigned)__popc(m_nh);
+        s_wtot[64 + (it & 1) * 32 + wid] = (unsigned)__popc(m_nh);
       }
       __syncthreads();
       unsigned excl_w, tot, excl_n, tot_n;
       warp_totals_scan<W>(s_wtot + (it & 1) * 32, excl_w, tot);
-      warp_totals_scan<W>(s_wtot + 96 + (it & 1) * 32, excl_n, tot_n);
+      warp_totals_scan<W>(s_wtot + 64 + (it & 1) * 32, excl_n, tot_n);
       if (f_tw || f_ph || f_nh) {
-        const uint32_t code = kk & code_mask;
-        const int e = (int)(kk >> EV_SHIFT);
-        const int b = (int)(code >> JB), j = (int)(code & j_mask);
-        const int tower = s_offset[b] + j;
+        const int e = multi ? (int)s_ev[h] : 0;
+        int b = (int)s_binlut[tower >> 5];
+        while (tower >= s_offset[b + 1]) ++b;
+        const int j = tower - s_offset[b];
         const float eta_c = s_eta_c[b];
         const float phi_c = fmaf((float)j + 0.5f, s_w[b], -kPiF);
         const float ic = s_inv_cosh[b];
@@ -653,54 +639,60 @@ static int query_device() {
   return PD_OK;
 }
 
-// Tile plan from sizes the host knows (n_events, n_particles): G events per tile so that an average
-// tile fills ~85% of the on-chip capacity C.  Small events -> 256-thread CTAs, two per SM;
-// large events -> one 512-thread CTA per SM with the whole shared memory.
+// Tile plan from sizes the host knows (n_events, n_particles).  B200: 228 KB of shared memory per SM, 1 KB
+// reserved per CTA, 227 KB per CTA at most.  Preferred shape: two 512-thread CTAs per SM (113 KB each), so one
+// CTA's barriers and look-back waits are covered by the other; events too large for that get one 1024-thread CTA
+// with the whole SM.  G = events per tile: as many as fit the on-chip capacity C with ~4 sigma of head-room
+// for a Poisson-like sum, but no more than keeps every CTA slot of the GPU busy on small inputs.
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan) {
-  const int nb = c->sc.n_bins;
-  const size_t smem_sm = 227 * 1024;  // B200: 227 KB per CTA (opt-in), 228 KB per SM
+  const PdCardScalars &sc = c->sc;
   const double avg = n_events > 0 ? double(n_particles) / double(n_events) : 0.0;
-  auto cap_for = [&](int threads, size_t budget) {
-    const size_t fixed = pdk::make_layout(nb, threads, 0).total;
-    long cap = budget > fixed + 64 ? long((budget - fixed - 64) / 34) : 0;
-    cap = cap > long(threads) * pdk::r_max(threads) ? long(threads) * pdk::r_max(threads) : cap;
-    cap = cap > 65535 ? 65535 : cap;
-    return int(cap);
+  const size_t budget2 = (228 * 1024 - 2 * 1024) / 2, budget1 = 227 * 1024;
+  auto cap_for = [&](int G, size_t budget) {
+    const size_t fixed = pdk::make_layout(sc.n_bins, 2 * sc.lut_side, sc.n_towers, sc.words_per_event, G, 0).total;
+    const size_t per = 22 + (G > 1 ? 1 : 0);
+    long cap = budget > fixed + 7 * 16 ? long((budget - fixed - 7 * 16) / per) : 0;
+    cap &= ~3L;
+    return int(cap > pdk::C_MAX ? pdk::C_MAX : cap);
   };
-  const int c_small = cap_for(256, (228 * 1024 - 2 * 1024) / 2);
-  static const int large_threads = std::getenv("PD_LARGE_THREADS") ? std::atoi(std::getenv("PD_LARGE_THREADS")) : 1024;
-  const int c_large = cap_for(large_threads, smem_sm);
-  const bool small = avg * 1.3 + 64.0 <= double(c_small) * 0.5;
-  plan->threads = small ? 256 : large_threads;
-  plan->capacity = small ? c_small : c_large;
-  long g = 1;
-  if (avg > 0.0) {
-    // leave head-room of ~4 sigma of a Poisson-like sum
-    const double target = double(plan->capacity) - 4.0 * std::sqrt(double(plan->capacity)) - 2.0 * avg;
-    g = long(target / avg);
-  } else {
-    g = pdk::G_MAX;
+  auto fits = [&](int G, size_t budget) {
+    const double C = cap_for(G, budget);
+    return double(G) * avg + 4.0 * std::sqrt(double(G) * avg + 1.0) + 16.0 <= C;
+  };
+  static const int force_threads = std::getenv("PD_THREADS") ? std::atoi(std::getenv("PD_THREADS")) : 0;
+  size_t budget = budget2;
+  plan->threads = 512;
+  if (force_threads == 1024 || (force_threads == 0 && !fits(1, budget2))) {
+    budget = budget1;
+    plan->threads = 1024;
   }
-  g = g < 1 ? 1 : (g > pdk::G_MAX ? pdk::G_MAX : g);
-  plan->events_per_tile = int(g);
+  int g = 1;
+  while (g < pdk::G_MAX && fits(g + 1, budget)) ++g;
+  // keep all CTA slots busy: aim for >= 4 tiles per resident CTA when the input is small
+  const long slots = 148L * (plan->threads == 512 ? 2 : 1);
+  const long g_bal = long((n_events + 4 * slots - 1) / (4 * slots));
+  if (g > g_bal) g = int(g_bal < 1 ? 1 : g_bal);
+  plan->events_per_tile = g;
+  plan->capacity = cap_for(g, budget);
   plan->n_tiles = int((n_events + g - 1) / g);
-  int eb = 0;
-  while ((1 << eb) < g) ++eb;
-  plan->event_bits = eb;
-  plan->smem_bytes = pdk::make_layout(nb, plan->threads, plan->capacity).total;
-  plan->grid = 0;
+  plan->smem_bytes = pdk::make_layout(sc.n_bins, 2 * sc.lut_side, sc.n_towers, sc.words_per_event, g, plan->capacity).total;
   return PD_OK;
 }
 
 template <int THREADS, bool DEBUG>
 static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
-  auto kern = pdk::pd_chain_kernel<THREADS, (THREADS == 256 ? 2 : 1), DEBUG>;
+  constexpr int CTAS = THREADS == 512 ? 2 : 1;
+  auto kern = pdk::pd_chain_kernel<THREADS, CTAS, DEBUG>;
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g_max_smem_optin) != cudaSuccess) return PD_ECUDA;
     configured = true;
   }
-  const int per_sm = THREADS == 256 ? 2 : 1;
+  // persistent CTAs wait on one another through the look-back chains: the grid must be co-resident
+  int per_sm = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, THREADS, plan.smem_bytes) != cudaSuccess) return PD_ECUDA;
+  if (per_sm < 1) return PD_ECUDA;
+  if (per_sm > CTAS) per_sm = CTAS;
   int grid = g_num_sms * per_sm;
   if (grid > plan.n_tiles) grid = plan.n_tiles;
   if (grid < 1) grid = 1;
@@ -712,7 +704,6 @@ int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, v
   if (query_device() != PD_OK) return PD_ECUDA;
   if (plan.smem_bytes > (size_t)g_max_smem_optin) return PD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
-  if (plan.threads == 256) return debug ? launch_variant<256, true>(prm, plan, st) : launch_variant<256, false>(prm, plan, st);
   if (plan.threads == 1024) return debug ? launch_variant<1024, true>(prm, plan, st) : launch_variant<1024, false>(prm, plan, st);
   return debug ? launch_variant<512, true>(prm, plan, st) : launch_variant<512, false>(prm, plan, st);
 }

@@ -1,6 +1,11 @@
 // pd_math.cuh -- per-particle and per-tower arithmetic of the chain (device only, fp32 with a few fp64
 // operations where SURVEY.md 7.2-1 shows fp32 cannot hold the 1e-6 band).  Product code; written from
-// DESIGN.md readings, shares nothing with oracle/.
+// the DESIGN.md readings, shares nothing with oracle/.
+//
+// v3: the instruction count per particle is the binding resource, so the math is
+// written for few issue slots: MUFU reciprocals / rsqrt, one polynomial atan2, no binary searches
+// (eta bin through a float-bits lookup table, efficiency through a cell grid built at card load), and
+// the barrel/endcap decision without an arctangent.
 #pragma once
 
 #include <cstdint>
@@ -10,13 +15,16 @@
 namespace pdk {
 
 constexpr float kPiF = 3.14159265358979323846f;
+constexpr float kHalfPiF = 1.57079632679489661923f;
 constexpr float kTwoM24 = 5.9604644775390625e-08f;  // 2^-24
+constexpr float kInfF = __builtin_huge_valf();
 
 // Card tables staged in shared memory (pointers into the CTA's dynamic shared memory).
 struct SmCard {
   const float *tb;
   const int *nphi, *offset;
   const float *inv_w, *half, *w, *eta_c, *inv_cosh;
+  const unsigned short *lut;
 };
 
 // ---- S-RNG: Philox4x32-10 (Salmon et al., SC'11), reading A26: key = (seed lo, seed hi),
@@ -25,12 +33,12 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
                                               uint32_t k1, uint32_t (&out)[4]) {
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-    c0 = hi1 ^ c1 ^ k0;
-    c1 = lo1;
-    c2 = hi0 ^ c3 ^ k1;
-    c3 = lo0;
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;  // one IMAD.WIDE each
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    c1 = (uint32_t)p1;
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c3 = (uint32_t)p0;
     k0 += 0x9E3779B9u;
     k1 += 0xBB67AE85u;
   }
@@ -46,18 +54,55 @@ __device__ __forceinline__ void rng_block(unsigned long long seed, long long eve
 // u in [0,1) on the 2^-24 lattice (exact in fp32)
 __device__ __forceinline__ float uniform24(uint32_t x) { return (float)(x >> 8) * kTwoM24; }
 
+__device__ __forceinline__ float fast_rcp(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float fast_rsqrt(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float fast_sqrt(float x) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// atan2(y, x) in (-pi, pi]: octant reduction + odd minimax polynomial (|error| < 7e-8 on [0,1] in
+// fp32 Horner form, coefficients fitted for t + t s Q(s), s = t^2) + fix-ups.  atan2(0, 0) = 0.
+__device__ __forceinline__ float fast_atan2(float y, float x) {
+  const float ax = fabsf(x), ay = fabsf(y);
+  const float mx = fmaxf(ax, ay), mn = fminf(ax, ay);
+  const float t = mn * fast_rcp(fmaxf(mx, 1e-37f));
+  const float s = t * t;
+  float q = 2.622228581e-03f;
+  q = fmaf(q, s, -1.513247099e-02f);
+  q = fmaf(q, s, 4.112175107e-02f);
+  q = fmaf(q, s, -7.366696745e-02f);
+  q = fmaf(q, s, 1.057392731e-01f);
+  q = fmaf(q, s, -1.418597400e-01f);
+  q = fmaf(q, s, 1.999039650e-01f);
+  q = fmaf(q, s, -3.333298564e-01f);
+  float r = fmaf(t * s, q, t);
+  r = ay > ax ? kHalfPiF - r : r;
+  r = x < 0.f ? kPiF - r : r;
+  return copysignf(r, y);
+}
+
 // Box-Muller, cosine branch: z = sqrt(-2 ln u+) cos(2 pi u), u+ = ((xa>>8)+1) 2^-24, u = (xb>>8) 2^-24
 __device__ __forceinline__ float normal_bm(uint32_t xa, uint32_t xb) {
   const float up = (float)((xa >> 8) + 1u) * kTwoM24;   // exact
   const float u2 = (float)(xb >> 8) * (2.0f * kTwoM24);  // 2u, exact
-  return sqrtf(-2.0f * logf(up)) * cospif(u2);
+  return fast_sqrt(-2.0f * logf(up)) * cospif(u2);
 }
 
 // log-normal with mean m and relative standard deviation^2 rel2 = (s/m)^2 (reading A21):
 // m exp(-b2/2 + b z), b2 = ln(1 + rel2).  Caller guarantees m > 0, rel2 > 0.
 __device__ __forceinline__ float lognormal_rel(float m, float rel2, float z) {
   const float b2 = log1pf(rel2);
-  return m * expf(fmaf(sqrtf(b2), z, -0.5f * b2));
+  return m * __expf(fmaf(fast_sqrt(b2), z, -0.5f * b2));
 }
 
 // calorimeter component: E' = LN(E, sigma(E)), sigma^2 = C2 E^2 + S2 E + N2
@@ -65,33 +110,21 @@ __device__ __forceinline__ float smear_component(float E, const float (&csn2)[3]
   if (!(E > 0.f)) return 0.f;
   const float s2 = fmaf(csn2[0] * E, E, fmaf(csn2[1], E, csn2[2]));
   if (!(s2 > 0.f)) return E;
-  return lognormal_rel(E, s2 / (E * E), normal_bm(xa, xb));
+  const float iE = fast_rcp(E);
+  return lognormal_rel(E, s2 * iE * iE, normal_bm(xa, xb));
 }
 
-// ---- S1..S4 for one particle -------------------------------------------------------------------
-struct ParticleOut {
-  uint32_t status;  // PD_DROPPED / PD_BARREL / PD_ENDCAP | PD_LOOPER
-  int bin, j;       // eta/theta bin and phi bin of the hit; bin = -1: outside the grid
-  int eps_row;      // -1 none
-  bool accepted;
-  float u, phi_pos;  // hit: u = z/r (or -z/r for a theta grid), azimuth
-};
-
-// smeared track quantities (S3), computed in a separate, converged pass over the accepted tracks
-struct TrackOut {
-  float pt_s, eta_mom, phi0, E_trk;
-};
-
-// bin i with tb[i] <= u < tb[i+1], -1 if outside or NaN
-__device__ __forceinline__ int grid_bin(const SmCard &cd, int nb, float u) {
+// bin i with tb[i] <= u < tb[i+1], -1 if outside or NaN.  The lookup table gives the bin that holds
+// the lower bound of u's cell; the forward steps make the result exact for any monotone edge list.
+__device__ __forceinline__ int grid_bin(const SmCard &cd, const PdCardScalars &sc, float u) {
+  const int nb = sc.n_bins;
   if (!(u >= cd.tb[0]) || !(u < cd.tb[nb])) return -1;
-  int lo = 0, hi = nb;
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (u >= cd.tb[mid]) lo = mid;
-    else hi = mid;
-  }
-  return lo;
+  int ca = (__float_as_int(fabsf(u)) >> PD_LUT_SHIFT) - sc.lut_base;
+  ca = min(max(ca, 0), sc.lut_side - 1);
+  const int cell = u < 0.f ? sc.lut_side - 1 - ca : sc.lut_side + ca;
+  int b = cd.lut[cell];
+  while (u >= cd.tb[b + 1]) ++b;  // terminates: u < tb[nb]
+  return b;
 }
 
 __device__ __forceinline__ int phi_bin(const SmCard &cd, int i, float phi) {
@@ -101,12 +134,44 @@ __device__ __forceinline__ int phi_bin(const SmCard &cd, int i, float phi) {
   return j > n - 1 ? n - 1 : j;
 }
 
-__device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const SmCard &cd, int pid, int q, float px,
-                                               float py, float pz, float vx, float vy, float vz,
-                                               unsigned long long seed, long long event, uint32_t pidx,
-                                               ParticleOut &o) {
+// eta of a hit from u (only tracks and debug need it as a number)
+__device__ __forceinline__ float eta_from_u(const PdCardScalars &sc, float u) { return asinhf(sc.grid_theta ? -u : u); }
+
+// ---- S1..S4 for one particle -------------------------------------------------------------------
+struct ParticleOut {
+  uint32_t status;   // PD_DROPPED / PD_BARREL / PD_ENDCAP | PD_LOOPER
+  int tower;         // tower id of the hit, -1: outside the grid or dropped
+  int eps_row;       // row of the card's efficiency table, -1 none
+  bool accepted;
+  float u, phi_pos;  // hit: u = z/r (or -z/r for a theta grid), azimuth
+};
+
+// Rare path: a helix grazing the barrel (within a few % of the looper threshold).  The crossing angle
+// amplifies the rounding of rho by 1/sqrt(distance to tangency), so the quadratic is redone in double.
+__device__ __noinline__ bool graze_double(const PdCardScalars &sc, float px, float py, float vx, float vy, float aq,
+                                          float s, float &cc, float &ss) {
+  const double pxd = px, pyd = py, vxd = vx, vyd = vy, Rd = sc.R;
+  const double ptd = sqrt(pxd * pxd + pyd * pyd);
+  const double rhod = ptd / (sc.kB_d * (double)aq);
+  const double ipt = 1.0 / ptd;
+  const double ad = (vxd * pxd + vyd * pyd) * ipt;
+  const double bd = (double)s * (vyd * pxd - vxd * pyd) * ipt;
+  const double Dd = Rd * Rd - (vxd * vxd + vyd * vyd);
+  const double Pd = 2.0 * rhod * ad;
+  const double Qd = 4.0 * rhod * (rhod + bd) - Dd;
+  const double dd = Pd * Pd + Qd * Dd;
+  if (!(dd >= 0.0)) return false;
+  const double Sd = sqrt(dd);
+  if (Pd >= 0.0) cc = (float)(Pd + Sd), ss = (float)Dd;
+  else cc = (float)Qd, ss = (float)(Sd - Pd);
+  return true;
+}
+
+__device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const SmCard &cd, int q, float px, float py,
+                                               float pz, float vx, float vy, float vz, unsigned long long seed,
+                                               long long event, uint32_t pidx, ParticleOut &o) {
   o.status = PD_DROPPED;
-  o.bin = -1, o.j = 0;
+  o.tower = -1;
   o.eps_row = -1;
   o.accepted = false;
   o.u = __int_as_float(0x7fc00000);
@@ -116,34 +181,32 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
   const float r02 = fmaf(vx, vx, vy * vy);
   // readings A4, A5: born on/outside the cylinder, or no transverse momentum -> dropped
   if (r02 >= sc.R2 || fabsf(vz) >= sc.L || pt2 < 1e-9f) return;
-  const float pt = sqrtf(pt2);
+  const float ipt = fast_rsqrt(pt2);
+  const float pt = pt2 * ipt;
+  const float apz = fabsf(pz);
   const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
-  const float D = sc.R2 - r02;  // > 0
-  float x, y, z, r;
-  uint32_t face, looper = 0;
+  const float zdist = sc.L - sgnz * vz;  // distance to the endcap the particle flies towards (> 0)
+  const float D = sc.R2 - r02;           // > 0
+  float x, y, z;
+  bool endcap;
+  uint32_t looper = 0;
 
   if (q == 0 || sc.sB == 0.f) {
-    // straight line to r = R or |z| = L, whichever comes first
+    // straight line to r = R or |z| = L, whichever comes first: t_R = num / den, t_Z = zdist / |pz|
     const float b = fmaf(vx, px, vy * py);
-    const float sq = sqrtf(fmaf(b, b, pt2 * D));
-    const float tR = b > 0.f ? D / (b + sq) : (sq - b) / pt2;
-    const float tZ = pz != 0.f ? (sgnz * sc.L - vz) / pz : __int_as_float(0x7f800000);
-    if (tZ < tR) {
-      x = fmaf(tZ, px, vx), y = fmaf(tZ, py, vy), z = sgnz * sc.L;
-      r = sqrtf(fmaf(x, x, y * y));
-      face = PD_ENDCAP;
-    } else {
-      x = fmaf(tR, px, vx), y = fmaf(tR, py, vy), z = fmaf(tR, pz, vz);
-      r = sc.R;
-      face = PD_BARREL;
-    }
+    const float sq = fast_sqrt(fmaf(b, b, pt2 * D));
+    const float num = b > 0.f ? D : sq - b;
+    const float den = b > 0.f ? b + sq : pt2;
+    endcap = apz > 0.f && zdist * den < num * apz;
+    const float t = endcap ? zdist * fast_rcp(apz) : num * fast_rcp(den);
+    x = fmaf(t, px, vx), y = fmaf(t, py, vy);
+    z = endcap ? sgnz * sc.L : fmaf(t, pz, vz);
   } else {
     // helix of radius rho; momentum azimuth phi0 + s alpha (reading A3: q > 0 in +z field turns clockwise)
     const float aq = fabsf((float)q);
-    const float kq = sc.kB * aq;
-    const float rho = pt / kq;
+    const float rho = aq == 1.f ? pt * sc.inv_kB : pt * sc.inv_kB * fast_rcp(aq);
     const float s = ((q > 0) == (sc.sB > 0.f)) ? -1.f : 1.f;
-    const float c0 = px / pt, s0 = py / pt;
+    const float c0 = px * ipt, s0 = py * ipt;
     // vertex in the (u0, s n0) frame: a = v.u0, b = s v.n0
     const float a_ = fmaf(vx, c0, vy * s0);
     const float b_ = s * fmaf(vy, c0, -vx * s0);
@@ -153,101 +216,79 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
     const float disc = fmaf(P, P, Q * D);
     const float scale = fmaf(P, P, 4.f * rho * rho * D);
     bool reach;
-    float cc = 1.f, ss = 0.f;
+    float cc = 1.f, ss = 0.f;  // (cos, sin) of the barrel half-angle h_R, unnormalised, ss >= 0
     if (disc >= 0.f ? disc < 0.08f * scale : -disc < 1e-3f * scale) {
-      // grazing the barrel (within a few % of the looper threshold): the crossing angle amplifies the
-      // rounding of rho by 1/sqrt(distance to tangency), so this rare case is redone in double
-      const double pxd = px, pyd = py, vxd = vx, vyd = vy, Rd = sc.R;
-      const double ptd = sqrt(pxd * pxd + pyd * pyd);
-      const double rhod = ptd / (sc.kB_d * (double)aq);
-      const double ipt = 1.0 / ptd;
-      const double ad = (vxd * pxd + vyd * pyd) * ipt;
-      const double bd = (double)s * (vyd * pxd - vxd * pyd) * ipt;
-      const double Dd = Rd * Rd - (vxd * vxd + vyd * vyd);
-      const double Pd = 2.0 * rhod * ad;
-      const double Qd = 4.0 * rhod * (rhod + bd) - Dd;
-      const double dd = Pd * Pd + Qd * Dd;
-      reach = dd >= 0.0;
-      if (reach) {
-        const double Sd = sqrt(dd);
-        if (Pd >= 0.0) cc = (float)(Pd + Sd), ss = (float)Dd;
-        else cc = (float)Qd, ss = (float)(Sd - Pd);
-      }
+      reach = graze_double(sc, px, py, vx, vy, aq, s, cc, ss);
     } else {
       reach = disc >= 0.f;
-      if (reach) {
-        const float S = sqrtf(disc);
-        // first crossing: (cos h, sin h) proportional to (P + S, D) if P >= 0 else (Q, S - P)
-        if (P >= 0.f) cc = P + S, ss = D;
-        else cc = Q, ss = S - P;
-      }
+      const float S = fast_sqrt(fmaxf(disc, 0.f));
+      // first crossing: (cos h, sin h) proportional to (P + S, D) if P >= 0 else (Q, S - P)
+      cc = P >= 0.f ? P + S : Q;
+      ss = P >= 0.f ? D : S - P;
     }
-    float sh = 0.f, ch = 1.f, hR = 0.f;
-    float aR = __int_as_float(0x7f800000), aZ = aR;
-    if (reach) {
-      const float inv = 1.0f / sqrtf(fmaf(cc, cc, ss * ss));
-      ch = cc * inv, sh = ss * inv;
-      hR = atan2f(ss, cc);
-      aR = 2.f * hR;
-    } else {
-      looper = PD_LOOPER;
-    }
-    double hz = 0.0;
-    if (pz != 0.f) {
-      // alpha_Z / 2 in double: the turning angle of a looper can be ~1e5 rad
-      hz = 0.5 * ((double)sc.L - (double)(sgnz * vz)) * (sc.kB_d * (double)aq) / (double)fabsf(pz);
-      aZ = (float)(2.0 * hz);
-    }
-    if (!reach && pz == 0.f) {
+    if (!reach) looper = PD_LOOPER;
+    if (!reach && apz == 0.f) {
       o.status = PD_DROPPED | looper;  // trapped (reading A6)
       return;
     }
-    if (aZ < aR) {
-      // reduce h modulo pi in double: the chord formulas are pi-periodic in h
-      double f = hz * 0.31830988618379067154;
-      f -= rint(f);
-      sincospif((float)f, &sh, &ch);
-      z = sgnz * sc.L;
-      face = PD_ENDCAP;
-    } else {
-      z = fmaf(aR, pz / kq, vz);
-      face = PD_BARREL;
+    // endcap half-angle h_Z = zdist kappa |q| B / (2 |pz|), as f = h_Z / pi in double: the turning angle of a
+    // looper can be ~1e5 rad.  1/|pz| = MUFU seed + one Newton step in double.
+    float sh = 0.f, ch = 1.f;
+    endcap = false;
+    if (apz > 0.f) {
+      const double pzd = (double)apz;
+      const double r0 = (double)fast_rcp(apz);
+      const double r1 = fma(r0, fma(-pzd, r0, 1.0), r0);
+      const double zd = (double)sc.L - (double)(sgnz * vz);
+      const double fd = zd * (sc.kB_d * (0.5 * 0.31830988618379067154) * (double)aq) * r1;
+      const double nd = (fd + 6755399441055744.0) - 6755399441055744.0;  // rint
+      const float frac = (float)(fd - nd);                                // in [-0.5, 0.5]
+      const float ff = (float)fd;
+      sincospif(frac, &sh, &ch);  // (sin, cos)(h_Z) up to a common sign (-1)^n
+      // h_Z < h_R  <=>  h_Z < pi and sin(h_R - h_Z) > 0   (both half-angles lie in (0, pi))
+      const float cross = fmaf(ss, ch, -cc * sh);
+      endcap = !reach || (ff < 1.f && (frac < 0.f ? -cross : cross) > 0.f);
     }
+    if (endcap) {
+      z = sgnz * sc.L;
+    } else {
+      const float inv = fast_rsqrt(fmaf(cc, cc, ss * ss));
+      ch = cc * inv, sh = ss * inv;
+      const float hR = fast_atan2(ss, cc);
+      z = fmaf(2.f * hR, pz * sc.inv_kB * (aq == 1.f ? 1.f : fast_rcp(aq)), vz);
+    }
+    // chord form (pi-periodic in h): position = v + 2 rho sin h u(phi0 + s h)
     const float l2 = 2.f * rho * sh;
     x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
     y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
-    r = face == PD_BARREL ? sc.R : sqrtf(fmaf(x, x, y * y));
   }
-  o.status = face | looper;
-  const float u = sc.grid_theta ? -z / r : z / r;
-  const float phi_pos = atan2f(y, x);
+  o.status = (endcap ? PD_ENDCAP : PD_BARREL) | looper;
+  const float ir = endcap ? fast_rsqrt(fmaf(x, x, y * y)) : sc.inv_R;
+  const float u = (sc.grid_theta ? -z : z) * ir;
+  const float phi_pos = fast_atan2(y, x);
   o.u = u;
   o.phi_pos = phi_pos;
 
-  // S2/S3 track: efficiency at the true vertex momentum (A7); accept iff u24 < eps (A11)
+  // S2 track: efficiency cell at the true vertex momentum (A7); accept iff u24 < eps (A11)
   if (q != 0) {
-    const float T = fabsf(pz) / pt;  // sinh |eta_mom|
-    float eps = 0.f;
-    int row = -1;
-    if (!(sc.has_cos && T >= sc.t_cos)) {
-      for (int k = 0; k < sc.n_eff; ++k) {
-        const float lo = sc.eff[k][0], hi = sc.eff[k][1];
-        bool above_lo = pt > lo, below_hi = pt <= hi;
-        if (fabsf(pt - lo) <= 2e-6f * lo || fabsf(pt - hi) <= 2e-6f * hi) {
-          // pT within rounding of a table edge (e.g. a generator floor at exactly 0.1 GeV): decide on
-          // pT^2 in double, where px^2 + py^2 is (almost) exact
-          const double p2 = (double)px * (double)px + (double)py * (double)py;
-          above_lo = p2 > (double)lo * (double)lo;
-          below_hi = p2 <= (double)hi * (double)hi;
-        }
-        if (above_lo && below_hi && (sc.eff[k][2] <= 0.f || T >= sc.eff[k][2]) && T < sc.eff[k][3]) {
-          row = k;
-          eps = sc.eff[k][4];
-          break;
-        }
-      }
+    int ip = 0, it = 0;
+    bool near = false;
+    for (int k = 0; k < sc.n_pt; ++k) {
+      const float e2 = sc.pt_edge2[k];
+      ip += pt2 > e2 ? 1 : 0;
+      near = near || fabsf(pt2 - e2) <= 4e-6f * e2;
     }
-    o.eps_row = row;
+    if (near) {
+      // pT within rounding of a table edge (e.g. a generator floor at exactly 0.1 GeV): decide on pT^2 in
+      // double, where px^2 + py^2 is (almost) exact
+      const double p2 = (double)px * (double)px + (double)py * (double)py;
+      ip = 0;
+      for (int k = 0; k < sc.n_pt; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
+    }
+    for (int k = 0; k < sc.n_T; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
+    const int cell = ip * (sc.n_T + 1) + it;
+    const float eps = sc.cell_eps[cell];
+    o.eps_row = sc.cell_row[cell];
     if (eps > 0.f) {
       uint32_t rn[4];
       rng_block(seed, event, pidx, 0u, rn);
@@ -256,25 +297,29 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
   }
 
   // S4 tower of the hit
-  const int i = grid_bin(cd, sc.n_bins, u);
-  o.bin = i;
-  if (i >= 0) o.j = phi_bin(cd, i, phi_pos);
+  const int i = grid_bin(cd, sc, u);
+  if (i >= 0) o.tower = cd.offset[i] + phi_bin(cd, i, phi_pos);
 }
 
 // S3 for one accepted track (A12/A13): log-normal with mean pT and std sigma_rel pT, driven by words
 // 1 and 2 of the particle's Philox block; eta, phi unchanged; E = pT' cosh(eta) = pT' |p| / pT.
+struct TrackOut {
+  float pt_s, eta_mom, phi0, E_trk;
+};
+
 __device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, float py, float pz,
                                             unsigned long long seed, long long event, uint32_t pidx, TrackOut &t) {
   const float pt2 = fmaf(px, px, py * py);
-  const float pt = sqrtf(pt2);
+  const float ipt = fast_rsqrt(pt2);
+  const float pt = pt2 * ipt;
   uint32_t rn[4];
   rng_block(seed, event, pidx, 0u, rn);
   const float bp = sc.trk_b * pt;
   const float rel2 = fmaf(bp, bp, sc.trk_a2);
   t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(rn[1], rn[2])) : pt;
-  t.E_trk = t.pt_s * (sqrtf(fmaf(pz, pz, pt2)) / pt);
-  t.eta_mom = asinhf(pz / pt);
-  t.phi0 = atan2f(py, px);
+  t.E_trk = t.pt_s * (fast_sqrt(fmaf(pz, pz, pt2)) * ipt);
+  t.eta_mom = asinhf(pz * ipt);
+  t.phi0 = fast_atan2(py, px);
 }
 
 // per-tower smear of both components (S6): the common case of a single non-zero component runs one
@@ -289,14 +334,12 @@ __device__ __forceinline__ void tower_smear(const PdCardScalars &sc, float Eem, 
   float sp = 0.f;
   if (Ep > 0.f) {
     const float v = fmaf(c2 * Ep, Ep, fmaf(s2c, Ep, n2));
-    sp = v > 0.f ? lognormal_rel(Ep, v / (Ep * Ep), normal_bm(xa, xb)) : Ep;
+    const float iE = fast_rcp(Ep);
+    sp = v > 0.f ? lognormal_rel(Ep, v * iE * iE, normal_bm(xa, xb)) : Ep;
   }
   em_s = prim_em ? sp : 0.f;
   had_s = prim_em ? 0.f : sp;
   if (prim_em && Ehad > 0.f) had_s = smear_component(Ehad, sc.hcal2, rn[2], rn[3]);
 }
-
-// eta of a hit from u (only tracks and debug need it as a number)
-__device__ __forceinline__ float eta_from_u(const PdCardScalars &sc, float u) { return asinhf(sc.grid_theta ? -u : u); }
 
 }  // namespace pdk
