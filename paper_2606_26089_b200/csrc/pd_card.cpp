@@ -226,11 +226,10 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     std::sort(te.begin(), te.end());
     if (pte.size() > size_t(PD_MAX_EFF_EDGES) || te.size() > size_t(PD_MAX_EFF_EDGES)) return PD_ECARD;
     s.n_pt = int(pte.size()), s.n_T = int(te.size());
-    for (int k = 0; k < s.n_pt; ++k) {
-      s.pt_edge2_d[k] = pte[size_t(k)] * pte[size_t(k)];
-      s.pt_edge2[k] = float(s.pt_edge2_d[k]);
+    for (int k = 0; k < PD_MAX_EFF_EDGES; ++k) {
+      s.pt_edge2_d[k] = k < s.n_pt ? pte[size_t(k)] * pte[size_t(k)] : std::numeric_limits<double>::max();
+      s.T_edge[k] = k < s.n_T ? float(te[size_t(k)]) : std::numeric_limits<float>::infinity();
     }
-    for (int k = 0; k < s.n_T; ++k) s.T_edge[k] = float(te[size_t(k)]);
     for (int ip = 0; ip <= s.n_pt; ++ip) {
       // representative pT of the interval (e[ip-1], e[ip]]: its closed upper end, or beyond the last edge
       const double pt_rep = ip < s.n_pt ? pte[size_t(ip)] : (s.n_pt ? 2.0 * pte.back() + 1.0 : 1.0);

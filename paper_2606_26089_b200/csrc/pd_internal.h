@@ -30,9 +30,8 @@ struct PdCardScalars {
   // efficiency table resolved into a grid at load (reading A8: first matching row wins):
   // cell = (#pT edges with pT > e) * (n_T + 1) + (#T edges with |pz|/pT >= t)
   int n_pt, n_T;
-  float pt_edge2[PD_MAX_EFF_EDGES];   // e^2 (fp32) for the fast test
-  double pt_edge2_d[PD_MAX_EFF_EDGES];  // e^2 in double for pT within rounding of an edge
-  float T_edge[PD_MAX_EFF_EDGES];     // sinh |eta| edges (incl. the |cos theta| cut)
+  double pt_edge2_d[PD_MAX_EFF_EDGES];  // e^2 in double; unused entries are DBL_MAX
+  float T_edge[PD_MAX_EFF_EDGES];       // sinh |eta| edges (incl. the |cos theta| cut); unused entries +inf
   float cell_eps[PD_MAX_EFF_CELLS];
   signed char cell_row[PD_MAX_EFF_CELLS];  // row of the card's table, -1 none
   float trk_a2, trk_b;       // sigma_rel^2 = a^2 + (b pT)^2

@@ -10,14 +10,14 @@
 //   pass B   S5         every deposit pushes itself on its slot's list (one integer atomicExch)
 //   chain T             decoupled look-back over tiles -> global track offset (overlaps pass B)
 //   pass T   S3         one thread per accepted track: pT smear, track record written to HBM
-//   pass W   S5-S7      one thread per occupied tower: sum of its list IN PARTICLE ORDER (fp32, sequential),
+//   pass W   S5-S7      one thread per occupied tower: exact fixed-point sum of its list (order-independent),
 //                       Philox tower stream, log-normal smear, thresholds, EFlow subtraction
 //   chain W             look-back for the tower and neutral offsets (one packed 64-bit word)
 //   pass O   S8         ordered compaction of towers / photons / neutral hadrons, EFlow track entries,
 //                       CSR offsets
 // Nothing but the inputs and the final collections touches HBM.  Sums are order-stable: each tower's
-// deposits are added sequentially in ascending particle index whatever order the list was built in, and
-// the only atomics are integer (bitmap OR, list exchange, counters).
+// deposits are added as 64-bit fixed-point integers (exact, hence independent of the order in which the
+// list was built), and the only atomics are integer (bitmap OR, list exchange, counters).
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -189,13 +189,20 @@ struct ParticleIn {
   float px, py, pz, E, vx, vy, vz;
 };
 
-__device__ __forceinline__ ParticleIn load_particle(const PdParams &prm, long long g) {
+// input arrays rebased to the first particle of the tile (uniform pointers + a 32-bit particle index)
+struct TileIn {
+  const int *pid;
+  const signed char *charge;
+  const float *px, *py, *pz, *E, *vx, *vy, *vz;
+};
+
+__device__ __forceinline__ ParticleIn load_particle(const TileIn &t, unsigned i) {
   ParticleIn p;
-  p.pid = __ldg(prm.pid + g);
-  p.q = (int)__ldg(prm.charge + g);
-  p.px = __ldg(prm.px + g), p.py = __ldg(prm.py + g), p.pz = __ldg(prm.pz + g);
-  p.E = __ldg(prm.E + g);
-  p.vx = __ldg(prm.vx + g), p.vy = __ldg(prm.vy + g), p.vz = __ldg(prm.vz + g);
+  p.pid = __ldg(t.pid + i);
+  p.q = (int)__ldg(t.charge + i);
+  p.px = __ldg(t.px + i), p.py = __ldg(t.py + i), p.pz = __ldg(t.pz + i);
+  p.E = __ldg(t.E + i);
+  p.vx = __ldg(t.vx + i), p.vy = __ldg(t.vy + i), p.vz = __ldg(t.vz + i);
   return p;
 }
 
@@ -316,11 +323,13 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
 
     // ------------------------------------------------------------------ pass A: S0-S2, S4 per particle
     {
+      const TileIn tin{prm.pid + p0, prm.charge + p0, prm.px + p0, prm.py + p0, prm.pz + p0, prm.E + p0,
+                       prm.vx + p0, prm.vy + p0, prm.vz + p0};
       ParticleIn nxt;
-      if (tid < n) nxt = load_particle(prm, p0 + tid);
+      if (tid < n) nxt = load_particle(tin, (unsigned)tid);
       for (int i = tid; i < n; i += THREADS) {
         const ParticleIn c = nxt;
-        if (i + THREADS < n) nxt = load_particle(prm, p0 + i + THREADS);
+        if (i + THREADS < n) nxt = load_particle(tin, (unsigned)(i + THREADS));
         const int e = multi ? (int)s_ev[i] : 0;
         ParticleOut o;
         particle_chain(sc, cd, c.q, c.px, c.py, c.pz, c.vx, c.vy, c.vz, prm.seed, prm.event_base + e0 + e,
@@ -448,32 +457,23 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         const uint32_t rh = s_res[h];
         const int tower = (int)(rh & RES_TOWER);
         const int e = multi ? (int)s_ev[h] : 0;
-        float Eem = 0.f, Ehad = 0.f, Tem = 0.f, Thad = 0.f;
+        // S5: exact fixed-point sums (units of 2^-32 GeV, 64-bit integers) over the slot's list.  Integer
+        // addition is associative, so the sums do not depend on the order in which the deposits arrived:
+        // bitwise reproducible, and closer to the fp64 definition than a sequential fp32 sum.
+        long long a_em = 0, a_had = 0, t_em = 0, t_had = 0;
         int first = h;
-        if ((rh >> RES_LINK_SHIFT) == LINK_END) {
-          const float Ev = s_Ev[h], Tv = (rh & RES_ACC) ? s_uT[h] : 0.f;
-          if (rh & RES_HCAL) Ehad = Ev, Thad = Tv;
-          else Eem = Ev, Tem = Tv;
-        } else {
-          // several deposits: add them in ascending particle index (the list is in arrival order)
-          int last = -1;
-          first = -1;
-          for (;;) {
-            int best = 0x7fffffff;
-            uint32_t rbest = 0;
-            for (int c = h; c != (int)LINK_END;) {
-              const uint32_t rc = s_res[c];
-              if (c > last && c < best) best = c, rbest = rc;
-              c = (int)(rc >> RES_LINK_SHIFT);
-            }
-            if (best == 0x7fffffff) break;
-            if (first < 0) first = best;
-            const float Ev = s_Ev[best], Tv = (rbest & RES_ACC) ? s_uT[best] : 0.f;
-            if (rbest & RES_HCAL) Ehad += Ev, Thad += Tv;
-            else Eem += Ev, Tem += Tv;
-            last = best;
-          }
+        for (int c = h;;) {
+          const uint32_t rc = c == h ? rh : s_res[c];
+          const long long Ev = __float2ll_rn(s_Ev[c] * 4294967296.f);
+          const long long Tv = (rc & RES_ACC) ? __float2ll_rn(s_uT[c] * 4294967296.f) : 0ll;
+          if (rc & RES_HCAL) a_had += Ev, t_had += Tv;
+          else a_em += Ev, t_em += Tv;
+          first = min(first, c);
+          c = (int)(rc >> RES_LINK_SHIFT);
+          if (c == (int)LINK_END) break;
         }
+        const float Eem = (float)a_em * 2.3283064365386963e-10f, Ehad = (float)a_had * 2.3283064365386963e-10f;
+        const float Tem = (float)t_em * 2.3283064365386963e-10f, Thad = (float)t_had * 2.3283064365386963e-10f;
         uint32_t rn[4];
         rng_block(prm.seed, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
         float em_s, had_s;

@@ -91,6 +91,21 @@ __device__ __forceinline__ float fast_atan2(float y, float x) {
   return copysignf(r, y);
 }
 
+// (sin, cos)(pi x) for |x| <= 1/2: fold to [0, 1/4] and two short minimax polynomials (|error| < 3e-9
+// before rounding); sin takes the sign of x.
+__device__ __forceinline__ void sincospi_half(float x, float &sn, float &cs) {
+  const float ax = fabsf(x);
+  const bool hi = ax > 0.25f;
+  const float y = hi ? 0.5f - ax : ax;
+  const float t = y * y;
+  float sp = fmaf(fmaf(-5.888253450e-01f, t, 2.549749374e+00f), t, -5.167707920e+00f);
+  sp = fmaf(y * t, sp, kPiF * y);
+  float cp = fmaf(fmaf(fmaf(2.314294875e-01f, t, -1.335058451e+00f), t, 4.058707714e+00f), t, -4.934802055e+00f);
+  cp = fmaf(t, cp, 1.f);
+  sn = copysignf(hi ? cp : sp, x);
+  cs = hi ? sp : cp;
+}
+
 // Box-Muller, cosine branch: z = sqrt(-2 ln u+) cos(2 pi u), u+ = ((xa>>8)+1) 2^-24, u = (xb>>8) 2^-24
 __device__ __forceinline__ float normal_bm(uint32_t xa, uint32_t xb) {
   const float up = (float)((xa >> 8) + 1u) * kTwoM24;   // exact
@@ -244,7 +259,7 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
       const double nd = (fd + 6755399441055744.0) - 6755399441055744.0;  // rint
       const float frac = (float)(fd - nd);                                // in [-0.5, 0.5]
       const float ff = (float)fd;
-      sincospif(frac, &sh, &ch);  // (sin, cos)(h_Z) up to a common sign (-1)^n
+      sincospi_half(frac, sh, ch);  // (sin, cos)(h_Z) up to a common sign (-1)^n
       // h_Z < h_R  <=>  h_Z < pi and sin(h_R - h_Z) > 0   (both half-angles lie in (0, pi))
       const float cross = fmaf(ss, ch, -cc * sh);
       endcap = !reach || (ff < 1.f && (frac < 0.f ? -cross : cross) > 0.f);
@@ -271,21 +286,22 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
 
   // S2 track: efficiency cell at the true vertex momentum (A7); accept iff u24 < eps (A11)
   if (q != 0) {
+    // pT edges are compared on pT^2 in double (px^2 + py^2 is then exact to ~1e-16, so a generator floor at
+    // exactly an edge, e.g. pT = 0.1 GeV, is decided like the fp64 definition); unused edges are +max
+    const double p2 = (double)px * (double)px + (double)py * (double)py;
     int ip = 0, it = 0;
-    bool near = false;
-    for (int k = 0; k < sc.n_pt; ++k) {
-      const float e2 = sc.pt_edge2[k];
-      ip += pt2 > e2 ? 1 : 0;
-      near = near || fabsf(pt2 - e2) <= 4e-6f * e2;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
+    if (sc.n_pt > 4) {
+#pragma unroll
+      for (int k = 4; k < PD_MAX_EFF_EDGES; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
     }
-    if (near) {
-      // pT within rounding of a table edge (e.g. a generator floor at exactly 0.1 GeV): decide on pT^2 in
-      // double, where px^2 + py^2 is (almost) exact
-      const double p2 = (double)px * (double)px + (double)py * (double)py;
-      ip = 0;
-      for (int k = 0; k < sc.n_pt; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
+    if (sc.n_T > 4) {
+#pragma unroll
+      for (int k = 4; k < PD_MAX_EFF_EDGES; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
     }
-    for (int k = 0; k < sc.n_T; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
     const int cell = ip * (sc.n_T + 1) + it;
     const float eps = sc.cell_eps[cell];
     o.eps_row = sc.cell_row[cell];
