@@ -180,6 +180,10 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
   p.pid = ev->pid, p.charge = ev->charge;
   p.px = ev->px, p.py = ev->py, p.pz = ev->pz, p.E = ev->E, p.vx = ev->vx, p.vy = ev->vy, p.vz = ev->vz;
   p.seed = seed, p.event_base = event_base;
+  for (int r = 0; r < 10; ++r) {
+    p.rk.k0[r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+    p.rk.k1[r] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+  }
   p.trk_offsets = (long long *)trk->offsets;
   p.trk_src = trk->src, p.trk_pid = trk->pid, p.trk_charge = trk->charge;
   p.trk_pt = trk->pt, p.trk_eta = trk->eta, p.trk_phi = trk->phi, p.trk_E = trk->E;

@@ -68,6 +68,11 @@ struct pd_card {
   mutable PdCardTables dev_tab{};
 };
 
+// Philox4x32-10 round keys of the call's seed: (seed lo + r W0, seed hi + r W1), r = 0..9
+struct PdPhiloxKeys {
+  uint32_t k0[10], k1[10];
+};
+
 // Kernel parameters (passed by value).
 struct PdParams {
   PdCardScalars sc;
@@ -79,6 +84,7 @@ struct PdParams {
   const signed char *charge;
   const float *px, *py, *pz, *E, *vx, *vy, *vz;
   unsigned long long seed;
+  PdPhiloxKeys rk;
   long long event_base;
   // outputs
   long long *trk_offsets;

@@ -45,6 +45,7 @@ struct Layout {
   size_t tb, nphi, offset, inv_w, half, w, eta_c, inv_cosh, lut, binlut;  // card tables
   size_t off32, ntrk, ntow, nph, nnh;                                     // per-event arrays [G+1]
   size_t misc;                                                            // scratch words
+  size_t cnt;                                                             // pass W warp counts -> prefixes [2][256]
   size_t bitmap, gprefix;                                                 // per event: tower bits, group prefix
   size_t res, uT, phi, Ev, head, stg, ev;                                 // per particle / per slot
   size_t total;
@@ -75,6 +76,7 @@ __host__ __device__ inline Layout make_layout(int n_bins, int lut_cells, int n_t
   l.nph = take(4 * (G + 1));
   l.nnh = take(4 * (G + 1));
   l.misc = take(8 * 64);
+  l.cnt = take(4 * 2 * 256);
   l.bitmap = take(4 * (size_t)G * words_per_event);
   l.gprefix = take(2 * ((size_t)G * (words_per_event / 4) + 1));
   l.res = take(4 * (size_t)C);
@@ -119,9 +121,11 @@ __device__ unsigned long long chain_lookback(unsigned long long *st, int tile, u
     const int idx = pos - lane;
     unsigned long long v = FLAG_P;  // before the first tile: prefix 0
     if (idx >= 0) {
-      do {
+      v = ld_relaxed(st + idx);
+      while ((v >> 62) == 0) {
+        __nanosleep(40);
         v = ld_relaxed(st + idx);
-      } while ((v >> 62) == 0);
+      }
     }
     const unsigned pm = __ballot_sync(0xffffffffu, (v >> 62) == 2);
     if (pm) {
@@ -245,8 +249,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
   int *s_nph = (int *)(smem + L.nph);
   int *s_nnh = (int *)(smem + L.nnh);
   unsigned long long *s_misc = (unsigned long long *)(smem + L.misc);
-  unsigned *s_tot = (unsigned *)(s_misc + 4);    // [0] towers | photons << 16, [1] neutral hadrons
-  unsigned *s_wtot = (unsigned *)(s_misc + 8);   // [3][32] per-warp totals
+  unsigned *s_wtot = (unsigned *)(s_misc + 8);   // [32] per-warp totals of scan 1
+  unsigned *s_preA = (unsigned *)(smem + L.cnt);  // per (iteration, warp) of pass W: towers | photons << 16 ...
+  unsigned *s_preB = s_preA + 256;                // ... and neutral hadrons (counts, then exclusive prefixes)
   uint32_t *s_bitmap = (uint32_t *)(smem + L.bitmap);
   unsigned short *s_gp = (unsigned short *)(smem + L.gprefix);
   uint32_t *s_res = (uint32_t *)(smem + L.res);
@@ -289,10 +294,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
 
   for (;;) {
     __syncthreads();  // previous tile fully done with shared memory (and card tables staged)
-    if (tid == 0) {
-      s_misc[0] = atomicAdd(prm.tile_counter, 1u);
-      s_tot[0] = 0u, s_tot[1] = 0u;
-    }
+    if (tid == 0) s_misc[0] = atomicAdd(prm.tile_counter, 1u);
     __syncthreads();
     const int tile = (int)s_misc[0];
     if (tile >= prm.n_tiles) break;
@@ -332,7 +334,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         if (i + THREADS < n) nxt = load_particle(tin, (unsigned)(i + THREADS));
         const int e = multi ? (int)s_ev[i] : 0;
         ParticleOut o;
-        particle_chain(sc, cd, c.q, c.px, c.py, c.pz, c.vx, c.vy, c.vz, prm.seed, prm.event_base + e0 + e,
+        particle_chain(sc, cd, c.q, c.px, c.py, c.pz, c.vx, c.vy, c.vz, prm.rk, prm.event_base + e0 + e,
                        (uint32_t)(i - s_off32[e]), o);
         const int apid = c.pid < 0 ? -c.pid : c.pid;
         const bool to_ecal = apid == 11 || apid == 22;                             // reading A18
@@ -430,7 +432,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       const float px = __ldg(prm.px + src), py = __ldg(prm.py + src), pz = __ldg(prm.pz + src);
       const int e = multi ? (int)s_ev[i] : 0;
       TrackOut t;
-      track_smear(sc, px, py, pz, prm.seed, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), t);
+      track_smear(sc, px, py, pz, prm.rk, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), t);
       const float u = s_uT[i];
       s_uT[i] = t.E_trk;  // from here on: the track energy that pass W subtracts
       prm.trk_src[g] = (int)src;
@@ -449,7 +451,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
     __syncthreads();
 
     // ------------------------------------------------------------------ pass W: S5-S7, one thread per tower
-    for (int it = 0; it * THREADS < n_slots; ++it) {
+    const int n_it = (n_slots + THREADS - 1) / THREADS;  // <= C_MAX / THREADS + 1, so n_it * W <= 256
+    for (int it = 0; it < n_it; ++it) {
       const int d = it * THREADS + tid;
       bool f_tw = false, f_ph = false, f_nh = false;
       if (d < n_slots) {
@@ -475,7 +478,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         const float Eem = (float)a_em * 2.3283064365386963e-10f, Ehad = (float)a_had * 2.3283064365386963e-10f;
         const float Tem = (float)t_em * 2.3283064365386963e-10f, Thad = (float)t_had * 2.3283064365386963e-10f;
         uint32_t rn[4];
-        rng_block(prm.seed, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
+        rng_block(prm.rk, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
         float em_s, had_s;
         tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
         // reading A22: the threshold is applied twice, strictly, per component
@@ -507,18 +510,39 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
                                                 (f_ph ? PD_DEC_NEM : 0) | (f_nh ? PD_DEC_NHAD : 0));
         }
       }
+      // counts of this warp's 32 slots; scanned over all (iteration, warp) pairs below = slot order
       const unsigned m_tw = __ballot_sync(0xffffffffu, f_tw), m_ph = __ballot_sync(0xffffffffu, f_ph),
                      m_nh = __ballot_sync(0xffffffffu, f_nh);
       if (lane == 0) {
-        if (m_tw | m_ph) atomicAdd(&s_tot[0], (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 16));
-        if (m_nh) atomicAdd(&s_tot[1], (unsigned)__popc(m_nh));
+        s_preA[it * W + wid] = (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 16);
+        s_preB[it * W + wid] = (unsigned)__popc(m_nh);
       }
     }
     __syncthreads();
 
-    // ------------------------------------------------------------------ chain W (towers | neutrals)
-    const int n_tow = (int)(s_tot[0] & 0xffffu), n_ph = (int)(s_tot[0] >> 16), n_nh = (int)s_tot[1];
+    // ------------------------------------------------------------------ scan W + chain W (towers | neutrals)
     if (wid == 0) {
+      // exclusive prefix over the <= 256 (iteration, warp) counts: eight consecutive entries per lane
+      const int n_ent = n_it * W;
+      unsigned va[8], vb[8], sa = 0, sb = 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int idx = lane * 8 + k;
+        va[k] = idx < n_ent ? s_preA[idx] : 0u;
+        vb[k] = idx < n_ent ? s_preB[idx] : 0u;
+        sa += va[k], sb += vb[k];
+      }
+      const unsigned ia = warp_incl_scan(sa), ib = warp_incl_scan(sb);
+      const unsigned ta = __shfl_sync(0xffffffffu, ia, 31), tb = __shfl_sync(0xffffffffu, ib, 31);
+      unsigned ra = ia - sa, rb = ib - sb;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int idx = lane * 8 + k;
+        if (idx < n_ent) s_preA[idx] = ra, s_preB[idx] = rb;
+        ra += va[k], rb += vb[k];
+      }
+      const int n_tow = (int)(ta & 0xffffu), n_ph = (int)(ta >> 16), n_nh = (int)tb;
+      if (!multi && lane == 0) s_ntow[0] = 0, s_ntow[1] = n_tow, s_nph[0] = 0, s_nph[1] = n_ph, s_nnh[0] = 0, s_nnh[1] = n_nh;
       const unsigned long long agg = (unsigned long long)n_tow | ((unsigned long long)(n_ph + n_nh) << 31);
       const unsigned long long ex = chain_lookback(prm.chain + prm.n_tiles, tile, agg);
       if (lane == 0) s_misc[2] = ex;
@@ -526,8 +550,6 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       if (wid == 1) event_scan(s_ntow, ne);
       else if (wid == 2) event_scan(s_nph, ne);
       else if (wid == 3) event_scan(s_nnh, ne);
-    } else if (tid == 32) {
-      s_ntow[0] = 0, s_ntow[1] = n_tow, s_nph[0] = 0, s_nph[1] = n_ph, s_nnh[0] = 0, s_nnh[1] = n_nh;
     }
     __syncthreads();
     const long long base_tow = (long long)(s_misc[2] & FIELD_MASK);
@@ -553,8 +575,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       prm.efl_phi[at] = __ldcg(prm.trk_phi + g);
       prm.efl_E[at] = __ldcg(prm.trk_E + g);
     }
-    int tw_run = 0, ph_run = 0, nh_run = 0;
-    for (int it = 0; it * THREADS < n_slots; ++it) {
+    for (int it = 0; it < n_it; ++it) {
       const int d = it * THREADS + tid;
       bool f_tw = false, f_ph = false, f_nh = false;
       int h = 0, tower = 0;
@@ -569,15 +590,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       }
       const unsigned m_tw = __ballot_sync(0xffffffffu, f_tw), m_ph = __ballot_sync(0xffffffffu, f_ph),
                      m_nh = __ballot_sync(0xffffffffu, f_nh);
-      if (lane == 0) {
-        s_wtot[(it & 1) * 32 + wid] = (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 16);
-        s_wtot[64 + (it & 1) * 32 + wid] = (unsigned)__popc(m_nh);
-      }
-      __syncthreads();
-      unsigned excl_w, tot, excl_n, tot_n;
-      warp_totals_scan<W>(s_wtot + (it & 1) * 32, excl_w, tot);
-      warp_totals_scan<W>(s_wtot + 64 + (it & 1) * 32, excl_n, tot_n);
       if (f_tw || f_ph || f_nh) {
+        const unsigned pa = s_preA[it * W + wid], pb = s_preB[it * W + wid];
         const int e = multi ? (int)s_ev[h] : 0;
         int b = (int)s_binlut[tower >> 5];
         while (tower >= s_offset[b + 1]) ++b;
@@ -586,7 +600,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         const float phi_c = fmaf((float)j + 0.5f, s_w[b], -kPiF);
         const float ic = s_inv_cosh[b];
         if (f_tw) {
-          const long long at = base_tow + tw_run + (int)(excl_w & 0xffffu) + __popc(m_tw & lt_mask);
+          const long long at = base_tow + (int)(pa & 0xffffu) + __popc(m_tw & lt_mask);
           prm.tow_tower[at] = tower;
           prm.tow_eta[at] = eta_c;
           prm.tow_phi[at] = phi_c;
@@ -596,7 +610,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
           prm.tow_ET[at] = (em + had) * ic;
         }
         if (f_ph) {
-          const int slot = ph_run + (int)(excl_w >> 16) + __popc(m_ph & lt_mask);
+          const int slot = (int)(pa >> 16) + __popc(m_ph & lt_mask);
           const long long at = base_efl + s_ntrk[e + 1] + s_nnh[e] + slot;
           prm.efl_cls[at] = (signed char)PD_CLS_PHOTON;
           prm.efl_src[at] = tower;
@@ -606,7 +620,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
           prm.efl_E[at] = nem;
         }
         if (f_nh) {
-          const int slot = nh_run + (int)excl_n + __popc(m_nh & lt_mask);
+          const int slot = (int)pb + __popc(m_nh & lt_mask);
           const long long at = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + slot;
           prm.efl_cls[at] = (signed char)PD_CLS_NEUHAD;
           prm.efl_src[at] = tower;
@@ -616,9 +630,6 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
           prm.efl_E[at] = nhad;
         }
       }
-      tw_run += (int)(tot & 0xffffu);
-      ph_run += (int)(tot >> 16);
-      nh_run += (int)tot_n;
     }
   }
 }

@@ -29,26 +29,28 @@ struct SmCard {
 
 // ---- S-RNG: Philox4x32-10 (Salmon et al., SC'11), reading A26: key = (seed lo, seed hi),
 // counter = (object, event lo, event hi, stream << 16) -----------------------------------------
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
-                                              uint32_t k1, uint32_t (&out)[4]) {
+// The ten round keys (k0 + r W0, k1 + r W1) are computed once on the host (PdParams::rk): in the kernel
+// they are constant-bank operands of the XORs, so a block costs 20 wide multiplies and 20 three-input XORs.
+using PhiloxKeys = PdPhiloxKeys;
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxKeys &rk,
+                                              uint32_t (&out)[4]) {
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
     const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;  // one IMAD.WIDE each
     const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
-    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk.k0[r];
     c1 = (uint32_t)p1;
-    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk.k1[r];
     c3 = (uint32_t)p0;
-    k0 += 0x9E3779B9u;
-    k1 += 0xBB67AE85u;
   }
   out[0] = c0, out[1] = c1, out[2] = c2, out[3] = c3;
 }
 
-__device__ __forceinline__ void rng_block(unsigned long long seed, long long event, uint32_t object, uint32_t stream,
+__device__ __forceinline__ void rng_block(const PhiloxKeys &rk, long long event, uint32_t object, uint32_t stream,
                                           uint32_t (&out)[4]) {
   const unsigned long long ev = (unsigned long long)event;
-  philox4x32_10(object, (uint32_t)ev, (uint32_t)(ev >> 32), stream << 16, (uint32_t)seed, (uint32_t)(seed >> 32), out);
+  philox4x32_10(object, (uint32_t)ev, (uint32_t)(ev >> 32), stream << 16, rk, out);
 }
 
 // u in [0,1) on the 2^-24 lattice (exact in fp32)
@@ -106,18 +108,77 @@ __device__ __forceinline__ void sincospi_half(float x, float &sn, float &cs) {
   cs = hi ? sp : cp;
 }
 
+__device__ __forceinline__ float fast_lg2(float x) {
+  float r;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float fast_ex2(float x) {
+  float r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// -ln(x) for a normal x in (0, 1] to ~2e-7 relative (also next to x = 1, where lg2.approx is only good to an
+// absolute 2^-22): x = m 2^e with m in [sqrt(1/2), sqrt(2)), ln m = f - f^2/2 + f^3 R(f), f = m - 1.
+__device__ __forceinline__ float neg_ln01(float x) {
+  const int ix = __float_as_int(x);
+  const int e = (ix - 0x3f3504f3) >> 23;
+  const float f = __int_as_float(ix - (e << 23)) - 1.0f;
+  float r = 8.917524944e-02f;
+  r = fmaf(r, f, -1.435014855e-01f);
+  r = fmaf(r, f, 1.487704477e-01f);
+  r = fmaf(r, f, -1.656564099e-01f);
+  r = fmaf(r, f, 1.996539170e-01f);
+  r = fmaf(r, f, -2.500174683e-01f);
+  r = fmaf(r, f, 3.333385820e-01f);
+  const float f2 = f * f;
+  const float lnm = fmaf(f2, fmaf(f, r, -0.5f), f);
+  return -fmaf((float)e, 0.693147180559945f, lnm);
+}
+
+// cos(pi v) for v in [0, 2]: fold to [0, 1/2] and one even polynomial (|error| < 3e-10 before rounding)
+__device__ __forceinline__ float cospi_02(float v) {
+  const float a = fabsf(v - 1.0f);        // cos(pi v) = -cos(pi a), a in [0, 1]
+  const bool flip = a > 0.5f;
+  const float b = flip ? 1.0f - a : a;    // cos(pi a) = flip ? -cos(pi b) : cos(pi b)
+  const float t = b * b;
+  float c = -2.439671581e-02f;
+  c = fmaf(c, t, 2.349375585e-01f);
+  c = fmaf(c, t, -1.335212057e+00f);
+  c = fmaf(c, t, 4.058709164e+00f);
+  c = fmaf(c, t, -4.934802137e+00f);
+  c = fmaf(c, t, 1.0f);
+  return flip ? c : -c;
+}
+
 // Box-Muller, cosine branch: z = sqrt(-2 ln u+) cos(2 pi u), u+ = ((xa>>8)+1) 2^-24, u = (xb>>8) 2^-24
 __device__ __forceinline__ float normal_bm(uint32_t xa, uint32_t xb) {
   const float up = (float)((xa >> 8) + 1u) * kTwoM24;   // exact
   const float u2 = (float)(xb >> 8) * (2.0f * kTwoM24);  // 2u, exact
-  return fast_sqrt(-2.0f * logf(up)) * cospif(u2);
+  return fast_sqrt(2.0f * neg_ln01(up)) * cospi_02(u2);
 }
 
 // log-normal with mean m and relative standard deviation^2 rel2 = (s/m)^2 (reading A21):
-// m exp(-b2/2 + b z), b2 = ln(1 + rel2).  Caller guarantees m > 0, rel2 > 0.
+// m exp(-b2/2 + b z), b2 = ln(1 + rel2), i.e. m (1 + rel2)^(-1/2) exp(b z).  Caller guarantees m > 0, rel2 > 0.
+// ln(1 + x): for x < 1/2 the series 2 s (1 + t Q(t)), s = x / (2 + x), t = s^2 (relative error ~1e-8, so that
+// b = sqrt(b2) keeps its relative accuracy for the small x of the track smear); lg2.approx above.
 __device__ __forceinline__ float lognormal_rel(float m, float rel2, float z) {
-  const float b2 = log1pf(rel2);
-  return m * __expf(fmaf(fast_sqrt(b2), z, -0.5f * b2));
+  const float y = 1.0f + rel2;
+  const float s = rel2 * fast_rcp(2.0f + rel2);
+  const float t = s * s;
+  const float q = fmaf(fmaf(1.497972671e-01f, t, 1.998943251e-01f), t, 3.333335706e-01f);
+  const float s2 = s + s;
+  const float b2 = rel2 < 0.5f ? fmaf(s2 * t, q, s2) : 0.693147180559945f * fast_lg2(y);
+  const float b = fast_sqrt(b2);
+  return m * fast_rsqrt(y) * fast_ex2(1.4426950408889634f * b * z);
+}
+
+// asinh(x) to ~2e-7 absolute / relative (outputs only: eta of a track, eta of its calorimeter hit)
+__device__ __forceinline__ float fast_asinh(float x) {
+  const float ax = fabsf(x);
+  const float y = ax + fast_sqrt(fmaf(ax, ax, 1.0f));
+  return copysignf(0.693147180559945f * fast_lg2(y), x);
 }
 
 // calorimeter component: E' = LN(E, sigma(E)), sigma^2 = C2 E^2 + S2 E + N2
@@ -150,7 +211,7 @@ __device__ __forceinline__ int phi_bin(const SmCard &cd, int i, float phi) {
 }
 
 // eta of a hit from u (only tracks and debug need it as a number)
-__device__ __forceinline__ float eta_from_u(const PdCardScalars &sc, float u) { return asinhf(sc.grid_theta ? -u : u); }
+__device__ __forceinline__ float eta_from_u(const PdCardScalars &sc, float u) { return fast_asinh(sc.grid_theta ? -u : u); }
 
 // ---- S1..S4 for one particle -------------------------------------------------------------------
 struct ParticleOut {
@@ -183,7 +244,7 @@ __device__ __noinline__ bool graze_double(const PdCardScalars &sc, float px, flo
 }
 
 __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const SmCard &cd, int q, float px, float py,
-                                               float pz, float vx, float vy, float vz, unsigned long long seed,
+                                               float pz, float vx, float vy, float vz, const PhiloxKeys &seed,
                                                long long event, uint32_t pidx, ParticleOut &o) {
   o.status = PD_DROPPED;
   o.tower = -1;
@@ -324,7 +385,7 @@ struct TrackOut {
 };
 
 __device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, float py, float pz,
-                                            unsigned long long seed, long long event, uint32_t pidx, TrackOut &t) {
+                                            const PhiloxKeys &seed, long long event, uint32_t pidx, TrackOut &t) {
   const float pt2 = fmaf(px, px, py * py);
   const float ipt = fast_rsqrt(pt2);
   const float pt = pt2 * ipt;
@@ -334,7 +395,7 @@ __device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, f
   const float rel2 = fmaf(bp, bp, sc.trk_a2);
   t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(rn[1], rn[2])) : pt;
   t.E_trk = t.pt_s * (fast_sqrt(fmaf(pz, pz, pt2)) * ipt);
-  t.eta_mom = asinhf(pz * ipt);
+  t.eta_mom = fast_asinh(pz * ipt);
   t.phi0 = fast_atan2(py, px);
 }
 
