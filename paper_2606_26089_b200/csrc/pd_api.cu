@@ -31,6 +31,12 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 }  // namespace
 
+// header + look-back words, rounded up so that the ring behind them is 256-byte aligned
+static size_t ws_chain_bytes(const PdLaunchPlan &plan) {
+  const size_t b = kWsHeader + 2 * sizeof(unsigned long long) * (size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1);
+  return (b + 255) & ~size_t(255);
+}
+
 extern "C" {
 
 const char *pd_strerror(int code) {
@@ -81,7 +87,7 @@ int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_part
   if (!card || n_events < 0 || n_particles < 0) return PD_EINVAL;
   PdLaunchPlan plan;
   pd_plan(card, n_events, n_particles, &plan);
-  return (int64_t)(kWsHeader + 2 * sizeof(unsigned long long) * (size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1));
+  return (int64_t)(ws_chain_bytes(plan) + sizeof(float) * 6 * (size_t)plan.max_ctas * (size_t)plan.capacity);
 }
 
 int pd_last_launch_count(void) { return t_launches; }
@@ -158,7 +164,9 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
   if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15u)) return PD_EWORKSPACE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
 
-  PD_CUDA(cudaMemsetAsync(workspace, 0, (size_t)need, st));
+  PdLaunchPlan plan;
+  pd_plan(card, ev->n_events, n, &plan);
+  PD_CUDA(cudaMemsetAsync(workspace, 0, ws_chain_bytes(plan), st));  // counters + look-back words; the ring needs no init
   if (ev->n_events == 0) {
     PD_CUDA(cudaMemsetAsync(trk->offsets, 0, sizeof(int64_t), st));
     PD_CUDA(cudaMemsetAsync(tow->offsets, 0, sizeof(int64_t), st));
@@ -167,9 +175,6 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
   }
   int rc = pd_card_to_device(card);
   if (rc != PD_OK) return rc;
-
-  PdLaunchPlan plan;
-  pd_plan(card, ev->n_events, n, &plan);
 
   PdParams p;
   std::memset(&p, 0, sizeof(p));
@@ -208,6 +213,7 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
   p.tile_counter = (unsigned int *)ws;
   p.status_word = (int *)(ws + 4);
   p.chain = (unsigned long long *)(ws + kWsHeader);
+  p.ring = (float *)(ws + ws_chain_bytes(plan));
 
   rc = pd_launch_chain(p, plan, dbg != nullptr, cuda_stream);
   if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "kernel launch");

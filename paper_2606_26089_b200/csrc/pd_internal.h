@@ -113,6 +113,7 @@ struct PdParams {
   int n_tiles;
   int capacity;          // C: particles a tile may hold on chip
   unsigned long long *chain;  // [2][n_tiles] look-back words: tracks; towers | neutrals
+  float *ring;                // [max_ctas][6][capacity] smeared track records parked between pass T and pass O
   unsigned int *tile_counter;
   int *status_word;
 };
@@ -127,6 +128,7 @@ struct PdLaunchPlan {
   int capacity;      // C
   int events_per_tile;
   int n_tiles;
+  int max_ctas;      // upper bound of the grid (sizes the workspace ring)
   size_t smem_bytes;
 };
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);

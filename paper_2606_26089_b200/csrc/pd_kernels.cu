@@ -106,38 +106,61 @@ __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v)
   return v;
 }
 
-// Called by one full warp.  Publishes this tile's aggregate, returns the exclusive prefix over all
-// earlier tiles to every lane, then publishes the inclusive prefix.  (Packed fields add independently.)
-__device__ unsigned long long chain_lookback(unsigned long long *st, int tile, unsigned long long agg) {
+// Decoupled look-back, split in two: chain_publish() makes the tile's aggregate visible as soon as it is
+// known; chain_resolve() (one full warp, later) returns the exclusive prefix over all earlier tiles to every
+// lane and publishes the inclusive prefix.  All resident CTAs run nearly in phase, so the nearest predecessor
+// already holding an inclusive prefix is typically a whole grid (~300 tiles) back: the warp looks at
+// LB_K * 32 predecessors per round trip to L2 (LB_K independent loads per lane).  Packed fields add independently.
+template <int LB_K>
+__device__ __forceinline__ unsigned long long chain_resolve(unsigned long long *st, int tile, unsigned long long agg) {
   const int lane = threadIdx.x & 31;
   if (tile == 0) {
     if (lane == 0) st_relaxed(st, FLAG_P | agg);
     return 0;
   }
-  if (lane == 0) st_relaxed(st + tile, FLAG_A | agg);
   unsigned long long excl = 0;
   int pos = tile - 1;
   for (;;) {
-    const int idx = pos - lane;
-    unsigned long long v = FLAG_P;  // before the first tile: prefix 0
-    if (idx >= 0) {
-      v = ld_relaxed(st + idx);
-      while ((v >> 62) == 0) {
-        __nanosleep(40);
-        v = ld_relaxed(st + idx);
+    unsigned long long v[LB_K];
+#pragma unroll
+    for (int k = 0; k < LB_K; ++k) {
+      const int idx = pos - (k * 32 + lane);
+      v[k] = idx >= 0 ? ld_relaxed(st + idx) : FLAG_P;  // before the first tile: prefix 0
+    }
+    bool done = false;
+#pragma unroll
+    for (int k = 0; k < LB_K; ++k) {
+      if (done) break;
+      const int idx = pos - (k * 32 + lane);
+      unsigned long long w = v[k];
+      unsigned pm;
+      for (;;) {
+        pm = __ballot_sync(0xffffffffu, (w >> 62) == 2);
+        const unsigned zm = __ballot_sync(0xffffffffu, (w >> 62) == 0);
+        // every entry up to and including the nearest inclusive prefix must have been published
+        const unsigned upto = pm ? (0xffffffffu >> (32 - __ffs(pm))) : 0xffffffffu;
+        if ((zm & upto) == 0u) break;
+        if ((w >> 62) == 0) {
+          __nanosleep(40);
+          w = ld_relaxed(st + idx);
+        }
+      }
+      if (pm) {
+        const int first = __ffs(pm) - 1;
+        excl += warp_sum_u64(lane <= first ? (w & VAL_MASK) : 0ull);
+        done = true;
+      } else {
+        excl += warp_sum_u64(w & VAL_MASK);
       }
     }
-    const unsigned pm = __ballot_sync(0xffffffffu, (v >> 62) == 2);
-    if (pm) {
-      const int first = __ffs(pm) - 1;  // nearest predecessor holding an inclusive prefix
-      excl += warp_sum_u64(lane <= first ? (v & VAL_MASK) : 0ull);
-      break;
-    }
-    excl += warp_sum_u64(v & VAL_MASK);
-    pos -= 32;
+    if (done) break;
+    pos -= 32 * LB_K;
   }
   if (lane == 0) st_relaxed(st + tile, FLAG_P | (excl + agg));
   return excl;
+}
+__device__ __forceinline__ void chain_publish(unsigned long long *st, int tile, unsigned long long agg) {
+  if (tile > 0) st_relaxed(st + tile, FLAG_A | agg);
 }
 
 // counts a[0..ne) -> exclusive prefix in place, a[ne] = total.  One warp; ne <= G_MAX = 256.
@@ -401,11 +424,11 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
     }
     __syncthreads();
 
-    // ------------------------------------------------------------------ chain T (one warp) beside pass B
-    if (wid == 0) {
-      const unsigned long long ex = chain_lookback(prm.chain, tile, (unsigned long long)n_trk);
-      if (lane == 0) s_misc[1] = ex;
-    } else if (wid == 1) {
+    // ------------------------------------------------------------------ publish chain T; pass B
+    // the track aggregate is published now and its prefix resolved only at the end of the tile (pass O), when
+    // the predecessors have long published theirs: no CTA ever waits on the track chain
+    if (tid == 0) chain_publish(prm.chain, tile, (unsigned long long)n_trk);
+    if (wid == 1) {
       if (multi) event_scan(s_ntrk, ne);
       else if (lane == 0) s_ntrk[0] = 0, s_ntrk[1] = n_trk;
     }
@@ -421,33 +444,28 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       }
     }
     __syncthreads();
-    const long long base_trk = (long long)s_misc[1];
 
     // ------------------------------------------------------------------ pass T: S3 on the accepted tracks
-    // (converged: one thread per track), written straight to the track collection
+    // (converged: one thread per track).  The smeared record is parked in this CTA's slice of the workspace ring
+    // (L2-resident, rewritten every tile) until pass O knows where the tile's tracks go.
+    float *ring = prm.ring + (size_t)blockIdx.x * 6u * (size_t)C;
     for (int s = tid; s < n_trk; s += THREADS) {
       const int i = s_tk[s];
-      const long long src = p0 + i, g = base_trk + s;
-      const int pid = __ldg(prm.pid + src);
+      const long long src = p0 + i;
       const float px = __ldg(prm.px + src), py = __ldg(prm.py + src), pz = __ldg(prm.pz + src);
       const int e = multi ? (int)s_ev[i] : 0;
       TrackOut t;
       track_smear(sc, px, py, pz, prm.rk, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), t);
       const float u = s_uT[i];
       s_uT[i] = t.E_trk;  // from here on: the track energy that pass W subtracts
-      prm.trk_src[g] = (int)src;
-      prm.trk_pid[g] = pid;
-      prm.trk_charge[g] = __ldg(prm.charge + src);
-      prm.trk_pt[g] = t.pt_s;
-      prm.trk_eta[g] = t.eta_mom;
-      prm.trk_phi[g] = t.phi0;
-      prm.trk_E[g] = t.E_trk;
-      prm.trk_eta_out[g] = eta_from_u(sc, u);
-      prm.trk_phi_out[g] = s_phi[i];
+      __stcg(ring + s, t.pt_s);
+      __stcg(ring + C + s, t.eta_mom);
+      __stcg(ring + 2 * C + s, t.phi0);
+      __stcg(ring + 3 * C + s, t.E_trk);
+      __stcg(ring + 4 * C + s, eta_from_u(sc, u));
+      __stcg(ring + 5 * C + s, s_phi[i]);
       if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[src] = t.pt_s;
     }
-    for (int e = tid; e < ne; e += THREADS) prm.trk_offsets[e0 + e + 1] = base_trk + s_ntrk[e + 1];
-    if (tile == 0 && tid == 0) prm.trk_offsets[0] = 0, prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
     __syncthreads();
 
     // ------------------------------------------------------------------ pass W: S5-S7, one thread per tower
@@ -544,36 +562,56 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       const int n_tow = (int)(ta & 0xffffu), n_ph = (int)(ta >> 16), n_nh = (int)tb;
       if (!multi && lane == 0) s_ntow[0] = 0, s_ntow[1] = n_tow, s_nph[0] = 0, s_nph[1] = n_ph, s_nnh[0] = 0, s_nnh[1] = n_nh;
       const unsigned long long agg = (unsigned long long)n_tow | ((unsigned long long)(n_ph + n_nh) << 31);
-      const unsigned long long ex = chain_lookback(prm.chain + prm.n_tiles, tile, agg);
+      if (lane == 0) chain_publish(prm.chain + prm.n_tiles, tile, agg);
+      const unsigned long long ex = chain_resolve<1>(prm.chain + prm.n_tiles, tile, agg);
       if (lane == 0) s_misc[2] = ex;
+    } else if (wid == 1) {
+      // the track prefix: published long ago by every predecessor, so this never waits
+      const unsigned long long ex = chain_resolve<10>(prm.chain, tile, (unsigned long long)n_trk);
+      if (lane == 0) s_misc[1] = ex;
     } else if (multi) {
-      if (wid == 1) event_scan(s_ntow, ne);
-      else if (wid == 2) event_scan(s_nph, ne);
-      else if (wid == 3) event_scan(s_nnh, ne);
+      if (wid == 2) event_scan(s_ntow, ne);
+      else if (wid == 3) event_scan(s_nph, ne);
+      else if (wid == 4) event_scan(s_nnh, ne);
     }
     __syncthreads();
+    const long long base_trk = (long long)s_misc[1];
     const long long base_tow = (long long)(s_misc[2] & FIELD_MASK);
     const long long base_efl = base_trk + (long long)((s_misc[2] >> 31) & FIELD_MASK);
 
     // ------------------------------------------------------------------ pass O: ordered outputs
     for (int e = tid; e < ne; e += THREADS) {
+      prm.trk_offsets[e0 + e + 1] = base_trk + s_ntrk[e + 1];
       prm.tow_offsets[e0 + e + 1] = base_tow + s_ntow[e + 1];
       prm.efl_offsets[e0 + e + 1] = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + s_nnh[e + 1];
     }
-    // EFlow entries of the tracks: copied from the track arrays this CTA wrote above (L2 hits)
+    if (tile == 0 && tid == 0) prm.trk_offsets[0] = 0, prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
+    // tracks and their EFlow entries, from the records pass T parked in the ring (L2 hits)
     for (int s = tid; s < n_trk; s += THREADS) {
-      const long long g = base_trk + s;
-      const int src = __ldcg(prm.trk_src + g);
-      const int e = multi ? (int)s_ev[(int)((long long)src - p0)] : 0;
+      const int i = s_tk[s];
+      const long long src = p0 + i, g = base_trk + s;
+      const float pt = __ldcg(ring + s), eta = __ldcg(ring + C + s), phi = __ldcg(ring + 2 * C + s),
+                  Et = __ldcg(ring + 3 * C + s), eta_o = __ldcg(ring + 4 * C + s), phi_o = __ldcg(ring + 5 * C + s);
+      const int pid = __ldg(prm.pid + src);
+      const signed char q = __ldg(prm.charge + src);
+      const int e = multi ? (int)s_ev[i] : 0;
       const long long at = base_efl + s + s_nph[e] + s_nnh[e];
-      const int pid = __ldcg(prm.trk_pid + g);
       const int apid = pid < 0 ? -pid : pid;
+      prm.trk_src[g] = (int)src;
+      prm.trk_pid[g] = pid;
+      prm.trk_charge[g] = q;
+      prm.trk_pt[g] = pt;
+      prm.trk_eta[g] = eta;
+      prm.trk_phi[g] = phi;
+      prm.trk_E[g] = Et;
+      prm.trk_eta_out[g] = eta_o;
+      prm.trk_phi_out[g] = phi_o;
       prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
-      prm.efl_src[at] = src;
-      prm.efl_pt[at] = __ldcg(prm.trk_pt + g);
-      prm.efl_eta[at] = __ldcg(prm.trk_eta + g);
-      prm.efl_phi[at] = __ldcg(prm.trk_phi + g);
-      prm.efl_E[at] = __ldcg(prm.trk_E + g);
+      prm.efl_src[at] = (int)src;
+      prm.efl_pt[at] = pt;
+      prm.efl_eta[at] = eta;
+      prm.efl_phi[at] = phi;
+      prm.efl_E[at] = Et;
     }
     for (int it = 0; it < n_it; ++it) {
       const int d = it * THREADS + tid;
@@ -686,6 +724,12 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   plan->events_per_tile = g;
   plan->capacity = cap_for(g, budget);
   plan->n_tiles = int((n_events + g - 1) / g);
+  {
+    // grid <= resident CTAs of the device (256 SMs assumed when no device can be queried yet)
+    const long sms = query_device() == PD_OK ? g_num_sms : 256;
+    const long ctas = sms * (plan->threads == 1024 ? 1 : 2);
+    plan->max_ctas = int(plan->n_tiles < ctas ? (plan->n_tiles > 0 ? plan->n_tiles : 1) : ctas);
+  }
   plan->smem_bytes = pdk::make_layout(sc.n_bins, 2 * sc.lut_side, sc.n_towers, sc.words_per_event, g, plan->capacity).total;
   return PD_OK;
 }
