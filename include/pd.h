@@ -125,7 +125,7 @@ void pd_free_card(pd_card *card);
 int pd_card_info(const pd_card *card, pd_card_info_t *out);
 
 /* Bytes of DEVICE workspace pd_simulate needs for a call of this size (look-back chains, tile
- * counter, status word).  Negative pd_status on invalid arguments. */
+ * counter, status word, the ring in which smeared track records wait for their output offsets).  Negative pd_status on invalid arguments. */
 int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles);
 
 /* One pass of the whole chain S0..S8 over a batch of events.
@@ -145,11 +145,21 @@ int pd_simulate(const pd_card *card, const pd_events *events, uint64_t seed, int
 
 /* Reads back (synchronising the stream) the device-side status word a pd_simulate call left in its
  * workspace: PD_OK, or PD_EEVENTSIZE if some tile of events did not fit on chip (its events then
- * produced no objects). */
+ * produced no objects; see pd_set_tile_events). */
 int pd_last_status(const void *workspace, void *cuda_stream);
 
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
+
+/* Events per on-chip tile for the calls this thread makes from now on: 0 (default) = chosen from the
+ * average event size with head-room for Poisson-like fluctuations; g >= 1 = at most g (<= 256).  A batch
+ * whose event sizes are far from Poisson (a few huge events among many small ones) can make a tile of the
+ * automatic plan exceed the on-chip capacity: pd_last_status() then reports PD_EEVENTSIZE and the caller
+ * re-runs the call after pd_set_tile_events(1) (pd_simulate_host does that itself).  With one event per
+ * tile the only limit left is the capacity of a CTA, 8,191 particles per event.  Results do not depend on
+ * the tiling.  pd_workspace_bytes() depends on it: call it after changing the setting.  Returns the
+ * previous value. */
+int pd_set_tile_events(int g);
 
 /* Same computation with HOST pointers everywhere (inputs and outputs in host memory, pinned or
  * pageable).  Copies inputs to the device, runs pd_simulate, copies the three collections back and

@@ -4,4 +4,4 @@
 There is no CPU fallback."""
 from . import binding  # noqa: F401
 from .binding import (Card, DeviceEvents, DeviceOutputs, HostBuffers, PdError, last_launch_count, last_status,  # noqa: F401
-                      simulate, simulate_host, workspace_bytes)
+                      set_tile_events, simulate, simulate_host, workspace_bytes)

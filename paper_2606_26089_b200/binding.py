@@ -18,7 +18,7 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_set_tile_events", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
@@ -87,6 +87,7 @@ def lib():
                                   C.POINTER(EFlow), C.POINTER(Debug), _p, C.c_int64, _p]
         L.pd_last_status.argtypes = [_p, _p]
         L.pd_last_launch_count.argtypes = []
+        L.pd_set_tile_events.argtypes = [C.c_int]
         L.pd_simulate_host.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks),
                                        C.POINTER(Towers), C.POINTER(EFlow), _p]
         L.pd_strerror.argtypes = [C.c_int]
@@ -135,6 +136,12 @@ def workspace_bytes(card: Card, n_events: int, n_particles: int) -> int:
 
 def last_launch_count() -> int:
     return int(lib().pd_last_launch_count())
+
+
+def set_tile_events(g: int) -> int:
+    """pd_set_tile_events: events per on-chip tile (0 = automatic); returns the previous setting.  Buffers
+    made by DeviceOutputs before the call keep the workspace size of the old setting."""
+    return int(lib().pd_set_tile_events(int(g)))
 
 
 def _torch():

@@ -92,6 +92,8 @@ int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_part
 
 int pd_last_launch_count(void) { return t_launches; }
 
+int pd_set_tile_events(int g) { return pd_plan_set_tile_events(g); }
+
 }  // extern "C"
 
 // Upload the per-bin tables of a card to the current device (once).
@@ -229,8 +231,10 @@ int pd_last_status(const void *workspace, void *cuda_stream) {
   return word;
 }
 
-int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
-                     pd_towers *tow, pd_eflow *efl, void *cuda_stream) {
+}  // extern "C"
+
+static int simulate_host_once(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                              pd_towers *tow, pd_eflow *efl, void *cuda_stream) {
   t_launches = 0;
   if (!card || !ev || !trk || !tow || !efl) return PD_EINVAL;
   if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 30)) return PD_EINVAL;
@@ -338,6 +342,22 @@ int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, in
   cudaFreeAsync(base, st);
   cudaStreamSynchronize(st);
   t_launches = launches;
+  return rc;
+}
+
+extern "C" {
+
+int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                     pd_towers *tow, pd_eflow *efl, void *cuda_stream) {
+  int rc = simulate_host_once(card, ev, seed, event_base, trk, tow, efl, cuda_stream);
+  if (rc == PD_EEVENTSIZE) {
+    // a tile of the automatic plan did not fit on chip (event sizes far from Poisson): one event per tile
+    const int launches = t_launches;
+    const int prev = pd_plan_set_tile_events(1);
+    if (prev != 1) rc = simulate_host_once(card, ev, seed, event_base, trk, tow, efl, cuda_stream);
+    pd_plan_set_tile_events(prev);
+    t_launches += launches;
+  }
   return rc;
 }
 

@@ -131,5 +131,6 @@ struct PdLaunchPlan {
   int max_ctas;      // upper bound of the grid (sizes the workspace ring)
   size_t smem_bytes;
 };
+int pd_plan_set_tile_events(int g);
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);
 int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, void *stream);

@@ -691,8 +691,15 @@ static int query_device() {
 // Tile plan from sizes the host knows (n_events, n_particles).  B200: 228 KB of shared memory per SM, 1 KB
 // reserved per CTA, 227 KB per CTA at most.  Preferred shape: two 512-thread CTAs per SM (113 KB each), so one
 // CTA's barriers and look-back waits are covered by the other; events too large for that get one 1024-thread CTA
-// with the whole SM.  G = events per tile: as many as fit the on-chip capacity C with ~4 sigma of head-room
+// with the whole SM.  G = events per tile: as many as fit the on-chip capacity C with 6 sigma of head-room
 // for a Poisson-like sum, but no more than keeps every CTA slot of the GPU busy on small inputs.
+static thread_local int t_tile_events = 0;  // pd_set_tile_events: 0 = automatic
+int pd_plan_set_tile_events(int g) {
+  const int prev = t_tile_events;
+  t_tile_events = g < 0 ? 0 : (g > pdk::G_MAX ? pdk::G_MAX : g);
+  return prev;
+}
+
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan) {
   const PdCardScalars &sc = c->sc;
   const double avg = n_events > 0 ? double(n_particles) / double(n_events) : 0.0;
@@ -706,7 +713,7 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   };
   auto fits = [&](int G, size_t budget) {
     const double C = cap_for(G, budget);
-    return double(G) * avg + 4.0 * std::sqrt(double(G) * avg + 1.0) + 16.0 <= C;
+    return double(G) * avg + 6.0 * std::sqrt(double(G) * avg + 1.0) + 16.0 <= C;
   };
   static const int force_threads = std::getenv("PD_THREADS") ? std::atoi(std::getenv("PD_THREADS")) : 0;
   size_t budget = budget2;
@@ -721,6 +728,7 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   const long slots = 148L * (plan->threads == 512 ? 2 : 1);
   const long g_bal = long((n_events + 4 * slots - 1) / (4 * slots));
   if (g > g_bal) g = int(g_bal < 1 ? 1 : g_bal);
+  if (t_tile_events > 0 && g > t_tile_events) g = t_tile_events;
   plan->events_per_tile = g;
   plan->capacity = cap_for(g, budget);
   plan->n_tiles = int((n_events + g - 1) / g);

@@ -114,3 +114,32 @@ def test_host_pointer_entry_matches_device_entry():
     got = hb.to_numpy()
     for k, v in got.items():
         assert v.tobytes() == ref[k].tobytes(), k
+
+
+def test_skewed_event_sizes_need_one_event_per_tile():
+    """A few huge events among many tiny ones: a tile of the automatic plan overflows the on-chip capacity
+    (PD_EEVENTSIZE); with pd_set_tile_events(1) the same batch runs and matches the oracle, and
+    pd_simulate_host falls back by itself."""
+    import paper_2606_26089_b200 as pd
+    from gpu_util import run_gpu
+    from parity import compare
+
+    big = wl.generate(2, 3)                      # ~4,000 particles each
+    small = wl.generate(0, 40000)                # ~60 particles each: the automatic plan packs ~30 per tile
+    ev = wl.concat_events([wl.slice_events(small, 0, 7000), wl.slice_events(big, 0, 1), wl.slice_events(small, 7000, 39000),
+                           wl.slice_events(big, 1, 3), wl.slice_events(small, 39000, 40000)])
+    auto = run_gpu("cms_like", ev, 21, debug=False)
+    assert auto["status_word"] == pd.binding.PD_EEVENTSIZE
+    prev = pd.set_tile_events(1)
+    try:
+        one = run_gpu("cms_like", ev, 21)
+        assert one["status_word"] == 0
+        _check(compare("cms_like", ev, 21, one))
+    finally:
+        pd.set_tile_events(prev)
+    card = pd.Card("cms_like")
+    hb = pd.HostBuffers(ev)
+    pd.simulate_host(card, hb, 21)               # retries with one event per tile internally
+    got = hb.to_numpy()
+    for k, v in got.items():
+        assert v.tobytes() == one[k].tobytes(), k
