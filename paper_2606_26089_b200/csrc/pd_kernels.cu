@@ -1,4 +1,4 @@
-// pd_kernels.cu -- the fused Delphes-chain kernel for sm_100a (steps S0..S8 of SURVEY.md section 8a), v3.
+// pd_kernels.cu -- the fused Delphes-chain kernel for sm_100a (steps S0..S8 of SURVEY.md section 8a), v5.
 //
 // Persistent CTAs (two 512-thread CTAs per SM, or one 1024-thread CTA for large events); a CTA repeatedly
 // claims a TILE (a run of G whole events, <= C particles) from an atomic counter and takes it through
@@ -7,17 +7,18 @@
 //   scan 1              one block scan for two things: the ordered list of accepted tracks, and the
 //                       popcount prefix of the bitmaps = the rank ("slot") of every occupied tower in
 //                       (event, tower id) order -- this replaces a sort of the deposits
-//   pass B   S5         every deposit pushes itself on its slot's list (one integer atomicExch)
-//   chain T             decoupled look-back over tiles -> global track offset (overlaps pass B)
-//   pass T   S3         one thread per accepted track: pT smear, track record written to HBM
+//   pass B   S5         every deposit pushes itself on its slot's list (one integer atomicExch); the tile's
+//                       track count is published on chain T
+//   pass T   S3         one thread per accepted track: pT smear; E_trk stays on chip, the track record is
+//                       parked in this CTA's slice of the workspace ring (L2) until its offset is known
 //   pass W   S5-S7      one thread per occupied tower: exact fixed-point sum of its list (order-independent),
 //                       Philox tower stream, log-normal smear, thresholds, EFlow subtraction
-//   chain W             look-back for the tower and neutral offsets (one packed 64-bit word)
-//   pass O   S8         ordered compaction of towers / photons / neutral hadrons, EFlow track entries,
-//                       CSR offsets
-// Nothing but the inputs and the final collections touches HBM.  Sums are order-stable: each tower's
-// deposits are added as 64-bit fixed-point integers (exact, hence independent of the order in which the
-// list was built), and the only atomics are integer (bitmap OR, list exchange, counters).
+//   scan W              one scan over the per-warp counts; chain W published and resolved (decoupled
+//                       look-back), chain T resolved (never waits: published a whole phase ago)
+//   pass O   S8         ordered compaction of tracks / towers / photons / neutral hadrons, CSR offsets
+// Nothing but the inputs, the final collections and the ring touches memory.  Sums are order-stable: each
+// tower's deposits are added as 64-bit fixed-point integers (exact, hence independent of the order in which
+// the list was built), and the only atomics are integer (bitmap OR, list exchange, counters).
 #include <cuda_runtime.h>
 
 #include <cmath>
