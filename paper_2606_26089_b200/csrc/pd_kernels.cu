@@ -590,13 +590,14 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
     // tracks and their EFlow entries, from the records pass T parked in the ring (L2 hits)
     for (int s = tid; s < n_trk; s += THREADS) {
       const int i = s_tk[s];
-      const long long src = p0 + i, g = base_trk + s;
+      const long long src = p0 + i;
+      const unsigned g = (unsigned)base_trk + (unsigned)s;  // all output indices fit 32 bits (n_particles < 2^30)
       const float pt = __ldcg(ring + s), eta = __ldcg(ring + C + s), phi = __ldcg(ring + 2 * C + s),
                   Et = __ldcg(ring + 3 * C + s), eta_o = __ldcg(ring + 4 * C + s), phi_o = __ldcg(ring + 5 * C + s);
       const int pid = __ldg(prm.pid + src);
       const signed char q = __ldg(prm.charge + src);
       const int e = multi ? (int)s_ev[i] : 0;
-      const long long at = base_efl + s + s_nph[e] + s_nnh[e];
+      const unsigned at = (unsigned)base_efl + (unsigned)(s + s_nph[e] + s_nnh[e]);
       const int apid = pid < 0 ? -pid : pid;
       prm.trk_src[g] = (int)src;
       prm.trk_pid[g] = pid;
@@ -639,7 +640,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         const float phi_c = fmaf((float)j + 0.5f, s_w[b], -kPiF);
         const float ic = s_inv_cosh[b];
         if (f_tw) {
-          const long long at = base_tow + (int)(pa & 0xffffu) + __popc(m_tw & lt_mask);
+          const unsigned at = (unsigned)base_tow + (pa & 0xffffu) + (unsigned)__popc(m_tw & lt_mask);
           prm.tow_tower[at] = tower;
           prm.tow_eta[at] = eta_c;
           prm.tow_phi[at] = phi_c;
@@ -650,7 +651,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         }
         if (f_ph) {
           const int slot = (int)(pa >> 16) + __popc(m_ph & lt_mask);
-          const long long at = base_efl + s_ntrk[e + 1] + s_nnh[e] + slot;
+          const unsigned at = (unsigned)base_efl + (unsigned)(s_ntrk[e + 1] + s_nnh[e] + slot);
           prm.efl_cls[at] = (signed char)PD_CLS_PHOTON;
           prm.efl_src[at] = tower;
           prm.efl_pt[at] = nem * ic;
@@ -660,7 +661,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         }
         if (f_nh) {
           const int slot = (int)pb + __popc(m_nh & lt_mask);
-          const long long at = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + slot;
+          const unsigned at = (unsigned)base_efl + (unsigned)(s_ntrk[e + 1] + s_nph[e + 1] + slot);
           prm.efl_cls[at] = (signed char)PD_CLS_NEUHAD;
           prm.efl_src[at] = tower;
           prm.efl_pt[at] = nhad * ic;

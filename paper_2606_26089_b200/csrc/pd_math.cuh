@@ -224,12 +224,26 @@ struct ParticleOut {
 
 // Rare path: a helix grazing the barrel (within a few % of the looper threshold).  The crossing angle
 // amplifies the rounding of rho by 1/sqrt(distance to tangency), so the quadratic is redone in double.
+// 1/sqrt(x) and 1/x in double from the fp32 MUFU seed and two Newton steps (relative error ~1e-14): no
+// double-precision divide or square-root routine on this path.
+__device__ __forceinline__ double rsqrt_d(double x) {
+  double y = (double)fast_rsqrt((float)x);
+  y = y * fma(-0.5 * x, y * y, 1.5);
+  return y * fma(-0.5 * x, y * y, 1.5);
+}
+__device__ __forceinline__ double rcp_d(double x) {
+  double y = (double)fast_rcp((float)x);
+  y = y * fma(-x, y, 2.0);
+  return y * fma(-x, y, 2.0);
+}
+
 __device__ __noinline__ bool graze_double(const PdCardScalars &sc, float px, float py, float vx, float vy, float aq,
                                           float s, float &cc, float &ss) {
   const double pxd = px, pyd = py, vxd = vx, vyd = vy, Rd = sc.R;
-  const double ptd = sqrt(pxd * pxd + pyd * pyd);
-  const double rhod = ptd / (sc.kB_d * (double)aq);
-  const double ipt = 1.0 / ptd;
+  const double p2 = pxd * pxd + pyd * pyd;
+  const double ipt = rsqrt_d(p2);
+  const double ptd = p2 * ipt;
+  const double rhod = ptd * rcp_d(sc.kB_d * (double)aq);
   const double ad = (vxd * pxd + vyd * pyd) * ipt;
   const double bd = (double)s * (vyd * pxd - vxd * pyd) * ipt;
   const double Dd = Rd * Rd - (vxd * vxd + vyd * vyd);
@@ -237,7 +251,7 @@ __device__ __noinline__ bool graze_double(const PdCardScalars &sc, float px, flo
   const double Qd = 4.0 * rhod * (rhod + bd) - Dd;
   const double dd = Pd * Pd + Qd * Dd;
   if (!(dd >= 0.0)) return false;
-  const double Sd = sqrt(dd);
+  const double Sd = dd > 1e-30 ? dd * rsqrt_d(dd) : 0.0;
   if (Pd >= 0.0) cc = (float)(Pd + Sd), ss = (float)Dd;
   else cc = (float)Qd, ss = (float)(Sd - Pd);
   return true;
@@ -351,18 +365,13 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
     // exactly an edge, e.g. pT = 0.1 GeV, is decided like the fp64 definition); unused edges are +max
     const double p2 = (double)px * (double)px + (double)py * (double)py;
     int ip = 0, it = 0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
-    if (sc.n_pt > 4) {
-#pragma unroll
-      for (int k = 4; k < PD_MAX_EFF_EDGES; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
-    }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
-    if (sc.n_T > 4) {
-#pragma unroll
-      for (int k = 4; k < PD_MAX_EFF_EDGES; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
-    }
+    // the first two edges of either kind without a branch, the rest (cards with finer tables) in uniform loops
+    ip += p2 > sc.pt_edge2_d[0] ? 1 : 0;
+    ip += p2 > sc.pt_edge2_d[1] ? 1 : 0;
+    for (int k = 2; k < sc.n_pt; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
+    it += apz >= sc.T_edge[0] * pt ? 1 : 0;
+    it += apz >= sc.T_edge[1] * pt ? 1 : 0;
+    for (int k = 2; k < sc.n_T; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
     const int cell = ip * (sc.n_T + 1) + it;
     const float eps = sc.cell_eps[cell];
     o.eps_row = sc.cell_row[cell];
