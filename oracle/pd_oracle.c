@@ -888,3 +888,58 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
   if (rc == PDO_OK && rejected > 0) rc = PDO_EOVERRIDE;
   return rc;
 }
+
+/* ---- event features and lepton isolation: see pd_oracle.h (Eq. 1) ---- */
+int pdo_event_features(const pdo_objects *obj, double dr_max, double fsr_dr, double *ht, double *met_x,
+                       double *met_y, double *met, double *iso_charged, double *iso_neutral, double *iso_photon,
+                       double *r_iso, double *iso_amb) {
+  const double PI = 3.14159265358979323846;
+  int64_t e, i, j;
+  if (!obj || obj->n_events < 0 || !obj->offsets || !ht || !met_x || !met_y || !met) return PDO_EINVAL;
+  if (!iso_charged || !iso_neutral || !iso_photon || !r_iso || !(dr_max >= 0.0) || !(fsr_dr >= 0.0)) return PDO_EINVAL;
+  for (e = 0; e < obj->n_events; ++e) {
+    const int64_t a = obj->offsets[e], b = obj->offsets[e + 1];
+    double sum_pt = 0.0, sx = 0.0, sy = 0.0;
+    /* H_T and the missing transverse momentum: plain sums in object order */
+    for (i = a; i < b; ++i) {
+      const double pt = (double)obj->pt[i], phi = (double)obj->phi[i];
+      sum_pt += pt;
+      sx += pt * cos(phi);
+      sy += pt * sin(phi);
+    }
+    ht[e] = sum_pt;
+    met_x[e] = -sx;
+    met_y[e] = -sy;
+    met[e] = sqrt(sx * sx + sy * sy);
+    /* Eq. 1 for every electron / muon of the event */
+    for (i = a; i < b; ++i) {
+      double s_ch = 0.0, s_nh = 0.0, s_ph = 0.0, amb = 0.0;
+      const int is_lepton = obj->cls[i] == PDO_CLS_ELECTRON || obj->cls[i] == PDO_CLS_MUON;
+      if (is_lepton) {
+        for (j = a; j < b; ++j) {
+          double deta, dphi, dr;
+          if (j == i) continue; /* "the sums exclude the lepton itself" */
+          deta = (double)obj->eta[j] - (double)obj->eta[i];
+          dphi = (double)obj->phi[j] - (double)obj->phi[i];
+          while (dphi > PI) dphi -= 2.0 * PI;
+          while (dphi <= -PI) dphi += 2.0 * PI;
+          dr = sqrt(deta * deta + dphi * dphi);
+          if (fabs(dr - dr_max) <= 1e-6 || (obj->cls[j] == PDO_CLS_PHOTON && fsr_dr > 0.0 && fabs(dr - fsr_dr) <= 1e-6))
+            amb += (double)obj->pt[j];
+          if (!(dr < dr_max)) continue;
+          if (obj->cls[j] == PDO_CLS_PHOTON) {
+            if (!(dr < fsr_dr)) s_ph += (double)obj->pt[j]; /* reading F4 */
+          } else if (obj->cls[j] == PDO_CLS_NEUHAD) {
+            s_nh += (double)obj->pt[j];
+          } else {
+            s_ch += (double)obj->pt[j];
+          }
+        }
+      }
+      iso_charged[i] = s_ch, iso_neutral[i] = s_nh, iso_photon[i] = s_ph;
+      r_iso[i] = is_lepton ? (s_ch + s_nh + s_ph) / (double)obj->pt[i] : 0.0;
+      if (iso_amb) iso_amb[i] = amb;
+    }
+  }
+  return PDO_OK;
+}

@@ -137,6 +137,32 @@ int pdo_simulate(const pdo_card *card, const pdo_events *ev, uint64_t seed, int6
                  pdo_tracks *tracks, pdo_towers *towers, pdo_eflow *eflow, pdo_debug *debug,
                  const pdo_overrides *ov);
 
+/* ---- event features and lepton isolation (section 2.4 Eq. 1, Table 2) ----
+ * Computed from an EFlow ("PFlow") collection in CSR form, per event:
+ *   H_T = sum_i pT_i,   E_T^miss vector = -( sum_i pT_i cos phi_i, sum_i pT_i sin phi_i ),   E_T^miss = its length
+ *   (readings F1, F2 of DESIGN.md section 11: the "cached scalar event features (H_T and E_T^miss)" of P:L119,
+ *   "H_T, E_T^miss values for ... PFlow collections" of P:L141, taken over every object of the collection);
+ * and, for every object of class electron or muon, Eq. 1 of P:L121-127:
+ *   R_iso = ( sum_{dR<dr_max} pT^charged + sum_{dR<dr_max} pT^neutral + sum_{dR<dr_max} pT^gamma ) / pT^lepton,
+ *   dR = sqrt(d_eta^2 + d_phi^2), d_phi wrapped into (-pi, pi], "where the sums exclude the lepton itself"
+ *   (by index), charged = classes 0,1,2, neutral = class 3, gamma = class 4.  "The last term excludes photons
+ *   that are candidates for final-state radiation" -- the paper gives no criterion; reading F4: photons with
+ *   dR < fsr_dr are left out of the photon term (fsr_dr = 0 keeps them all).  The cone is strict (dR < dr_max).
+ *   Objects of the other classes get 0 in all four isolation arrays.
+ * Sums are taken in fp64 in object order.  iso_amb[i] (nullable) receives the pT sum of the objects whose dR
+ * lies within 1e-6 of dr_max or fsr_dr (near-edge: either outcome is allowed for those). */
+typedef struct {
+  int64_t n_events;
+  const int64_t *offsets; /* [n_events+1] */
+  const int8_t *cls;
+  const float *pt, *eta, *phi;
+} pdo_objects;
+
+int pdo_event_features(const pdo_objects *obj, double dr_max, double fsr_dr,
+                       double *ht, double *met_x, double *met_y, double *met, /* [n_events] */
+                       double *iso_charged, double *iso_neutral, double *iso_photon, double *r_iso, /* [n_objects] */
+                       double *iso_amb /* [n_objects], may be NULL */);
+
 const char *pdo_strerror(int code);
 
 /* ---- building blocks exposed so that tests can pin them one by one ---- */

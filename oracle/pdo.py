@@ -56,6 +56,10 @@ class _Debug(C.Structure):
                 ("tw_near", _p)]
 
 
+class _Objects(C.Structure):
+    _fields_ = [("n_events", C.c_int64), ("offsets", _p), ("cls", _p), ("pt", _p), ("eta", _p), ("phi", _p)]
+
+
 class _Overrides(C.Structure):
     _fields_ = [("face", _p), ("tower", _p), ("eps_row", _p), ("n_tower_ov", C.c_int64),
                 ("tw_event", _p), ("tw_id", _p), ("tw_mask", _p), ("tw_value", _p), ("n_rejected", _p)]
@@ -92,6 +96,7 @@ def lib():
         L.pdo_tower_index.restype = C.c_int32
         L.pdo_efficiency.argtypes = [_p, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int)]
         L.pdo_efficiency.restype = C.c_double
+        L.pdo_event_features.argtypes = [C.POINTER(_Objects), C.c_double, C.c_double] + [_p] * 9
         _lib = L
     return _lib
 
@@ -251,4 +256,26 @@ def simulate(card: Card, ev, seed: int, event_base: int = 0, overrides: dict | N
         tot = int(DT["tw_offsets"][-1])
         for k, a in DT.items():
             out["dtw_" + k.replace("tw_", "")] = a if k == "tw_offsets" else a[:tot]
+    return out
+
+
+def event_features(offsets, cls, pt, eta, phi, dr_max: float = 0.4, fsr_dr: float = 0.0) -> dict:
+    """pdo_event_features on an EFlow-like CSR collection (Eq. 1): per event ht, met_x,
+    met_y, met; per object iso_charged, iso_neutral, iso_photon, r_iso, and iso_amb (pT of the objects whose
+    dR is within 1e-6 of a cone edge).  All float64."""
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    cls = np.ascontiguousarray(cls, dtype=np.int8)
+    pt, eta, phi = (np.ascontiguousarray(a, dtype=np.float32) for a in (pt, eta, phi))
+    ne, n = int(offsets.shape[0] - 1), int(offsets[-1])
+    assert cls.shape[0] >= n and pt.shape[0] >= n and eta.shape[0] >= n and phi.shape[0] >= n
+    ev = {k: np.zeros(max(ne, 1), dtype=np.float64) for k in ("ht", "met_x", "met_y", "met")}
+    ob = {k: np.zeros(max(n, 1), dtype=np.float64) for k in ("iso_charged", "iso_neutral", "iso_photon", "r_iso", "iso_amb")}
+    o = _Objects(ne, _ptr(offsets), _ptr(cls), _ptr(pt), _ptr(eta), _ptr(phi))
+    rc = lib().pdo_event_features(C.byref(o), float(dr_max), float(fsr_dr), _ptr(ev["ht"]), _ptr(ev["met_x"]),
+                                  _ptr(ev["met_y"]), _ptr(ev["met"]), _ptr(ob["iso_charged"]), _ptr(ob["iso_neutral"]),
+                                  _ptr(ob["iso_photon"]), _ptr(ob["r_iso"]), _ptr(ob["iso_amb"]))
+    if rc != 0:
+        raise OracleError(rc)
+    out = {k: v[:ne] for k, v in ev.items()}
+    out.update({k: v[:n] for k, v in ob.items()})
     return out
