@@ -148,6 +148,28 @@ int pd_simulate(const pd_card *card, const pd_events *events, uint64_t seed, int
  * produced no objects; see pd_set_tile_events). */
 int pd_last_status(const void *workspace, void *cuda_stream);
 
+/* ---- Event features and lepton isolation (section 2.4 Eq. 1; L141 Table 2) ----
+ * From an EFlow ("PFlow") collection, per event (readings F1, F2 of DESIGN.md section 11):
+ *   ht = sum_i pT_i;  (met_x, met_y) = -(sum_i pT_i cos phi_i, sum_i pT_i sin phi_i);  met = its length;
+ * and for every object of class PD_CLS_ELECTRON or PD_CLS_MUON, Eq. 1:
+ *   r_iso = (iso_charged + iso_neutral + iso_photon) / pT_lepton, the three terms being the pT sums of the event's
+ *   other objects of classes {0,1,2}, {3}, {4} with dR = sqrt(d_eta^2 + d_phi^2) < dr_max around the lepton
+ *   (d_phi wrapped; the lepton itself excluded; photons with dR < fsr_dr -- final-state-radiation candidates,
+ *   reading F4 -- left out of the photon term; fsr_dr = 0 keeps them all).  Objects of other classes get 0.
+ * All pointers are DEVICE pointers owned by the caller; per-event arrays have n_events elements, per-object arrays
+ * as many as the collection holds (eflow->offsets[n_events], at most eflow->capacity).  Sums are exact
+ * fixed-point sums (units of 2^-32 GeV), hence independent of order and bitwise reproducible. */
+typedef struct {
+  float *ht, *met_x, *met_y, *met;                       /* [n_events]  */
+  float *iso_charged, *iso_neutral, *iso_photon, *r_iso; /* [n_objects] */
+} pd_features;
+
+/* Asynchronous on cuda_stream; allocates nothing; needs no workspace (events are independent, no output is
+ * compacted).  Only eflow->offsets, cls, pt, eta, phi are read.  Errors: PD_EINVAL (null pointers, negative
+ * n_events, dr_max or fsr_dr negative or not finite), PD_ECUDA. */
+int pd_event_features(const pd_eflow *eflow, int64_t n_events, float dr_max, float fsr_dr, pd_features *out,
+                      void *cuda_stream);
+
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 

@@ -18,7 +18,7 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_set_tile_events", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
@@ -27,6 +27,10 @@ _lib = None
 class CardInfo(C.Structure):
     _fields_ = [("n_towers", C.c_int32), ("n_eta_bins", C.c_int32), ("grid_coord", C.c_int32), ("bz", C.c_float),
                 ("radius", C.c_float), ("half_length", C.c_float), ("n_eff_rows", C.c_int32)]
+
+
+class Features(C.Structure):
+    _fields_ = [(k, _p) for k in ("ht", "met_x", "met_y", "met", "iso_charged", "iso_neutral", "iso_photon", "r_iso")]
 
 
 class Events(C.Structure):
@@ -88,6 +92,7 @@ def lib():
         L.pd_last_status.argtypes = [_p, _p]
         L.pd_last_launch_count.argtypes = []
         L.pd_set_tile_events.argtypes = [C.c_int]
+        L.pd_event_features.argtypes = [C.POINTER(EFlow), C.c_int64, C.c_float, C.c_float, C.POINTER(Features), _p]
         L.pd_simulate_host.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks),
                                        C.POINTER(Towers), C.POINTER(EFlow), _p]
         L.pd_strerror.argtypes = [C.c_int]
@@ -206,6 +211,54 @@ class DeviceOutputs:
             for k, t in self.dbg.items():
                 out["dbg_" + k] = t[: self.n_particles].cpu().numpy()
         return out
+
+
+class DeviceFeatures:
+    """Buffers of pd_event_features for a DeviceOutputs' EFlow collection (per event: ht, met_x, met_y, met; per
+    EFlow object: iso_charged, iso_neutral, iso_photon, r_iso)."""
+
+    EVENT_FIELDS = ("ht", "met_x", "met_y", "met")
+    OBJECT_FIELDS = ("iso_charged", "iso_neutral", "iso_photon", "r_iso")
+
+    def __init__(self, n_events: int, capacity: int, device="cuda"):
+        torch = _torch()
+        self.n_events = int(n_events)
+        self.ev = {k: torch.empty(max(self.n_events, 1), dtype=torch.float32, device=device) for k in self.EVENT_FIELDS}
+        self.ob = {k: torch.empty(max(int(capacity), 1), dtype=torch.float32, device=device) for k in self.OBJECT_FIELDS}
+        self.c = Features(*[_tptr(self.ev[k]) for k in self.EVENT_FIELDS], *[_tptr(self.ob[k]) for k in self.OBJECT_FIELDS])
+
+    def to_numpy(self, n_objects: int) -> dict:
+        _torch().cuda.synchronize()
+        out = {k: t[: self.n_events].cpu().numpy() for k, t in self.ev.items()}
+        out.update({k: t[: int(n_objects)].cpu().numpy() for k, t in self.ob.items()})
+        return out
+
+
+class DeviceObjects:
+    """An EFlow-like collection uploaded from numpy (offsets, cls, pt, eta, phi): the input of pd_event_features
+    when it does not come from a DeviceOutputs."""
+
+    def __init__(self, offsets, cls, pt, eta, phi, device="cuda"):
+        torch = _torch()
+        import numpy as np
+
+        self.n_events = int(len(offsets) - 1)
+        self.n_objects = int(offsets[-1])
+        pad = lambda a, dt: torch.from_numpy(np.ascontiguousarray(np.concatenate([np.asarray(a, dtype=dt), np.zeros(1, dtype=dt)]))).to(device)  # noqa: E731
+        self.t = {"offsets": torch.from_numpy(np.ascontiguousarray(offsets, dtype=np.int64)).to(device), "cls": pad(cls, np.int8),
+                  "pt": pad(pt, np.float32), "eta": pad(eta, np.float32), "phi": pad(phi, np.float32)}
+        self.c_efl = EFlow(self.n_objects, _tptr(self.t["offsets"]), _tptr(self.t["cls"]), None, _tptr(self.t["pt"]),
+                           _tptr(self.t["eta"]), _tptr(self.t["phi"]), None)
+
+
+def event_features(out, feat: DeviceFeatures, dr_max: float = 0.4, fsr_dr: float = 0.0, stream=None):
+    """pd_event_features on the EFlow collection of `out` (torch's current stream or `stream`).  Asynchronous."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().pd_event_features(C.byref(out.c_efl), int(out.n_events), float(dr_max), float(fsr_dr), C.byref(feat.c),
+                                   C.c_void_p(st.cuda_stream)))
 
 
 def simulate(card: Card, dev_events: DeviceEvents, out: DeviceOutputs, seed: int, event_base: int = 0, stream=None):

@@ -94,6 +94,28 @@ int pd_last_launch_count(void) { return t_launches; }
 
 int pd_set_tile_events(int g) { return pd_plan_set_tile_events(g); }
 
+int pd_event_features(const pd_eflow *efl, int64_t n_events, float dr_max, float fsr_dr, pd_features *out,
+                      void *cuda_stream) {
+  t_launches = 0;
+  if (!efl || !out || n_events < 0) return PD_EINVAL;
+  if (!(dr_max >= 0.f) || !(fsr_dr >= 0.f) || !std::isfinite(dr_max) || !std::isfinite(fsr_dr)) return PD_EINVAL;
+  if (!efl->offsets || !out->ht || !out->met_x || !out->met_y || !out->met) return PD_EINVAL;
+  if (n_events == 0) return PD_OK;
+  if (!efl->cls || !efl->pt || !efl->eta || !efl->phi) return PD_EINVAL;
+  if (!out->iso_charged || !out->iso_neutral || !out->iso_photon || !out->r_iso) return PD_EINVAL;
+  PdFeatParams p;
+  p.n_events = n_events;
+  p.offsets = (const long long *)efl->offsets;
+  p.cls = efl->cls, p.pt = efl->pt, p.eta = efl->eta, p.phi = efl->phi;
+  p.dr_max2 = (float)((double)dr_max * (double)dr_max), p.fsr2 = (float)((double)fsr_dr * (double)fsr_dr);
+  p.ht = out->ht, p.met_x = out->met_x, p.met_y = out->met_y, p.met = out->met;
+  p.iso_charged = out->iso_charged, p.iso_neutral = out->iso_neutral, p.iso_photon = out->iso_photon, p.r_iso = out->r_iso;
+  const int rc = pd_launch_features(p, cuda_stream);
+  if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "features kernel launch");
+  t_launches = 1;
+  return PD_OK;
+}
+
 }  // extern "C"
 
 // Upload the per-bin tables of a card to the current device (once).

@@ -1,0 +1,146 @@
+// pd_features.cu -- event features (H_T, E_T^miss) and lepton isolation (Eq. 1 of the paper) from an EFlow
+// collection: the step right after the detector-response chain (
+// readings F1-F4 of DESIGN.md section 11).  Product code; shares nothing with oracle/.
+//
+// Events are independent and nothing is compacted, so there is no chain and no workspace.  A 256-thread CTA
+// (three per SM) walks over chunks of consecutive events (static, strided assignment); inside a chunk it takes
+// RUNS of whole events whose objects fit its shared-memory cache (pT, eta, phi, class: 13 bytes per object), so
+// the O(leptons x objects) cone sums read shared memory only.  An event larger than the cache is streamed from
+// global memory through the same code (generic pointers).
+//   step 1  objects of the run -> shared memory (coalesced); isolation outputs of non-leptons zeroed
+//   step 2  H_T and E_T^miss: a warp per event, lanes over its objects, exact 64-bit fixed-point sums
+//   step 3  isolation: a warp per lepton, lanes over the objects of its event, three exact fixed-point sums
+// Fixed-point sums (units of 2^-32 GeV) are associative: results do not depend on the order of the objects,
+// the chunking or the launch shape.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "pd_internal.h"
+
+namespace pdf {
+
+constexpr int THREADS = 256;
+constexpr int W = THREADS / 32;
+constexpr int CAP = 3456;         // objects cached per run
+constexpr int RUN_EVENTS = 256;   // events per run at most
+constexpr float kPi = 3.14159265358979323846f;
+constexpr float kTwoPi = 6.28318530717958647692f;
+constexpr double kInvFix = 2.3283064365386963e-10;  // 2^-32
+
+__device__ __forceinline__ long long warp_sum_ll(long long v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ long long to_fix(float x) { return __float2ll_rn(x * 4294967296.f); }
+
+__global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_constant__ PdFeatParams prm,
+                                                                 int events_per_chunk, long long n_chunks) {
+  __shared__ float s_pt[CAP], s_eta[CAP], s_phi[CAP];
+  __shared__ signed char s_cls[CAP];
+  __shared__ int s_off[RUN_EVENTS + 1];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+
+  for (long long chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
+    const long long c0 = chunk * events_per_chunk;
+    const long long c1 = min(c0 + (long long)events_per_chunk, prm.n_events);
+    long long e0 = c0;
+    while (e0 < c1) {
+      // ---- the run [e0, e0 + ne): as many whole events as fit the cache (offsets are non-decreasing)
+      const long long a0 = __ldg(prm.offsets + e0);
+      bool fits_t = false;
+      if (e0 + tid + 1 <= c1) fits_t = __ldg(prm.offsets + e0 + tid + 1) - a0 <= (long long)CAP;
+      int ne = __syncthreads_count(fits_t);
+      const bool cached = ne > 0;  // else: one event larger than the cache, streamed from global memory
+      if (!cached) ne = 1;
+      for (int e = tid; e <= ne; e += THREADS) s_off[e] = (int)min(__ldg(prm.offsets + e0 + e) - a0, (long long)0x7fffffff);
+      __syncthreads();
+      const int n = s_off[ne];
+      const float *o_pt = cached ? s_pt : prm.pt + a0, *o_eta = cached ? s_eta : prm.eta + a0,
+                  *o_phi = cached ? s_phi : prm.phi + a0;
+      const signed char *o_cls = cached ? s_cls : prm.cls + a0;
+
+      // ---- step 1: cache the run; zero the isolation of everything that is not a lepton
+      for (int i = tid; i < n; i += THREADS) {
+        const signed char c = __ldg(prm.cls + a0 + i);
+        if (cached) {
+          s_cls[i] = c;
+          s_pt[i] = __ldg(prm.pt + a0 + i), s_eta[i] = __ldg(prm.eta + a0 + i), s_phi[i] = __ldg(prm.phi + a0 + i);
+        }
+        if (c != PD_CLS_ELECTRON && c != PD_CLS_MUON) {
+          prm.iso_charged[a0 + i] = 0.f, prm.iso_neutral[a0 + i] = 0.f, prm.iso_photon[a0 + i] = 0.f;
+          prm.r_iso[a0 + i] = 0.f;
+        }
+      }
+      __syncthreads();
+
+      // ---- step 2: H_T and E_T^miss, a warp per event
+      for (int e = wid; e < ne; e += W) {
+        long long s_ht = 0, s_x = 0, s_y = 0;
+        for (int i = s_off[e] + lane; i < s_off[e + 1]; i += 32) {
+          const float pt = o_pt[i];
+          float sn, cs;
+          sincosf(o_phi[i], &sn, &cs);
+          s_ht += to_fix(pt), s_x += to_fix(pt * cs), s_y += to_fix(pt * sn);
+        }
+        s_ht = warp_sum_ll(s_ht), s_x = warp_sum_ll(s_x), s_y = warp_sum_ll(s_y);
+        if (lane == 0) {
+          const double mx = -(double)s_x * kInvFix, my = -(double)s_y * kInvFix;
+          prm.ht[e0 + e] = (float)((double)s_ht * kInvFix);
+          prm.met_x[e0 + e] = (float)mx, prm.met_y[e0 + e] = (float)my;
+          prm.met[e0 + e] = (float)sqrt(mx * mx + my * my);
+        }
+      }
+
+      // ---- step 3: Eq. 1, a warp per lepton (the class test is warp-uniform), lanes over its event
+      for (int e = 0; e < ne; ++e) {
+        const int ea = s_off[e], eb = s_off[e + 1];
+        for (int i = ea + wid; i < eb; i += W) {
+          const signed char ci = o_cls[i];
+          if (ci != PD_CLS_ELECTRON && ci != PD_CLS_MUON) continue;
+          const float eta_i = o_eta[i], phi_i = o_phi[i];
+          long long s_ch = 0, s_nh = 0, s_ph = 0;
+          for (int j = ea + lane; j < eb; j += 32) {
+            const float deta = o_eta[j] - eta_i;
+            float dphi = o_phi[j] - phi_i;
+            dphi = dphi > kPi ? dphi - kTwoPi : (dphi <= -kPi ? dphi + kTwoPi : dphi);
+            const float dr2 = fmaf(deta, deta, dphi * dphi);
+            const int cj = (int)o_cls[j];
+            const long long fx = (dr2 < prm.dr_max2 && j != i) ? to_fix(o_pt[j]) : 0ll;
+            s_ch += cj <= PD_CLS_MUON ? fx : 0ll;
+            s_nh += cj == PD_CLS_NEUHAD ? fx : 0ll;
+            s_ph += (cj == PD_CLS_PHOTON && !(dr2 < prm.fsr2)) ? fx : 0ll;
+          }
+          s_ch = warp_sum_ll(s_ch), s_nh = warp_sum_ll(s_nh), s_ph = warp_sum_ll(s_ph);
+          if (lane == 0) {
+            prm.iso_charged[a0 + i] = (float)((double)s_ch * kInvFix);
+            prm.iso_neutral[a0 + i] = (float)((double)s_nh * kInvFix);
+            prm.iso_photon[a0 + i] = (float)((double)s_ph * kInvFix);
+            prm.r_iso[a0 + i] = (float)((double)(s_ch + s_nh + s_ph) * kInvFix / (double)o_pt[i]);
+          }
+        }
+      }
+      __syncthreads();  // the cache is reused by the next run
+      e0 += ne;
+    }
+  }
+}
+
+}  // namespace pdf
+
+int pd_launch_features(const PdFeatParams &prm, void *stream) {
+  if (prm.n_events <= 0) return PD_OK;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PD_ECUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PD_ECUDA;
+  const long long ctas = 3LL * sms;
+  // chunks of consecutive events, about eight per resident CTA, at most one run's worth of events each
+  long long epc = (prm.n_events + 8 * ctas - 1) / (8 * ctas);
+  if (epc < 1) epc = 1;
+  if (epc > pdf::RUN_EVENTS) epc = pdf::RUN_EVENTS;
+  const long long n_chunks = (prm.n_events + epc - 1) / epc;
+  const long long grid = n_chunks < ctas ? n_chunks : ctas;
+  pdf::pd_features_kernel<<<(unsigned)grid, pdf::THREADS, 0, (cudaStream_t)stream>>>(prm, (int)epc, n_chunks);
+  return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
+}

@@ -134,3 +134,15 @@ struct PdLaunchPlan {
 int pd_plan_set_tile_events(int g);
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);
 int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, void *stream);
+
+// pd_features.cu: event features + lepton isolation (pd_event_features)
+struct PdFeatParams {
+  long long n_events;
+  const long long *offsets;
+  const signed char *cls;
+  const float *pt, *eta, *phi;
+  float dr_max2, fsr2;  // squared cone radii (rounded to fp32 from double)
+  float *ht, *met_x, *met_y, *met;
+  float *iso_charged, *iso_neutral, *iso_photon, *r_iso;
+};
+int pd_launch_features(const PdFeatParams &prm, void *stream);
