@@ -225,6 +225,22 @@ def run_ours(args, rank, world, local_rank):
     e2e_value = world * n / float(t.item())
     h2d, d2h = hb.h2d_bytes(), hb.d2h_bytes()
 
+    # ---- the next step after the hot path: event features + lepton isolation on the EFlow
+    # collection the chain just produced (device-resident).  Reported beside the step, not part of it.
+    feat = pd.DeviceFeatures(ne, 2 * max(n, 1))
+    for _ in range(2):
+        pd.event_features(out, feat)
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    f_steps = max(1, min(args.steps, 5))
+    f0.record(stream)
+    for _ in range(f_steps):
+        pd.event_features(out, feat)
+    f1.record(stream)
+    barrier()
+    feat_ms = f0.elapsed_time(f1) / f_steps
+    del feat
+
     if dist is not None:
         # CSR rebasing of shard outputs: one all-gather of three int64 per rank, outside the data path
         from paper_2606_26089_b200 import shard
@@ -256,6 +272,10 @@ def run_ours(args, rank, world, local_rank):
         "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": cpu_what},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
         "gpu_launches": launches, "clocks": clk,
+        "next": {"event_features": {"ms": feat_ms, "objects_per_s": totals[2] / (feat_ms * 1e-3), "kernel": "pd_features_kernel",
+                                    "algorithmic_bytes": 29 * totals[2] + 24 * ne,
+                                    "hbm_frac": (29 * totals[2] + 24 * ne) / (feat_ms * 1e-3) / 1e9 / peak,
+                                    "note": "H_T, MET, lepton isolation (Eq. 1) on the step's EFlow output; rank 0, not in value"}},
     }
     print(json.dumps(line))
     if dist is not None:

@@ -22,25 +22,119 @@ namespace pdf {
 
 constexpr int THREADS = 256;
 constexpr int W = THREADS / 32;
-constexpr int CAP = 3456;         // objects cached per run
+constexpr int CAP = 3072;         // objects cached per run
 constexpr int RUN_EVENTS = 256;   // events per run at most
 constexpr float kPi = 3.14159265358979323846f;
 constexpr float kTwoPi = 6.28318530717958647692f;
 constexpr double kInvFix = 2.3283064365386963e-10;  // 2^-32
 
+// Sum of a 64-bit integer over the warp (two's complement, modulo 2^64) with three integer REDUX instructions
+// instead of ten dependent shuffles: pieces of 24 + 24 + 16 bits cannot overflow 32 bits when 32 of them are added.
 __device__ __forceinline__ long long warp_sum_ll(long long v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
+  const unsigned long long u = (unsigned long long)v;
+  const unsigned a = __reduce_add_sync(0xffffffffu, (unsigned)(u & 0xffffffu));
+  const unsigned b = __reduce_add_sync(0xffffffffu, (unsigned)((u >> 24) & 0xffffffu));
+  const unsigned c = __reduce_add_sync(0xffffffffu, (unsigned)(u >> 48));
+  return (long long)((unsigned long long)a + ((unsigned long long)b << 24) + ((unsigned long long)c << 48));
 }
 __device__ __forceinline__ long long to_fix(float x) { return __float2ll_rn(x * 4294967296.f); }
+
+// Steps 2 and 3 for one run.  Two instances: the objects in shared memory (plain LDS addressing) or, for an event
+// larger than the cache, in global memory.
+template <typename PF, typename PC>
+__device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, PF o_eta, PF o_phi, PC o_cls, const int *s_off,
+                                             unsigned long long *s_acc, const unsigned short *s_lep, int n_lep, int ne, int n, long long e0,
+                                             long long a0) {
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  // ---- step 2: H_T and E_T^miss.  A run that is one big event: all warps share it (integer atomics in
+  // shared memory); otherwise a warp per event.
+  if (ne == 1 && n > 8 * 32) {
+    long long s_ht = 0, s_x = 0, s_y = 0;
+    for (int i = tid; i < n; i += THREADS) {
+      const float pt = o_pt[i];
+      float sn, cs;
+      sincosf(o_phi[i], &sn, &cs);
+      s_ht += to_fix(pt), s_x += to_fix(pt * cs), s_y += to_fix(pt * sn);
+    }
+    s_ht = warp_sum_ll(s_ht), s_x = warp_sum_ll(s_x), s_y = warp_sum_ll(s_y);
+    if (lane == 0) {
+      atomicAdd(&s_acc[0], (unsigned long long)s_ht);
+      atomicAdd(&s_acc[1], (unsigned long long)s_x);
+      atomicAdd(&s_acc[2], (unsigned long long)s_y);
+    }
+  } else
+  for (int e = wid; e < ne; e += W) {
+    long long s_ht = 0, s_x = 0, s_y = 0;
+    for (int i = s_off[e] + lane; i < s_off[e + 1]; i += 32) {
+      const float pt = o_pt[i];
+      float sn, cs;
+      sincosf(o_phi[i], &sn, &cs);
+      s_ht += to_fix(pt), s_x += to_fix(pt * cs), s_y += to_fix(pt * sn);
+    }
+    s_ht = warp_sum_ll(s_ht), s_x = warp_sum_ll(s_x), s_y = warp_sum_ll(s_y);
+    if (lane == 0) {
+      const double mx = -(double)s_x * kInvFix, my = -(double)s_y * kInvFix;
+      prm.ht[e0 + e] = (float)((double)s_ht * kInvFix);
+      prm.met_x[e0 + e] = (float)mx, prm.met_y[e0 + e] = (float)my;
+      prm.met[e0 + e] = (float)sqrt(mx * mx + my * my);
+    }
+  }
+
+  // ---- step 3: Eq. 1, a warp per lepton, lanes over the objects of its event
+  auto isolate = [&](int i, int ea, int eb) {
+    const float eta_i = o_eta[i], phi_i = o_phi[i];
+    long long s_ch = 0, s_nh = 0, s_ph = 0;
+    for (int j = ea + lane; j < eb; j += 32) {
+      const float deta = o_eta[j] - eta_i;
+      float dphi = o_phi[j] - phi_i;
+      dphi = dphi > kPi ? dphi - kTwoPi : (dphi <= -kPi ? dphi + kTwoPi : dphi);
+      const float dr2 = fmaf(deta, deta, dphi * dphi);
+      if (dr2 < prm.dr_max2 && j != i) {  // rare (the cone is ~1 % of the acceptance): the sums stay off the common path
+        const int cj = (int)o_cls[j];
+        const long long fx = to_fix(o_pt[j]);
+        if (cj <= PD_CLS_MUON) s_ch += fx;
+        else if (cj == PD_CLS_NEUHAD) s_nh += fx;
+        else if (!(dr2 < prm.fsr2)) s_ph += fx;
+      }
+    }
+    s_ch = warp_sum_ll(s_ch), s_nh = warp_sum_ll(s_nh), s_ph = warp_sum_ll(s_ph);
+    if (lane == 0) {
+      prm.iso_charged[a0 + i] = (float)((double)s_ch * kInvFix);
+      prm.iso_neutral[a0 + i] = (float)((double)s_nh * kInvFix);
+      prm.iso_photon[a0 + i] = (float)((double)s_ph * kInvFix);
+      prm.r_iso[a0 + i] = (float)((double)(s_ch + s_nh + s_ph) * kInvFix / (double)o_pt[i]);
+    }
+  };
+  if (s_lep != nullptr) {
+    // cached run: the leptons were listed by step 1; its event is found by bisection of the run's offsets
+    for (int k = wid; k < n_lep; k += W) {
+      const int i = (int)s_lep[k];
+      int lo = 0, hi = ne;  // s_off[lo] <= i < s_off[hi]
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (s_off[mid] <= i) lo = mid;
+        else hi = mid;
+      }
+      isolate(i, s_off[lo], s_off[lo + 1]);
+    }
+  } else {
+    // an event larger than the cache: every warp looks for the leptons among its share of the objects
+    for (int i = wid; i < n; i += W) {
+      const signed char ci = o_cls[i];
+      if (ci == PD_CLS_ELECTRON || ci == PD_CLS_MUON) isolate(i, 0, n);
+    }
+  }
+}
 
 __global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_constant__ PdFeatParams prm,
                                                                  int events_per_chunk, long long n_chunks) {
   __shared__ float s_pt[CAP], s_eta[CAP], s_phi[CAP];
   __shared__ signed char s_cls[CAP];
   __shared__ int s_off[RUN_EVENTS + 1];
-  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  __shared__ unsigned short s_lep[CAP];    // the run's leptons (indices into the cache), in arrival order
+  __shared__ unsigned s_nlep;
+  __shared__ unsigned long long s_acc[3];  // H_T, sum pT cos, sum pT sin of a run that is one big event
+  const int tid = threadIdx.x;
 
   for (long long chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
     const long long c0 = chunk * events_per_chunk;
@@ -54,12 +148,11 @@ __global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_co
       int ne = __syncthreads_count(fits_t);
       const bool cached = ne > 0;  // else: one event larger than the cache, streamed from global memory
       if (!cached) ne = 1;
+      if (tid < 3) s_acc[tid] = 0ull;
+      if (tid == 3) s_nlep = 0u;
       for (int e = tid; e <= ne; e += THREADS) s_off[e] = (int)min(__ldg(prm.offsets + e0 + e) - a0, (long long)0x7fffffff);
       __syncthreads();
       const int n = s_off[ne];
-      const float *o_pt = cached ? s_pt : prm.pt + a0, *o_eta = cached ? s_eta : prm.eta + a0,
-                  *o_phi = cached ? s_phi : prm.phi + a0;
-      const signed char *o_cls = cached ? s_cls : prm.cls + a0;
 
       // ---- step 1: cache the run; zero the isolation of everything that is not a lepton
       for (int i = tid; i < n; i += THREADS) {
@@ -68,60 +161,24 @@ __global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_co
           s_cls[i] = c;
           s_pt[i] = __ldg(prm.pt + a0 + i), s_eta[i] = __ldg(prm.eta + a0 + i), s_phi[i] = __ldg(prm.phi + a0 + i);
         }
-        if (c != PD_CLS_ELECTRON && c != PD_CLS_MUON) {
+        if (c == PD_CLS_ELECTRON || c == PD_CLS_MUON) {
+          if (cached) s_lep[atomicAdd(&s_nlep, 1u)] = (unsigned short)i;
+        } else {
           prm.iso_charged[a0 + i] = 0.f, prm.iso_neutral[a0 + i] = 0.f, prm.iso_photon[a0 + i] = 0.f;
           prm.r_iso[a0 + i] = 0.f;
         }
       }
       __syncthreads();
 
-      // ---- step 2: H_T and E_T^miss, a warp per event
-      for (int e = wid; e < ne; e += W) {
-        long long s_ht = 0, s_x = 0, s_y = 0;
-        for (int i = s_off[e] + lane; i < s_off[e + 1]; i += 32) {
-          const float pt = o_pt[i];
-          float sn, cs;
-          sincosf(o_phi[i], &sn, &cs);
-          s_ht += to_fix(pt), s_x += to_fix(pt * cs), s_y += to_fix(pt * sn);
-        }
-        s_ht = warp_sum_ll(s_ht), s_x = warp_sum_ll(s_x), s_y = warp_sum_ll(s_y);
-        if (lane == 0) {
-          const double mx = -(double)s_x * kInvFix, my = -(double)s_y * kInvFix;
-          prm.ht[e0 + e] = (float)((double)s_ht * kInvFix);
-          prm.met_x[e0 + e] = (float)mx, prm.met_y[e0 + e] = (float)my;
-          prm.met[e0 + e] = (float)sqrt(mx * mx + my * my);
-        }
-      }
-
-      // ---- step 3: Eq. 1, a warp per lepton (the class test is warp-uniform), lanes over its event
-      for (int e = 0; e < ne; ++e) {
-        const int ea = s_off[e], eb = s_off[e + 1];
-        for (int i = ea + wid; i < eb; i += W) {
-          const signed char ci = o_cls[i];
-          if (ci != PD_CLS_ELECTRON && ci != PD_CLS_MUON) continue;
-          const float eta_i = o_eta[i], phi_i = o_phi[i];
-          long long s_ch = 0, s_nh = 0, s_ph = 0;
-          for (int j = ea + lane; j < eb; j += 32) {
-            const float deta = o_eta[j] - eta_i;
-            float dphi = o_phi[j] - phi_i;
-            dphi = dphi > kPi ? dphi - kTwoPi : (dphi <= -kPi ? dphi + kTwoPi : dphi);
-            const float dr2 = fmaf(deta, deta, dphi * dphi);
-            const int cj = (int)o_cls[j];
-            const long long fx = (dr2 < prm.dr_max2 && j != i) ? to_fix(o_pt[j]) : 0ll;
-            s_ch += cj <= PD_CLS_MUON ? fx : 0ll;
-            s_nh += cj == PD_CLS_NEUHAD ? fx : 0ll;
-            s_ph += (cj == PD_CLS_PHOTON && !(dr2 < prm.fsr2)) ? fx : 0ll;
-          }
-          s_ch = warp_sum_ll(s_ch), s_nh = warp_sum_ll(s_nh), s_ph = warp_sum_ll(s_ph);
-          if (lane == 0) {
-            prm.iso_charged[a0 + i] = (float)((double)s_ch * kInvFix);
-            prm.iso_neutral[a0 + i] = (float)((double)s_nh * kInvFix);
-            prm.iso_photon[a0 + i] = (float)((double)s_ph * kInvFix);
-            prm.r_iso[a0 + i] = (float)((double)(s_ch + s_nh + s_ph) * kInvFix / (double)o_pt[i]);
-          }
-        }
-      }
+      if (cached) run_features(prm, (const float *)s_pt, (const float *)s_eta, (const float *)s_phi, (const signed char *)s_cls, s_off, s_acc, s_lep, (int)s_nlep, ne, n, e0, a0);
+      else run_features(prm, prm.pt + a0, prm.eta + a0, prm.phi + a0, prm.cls + a0, s_off, s_acc, (const unsigned short *)nullptr, 0, ne, n, e0, a0);
       __syncthreads();  // the cache is reused by the next run
+      if (ne == 1 && n > 8 * 32 && tid == 0) {
+        const double mx = -(double)(long long)s_acc[1] * kInvFix, my = -(double)(long long)s_acc[2] * kInvFix;
+        prm.ht[e0] = (float)((double)(long long)s_acc[0] * kInvFix);
+        prm.met_x[e0] = (float)mx, prm.met_y[e0] = (float)my;
+        prm.met[e0] = (float)sqrt(mx * mx + my * my);
+      }
       e0 += ne;
     }
   }
