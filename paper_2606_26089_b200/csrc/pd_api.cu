@@ -108,6 +108,7 @@ int pd_event_features(const pd_eflow *efl, int64_t n_events, float dr_max, float
   p.offsets = (const long long *)efl->offsets;
   p.cls = efl->cls, p.pt = efl->pt, p.eta = efl->eta, p.phi = efl->phi;
   p.dr_max2 = (float)((double)dr_max * (double)dr_max), p.fsr2 = (float)((double)fsr_dr * (double)fsr_dr);
+  p.inv_strip = 1.f / std::fmax(dr_max * 1.000001f, 0.375f);  // strip width >= dr_max (with a ulp of margin)
   p.ht = out->ht, p.met_x = out->met_x, p.met_y = out->met_y, p.met = out->met;
   p.iso_charged = out->iso_charged, p.iso_neutral = out->iso_neutral, p.iso_photon = out->iso_photon, p.r_iso = out->r_iso;
   const int rc = pd_launch_features(p, cuda_stream);

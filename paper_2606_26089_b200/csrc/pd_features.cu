@@ -6,10 +6,12 @@
 // (three per SM) walks over chunks of consecutive events (static, strided assignment); inside a chunk it takes
 // RUNS of whole events whose objects fit its shared-memory cache (pT, eta, phi, class: 13 bytes per object), so
 // the O(leptons x objects) cone sums read shared memory only.  An event larger than the cache is streamed from
-// global memory through the same code (generic pointers).
-//   step 1  objects of the run -> shared memory (coalesced); isolation outputs of non-leptons zeroed
-//   step 2  H_T and E_T^miss: a warp per event, lanes over its objects, exact 64-bit fixed-point sums
-//   step 3  isolation: a warp per lepton, lanes over the objects of its event, three exact fixed-point sums
+// global memory through a second instance of the same code.
+//   step 1  objects of the run -> shared memory (coalesced); leptons listed; isolation of non-leptons zeroed
+//   step 1b a run that is one big event: counting sort of its object indices by eta strip (width >= dr_max), so
+//           that a lepton only meets the objects of its own strip and the two next to it
+//   step 2  H_T and E_T^miss: a warp per event (all warps for one big event), exact 64-bit fixed-point sums
+//   step 3  isolation: a warp per lepton, lanes over the candidate objects, three exact fixed-point sums
 // Fixed-point sums (units of 2^-32 GeV) are associative: results do not depend on the order of the objects,
 // the chunking or the launch shape.
 #include <cuda_runtime.h>
@@ -24,6 +26,9 @@ constexpr int THREADS = 256;
 constexpr int W = THREADS / 32;
 constexpr int CAP = 3072;         // objects cached per run
 constexpr int RUN_EVENTS = 256;   // events per run at most
+constexpr int N_STRIPS = 32;      // eta strips of a big event (cone pre-selection)
+constexpr int STRIP_MIN_OBJECTS = 512;
+constexpr int SMEM_BYTES = 17 * CAP;  // pT, eta, phi (4 B each), lepton list, strip list (2 B each), class (1 B)
 constexpr float kPi = 3.14159265358979323846f;
 constexpr float kTwoPi = 6.28318530717958647692f;
 constexpr double kInvFix = 2.3283064365386963e-10;  // 2^-32
@@ -38,13 +43,17 @@ __device__ __forceinline__ long long warp_sum_ll(long long v) {
   return (long long)((unsigned long long)a + ((unsigned long long)b << 24) + ((unsigned long long)c << 48));
 }
 __device__ __forceinline__ long long to_fix(float x) { return __float2ll_rn(x * 4294967296.f); }
+// eta strip of an object: N_STRIPS strips of width 1 / inv_strip >= dr_max from eta = -6, the outer ones open-ended
+__device__ __forceinline__ int eta_strip(float eta, float inv_strip) {
+  return min(max((int)floorf((eta + 6.f) * inv_strip), 0), N_STRIPS - 1);
+}
 
 // Steps 2 and 3 for one run.  Two instances: the objects in shared memory (plain LDS addressing) or, for an event
 // larger than the cache, in global memory.
 template <typename PF, typename PC>
 __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, PF o_eta, PF o_phi, PC o_cls, const int *s_off,
-                                             unsigned long long *s_acc, const unsigned short *s_lep, int n_lep, int ne, int n, long long e0,
-                                             long long a0) {
+                                             unsigned long long *s_acc, const unsigned short *s_lep, int n_lep, const unsigned short *s_idx,
+                                             const int *s_sstart, int ne, int n, long long e0, long long a0) {
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   // ---- step 2: H_T and E_T^miss.  A run that is one big event: all warps share it (integer atomics in
   // shared memory); otherwise a warp per event.
@@ -84,7 +93,14 @@ __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, P
   auto isolate = [&](int i, int ea, int eb) {
     const float eta_i = o_eta[i], phi_i = o_phi[i];
     long long s_ch = 0, s_nh = 0, s_ph = 0;
-    for (int j = ea + lane; j < eb; j += 32) {
+    if (s_idx != nullptr) {
+      // one big event, its objects listed by eta strip (strip width >= dr_max): only the lepton's strip and its two
+      // neighbours can hold objects of the cone; they are contiguous in the list
+      const int st = eta_strip(eta_i, prm.inv_strip);
+      ea = s_sstart[max(st - 1, 0)], eb = s_sstart[min(st + 2, N_STRIPS)];
+    }
+    for (int jj = ea + lane; jj < eb; jj += 32) {
+      const int j = s_idx != nullptr ? (int)s_idx[jj] : jj;
       const float deta = o_eta[j] - eta_i;
       float dphi = o_phi[j] - phi_i;
       dphi = dphi > kPi ? dphi - kTwoPi : (dphi <= -kPi ? dphi + kTwoPi : dphi);
@@ -128,13 +144,16 @@ __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, P
 
 __global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_constant__ PdFeatParams prm,
                                                                  int events_per_chunk, long long n_chunks) {
-  __shared__ float s_pt[CAP], s_eta[CAP], s_phi[CAP];
-  __shared__ signed char s_cls[CAP];
+  extern __shared__ __align__(16) unsigned char fsm[];
+  float *s_pt = (float *)fsm, *s_eta = s_pt + CAP, *s_phi = s_eta + CAP;
+  unsigned short *s_lep = (unsigned short *)(s_phi + CAP);  // the run's leptons (indices into the cache), in arrival order
+  unsigned short *s_idx = s_lep + CAP;                       // a big event's objects listed by eta strip
+  signed char *s_cls = (signed char *)(s_idx + CAP);
   __shared__ int s_off[RUN_EVENTS + 1];
-  __shared__ unsigned short s_lep[CAP];    // the run's leptons (indices into the cache), in arrival order
+  __shared__ int s_scnt[N_STRIPS], s_sstart[N_STRIPS + 1];
   __shared__ unsigned s_nlep;
   __shared__ unsigned long long s_acc[3];  // H_T, sum pT cos, sum pT sin of a run that is one big event
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
 
   for (long long chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
     const long long c0 = chunk * events_per_chunk;
@@ -150,6 +169,7 @@ __global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_co
       if (!cached) ne = 1;
       if (tid < 3) s_acc[tid] = 0ull;
       if (tid == 3) s_nlep = 0u;
+      if (tid >= 32 && tid < 32 + N_STRIPS) s_scnt[tid - 32] = 0;
       for (int e = tid; e <= ne; e += THREADS) s_off[e] = (int)min(__ldg(prm.offsets + e0 + e) - a0, (long long)0x7fffffff);
       __syncthreads();
       const int n = s_off[ne];
@@ -169,9 +189,33 @@ __global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_co
         }
       }
       __syncthreads();
+      const bool strips = cached && ne == 1 && n >= STRIP_MIN_OBJECTS;
+      if (strips) {
+        // counting sort of the event's object indices by eta strip (integer atomics; the order inside a strip is
+        // arbitrary and irrelevant: the cone sums are exact)
+        for (int i = tid; i < n; i += THREADS) atomicAdd(&s_scnt[eta_strip(s_eta[i], prm.inv_strip)], 1);
+        __syncthreads();
+        if (wid == 0) {
+          const int c = s_scnt[lane];
+          int incl = c;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+          }
+          s_sstart[lane + 1] = incl;
+          if (lane == 0) s_sstart[0] = 0;
+          s_scnt[lane] = incl - c;  // running write position of the strip
+        }
+        __syncthreads();
+        for (int i = tid; i < n; i += THREADS) s_idx[atomicAdd(&s_scnt[eta_strip(s_eta[i], prm.inv_strip)], 1)] = (unsigned short)i;
+        __syncthreads();
+      }
 
-      if (cached) run_features(prm, (const float *)s_pt, (const float *)s_eta, (const float *)s_phi, (const signed char *)s_cls, s_off, s_acc, s_lep, (int)s_nlep, ne, n, e0, a0);
-      else run_features(prm, prm.pt + a0, prm.eta + a0, prm.phi + a0, prm.cls + a0, s_off, s_acc, (const unsigned short *)nullptr, 0, ne, n, e0, a0);
+      if (cached) run_features(prm, (const float *)s_pt, (const float *)s_eta, (const float *)s_phi, (const signed char *)s_cls, s_off, s_acc, s_lep, (int)s_nlep,
+                               strips ? (const unsigned short *)s_idx : (const unsigned short *)nullptr, s_sstart, ne, n, e0, a0);
+      else run_features(prm, prm.pt + a0, prm.eta + a0, prm.phi + a0, prm.cls + a0, s_off, s_acc, (const unsigned short *)nullptr, 0, (const unsigned short *)nullptr, s_sstart,
+                        ne, n, e0, a0);
       __syncthreads();  // the cache is reused by the next run
       if (ne == 1 && n > 8 * 32 && tid == 0) {
         const double mx = -(double)(long long)s_acc[1] * kInvFix, my = -(double)(long long)s_acc[2] * kInvFix;
@@ -198,6 +242,11 @@ int pd_launch_features(const PdFeatParams &prm, void *stream) {
   if (epc > pdf::RUN_EVENTS) epc = pdf::RUN_EVENTS;
   const long long n_chunks = (prm.n_events + epc - 1) / epc;
   const long long grid = n_chunks < ctas ? n_chunks : ctas;
-  pdf::pd_features_kernel<<<(unsigned)grid, pdf::THREADS, 0, (cudaStream_t)stream>>>(prm, (int)epc, n_chunks);
+  static bool configured = false;
+  if (!configured) {
+    if (cudaFuncSetAttribute(pdf::pd_features_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pdf::SMEM_BYTES) != cudaSuccess) return PD_ECUDA;
+    configured = true;
+  }
+  pdf::pd_features_kernel<<<(unsigned)grid, pdf::THREADS, pdf::SMEM_BYTES, (cudaStream_t)stream>>>(prm, (int)epc, n_chunks);
   return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
 }

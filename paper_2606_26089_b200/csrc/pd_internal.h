@@ -142,6 +142,7 @@ struct PdFeatParams {
   const signed char *cls;
   const float *pt, *eta, *phi;
   float dr_max2, fsr2;  // squared cone radii (rounded to fp32 from double)
+  float inv_strip;      // 1 / width of the eta strips that pre-select cone candidates (width >= dr_max)
   float *ht, *met_x, *met_y, *met;
   float *iso_charged, *iso_neutral, *iso_photon, *r_iso;
 };

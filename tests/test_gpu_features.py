@@ -77,6 +77,11 @@ def test_dense_random_collections_and_edge_cases():
     args = _random_objects(5, sizes)
     for dr_max, fsr in ((0.4, 0.0), (0.4, 0.1), (0.0, 0.0), (10.0, 0.0)):
         _check(_run_gpu(*args, dr_max, fsr), pdo.event_features(*args, dr_max, fsr), args[2])
+    # single big events per run (eta-strip pre-selection), wide eta range incl. beyond the strips' span, cones
+    # narrower and wider than the minimum strip width
+    args = _random_objects(7, [2500, 3000, 3072, 600, 2900], eta_max=7.0, lepton_frac=0.05)
+    for dr_max, fsr in ((0.4, 0.0), (0.2, 0.05), (1.0, 0.0), (0.375, 0.0), (0.0, 0.0)):
+        _check(_run_gpu(*args, dr_max, fsr), pdo.event_features(*args, dr_max, fsr), args[2])
     # many small events (several runs per chunk, several chunks per CTA)
     args = _random_objects(6, np.random.default_rng(1).poisson(30, 20000))
     _check(_run_gpu(*args), pdo.event_features(*args), args[2])
