@@ -149,7 +149,7 @@ int pd_simulate(const pd_card *card, const pd_events *events, uint64_t seed, int
 int pd_last_status(const void *workspace, void *cuda_stream);
 
 /* ---- Event features and lepton isolation (section 2.4 Eq. 1; L141 Table 2) ----
- * From an EFlow ("PFlow") collection, per event (readings F1, F2 of DESIGN.md section 11):
+ * From an EFlow ("PFlow") collection, per event (readings F1, F2 of DESIGN.md section 10):
  *   ht = sum_i pT_i;  (met_x, met_y) = -(sum_i pT_i cos phi_i, sum_i pT_i sin phi_i);  met = its length;
  * and for every object of class PD_CLS_ELECTRON or PD_CLS_MUON, Eq. 1:
  *   r_iso = (iso_charged + iso_neutral + iso_photon) / pT_lepton, the three terms being the pT sums of the event's

@@ -140,7 +140,7 @@ int pdo_simulate(const pdo_card *card, const pdo_events *ev, uint64_t seed, int6
 /* ---- event features and lepton isolation (section 2.4 Eq. 1, Table 2) ----
  * Computed from an EFlow ("PFlow") collection in CSR form, per event:
  *   H_T = sum_i pT_i,   E_T^miss vector = -( sum_i pT_i cos phi_i, sum_i pT_i sin phi_i ),   E_T^miss = its length
- *   (readings F1, F2 of DESIGN.md section 11: the "cached scalar event features (H_T and E_T^miss)" of P:L119,
+ *   (readings F1, F2 of DESIGN.md section 10: the "cached scalar event features (H_T and E_T^miss)" of P:L119,
  *   "H_T, E_T^miss values for ... PFlow collections" of P:L141, taken over every object of the collection);
  * and, for every object of class electron or muon, Eq. 1 of P:L121-127:
  *   R_iso = ( sum_{dR<dr_max} pT^charged + sum_{dR<dr_max} pT^neutral + sum_{dR<dr_max} pT^gamma ) / pT^lepton,

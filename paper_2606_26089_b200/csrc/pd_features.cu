@@ -1,6 +1,6 @@
 // pd_features.cu -- event features (H_T, E_T^miss) and lepton isolation (Eq. 1 of the paper) from an EFlow
 // collection: the step right after the detector-response chain (
-// readings F1-F4 of DESIGN.md section 11).  Product code; shares nothing with oracle/.
+// readings F1-F4 of DESIGN.md section 10).  Product code; shares nothing with oracle/.
 //
 // Events are independent and nothing is compacted, so there is no chain and no workspace.  A 256-thread CTA
 // (three per SM) walks over chunks of consecutive events (static, strided assignment); inside a chunk it takes

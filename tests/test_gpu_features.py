@@ -2,7 +2,7 @@
 against the fp64 oracle, element by element.  The input collections come from the ORACLE's own chain output and
 from seeded synthetic generators -- never from the CUDA chain.
 
-Tolerances (DESIGN.md section 11): H_T and the isolation sums are exact fixed-point sums of fp32 terms, compared
+Tolerances (DESIGN.md section 10): H_T and the isolation sums are exact fixed-point sums of fp32 terms, compared
 at the north-star 1e-5 relative / 1e-6 absolute; the components of E_T^miss are sums of products pT cos(phi)
 each rounded to fp32 (relative 2^-23, plus a 1e-7 cosine error), so their absolute error scales with H_T, not
 with the (possibly cancelling) result: |g - o| <= 1e-6 H_T + 1e-6.  A cone decision within 1e-6 of its edge may go
