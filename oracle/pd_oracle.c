@@ -943,3 +943,60 @@ int pdo_event_features(const pdo_objects *obj, double dr_max, double fsr_dr, dou
   }
   return PDO_OK;
 }
+
+/* ---- particle filter: see pd_oracle.h (Table C.13) ---- */
+static int pdo_condition_holds(const pdo_condition *c, float x) {
+  int k;
+  if (c->use_abs) x = fabsf(x);
+  switch (c->op) {
+    case PDO_OP_GT: return x > c->value;
+    case PDO_OP_GE: return x >= c->value;
+    case PDO_OP_LT: return x < c->value;
+    case PDO_OP_LE: return x <= c->value;
+    case PDO_OP_EQ: return x == c->value;
+    case PDO_OP_NE: return x != c->value;
+    case PDO_OP_IN:
+      for (k = 0; k < c->n_values; ++k)
+        if (x == c->values[k]) return 1;
+      return 0;
+    case PDO_OP_NOT_IN:
+      for (k = 0; k < c->n_values; ++k)
+        if (x == c->values[k]) return 0;
+      return 1;
+    default: return 0;
+  }
+}
+
+int pdo_filter_eflow(int64_t n_events, const int64_t *offsets, const int8_t *cls, const int32_t *src, const float *pt,
+                     const float *eta, const float *phi, const float *E, const pdo_condition *conds, int32_t n_conds,
+                     int32_t combine_any, int64_t *out_offsets, int8_t *out_cls, int32_t *out_src, float *out_pt,
+                     float *out_eta, float *out_phi, float *out_E, uint8_t *keep) {
+  int64_t e, i, n_out = 0;
+  int32_t k;
+  if (n_events < 0 || !offsets || !out_offsets || n_conds < 0 || (n_conds > 0 && !conds)) return PDO_EINVAL;
+  for (k = 0; k < n_conds; ++k)
+    if (conds[k].field < PDO_FIELD_PT || conds[k].field > PDO_FIELD_CLS || conds[k].op < PDO_OP_GT ||
+        conds[k].op > PDO_OP_NOT_IN || conds[k].n_values < 0 || conds[k].n_values > 8)
+      return PDO_EINVAL;
+  out_offsets[0] = 0;
+  for (e = 0; e < n_events; ++e) {
+    for (i = offsets[e]; i < offsets[e + 1]; ++i) {
+      int n_true = 0, kept;
+      for (k = 0; k < n_conds; ++k) {
+        const pdo_condition *c = &conds[k];
+        const float x = c->field == PDO_FIELD_PT ? pt[i] : c->field == PDO_FIELD_ETA ? eta[i]
+                      : c->field == PDO_FIELD_PHI ? phi[i] : c->field == PDO_FIELD_E ? E[i] : (float)cls[i];
+        n_true += pdo_condition_holds(c, x);
+      }
+      kept = n_conds == 0 ? 1 : (combine_any ? n_true > 0 : n_true == n_conds);
+      if (keep) keep[i] = (uint8_t)kept;
+      if (kept) {
+        out_cls[n_out] = cls[i], out_src[n_out] = src[i];
+        out_pt[n_out] = pt[i], out_eta[n_out] = eta[i], out_phi[n_out] = phi[i], out_E[n_out] = E[i];
+        ++n_out;
+      }
+    }
+    out_offsets[e + 1] = n_out;
+  }
+  return PDO_OK;
+}

@@ -163,6 +163,32 @@ int pdo_event_features(const pdo_objects *obj, double dr_max, double fsr_dr,
                        double *iso_charged, double *iso_neutral, double *iso_photon, double *r_iso, /* [n_objects] */
                        double *iso_amb /* [n_objects], may be NULL */);
 
+/* ---- particle filter (section 2.4, P:L634-647 Table C.13) ----
+ * "Particle filtering drops particles from a target collection in place according to declarative per-field
+ * conditions (e.g. pT, eta, or PDG-ID cuts), combined with logical all (AND) or any (OR) semantics."
+ * A condition is (field, op, value | set of values, abs): the object's attribute (its magnitude if abs) is
+ * compared with `value` by >, >=, <, <=, ==, != or tested for membership in `values` (in, not in).
+ * Attributes of an EFlow object: pt, eta, phi, E (fp32) and the class id (int8, compared as a number).
+ * All comparisons are made on the fp32 values as they are (no arithmetic), hence exactly.  An object is
+ * kept iff all (combine_any = 0) or any (combine_any = 1) of the conditions hold; an empty condition list
+ * keeps everything (reading G1 of DESIGN.md section 11).  Survivors keep their order; the output is the
+ * compacted CSR collection.  (Event features are then recomputed from the survivors with
+ * pdo_event_features -- "update_event_features", Table C.13.) */
+enum { PDO_FIELD_PT = 0, PDO_FIELD_ETA = 1, PDO_FIELD_PHI = 2, PDO_FIELD_E = 3, PDO_FIELD_CLS = 4 };
+enum { PDO_OP_GT = 0, PDO_OP_GE = 1, PDO_OP_LT = 2, PDO_OP_LE = 3, PDO_OP_EQ = 4, PDO_OP_NE = 5, PDO_OP_IN = 6, PDO_OP_NOT_IN = 7 };
+typedef struct {
+  int32_t field, op, use_abs, n_values; /* n_values: members of `values` (in / not in), at most 8 */
+  float value;                          /* scalar comparisons */
+  float values[8];
+} pdo_condition;
+
+/* in: offsets [n_events+1], cls, src, pt, eta, phi, E of the collection; out_*: same arrays with room for
+ * as many objects; out_offsets [n_events+1].  keep (nullable): per input object 1 / 0. */
+int pdo_filter_eflow(int64_t n_events, const int64_t *offsets, const int8_t *cls, const int32_t *src, const float *pt,
+                     const float *eta, const float *phi, const float *E, const pdo_condition *conds, int32_t n_conds,
+                     int32_t combine_any, int64_t *out_offsets, int8_t *out_cls, int32_t *out_src, float *out_pt,
+                     float *out_eta, float *out_phi, float *out_E, uint8_t *keep);
+
 const char *pdo_strerror(int code);
 
 /* ---- building blocks exposed so that tests can pin them one by one ---- */

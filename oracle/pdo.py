@@ -60,6 +60,15 @@ class _Objects(C.Structure):
     _fields_ = [("n_events", C.c_int64), ("offsets", _p), ("cls", _p), ("pt", _p), ("eta", _p), ("phi", _p)]
 
 
+class _Condition(C.Structure):
+    _fields_ = [("field", C.c_int32), ("op", C.c_int32), ("use_abs", C.c_int32), ("n_values", C.c_int32),
+                ("value", C.c_float), ("values", C.c_float * 8)]
+
+
+FIELDS = {"pt": 0, "eta": 1, "phi": 2, "E": 3, "cls": 4}
+OPS = {">": 0, ">=": 1, "<": 2, "<=": 3, "==": 4, "!=": 5, "in": 6, "not in": 7}
+
+
 class _Overrides(C.Structure):
     _fields_ = [("face", _p), ("tower", _p), ("eps_row", _p), ("n_tower_ov", C.c_int64),
                 ("tw_event", _p), ("tw_id", _p), ("tw_mask", _p), ("tw_value", _p), ("n_rejected", _p)]
@@ -96,6 +105,7 @@ def lib():
         L.pdo_tower_index.restype = C.c_int32
         L.pdo_efficiency.argtypes = [_p, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int)]
         L.pdo_efficiency.restype = C.c_double
+        L.pdo_filter_eflow.argtypes = [C.c_int64] + [_p] * 7 + [C.POINTER(_Condition), C.c_int32, C.c_int32] + [_p] * 8
         L.pdo_event_features.argtypes = [C.POINTER(_Objects), C.c_double, C.c_double] + [_p] * 9
         _lib = L
     return _lib
@@ -279,3 +289,41 @@ def event_features(offsets, cls, pt, eta, phi, dr_max: float = 0.4, fsr_dr: floa
     out = {k: v[:ne] for k, v in ev.items()}
     out.update({k: v[:n] for k, v in ob.items()})
     return out
+
+
+def make_conditions(conditions, ctype=_Condition):
+    """[{field, op, value, abs}] (the paper's Table C.13 grammar) -> ctypes array."""
+    arr = (ctype * max(len(conditions), 1))()
+    for k, c in enumerate(conditions):
+        arr[k].field, arr[k].op, arr[k].use_abs = FIELDS[c["field"]], OPS[c["op"]], int(bool(c.get("abs", False)))
+        if c["op"] in ("in", "not in"):
+            vals = list(c["value"])
+            assert len(vals) <= 8
+            arr[k].n_values = len(vals)
+            for j, v in enumerate(vals):
+                arr[k].values[j] = float(v)
+        else:
+            arr[k].n_values, arr[k].value = 0, float(c["value"])
+    return arr
+
+
+def filter_eflow(offsets, cls, src, pt, eta, phi, E, conditions, combine: str = "all") -> dict:
+    """pdo_filter_eflow (Table C.13): returns offsets, cls, src, pt, eta, phi, E of the survivors and keep."""
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    ne, n = int(offsets.shape[0] - 1), int(offsets[-1])
+    cls, src = np.ascontiguousarray(cls, dtype=np.int8), np.ascontiguousarray(src, dtype=np.int32)
+    fl = [np.ascontiguousarray(a, dtype=np.float32) for a in (pt, eta, phi, E)]
+    out = {"offsets": np.zeros(ne + 1, dtype=np.int64), "cls": np.zeros(max(n, 1), dtype=np.int8), "src": np.zeros(max(n, 1), dtype=np.int32)}
+    for k in ("pt", "eta", "phi", "E"):
+        out[k] = np.zeros(max(n, 1), dtype=np.float32)
+    keep = np.zeros(max(n, 1), dtype=np.uint8)
+    conds = make_conditions(conditions)
+    rc = lib().pdo_filter_eflow(ne, _ptr(offsets), _ptr(cls), _ptr(src), *[_ptr(a) for a in fl], conds, len(conditions),
+                                1 if combine == "any" else 0, _ptr(out["offsets"]), _ptr(out["cls"]), _ptr(out["src"]),
+                                _ptr(out["pt"]), _ptr(out["eta"]), _ptr(out["phi"]), _ptr(out["E"]), _ptr(keep))
+    if rc != 0:
+        raise OracleError(rc)
+    m = int(out["offsets"][-1])
+    res = {k: (v if k == "offsets" else v[:m]) for k, v in out.items()}
+    res["keep"] = keep[:n]
+    return res
