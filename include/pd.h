@@ -170,6 +170,34 @@ typedef struct {
 int pd_event_features(const pd_eflow *eflow, int64_t n_events, float dr_max, float fsr_dr, pd_features *out,
                       void *cuda_stream);
 
+/* ---- Particle filter (section 2.4; Table C.13) ----
+ * "Particle filtering drops particles from a target collection ... according to declarative per-field conditions
+ * (e.g. pT, eta, or PDG-ID cuts), combined with logical all (AND) or any (OR) semantics."  Here: the EFlow
+ * ("pflow", the paper's default) collection, as an ordered stream compaction into a second collection.
+ * A condition compares an attribute of the object (its magnitude if use_abs) with `value` (ops >, >=, <, <=,
+ * ==, !=) or tests it for membership in values[0..n_values) (ops in, not in).  Attributes: pt, eta, phi, E
+ * (fp32, compared as they are, hence exactly) and the class id (compared as a number).  An object is kept iff
+ * all (combine_any = 0) or any (combine_any != 0) of the conditions hold; no condition keeps everything.
+ * Survivors keep their order.  The paper's update_event_features is a pd_event_features call on the output. */
+enum { PD_FIELD_PT = 0, PD_FIELD_ETA = 1, PD_FIELD_PHI = 2, PD_FIELD_E = 3, PD_FIELD_CLS = 4 };
+enum { PD_OP_GT = 0, PD_OP_GE = 1, PD_OP_LT = 2, PD_OP_LE = 3, PD_OP_EQ = 4, PD_OP_NE = 5, PD_OP_IN = 6, PD_OP_NOT_IN = 7 };
+enum { PD_MAX_CONDITIONS = 16, PD_MAX_SET_VALUES = 8 };
+typedef struct {
+  int32_t field, op, use_abs, n_values;
+  float value;
+  float values[8];
+} pd_condition;
+
+/* Bytes of DEVICE workspace pd_filter_eflow needs for an input collection of this capacity. */
+int64_t pd_filter_workspace_bytes(int64_t capacity);
+
+/* in, out: structs in HOST memory whose pointer members are DEVICE pointers (in->offsets [n_events+1]; the number
+ * of objects is read on the device).  out->capacity >= in->capacity; out->offsets [n_events+1]; in and out must
+ * not overlap.  conds: HOST array.  Asynchronous on cuda_stream, two kernel launches, allocates nothing.
+ * Errors: PD_EINVAL (null pointers, bad field / op / counts), PD_ECAPACITY, PD_EWORKSPACE, PD_ECUDA. */
+int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *conds, int32_t n_conds, int32_t combine_any,
+                    pd_eflow *out, void *workspace, int64_t workspace_bytes, void *cuda_stream);
+
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 

@@ -18,7 +18,7 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
@@ -31,6 +31,15 @@ class CardInfo(C.Structure):
 
 class Features(C.Structure):
     _fields_ = [(k, _p) for k in ("ht", "met_x", "met_y", "met", "iso_charged", "iso_neutral", "iso_photon", "r_iso")]
+
+
+class Condition(C.Structure):
+    _fields_ = [("field", C.c_int32), ("op", C.c_int32), ("use_abs", C.c_int32), ("n_values", C.c_int32),
+                ("value", C.c_float), ("values", C.c_float * 8)]
+
+
+FIELDS = {"pt": 0, "eta": 1, "phi": 2, "E": 3, "cls": 4}
+OPS = {">": 0, ">=": 1, "<": 2, "<=": 3, "==": 4, "!=": 5, "in": 6, "not in": 7}
 
 
 class Events(C.Structure):
@@ -92,6 +101,10 @@ def lib():
         L.pd_last_status.argtypes = [_p, _p]
         L.pd_last_launch_count.argtypes = []
         L.pd_set_tile_events.argtypes = [C.c_int]
+        L.pd_filter_workspace_bytes.argtypes = [C.c_int64]
+        L.pd_filter_workspace_bytes.restype = C.c_int64
+        L.pd_filter_eflow.argtypes = [C.POINTER(EFlow), C.c_int64, C.POINTER(Condition), C.c_int32, C.c_int32, C.POINTER(EFlow), _p,
+                                      C.c_int64, _p]
         L.pd_event_features.argtypes = [C.POINTER(EFlow), C.c_int64, C.c_float, C.c_float, C.POINTER(Features), _p]
         L.pd_simulate_host.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks),
                                        C.POINTER(Towers), C.POINTER(EFlow), _p]
@@ -249,6 +262,65 @@ class DeviceObjects:
                   "pt": pad(pt, np.float32), "eta": pad(eta, np.float32), "phi": pad(phi, np.float32)}
         self.c_efl = EFlow(self.n_objects, _tptr(self.t["offsets"]), _tptr(self.t["cls"]), None, _tptr(self.t["pt"]),
                            _tptr(self.t["eta"]), _tptr(self.t["phi"]), None)
+
+
+class DeviceEFlow:
+    """An EFlow collection on the device with all its fields: the input (from numpy) or the output (empty, of a
+    given capacity) of pd_filter_eflow; also accepted by event_features."""
+
+    def __init__(self, n_events: int, capacity: int, arrays: dict | None = None, device="cuda"):
+        torch = _torch()
+        import numpy as np
+
+        self.n_events, self.capacity = int(n_events), int(capacity)
+        cap = max(self.capacity, 1)
+        if arrays is None:
+            self.t = {"offsets": torch.empty(self.n_events + 1, dtype=torch.int64, device=device)}
+            self.t.update({k: torch.empty(cap, dtype=getattr(torch, dt), device=device) for k, dt in EFLOW_FIELDS})
+        else:
+            self.t = {"offsets": torch.from_numpy(np.ascontiguousarray(arrays["offsets"], dtype=np.int64)).to(device)}
+            for k, dt in EFLOW_FIELDS:
+                a = np.zeros(cap, dtype=dt)
+                a[: len(arrays[k])] = arrays[k]
+                self.t[k] = torch.from_numpy(a).to(device)
+        self.c_efl = EFlow(self.capacity, _tptr(self.t["offsets"]), *[_tptr(self.t[k]) for k, _ in EFLOW_FIELDS])
+
+    def to_numpy(self) -> dict:
+        _torch().cuda.synchronize()
+        off = self.t["offsets"].cpu().numpy()
+        out = {"offsets": off}
+        out.update({k: self.t[k][: int(off[-1])].cpu().numpy() for k, _ in EFLOW_FIELDS})
+        return out
+
+
+def make_conditions(conditions):
+    """[{field, op, value, abs}] (the paper's Table C.13 grammar) -> ctypes array of pd_condition."""
+    arr = (Condition * max(len(conditions), 1))()
+    for k, c in enumerate(conditions):
+        arr[k].field, arr[k].op, arr[k].use_abs = FIELDS[c["field"]], OPS[c["op"]], int(bool(c.get("abs", False)))
+        if c["op"] in ("in", "not in"):
+            vals = list(c["value"])
+            arr[k].n_values = len(vals)
+            for j, v in enumerate(vals[:8]):
+                arr[k].values[j] = float(v)
+        else:
+            arr[k].n_values, arr[k].value = 0, float(c["value"])
+    return arr
+
+
+def filter_eflow(src, dst: "DeviceEFlow", conditions, combine: str = "all", stream=None):
+    """pd_filter_eflow: `src` is a DeviceOutputs (its EFlow collection) or a DeviceEFlow; survivors go to `dst`.
+    Asynchronous.  Returns the workspace tensor (kept alive by the caller until the stream is synchronised)."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    cap = int(src.c_efl.capacity)
+    nbytes = int(lib().pd_filter_workspace_bytes(cap))
+    ws = torch.empty(nbytes + 16, dtype=torch.uint8, device="cuda")
+    _check(lib().pd_filter_eflow(C.byref(src.c_efl), int(src.n_events), make_conditions(conditions), len(conditions),
+                                 1 if combine == "any" else 0, C.byref(dst.c_efl), _tptr(ws), nbytes, C.c_void_p(st.cuda_stream)))
+    return ws
 
 
 def event_features(out, feat: DeviceFeatures, dr_max: float = 0.4, fsr_dr: float = 0.0, stream=None):

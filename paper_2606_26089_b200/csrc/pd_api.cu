@@ -94,6 +94,57 @@ int pd_last_launch_count(void) { return t_launches; }
 
 int pd_set_tile_events(int g) { return pd_plan_set_tile_events(g); }
 
+// filter workspace: [tile counter, pad] 16 B | look-back words, one per tile | exclusive ranks of positions 0..capacity
+static size_t filter_chain_bytes(int64_t capacity) {
+  const size_t tiles = (size_t)((capacity + 1 + PD_FILTER_TILE - 1) / PD_FILTER_TILE);
+  return (16 + 8 * tiles + 255) & ~size_t(255);
+}
+
+int64_t pd_filter_workspace_bytes(int64_t capacity) {
+  if (capacity < 0) return PD_EINVAL;
+  return (int64_t)(filter_chain_bytes(capacity) + 4 * (size_t)(capacity + 1));
+}
+
+int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *conds, int32_t n_conds, int32_t combine_any,
+                    pd_eflow *out, void *workspace, int64_t workspace_bytes, void *cuda_stream) {
+  t_launches = 0;
+  if (!in || !out || n_events < 0 || n_conds < 0 || n_conds > PD_MAX_CONDITIONS || (n_conds > 0 && !conds)) return PD_EINVAL;
+  if (in->capacity < 0 || in->capacity >= (int64_t(1) << 31) - 1) return PD_EINVAL;
+  if (!in->offsets || !out->offsets) return PD_EINVAL;
+  if (in->capacity > 0) {
+    if (!in->cls || !in->src || !in->pt || !in->eta || !in->phi || !in->E) return PD_EINVAL;
+    if (!out->cls || !out->src || !out->pt || !out->eta || !out->phi || !out->E) return PD_EINVAL;
+  }
+  for (int k = 0; k < n_conds; ++k) {
+    const pd_condition &c = conds[k];
+    if (c.field < PD_FIELD_PT || c.field > PD_FIELD_CLS || c.op < PD_OP_GT || c.op > PD_OP_NOT_IN) return PD_EINVAL;
+    if (c.n_values < 0 || c.n_values > PD_MAX_SET_VALUES) return PD_EINVAL;
+  }
+  if (out->capacity < in->capacity) return PD_ECAPACITY;
+  const int64_t need = pd_filter_workspace_bytes(in->capacity);
+  if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15u)) return PD_EWORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t chain_bytes = filter_chain_bytes(in->capacity);
+  PD_CUDA(cudaMemsetAsync(workspace, 0, chain_bytes, st));
+  PdFilterParams p;
+  std::memset(&p, 0, sizeof(p));
+  p.n_events = n_events;
+  p.offsets = (const long long *)in->offsets;
+  p.cls = in->cls, p.src = in->src, p.pt = in->pt, p.eta = in->eta, p.phi = in->phi, p.E = in->E;
+  p.out_offsets = (long long *)out->offsets;
+  p.out_cls = out->cls, p.out_src = out->src, p.out_pt = out->pt, p.out_eta = out->eta, p.out_phi = out->phi, p.out_E = out->E;
+  for (int k = 0; k < n_conds; ++k) p.conds[k] = conds[k];
+  p.n_conds = n_conds, p.combine_any = combine_any ? 1 : 0;
+  unsigned char *ws = (unsigned char *)workspace;
+  p.tile_counter = (unsigned int *)ws;
+  p.chain = (unsigned long long *)(ws + 16);
+  p.rank = (int *)(ws + chain_bytes);
+  const int rc = pd_launch_filter(p, cuda_stream);
+  if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "filter kernel launch");
+  t_launches = 2;
+  return PD_OK;
+}
+
 int pd_event_features(const pd_eflow *efl, int64_t n_events, float dr_max, float fsr_dr, pd_features *out,
                       void *cuda_stream) {
   t_launches = 0;

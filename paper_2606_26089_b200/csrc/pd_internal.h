@@ -147,3 +147,23 @@ struct PdFeatParams {
   float *iso_charged, *iso_neutral, *iso_photon, *r_iso;
 };
 int pd_launch_features(const PdFeatParams &prm, void *stream);
+
+// pd_filter.cu: particle filter = predicated, ordered stream compaction of an EFlow collection
+constexpr int PD_FILTER_TILE = 2048;  // objects per tile (256 threads x 8)
+struct PdFilterParams {
+  long long n_events;
+  const long long *offsets;
+  const signed char *cls;
+  const int *src;
+  const float *pt, *eta, *phi, *E;
+  long long *out_offsets;
+  signed char *out_cls;
+  int *out_src;
+  float *out_pt, *out_eta, *out_phi, *out_E;
+  pd_condition conds[PD_MAX_CONDITIONS];
+  int n_conds, combine_any;
+  unsigned int *tile_counter;     // workspace: next tile
+  unsigned long long *chain;      // workspace: look-back word per tile
+  int *rank;                      // workspace: exclusive rank of every input position 0..n
+};
+int pd_launch_filter(const PdFilterParams &prm, void *stream);
