@@ -240,6 +240,20 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     feat_ms = f0.elapsed_time(f1) / f_steps
     del feat
+    # ---- the particle filter (pT > 0.5 GeV and |eta| < 2.5, AND) on the same EFlow collection
+    conds = [{"field": "pt", "op": ">", "value": 0.5}, {"field": "eta", "op": "<", "value": 2.5, "abs": True}]
+    dst = pd.DeviceEFlow(ne, 2 * max(n, 1))
+    ws_keep = pd.filter_eflow(out, dst, conds, "all")
+    pd.filter_eflow(out, dst, conds, "all", workspace=ws_keep)
+    barrier()
+    f0.record(stream)
+    for _ in range(f_steps):
+        pd.filter_eflow(out, dst, conds, "all", workspace=ws_keep)
+    f1.record(stream)
+    barrier()
+    filt_ms = f0.elapsed_time(f1) / f_steps
+    kept = int(dst.t["offsets"][-1])
+    del dst, ws_keep
 
     if dist is not None:
         # CSR rebasing of shard outputs: one all-gather of three int64 per rank, outside the data path
@@ -275,7 +289,11 @@ def run_ours(args, rank, world, local_rank):
         "next": {"event_features": {"ms": feat_ms, "objects_per_s": totals[2] / (feat_ms * 1e-3), "kernel": "pd_features_kernel",
                                     "algorithmic_bytes": 29 * totals[2] + 24 * ne,
                                     "hbm_frac": (29 * totals[2] + 24 * ne) / (feat_ms * 1e-3) / 1e9 / peak,
-                                    "note": "H_T, MET, lepton isolation (Eq. 1) on the step's EFlow output; rank 0, not in value"}},
+                                    "note": "H_T, MET, lepton isolation (Eq. 1) on the step's EFlow output; rank 0, not in value"},
+                 "particle_filter": {"ms": filt_ms, "objects_per_s": totals[2] / (filt_ms * 1e-3), "kept": kept, "kernel": "pd_filter_kernel",
+                                     "algorithmic_bytes": 21 * totals[2] + 21 * kept + 16 * (ne + 1),
+                                     "hbm_frac": (21 * totals[2] + 21 * kept + 16 * (ne + 1)) / (filt_ms * 1e-3) / 1e9 / peak,
+                                     "note": "pT > 0.5 and |eta| < 2.5 on the step's EFlow output; 2 launches; rank 0, not in value"}},
     }
     print(json.dumps(line))
     if dist is not None:

@@ -308,16 +308,18 @@ def make_conditions(conditions):
     return arr
 
 
-def filter_eflow(src, dst: "DeviceEFlow", conditions, combine: str = "all", stream=None):
+def filter_eflow(src, dst: "DeviceEFlow", conditions, combine: str = "all", stream=None, workspace=None):
     """pd_filter_eflow: `src` is a DeviceOutputs (its EFlow collection) or a DeviceEFlow; survivors go to `dst`.
-    Asynchronous.  Returns the workspace tensor (kept alive by the caller until the stream is synchronised)."""
+    Asynchronous.  Returns the workspace tensor (to be kept alive until the stream is synchronised; pass it back as
+    `workspace` to reuse it)."""
     torch = _torch()
     if not torch.cuda.is_available():
         raise PdError(PD_ECUDA)
     st = torch.cuda.current_stream() if stream is None else stream
     cap = int(src.c_efl.capacity)
     nbytes = int(lib().pd_filter_workspace_bytes(cap))
-    ws = torch.empty(nbytes + 16, dtype=torch.uint8, device="cuda")
+    ws = workspace if workspace is not None else torch.empty(nbytes + 16, dtype=torch.uint8, device="cuda")
+    assert ws.numel() >= nbytes
     _check(lib().pd_filter_eflow(C.byref(src.c_efl), int(src.n_events), make_conditions(conditions), len(conditions),
                                  1 if combine == "any" else 0, C.byref(dst.c_efl), _tptr(ws), nbytes, C.c_void_p(st.cuda_stream)))
     return ws
