@@ -1000,3 +1000,92 @@ int pdo_filter_eflow(int64_t n_events, const int64_t *offsets, const int8_t *cls
   }
   return PDO_OK;
 }
+
+/* ---- pile-up merging: see pd_oracle.h (Listing 8, Table C.9) ---- */
+static int pdo_poisson_inverse(double mu, double u) {
+  /* smallest n with sum_{k<=n} p_k > u; p_0 = exp(-mu), p_k = p_{k-1} mu / k */
+  const int n_max = (int)ceil(mu + 10.0 * sqrt(mu) + 20.0);
+  double p = exp(-mu), cdf = p;
+  int n = 0;
+  while (!(cdf > u) && n < n_max) {
+    ++n;
+    p = p * mu / (double)n;
+    cdf = cdf + p;
+  }
+  return n;
+}
+
+/* standard normal quantile for 0 < q <= 1/2 by bisection of Phi(x) = erfc(-x / sqrt(2)) / 2 on [-40, 0] */
+static double pdo_norm_quantile_lower(double q) {
+  double lo = -40.0, hi = 0.0;
+  int it;
+  for (it = 0; it < 200; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    if (0.5 * erfc(-mid / sqrt(2.0)) < q) lo = mid;
+    else hi = mid;
+  }
+  return 0.5 * (lo + hi);
+}
+
+/* reading H4: normal of width sigma_z truncated to |z| <= max_z, by inversion of its distribution function with
+ * the 24-bit uniform of word r1 (word r2 is not used): u = ((r1 >> 8) + 1/2) 2^-24 in (0, 1); sign = -1 if
+ * u < 1/2 else +1; v = |2 u - 1| in (0, 1); |z| = -sigma_z Phi^-1(q), q = Phi(-a) + (1 - v) (1/2 - Phi(-a)),
+ * a = max_z / sigma_z.  (Written through the lower tail so that the far tail keeps its relative precision.) */
+static double pdo_truncated_z(uint32_t r1, double sigma_z, double max_z) {
+  const double u = ((double)(r1 >> 8) + 0.5) * (1.0 / 16777216.0);
+  const double sign = u < 0.5 ? -1.0 : 1.0, v = fabs(2.0 * u - 1.0);
+  double lo, q;
+  if (!(sigma_z > 0.0)) return 0.0;
+  lo = 0.5 * erfc((max_z / sigma_z) / sqrt(2.0)); /* Phi(-a) */
+  q = lo + (1.0 - v) * (0.5 - lo);
+  return -sign * sigma_z * pdo_norm_quantile_lower(q);
+}
+
+int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_pileup, double sigma_z,
+                     double max_z_spread, int smear_hs_vertex, uint64_t seed, int64_t event_base, int64_t out_capacity,
+                     int64_t *out_offsets, int32_t *out_pid, int8_t *out_charge, float *out_px, float *out_py,
+                     float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz, uint8_t *is_pu,
+                     int32_t *n_pileup) {
+  int64_t e, n_out = 0;
+  int rc = PDO_OK;
+  if (!hs || !pool || !out_offsets || hs->n_events < 0 || pool->n_events < 1 || !hs->offsets || !pool->offsets) return PDO_EINVAL;
+  if (!(mean_pileup >= 0.0) || mean_pileup > 500.0 || !(sigma_z >= 0.0) || !(max_z_spread >= 0.0)) return PDO_EINVAL;
+  out_offsets[0] = 0;
+  for (e = 0; e < hs->n_events; ++e) {
+    const int64_t event = event_base + e;
+    uint32_t r[4];
+    int n, k, s;
+    double dz_hs;
+    pdo_rng_block(seed, event, 0u, 2u, r);
+    n = pdo_poisson_inverse(mean_pileup, pdo_uniform(r[0]));
+    dz_hs = smear_hs_vertex ? pdo_truncated_z(r[1], sigma_z, max_z_spread) : 0.0;
+    if (n_pileup) n_pileup[e] = n;
+    /* sources: s = -1 the hard-scatter event, s = k the k-th pile-up interaction */
+    for (s = -1; s < n; ++s) {
+      const pdo_events *src = hs;
+      int64_t a = hs->offsets[e], b = hs->offsets[e + 1], i;
+      double dz = dz_hs;
+      k = s;
+      if (s >= 0) {
+        int64_t j;
+        pdo_rng_block(seed, event, (uint32_t)(1 + k), 2u, r);
+        j = (int64_t)(((uint64_t)(r[0] >> 8) * (uint64_t)pool->n_events) >> 24);
+        dz = pdo_truncated_z(r[1], sigma_z, max_z_spread);
+        src = pool, a = pool->offsets[j], b = pool->offsets[j + 1];
+      }
+      for (i = a; i < b; ++i, ++n_out) {
+        if (n_out >= out_capacity) {
+          rc = PDO_ECAPACITY;
+          continue;
+        }
+        out_pid[n_out] = src->pid[i], out_charge[n_out] = src->charge[i];
+        out_px[n_out] = src->px[i], out_py[n_out] = src->py[i], out_pz[n_out] = src->pz[i], out_E[n_out] = src->E[i];
+        out_vx[n_out] = src->vx[i], out_vy[n_out] = src->vy[i];
+        out_vz[n_out] = (float)((double)src->vz[i] + dz);
+        if (is_pu) is_pu[n_out] = (uint8_t)(s >= 0);
+      }
+    }
+    out_offsets[e + 1] = n_out;
+  }
+  return rc;
+}

@@ -189,6 +189,29 @@ int pdo_filter_eflow(int64_t n_events, const int64_t *offsets, const int8_t *cls
                      int32_t combine_any, int64_t *out_offsets, int8_t *out_cls, int32_t *out_src, float *out_pt,
                      float *out_eta, float *out_phi, float *out_E, uint8_t *keep);
 
+/* ---- pile-up merging ("merges minimum-bias interactions with the hard-scatter event
+ * using a Delphes-compatible PileUpMerger before applying the detector card"; Listing 8; Table C.9
+ * mean_pileup, sigma_z 0.053 m, max_z_spread 0.25 m, smear_hs_vertex; sigma_t / max_t_spread have no
+ * effect here because the chain carries no time coordinate, reading A29).  Readings H1-H6 of DESIGN.md
+ * section 12.  For hard-scatter event e (RNG event index E = event_base + e, Philox stream 2):
+ *   block 0:  n = Poisson(mean_pileup) by inversion of u(r0): the smallest n with sum_{k<=n} p_k > u,
+ *             p_0 = exp(-mu), p_k = p_{k-1} mu / k in fp64, n <= n_max = ceil(mu + 10 sqrt(mu) + 20);
+ *             dz_hs = truncated normal from r1 if smear_hs_vertex, else 0;
+ *   block 1+k (k = 0..n-1):  pool event j_k = ((r0 >> 8) * n_pool) >> 24;  dz_k = truncated normal from r1;
+ *   truncated normal (reading H4): the normal of width sigma_z cut at |z| <= max_z_spread, sampled by inversion
+ *             of its distribution function (one uniform, no rejection): u = ((r1 >> 8) + 1/2) 2^-24,
+ *             sign = -1 if u < 1/2 else +1, v = |2u - 1|, |z| = -sigma_z Phi^-1(Phi(-a) + (1 - v)(1/2 - Phi(-a))),
+ *             a = max_z_spread / sigma_z.
+ * Output event e = the hard-scatter particles (vz + dz_hs) followed by the particles of pool events j_0, j_1, ...
+ * in draw order (vz + dz_k); every other field is copied.  is_pu marks the pile-up particles.
+ * out arrays need room for the total; returns PDO_ECAPACITY if out_capacity is too small (out_offsets is then
+ * still complete, so out_offsets[n_events] tells the room needed). */
+int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_pileup, double sigma_z,
+                     double max_z_spread, int smear_hs_vertex, uint64_t seed, int64_t event_base, int64_t out_capacity,
+                     int64_t *out_offsets, int32_t *out_pid, int8_t *out_charge, float *out_px, float *out_py,
+                     float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz, uint8_t *is_pu,
+                     int32_t *n_pileup /* [n_events], may be NULL */);
+
 const char *pdo_strerror(int code);
 
 /* ---- building blocks exposed so that tests can pin them one by one ---- */

@@ -105,6 +105,8 @@ def lib():
         L.pdo_tower_index.restype = C.c_int32
         L.pdo_efficiency.argtypes = [_p, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int)]
         L.pdo_efficiency.restype = C.c_double
+        L.pdo_pileup_merge.argtypes = [C.POINTER(_Events), C.POINTER(_Events), C.c_double, C.c_double, C.c_double, C.c_int,
+                                       C.c_uint64, C.c_int64, C.c_int64] + [_p] * 12
         L.pdo_filter_eflow.argtypes = [C.c_int64] + [_p] * 7 + [C.POINTER(_Condition), C.c_int32, C.c_int32] + [_p] * 8
         L.pdo_event_features.argtypes = [C.POINTER(_Objects), C.c_double, C.c_double] + [_p] * 9
         _lib = L
@@ -326,4 +328,35 @@ def filter_eflow(offsets, cls, src, pt, eta, phi, E, conditions, combine: str = 
     m = int(out["offsets"][-1])
     res = {k: (v if k == "offsets" else v[:m]) for k, v in out.items()}
     res["keep"] = keep[:n]
+    return res
+
+
+def _events_struct(ev):
+    keep = [np.ascontiguousarray(getattr(ev, k)) for k in ("offsets", "pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")]
+    return _Events(int(ev.offsets.shape[0] - 1), int(ev.offsets[-1]), *[_ptr(a) for a in keep]), keep
+
+
+def pileup_merge(hs, pool, mean_pileup: float, sigma_z: float = 0.053, max_z_spread: float = 0.25,
+                 smear_hs_vertex: bool = True, seed: int = 0, event_base: int = 0) -> dict:
+    """pdo_pileup_merge (Listing 8, Table C.9): returns offsets, pid, charge, px..vz, is_pu, n_pileup."""
+    chs, k1 = _events_struct(hs)
+    cpool, k2 = _events_struct(pool)
+    ne = chs.n_events
+    off = np.zeros(ne + 1, dtype=np.int64)
+    npu = np.zeros(max(ne, 1), dtype=np.int32)
+    dt = dict(pid=np.int32, charge=np.int8, px=np.float32, py=np.float32, pz=np.float32, E=np.float32, vx=np.float32,
+              vy=np.float32, vz=np.float32, is_pu=np.uint8)
+    cap = 0
+    for _ in range(2):  # first pass sizes the output (PDO_ECAPACITY with complete offsets), second fills it
+        out = {k: np.zeros(max(cap, 1), dtype=d) for k, d in dt.items()}
+        rc = lib().pdo_pileup_merge(C.byref(chs), C.byref(cpool), float(mean_pileup), float(sigma_z), float(max_z_spread),
+                                    int(bool(smear_hs_vertex)), int(seed) & (2**64 - 1), int(event_base), cap, _ptr(off),
+                                    *[_ptr(out[k]) for k in dt], _ptr(npu))
+        if rc == 0:
+            break
+        if rc != -3:
+            raise OracleError(rc)
+        cap = int(off[-1])
+    res = {k: v[: int(off[-1])] for k, v in out.items()}
+    res["offsets"], res["n_pileup"] = off, npu[:ne]
     return res
