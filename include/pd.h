@@ -198,6 +198,49 @@ int64_t pd_filter_workspace_bytes(int64_t capacity);
 int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *conds, int32_t n_conds, int32_t combine_any,
                     pd_eflow *out, void *workspace, int64_t workspace_bytes, void *cuda_stream);
 
+/* ---- Pile-up merging (Listing 8; Table C.9) ----
+ * "When configured with a pile-up block, the parametric path first merges minimum-bias interactions with the
+ * hard-scatter event using a Delphes-compatible PileUpMerger before applying the detector card."  Readings H1-H6
+ * of DESIGN.md section 12.  For hard-scatter event e (RNG event index event_base + e, Philox stream 2):
+ *   block 0: n = Poisson(mean_pileup) by inversion of the 24-bit uniform of word 0 (fp64 recurrence, the same
+ *            operations in the same order as the oracle, so n is bit-exact); the hard-scatter vertex shift from
+ *            word 1 if smear_hs_vertex;
+ *   block 1+k, k < n: pool event ((r0 >> 8) * n_pool) >> 24; its vertex shift from word 1;
+ *   vertex shift: normal of width sigma_z truncated to |z| <= max_z_spread, sampled by inversion of its
+ *            distribution function (one uniform, no rejection).
+ * Output event e = the hard-scatter particles (vz shifted) followed by the particles of the n picked pool
+ * events in draw order (vz shifted); every other field is copied.  sigma_t / max_t_spread of Table C.9 have no
+ * effect: the chain carries no time coordinate (reading A29).  The output is a pd_events-shaped CSR batch that
+ * pd_simulate takes as it is. */
+typedef struct {
+  float mean_pileup;  /* 0 <= mean <= 500 */
+  float sigma_z;      /* metres, >= 0 (Table C.9 default 0.053) */
+  float max_z_spread; /* metres, >= 0 (default 0.25) */
+  int32_t smear_hs_vertex;
+} pd_pileup_config;
+
+typedef struct {
+  int64_t capacity;  /* particles the arrays below can hold */
+  int64_t *offsets;  /* [n_events+1] */
+  int32_t *pid;
+  int8_t *charge;
+  float *px, *py, *pz, *E, *vx, *vy, *vz;
+  uint8_t *is_pu;    /* 1 for pile-up particles */
+  int32_t *n_pileup; /* [n_events] interactions merged into each event */
+} pd_merged_events;
+
+/* Bytes of DEVICE workspace pd_pileup_merge needs (status word, per-event counts, scan words). */
+int64_t pd_pileup_workspace_bytes(int64_t n_events);
+
+/* hs, pool, out: structs in HOST memory whose pointer members are DEVICE pointers; pool->n_events >= 1.
+ * Asynchronous on cuda_stream, three kernel launches, allocates nothing.  The merged size is only known on
+ * the device: out->offsets is always complete, and if out->offsets[n_events] exceeds out->capacity nothing else
+ * is written and pd_last_status(workspace) reports PD_ECAPACITY (re-run with that much room).
+ * Errors: PD_EINVAL, PD_EWORKSPACE, PD_ECUDA. */
+int pd_pileup_merge(const pd_events *hs, const pd_events *pool, const pd_pileup_config *cfg, uint64_t seed,
+                    int64_t event_base, pd_merged_events *out, void *workspace, int64_t workspace_bytes,
+                    void *cuda_stream);
+
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 

@@ -18,7 +18,7 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
@@ -40,6 +40,15 @@ class Condition(C.Structure):
 
 FIELDS = {"pt": 0, "eta": 1, "phi": 2, "E": 3, "cls": 4}
 OPS = {">": 0, ">=": 1, "<": 2, "<=": 3, "==": 4, "!=": 5, "in": 6, "not in": 7}
+
+
+class PileupConfig(C.Structure):
+    _fields_ = [("mean_pileup", C.c_float), ("sigma_z", C.c_float), ("max_z_spread", C.c_float), ("smear_hs_vertex", C.c_int32)]
+
+
+class MergedEvents(C.Structure):
+    _fields_ = [("capacity", C.c_int64)] + [(k, _p) for k in ("offsets", "pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz",
+                                                        "is_pu", "n_pileup")]
 
 
 class Events(C.Structure):
@@ -101,6 +110,10 @@ def lib():
         L.pd_last_status.argtypes = [_p, _p]
         L.pd_last_launch_count.argtypes = []
         L.pd_set_tile_events.argtypes = [C.c_int]
+        L.pd_pileup_workspace_bytes.argtypes = [C.c_int64]
+        L.pd_pileup_workspace_bytes.restype = C.c_int64
+        L.pd_pileup_merge.argtypes = [C.POINTER(Events), C.POINTER(Events), C.POINTER(PileupConfig), C.c_uint64, C.c_int64,
+                                      C.POINTER(MergedEvents), _p, C.c_int64, _p]
         L.pd_filter_workspace_bytes.argtypes = [C.c_int64]
         L.pd_filter_workspace_bytes.restype = C.c_int64
         L.pd_filter_eflow.argtypes = [C.POINTER(EFlow), C.c_int64, C.POINTER(Condition), C.c_int32, C.c_int32, C.POINTER(EFlow), _p,
@@ -345,6 +358,62 @@ def simulate(card: Card, dev_events: DeviceEvents, out: DeviceOutputs, seed: int
                            C.byref(out.c_tow), C.byref(out.c_efl), C.byref(out.c_dbg) if out.c_dbg is not None else None,
                            _tptr(out.ws), out.ws_bytes, C.c_void_p(st.cuda_stream))
     _check(rc)
+
+
+class DeviceMerged:
+    """Output buffers of pd_pileup_merge: a pd_events-shaped batch (plus is_pu, n_pileup) of a given capacity."""
+
+    def __init__(self, n_events: int, capacity: int, device="cuda"):
+        torch = _torch()
+        self.n_events, self.capacity = int(n_events), int(capacity)
+        cap = max(self.capacity, 1)
+        self.t = {"offsets": torch.empty(self.n_events + 1, dtype=torch.int64, device=device)}
+        for name, dt in EVENT_FIELDS[1:]:
+            self.t[name] = torch.empty(cap, dtype=getattr(torch, dt), device=device)
+        self.t["is_pu"] = torch.empty(cap, dtype=torch.uint8, device=device)
+        self.t["n_pileup"] = torch.empty(max(self.n_events, 1), dtype=torch.int32, device=device)
+        nbytes = int(lib().pd_pileup_workspace_bytes(self.n_events))
+        self.ws_bytes = nbytes
+        self.ws = torch.empty(nbytes + 16, dtype=torch.uint8, device=device)
+        self.c = MergedEvents(self.capacity, *[_tptr(self.t[k]) for k in ("offsets", "pid", "charge", "px", "py", "pz", "E", "vx", "vy",
+                                                                            "vz", "is_pu", "n_pileup")])
+
+    def total(self) -> int:
+        _torch().cuda.synchronize()
+        return int(self.t["offsets"][-1])
+
+    def as_events(self):
+        """The merged batch as the input of pd_simulate (synchronises to learn the particle count)."""
+        ev = DeviceEvents.__new__(DeviceEvents)
+        ev.n_events, ev.n_particles = self.n_events, self.total()
+        ev.t = {k: self.t[k] for k, _ in EVENT_FIELDS}
+        ev.c = Events(ev.n_events, ev.n_particles, *[_tptr(ev.t[k]) for k, _ in EVENT_FIELDS])
+        return ev
+
+    def to_numpy(self) -> dict:
+        n = self.total()
+        out = {"offsets": self.t["offsets"].cpu().numpy(), "n_pileup": self.t["n_pileup"][: self.n_events].cpu().numpy()}
+        for k in [name for name, _ in EVENT_FIELDS[1:]] + ["is_pu"]:
+            out[k] = self.t[k][:n].cpu().numpy()
+        return out
+
+
+def pileup_merge(hs: "DeviceEvents", pool: "DeviceEvents", out: DeviceMerged, mean_pileup: float, sigma_z: float = 0.053,
+                 max_z_spread: float = 0.25, smear_hs_vertex: bool = True, seed: int = 0, event_base: int = 0, stream=None):
+    """pd_pileup_merge (asynchronous).  pileup_status(out) afterwards reports PD_ECAPACITY if `out` was too small."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    cfg = PileupConfig(float(mean_pileup), float(sigma_z), float(max_z_spread), int(bool(smear_hs_vertex)))
+    _check(lib().pd_pileup_merge(C.byref(hs.c), C.byref(pool.c), C.byref(cfg), int(seed) & (2**64 - 1), int(event_base),
+                                 C.byref(out.c), _tptr(out.ws), out.ws_bytes, C.c_void_p(st.cuda_stream)))
+
+
+def pileup_status(out: DeviceMerged, stream=None) -> int:
+    torch = _torch()
+    st = torch.cuda.current_stream() if stream is None else stream
+    return int(lib().pd_last_status(_tptr(out.ws), C.c_void_p(st.cuda_stream)))
 
 
 def last_status(out: DeviceOutputs, stream=None) -> int:

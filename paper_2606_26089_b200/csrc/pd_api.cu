@@ -94,6 +94,73 @@ int pd_last_launch_count(void) { return t_launches; }
 
 int pd_set_tile_events(int g) { return pd_plan_set_tile_events(g); }
 
+// pile-up workspace: [tile counter, status word, pad] 16 B | scan words, one per 1,024 events | sizes, 8 B per event
+static size_t pileup_chain_bytes(int64_t n_events) {
+  const size_t tiles = (size_t)((n_events + PD_PILEUP_SCAN_TILE - 1) / PD_PILEUP_SCAN_TILE) + 1;
+  return (16 + 8 * tiles + 255) & ~size_t(255);
+}
+
+int64_t pd_pileup_workspace_bytes(int64_t n_events) {
+  if (n_events < 0) return PD_EINVAL;
+  return (int64_t)(pileup_chain_bytes(n_events) + 8 * (size_t)(n_events > 0 ? n_events : 1));
+}
+
+int pd_pileup_merge(const pd_events *hs, const pd_events *pool, const pd_pileup_config *cfg, uint64_t seed,
+                    int64_t event_base, pd_merged_events *out, void *workspace, int64_t workspace_bytes,
+                    void *cuda_stream) {
+  t_launches = 0;
+  if (!hs || !pool || !cfg || !out || hs->n_events < 0 || pool->n_events < 1 || !hs->offsets || !pool->offsets) return PD_EINVAL;
+  if (!(cfg->mean_pileup >= 0.f) || cfg->mean_pileup > 500.f || !(cfg->sigma_z >= 0.f) || !(cfg->max_z_spread >= 0.f)) return PD_EINVAL;
+  if (!std::isfinite(cfg->sigma_z) || !std::isfinite(cfg->max_z_spread)) return PD_EINVAL;
+  if (!out->offsets || out->capacity < 0) return PD_EINVAL;
+  if (hs->n_events > 0 && !out->n_pileup) return PD_EINVAL;
+  if (out->capacity > 0 && (!out->pid || !out->charge || !out->px || !out->py || !out->pz || !out->E || !out->vx || !out->vy ||
+                            !out->vz || !out->is_pu)) return PD_EINVAL;
+  if (hs->n_particles > 0 && (!hs->pid || !hs->charge || !hs->px || !hs->py || !hs->pz || !hs->E || !hs->vx || !hs->vy || !hs->vz)) return PD_EINVAL;
+  if (pool->n_particles > 0 && (!pool->pid || !pool->charge || !pool->px || !pool->py || !pool->pz || !pool->E || !pool->vx || !pool->vy || !pool->vz)) return PD_EINVAL;
+  const int64_t need = pd_pileup_workspace_bytes(hs->n_events);
+  if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15u)) return PD_EWORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t chain_bytes = pileup_chain_bytes(hs->n_events);
+  PD_CUDA(cudaMemsetAsync(workspace, 0, chain_bytes, st));
+  if (hs->n_events == 0) {
+    PD_CUDA(cudaMemsetAsync(out->offsets, 0, sizeof(int64_t), st));
+    return PD_OK;
+  }
+  PdPileupParams p;
+  std::memset(&p, 0, sizeof(p));
+  p.n_hs = hs->n_events, p.n_pool = pool->n_events;
+  p.hs_off = (const long long *)hs->offsets, p.pool_off = (const long long *)pool->offsets;
+  p.hs_pid = hs->pid, p.pool_pid = pool->pid, p.hs_charge = hs->charge, p.pool_charge = pool->charge;
+  const float *hf[7] = {hs->px, hs->py, hs->pz, hs->E, hs->vx, hs->vy, hs->vz};
+  const float *pf[7] = {pool->px, pool->py, pool->pz, pool->E, pool->vx, pool->vy, pool->vz};
+  float *of[7] = {out->px, out->py, out->pz, out->E, out->vx, out->vy, out->vz};
+  for (int f = 0; f < 7; ++f) p.hs_f[f] = hf[f], p.pool_f[f] = pf[f], p.out_f[f] = of[f];
+  // card-like constants in double on the host, exactly as the definition writes them (readings H3, H4)
+  const double mu = (double)cfg->mean_pileup, sz = (double)cfg->sigma_z, zmax = (double)cfg->max_z_spread;
+  p.mu = mu, p.p0 = std::exp(-mu);
+  p.n_max = (int)std::ceil(mu + 10.0 * std::sqrt(mu) + 20.0);
+  p.smear_hs = cfg->smear_hs_vertex ? 1 : 0;
+  p.sigma_z = cfg->sigma_z;
+  const double lo = sz > 0.0 ? 0.5 * std::erfc((zmax / sz) / std::sqrt(2.0)) : 0.0;
+  p.phi_lo = (float)lo, p.half_minus_lo = (float)(0.5 - lo);
+  for (int r = 0; r < 10; ++r) {
+    p.rk.k0[r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+    p.rk.k1[r] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+  }
+  p.event_base = event_base, p.capacity = out->capacity;
+  p.out_off = (long long *)out->offsets, p.out_pid = out->pid, p.out_charge = out->charge;
+  p.is_pu = out->is_pu, p.n_pileup = out->n_pileup;
+  unsigned char *ws = (unsigned char *)workspace;
+  p.tile_counter = (unsigned int *)ws, p.status_word = (int *)(ws + 4);
+  p.chain = (unsigned long long *)(ws + 16);
+  p.cnt = (long long *)(ws + chain_bytes);
+  const int rc = pd_launch_pileup(p, cuda_stream);
+  if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "pile-up kernel launch");
+  t_launches = 3;
+  return PD_OK;
+}
+
 // filter workspace: [tile counter, pad] 16 B | look-back words, one per tile | exclusive ranks of positions 0..capacity
 static size_t filter_chain_bytes(int64_t capacity) {
   const size_t tiles = (size_t)((capacity + 1 + PD_FILTER_TILE - 1) / PD_FILTER_TILE);

@@ -167,3 +167,30 @@ struct PdFilterParams {
   int *rank;                      // workspace: exclusive rank of every input position 0..n
 };
 int pd_launch_filter(const PdFilterParams &prm, void *stream);
+
+// pd_pileup.cu: pile-up merging (pd_pileup_merge)
+constexpr int PD_PILEUP_SCAN_TILE = 1024;  // events per scan tile
+struct PdPileupParams {
+  long long n_hs, n_pool;
+  const long long *hs_off, *pool_off;
+  const int *hs_pid, *pool_pid;
+  const signed char *hs_charge, *pool_charge;
+  const float *hs_f[7], *pool_f[7];  // px, py, pz, E, vx, vy, vz
+  double mu, p0;                     // mean, exp(-mean)
+  int n_max, smear_hs;
+  float sigma_z, phi_lo, half_minus_lo;  // Phi(-a), 1/2 - Phi(-a), a = max_z / sigma_z
+  PdPhiloxKeys rk;
+  long long event_base;
+  long long capacity;
+  long long *out_off;
+  int *out_pid;
+  signed char *out_charge;
+  float *out_f[7];
+  unsigned char *is_pu;
+  int *n_pileup;
+  unsigned int *tile_counter;  // workspace
+  int *status_word;            // workspace + 4 (same place as pd_simulate's: pd_last_status reads it)
+  long long *cnt;              // workspace: particles per merged event
+  unsigned long long *chain;   // workspace: one self-flagged look-back word per scan tile
+};
+int pd_launch_pileup(const PdPileupParams &prm, void *stream);

@@ -1,0 +1,230 @@
+// pd_pileup.cu -- pile-up merging, the step right before the detector-response chain (Listing 8
+// L541-567, Table C.9; readings H1-H6 of DESIGN.md section 12).  Product code;
+// shares nothing with oracle/.
+//   kernel 1 (count)  a thread per hard-scatter event: Poisson draw, pool picks, size of the merged event
+//   kernel 2 (scan)   exclusive prefix of the sizes = CSR offsets of the output (decoupled look-back over
+//                     tiles of 1,024 events claimed from an atomic counter)
+//   kernel 3 (fill)   a warp per event: the hard-scatter particles, then every picked pool event, copied with
+//                     coalesced loads and stores; vz shifted by the source's truncated-normal draw
+// The random numbers are recomputed from their counters where they are needed (Philox4x32-10, stream 2).
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "pd_internal.h"
+
+namespace pdm {
+
+constexpr unsigned long long FLAG_A = 1ull << 62, FLAG_P = 2ull << 62, VAL_MASK = (1ull << 62) - 1;
+
+__device__ __forceinline__ unsigned long long ld_relaxed(const unsigned long long *p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_relaxed(unsigned long long *p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// Philox4x32-10, counter = (block, event lo, event hi, 2 << 16): stream 2 of reading A26
+__device__ __forceinline__ void rng_block2(const PdPhiloxKeys &rk, long long event, uint32_t block, uint32_t (&out)[4]) {
+  uint32_t c0 = block, c1 = (uint32_t)(unsigned long long)event, c2 = (uint32_t)((unsigned long long)event >> 32), c3 = 2u << 16;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    c0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk.k0[r];
+    c1 = (uint32_t)p1;
+    c2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk.k1[r];
+    c3 = (uint32_t)p0;
+  }
+  out[0] = c0, out[1] = c1, out[2] = c2, out[3] = c3;
+}
+
+// reading H3: smallest n with sum_{k<=n} p_k > u; explicit round-to-nearest operations in the oracle's order
+// (no fused multiply-add), so the integer is the oracle's
+__device__ __forceinline__ int poisson_inverse(const PdPileupParams &prm, uint32_t r0) {
+  const double u = (double)(r0 >> 8) * (1.0 / 16777216.0);
+  double p = prm.p0, cdf = p;
+  int n = 0;
+  while (!(cdf > u) && n < prm.n_max) {
+    ++n;
+    p = __ddiv_rn(__dmul_rn(p, prm.mu), (double)n);
+    cdf = __dadd_rn(cdf, p);
+  }
+  return n;
+}
+
+// reading H4: truncated normal by inversion, through the lower tail
+__device__ __forceinline__ float truncated_z(const PdPileupParams &prm, uint32_t r1) {
+  if (!(prm.sigma_z > 0.f)) return 0.f;
+  // u = (k + 1/2) 2^-24, v = |2u - 1|: 1 - v = (2^24 - |2k + 1 - 2^24|) 2^-24, formed in integers so that the far
+  // tail (u next to 0 or 1) keeps its relative precision
+  const int k2 = 2 * (int)(r1 >> 8) + 1 - (1 << 24);
+  const float t = (float)((1 << 24) - (k2 < 0 ? -k2 : k2)) * 5.9604644775390625e-08f;  // exact
+  const float q = fmaf(t, prm.half_minus_lo, prm.phi_lo);
+  const float z = -prm.sigma_z * normcdfinvf(q);
+  return k2 < 0 ? -z : z;
+}
+
+__device__ __forceinline__ long long pool_pick(const PdPileupParams &prm, uint32_t r0) {
+  return (long long)(((unsigned long long)(r0 >> 8) * (unsigned long long)prm.n_pool) >> 24);
+}
+
+__global__ void __launch_bounds__(256) pd_pileup_count_kernel(const __grid_constant__ PdPileupParams prm) {
+  for (long long e = blockIdx.x * 256LL + threadIdx.x; e < prm.n_hs; e += 256LL * gridDim.x) {
+    const long long event = prm.event_base + e;
+    uint32_t r[4];
+    rng_block2(prm.rk, event, 0u, r);
+    const int n = poisson_inverse(prm, r[0]);
+    long long cnt = __ldg(prm.hs_off + e + 1) - __ldg(prm.hs_off + e);
+    for (int k = 0; k < n; ++k) {
+      rng_block2(prm.rk, event, (uint32_t)(1 + k), r);
+      const long long j = pool_pick(prm, r[0]);
+      cnt += __ldg(prm.pool_off + j + 1) - __ldg(prm.pool_off + j);
+    }
+    prm.n_pileup[e] = n;
+    prm.cnt[e] = cnt;
+  }
+}
+
+// exclusive scan of cnt[0..n_hs) into out_off[0..n_hs]
+__global__ void __launch_bounds__(256) pd_pileup_scan_kernel(const __grid_constant__ PdPileupParams prm) {
+  __shared__ long long s_w[8];
+  __shared__ long long s_excl;
+  __shared__ unsigned s_tile;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const long long n_tiles = (prm.n_hs + PD_PILEUP_SCAN_TILE - 1) / PD_PILEUP_SCAN_TILE;
+  for (;;) {
+    __syncthreads();
+    if (tid == 0) s_tile = atomicAdd(prm.tile_counter, 1u);
+    __syncthreads();
+    const long long tile = s_tile;
+    if (tile >= n_tiles) break;
+    const long long base = tile * PD_PILEUP_SCAN_TILE + 4LL * tid;  // four consecutive events per thread
+    long long v[4], sum = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      v[k] = base + k < prm.n_hs ? prm.cnt[base + k] : 0;
+      sum += v[k];
+    }
+    long long incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const long long t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
+    }
+    if (lane == 31) s_w[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+      long long w = lane < 8 ? s_w[lane] : 0, wi = w;
+#pragma unroll
+      for (int o = 1; o < 8; o <<= 1) {
+        const long long t = __shfl_up_sync(0xffffffffu, wi, o);
+        if (lane >= o) wi += t;
+      }
+      const long long total = __shfl_sync(0xffffffffu, wi, 7);
+      if (lane < 8) s_w[lane] = wi - w;
+      unsigned long long excl = 0;
+      if (tile == 0) {
+        if (lane == 0) st_relaxed(prm.chain, FLAG_P | (unsigned long long)total);
+      } else {
+        if (lane == 0) st_relaxed(prm.chain + tile, FLAG_A | (unsigned long long)total);
+        long long pos = tile - 1;
+        for (;;) {
+          const long long idx = pos - lane;
+          unsigned long long x = FLAG_P;
+          if (idx >= 0) {
+            x = ld_relaxed(prm.chain + idx);
+            while ((x >> 62) == 0) {
+              __nanosleep(40);
+              x = ld_relaxed(prm.chain + idx);
+            }
+          }
+          const unsigned pm = __ballot_sync(0xffffffffu, (x >> 62) == 2);
+          unsigned long long part = x & VAL_MASK;
+          if (pm && lane > __ffs(pm) - 1) part = 0;
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+          excl += part;
+          if (pm) break;
+          pos -= 32;
+        }
+        if (lane == 0) st_relaxed(prm.chain + tile, FLAG_P | (excl + (unsigned long long)total));
+      }
+      if (lane == 0) {
+        s_excl = (long long)excl;
+        if (tile == n_tiles - 1) {
+          prm.out_off[prm.n_hs] = (long long)excl + total;
+          if ((long long)excl + total > prm.capacity) atomicExch(prm.status_word, (int)PD_ECAPACITY);
+        }
+      }
+    }
+    __syncthreads();
+    long long run = s_excl + s_w[wid] + incl - sum;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (base + k < prm.n_hs) prm.out_off[base + k] = run;
+      run += v[k];
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_constant__ PdPileupParams prm) {
+  const int lane = threadIdx.x & 31;
+  const long long warp = (blockIdx.x * 256LL + threadIdx.x) >> 5, n_warps = (256LL * gridDim.x) >> 5;
+  if (prm.out_off[prm.n_hs] > prm.capacity) return;  // reported by the scan kernel through the status word
+  for (long long e = warp; e < prm.n_hs; e += n_warps) {
+    const long long event = prm.event_base + e;
+    const int n = prm.n_pileup[e];
+    long long o = prm.out_off[e];
+    for (int s = -1; s < n; ++s) {
+      uint32_t r[4];
+      rng_block2(prm.rk, event, (uint32_t)(s + 1), r);  // block 0: the hard scatter; block 1 + k: interaction k
+      long long a, b;
+      float dz;
+      const bool pu = s >= 0;
+      if (pu) {
+        const long long j = pool_pick(prm, r[0]);
+        a = __ldg(prm.pool_off + j), b = __ldg(prm.pool_off + j + 1);
+        dz = truncated_z(prm, r[1]);
+      } else {
+        a = __ldg(prm.hs_off + e), b = __ldg(prm.hs_off + e + 1);
+        dz = prm.smear_hs ? truncated_z(prm, r[1]) : 0.f;
+      }
+      const int *s_pid = pu ? prm.pool_pid : prm.hs_pid;
+      const signed char *s_q = pu ? prm.pool_charge : prm.hs_charge;
+      for (long long i = a + lane; i < b; i += 32) {
+        const long long d = o + (i - a);
+        prm.out_pid[d] = __ldg(s_pid + i);
+        prm.out_charge[d] = __ldg(s_q + i);
+#pragma unroll
+        for (int f = 0; f < 6; ++f) prm.out_f[f][d] = __ldg((pu ? prm.pool_f[f] : prm.hs_f[f]) + i);
+        prm.out_f[6][d] = __ldg((pu ? prm.pool_f[6] : prm.hs_f[6]) + i) + dz;
+        prm.is_pu[d] = pu ? 1 : 0;
+      }
+      o += b - a;
+    }
+  }
+}
+
+}  // namespace pdm
+
+int pd_launch_pileup(const PdPileupParams &prm, void *stream) {
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PD_ECUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PD_ECUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  long long blocks = (prm.n_hs + 255) / 256;
+  if (blocks > 8LL * sms) blocks = 8LL * sms;
+  if (blocks < 1) blocks = 1;
+  pdm::pd_pileup_count_kernel<<<(unsigned)blocks, 256, 0, st>>>(prm);
+  if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
+  pdm::pd_pileup_scan_kernel<<<4 * sms, 256, 0, st>>>(prm);
+  if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
+  long long fb = (prm.n_hs + 7) / 8;  // a warp per event, eight per block
+  if (fb > 8LL * sms) fb = 8LL * sms;
+  if (fb < 1) fb = 1;
+  pdm::pd_pileup_fill_kernel<<<(unsigned)fb, 256, 0, st>>>(prm);
+  return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
+}
