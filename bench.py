@@ -255,6 +255,24 @@ def run_ours(args, rank, world, local_rank):
     kept = int(dst.t["offsets"][-1])
     del dst, ws_keep
 
+    # ---- pile-up merging, the step right before the hot path: 5,000 cfg0-like hard-scatter
+    # events, a pool of 20,000 cfg3-like minimum-bias events, mean pile-up 50 (Table C.9 defaults otherwise)
+    hs_ev, pool_ev = wl.generate(0, 5000), wl.generate(3, 20000)
+    d_hs, d_pool = pd.DeviceEvents(hs_ev), pd.DeviceEvents(pool_ev)
+    merged = pd.DeviceMerged(hs_ev.n_events, int(hs_ev.n_particles + hs_ev.n_events * 80 * 48))
+    for _ in range(2):
+        pd.pileup_merge(d_hs, d_pool, merged, 50.0, seed=seed)
+    barrier()
+    f0.record(stream)
+    for _ in range(f_steps):
+        pd.pileup_merge(d_hs, d_pool, merged, 50.0, seed=seed)
+    f1.record(stream)
+    barrier()
+    pu_ms = f0.elapsed_time(f1) / f_steps
+    pu_total = merged.total()
+    assert pd.pileup_status(merged) == 0
+    del merged, d_hs, d_pool
+
     if dist is not None:
         # CSR rebasing of shard outputs: one all-gather of three int64 per rank, outside the data path
         from paper_2606_26089_b200 import shard
@@ -290,6 +308,10 @@ def run_ours(args, rank, world, local_rank):
                                     "algorithmic_bytes": 29 * totals[2] + 24 * ne,
                                     "hbm_frac": (29 * totals[2] + 24 * ne) / (feat_ms * 1e-3) / 1e9 / peak,
                                     "note": "H_T, MET, lepton isolation (Eq. 1) on the step's EFlow output; rank 0, not in value"},
+                 "pileup_merge": {"ms": pu_ms, "merged_particles_per_s": pu_total / (pu_ms * 1e-3), "merged_particles": pu_total,
+                                  "kernels": "pd_pileup_count/scan/fill_kernel", "algorithmic_bytes": 67 * pu_total + 20 * hs_ev.n_events,
+                                  "hbm_frac": (67 * pu_total + 20 * hs_ev.n_events) / (pu_ms * 1e-3) / 1e9 / peak,
+                                  "note": "5,000 cfg0-like events + Poisson(50) of 20,000 cfg3-like min-bias events; 3 launches; rank 0, not in value"},
                  "particle_filter": {"ms": filt_ms, "objects_per_s": totals[2] / (filt_ms * 1e-3), "kept": kept, "kernel": "pd_filter_kernel",
                                      "algorithmic_bytes": 21 * totals[2] + 21 * kept + 16 * (ne + 1),
                                      "hbm_frac": (21 * totals[2] + 21 * kept + 16 * (ne + 1)) / (filt_ms * 1e-3) / 1e9 / peak,

@@ -4,8 +4,9 @@
 //   kernel 1 (count)  a thread per hard-scatter event: Poisson draw, pool picks, size of the merged event
 //   kernel 2 (scan)   exclusive prefix of the sizes = CSR offsets of the output (decoupled look-back over
 //                     tiles of 1,024 events claimed from an atomic counter)
-//   kernel 3 (fill)   a warp per event: the hard-scatter particles, then every picked pool event, copied with
-//                     coalesced loads and stores; vz shifted by the source's truncated-normal draw
+//   kernel 3 (fill)   a CTA per event: warp 0 lists the sources (hard scatter, then every picked pool event) and
+//                     scans their sizes, the eight warps copy them side by side with coalesced loads and stores;
+//                     vz shifted by the source's truncated-normal draw
 // The random numbers are recomputed from their counters where they are needed (Philox4x32-10, stream 2).
 #include <cuda_runtime.h>
 
@@ -170,40 +171,66 @@ __global__ void __launch_bounds__(256) pd_pileup_scan_kernel(const __grid_consta
   }
 }
 
+// A 256-thread CTA per merged event.  Warp 0 lists the event's sources (the hard scatter, then the n picked pool
+// events): start and length in their input batch, vertex shift, and -- by a warp scan -- where each lands in the
+// output; then the eight warps copy the sources side by side.
+constexpr int MAX_SOURCES = 768;  // n_max + 1 <= ceil(500 + 10 sqrt(500) + 20) + 1 = 745
 __global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_constant__ PdPileupParams prm) {
-  const int lane = threadIdx.x & 31;
-  const long long warp = (blockIdx.x * 256LL + threadIdx.x) >> 5, n_warps = (256LL * gridDim.x) >> 5;
+  __shared__ long long s_a[MAX_SOURCES], s_o[MAX_SOURCES];
+  __shared__ int s_len[MAX_SOURCES];
+  __shared__ float s_dz[MAX_SOURCES];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   if (prm.out_off[prm.n_hs] > prm.capacity) return;  // reported by the scan kernel through the status word
-  for (long long e = warp; e < prm.n_hs; e += n_warps) {
+  for (long long e = blockIdx.x; e < prm.n_hs; e += gridDim.x) {
     const long long event = prm.event_base + e;
-    const int n = prm.n_pileup[e];
-    long long o = prm.out_off[e];
-    for (int s = -1; s < n; ++s) {
-      uint32_t r[4];
-      rng_block2(prm.rk, event, (uint32_t)(s + 1), r);  // block 0: the hard scatter; block 1 + k: interaction k
-      long long a, b;
-      float dz;
-      const bool pu = s >= 0;
-      if (pu) {
-        const long long j = pool_pick(prm, r[0]);
-        a = __ldg(prm.pool_off + j), b = __ldg(prm.pool_off + j + 1);
-        dz = truncated_z(prm, r[1]);
-      } else {
-        a = __ldg(prm.hs_off + e), b = __ldg(prm.hs_off + e + 1);
-        dz = prm.smear_hs ? truncated_z(prm, r[1]) : 0.f;
-      }
-      const int *s_pid = pu ? prm.pool_pid : prm.hs_pid;
-      const signed char *s_q = pu ? prm.pool_charge : prm.hs_charge;
-      for (long long i = a + lane; i < b; i += 32) {
-        const long long d = o + (i - a);
-        prm.out_pid[d] = __ldg(s_pid + i);
-        prm.out_charge[d] = __ldg(s_q + i);
+    const int n_src = prm.n_pileup[e] + 1;
+    __syncthreads();  // the previous event's lists are no longer read
+    if (wid == 0) {
+      long long run = prm.out_off[e];
+      for (int s0 = 0; s0 < n_src; s0 += 32) {
+        const int s = s0 + lane;  // source s: block s of the event's stream (0 = the hard scatter)
+        long long a = 0;
+        int len = 0;
+        float dz = 0.f;
+        if (s < n_src) {
+          uint32_t r[4];
+          rng_block2(prm.rk, event, (uint32_t)s, r);
+          if (s == 0) {
+            a = __ldg(prm.hs_off + e), len = (int)(__ldg(prm.hs_off + e + 1) - a);
+            dz = prm.smear_hs ? truncated_z(prm, r[1]) : 0.f;
+          } else {
+            const long long j = pool_pick(prm, r[0]);
+            a = __ldg(prm.pool_off + j), len = (int)(__ldg(prm.pool_off + j + 1) - a);
+            dz = truncated_z(prm, r[1]);
+          }
+        }
+        int incl = len;
 #pragma unroll
-        for (int f = 0; f < 6; ++f) prm.out_f[f][d] = __ldg((pu ? prm.pool_f[f] : prm.hs_f[f]) + i);
-        prm.out_f[6][d] = __ldg((pu ? prm.pool_f[6] : prm.hs_f[6]) + i) + dz;
+        for (int o = 1; o < 32; o <<= 1) {
+          const int t = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += t;
+        }
+        if (s < n_src) s_a[s] = a, s_len[s] = len, s_dz[s] = dz, s_o[s] = run + (incl - len);
+        run += __shfl_sync(0xffffffffu, incl, 31);
+      }
+    }
+    __syncthreads();
+    for (int s = wid; s < n_src; s += 8) {
+      const bool pu = s > 0;
+      const long long a = s_a[s], o = s_o[s];
+      const int len = s_len[s];
+      const float dz = s_dz[s];
+      const int *src_pid = pu ? prm.pool_pid : prm.hs_pid;
+      const signed char *src_q = pu ? prm.pool_charge : prm.hs_charge;
+      for (int i = lane; i < len; i += 32) {
+        const long long d = o + i;
+        prm.out_pid[d] = __ldg(src_pid + a + i);
+        prm.out_charge[d] = __ldg(src_q + a + i);
+#pragma unroll
+        for (int f = 0; f < 6; ++f) prm.out_f[f][d] = __ldg((pu ? prm.pool_f[f] : prm.hs_f[f]) + a + i);
+        prm.out_f[6][d] = __ldg((pu ? prm.pool_f[6] : prm.hs_f[6]) + a + i) + dz;
         prm.is_pu[d] = pu ? 1 : 0;
       }
-      o += b - a;
     }
   }
 }
@@ -222,7 +249,7 @@ int pd_launch_pileup(const PdPileupParams &prm, void *stream) {
   if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
   pdm::pd_pileup_scan_kernel<<<4 * sms, 256, 0, st>>>(prm);
   if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
-  long long fb = (prm.n_hs + 7) / 8;  // a warp per event, eight per block
+  long long fb = prm.n_hs;  // a CTA per event
   if (fb > 8LL * sms) fb = 8LL * sms;
   if (fb < 1) fb = 1;
   pdm::pd_pileup_fill_kernel<<<(unsigned)fb, 256, 0, st>>>(prm);
