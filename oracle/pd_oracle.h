@@ -16,7 +16,9 @@
  *
  * Parity status: every function below is pinned by tests/test_oracle_*.py (Philox known-answer
  * vectors, RK4 integration of the Lorentz force, closed forms, the worked values of
- * the text fixtures under tests/golden, invariants, a brute-force tiny event).  What stays UNPINNED is the choice of
+ * the text fixtures under tests/golden, invariants, a brute-force tiny event; the event features / isolation,
+ * the particle filter and the pile-up merging further down by tests/test_oracle_features.py, _filter.py,
+ * _pileup.py: hand-worked cases, scipy quantiles, numpy re-derivations).  What stays UNPINNED is the choice of
  * readings versus the paper's own software (not in the container): "parity with the paper's
  * software: unpinned" -- see DESIGN.md.
  *
