@@ -563,9 +563,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       const int n_tow = (int)(ta & 0xffffu), n_ph = (int)(ta >> 16), n_nh = (int)tb;
       if (!multi && lane == 0) s_ntow[0] = 0, s_ntow[1] = n_tow, s_nph[0] = 0, s_nph[1] = n_ph, s_nnh[0] = 0, s_nnh[1] = n_nh;
       const unsigned long long agg = (unsigned long long)n_tow | ((unsigned long long)(n_ph + n_nh) << 31);
-      if (lane == 0) chain_publish(prm.chain + prm.n_tiles, tile, agg);
-      const unsigned long long ex = chain_resolve<1>(prm.chain + prm.n_tiles, tile, agg);
-      if (lane == 0) s_misc[2] = ex;
+      if (lane == 0) chain_publish(prm.chain + prm.n_tiles, tile, agg), s_misc[3] = agg;
     } else if (wid == 1) {
       // the track prefix: published long ago by every predecessor, so this never waits
       const unsigned long long ex = chain_resolve<10>(prm.chain, tile, (unsigned long long)n_trk);
@@ -577,37 +575,45 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
     }
     __syncthreads();
     const long long base_trk = (long long)s_misc[1];
+    // The track collection needs the track prefix only: it is written between publishing the tower / neutral
+    // aggregate and resolving its prefix, which gives the slower predecessors that much time to publish theirs.
+    for (int e = tid; e < ne; e += THREADS) prm.trk_offsets[e0 + e + 1] = base_trk + s_ntrk[e + 1];
+    for (int s = tid; s < n_trk; s += THREADS) {
+      const long long src = p0 + s_tk[s];
+      const unsigned g = (unsigned)base_trk + (unsigned)s;  // all output indices fit 32 bits (n_particles < 2^30)
+      prm.trk_src[g] = (int)src;
+      prm.trk_pid[g] = __ldg(prm.pid + src);
+      prm.trk_charge[g] = __ldg(prm.charge + src);
+      prm.trk_pt[g] = __ldcg(ring + s);
+      prm.trk_eta[g] = __ldcg(ring + C + s);
+      prm.trk_phi[g] = __ldcg(ring + 2 * C + s);
+      prm.trk_E[g] = __ldcg(ring + 3 * C + s);
+      prm.trk_eta_out[g] = __ldcg(ring + 4 * C + s);
+      prm.trk_phi_out[g] = __ldcg(ring + 5 * C + s);
+    }
+    if (wid == 0) {
+      const unsigned long long ex = chain_resolve<1>(prm.chain + prm.n_tiles, tile, s_misc[3]);
+      if (lane == 0) s_misc[2] = ex;
+    }
+    __syncthreads();
     const long long base_tow = (long long)(s_misc[2] & FIELD_MASK);
     const long long base_efl = base_trk + (long long)((s_misc[2] >> 31) & FIELD_MASK);
 
     // ------------------------------------------------------------------ pass O: ordered outputs
     for (int e = tid; e < ne; e += THREADS) {
-      prm.trk_offsets[e0 + e + 1] = base_trk + s_ntrk[e + 1];
       prm.tow_offsets[e0 + e + 1] = base_tow + s_ntow[e + 1];
       prm.efl_offsets[e0 + e + 1] = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + s_nnh[e + 1];
     }
     if (tile == 0 && tid == 0) prm.trk_offsets[0] = 0, prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
-    // tracks and their EFlow entries, from the records pass T parked in the ring (L2 hits)
+    // the EFlow entries of the tracks, from the records pass T parked in the ring (L2 hits)
     for (int s = tid; s < n_trk; s += THREADS) {
       const int i = s_tk[s];
       const long long src = p0 + i;
-      const unsigned g = (unsigned)base_trk + (unsigned)s;  // all output indices fit 32 bits (n_particles < 2^30)
-      const float pt = __ldcg(ring + s), eta = __ldcg(ring + C + s), phi = __ldcg(ring + 2 * C + s),
-                  Et = __ldcg(ring + 3 * C + s), eta_o = __ldcg(ring + 4 * C + s), phi_o = __ldcg(ring + 5 * C + s);
+      const float pt = __ldcg(ring + s), eta = __ldcg(ring + C + s), phi = __ldcg(ring + 2 * C + s), Et = __ldcg(ring + 3 * C + s);
       const int pid = __ldg(prm.pid + src);
-      const signed char q = __ldg(prm.charge + src);
       const int e = multi ? (int)s_ev[i] : 0;
       const unsigned at = (unsigned)base_efl + (unsigned)(s + s_nph[e] + s_nnh[e]);
       const int apid = pid < 0 ? -pid : pid;
-      prm.trk_src[g] = (int)src;
-      prm.trk_pid[g] = pid;
-      prm.trk_charge[g] = q;
-      prm.trk_pt[g] = pt;
-      prm.trk_eta[g] = eta;
-      prm.trk_phi[g] = phi;
-      prm.trk_E[g] = Et;
-      prm.trk_eta_out[g] = eta_o;
-      prm.trk_phi_out[g] = phi_o;
       prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
       prm.efl_src[at] = (int)src;
       prm.efl_pt[at] = pt;
