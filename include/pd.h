@@ -17,8 +17,9 @@
  *   - `pd_simulate` takes DEVICE pointers (memory of the current CUDA device, owned by the caller,
  *     typically torch tensors) and a CUDA stream handle; it allocates nothing, launches its kernels
  *     on that stream and returns without synchronising.  `pd_simulate_host` takes HOST pointers and
- *     performs the host<->device copies itself (stream-ordered allocations), returning after the
- *     results are in host memory.
+ *     performs the host<->device copies itself (stream-ordered allocations; batches of more than 4M
+ *     particles in pipelined chunks so that the copies in both directions overlap the kernels),
+ *     returning after the results are in host memory.
  *   - There is no CPU fallback: with no CUDA device both simulate calls fail with PD_ECUDA.
  */
 #ifndef PD_H

@@ -2,7 +2,10 @@
 // kernel launch, and the host-pointer convenience entry point.  No torch types, no CPU fallback.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
+#include <cstdlib>
+#include <vector>
 #include <cstdio>
 #include <cstring>
 #include <mutex>
@@ -374,6 +377,21 @@ int pd_last_status(const void *workspace, void *cuda_stream) {
 
 }  // extern "C"
 
+// keep freed blocks in the stream-ordered pool between calls (the default threshold releases them at every sync)
+static int keep_pool_blocks() {
+  static thread_local int pool_dev = -1;
+  int dev = 0;
+  PD_CUDA(cudaGetDevice(&dev));
+  if (pool_dev != dev) {
+    cudaMemPool_t pool;
+    PD_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
+    unsigned long long keep = ~0ull;
+    PD_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+    pool_dev = dev;
+  }
+  return PD_OK;
+}
+
 static int simulate_host_once(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
                               pd_towers *tow, pd_eflow *efl, void *cuda_stream) {
   t_launches = 0;
@@ -394,19 +412,7 @@ static int simulate_host_once(const pd_card *card, const pd_events *ev, uint64_t
   const size_t efl_bytes = b_off + up(2 * np) + up(8 * np) + 4 * up(8 * np);
   const size_t total = in_bytes + trk_bytes + tow_bytes + efl_bytes + up((size_t)ws_bytes);
   unsigned char *base = nullptr;
-  {
-    // keep freed blocks in the stream-ordered pool between calls (default threshold releases them at every sync)
-    static thread_local int pool_dev = -1;
-    int dev = 0;
-    PD_CUDA(cudaGetDevice(&dev));
-    if (pool_dev != dev) {
-      cudaMemPool_t pool;
-      PD_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
-      unsigned long long keep = ~0ull;
-      PD_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-      pool_dev = dev;
-    }
-  }
+  if (int prc = keep_pool_blocks()) return prc;
   PD_CUDA(cudaMallocAsync((void **)&base, total, st));
   size_t o = 0;
   auto take = [&](size_t bytes) {
@@ -486,11 +492,191 @@ static int simulate_host_once(const pd_card *card, const pd_events *ev, uint64_t
   return rc;
 }
 
+// Large batches: the same call in K chunks of consecutive events, pipelined over three streams so that the
+// host->device copy of chunk c+1, the kernel of chunk c and the device->host copy of chunk c-1 overlap (the link is
+// full duplex).  Events are independent and offsets / particle indices are kept absolute, so the result is
+// bit for bit that of the single-shot path.
+static int simulate_host_pipelined(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                                   pd_towers *tow, pd_eflow *efl, void *cuda_stream, int K) {
+  t_launches = 0;
+  const int64_t n = ev->n_particles, ne = ev->n_events;
+  if (trk->capacity < n || tow->capacity < n || efl->capacity < 2 * n) return PD_ECAPACITY;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // chunk boundaries: consecutive events, balanced by particle count (host offsets)
+  std::vector<int64_t> eb(K + 1, 0);
+  for (int c = 1; c < K; ++c) {
+    const int64_t want = n * c / K;
+    const int64_t *pos = std::upper_bound(ev->offsets, ev->offsets + ne + 1, want);
+    int64_t e = (pos - ev->offsets) - 1;
+    eb[c] = std::min(std::max(e, eb[c - 1]), ne);
+  }
+  eb[K] = ne;
+  int64_t ws_bytes = 0, n_max = 0;
+  for (int c = 0; c < K; ++c) {
+    const int64_t nc = ev->offsets[eb[c + 1]] - ev->offsets[eb[c]];
+    ws_bytes = std::max(ws_bytes, pd_workspace_bytes(card, eb[c + 1] - eb[c], nc));
+    n_max = std::max(n_max, nc);
+  }
+  auto up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  const size_t np = (size_t)n;
+  const size_t b_off = up(8 * (size_t)(ne + 1 + K));
+  const size_t total = b_off + up(4 * np) + up(np) + 7 * up(4 * np)            // inputs
+                       + b_off + 2 * up(4 * np) + up(np) + 6 * up(4 * np)      // tracks
+                       + b_off + 7 * up(4 * np)                                // towers
+                       + b_off + up(2 * np) + 5 * up(8 * np)                   // eflow
+                       + up((size_t)ws_bytes) + up(64);
+  unsigned char *base = nullptr;
+  if (int prc = keep_pool_blocks()) return prc;
+  PD_CUDA(cudaMallocAsync((void **)&base, total, st));
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    unsigned char *ptr = base + o;
+    o += up(bytes);
+    return ptr;
+  };
+  int64_t *d_off = (int64_t *)take(8 * (size_t)(ne + 1 + K));
+  int32_t *d_pid = (int32_t *)take(4 * np);
+  int8_t *d_q = (int8_t *)take(np);
+  float *d_in[7];
+  for (auto &ptr : d_in) ptr = (float *)take(4 * np);
+  int64_t *t_off = (int64_t *)take(8 * (size_t)(ne + 1 + K));
+  int32_t *t_src = (int32_t *)take(4 * np), *t_pid = (int32_t *)take(4 * np);
+  int8_t *t_q = (int8_t *)take(np);
+  float *t_f[6];
+  for (auto &ptr : t_f) ptr = (float *)take(4 * np);
+  int64_t *w_off = (int64_t *)take(8 * (size_t)(ne + 1 + K));
+  int32_t *w_id = (int32_t *)take(4 * np);
+  float *w_f[6];
+  for (auto &ptr : w_f) ptr = (float *)take(4 * np);
+  int64_t *f_off = (int64_t *)take(8 * (size_t)(ne + 1 + K));
+  int8_t *f_cls = (int8_t *)take(2 * np);
+  int32_t *f_src = (int32_t *)take(8 * np);
+  float *f_f[4];
+  for (auto &ptr : f_f) ptr = (float *)take(8 * np);
+  void *ws = take((size_t)ws_bytes);
+  int *d_words = (int *)take(64);  // the chunks' status words, gathered for one read at the end
+
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  std::vector<cudaEvent_t> e_in(K, nullptr), e_k(K, nullptr);
+  cudaEvent_t e_start = nullptr;
+  cudaError_t ce = cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking);
+  if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking);
+  for (int c = 0; c < K && ce == cudaSuccess; ++c) {
+    ce = cudaEventCreateWithFlags(&e_in[c], cudaEventDisableTiming);
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e_k[c], cudaEventDisableTiming);
+  }
+  if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&e_start, cudaEventDisableTiming);
+  // the side streams start after the allocation (and whatever precedes the call) on the caller's stream
+  if (ce == cudaSuccess) ce = cudaEventRecord(e_start, st);
+  if (ce == cudaSuccess) ce = cudaStreamWaitEvent(s_in, e_start, 0);
+  if (ce == cudaSuccess) ce = cudaStreamWaitEvent(s_out, e_start, 0);
+  int rc = ce == cudaSuccess ? PD_OK : cuda_fail(ce, "pipeline set-up");
+
+  const float *h_in[7] = {ev->px, ev->py, ev->pz, ev->E, ev->vx, ev->vy, ev->vz};
+  float *h_tf[6] = {trk->pt, trk->eta, trk->phi, trk->E, trk->eta_out, trk->phi_out};
+  float *h_wf[6] = {tow->eta, tow->phi, tow->E, tow->Eem, tow->Ehad, tow->ET};
+  float *h_ff[4] = {efl->pt, efl->eta, efl->phi, efl->E};
+  auto cp = [&](void *dst, const void *src, size_t bytes, cudaMemcpyKind kind, cudaStream_t s) {
+    if (ce == cudaSuccess && bytes > 0 && dst && src) ce = cudaMemcpyAsync(dst, src, bytes, kind, s);
+  };
+  auto upload = [&](int c) {
+    const int64_t e0 = eb[c], e1 = eb[c + 1], p0 = ev->offsets[e0], nc = ev->offsets[e1] - p0;
+    cp(d_off + e0 + c, ev->offsets + e0, 8 * (size_t)(e1 - e0 + 1), cudaMemcpyHostToDevice, s_in);  // absolute offsets
+    cp(d_pid + p0, ev->pid + p0, 4 * (size_t)nc, cudaMemcpyHostToDevice, s_in);
+    cp(d_q + p0, ev->charge + p0, (size_t)nc, cudaMemcpyHostToDevice, s_in);
+    for (int f = 0; f < 7; ++f) cp(d_in[f] + p0, h_in[f] + p0, 4 * (size_t)nc, cudaMemcpyHostToDevice, s_in);
+    if (ce == cudaSuccess) ce = cudaEventRecord(e_in[c], s_in);
+  };
+  std::vector<int64_t> tot(3 * (size_t)K, 0), basec(3 * (size_t)(K + 1), 0);
+  int launches = 0;
+  if (rc == PD_OK) upload(0);
+  for (int c = 0; c < K && rc == PD_OK; ++c) {
+    if (c + 1 < K) upload(c + 1);  // one chunk ahead of the kernel
+    const int64_t e0 = eb[c], e1 = eb[c + 1], p0 = ev->offsets[e0], nc = ev->offsets[e1] - p0, nec = e1 - e0;
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(st, e_in[c], 0);
+    if (ce != cudaSuccess) {
+      rc = cuda_fail(ce, "pipeline H2D");
+      break;
+    }
+    // the chunk as a call of its own: absolute offsets and whole-batch input arrays (particle indices stay those of
+    // the full call), outputs at the chunk's slice of the device arrays
+    pd_events cev = {nec, nc, d_off + e0 + c, d_pid, d_q, d_in[0], d_in[1], d_in[2], d_in[3], d_in[4], d_in[5], d_in[6]};
+    pd_tracks ct = {nc, t_off + e0 + c, t_src + p0, t_pid + p0, t_q + p0, t_f[0] + p0, t_f[1] + p0, t_f[2] + p0, t_f[3] + p0, t_f[4] + p0, t_f[5] + p0};
+    pd_towers cw = {nc, w_off + e0 + c, w_id + p0, w_f[0] + p0, w_f[1] + p0, w_f[2] + p0, w_f[3] + p0, w_f[4] + p0, w_f[5] + p0};
+    pd_eflow cf = {2 * nc, f_off + e0 + c, f_cls + 2 * p0, f_src + 2 * p0, f_f[0] + 2 * p0, f_f[1] + 2 * p0, f_f[2] + 2 * p0, f_f[3] + 2 * p0};
+    rc = pd_simulate(card, &cev, seed, event_base + e0, &ct, &cw, &cf, nullptr, ws, ws_bytes, cuda_stream);
+    if (rc != PD_OK) break;
+    launches += t_launches;
+    cp(&tot[3 * (size_t)c + 0], t_off + e0 + c + nec, 8, cudaMemcpyDeviceToHost, st);
+    cp(&tot[3 * (size_t)c + 1], w_off + e0 + c + nec, 8, cudaMemcpyDeviceToHost, st);
+    cp(&tot[3 * (size_t)c + 2], f_off + e0 + c + nec, 8, cudaMemcpyDeviceToHost, st);
+    cp(d_words + c, (unsigned char *)ws + 4, 4, cudaMemcpyDeviceToDevice, st);
+    if (ce == cudaSuccess) ce = cudaEventRecord(e_k[c], st);
+    if (ce == cudaSuccess) ce = cudaEventSynchronize(e_k[c]);  // the totals say how much to copy back, and where to
+    if (ce != cudaSuccess) {
+      rc = cuda_fail(ce, "pipeline kernel");
+      break;
+    }
+    const size_t nt = (size_t)tot[3 * (size_t)c], nw = (size_t)tot[3 * (size_t)c + 1], nf = (size_t)tot[3 * (size_t)c + 2];
+    const size_t bt = (size_t)basec[3 * (size_t)c], bw = (size_t)basec[3 * (size_t)c + 1], bf = (size_t)basec[3 * (size_t)c + 2];
+    for (int k = 0; k < 3; ++k) basec[3 * (size_t)(c + 1) + k] = basec[3 * (size_t)c + k] + tot[3 * (size_t)c + k];
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(s_out, e_k[c], 0);
+    // chunk-relative offsets land behind the chunk's first entry; rebased on the host at the end
+    cp(trk->offsets + e0 + 1, t_off + e0 + c + 1, 8 * (size_t)nec, cudaMemcpyDeviceToHost, s_out);
+    cp(tow->offsets + e0 + 1, w_off + e0 + c + 1, 8 * (size_t)nec, cudaMemcpyDeviceToHost, s_out);
+    cp(efl->offsets + e0 + 1, f_off + e0 + c + 1, 8 * (size_t)nec, cudaMemcpyDeviceToHost, s_out);
+    cp(trk->src + bt, t_src + p0, 4 * nt, cudaMemcpyDeviceToHost, s_out), cp(trk->pid + bt, t_pid + p0, 4 * nt, cudaMemcpyDeviceToHost, s_out);
+    cp(trk->charge + bt, t_q + p0, nt, cudaMemcpyDeviceToHost, s_out);
+    for (int f = 0; f < 6; ++f) cp(h_tf[f] + bt, t_f[f] + p0, 4 * nt, cudaMemcpyDeviceToHost, s_out);
+    cp(tow->tower + bw, w_id + p0, 4 * nw, cudaMemcpyDeviceToHost, s_out);
+    for (int f = 0; f < 6; ++f) cp(h_wf[f] + bw, w_f[f] + p0, 4 * nw, cudaMemcpyDeviceToHost, s_out);
+    cp(efl->cls + bf, f_cls + 2 * p0, nf, cudaMemcpyDeviceToHost, s_out), cp(efl->src + bf, f_src + 2 * p0, 4 * nf, cudaMemcpyDeviceToHost, s_out);
+    for (int f = 0; f < 4; ++f) cp(h_ff[f] + bf, f_f[f] + 2 * p0, 4 * nf, cudaMemcpyDeviceToHost, s_out);
+  }
+  int words[16] = {0};
+  if (rc == PD_OK) {
+    cp(words, d_words, 4 * (size_t)K, cudaMemcpyDeviceToHost, st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+    if (ce == cudaSuccess) ce = cudaStreamSynchronize(s_out);
+    if (ce != cudaSuccess) rc = cuda_fail(ce, "pipeline D2H");
+  }
+  if (rc == PD_OK) {
+    trk->offsets[0] = 0, tow->offsets[0] = 0, efl->offsets[0] = 0;
+    for (int c = 0; c < K; ++c) {
+      if (words[c] != 0) rc = words[c];
+      for (int64_t e = eb[c] + 1; e <= eb[c + 1]; ++e) {
+        trk->offsets[e] += basec[3 * (size_t)c], tow->offsets[e] += basec[3 * (size_t)c + 1], efl->offsets[e] += basec[3 * (size_t)c + 2];
+      }
+    }
+  }
+  cudaStreamSynchronize(s_in), cudaStreamSynchronize(s_out), cudaStreamSynchronize(st);
+  for (int c = 0; c < K; ++c) {
+    if (e_in[c]) cudaEventDestroy(e_in[c]);
+    if (e_k[c]) cudaEventDestroy(e_k[c]);
+  }
+  if (e_start) cudaEventDestroy(e_start);
+  if (s_in) cudaStreamDestroy(s_in);
+  if (s_out) cudaStreamDestroy(s_out);
+  cudaFreeAsync(base, st);
+  cudaStreamSynchronize(st);
+  t_launches = launches;
+  return rc;
+}
+
 extern "C" {
 
 int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
                      pd_towers *tow, pd_eflow *efl, void *cuda_stream) {
-  int rc = simulate_host_once(card, ev, seed, event_base, trk, tow, efl, cuda_stream);
+  // large batches go through in pipelined chunks (copies in both directions overlap the kernels)
+  int K = 1;
+  if (card && ev && trk && tow && efl && ev->offsets && trk->offsets && tow->offsets && efl->offsets && ev->n_events >= 1 &&
+      ev->n_particles >= 1 && ev->n_particles < (int64_t(1) << 30)) {
+    if (ev->n_events >= 64 && ev->n_particles >= (int64_t(1) << 22)) K = (int)std::min<int64_t>(8, ev->n_particles >> 21);
+    if (const char *env = std::getenv("PD_HOST_CHUNKS")) K = std::max(1, std::min(16, std::atoi(env)));  // testing / tuning
+    K = (int)std::min<int64_t>(K, ev->n_events);
+  }
+  int rc = K > 1 ? simulate_host_pipelined(card, ev, seed, event_base, trk, tow, efl, cuda_stream, K)
+                 : simulate_host_once(card, ev, seed, event_base, trk, tow, efl, cuda_stream);
   if (rc == PD_EEVENTSIZE) {
     // a tile of the automatic plan did not fit on chip (event sizes far from Poisson): one event per tile
     const int launches = t_launches;

@@ -102,18 +102,25 @@ def test_bitwise_reproducible_and_event_base():
         assert np.array_equal(off, a[prefix + "_offsets"])
 
 
-def test_host_pointer_entry_matches_device_entry():
+def test_host_pointer_entry_matches_device_entry(monkeypatch):
+    """pd_simulate_host, single-shot and in pipelined chunks (large batches take that path by themselves; forced
+    here on a small one), reproduces the device entry bit for bit."""
     import paper_2606_26089_b200 as pd
     from gpu_util import run_gpu
 
-    ev = wl.generate(0, 200)
+    ev = wl.concat_events([wl.generate(0, 200), wl.from_lists([[], []]), wl.generate(1, 30), wl.from_lists([[]])])
     ref = run_gpu("cms_like", ev, 9, debug=False)
     card = pd.Card("cms_like")
-    hb = pd.HostBuffers(ev)
-    pd.simulate_host(card, hb, 9)
-    got = hb.to_numpy()
-    for k, v in got.items():
-        assert v.tobytes() == ref[k].tobytes(), k
+    for chunks in (None, "2", "5", "16"):
+        if chunks is None:
+            monkeypatch.delenv("PD_HOST_CHUNKS", raising=False)
+        else:
+            monkeypatch.setenv("PD_HOST_CHUNKS", chunks)
+        hb = pd.HostBuffers(ev)
+        pd.simulate_host(card, hb, 9)
+        got = hb.to_numpy()
+        for k, v in got.items():
+            assert v.tobytes() == ref[k].tobytes(), (chunks, k)
 
 
 def test_skewed_event_sizes_need_one_event_per_tile():
