@@ -249,8 +249,8 @@ int pd_last_launch_count(void);
  * average event size with head-room for Poisson-like fluctuations; g >= 1 = at most g (<= 256).  A batch
  * whose event sizes are far from Poisson (a few huge events among many small ones) can make a tile of the
  * automatic plan exceed the on-chip capacity: pd_last_status() then reports PD_EEVENTSIZE and the caller
- * re-runs the call after pd_set_tile_events(1) (pd_simulate_host does that itself).  With one event per
- * tile the only limit left is the capacity of a CTA, 8,191 particles per event.  Results do not depend on
+ * re-runs the call after pd_set_tile_events(1) (pd_simulate_host does that itself): one event per tile in
+ * the one-CTA-per-SM variant of the kernel, whose only limit is 8,191 particles per event.  Results do not depend on
  * the tiling.  pd_workspace_bytes() depends on it: call it after changing the setting.  Returns the
  * previous value. */
 int pd_set_tile_events(int g);

@@ -726,7 +726,9 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   static const int force_threads = std::getenv("PD_THREADS") ? std::atoi(std::getenv("PD_THREADS")) : 0;
   size_t budget = budget2;
   plan->threads = 512;
-  if (force_threads == 1024 || (force_threads == 0 && !fits(1, budget2))) {
+  // one event per tile on request (pd_set_tile_events(1), the fall-back for batches with outlier events): the
+  // large variant, so that the only limit left is the capacity of a whole SM
+  if (force_threads == 1024 || t_tile_events == 1 || (force_threads == 0 && !fits(1, budget2))) {
     budget = budget1;
     plan->threads = 1024;
   }

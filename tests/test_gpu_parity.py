@@ -150,3 +150,41 @@ def test_skewed_event_sizes_need_one_event_per_tile():
     got = hb.to_numpy()
     for k, v in got.items():
         assert v.tobytes() == one[k].tobytes(), k
+
+
+def test_huge_events_take_the_1024_thread_kernel_and_the_limit_is_reported():
+    """Events too large for half an SM's shared memory (> ~4,900 particles) run in the one-CTA-per-SM variant of the
+    kernel (1,024 threads, up to 8,191 particles on chip); beyond that the call reports PD_EEVENTSIZE."""
+    import paper_2606_26089_b200 as pd
+    from gpu_util import run_gpu
+    from parity import compare
+
+    def big_event(n_particles, seed):
+        ev = wl.generate(2, 3)                       # ~4,060 particles each: glue them into one event
+        one = wl.Events(offsets=np.array([0, ev.n_particles], dtype=np.int64),
+                        **{k: getattr(ev, k) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
+        keep = n_particles
+        return wl.Events(offsets=np.array([0, keep], dtype=np.int64),
+                         **{k: np.ascontiguousarray(getattr(one, k)[:keep]) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
+
+    # a batch of uniformly huge events: the plan picks the large variant by itself
+    ev = wl.concat_events([big_event(7000, 1), big_event(8191, 2), big_event(5200, 3)])
+    gpu = run_gpu("cms_like", ev, 31)
+    assert gpu["status_word"] == 0
+    _check(compare("cms_like", ev, 31, gpu))
+    # outliers among small events: the automatic plan (made from the average) overflows; one event per tile works
+    mixed = wl.concat_events([big_event(7000, 1), wl.generate(0, 50), big_event(8191, 2), big_event(5200, 3)])
+    assert run_gpu("cms_like", mixed, 31, debug=False)["status_word"] == pd.binding.PD_EEVENTSIZE
+    too_big = wl.concat_events([wl.generate(0, 3), big_event(8192, 4)])
+    prev = pd.set_tile_events(1)
+    try:
+        for card in ("cms_like", "atlas_like", "aleph_like"):
+            g = run_gpu(card, mixed, 31)
+            assert g["status_word"] == 0
+            _check(compare(card, mixed, 31, g))
+        assert run_gpu("cms_like", too_big, 31, debug=False)["status_word"] == pd.binding.PD_EEVENTSIZE
+    finally:
+        pd.set_tile_events(prev)
+    hb = pd.HostBuffers(mixed)                       # the host entry falls back by itself
+    pd.simulate_host(pd.Card("cms_like"), hb, 31)
+    assert int(hb.to_numpy()["trk_offsets"][-1]) > 0
