@@ -188,3 +188,40 @@ def test_huge_events_take_the_1024_thread_kernel_and_the_limit_is_reported():
     hb = pd.HostBuffers(mixed)                       # the host entry falls back by itself
     pd.simulate_host(pd.Card("cms_like"), hb, 31)
     assert int(hb.to_numpy()["trk_offsets"][-1]) > 0
+
+
+def test_card_file_variants_and_multiply_charged_particles(tmp_path):
+    """Cards loaded from files exercise what the built-in ones do not: field reversed or off, zero thresholds, zero
+    resolutions, kappa = 0.3, a finer efficiency table (more pT and |eta| edges than the built-in three rows), an
+    irregular coarse grid with odd phi counts -- and particles of charge +-2, +-3."""
+    import cards
+    from gpu_util import run_gpu
+    from oracle import pdo
+    from parity import compare
+
+    ev = wl.generate(1, 120)
+    q = ev.charge.copy()
+    rng = np.random.default_rng(8)
+    sel = (q != 0) & (rng.random(len(q)) < 0.2)
+    q[sel] = (q[sel] * rng.integers(2, 4, int(sel.sum()))).astype(np.int8)
+    ev = wl.Events(offsets=ev.offsets, **{k: (q if k == "charge" else getattr(ev, k)) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
+    cms, aleph = pdo.Card("cms_like"), pdo.Card("aleph_like")
+    fine_eff = [(20.0, "inf", 0.0, 0.8, 0.99), (5.0, 20.0, 0.0, 1.5, 0.95), (1.0, 5.0, 0.0, 2.0, 0.9), (1.0, "inf", 1.5, 2.5, 0.8),
+                (0.5, 1.0, 0.0, 2.5, 0.6), (0.1, 0.5, 0.0, 2.0, 0.4), (0.3, "inf", 2.5, 3.0, 0.2)]
+    coarse_edges = [-4.7, -3.1, -2.2, -1.3, -0.45, 0.0, 0.5, 1.1, 1.9, 2.6, 3.3, 4.9]
+    coarse_nphi = [5, 9, 18, 36, 71, 72, 37, 36, 17, 8, 3]
+    variants = {
+        "reversed": cards.variant(tmp_path / "a.card", cms.edges, cms.nphi, bz=-2.5),
+        "no_field": cards.variant(tmp_path / "b.card", cms.edges, cms.nphi, bz=0.0),
+        "no_thresholds": cards.variant(tmp_path / "c.card", cms.edges, cms.nphi, ecal_thr=0.0, hcal_thr=0.0),
+        "perfect": cards.variant(tmp_path / "d.card", cms.edges, cms.nphi, track_res=(0.0, 0.0), ecal=(0.0, 0.0, 0.0), hcal=(0.0, 0.0, 0.0)),
+        "kappa_fine_eff": cards.variant(tmp_path / "e.card", cms.edges, cms.nphi, kappa=0.3, eff=fine_eff),
+        "coarse_grid": cards.variant(tmp_path / "f.card", coarse_edges, coarse_nphi, radius=1.0, half_length=2.0, eff=fine_eff),
+        "theta_reversed": cards.variant(tmp_path / "g.card", aleph.edges, aleph.nphi, base="aleph_like", bz=-1.0, eff=fine_eff),
+    }
+    for name, path in variants.items():
+        gpu = run_gpu(path, ev, 17, event_base=1000)
+        assert gpu["status_word"] == 0, name
+        rep = _check(compare(path, ev, 17, gpu, event_base=1000), max_override_frac=5e-3)
+        assert int(gpu["efl_offsets"][-1]) > 0, name
+        print(name, {k: rep[k] for k in ("flagged_particles", "overridden_particles", "flagged_towers", "overridden_towers")})
