@@ -3,7 +3,7 @@
 // readings F1-F4 of DESIGN.md section 10).  Product code; shares nothing with oracle/.
 //
 // Events are independent and nothing is compacted, so there is no chain and no workspace.  A 256-thread CTA
-// (three per SM) walks over chunks of consecutive events (static, strided assignment); inside a chunk it takes
+// (four per SM) walks over chunks of consecutive events (static, strided assignment); inside a chunk it takes
 // RUNS of whole events whose objects fit its shared-memory cache (pT, eta, phi, class: 13 bytes per object), so
 // the O(leptons x objects) cone sums read shared memory only.  An event larger than the cache is streamed from
 // global memory through a second instance of the same code.
@@ -142,7 +142,7 @@ __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, P
   }
 }
 
-__global__ void __launch_bounds__(THREADS, 3) pd_features_kernel(const __grid_constant__ PdFeatParams prm,
+__global__ void __launch_bounds__(THREADS, 4) pd_features_kernel(const __grid_constant__ PdFeatParams prm,
                                                                  int events_per_chunk, long long n_chunks) {
   extern __shared__ __align__(16) unsigned char fsm[];
   float *s_pt = (float *)fsm, *s_eta = s_pt + CAP, *s_phi = s_eta + CAP;
@@ -235,7 +235,7 @@ int pd_launch_features(const PdFeatParams &prm, void *stream) {
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return PD_ECUDA;
   if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PD_ECUDA;
-  const long long ctas = 3LL * sms;
+  const long long ctas = 4LL * sms;
   // chunks of consecutive events, about eight per resident CTA, at most one run's worth of events each
   long long epc = (prm.n_events + 8 * ctas - 1) / (8 * ctas);
   if (epc < 1) epc = 1;
