@@ -74,3 +74,13 @@ def test_no_cpu_fallback():
         dev = B.DeviceEvents(ev, device="cuda")
         out = B.DeviceOutputs(B.Card("cms_like"), dev.n_events, dev.n_particles)
         B.simulate(B.Card("cms_like"), dev, out, 1)
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/pd.h is a C ABI: it must compile as C99 on its own (no C++ types, no torch types)."""
+    import subprocess
+
+    src = tmp_path / "t.c"
+    src.write_text('#include "pd.h"\nint main(void) { pd_events e; pd_condition c; pd_pileup_config p; (void)e; (void)c; (void)p; return 0; }\n')
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
+                           "-fsyntax-only", str(src)])
