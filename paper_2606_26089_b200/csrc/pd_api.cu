@@ -230,6 +230,12 @@ int pd_event_features(const pd_eflow *efl, int64_t n_events, float dr_max, float
   p.cls = efl->cls, p.pt = efl->pt, p.eta = efl->eta, p.phi = efl->phi;
   p.dr_max2 = (float)((double)dr_max * (double)dr_max), p.fsr2 = (float)((double)fsr_dr * (double)fsr_dr);
   p.inv_strip = 1.f / std::fmax(dr_max * 1.000001f, 0.375f);  // strip width >= dr_max (with a ulp of margin)
+  {
+    const double two_pi = 6.283185307179586;
+    const double cells = dr_max > 0.f ? std::floor(two_pi / ((double)dr_max * 1.000001)) : 12.0;
+    p.n_phi = (int)std::fmin(12.0, std::fmax(1.0, cells));
+    p.inv_phi_cell = (float)((double)p.n_phi / two_pi);
+  }
   p.ht = out->ht, p.met_x = out->met_x, p.met_y = out->met_y, p.met = out->met;
   p.iso_charged = out->iso_charged, p.iso_neutral = out->iso_neutral, p.iso_photon = out->iso_photon, p.r_iso = out->r_iso;
   const int rc = pd_launch_features(p, cuda_stream);

@@ -8,8 +8,8 @@
 // the O(leptons x objects) cone sums read shared memory only.  An event larger than the cache is streamed from
 // global memory through a second instance of the same code.
 //   step 1  objects of the run -> shared memory (coalesced); leptons listed; isolation of non-leptons zeroed
-//   step 1b a run that is one big event: counting sort of its object indices by eta strip (width >= dr_max), so
-//           that a lepton only meets the objects of its own strip and the two next to it
+//   step 1b a run that is one big event: counting sort of its object indices by (eta strip, phi cell), both at
+//           least dr_max wide, so that a lepton only meets the objects of the 3 x 3 cells around it
 //   step 2  H_T and E_T^miss: a warp per event (all warps for one big event), exact 64-bit fixed-point sums
 //   step 3  isolation: a warp per lepton, lanes over the candidate objects, three exact fixed-point sums
 // Fixed-point sums (units of 2^-32 GeV) are associative: results do not depend on the order of the objects,
@@ -27,6 +27,8 @@ constexpr int W = THREADS / 32;
 constexpr int CAP = 3072;         // objects cached per run
 constexpr int RUN_EVENTS = 256;   // events per run at most
 constexpr int N_STRIPS = 32;      // eta strips of a big event (cone pre-selection)
+constexpr int N_PHI_MAX = 12;     // phi cells per strip at most
+constexpr int N_CELLS = N_STRIPS * N_PHI_MAX;
 constexpr int STRIP_MIN_OBJECTS = 512;
 constexpr int SMEM_BYTES = 17 * CAP;  // pT, eta, phi (4 B each), lepton list, strip list (2 B each), class (1 B)
 constexpr float kPi = 3.14159265358979323846f;
@@ -47,13 +49,17 @@ __device__ __forceinline__ long long to_fix(float x) { return __float2ll_rn(x * 
 __device__ __forceinline__ int eta_strip(float eta, float inv_strip) {
   return min(max((int)floorf((eta + 6.f) * inv_strip), 0), N_STRIPS - 1);
 }
+// phi cell: n_phi cells of width 2 pi / n_phi >= dr_max over [-pi, pi]
+__device__ __forceinline__ int phi_cell(float phi, const PdFeatParams &prm) {
+  return min(max((int)floorf((phi + kPi) * prm.inv_phi_cell), 0), prm.n_phi - 1);
+}
 
 // Steps 2 and 3 for one run.  Two instances: the objects in shared memory (plain LDS addressing) or, for an event
 // larger than the cache, in global memory.
 template <typename PF, typename PC>
 __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, PF o_eta, PF o_phi, PC o_cls, const int *s_off,
                                              unsigned long long *s_acc, const unsigned short *s_lep, int n_lep, const unsigned short *s_idx,
-                                             const int *s_sstart, int ne, int n, long long e0, long long a0) {
+                                             const unsigned short *s_cstart, int ne, int n, long long e0, long long a0) {
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   // ---- step 2: H_T and E_T^miss.  A run that is one big event: all warps share it (integer atomics in
   // shared memory); otherwise a warp per event.
@@ -93,25 +99,41 @@ __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, P
   auto isolate = [&](int i, int ea, int eb) {
     const float eta_i = o_eta[i], phi_i = o_phi[i];
     long long s_ch = 0, s_nh = 0, s_ph = 0;
-    if (s_idx != nullptr) {
-      // one big event, its objects listed by eta strip (strip width >= dr_max): only the lepton's strip and its two
-      // neighbours can hold objects of the cone; they are contiguous in the list
-      const int st = eta_strip(eta_i, prm.inv_strip);
-      ea = s_sstart[max(st - 1, 0)], eb = s_sstart[min(st + 2, N_STRIPS)];
-    }
-    for (int jj = ea + lane; jj < eb; jj += 32) {
-      const int j = s_idx != nullptr ? (int)s_idx[jj] : jj;
-      const float deta = o_eta[j] - eta_i;
-      float dphi = o_phi[j] - phi_i;
-      dphi = dphi > kPi ? dphi - kTwoPi : (dphi <= -kPi ? dphi + kTwoPi : dphi);
-      const float dr2 = fmaf(deta, deta, dphi * dphi);
-      if (dr2 < prm.dr_max2 && j != i) {  // rare (the cone is ~1 % of the acceptance): the sums stay off the common path
-        const int cj = (int)o_cls[j];
-        const long long fx = to_fix(o_pt[j]);
-        if (cj <= PD_CLS_MUON) s_ch += fx;
-        else if (cj == PD_CLS_NEUHAD) s_nh += fx;
-        else if (!(dr2 < prm.fsr2)) s_ph += fx;
+    auto scan = [&](int lo, int hi, bool listed) {
+      for (int jj = lo + lane; jj < hi; jj += 32) {
+        const int j = listed ? (int)s_idx[jj] : jj;
+        const float deta = o_eta[j] - eta_i;
+        float dphi = o_phi[j] - phi_i;
+        dphi = dphi > kPi ? dphi - kTwoPi : (dphi <= -kPi ? dphi + kTwoPi : dphi);
+        const float dr2 = fmaf(deta, deta, dphi * dphi);
+        if (dr2 < prm.dr_max2 && j != i) {  // rare (the cone is ~1 % of the acceptance): the sums stay off the common path
+          const int cj = (int)o_cls[j];
+          const long long fx = to_fix(o_pt[j]);
+          if (cj <= PD_CLS_MUON) s_ch += fx;
+          else if (cj == PD_CLS_NEUHAD) s_nh += fx;
+          else if (!(dr2 < prm.fsr2)) s_ph += fx;
+        }
       }
+    };
+    if (s_idx != nullptr) {
+      // one big event, its objects listed by (eta strip, phi cell), strips and cells at least dr_max wide: only the
+      // lepton's strip and its two neighbours, and in each its phi cell and the two next to it (cyclically), can hold
+      // objects of the cone; the cells of a strip are contiguous in the list
+      const int st = eta_strip(eta_i, prm.inv_strip), pc = phi_cell(phi_i, prm), np = prm.n_phi;
+      for (int s2 = max(st - 1, 0); s2 <= min(st + 1, N_STRIPS - 1); ++s2) {
+        const unsigned short *row = s_cstart + s2 * N_PHI_MAX;  // row[c] = first list position of cell c; row[np] = end of the strip
+        if (np <= 3) {
+          scan(row[0], row[np], true);
+        } else if (pc == 0) {
+          scan(row[0], row[2], true), scan(row[np - 1], row[np], true);
+        } else if (pc == np - 1) {
+          scan(row[0], row[1], true), scan(row[np - 2], row[np], true);
+        } else {
+          scan(row[pc - 1], row[pc + 2], true);
+        }
+      }
+    } else {
+      scan(ea, eb, false);
     }
     s_ch = warp_sum_ll(s_ch), s_nh = warp_sum_ll(s_nh), s_ph = warp_sum_ll(s_ph);
     if (lane == 0) {
@@ -150,7 +172,8 @@ __global__ void __launch_bounds__(THREADS, 4) pd_features_kernel(const __grid_co
   unsigned short *s_idx = s_lep + CAP;                       // a big event's objects listed by eta strip
   signed char *s_cls = (signed char *)(s_idx + CAP);
   __shared__ int s_off[RUN_EVENTS + 1];
-  __shared__ int s_scnt[N_STRIPS], s_sstart[N_STRIPS + 1];
+  __shared__ int s_ccnt[N_CELLS];                 // objects per (strip, phi cell), then running write positions
+  __shared__ unsigned short s_cstart[N_CELLS + 1];  // first list position of every cell
   __shared__ unsigned s_nlep;
   __shared__ unsigned long long s_acc[3];  // H_T, sum pT cos, sum pT sin of a run that is one big event
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -169,7 +192,7 @@ __global__ void __launch_bounds__(THREADS, 4) pd_features_kernel(const __grid_co
       if (!cached) ne = 1;
       if (tid < 3) s_acc[tid] = 0ull;
       if (tid == 3) s_nlep = 0u;
-      if (tid >= 32 && tid < 32 + N_STRIPS) s_scnt[tid - 32] = 0;
+      for (int c = tid; c < N_CELLS; c += THREADS) s_ccnt[c] = 0;
       for (int e = tid; e <= ne; e += THREADS) s_off[e] = (int)min(__ldg(prm.offsets + e0 + e) - a0, (long long)0x7fffffff);
       __syncthreads();
       const int n = s_off[ne];
@@ -191,30 +214,39 @@ __global__ void __launch_bounds__(THREADS, 4) pd_features_kernel(const __grid_co
       __syncthreads();
       const bool strips = cached && ne == 1 && n >= STRIP_MIN_OBJECTS;
       if (strips) {
-        // counting sort of the event's object indices by eta strip (integer atomics; the order inside a strip is
-        // arbitrary and irrelevant: the cone sums are exact)
-        for (int i = tid; i < n; i += THREADS) atomicAdd(&s_scnt[eta_strip(s_eta[i], prm.inv_strip)], 1);
+        // counting sort of the event's object indices by (eta strip, phi cell) (integer atomics; the order inside a
+        // cell is arbitrary and irrelevant: the cone sums are exact)
+        for (int i = tid; i < n; i += THREADS)
+          atomicAdd(&s_ccnt[eta_strip(s_eta[i], prm.inv_strip) * N_PHI_MAX + phi_cell(s_phi[i], prm)], 1);
         __syncthreads();
         if (wid == 0) {
-          const int c = s_scnt[lane];
-          int incl = c;
+          constexpr int PER = N_CELLS / 32;  // 12 consecutive cells per lane
+          int v[PER], sum = 0;
+#pragma unroll
+          for (int k = 0; k < PER; ++k) v[k] = s_ccnt[lane * PER + k], sum += v[k];
+          int incl = sum;
 #pragma unroll
           for (int o = 1; o < 32; o <<= 1) {
             const int t = __shfl_up_sync(0xffffffffu, incl, o);
             if (lane >= o) incl += t;
           }
-          s_sstart[lane + 1] = incl;
-          if (lane == 0) s_sstart[0] = 0;
-          s_scnt[lane] = incl - c;  // running write position of the strip
+          int run = incl - sum;
+#pragma unroll
+          for (int k = 0; k < PER; ++k) {
+            s_cstart[lane * PER + k] = (unsigned short)run, s_ccnt[lane * PER + k] = run;
+            run += v[k];
+          }
+          if (lane == 31) s_cstart[N_CELLS] = (unsigned short)run;
         }
         __syncthreads();
-        for (int i = tid; i < n; i += THREADS) s_idx[atomicAdd(&s_scnt[eta_strip(s_eta[i], prm.inv_strip)], 1)] = (unsigned short)i;
+        for (int i = tid; i < n; i += THREADS)
+          s_idx[atomicAdd(&s_ccnt[eta_strip(s_eta[i], prm.inv_strip) * N_PHI_MAX + phi_cell(s_phi[i], prm)], 1)] = (unsigned short)i;
         __syncthreads();
       }
 
       if (cached) run_features(prm, (const float *)s_pt, (const float *)s_eta, (const float *)s_phi, (const signed char *)s_cls, s_off, s_acc, s_lep, (int)s_nlep,
-                               strips ? (const unsigned short *)s_idx : (const unsigned short *)nullptr, s_sstart, ne, n, e0, a0);
-      else run_features(prm, prm.pt + a0, prm.eta + a0, prm.phi + a0, prm.cls + a0, s_off, s_acc, (const unsigned short *)nullptr, 0, (const unsigned short *)nullptr, s_sstart,
+                               strips ? (const unsigned short *)s_idx : (const unsigned short *)nullptr, s_cstart, ne, n, e0, a0);
+      else run_features(prm, prm.pt + a0, prm.eta + a0, prm.phi + a0, prm.cls + a0, s_off, s_acc, (const unsigned short *)nullptr, 0, (const unsigned short *)nullptr, s_cstart,
                         ne, n, e0, a0);
       __syncthreads();  // the cache is reused by the next run
       if (ne == 1 && n > 8 * 32 && tid == 0) {

@@ -143,6 +143,8 @@ struct PdFeatParams {
   const float *pt, *eta, *phi;
   float dr_max2, fsr2;  // squared cone radii (rounded to fp32 from double)
   float inv_strip;      // 1 / width of the eta strips that pre-select cone candidates (width >= dr_max)
+  float inv_phi_cell;   // n_phi / (2 pi): phi cells of width >= dr_max
+  int n_phi;            // 1..12
   float *ht, *met_x, *met_y, *met;
   float *iso_charged, *iso_neutral, *iso_photon, *r_iso;
 };
