@@ -30,9 +30,12 @@ struct pdo_card {
   int n_towers;
   int n_eff;
   double eff[PDO_MAX_EFF_ROWS][5]; /* pt_lo, pt_hi, aeta_lo, aeta_hi, eps   (reading A8)      */
+  int eff_species[PDO_MAX_EFF_ROWS]; /* 0: every charged particle, 1 electrons, 2 muons, 3 charged hadrons (reading J1) */
   int has_cos;
   double abs_costheta_max; /* reading A9 */
   double trk_a, trk_b;     /* sigma_rel = sqrt(a^2 + (b pT)^2) */
+  int has_trk_species[4];  /* reading J2: track_res given for species 1..3 */
+  double trk_a_species[4], trk_b_species[4];
   double ecal[3], hcal[3]; /* (C, S, N): sigma = sqrt(C^2 E^2 + S^2 E + N^2)  (reading A20)   */
   double thr_ecal, thr_hcal;
 };
@@ -80,6 +83,7 @@ static void card_finish(pdo_card *c) {
   c->abs_costheta_max = f32(c->abs_costheta_max);
   c->trk_a = f32(c->trk_a);
   c->trk_b = f32(c->trk_b);
+  for (i = 1; i < 4; ++i) c->trk_a_species[i] = f32(c->trk_a_species[i]), c->trk_b_species[i] = f32(c->trk_b_species[i]);
   for (i = 0; i < 3; ++i) {
     c->ecal[i] = f32(c->ecal[i]);
     c->hcal[i] = f32(c->hcal[i]);
@@ -223,12 +227,17 @@ static int card_from_file(pdo_card *c, const char *path) {
     else if (!strcmp(key, "kappa") && nv == 1) c->kappa = v[0];
     else if (!strcmp(key, "abs_costheta_max") && nv == 1) c->has_cos = 1, c->abs_costheta_max = v[0];
     else if (!strcmp(key, "track_res") && nv == 2) c->trk_a = v[0], c->trk_b = v[1];
+    else if (!strcmp(key, "track_res") && nv == 3 && (v[2] == 1.0 || v[2] == 2.0 || v[2] == 3.0))
+      c->has_trk_species[(int)v[2]] = 1, c->trk_a_species[(int)v[2]] = v[0], c->trk_b_species[(int)v[2]] = v[1];
     else if (!strcmp(key, "ecal_res") && nv == 3) memcpy(c->ecal, v, 3 * sizeof(double));
     else if (!strcmp(key, "hcal_res") && nv == 3) memcpy(c->hcal, v, 3 * sizeof(double));
     else if (!strcmp(key, "ecal_thr") && nv == 1) c->thr_ecal = v[0];
     else if (!strcmp(key, "hcal_thr") && nv == 1) c->thr_hcal = v[0];
-    else if (!strcmp(key, "eff") && nv == 5 && c->n_eff < PDO_MAX_EFF_ROWS)
+    else if (!strcmp(key, "eff") && (nv == 5 || (nv == 6 && (v[5] == 0.0 || v[5] == 1.0 || v[5] == 2.0 || v[5] == 3.0))) &&
+             c->n_eff < PDO_MAX_EFF_ROWS) {
+      c->eff_species[c->n_eff] = nv == 6 ? (int)v[5] : 0;
       memcpy(c->eff[c->n_eff++], v, 5 * sizeof(double));
+    }
     else ok = 0;
   }
   fclose(f);
@@ -452,11 +461,18 @@ int pdo_tower_centre(const pdo_card *c, int32_t tower, double *eta_c, double *ph
 /* ------------------------------------------------------------------ O3: efficiency --------- */
 
 /* mode 0: exact; +1: loose (conditions widened by the tolerance); -1: strict (narrowed) */
-static int eff_row_match(const pdo_card *c, int r, double pt, double aeta, int mode) {
+/* reading J1: a row applies to every charged particle (species 0) or to one species only */
+static int species_of(int32_t pid) {
+  const int32_t a = pid < 0 ? -pid : pid;
+  return a == 11 ? PDO_SPECIES_ELECTRON : (a == 13 ? PDO_SPECIES_MUON : PDO_SPECIES_CHHAD);
+}
+
+static int eff_row_match(const pdo_card *c, int r, double pt, double aeta, int mode, int species) {
   const double *row = c->eff[r];
   double m = (double)mode;
   double t0 = m * PDO_REL_TOL * fabs(row[0]), t1 = isinf(row[1]) ? 0.0 : m * PDO_REL_TOL * fabs(row[1]);
   double t2 = m * tol_angle(row[2]), t3 = isinf(row[3]) ? 0.0 : m * tol_angle(row[3]);
+  if (c->eff_species[r] != 0 && c->eff_species[r] != species) return 0;
   if (!(pt > row[0] - t0)) return 0;
   if (!(pt <= row[1] + t1)) return 0;
   if (row[2] > 0.0 ? !(aeta >= row[2] - t2) : 0) return 0;
@@ -465,19 +481,23 @@ static int eff_row_match(const pdo_card *c, int r, double pt, double aeta, int m
 }
 
 double pdo_efficiency(const pdo_card *c, double pt, double eta_mom, double abs_costheta, int *row) {
+  return pdo_efficiency_species(c, pt, eta_mom, abs_costheta, PDO_SPECIES_CHHAD, row);
+}
+
+double pdo_efficiency_species(const pdo_card *c, double pt, double eta_mom, double abs_costheta, int species, int *row) {
   int r;
   double aeta = fabs(eta_mom);
   if (row) *row = -1;
   if (c->has_cos && abs_costheta >= c->abs_costheta_max) return 0.0;
   for (r = 0; r < c->n_eff; ++r)
-    if (eff_row_match(c, r, pt, aeta, 0)) {
+    if (eff_row_match(c, r, pt, aeta, 0, species)) {
       if (row) *row = r;
       return c->eff[r][4];
     }
   return 0.0;
 }
 
-static int eff_row_allowed(const pdo_card *c, double pt, double aeta, double abs_costheta, int row) {
+static int eff_row_allowed(const pdo_card *c, double pt, double aeta, double abs_costheta, int row, int species) {
   int r;
   if (row >= c->n_eff) return 0;
   if (c->has_cos) {
@@ -486,8 +506,8 @@ static int eff_row_allowed(const pdo_card *c, double pt, double aeta, double abs
     if (row < 0 && abs_costheta >= c->abs_costheta_max - t) return 1;
   }
   for (r = 0; r < (row < 0 ? c->n_eff : row); ++r)
-    if (eff_row_match(c, r, pt, aeta, -1)) return 0;
-  return row < 0 ? 1 : eff_row_match(c, row, pt, aeta, +1);
+    if (eff_row_match(c, r, pt, aeta, -1, species)) return 0;
+  return row < 0 ? 1 : eff_row_match(c, row, pt, aeta, +1, species);
 }
 
 static uint32_t eff_near(const pdo_card *c, double pt, double aeta, double abs_costheta) {
@@ -713,11 +733,12 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
         /* O3 track: efficiency at the true vertex momentum (A7), accept iff u < eps (A11) */
         if (q != 0) {
           double eta_mom = asinh(pz / pt), p = sqrt(pt * pt + pz * pz), act = fabs(pz) / p;
-          double eps = pdo_efficiency(c, pt, eta_mom, act, &row);
+          const int species = species_of(ev->pid[i]);
+          double eps = pdo_efficiency_species(c, pt, eta_mom, act, species, &row);
           uint32_t r[4];
           near |= eff_near(c, pt, fabs(eta_mom), act);
           if (ov && ov->eps_row && ov->eps_row[i] != -2 && ov->eps_row[i] != row) {
-            if ((near & PDO_NEAR_EFF) && eff_row_allowed(c, pt, fabs(eta_mom), act, ov->eps_row[i])) {
+            if ((near & PDO_NEAR_EFF) && eff_row_allowed(c, pt, fabs(eta_mom), act, ov->eps_row[i], species)) {
               row = ov->eps_row[i];
               eps = row < 0 ? 0.0 : c->eff[row][4];
             } else {
@@ -728,7 +749,10 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
           accepted = pdo_uniform(r[0]) < eps;
           if (accepted) {
             /* track smearing (A12, A13): log-normal, mean pT, std sigma_rel pT; eta, phi unchanged */
-            double srel = sqrt(c->trk_a * c->trk_a + (c->trk_b * pt) * (c->trk_b * pt));
+            /* reading J2: the resolution given for the particle's species, else the card's common one */
+            const double ta = c->has_trk_species[species] ? c->trk_a_species[species] : c->trk_a;
+            const double tb = c->has_trk_species[species] ? c->trk_b_species[species] : c->trk_b;
+            double srel = sqrt(ta * ta + (tb * pt) * (tb * pt));
             pt_smeared = pdo_lognormal(pt, srel * pt, pdo_normal(r[1], r[2]));
             Etrk = pt_smeared * cosh(eta_mom);
             if (n_trk >= trk->capacity || n_efl >= efl->capacity) {

@@ -233,6 +233,10 @@ int32_t pdo_tower_index(const pdo_card *card, double coord, double phi_pos);
 /* efficiency of O3 for true (pt, eta_mom, |cos theta|); *row receives the row index or -1 */
 double pdo_efficiency(const pdo_card *card, double pt, double eta_mom, double abs_costheta,
                       int *row);
+/* reading J1 (per-species cards): the same for a particle of the given species; pdo_efficiency is the
+ * charged-hadron case (identical for cards whose rows name no species) */
+enum { PDO_SPECIES_ALL = 0, PDO_SPECIES_ELECTRON = 1, PDO_SPECIES_MUON = 2, PDO_SPECIES_CHHAD = 3 };
+double pdo_efficiency_species(const pdo_card *c, double pt, double eta_mom, double abs_costheta, int species, int *row);
 
 #ifdef __cplusplus
 }

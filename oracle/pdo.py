@@ -105,6 +105,8 @@ def lib():
         L.pdo_tower_index.restype = C.c_int32
         L.pdo_efficiency.argtypes = [_p, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_int)]
         L.pdo_efficiency.restype = C.c_double
+        L.pdo_efficiency_species.argtypes = [_p, C.c_double, C.c_double, C.c_double, C.c_int, C.POINTER(C.c_int)]
+        L.pdo_efficiency_species.restype = C.c_double
         L.pdo_pileup_merge.argtypes = [C.POINTER(_Events), C.POINTER(_Events), C.c_double, C.c_double, C.c_double, C.c_int,
                                        C.c_uint64, C.c_int64, C.c_int64] + [_p] * 12
         L.pdo_filter_eflow.argtypes = [C.c_int64] + [_p] * 7 + [C.POINTER(_Condition), C.c_int32, C.c_int32] + [_p] * 8
@@ -157,9 +159,13 @@ class Card:
     def tower_index(self, coord: float, phi: float) -> int:
         return int(lib().pdo_tower_index(self._h, float(coord), float(phi)))
 
-    def efficiency(self, pt, eta_mom, abs_costheta=0.0):
+    def efficiency(self, pt, eta_mom, abs_costheta=0.0, species=None):
+        """(eps, row) of the card's table; species: None (a charged hadron), 1 electron, 2 muon, 3 charged hadron."""
         row = C.c_int(-1)
-        eps = lib().pdo_efficiency(self._h, float(pt), float(eta_mom), float(abs_costheta), C.byref(row))
+        if species is None:
+            eps = lib().pdo_efficiency(self._h, float(pt), float(eta_mom), float(abs_costheta), C.byref(row))
+        else:
+            eps = lib().pdo_efficiency_species(self._h, float(pt), float(eta_mom), float(abs_costheta), int(species), C.byref(row))
         return eps, row.value
 
     def propagate(self, q, px, py, pz, vx=0.0, vy=0.0, vz=0.0):
