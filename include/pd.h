@@ -118,7 +118,9 @@ typedef struct {
 /* Load a detector card: a built-in name ("cms_like" | "atlas_like" | "aleph_like", the parameter
  * sets of BASELINE.json configs[0], [3], [4]) or the path of a card text file ("key = values" lines,
  * '#' comments; keys name, bz, radius, half_length, kappa, grid (eta|theta), edges, nphi, eff,
- * abs_costheta_max, track_res, ecal_res, hcal_res, ecal_thr, hcal_thr).  Pure host work: no CUDA
+ * abs_costheta_max, track_res, ecal_res, hcal_res, ecal_thr, hcal_thr; an `eff` row may carry a sixth
+ * number and a `track_res` line a third one -- the species it applies to: 1 electrons, 2 muons, 3 charged
+ * hadrons, 0 / absent every charged particle -- PAPER.md L653-655).  Pure host work: no CUDA
  * call is made until the card is first used by a simulate call.  Every card number is rounded to
  * fp32 at load (reading A28).  *out is owned by the library until pd_free_card. */
 int pd_load_card(const char *name_or_path, pd_card **out);

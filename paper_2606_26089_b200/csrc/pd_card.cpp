@@ -26,10 +26,12 @@ struct RawCard {
   bool theta = false;
   std::vector<double> edges;
   std::vector<long> nphi;
-  std::vector<std::array<double, 5>> eff;
+  std::vector<std::array<double, 6>> eff;  // pt_lo, pt_hi, |eta|_lo, |eta|_hi, eps, species (0 all, 1 e, 2 mu, 3 charged hadron)
   bool has_cos = false;
   double cos_max = 0;
   double trk_a = 0.01, trk_b = 1.5e-4;
+  bool has_trk_sp[4] = {false, false, false, false};  // per-species track resolution (reading J2)
+  double trk_a_sp[4] = {0, 0, 0, 0}, trk_b_sp[4] = {0, 0, 0, 0};
   double ecal[3] = {0, 0, 0}, hcal[3] = {0, 0, 0};
   double thr_ecal = 0.5, thr_hcal = 1.0;
 };
@@ -39,7 +41,7 @@ const double kInf = std::numeric_limits<double>::infinity();
 
 void default_tracking(RawCard &r) {
   // BASELINE.json configs[0], reading A8: ordered rows (pt_lo, pt_hi, |eta|_lo, |eta|_hi, eps)
-  r.eff = {{{1.0, kInf, 0.0, 1.5, 0.97}}, {{1.0, kInf, 1.5, 2.5, 0.85}}, {{0.1, 1.0, 0.0, 2.5, 0.70}}};
+  r.eff = {{{1.0, kInf, 0.0, 1.5, 0.97, 0.0}}, {{1.0, kInf, 1.5, 2.5, 0.85, 0.0}}, {{0.1, 1.0, 0.0, 2.5, 0.70, 0.0}}};
 }
 
 void builtin_cms(RawCard &r) {
@@ -128,12 +130,15 @@ bool from_file(RawCard &r, const char *path) {
     else if (key == "kappa" && v.size() == 1) r.kappa = v[0];
     else if (key == "abs_costheta_max" && v.size() == 1) r.has_cos = true, r.cos_max = v[0];
     else if (key == "track_res" && v.size() == 2) r.trk_a = v[0], r.trk_b = v[1];
+    else if (key == "track_res" && v.size() == 3 && (v[2] == 1.0 || v[2] == 2.0 || v[2] == 3.0))
+      r.has_trk_sp[int(v[2])] = true, r.trk_a_sp[int(v[2])] = v[0], r.trk_b_sp[int(v[2])] = v[1];
     else if (key == "ecal_res" && v.size() == 3) std::copy(v.begin(), v.end(), r.ecal);
     else if (key == "hcal_res" && v.size() == 3) std::copy(v.begin(), v.end(), r.hcal);
     else if (key == "ecal_thr" && v.size() == 1) r.thr_ecal = v[0];
     else if (key == "hcal_thr" && v.size() == 1) r.thr_hcal = v[0];
-    else if (key == "eff" && v.size() == 5 && r.eff.size() < size_t(PD_MAX_EFF))
-      r.eff.push_back({{v[0], v[1], v[2], v[3], v[4]}});
+    else if (key == "eff" && (v.size() == 5 || (v.size() == 6 && (v[5] == 0.0 || v[5] == 1.0 || v[5] == 2.0 || v[5] == 3.0))) &&
+             r.eff.size() < size_t(PD_MAX_EFF))
+      r.eff.push_back({{v[0], v[1], v[2], v[3], v[4], v.size() == 6 ? v[5] : 0.0}});
     else return false;
   }
   return true;
@@ -180,11 +185,12 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
   s.n_bins = int(nb);
   s.n_towers = int(total);
   s.words_per_event = int((total + 127) / 128) * 4;
-  {
-    const double a = f32(r.trk_a);
-    s.trk_a2 = float(a * a);
-    s.trk_b = float(r.trk_b);
+  for (int sp = 1; sp <= 3; ++sp) {  // reading J2: the species' own resolution, else the card's common one
+    const double a = f32(r.has_trk_sp[sp] ? r.trk_a_sp[sp] : r.trk_a);
+    s.trk_a2[sp - 1] = float(a * a);
+    s.trk_b[sp - 1] = float(r.has_trk_sp[sp] ? r.trk_b_sp[sp] : r.trk_b);
   }
+  s.trk_per_species = (r.has_trk_sp[1] || r.has_trk_sp[2] || r.has_trk_sp[3]) ? 1 : 0;
   for (int k = 0; k < 3; ++k) {
     const double e = f32(r.ecal[k]), h = f32(r.hcal[k]);
     s.ecal2[k] = float(e * e);
@@ -206,7 +212,7 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     const double cm = f32(r.cos_max);
     // |cos theta| >= cmax  <=>  |pz|/pT >= cmax / sqrt(1 - cmax^2)
     const double t_cos = r.has_cos ? (cm < 1.0 ? double(float(cm / std::sqrt(1.0 - cm * cm))) : kInf) : kInf;
-    struct Row { double lo, hi, tlo, thi, eps; };
+    struct Row { double lo, hi, tlo, thi, eps; int species; };
     std::vector<Row> rows;
     for (const auto &row : r.eff) {
       Row w;
@@ -215,6 +221,7 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
       w.tlo = elo > 0 ? double(float(std::sinh(elo))) : -1.0;
       w.thi = std::isinf(ehi) ? kInf : double(float(std::sinh(ehi)));
       w.eps = f32(row[4]);
+      w.species = int(row[5]);
       rows.push_back(w);
       if (w.lo > 0) add(pte, w.lo);
       add(pte, w.hi);
@@ -230,27 +237,30 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
       s.pt_edge2_d[k] = k < s.n_pt ? pte[size_t(k)] * pte[size_t(k)] : std::numeric_limits<double>::max();
       s.T_edge[k] = k < s.n_T ? float(te[size_t(k)]) : std::numeric_limits<float>::infinity();
     }
-    for (int ip = 0; ip <= s.n_pt; ++ip) {
-      // representative pT of the interval (e[ip-1], e[ip]]: its closed upper end, or beyond the last edge
-      const double pt_rep = ip < s.n_pt ? pte[size_t(ip)] : (s.n_pt ? 2.0 * pte.back() + 1.0 : 1.0);
-      for (int it = 0; it <= s.n_T; ++it) {
-        // representative T of [t[it-1], t[it]): its closed lower end, or 0
-        const double T_rep = it > 0 ? te[size_t(it - 1)] : 0.0;
-        float eps = 0.f;
-        int rowi = -1;
-        if (!(r.has_cos && T_rep >= t_cos)) {
-          for (size_t k = 0; k < rows.size(); ++k) {
-            const Row &w = rows[k];
-            if (pt_rep > w.lo && pt_rep <= w.hi && (w.tlo <= 0 || T_rep >= w.tlo) && T_rep < w.thi) {
-              rowi = int(k), eps = float(w.eps);
-              break;
+    // one grid per species (reading J1: a row applies to every charged particle or to one species only)
+    for (int sp = 1; sp <= 3; ++sp)
+      for (int ip = 0; ip <= s.n_pt; ++ip) {
+        // representative pT of the interval (e[ip-1], e[ip]]: its closed upper end, or beyond the last edge
+        const double pt_rep = ip < s.n_pt ? pte[size_t(ip)] : (s.n_pt ? 2.0 * pte.back() + 1.0 : 1.0);
+        for (int it = 0; it <= s.n_T; ++it) {
+          // representative T of [t[it-1], t[it]): its closed lower end, or 0
+          const double T_rep = it > 0 ? te[size_t(it - 1)] : 0.0;
+          float eps = 0.f;
+          int rowi = -1;
+          if (!(r.has_cos && T_rep >= t_cos)) {
+            for (size_t k = 0; k < rows.size(); ++k) {
+              const Row &w = rows[k];
+              if (w.species != 0 && w.species != sp) continue;
+              if (pt_rep > w.lo && pt_rep <= w.hi && (w.tlo <= 0 || T_rep >= w.tlo) && T_rep < w.thi) {
+                rowi = int(k), eps = float(w.eps);
+                break;
+              }
             }
           }
+          s.cell_eps[sp - 1][ip * (s.n_T + 1) + it] = eps;
+          s.cell_row[sp - 1][ip * (s.n_T + 1) + it] = (signed char)rowi;
         }
-        s.cell_eps[ip * (s.n_T + 1) + it] = eps;
-        s.cell_row[ip * (s.n_T + 1) + it] = (signed char)rowi;
       }
-    }
   }
 
   c->edges.resize(nb + 1);

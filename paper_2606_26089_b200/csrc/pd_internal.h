@@ -32,9 +32,11 @@ struct PdCardScalars {
   int n_pt, n_T;
   double pt_edge2_d[PD_MAX_EFF_EDGES];  // e^2 in double; unused entries are DBL_MAX
   float T_edge[PD_MAX_EFF_EDGES];       // sinh |eta| edges (incl. the |cos theta| cut); unused entries +inf
-  float cell_eps[PD_MAX_EFF_CELLS];
-  signed char cell_row[PD_MAX_EFF_CELLS];  // row of the card's table, -1 none
-  float trk_a2, trk_b;       // sigma_rel^2 = a^2 + (b pT)^2
+  // one grid per species (0 electron, 1 muon, 2 charged hadron; reading J1 of DESIGN.md section 13)
+  float cell_eps[3][PD_MAX_EFF_CELLS];
+  signed char cell_row[3][PD_MAX_EFF_CELLS];  // row of the card's table, -1 none
+  float trk_a2[3], trk_b[3];  // sigma_rel^2 = a^2 + (b pT)^2, per species (reading J2)
+  int trk_per_species;        // 0: the three entries are equal (pass T then skips the pid lookup)
   float ecal2[3], hcal2[3];  // C^2, S^2, N^2 of sigma^2 = C^2 E^2 + S^2 E + N^2
   float thr_ecal, thr_hcal;
 };

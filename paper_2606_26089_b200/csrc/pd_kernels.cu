@@ -359,7 +359,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         const int e = multi ? (int)s_ev[i] : 0;
         ParticleOut o;
         particle_chain(sc, cd, c.q, c.px, c.py, c.pz, c.vx, c.vy, c.vz, prm.rk, prm.event_base + e0 + e,
-                       (uint32_t)(i - s_off32[e]), o);
+                       (uint32_t)(i - s_off32[e]), species_of(c.pid), o);
         const int apid = c.pid < 0 ? -c.pid : c.pid;
         const bool to_ecal = apid == 11 || apid == 22;                             // reading A18
         const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
@@ -456,7 +456,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       const float px = __ldg(prm.px + src), py = __ldg(prm.py + src), pz = __ldg(prm.pz + src);
       const int e = multi ? (int)s_ev[i] : 0;
       TrackOut t;
-      track_smear(sc, px, py, pz, prm.rk, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), t);
+      track_smear(sc, px, py, pz, prm.rk, prm.event_base + e0 + e, (uint32_t)(i - s_off32[e]), sc.trk_per_species ? species_of(__ldg(prm.pid + src)) : 2, t);
       const float u = s_uT[i];
       s_uT[i] = t.E_trk;  // from here on: the track energy that pass W subtracts
       __stcg(ring + s, t.pt_s);

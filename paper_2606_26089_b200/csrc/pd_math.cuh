@@ -213,6 +213,12 @@ __device__ __forceinline__ int phi_bin(const SmCard &cd, int i, float phi) {
 // eta of a hit from u (only tracks and debug need it as a number)
 __device__ __forceinline__ float eta_from_u(const PdCardScalars &sc, float u) { return fast_asinh(sc.grid_theta ? -u : u); }
 
+// species of a charged particle for the per-species card tables: 0 electron, 1 muon, 2 charged hadron
+__device__ __forceinline__ int species_of(int pid) {
+  const int a = pid < 0 ? -pid : pid;
+  return a == 11 ? 0 : (a == 13 ? 1 : 2);
+}
+
 // ---- S1..S4 for one particle -------------------------------------------------------------------
 struct ParticleOut {
   uint32_t status;   // PD_DROPPED / PD_BARREL / PD_ENDCAP | PD_LOOPER
@@ -259,7 +265,7 @@ __device__ __noinline__ bool graze_double(const PdCardScalars &sc, float px, flo
 
 __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const SmCard &cd, int q, float px, float py,
                                                float pz, float vx, float vy, float vz, const PhiloxKeys &seed,
-                                               long long event, uint32_t pidx, ParticleOut &o) {
+                                               long long event, uint32_t pidx, int species, ParticleOut &o) {
   o.status = PD_DROPPED;
   o.tower = -1;
   o.eps_row = -1;
@@ -373,8 +379,8 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
     it += apz >= sc.T_edge[1] * pt ? 1 : 0;
     for (int k = 2; k < sc.n_T; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
     const int cell = ip * (sc.n_T + 1) + it;
-    const float eps = sc.cell_eps[cell];
-    o.eps_row = sc.cell_row[cell];
+    const float eps = sc.cell_eps[species][cell];
+    o.eps_row = sc.cell_row[species][cell];
     if (eps > 0.f) {
       uint32_t rn[4];
       rng_block(seed, event, pidx, 0u, rn);
@@ -394,14 +400,14 @@ struct TrackOut {
 };
 
 __device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, float py, float pz,
-                                            const PhiloxKeys &seed, long long event, uint32_t pidx, TrackOut &t) {
+                                            const PhiloxKeys &seed, long long event, uint32_t pidx, int species, TrackOut &t) {
   const float pt2 = fmaf(px, px, py * py);
   const float ipt = fast_rsqrt(pt2);
   const float pt = pt2 * ipt;
   uint32_t rn[4];
   rng_block(seed, event, pidx, 0u, rn);
-  const float bp = sc.trk_b * pt;
-  const float rel2 = fmaf(bp, bp, sc.trk_a2);
+  const float bp = sc.trk_b[species] * pt;
+  const float rel2 = fmaf(bp, bp, sc.trk_a2[species]);
   t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(rn[1], rn[2])) : pt;
   t.E_trk = t.pt_s * (fast_sqrt(fmaf(pz, pz, pt2)) * ipt);
   t.eta_mom = fast_asinh(pz * ipt);

@@ -225,3 +225,23 @@ def test_card_file_variants_and_multiply_charged_particles(tmp_path):
         rep = _check(compare(path, ev, 17, gpu, event_base=1000), max_override_frac=5e-3)
         assert int(gpu["efl_offsets"][-1]) > 0, name
         print(name, {k: rep[k] for k in ("flagged_particles", "overridden_particles", "flagged_towers", "overridden_towers")})
+
+
+def test_per_species_card(tmp_path):
+    """Per-species efficiency rows and track resolutions on a lepton-rich sample."""
+    import cards
+    from gpu_util import run_gpu
+    from oracle import pdo
+    from parity import compare
+    from test_oracle_species import EFF, RES, _sample
+
+    b = pdo.Card("cms_like")
+    path = cards.variant(tmp_path / "species.card", b.edges, b.nphi, eff=EFF, track_res_species=RES)
+    ev = _sample(400)
+    gpu = run_gpu(path, ev, 23)
+    assert gpu["status_word"] == 0
+    rep = _check(compare(path, ev, 23, gpu), max_override_frac=5e-3)
+    # the species tables really are in use: the same events through the species-less card give other tracks
+    plain = run_gpu("cms_like", ev, 23, debug=False)
+    assert int(plain["trk_offsets"][-1]) != int(gpu["trk_offsets"][-1])
+    print({k: rep[k] for k in ("n_particles", "flagged_particles", "overridden_particles")}, int(gpu["trk_offsets"][-1]))
