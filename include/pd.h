@@ -102,7 +102,8 @@ typedef struct {
 /* Optional intermediate products (the paper's `debug` option, PAPER.md L589 / L669).  All arrays have
  * n_particles elements; any pointer may be NULL.  The per-tower fields describe every tower that
  * received a deposit (emitted or not) and are stored at the index of the FIRST particle (in particle
- * order) that deposited into that (event, tower); tw_first marks those indices. */
+ * order) that deposited into that (event, tower); tw_first marks those indices (the tw_* entries of all other indices
+ * are not written). */
 typedef struct {
   uint8_t *status;   /* PD_DROPPED / PD_BARREL / PD_ENDCAP | PD_LOOPER                     */
   float *eta_pos, *phi_pos; /* hit position on the calorimeter surface (NaN if dropped)    */
