@@ -237,6 +237,8 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
       s.pt_edge2_d[k] = k < s.n_pt ? pte[size_t(k)] * pte[size_t(k)] : std::numeric_limits<double>::max();
       s.T_edge[k] = k < s.n_T ? float(te[size_t(k)]) : std::numeric_limits<float>::infinity();
     }
+    s.eff_per_species = 0;
+    for (const Row &w : rows) s.eff_per_species |= w.species != 0 ? 1 : 0;
     // one grid per species (reading J1: a row applies to every charged particle or to one species only)
     for (int sp = 1; sp <= 3; ++sp)
       for (int ip = 0; ip <= s.n_pt; ++ip) {

@@ -37,6 +37,7 @@ struct PdCardScalars {
   signed char cell_row[3][PD_MAX_EFF_CELLS];  // row of the card's table, -1 none
   float trk_a2[3], trk_b[3];  // sigma_rel^2 = a^2 + (b pT)^2, per species (reading J2)
   int trk_per_species;        // 0: the three entries are equal (pass T then skips the pid lookup)
+  int eff_per_species;        // 0: no efficiency row names a species (the three grids are equal)
   float ecal2[3], hcal2[3];  // C^2, S^2, N^2 of sigma^2 = C^2 E^2 + S^2 E + N^2
   float thr_ecal, thr_hcal;
 };

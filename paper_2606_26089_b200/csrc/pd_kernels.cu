@@ -359,7 +359,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         const int e = multi ? (int)s_ev[i] : 0;
         ParticleOut o;
         particle_chain(sc, cd, c.q, c.px, c.py, c.pz, c.vx, c.vy, c.vz, prm.rk, prm.event_base + e0 + e,
-                       (uint32_t)(i - s_off32[e]), species_of(c.pid), o);
+                       (uint32_t)(i - s_off32[e]), sc.eff_per_species ? species_of(c.pid) : 2, o);
         const int apid = c.pid < 0 ? -c.pid : c.pid;
         const bool to_ecal = apid == 11 || apid == 22;                             // reading A18
         const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
