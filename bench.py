@@ -63,6 +63,21 @@ def _traffic(cfg):
     return val
 
 
+def _inst_count(cfg):
+    """Warp instructions per launch (smsp__inst_executed.sum) from the committed ncu --set full capture of this
+    config, if one exists: last matching row of profiles/inst_count.csv."""
+    val = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "inst_count.csv")) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 2 and c[0] == "cfg%d" % cfg:
+                    val = float(c[1])
+    except Exception:
+        return None
+    return val
+
+
 def _sample_events(ev, max_particles):
     """Leading events of the workload holding at most max_particles particles."""
     k = int(np.searchsorted(ev.offsets, max_particles, side="right") - 1)
@@ -288,6 +303,17 @@ def run_ours(args, rank, world, local_rank):
     kern_ms = float(np.mean(per_launch_ms))
     peak, peak_src = _peaks()
     achieved = alg_bytes / (kern_ms * 1e-3) / 1e9
+    # the ALU-side reading of the same launch: warp instructions (from the committed ncu capture)
+    # against the issue peak 148 SMs x 4 schedulers x SM clock
+    inst = _inst_count(cfg)
+    sm_mhz = (clk or {}).get("sm_mhz") or 1965.0
+    alu_view = None
+    if inst:
+        issue_peak = 148 * 4 * sm_mhz * 1e6
+        alu_view = {"warp_instructions_per_launch": inst, "warp_instructions_per_particle": inst / max(n, 1),
+                    "achieved_warp_inst_per_s": inst / (kern_ms * 1e-3), "issue_peak_warp_inst_per_s": issue_peak,
+                    "frac_of_issue_peak": inst / (kern_ms * 1e-3) / issue_peak,
+                    "note": "instruction count from profiles/ (ncu), time live; the path is issue- and barrier-bound, not HBM-bound"}
     cpu_rate, cpu_dt, cpu_what = _oracle_rate(cfg, ev, seed)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -300,7 +326,7 @@ def run_ours(args, rank, world, local_rank):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": _traffic(cfg), "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
                      "bytes_per_particle": alg_bytes / max(n, 1), "kernel_ms": kern_ms, "kernel": "pd_chain_kernel",
-                     "frac_of_8TBs_nominal": achieved / 8000.0},
+                     "frac_of_8TBs_nominal": achieved / 8000.0, "alu_view": alu_view},
         "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": cpu_what},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
         "gpu_launches": launches, "clocks": clk,
