@@ -444,7 +444,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
         s_res[i] = (r & ~(LINK_END << RES_LINK_SHIFT)) | ((prev & LINK_END) << RES_LINK_SHIFT);
       }
     }
-    __syncthreads();
+    // (no barrier: pass T touches nothing pass B does -- it reads the track list and (u, phi) of the accepted
+    // tracks and replaces u by E_trk; pass W, behind the next barrier, needs both)
 
     // ------------------------------------------------------------------ pass T: S3 on the accepted tracks
     // (converged: one thread per track).  The smeared record is parked in this CTA's slice of the workspace ring
