@@ -361,6 +361,7 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
   p.events_per_tile = plan.events_per_tile;
   p.n_tiles = plan.n_tiles;
   p.capacity = plan.capacity;
+  p.sparse = plan.sparse;
   unsigned char *ws = (unsigned char *)workspace;
   p.tile_counter = (unsigned int *)ws;
   p.status_word = (int *)(ws + 4);

@@ -115,6 +115,7 @@ struct PdParams {
   int events_per_tile;   // G
   int n_tiles;
   int capacity;          // C: particles a tile may hold on chip
+  int sparse;            // 1: two-level tower bitmap (large grids, small events), see make_layout
   unsigned long long *chain;  // [2][n_tiles] look-back words: tracks; towers | neutrals
   float *ring;                // [max_ctas][6][capacity] smeared track records parked between pass T and pass O
   unsigned int *tile_counter;
@@ -132,6 +133,7 @@ struct PdLaunchPlan {
   int events_per_tile;
   int n_tiles;
   int max_ctas;      // upper bound of the grid (sizes the workspace ring)
+  int sparse;        // two-level tower bitmap
   size_t smem_bytes;
 };
 int pd_plan_set_tile_events(int g);

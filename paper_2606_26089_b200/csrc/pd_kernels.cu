@@ -1,4 +1,4 @@
-// pd_kernels.cu -- the fused Delphes-chain kernel for sm_100a (steps S0..S8 of SURVEY.md section 8a), v5.
+// pd_kernels.cu -- the fused Delphes-chain kernel for sm_100a (steps S0..S8 of SURVEY.md section 8a), v5f.
 //
 // Persistent CTAs (two 512-thread CTAs per SM, or one 1024-thread CTA for large events); a CTA repeatedly
 // claims a TILE (a run of G whole events, <= C particles) from an atomic counter and takes it through
@@ -16,6 +16,8 @@
 //   scan W              one scan over the per-warp counts; chain W published and resolved (decoupled
 //                       look-back), chain T resolved (never waits: published a whole phase ago)
 //   pass O   S8         ordered compaction of tracks / towers / photons / neutral hadrons, CSR offsets
+// Large grids with small events use a two-level bitmap (sparse mode, see make_layout): groups first, then the
+// tower bits of the non-empty groups only.
 // Nothing but the inputs, the final collections and the ring touches memory.  Sums are order-stable: each
 // tower's deposits are added as 64-bit fixed-point integers (exact, hence independent of the order in which
 // the list was built), and the only atomics are integer (bitmap OR, list exchange, counters).
@@ -48,12 +50,17 @@ struct Layout {
   size_t misc;                                                            // scratch words
   size_t cnt;                                                             // pass W warp counts -> prefixes [2][256]
   size_t bitmap, gprefix;                                                 // per event: tower bits, group prefix
+  size_t l2p, pool;                                                       // sparse mode (see make_layout)
   size_t res, uT, phi, Ev, head, stg, ev;                                 // per particle / per slot
   size_t total;
 };
 
+// Dense mode: one bit per tower and event (bitmap), a prefix per 128-tower group (gprefix).
+// Sparse mode (large grids, small events: the bitmaps would be almost empty and take most of the shared memory):
+// `bitmap` holds one bit per 128-tower GROUP and event, `l2p` the rank of the first non-empty group of each of its
+// words, `pool` the tower bits of the non-empty groups only (at most one per deposit), `gprefix` their prefixes.
 __host__ __device__ inline Layout make_layout(int n_bins, int lut_cells, int n_towers, int words_per_event, int G,
-                                              int C) {
+                                              int C, int sparse) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) {
@@ -78,8 +85,17 @@ __host__ __device__ inline Layout make_layout(int n_bins, int lut_cells, int n_t
   l.nnh = take(4 * (G + 1));
   l.misc = take(8 * 64);
   l.cnt = take(4 * 2 * 256);
-  l.bitmap = take(4 * (size_t)G * words_per_event);
-  l.gprefix = take(2 * ((size_t)G * (words_per_event / 4) + 1));
+  const int gpe = words_per_event / 4, l2w = (gpe + 31) / 32;
+  l.l2p = 0, l.pool = 0;
+  if (!sparse) {
+    l.bitmap = take(4 * (size_t)G * words_per_event);
+    l.gprefix = take(2 * ((size_t)G * gpe + 1));
+  } else {
+    l.bitmap = take(4 * (size_t)G * l2w);
+    l.l2p = take(2 * ((size_t)G * l2w + 1));
+    l.pool = take(16 * (size_t)C);
+    l.gprefix = take(2 * ((size_t)C + 1));
+  }
   l.res = take(4 * (size_t)C);
   l.uT = take(4 * (size_t)C);
   l.phi = take(4 * (size_t)C);
@@ -256,7 +272,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
   const int nb = sc.n_bins;
   const int C = prm.capacity, G = prm.events_per_tile;
   const int wpe = sc.words_per_event, gpe = wpe >> 2;
-  const Layout L = make_layout(nb, 2 * sc.lut_side, sc.n_towers, wpe, G, C);
+  const bool sparse = prm.sparse != 0;
+  const int l2w = (gpe + 31) >> 5;  // words of the per-event group bitmap (sparse mode)
+  const Layout L = make_layout(nb, 2 * sc.lut_side, sc.n_towers, wpe, G, C, prm.sparse);
   float *s_tb = (float *)(smem + L.tb);
   int *s_nphi = (int *)(smem + L.nphi);
   int *s_offset = (int *)(smem + L.offset);
@@ -278,6 +296,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
   unsigned *s_preB = s_preA + 256;                // ... and neutral hadrons (counts, then exclusive prefixes)
   uint32_t *s_bitmap = (uint32_t *)(smem + L.bitmap);
   unsigned short *s_gp = (unsigned short *)(smem + L.gprefix);
+  unsigned short *s_l2p = (unsigned short *)(smem + L.l2p);  // sparse mode: rank of the first non-empty group of a word
+  uint4 *s_pool = (uint4 *)(smem + L.pool);                  // sparse mode: tower bits of the non-empty groups
   uint32_t *s_res = (uint32_t *)(smem + L.res);
   float *s_uT = (float *)(smem + L.uT);    // hit u of accepted tracks, then E_trk, then staged photon energy
   float *s_phi = (float *)(smem + L.phi);  // hit phi of accepted tracks, then staged Eem''
@@ -338,7 +358,12 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       s_ntrk[e] = 0, s_ntow[e] = 0, s_nph[e] = 0, s_nnh[e] = 0;
     }
     const int NG = ne * gpe;  // 128-tower bitmap groups of the tile
-    for (int k = tid; k < NG; k += THREADS) ((uint4 *)s_bitmap)[k] = make_uint4(0u, 0u, 0u, 0u);
+    const int NW = ne * l2w;  // sparse mode: words of the group bitmaps
+    if (!sparse) {
+      for (int k = tid; k < NG; k += THREADS) ((uint4 *)s_bitmap)[k] = make_uint4(0u, 0u, 0u, 0u);
+    } else {
+      for (int k = tid; k < NW; k += THREADS) s_bitmap[k] = 0u;
+    }
     __syncthreads();
     if (multi) {
       // event index of every particle of the tile: warp per event, lanes over its particles
@@ -368,7 +393,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
           res = (uint32_t)o.tower | (LINK_END << RES_LINK_SHIFT);
           if (!to_none) {
             res |= RES_DEP | (to_ecal ? 0u : RES_HCAL);
-            atomicOr(&s_bitmap[e * wpe + (o.tower >> 5)], 1u << (o.tower & 31));
+            if (!sparse) atomicOr(&s_bitmap[e * wpe + (o.tower >> 5)], 1u << (o.tower & 31));
+            else atomicOr(&s_bitmap[e * l2w + (o.tower >> 12)], 1u << ((o.tower >> 7) & 31));  // its 128-tower group
             s_Ev[i] = c.E;
           }
         }
@@ -403,10 +429,16 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       const int a0 = min(n, tid * ka), a1 = min(n, a0 + ka);
       unsigned cnt_a = 0;
       for (int i = a0; i < a1; ++i) cnt_a += (s_res[i] >> 17) & 1u;
-      const int kg = ((NG + THREADS - 1) / THREADS) | 1;
-      const int g0 = min(NG, tid * kg), g1 = min(NG, g0 + kg);
+      // dense: the groups' tower bits; sparse: the words of the group bitmaps (their bits = non-empty groups)
+      const int NS = sparse ? NW : NG;
+      const int kg = ((NS + THREADS - 1) / THREADS) | 1;
+      const int g0 = min(NS, tid * kg), g1 = min(NS, g0 + kg);
       unsigned cnt_g = 0;
-      for (int g = g0; g < g1; ++g) cnt_g += (unsigned)popc4(((const uint4 *)s_bitmap)[g]);
+      if (!sparse) {
+        for (int g = g0; g < g1; ++g) cnt_g += (unsigned)popc4(((const uint4 *)s_bitmap)[g]);
+      } else {
+        for (int g = g0; g < g1; ++g) cnt_g += (unsigned)__popc(s_bitmap[g]);
+      }
       const unsigned packed = cnt_a | (cnt_g << 16);
       const unsigned incl = warp_incl_scan(packed);
       if (lane == 31) s_wtot[wid] = incl;
@@ -417,13 +449,53 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       int ra = (int)(excl & 0xffffu), rg = (int)(excl >> 16);
       for (int i = a0; i < a1; ++i)
         if (s_res[i] & RES_ACC) s_tk[ra++] = (unsigned short)i;
-      for (int g = g0; g < g1; ++g) {
-        s_gp[g] = (unsigned short)rg;
-        rg += popc4(((const uint4 *)s_bitmap)[g]);
+      if (!sparse) {
+        for (int g = g0; g < g1; ++g) {
+          s_gp[g] = (unsigned short)rg;
+          rg += popc4(((const uint4 *)s_bitmap)[g]);
+        }
+      } else {
+        for (int g = g0; g < g1; ++g) {
+          s_l2p[g] = (unsigned short)rg;
+          rg += __popc(s_bitmap[g]);
+        }
       }
       n_trk = (int)(tot & 0xffffu), n_slots = (int)(tot >> 16);
     }
     __syncthreads();
+    if (sparse) {
+      // ---- sparse mode: n_slots is so far the number of NON-EMPTY GROUPS (<= deposits <= C).  Their tower bits go
+      // into the pool, at the rank of the group in (event, group) order; a second scan turns them into slots.
+      const int n_groups = n_slots;
+      for (int k = tid; k < n_groups; k += THREADS) s_pool[k] = make_uint4(0u, 0u, 0u, 0u);
+      __syncthreads();
+      for (int i = tid; i < n; i += THREADS) {
+        const uint32_t r = s_res[i];
+        if (r & RES_DEP) {
+          const int id = (int)(r & RES_TOWER);
+          const int w = (multi ? (int)s_ev[i] * l2w : 0) + (id >> 12);
+          const int pg = (int)s_l2p[w] + __popc(s_bitmap[w] & ((1u << ((id >> 7) & 31)) - 1u));
+          atomicOr(&((uint32_t *)s_pool)[4 * pg + ((id >> 5) & 3)], 1u << (id & 31));
+        }
+      }
+      __syncthreads();
+      const int kp = ((n_groups + THREADS - 1) / THREADS) | 1;
+      const int q0 = min(n_groups, tid * kp), q1 = min(n_groups, q0 + kp);
+      unsigned cnt_p = 0;
+      for (int g = q0; g < q1; ++g) cnt_p += (unsigned)popc4(s_pool[g]);
+      const unsigned incl_p = warp_incl_scan(cnt_p);
+      if (lane == 31) s_wtot[wid] = incl_p;
+      __syncthreads();
+      unsigned excl_wp, tot_p;
+      warp_totals_scan<W>(s_wtot, excl_wp, tot_p);
+      int rp = (int)(excl_wp + incl_p - cnt_p);
+      for (int g = q0; g < q1; ++g) {
+        s_gp[g] = (unsigned short)rp;
+        rp += popc4(s_pool[g]);
+      }
+      n_slots = (int)tot_p;
+      __syncthreads();
+    }
 
     // ------------------------------------------------------------------ publish chain T; pass B
     // the track aggregate is published now and its prefix resolved only at the end of the tile (pass O), when
@@ -438,8 +510,17 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
       const uint32_t r = s_res[i];
       if (r & RES_DEP) {
         const int id = (int)(r & RES_TOWER);
-        const int g = (multi ? (int)s_ev[i] * gpe : 0) + (id >> 7);
-        const int slot = (int)s_gp[g] + popc_below(((const uint4 *)s_bitmap)[g], id & 127);
+        int g;
+        uint4 bits;
+        if (!sparse) {
+          g = (multi ? (int)s_ev[i] * gpe : 0) + (id >> 7);
+          bits = ((const uint4 *)s_bitmap)[g];
+        } else {
+          const int w = (multi ? (int)s_ev[i] * l2w : 0) + (id >> 12);
+          g = (int)s_l2p[w] + __popc(s_bitmap[w] & ((1u << ((id >> 7) & 31)) - 1u));
+          bits = s_pool[g];
+        }
+        const int slot = (int)s_gp[g] + popc_below(bits, id & 127);
         const unsigned prev = atomicExch(&s_head[slot], (unsigned)i);
         s_res[i] = (r & ~(LINK_END << RES_LINK_SHIFT)) | ((prev & LINK_END) << RES_LINK_SHIFT);
       }
@@ -713,9 +794,10 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   const PdCardScalars &sc = c->sc;
   const double avg = n_events > 0 ? double(n_particles) / double(n_events) : 0.0;
   const size_t budget2 = (228 * 1024 - 2 * 1024) / 2, budget1 = 227 * 1024;
+  int sparse = 0;
   auto cap_for = [&](int G, size_t budget) {
-    const size_t fixed = pdk::make_layout(sc.n_bins, 2 * sc.lut_side, sc.n_towers, sc.words_per_event, G, 0).total;
-    const size_t per = 22 + (G > 1 ? 1 : 0);
+    const size_t fixed = pdk::make_layout(sc.n_bins, 2 * sc.lut_side, sc.n_towers, sc.words_per_event, G, 0, sparse).total;
+    const size_t per = 22 + (G > 1 ? 1 : 0) + (sparse ? 18 : 0);
     long cap = budget > fixed + 7 * 16 ? long((budget - fixed - 7 * 16) / per) : 0;
     cap &= ~3L;
     return int(cap > pdk::C_MAX ? pdk::C_MAX : cap);
@@ -735,6 +817,17 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   }
   int g = 1;
   while (g < pdk::G_MAX && fits(g + 1, budget)) ++g;
+  {
+    // sparse mode (two-level tower bitmap) when it packs clearly more events into a tile: large grids, small events
+    static const int force_sparse = std::getenv("PD_SPARSE") ? std::atoi(std::getenv("PD_SPARSE")) : -1;
+    const int g_dense = g;
+    sparse = 1;
+    int gs = 1;
+    while (gs < pdk::G_MAX && fits(gs + 1, budget)) ++gs;
+    const bool take = t_tile_events != 1 && (force_sparse >= 0 ? force_sparse != 0 : (g_dense > 1 && 2 * gs >= 3 * g_dense));
+    if (take && fits(1, budget)) g = gs;
+    else sparse = 0;
+  }
   // keep all CTA slots busy: aim for >= 4 tiles per resident CTA when the input is small
   const long slots = 148L * (plan->threads == 512 ? 2 : 1);
   const long g_bal = long((n_events + 4 * slots - 1) / (4 * slots));
@@ -749,7 +842,8 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
     const long ctas = sms * (plan->threads == 1024 ? 1 : 2);
     plan->max_ctas = int(plan->n_tiles < ctas ? (plan->n_tiles > 0 ? plan->n_tiles : 1) : ctas);
   }
-  plan->smem_bytes = pdk::make_layout(sc.n_bins, 2 * sc.lut_side, sc.n_towers, sc.words_per_event, g, plan->capacity).total;
+  plan->sparse = sparse;
+  plan->smem_bytes = pdk::make_layout(sc.n_bins, 2 * sc.lut_side, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse).total;
   return PD_OK;
 }
 

@@ -21,7 +21,7 @@ wl = importlib.import_module("workloads.generate")
 
 pytestmark = pytest.mark.gpu
 
-WINDOWS = {2: 3, 3: 300}  # events per sampled window
+WINDOWS = {2: 3, 3: 300, 4: 300}  # events per sampled window
 
 
 def _slice_outputs(full, prefix, e0, e1):
@@ -34,7 +34,7 @@ def _slice_outputs(full, prefix, e0, e1):
     return out
 
 
-@pytest.mark.parametrize("cfg", [2, 3])
+@pytest.mark.parametrize("cfg", [2, 3, 4])  # 4: the sparse (two-level bitmap) tiling
 def test_full_size_sampled_parity_and_invariants(cfg):
     import paper_2606_26089_b200 as pd
     from gpu_util import run_gpu
