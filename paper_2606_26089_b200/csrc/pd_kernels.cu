@@ -264,7 +264,7 @@ __device__ __forceinline__ int popc_below(const uint4 &v, int pos) {
   return c;
 }
 
-template <int THREADS, int CTAS, bool DEBUG>
+template <int THREADS, int CTAS, bool DEBUG, bool SPARSE>
 __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_constant__ PdParams prm) {
   constexpr int W = THREADS / 32;
   extern __shared__ __align__(16) unsigned char smem[];
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_chain_kernel(const __grid_co
   const int nb = sc.n_bins;
   const int C = prm.capacity, G = prm.events_per_tile;
   const int wpe = sc.words_per_event, gpe = wpe >> 2;
-  const bool sparse = prm.sparse != 0;
+  constexpr bool sparse = SPARSE;  // two-level tower bitmap, chosen by pd_plan (prm.sparse)
   const int l2w = (gpe + 31) >> 5;  // words of the per-event group bitmap (sparse mode)
   const Layout L = make_layout(nb, 2 * sc.lut_side, sc.n_towers, wpe, G, C, prm.sparse);
   float *s_tb = (float *)(smem + L.tb);
@@ -847,10 +847,10 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   return PD_OK;
 }
 
-template <int THREADS, bool DEBUG>
+template <int THREADS, bool DEBUG, bool SPARSE>
 static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
   constexpr int CTAS = THREADS == 512 ? 2 : 1;
-  auto kern = pdk::pd_chain_kernel<THREADS, CTAS, DEBUG>;
+  auto kern = pdk::pd_chain_kernel<THREADS, CTAS, DEBUG, SPARSE>;
   static bool configured = false;
   if (!configured) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g_max_smem_optin) != cudaSuccess) return PD_ECUDA;
@@ -872,6 +872,10 @@ int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, v
   if (query_device() != PD_OK) return PD_ECUDA;
   if (plan.smem_bytes > (size_t)g_max_smem_optin) return PD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
-  if (plan.threads == 1024) return debug ? launch_variant<1024, true>(prm, plan, st) : launch_variant<1024, false>(prm, plan, st);
-  return debug ? launch_variant<512, true>(prm, plan, st) : launch_variant<512, false>(prm, plan, st);
+  if (plan.threads == 1024) {
+    if (plan.sparse) return PD_EINVAL;  // pd_plan never pairs the two
+    return debug ? launch_variant<1024, true, false>(prm, plan, st) : launch_variant<1024, false, false>(prm, plan, st);
+  }
+  if (plan.sparse) return debug ? launch_variant<512, true, true>(prm, plan, st) : launch_variant<512, false, true>(prm, plan, st);
+  return debug ? launch_variant<512, true, false>(prm, plan, st) : launch_variant<512, false, false>(prm, plan, st);
 }
