@@ -1113,3 +1113,76 @@ int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_p
   }
   return rc;
 }
+
+/* ---- track impact parameters (Table 2) ----
+ * Geometry of one trajectory, written as the definition: the helix of step S1 (reading A3), extended in both
+ * directions, or the straight line when q B = 0.  See the header for the conventions. */
+int pdo_impact_true(const pdo_card *c, int q, double px, double py, double pz, double vx, double vy, double vz,
+                    double *d0, double *z0) {
+  const double pt = hypot(px, py), B = c->bz;
+  if (!(pt > 0.0)) return PDO_EINVAL;
+  if (q == 0 || B == 0.0) {
+    /* straight line: closest approach at t = -(v.p)_T / pT^2; the direction of flight is the same everywhere */
+    double t = -(vx * px + vy * py) / (pt * pt);
+    double xd = vx + t * px, yd = vy + t * py;
+    *d0 = (xd * py - yd * px) / pt;
+    *z0 = vz + t * pz;
+    return PDO_OK;
+  }
+  {
+    /* circle of S1: radius rho, rotation sense s, centre (cx, cy) */
+    double rho = pt / (c->kappa * fabs((double)q) * fabs(B));
+    double s = -sgn((double)q * B);
+    double phi0 = atan2(py, px);
+    double cx = vx - s * rho * sin(phi0), cy = vy + s * rho * cos(phi0);
+    double rc = hypot(cx, cy);
+    double xd, yd, tx, ty, psi_v, psi_d, alpha;
+    if (rc == 0.0) {
+      /* the circle is centred on the axis: every point is equally close; the vertex itself is taken */
+      *d0 = (vx * py - vy * px) / pt;
+      *z0 = vz;
+      return PDO_OK;
+    }
+    /* the point of the circle nearest to the axis lies on the line from the centre through the origin */
+    xd = cx - rho * cx / rc, yd = cy - rho * cy / rc;
+    /* direction of flight there: the radius vector (xd - cx, yd - cy) turned by s * 90 degrees */
+    tx = -s * (yd - cy) / rho, ty = s * (xd - cx) / rho;
+    *d0 = xd * ty - yd * tx;
+    /* turning angle from the vertex to that point, in the sense of rotation, the shorter way round */
+    psi_v = atan2(vy - cy, vx - cx), psi_d = atan2(yd - cy, xd - cx);
+    alpha = remainder(s * (psi_d - psi_v), PDO_TWO_PI);
+    *z0 = vz + rho * alpha * pz / pt;
+  }
+  return PDO_OK;
+}
+
+int pdo_track_impact(const pdo_card *c, const pdo_events *ev, const int64_t *trk_offsets, const int32_t *trk_src,
+                     double d0_a, double d0_b, double z0_a, double z0_b, uint64_t seed, int64_t event_base,
+                     double *d0_true, double *z0_true, double *d0, double *z0, double *d0_err, double *z0_err) {
+  int64_t e, t;
+  if (!c || !ev || !trk_offsets || !trk_src || !d0 || !z0 || !d0_err || !z0_err) return PDO_EINVAL;
+  if (d0_a < 0 || d0_b < 0 || z0_a < 0 || z0_b < 0) return PDO_EINVAL;
+  for (e = 0; e < ev->n_events; ++e) {
+    for (t = trk_offsets[e]; t < trk_offsets[e + 1]; ++t) {
+      const int64_t i = trk_src[t];
+      double dt, zt, pt, sd, sz;
+      uint32_t r[4];
+      int rc;
+      if (i < ev->offsets[e] || i >= ev->offsets[e + 1]) return PDO_EINVAL;
+      rc = pdo_impact_true(c, ev->charge[i], ev->px[i], ev->py[i], ev->pz[i], ev->vx[i], ev->vy[i], ev->vz[i], &dt, &zt);
+      if (rc != PDO_OK) return rc;
+      pt = hypot((double)ev->px[i], (double)ev->py[i]);
+      /* reading I2: sigma = a (+) b / pT, Gaussian, independent for d0 and z0; reported as the errors */
+      sd = sqrt(d0_a * d0_a + (d0_b / pt) * (d0_b / pt));
+      sz = sqrt(z0_a * z0_a + (z0_b / pt) * (z0_b / pt));
+      /* reading I3: stream 3 of A26, object = particle index within its event; words 0,1 -> d0, words 2,3 -> z0 */
+      pdo_rng_block(seed, event_base + e, (uint32_t)(i - ev->offsets[e]), 3u, r);
+      if (d0_true) d0_true[t] = dt;
+      if (z0_true) z0_true[t] = zt;
+      d0[t] = dt + sd * pdo_normal(r[0], r[1]);
+      z0[t] = zt + sz * pdo_normal(r[2], r[3]);
+      d0_err[t] = sd, z0_err[t] = sz;
+    }
+  }
+  return PDO_OK;
+}

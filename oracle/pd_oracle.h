@@ -214,6 +214,33 @@ int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_p
                      float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz, uint8_t *is_pu,
                      int32_t *n_pileup /* [n_events], may be NULL */);
 
+/* ---- track impact parameters ("where supported, track impact parameters"; P:L138
+ * Table 2 "d_0, z_0 and their errors for charged particles"; P:L424-426 PFlow.D0 / PFlow.Z0) ----
+ * The paper names the outputs and gives no formula; readings I1..I3 of DESIGN.md section 14:
+ *   I1 (geometry, the textbook definition): the trajectory is the helix of S1 (reading A3: q > 0 in a +z field turns
+ *      clockwise; radius rho = pT / (kappa |q| |B|)) through the production vertex, extended in BOTH directions
+ *      (the straight line through the vertex along the momentum when q B = 0).  (x_d, y_d) is its point nearest to
+ *      the beam (z) axis in the transverse plane and t^ the transverse direction of flight there:
+ *          d0 = x_d t^_y - y_d t^_x      (metres; sign of the z component of the angular momentum -- for a straight
+ *                                         line this is the familiar (vx py - vy px) / pT)
+ *          z0 = z of the trajectory at that point (reached from the vertex by the shorter arc, forwards or backwards).
+ *      A circle centred exactly on the axis has no nearest point: the vertex itself is taken.  A vertex exactly
+ *      half a turn away from the nearest point makes z0 two-valued (+- pi rho pz/pT): not covered by parity.
+ *   I2 (resolution): sigma_d0 = sqrt(d0_a^2 + (d0_b / pT)^2), sigma_z0 likewise (pT = truth transverse momentum in
+ *      GeV; a in metres, b in metres GeV: the usual a (+) b/pT form); the measured values are the true ones plus
+ *      sigma times a standard normal, independently for d0 and z0; the "errors" of Table 2 are the two sigmas.
+ *   I3 (random numbers): stream 3 of reading A26, object = index of the particle within its event, block 0;
+ *      words 0,1 drive d0 (pdo_normal), words 2,3 drive z0.
+ * pdo_impact_true is the geometry alone; pdo_track_impact runs over the tracks of a call (trk_offsets [n_events+1],
+ * trk_src = index of the truth particle within the call, both as produced by pdo_simulate).  d0_true / z0_true may
+ * be NULL.  Parity status: geometry pinned by RK4 integration of the Lorentz force, worked cases and invariance
+ * along the helix (tests/test_oracle_impact.py); the resolution model is a reading (the paper's own: unpinned). */
+int pdo_impact_true(const pdo_card *c, int q, double px, double py, double pz, double vx, double vy, double vz,
+                    double *d0, double *z0);
+int pdo_track_impact(const pdo_card *c, const pdo_events *ev, const int64_t *trk_offsets, const int32_t *trk_src,
+                     double d0_a, double d0_b, double z0_a, double z0_b, uint64_t seed, int64_t event_base,
+                     double *d0_true, double *z0_true, double *d0, double *z0, double *d0_err, double *z0_err);
+
 const char *pdo_strerror(int code);
 
 /* ---- building blocks exposed so that tests can pin them one by one ---- */

@@ -111,6 +111,8 @@ def lib():
                                        C.c_uint64, C.c_int64, C.c_int64] + [_p] * 12
         L.pdo_filter_eflow.argtypes = [C.c_int64] + [_p] * 7 + [C.POINTER(_Condition), C.c_int32, C.c_int32] + [_p] * 8
         L.pdo_event_features.argtypes = [C.POINTER(_Objects), C.c_double, C.c_double] + [_p] * 9
+        L.pdo_impact_true.argtypes = [_p, C.c_int] + [C.c_double] * 6 + [C.POINTER(C.c_double)] * 2
+        L.pdo_track_impact.argtypes = [_p, C.POINTER(_Events), _p, _p] + [C.c_double] * 4 + [C.c_uint64, C.c_int64] + [_p] * 6
         _lib = L
     return _lib
 
@@ -174,6 +176,15 @@ class Card:
                                  float(vz), *[C.byref(o) for o in out])
         x, y, z, alpha, eta_pos, phi_pos = [o.value for o in out]
         return dict(status=st, x=x, y=y, z=z, alpha=alpha, eta_pos=eta_pos, phi_pos=phi_pos)
+
+    def impact_true(self, q, px, py, pz, vx=0.0, vy=0.0, vz=0.0):
+        """pdo_impact_true (reading I1): (d0, z0) of one trajectory, metres."""
+        d0, z0 = C.c_double(), C.c_double()
+        rc = lib().pdo_impact_true(self._h, int(q), float(px), float(py), float(pz), float(vx), float(vy), float(vz),
+                                   C.byref(d0), C.byref(z0))
+        if rc != 0:
+            raise OracleError(rc)
+        return d0.value, z0.value
 
 
 def philox(ctr, key):
@@ -366,3 +377,19 @@ def pileup_merge(hs, pool, mean_pileup: float, sigma_z: float = 0.053, max_z_spr
     res = {k: v[: int(off[-1])] for k, v in out.items()}
     res["offsets"], res["n_pileup"] = off, npu[:ne]
     return res
+
+
+def track_impact(card: Card, ev, trk_offsets, trk_src, d0_res=(0.0, 0.0), z0_res=(0.0, 0.0), seed: int = 0,
+                 event_base: int = 0) -> dict:
+    """pdo_track_impact (readings I1..I3): d0_true, z0_true, d0, z0, d0_err, z0_err per track (fp64, metres)."""
+    cev, keep = _events_struct(ev)
+    off = np.ascontiguousarray(trk_offsets, dtype=np.int64)
+    src = np.ascontiguousarray(trk_src, dtype=np.int32)
+    n = int(off[-1])
+    out = {k: np.zeros(max(n, 1), dtype=np.float64) for k in ("d0_true", "z0_true", "d0", "z0", "d0_err", "z0_err")}
+    rc = lib().pdo_track_impact(card._h, C.byref(cev), _ptr(off), _ptr(src), float(d0_res[0]), float(d0_res[1]),
+                                float(z0_res[0]), float(z0_res[1]), int(seed) & (2**64 - 1), int(event_base),
+                                *[_ptr(out[k]) for k in ("d0_true", "z0_true", "d0", "z0", "d0_err", "z0_err")])
+    if rc != 0:
+        raise OracleError(rc)
+    return {k: v[:n] for k, v in out.items()}
