@@ -269,6 +269,19 @@ def run_ours(args, rank, world, local_rank):
     filt_ms = f0.elapsed_time(f1) / f_steps
     kept = int(dst.t["offsets"][-1])
     del dst, ws_keep
+    # ---- impact parameters d0, z0 and their errors for the step's tracks
+    imp = pd.DeviceImpact(max(n, 1))
+    ip_res = ((20e-6, 40e-6), (30e-6, 60e-6))
+    for _ in range(2):
+        pd.track_impact(card, dev, out, imp, *ip_res, seed=seed, event_base=event_base)
+    barrier()
+    f0.record(stream)
+    for _ in range(f_steps):
+        pd.track_impact(card, dev, out, imp, *ip_res, seed=seed, event_base=event_base)
+    f1.record(stream)
+    barrier()
+    imp_ms = f0.elapsed_time(f1) / f_steps
+    del imp
 
     # ---- pile-up merging, the step right before the hot path: 5,000 cfg0-like hard-scatter
     # events, a pool of 20,000 cfg3-like minimum-bias events, mean pile-up 50 (Table C.9 defaults otherwise)
@@ -338,6 +351,10 @@ def run_ours(args, rank, world, local_rank):
                                   "kernels": "pd_pileup_count/scan/fill_kernel", "algorithmic_bytes": 67 * pu_total + 20 * hs_ev.n_events,
                                   "hbm_frac": (67 * pu_total + 20 * hs_ev.n_events) / (pu_ms * 1e-3) / 1e9 / peak,
                                   "note": "5,000 cfg0-like events + Poisson(50) of 20,000 cfg3-like min-bias events; 3 launches; rank 0, not in value"},
+                 "track_impact": {"ms": imp_ms, "tracks_per_s": totals[0] / (imp_ms * 1e-3), "kernel": "pd_impact_kernel",
+                                  "algorithmic_bytes": 45 * totals[0] + 16 * (ne + 1),
+                                  "hbm_frac": (45 * totals[0] + 16 * (ne + 1)) / (imp_ms * 1e-3) / 1e9 / peak,
+                                  "note": "d0, z0 and errors (a (+) b/pT) for the step's tracks; truth particles gathered through trk.src; 1 launch; rank 0, not in value"},
                  "particle_filter": {"ms": filt_ms, "objects_per_s": totals[2] / (filt_ms * 1e-3), "kept": kept, "kernel": "pd_filter_kernel",
                                      "algorithmic_bytes": 21 * totals[2] + 21 * kept + 16 * (ne + 1),
                                      "hbm_frac": (21 * totals[2] + 21 * kept + 16 * (ne + 1)) / (filt_ms * 1e-3) / 1e9 / peak,

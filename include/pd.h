@@ -245,6 +245,35 @@ int pd_pileup_merge(const pd_events *hs, const pd_events *pool, const pd_pileup_
                     int64_t event_base, pd_merged_events *out, void *workspace, int64_t workspace_bytes,
                     void *cuda_stream);
 
+/* ---- Track impact parameters ("where supported, track impact parameters"; L138 Table 2 "d_0, z_0
+ * and their errors for charged particles"; L424-426 PFlow.D0 / PFlow.Z0) ----
+ * The paper names the outputs and prints no formula; readings I1-I3 of DESIGN.md section 14:
+ *   geometry: the trajectory is the helix of step S1 through the production vertex, extended in both directions
+ *     (a straight line when q B = 0); (x_d, y_d) is its point nearest to the beam (z) axis and t^ the transverse
+ *     direction of flight there: d0 = x_d t^_y - y_d t^_x, z0 = z of the trajectory at that point (metres; the
+ *     shorter arc from the vertex).  For a straight line d0 = (vx py - vy px) / pT.
+ *   resolution: sigma = sqrt(a^2 + (b / pT)^2) (pT = truth pT in GeV; a metres, b metres GeV) for d0 and for z0;
+ *     measured = true + sigma * standard normal, independent for the two; the sigmas are the reported errors.
+ *   random numbers: Philox stream 3, object = index of the particle within its event, words 0,1 -> d0, 2,3 -> z0
+ *     (same key and event numbering as pd_simulate, so splitting a batch does not change a value).
+ * One value per track of `tracks` (the collection a pd_simulate call wrote for `events` on the same stream or
+ * after synchronisation): only tracks->offsets and tracks->src are read.  a = b = 0 gives the true values. */
+typedef struct {
+  float d0_a, d0_b; /* metres, metres GeV; >= 0 */
+  float z0_a, z0_b;
+} pd_impact_config;
+
+typedef struct {
+  float *d0, *z0, *d0_err, *z0_err; /* DEVICE arrays of at least tracks->capacity (>= n_particles) elements */
+} pd_impact;
+
+/* card, events, tracks, out: structs in HOST memory whose pointer members are DEVICE pointers.  Asynchronous on
+ * cuda_stream, one kernel launch, no workspace, allocates nothing.  Errors: PD_EINVAL (null pointers, negative
+ * sizes or resolutions), PD_ECUDA. */
+int pd_track_impact(const pd_card *card, const pd_events *events, const pd_tracks *tracks,
+                    const pd_impact_config *cfg, uint64_t seed, int64_t event_base, pd_impact *out,
+                    void *cuda_stream);
+
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 

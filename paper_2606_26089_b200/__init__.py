@@ -3,5 +3,5 @@
 `binding` marshals torch tensors into libpd.so; every step of the chain runs in its CUDA kernels.
 There is no CPU fallback."""
 from . import binding  # noqa: F401
-from .binding import (Card, DeviceEFlow, DeviceEvents, DeviceFeatures, DeviceMerged, DeviceObjects, DeviceOutputs, HostBuffers, PdError, last_launch_count, last_status,  # noqa: F401
-                      event_features, filter_eflow, pileup_merge, pileup_status, set_tile_events, simulate, simulate_host, workspace_bytes)
+from .binding import (Card, DeviceEFlow, DeviceImpact, DeviceTrackRefs, DeviceEvents, DeviceFeatures, DeviceMerged, DeviceObjects, DeviceOutputs, HostBuffers, PdError, last_launch_count, last_status,  # noqa: F401
+                      event_features, filter_eflow, pileup_merge, pileup_status, set_tile_events, simulate, simulate_host, track_impact, workspace_bytes)

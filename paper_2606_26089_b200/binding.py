@@ -18,7 +18,7 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_track_impact", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
@@ -40,6 +40,14 @@ class Condition(C.Structure):
 
 FIELDS = {"pt": 0, "eta": 1, "phi": 2, "E": 3, "cls": 4}
 OPS = {">": 0, ">=": 1, "<": 2, "<=": 3, "==": 4, "!=": 5, "in": 6, "not in": 7}
+
+
+class ImpactConfig(C.Structure):
+    _fields_ = [("d0_a", C.c_float), ("d0_b", C.c_float), ("z0_a", C.c_float), ("z0_b", C.c_float)]
+
+
+class Impact(C.Structure):
+    _fields_ = [(k, _p) for k in ("d0", "z0", "d0_err", "z0_err")]
 
 
 class PileupConfig(C.Structure):
@@ -119,6 +127,8 @@ def lib():
         L.pd_filter_eflow.argtypes = [C.POINTER(EFlow), C.c_int64, C.POINTER(Condition), C.c_int32, C.c_int32, C.POINTER(EFlow), _p,
                                       C.c_int64, _p]
         L.pd_event_features.argtypes = [C.POINTER(EFlow), C.c_int64, C.c_float, C.c_float, C.POINTER(Features), _p]
+        L.pd_track_impact.argtypes = [_p, C.POINTER(Events), C.POINTER(Tracks), C.POINTER(ImpactConfig), C.c_uint64, C.c_int64,
+                                      C.POINTER(Impact), _p]
         L.pd_simulate_host.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks),
                                        C.POINTER(Towers), C.POINTER(EFlow), _p]
         L.pd_strerror.argtypes = [C.c_int]
@@ -346,6 +356,47 @@ def event_features(out, feat: DeviceFeatures, dr_max: float = 0.4, fsr_dr: float
     st = torch.cuda.current_stream() if stream is None else stream
     _check(lib().pd_event_features(C.byref(out.c_efl), int(out.n_events), float(dr_max), float(fsr_dr), C.byref(feat.c),
                                    C.c_void_p(st.cuda_stream)))
+
+
+class DeviceTrackRefs:
+    """The two arrays of a track collection that pd_track_impact reads (offsets, src), uploaded from numpy: its input
+    when the tracks do not come from a DeviceOutputs."""
+
+    def __init__(self, offsets, src, device="cuda"):
+        torch = _torch()
+        self.n_events = int(len(offsets) - 1)
+        self.n_tracks = int(offsets[-1])
+        self.offsets = torch.from_numpy(np.ascontiguousarray(offsets, dtype=np.int64)).to(device)
+        src = np.ascontiguousarray(src, dtype=np.int32)
+        self.src = torch.from_numpy(src if src.size else np.zeros(1, dtype=np.int32)).to(device)
+        self.c_trk = Tracks(max(self.n_tracks, 1), _tptr(self.offsets), _tptr(self.src), *([None] * (len(TRACK_FIELDS) - 1)))
+
+
+class DeviceImpact:
+    """Buffers of pd_track_impact: d0, z0, d0_err, z0_err per track (fp32, metres)."""
+
+    FIELDS = ("d0", "z0", "d0_err", "z0_err")
+
+    def __init__(self, capacity: int, device="cuda"):
+        torch = _torch()
+        self.t = {k: torch.empty(max(int(capacity), 1), dtype=torch.float32, device=device) for k in self.FIELDS}
+        self.c = Impact(*[_tptr(self.t[k]) for k in self.FIELDS])
+
+    def to_numpy(self, n_tracks: int) -> dict:
+        _torch().cuda.synchronize()
+        return {k: t[: int(n_tracks)].cpu().numpy() for k, t in self.t.items()}
+
+
+def track_impact(card: Card, dev_events: DeviceEvents, tracks, out: DeviceImpact, d0_res=(0.0, 0.0), z0_res=(0.0, 0.0),
+                 seed: int = 0, event_base: int = 0, stream=None):
+    """pd_track_impact for the tracks of `tracks` (a DeviceOutputs after simulate, or a DeviceTrackRefs).  Asynchronous."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    cfg = ImpactConfig(float(d0_res[0]), float(d0_res[1]), float(z0_res[0]), float(z0_res[1]))
+    _check(lib().pd_track_impact(card._h, C.byref(dev_events.c), C.byref(tracks.c_trk), C.byref(cfg), int(seed) & (2**64 - 1),
+                                 int(event_base), C.byref(out.c), C.c_void_p(st.cuda_stream)))
 
 
 def simulate(card: Card, dev_events: DeviceEvents, out: DeviceOutputs, seed: int, event_base: int = 0, stream=None):

@@ -244,6 +244,35 @@ int pd_event_features(const pd_eflow *efl, int64_t n_events, float dr_max, float
   return PD_OK;
 }
 
+int pd_track_impact(const pd_card *card, const pd_events *ev, const pd_tracks *trk, const pd_impact_config *cfg,
+                    uint64_t seed, int64_t event_base, pd_impact *out, void *cuda_stream) {
+  t_launches = 0;
+  if (!card || !ev || !trk || !cfg || !out || ev->n_events < 0 || ev->n_particles < 0) return PD_EINVAL;
+  if (!(cfg->d0_a >= 0.f) || !(cfg->d0_b >= 0.f) || !(cfg->z0_a >= 0.f) || !(cfg->z0_b >= 0.f)) return PD_EINVAL;
+  if (!std::isfinite(cfg->d0_a) || !std::isfinite(cfg->d0_b) || !std::isfinite(cfg->z0_a) || !std::isfinite(cfg->z0_b))
+    return PD_EINVAL;
+  if (ev->n_events == 0 || ev->n_particles == 0) return PD_OK;
+  if (!ev->offsets || !ev->charge || !ev->px || !ev->py || !ev->pz || !ev->vx || !ev->vy || !ev->vz) return PD_EINVAL;
+  if (!trk->offsets || !trk->src || !out->d0 || !out->z0 || !out->d0_err || !out->z0_err) return PD_EINVAL;
+  PdImpactParams p;
+  p.n_events = ev->n_events, p.n_particles = ev->n_particles;
+  p.ev_off = (const long long *)ev->offsets, p.trk_off = (const long long *)trk->offsets;
+  p.trk_src = trk->src, p.charge = ev->charge;
+  p.px = ev->px, p.py = ev->py, p.pz = ev->pz, p.vx = ev->vx, p.vy = ev->vy, p.vz = ev->vz;
+  p.inv_kB = card->sc.inv_kB, p.sB = card->sc.sB;
+  p.d0_a = cfg->d0_a, p.d0_b = cfg->d0_b, p.z0_a = cfg->z0_a, p.z0_b = cfg->z0_b;
+  for (int r = 0; r < 10; ++r) {
+    p.rk.k0[r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+    p.rk.k1[r] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+  }
+  p.event_base = event_base;
+  p.d0 = out->d0, p.z0 = out->z0, p.d0_err = out->d0_err, p.z0_err = out->z0_err;
+  const int rc = pd_launch_impact(p, cuda_stream);
+  if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "impact kernel launch");
+  t_launches = 1;
+  return PD_OK;
+}
+
 }  // extern "C"
 
 // Upload the per-bin tables of a card to the current device (once).

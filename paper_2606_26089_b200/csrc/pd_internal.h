@@ -201,3 +201,18 @@ struct PdPileupParams {
   unsigned long long *chain;   // workspace: one self-flagged look-back word per scan tile
 };
 int pd_launch_pileup(const PdPileupParams &prm, void *stream);
+
+// pd_impact.cu: track impact parameters (pd_track_impact)
+struct PdImpactParams {
+  long long n_events, n_particles;
+  const long long *ev_off, *trk_off;
+  const int *trk_src;
+  const signed char *charge;
+  const float *px, *py, *pz, *vx, *vy, *vz;
+  float inv_kB, sB;                 // 1 / (kappa |B|), sign of B (0: no field)
+  float d0_a, d0_b, z0_a, z0_b;     // sigma = a (+) b / pT
+  PdPhiloxKeys rk;
+  long long event_base;
+  float *d0, *z0, *d0_err, *z0_err;
+};
+int pd_launch_impact(const PdImpactParams &prm, void *stream);

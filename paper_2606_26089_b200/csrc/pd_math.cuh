@@ -243,7 +243,7 @@ __device__ __forceinline__ double rcp_d(double x) {
   return y * fma(-x, y, 2.0);
 }
 
-__device__ __noinline__ bool graze_double(const PdCardScalars &sc, float px, float py, float vx, float vy, float aq,
+static __device__ __noinline__ bool graze_double(const PdCardScalars &sc, float px, float py, float vx, float vy, float aq,
                                           float s, float &cc, float &ss) {
   const double pxd = px, pyd = py, vxd = vx, vyd = vy, Rd = sc.R;
   const double p2 = pxd * pxd + pyd * pyd;
