@@ -159,3 +159,33 @@ def test_reproducible_split_invariant_and_fed_by_the_chain():
     h = _run_gpu(name, sub, chain["trk_offsets"][cut:] - mt, chain["trk_src"][mt:] - m, *RES, seed=seed, event_base=cut)
     for k in a:
         assert h[k].tobytes() == a[k][mt:].tobytes(), k
+
+
+def test_unaligned_arrays_take_the_scalar_path():
+    """The C ABI accepts any 4-byte-aligned arrays: with src / outputs off the 16-byte grid the kernel must fall back
+    from its vector loads and stores and give the same bits."""
+    import paper_2606_26089_b200 as pd
+    from paper_2606_26089_b200 import binding as B
+    import torch
+
+    ev = _displaced(12, np.random.default_rng(4).poisson(40, 300), r_max=0.1)
+    off, src = _all_tracks(ev)
+    n = len(src)
+    card, dev = pd.Card("cms_like"), pd.DeviceEvents(ev)
+    refs = pd.DeviceTrackRefs(off, src)
+    out = pd.DeviceImpact(n)
+    pd.track_impact(card, dev, refs, out, *RES, seed=8)
+    a = out.to_numpy(n)
+    # same call with every array shifted by one element
+    big_src = torch.zeros(n + 1, dtype=torch.int32, device="cuda")
+    big_src[1:] = refs.src
+    refs.src = big_src[1:]
+    refs.c_trk = B.Tracks(n, B._tptr(refs.offsets), B._tptr(refs.src), *([None] * (len(B.TRACK_FIELDS) - 1)))
+    assert refs.src.data_ptr() % 16 == 4
+    out2 = pd.DeviceImpact(n + 1)
+    views = {k: t[1:] for k, t in out2.t.items()}
+    out2.c = B.Impact(*[B._tptr(views[k]) for k in out2.FIELDS])
+    pd.track_impact(card, dev, refs, out2, *RES, seed=8)
+    torch.cuda.synchronize()
+    for k in a:
+        assert views[k][:n].cpu().numpy().tobytes() == a[k].tobytes(), k
