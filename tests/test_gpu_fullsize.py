@@ -101,3 +101,71 @@ def test_full_size_sampled_parity_and_invariants(cfg):
         overridden += rep["overridden_particles"]
     print("cfg%d full size: %d particles, %d tracks, %d towers, %d eflow; sampled windows near-edge flagged %d, overridden %d"
           % (cfg, n, n_trk, n_tow, n_efl, flagged, overridden))
+
+
+def test_full_size_steps_around_the_chain():
+    """cfg2 at full size: impact parameters, event features and the particle filter run on the device-resident output
+    of the full-size chain call (as bench.py's `next` legs do).  Checked on sampled windows of events against the
+    oracle (whose inputs here are the window's slices of the chain output -- inputs, not expected values) and by
+    properties over the whole output."""
+    import paper_2606_26089_b200 as pd
+    from oracle import pdo
+
+    cfg = 2
+    ev = wl.generate(cfg, None)
+    seed, name = wl.CONFIGS[cfg]["seed"], wl.config_card(cfg)
+    ne, n = ev.n_events, ev.n_particles
+    card, dev = pd.Card(name), pd.DeviceEvents(ev)
+    out = pd.DeviceOutputs(card, ne, n)
+    pd.simulate(card, dev, out, seed)
+    res = ((20e-6, 40e-6), (30e-6, 60e-6))
+    imp = pd.DeviceImpact(n)
+    pd.track_impact(card, dev, out, imp, *res, seed=seed)
+    feat = pd.DeviceFeatures(ne, 2 * n)
+    pd.event_features(out, feat)
+    conds = [{"field": "pt", "op": ">", "value": 0.5}, {"field": "eta", "op": "<", "value": 2.5, "abs": True}]
+    dst = pd.DeviceEFlow(ne, 2 * n)
+    ws = pd.filter_eflow(out, dst, conds, "all")
+    chain = out.to_numpy()
+    n_trk, n_efl = int(chain["trk_offsets"][-1]), int(chain["efl_offsets"][-1])
+    gi, gf, gd = imp.to_numpy(n_trk), feat.to_numpy(n_efl), dst.to_numpy()
+    del ws
+
+    # ---- whole output: the filter is a boolean mask (exact), the impact errors a closed form
+    keep = (chain["efl_pt"] > np.float32(0.5)) & (np.abs(chain["efl_eta"]) < np.float32(2.5))
+    assert int(gd["offsets"][-1]) == int(keep.sum())
+    for k in ("pt", "eta", "phi", "E", "cls", "src"):
+        assert gd[k].tobytes() == chain["efl_" + k][keep].tobytes(), k
+    efl_ev = np.repeat(np.arange(ne), np.diff(chain["efl_offsets"]))
+    assert np.array_equal(np.diff(gd["offsets"]), np.bincount(efl_ev[keep], minlength=ne))
+    src = chain["trk_src"]
+    pt = np.hypot(ev.px[src].astype(np.float64), ev.py[src].astype(np.float64))
+    assert np.allclose(gi["d0_err"], np.sqrt(res[0][0] ** 2 + (res[0][1] / pt) ** 2), rtol=1e-5, atol=0)
+    assert np.allclose(gi["z0_err"], np.sqrt(res[1][0] ** 2 + (res[1][1] / pt) ** 2), rtol=1e-5, atol=0)
+    pull = (gi["z0"].astype(np.float64) - ev.vz[src]) / gi["z0_err"]  # vertices on the axis: z0_true = vz
+    assert abs(pull.mean()) < 5 / np.sqrt(n_trk) and abs(pull.std() - 1) < 5 / np.sqrt(2 * n_trk)
+    ht = np.bincount(efl_ev, weights=chain["efl_pt"].astype(np.float64), minlength=ne)
+    assert np.all(np.abs(gf["ht"] - ht) <= 1e-5 * ht + 1e-6)
+
+    # ---- sampled windows against the oracle
+    w = 3
+    for e0 in (0, ne // 2, ne - w):
+        e1 = e0 + w
+        sub = wl.slice_events(ev, e0, e1)
+        p0 = int(ev.offsets[e0])
+        t0, t1 = int(chain["trk_offsets"][e0]), int(chain["trk_offsets"][e1])
+        ri = pdo.track_impact(pdo.Card(name), sub, chain["trk_offsets"][e0:e1 + 1] - t0, chain["trk_src"][t0:t1] - p0, *res,
+                              seed=seed, event_base=e0)
+        for k in ("d0", "z0"):
+            g = gi[k][t0:t1]
+            assert np.all(np.abs(g - ri[k]) <= np.maximum(1e-5 * np.abs(ri[k]), 1e-6)), (e0, k)
+        f0, f1 = int(chain["efl_offsets"][e0]), int(chain["efl_offsets"][e1])
+        sl = {k: chain["efl_" + k][f0:f1] for k in ("cls", "pt", "eta", "phi")}
+        rf = pdo.event_features(chain["efl_offsets"][e0:e1 + 1] - f0, sl["cls"], sl["pt"], sl["eta"], sl["phi"])
+        assert np.all(np.abs(gf["ht"][e0:e1] - rf["ht"]) <= 1e-5 * rf["ht"] + 1e-6)
+        for k in ("met_x", "met_y", "met"):
+            assert np.all(np.abs(gf[k][e0:e1] - rf[k]) <= 1e-6 * rf["ht"] + 1e-6), (e0, k)
+        amb = rf["iso_amb"]
+        for k in ("iso_charged", "iso_neutral", "iso_photon"):
+            assert np.all(np.abs(gf[k][f0:f1] - rf[k]) <= np.maximum(1e-5 * np.abs(rf[k]), 1e-6) + amb * (1 + 1e-5)), (e0, k)
+    print("cfg2 full size: %d tracks with impact parameters, %d of %d eflow objects kept by the filter" % (n_trk, int(keep.sum()), n_efl))
