@@ -1186,3 +1186,21 @@ int pdo_track_impact(const pdo_card *c, const pdo_events *ev, const int64_t *trk
   }
   return PDO_OK;
 }
+
+/* ---- truth-level event features (Table 2 "H_T, E_T^miss values for Truth and PFlow collections";
+ * P:L398 "Truth HT") -- readings T1, T2 of DESIGN.md section 15 ---- */
+int pdo_truth_features(const pdo_events *ev, int skip_neutrinos, double *ht, double *met_x, double *met_y, double *met) {
+  int64_t e, i;
+  if (!ev || !ht || !met_x || !met_y || !met) return PDO_EINVAL;
+  for (e = 0; e < ev->n_events; ++e) {
+    double h = 0.0, sx = 0.0, sy = 0.0;
+    for (i = ev->offsets[e]; i < ev->offsets[e + 1]; ++i) {
+      const int32_t a = ev->pid[i] < 0 ? -ev->pid[i] : ev->pid[i];
+      if (skip_neutrinos && (a == 12 || a == 14 || a == 16)) continue; /* T2: invisible particles */
+      h += hypot((double)ev->px[i], (double)ev->py[i]);
+      sx += (double)ev->px[i], sy += (double)ev->py[i];
+    }
+    ht[e] = h, met_x[e] = -sx, met_y[e] = -sy, met[e] = hypot(sx, sy);
+  }
+  return PDO_OK;
+}

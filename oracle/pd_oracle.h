@@ -241,6 +241,15 @@ int pdo_track_impact(const pdo_card *c, const pdo_events *ev, const int64_t *trk
                      double d0_a, double d0_b, double z0_a, double z0_b, uint64_t seed, int64_t event_base,
                      double *d0_true, double *z0_true, double *d0, double *z0, double *d0_err, double *z0_err);
 
+/* ---- truth-level event features (Table 2: "Event-level quantities: Event number, H_T, E_T^miss values for
+ * Truth and PFlow collections"; P:L398 event.truth_ht) ----
+ * The same two quantities as pdo_event_features, taken over the truth collection (readings T1, T2 of DESIGN.md
+ * section 15):  T1  H_T = sum of pT = sqrt(px^2 + py^2) over the event's particles; E_T^miss vector = -(sum px, sum py),
+ * E_T^miss its length (the truth collection carries Cartesian momenta, so no angle is involved).
+ * T2  skip_neutrinos != 0 leaves out |pid| in {12, 14, 16} (the usual generator-level missing energy: the recoil of
+ * the visible particles); 0 sums the collection as it is.  Sums in fp64 in particle order. */
+int pdo_truth_features(const pdo_events *ev, int skip_neutrinos, double *ht, double *met_x, double *met_y, double *met);
+
 const char *pdo_strerror(int code);
 
 /* ---- building blocks exposed so that tests can pin them one by one ---- */

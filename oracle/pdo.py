@@ -111,6 +111,7 @@ def lib():
                                        C.c_uint64, C.c_int64, C.c_int64] + [_p] * 12
         L.pdo_filter_eflow.argtypes = [C.c_int64] + [_p] * 7 + [C.POINTER(_Condition), C.c_int32, C.c_int32] + [_p] * 8
         L.pdo_event_features.argtypes = [C.POINTER(_Objects), C.c_double, C.c_double] + [_p] * 9
+        L.pdo_truth_features.argtypes = [C.POINTER(_Events), C.c_int] + [_p] * 4
         L.pdo_impact_true.argtypes = [_p, C.c_int] + [C.c_double] * 6 + [C.POINTER(C.c_double)] * 2
         L.pdo_track_impact.argtypes = [_p, C.POINTER(_Events), _p, _p] + [C.c_double] * 4 + [C.c_uint64, C.c_int64] + [_p] * 6
         _lib = L
@@ -393,3 +394,14 @@ def track_impact(card: Card, ev, trk_offsets, trk_src, d0_res=(0.0, 0.0), z0_res
     if rc != 0:
         raise OracleError(rc)
     return {k: v[:n] for k, v in out.items()}
+
+
+def truth_features(ev, skip_neutrinos: bool = True) -> dict:
+    """pdo_truth_features (readings T1, T2): ht, met_x, met_y, met per event over the truth collection."""
+    cev, keep = _events_struct(ev)
+    ne = cev.n_events
+    out = {k: np.zeros(max(ne, 1), dtype=np.float64) for k in ("ht", "met_x", "met_y", "met")}
+    rc = lib().pdo_truth_features(C.byref(cev), int(bool(skip_neutrinos)), *[_ptr(out[k]) for k in ("ht", "met_x", "met_y", "met")])
+    if rc != 0:
+        raise OracleError(rc)
+    return {k: v[:ne] for k, v in out.items()}
