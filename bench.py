@@ -282,6 +282,18 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     imp_ms = f0.elapsed_time(f1) / f_steps
     del imp
+    # ---- H_T and E_T^miss of the truth collection (the step's input)
+    tfeat = pd.DeviceFeatures(ne, 1)
+    tws = pd.truth_features(dev, tfeat)
+    pd.truth_features(dev, tfeat, workspace=tws)
+    barrier()
+    f0.record(stream)
+    for _ in range(f_steps):
+        pd.truth_features(dev, tfeat, workspace=tws)
+    f1.record(stream)
+    barrier()
+    truth_ms = f0.elapsed_time(f1) / f_steps
+    del tfeat, tws
 
     # ---- pile-up merging, the step right before the hot path: 5,000 cfg0-like hard-scatter
     # events, a pool of 20,000 cfg3-like minimum-bias events, mean pile-up 50 (Table C.9 defaults otherwise)
@@ -351,6 +363,10 @@ def run_ours(args, rank, world, local_rank):
                                   "kernels": "pd_pileup_count/scan/fill_kernel", "algorithmic_bytes": 67 * pu_total + 20 * hs_ev.n_events,
                                   "hbm_frac": (67 * pu_total + 20 * hs_ev.n_events) / (pu_ms * 1e-3) / 1e9 / peak,
                                   "note": "5,000 cfg0-like events + Poisson(50) of 20,000 cfg3-like min-bias events; 3 launches; rank 0, not in value"},
+                 "truth_features": {"ms": truth_ms, "particles_per_s": n / (truth_ms * 1e-3), "kernels": "pd_truth_sum_kernel + pd_truth_finish_kernel",
+                                    "algorithmic_bytes": 12 * n + 8 * (ne + 1) + 16 * ne,
+                                    "hbm_frac": (12 * n + 8 * (ne + 1) + 16 * ne) / (truth_ms * 1e-3) / 1e9 / peak,
+                                    "note": "H_T, MET of the truth collection (neutrinos left out); 2 launches + a memset; rank 0, not in value"},
                  "track_impact": {"ms": imp_ms, "tracks_per_s": totals[0] / (imp_ms * 1e-3), "kernel": "pd_impact_kernel",
                                   "algorithmic_bytes": 45 * totals[0] + 16 * (ne + 1),
                                   "hbm_frac": (45 * totals[0] + 16 * (ne + 1)) / (imp_ms * 1e-3) / 1e9 / peak,

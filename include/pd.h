@@ -274,6 +274,19 @@ int pd_track_impact(const pd_card *card, const pd_events *events, const pd_track
                     const pd_impact_config *cfg, uint64_t seed, int64_t event_base, pd_impact *out,
                     void *cuda_stream);
 
+/* ---- Truth-level event features (Table 2 "Event-level quantities: ... H_T, E_T^miss values for Truth
+ * and PFlow collections"; L398 event.truth_ht; readings T1, T2 of DESIGN.md section 15) ----
+ * Per event of the truth collection:  ht = sum_i sqrt(px_i^2 + py_i^2);  (met_x, met_y) = -(sum_i px_i, sum_i py_i);
+ * met = its length.  skip_neutrinos != 0 leaves out |pid| in {12, 14, 16} (the generator-level missing energy: the
+ * recoil of the visible particles); 0 sums the collection as it is.  Exact fixed-point sums (units of 2^-32 GeV):
+ * independent of order, bitwise reproducible.  Writes out->ht, met_x, met_y, met ([n_events], DEVICE pointers); the
+ * isolation members of pd_features are not touched and may be NULL.  Only events->offsets, pid, px, py are read.
+ * workspace: >= pd_truth_workspace_bytes(n_events) bytes of DEVICE memory, 8-byte aligned, scratch.
+ * Asynchronous on cuda_stream, two kernel launches, allocates nothing.  Errors: PD_EINVAL, PD_EWORKSPACE, PD_ECUDA. */
+int64_t pd_truth_workspace_bytes(int64_t n_events);
+int pd_truth_features(const pd_events *events, int32_t skip_neutrinos, pd_features *out, void *workspace,
+                      int64_t workspace_bytes, void *cuda_stream);
+
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 

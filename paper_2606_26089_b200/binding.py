@@ -18,7 +18,7 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_track_impact", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_track_impact", "pd_truth_workspace_bytes", "pd_truth_features", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
@@ -127,6 +127,9 @@ def lib():
         L.pd_filter_eflow.argtypes = [C.POINTER(EFlow), C.c_int64, C.POINTER(Condition), C.c_int32, C.c_int32, C.POINTER(EFlow), _p,
                                       C.c_int64, _p]
         L.pd_event_features.argtypes = [C.POINTER(EFlow), C.c_int64, C.c_float, C.c_float, C.POINTER(Features), _p]
+        L.pd_truth_workspace_bytes.argtypes = [C.c_int64]
+        L.pd_truth_workspace_bytes.restype = C.c_int64
+        L.pd_truth_features.argtypes = [C.POINTER(Events), C.c_int32, C.POINTER(Features), _p, C.c_int64, _p]
         L.pd_track_impact.argtypes = [_p, C.POINTER(Events), C.POINTER(Tracks), C.POINTER(ImpactConfig), C.c_uint64, C.c_int64,
                                       C.POINTER(Impact), _p]
         L.pd_simulate_host.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks),
@@ -356,6 +359,21 @@ def event_features(out, feat: DeviceFeatures, dr_max: float = 0.4, fsr_dr: float
     st = torch.cuda.current_stream() if stream is None else stream
     _check(lib().pd_event_features(C.byref(out.c_efl), int(out.n_events), float(dr_max), float(fsr_dr), C.byref(feat.c),
                                    C.c_void_p(st.cuda_stream)))
+
+
+def truth_features(dev_events: "DeviceEvents", feat: "DeviceFeatures", skip_neutrinos: bool = True, stream=None, workspace=None):
+    """pd_truth_features: H_T and E_T^miss of the truth collection into feat's per-event arrays.  Asynchronous.
+    Returns the workspace tensor (pass it back in to reuse it)."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    need = int(lib().pd_truth_workspace_bytes(int(dev_events.n_events)))
+    if workspace is None or workspace.numel() * workspace.element_size() < need:
+        workspace = torch.empty((need + 7) // 8, dtype=torch.int64, device="cuda")
+    _check(lib().pd_truth_features(C.byref(dev_events.c), int(bool(skip_neutrinos)), C.byref(feat.c), _tptr(workspace),
+                                   workspace.numel() * workspace.element_size(), C.c_void_p(st.cuda_stream)))
+    return workspace
 
 
 class DeviceTrackRefs:

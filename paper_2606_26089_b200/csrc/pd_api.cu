@@ -244,6 +244,32 @@ int pd_event_features(const pd_eflow *efl, int64_t n_events, float dr_max, float
   return PD_OK;
 }
 
+int64_t pd_truth_workspace_bytes(int64_t n_events) {
+  if (n_events < 0) return PD_EINVAL;
+  return 24 * (n_events > 0 ? n_events : 1);
+}
+
+int pd_truth_features(const pd_events *ev, int32_t skip_neutrinos, pd_features *out, void *workspace, int64_t workspace_bytes,
+                      void *cuda_stream) {
+  t_launches = 0;
+  if (!ev || !out || ev->n_events < 0 || ev->n_particles < 0) return PD_EINVAL;
+  if (ev->n_events == 0) return PD_OK;
+  if (!ev->offsets || !out->ht || !out->met_x || !out->met_y || !out->met) return PD_EINVAL;
+  if (ev->n_particles > 0 && (!ev->pid || !ev->px || !ev->py)) return PD_EINVAL;
+  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 7)) return PD_EINVAL;
+  if (workspace_bytes < pd_truth_workspace_bytes(ev->n_events)) return PD_EWORKSPACE;
+  PdTruthParams p;
+  p.n_events = ev->n_events, p.n_particles = ev->n_particles;
+  p.ev_off = (const long long *)ev->offsets, p.pid = ev->pid, p.px = ev->px, p.py = ev->py;
+  p.skip_neutrinos = skip_neutrinos != 0;
+  p.acc = (unsigned long long *)workspace;
+  p.ht = out->ht, p.met_x = out->met_x, p.met_y = out->met_y, p.met = out->met;
+  const int rc = pd_launch_truth(p, cuda_stream);
+  if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "truth features launch");
+  t_launches = ev->n_particles > 0 ? 2 : 1;
+  return PD_OK;
+}
+
 int pd_track_impact(const pd_card *card, const pd_events *ev, const pd_tracks *trk, const pd_impact_config *cfg,
                     uint64_t seed, int64_t event_base, pd_impact *out, void *cuda_stream) {
   t_launches = 0;

@@ -216,3 +216,15 @@ struct PdImpactParams {
   float *d0, *z0, *d0_err, *z0_err;
 };
 int pd_launch_impact(const PdImpactParams &prm, void *stream);
+
+// pd_truth.cu: truth-level event features (pd_truth_features)
+struct PdTruthParams {
+  long long n_events, n_particles;
+  const long long *ev_off;
+  const int *pid;
+  const float *px, *py;
+  int skip_neutrinos;
+  unsigned long long *acc;  // workspace: [n_events][3] fixed-point sums (H_T, sum px, sum py)
+  float *ht, *met_x, *met_y, *met;
+};
+int pd_launch_truth(const PdTruthParams &prm, void *stream);

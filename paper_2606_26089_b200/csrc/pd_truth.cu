@@ -1,0 +1,214 @@
+// pd_truth.cu -- truth-level event features: H_T and E_T^miss over the truth collection (Table 2
+// "H_T, E_T^miss values for Truth and PFlow collections", L398 "Truth HT"; readings T1, T2
+// of DESIGN.md section 15).  Product code; shares nothing with oracle/.
+//
+// A segmented reduction over the CSR particle arrays, bound by reading px, py, pid (12 B per particle).
+// Kernel 1: CTAs walk over tiles of 2,048 consecutive particles: coalesced loads, (pT, px, py) of the visible
+// particles staged in shared memory; the events the tile touches are found by a warp-wide search of the offsets and
+// their offsets staged relative to the tile (a CTA walks over consecutive tiles, so a tile starts in the event the
+// previous one ended in and one window of 257 offsets, loaded with the particles, normally covers it); warps then
+// take (event, piece) work items, sum in 64-bit fixed point
+// (units of 2^-32 GeV: associative, so the result does not depend on tiles, pieces or the order of the atomics) and
+// add the three sums to the event's accumulators in the workspace.  Kernel 2: accumulators -> fp32 outputs.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "pd_internal.h"
+
+namespace pdt {
+
+constexpr int THREADS = 256, W = THREADS / 32, ITEMS = 8, TILE = THREADS * ITEMS;  // ITEMS: a multiple of 4
+constexpr double kInvFix = 2.3283064365386963e-10;  // 2^-32
+
+__device__ __forceinline__ long long warp_sum_ll(long long v) {
+  const unsigned long long u = (unsigned long long)v;  // pieces of 24 + 24 + 16 bits: 32 of them cannot overflow 32 bits
+  const unsigned a = __reduce_add_sync(0xffffffffu, (unsigned)(u & 0xffffffu));
+  const unsigned b = __reduce_add_sync(0xffffffffu, (unsigned)((u >> 24) & 0xffffffu));
+  const unsigned c = __reduce_add_sync(0xffffffffu, (unsigned)(u >> 48));
+  return (long long)((unsigned long long)a + ((unsigned long long)b << 24) + ((unsigned long long)c << 48));
+}
+__device__ __forceinline__ long long to_fix(float x) { return __float2ll_rn(x * 4294967296.f); }
+__device__ __forceinline__ float sqrt_approx(float x) {  // 2 ulp; pT only enters sums compared at 1e-5
+  float r;
+  asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// largest e in [lo, hi) with off[e] <= t, by a whole warp: 33-ary narrowing, then halving
+__device__ __forceinline__ long long find_event_warp(const long long *off, long long lo, long long hi, long long t, int lane) {
+  while (hi - lo > 32) {
+    const long long probe = lo + ((hi - lo) * (lane + 1)) / 33;  // lo < probe < hi, non-decreasing in lane
+    const unsigned m = __ballot_sync(0xffffffffu, __ldg(off + probe) <= t);  // a prefix of the lanes
+    const int k = __popc(m);
+    const long long new_lo = k > 0 ? __shfl_sync(0xffffffffu, probe, k - 1) : lo;
+    const long long new_hi = k < 32 ? __shfl_sync(0xffffffffu, probe, k & 31) : hi;
+    lo = new_lo, hi = new_hi;
+  }
+  while (hi - lo > 1) {
+    const long long mid = (lo + hi) >> 1;
+    if (__ldg(off + mid) <= t) lo = mid;
+    else hi = mid;
+  }
+  return lo;
+}
+
+__global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_constant__ PdTruthParams prm) {
+  __shared__ __align__(16) float s_pt[TILE], s_px[TILE], s_py[TILE];
+  __shared__ int s_off[THREADS + 1];  // offsets of the events e_cur .. e_cur + THREADS, relative to the tile, clamped
+  __shared__ long long s_first, s_last;
+  __shared__ int s_found;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const long long n = prm.n_particles, ne = prm.n_events;
+  const long long n_tiles = (n + TILE - 1) / TILE;
+  // a CTA takes a contiguous range of tiles, so that the first event of a tile is the last one of the tile before
+  const long long per = (n_tiles + gridDim.x - 1) / gridDim.x;
+  const long long tile_b = blockIdx.x * per, tile_e = min(tile_b + per, n_tiles);
+  if (tile_b >= tile_e) return;
+  if (wid == 0) {
+    const long long e = find_event_warp(prm.ev_off, 0, ne, tile_b * TILE, lane);
+    if (lane == 0) s_first = e;
+  }
+  __syncthreads();
+  long long e_cur = s_first;
+  // registers of the tile in flight: its particles (a thread takes groups of four adjacent ones: 16-byte loads when
+  // the caller's arrays allow it) and a window of THREADS + 1 offsets starting at its first event
+  constexpr int GROUPS = ITEMS / 4;
+  float4 r_px[GROUPS], r_py[GROUPS];
+  int4 r_pid[GROUPS];
+  long long w0, w1;
+  const bool vec_ok = ((reinterpret_cast<uintptr_t>(prm.px) | reinterpret_cast<uintptr_t>(prm.py) | reinterpret_cast<uintptr_t>(prm.pid)) & 15) == 0;
+  auto load_tile = [&](long long tile, long long e_first) {
+    const long long t0 = tile * TILE;
+    const int len = (int)(min(t0 + (long long)TILE, n) - t0);
+#pragma unroll
+    for (int g = 0; g < GROUPS; ++g) {
+      const int j = (g * THREADS + tid) * 4;
+      if (vec_ok && j + 3 < len) {
+        r_px[g] = __ldg(reinterpret_cast<const float4 *>(prm.px + t0 + j));
+        r_py[g] = __ldg(reinterpret_cast<const float4 *>(prm.py + t0 + j));
+        r_pid[g] = __ldg(reinterpret_cast<const int4 *>(prm.pid + t0 + j));
+      } else {
+        float x[4], y[4];
+        int q[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const bool in = j + c < len;
+          x[c] = in ? __ldg(prm.px + t0 + j + c) : 0.f, y[c] = in ? __ldg(prm.py + t0 + j + c) : 0.f;
+          q[c] = in ? __ldg(prm.pid + t0 + j + c) : 0;
+        }
+        r_px[g] = make_float4(x[0], x[1], x[2], x[3]), r_py[g] = make_float4(y[0], y[1], y[2], y[3]);
+        r_pid[g] = make_int4(q[0], q[1], q[2], q[3]);
+      }
+    }
+    const long long ke = min(e_first + tid, ne);
+    w0 = __ldg(prm.ev_off + ke), w1 = __ldg(prm.ev_off + min(ke + 1, ne));
+  };
+  auto visible = [&](int pid) {
+    const int a = abs(pid);
+    return !(prm.skip_neutrinos && (a == 12 || a == 14 || a == 16));
+  };
+  load_tile(tile_b, e_cur);
+  for (long long tile = tile_b; tile < tile_e; ++tile) {
+    const long long t0 = tile * TILE, t1 = min(t0 + (long long)TILE, n) - 1;
+    const int len = (int)(t1 - t0 + 1);
+    __syncthreads();  // the previous tile's sums are done with the staging arrays
+    if (tid == 0) s_found = 0;
+#pragma unroll
+    for (int g = 0; g < GROUPS; ++g) {
+      const int j = (g * THREADS + tid) * 4;  // positions >= len hold zeros and are never read
+      float4 x = r_px[g], y = r_py[g], t;
+      if (!visible(r_pid[g].x)) x.x = 0.f, y.x = 0.f;
+      if (!visible(r_pid[g].y)) x.y = 0.f, y.y = 0.f;
+      if (!visible(r_pid[g].z)) x.z = 0.f, y.z = 0.f;
+      if (!visible(r_pid[g].w)) x.w = 0.f, y.w = 0.f;
+      t.x = sqrt_approx(fmaf(x.x, x.x, y.x * y.x)), t.y = sqrt_approx(fmaf(x.y, x.y, y.y * y.y));
+      t.z = sqrt_approx(fmaf(x.z, x.z, y.z * y.z)), t.w = sqrt_approx(fmaf(x.w, x.w, y.w * y.w));
+      *reinterpret_cast<float4 *>(s_px + j) = x, *reinterpret_cast<float4 *>(s_py + j) = y, *reinterpret_cast<float4 *>(s_pt + j) = t;
+    }
+    s_off[tid] = (int)max(min(w0 - t0, (long long)len), 0LL);
+    if (tid == THREADS - 1) s_off[THREADS] = (int)max(min(w1 - t0, (long long)len), 0LL);
+    __syncthreads();
+    // the event that holds the tile's last particle: in the window unless the tile touches more than THREADS events
+    if (e_cur + tid < ne && w0 <= t1 && w1 > t1) s_last = e_cur + tid, s_found = 1;
+    __syncthreads();
+    if (!s_found) {  // CTA-uniform; rare (events of fewer than 8 particles on average, or runs of empty events)
+      if (wid == 0) {
+        const long long e = find_event_warp(prm.ev_off, e_cur, ne, t1, lane);
+        if (lane == 0) s_last = e;
+      }
+      __syncthreads();
+    }
+    const long long e_last = s_last;
+    const long long n_ev = e_last - e_cur + 1;  // events e_cur .. e_last
+    if (tile + 1 < tile_e) load_tile(tile + 1, e_last);  // in flight while this tile is summed
+    auto seg_of = [&](long long e, int &a, int &b) {
+      if (e < THREADS) {
+        a = s_off[e], b = s_off[e + 1];
+      } else {
+        a = (int)max(min(__ldg(prm.ev_off + e_cur + e) - t0, (long long)len), 0LL);
+        b = (int)max(min(__ldg(prm.ev_off + e_cur + e + 1) - t0, (long long)len), 0LL);
+      }
+    };
+    if (n_ev >= 32) {
+      // many small events: a thread per event, sequential sums (no cross-lane work)
+      for (long long e = tid; e < n_ev; e += THREADS) {
+        int a, b;
+        seg_of(e, a, b);
+        long long h = 0, x = 0, y = 0;
+        for (int j = a; j < b; ++j) h += to_fix(s_pt[j]), x += to_fix(s_px[j]), y += to_fix(s_py[j]);
+        if (h != 0) atomicAdd(prm.acc + 3 * (e_cur + e), (unsigned long long)h);
+        if (x != 0) atomicAdd(prm.acc + 3 * (e_cur + e) + 1, (unsigned long long)x);
+        if (y != 0) atomicAdd(prm.acc + 3 * (e_cur + e) + 2, (unsigned long long)y);
+      }
+    } else {
+      // (event, piece) work items per warp; few events in the tile -> every event's segment is cut into W pieces
+      const int P = n_ev < W ? W : 1;
+      for (int item = wid; item < (int)n_ev * P; item += W) {
+        const int e = item / P, piece = item - e * P;
+        int a, b;
+        seg_of(e, a, b);
+        const int seg = b - a;
+        const int pa = a + (seg * piece) / P, pb = a + (seg * (piece + 1)) / P;
+        if (pb <= pa) continue;  // warp-uniform
+        long long h = 0, x = 0, y = 0;
+        for (int j = pa + lane; j < pb; j += 32) h += to_fix(s_pt[j]), x += to_fix(s_px[j]), y += to_fix(s_py[j]);
+        h = warp_sum_ll(h), x = warp_sum_ll(x), y = warp_sum_ll(y);
+        if (lane < 3) {
+          const long long v = lane == 0 ? h : (lane == 1 ? x : y);
+          if (v != 0) atomicAdd(prm.acc + 3 * (e_cur + e) + lane, (unsigned long long)v);
+        }
+      }
+    }
+    e_cur = e_last;  // it may continue in the next tile
+  }
+}
+
+__global__ void pd_truth_finish_kernel(const __grid_constant__ PdTruthParams prm) {
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < prm.n_events; e += (long long)gridDim.x * blockDim.x) {
+    const double h = (double)(long long)prm.acc[3 * e] * kInvFix;
+    const double mx = -(double)(long long)prm.acc[3 * e + 1] * kInvFix, my = -(double)(long long)prm.acc[3 * e + 2] * kInvFix;
+    prm.ht[e] = (float)h, prm.met_x[e] = (float)mx, prm.met_y[e] = (float)my;
+    prm.met[e] = (float)sqrt(mx * mx + my * my);
+  }
+}
+
+}  // namespace pdt
+
+int pd_launch_truth(const PdTruthParams &prm, void *stream) {
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PD_ECUDA;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PD_ECUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemsetAsync(prm.acc, 0, 24 * (size_t)prm.n_events, st) != cudaSuccess) return PD_ECUDA;
+  if (prm.n_particles > 0) {
+    long long blocks = (prm.n_particles + pdt::TILE - 1) / pdt::TILE;
+    if (blocks > 4LL * sms) blocks = 4LL * sms;
+    pdt::pd_truth_sum_kernel<<<(unsigned)blocks, pdt::THREADS, 0, st>>>(prm);
+    if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
+  }
+  long long blocks = (prm.n_events + 255) / 256;
+  if (blocks > 4LL * sms) blocks = 4LL * sms;
+  pdt::pd_truth_finish_kernel<<<(unsigned)blocks, 256, 0, st>>>(prm);
+  return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
+}
