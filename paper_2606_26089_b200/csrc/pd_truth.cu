@@ -163,16 +163,31 @@ __global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_c
       }
     } else {
       // (event, piece) work items per warp; few events in the tile -> every event's segment is cut into W pieces
-      const int P = n_ev < W ? W : 1;
-      for (int item = wid; item < (int)n_ev * P; item += W) {
-        const int e = item / P, piece = item - e * P;
+      const int sh = n_ev < W ? 3 : 0, P = 1 << sh;  // W = 8 pieces
+      static_assert(W == 8, "pieces per event");
+      for (int item = wid; item < ((int)n_ev << sh); item += W) {
+        const int e = item >> sh, piece = item & (P - 1);
         int a, b;
         seg_of(e, a, b);
         const int seg = b - a;
-        const int pa = a + (seg * piece) / P, pb = a + (seg * (piece + 1)) / P;
+        const int pa = a + ((seg * piece) >> sh), pb = a + ((seg * (piece + 1)) >> sh);
         if (pb <= pa) continue;  // warp-uniform
         long long h = 0, x = 0, y = 0;
-        for (int j = pa + lane; j < pb; j += 32) h += to_fix(s_pt[j]), x += to_fix(s_px[j]), y += to_fix(s_py[j]);
+        auto add = [&](int j) { h += to_fix(s_pt[j]), x += to_fix(s_px[j]), y += to_fix(s_py[j]); };
+        const int ja = (pa + 3) & ~3, jb = pb & ~3;  // the 16-byte aligned middle [ja, jb)
+        if (ja < jb) {
+          if (lane < ja - pa) add(pa + lane);
+          if (lane < pb - jb) add(jb + lane);
+          for (int j = ja + 4 * lane; j < jb; j += 128) {
+            const float4 vt = *reinterpret_cast<const float4 *>(s_pt + j), vx = *reinterpret_cast<const float4 *>(s_px + j),
+                         vy = *reinterpret_cast<const float4 *>(s_py + j);
+            h += to_fix(vt.x) + to_fix(vt.y) + to_fix(vt.z) + to_fix(vt.w);
+            x += to_fix(vx.x) + to_fix(vx.y) + to_fix(vx.z) + to_fix(vx.w);
+            y += to_fix(vy.x) + to_fix(vy.y) + to_fix(vy.z) + to_fix(vy.w);
+          }
+        } else {
+          for (int j = pa + lane; j < pb; j += 32) add(j);
+        }
         h = warp_sum_ll(h), x = warp_sum_ll(x), y = warp_sum_ll(y);
         if (lane < 3) {
           const long long v = lane == 0 ? h : (lane == 1 ? x : y);
