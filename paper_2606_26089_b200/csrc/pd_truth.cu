@@ -2,14 +2,16 @@
 // "H_T, E_T^miss values for Truth and PFlow collections", L398 "Truth HT"; readings T1, T2
 // of DESIGN.md section 15).  Product code; shares nothing with oracle/.
 //
-// A segmented reduction over the CSR particle arrays, bound by reading px, py, pid (12 B per particle).
-// Kernel 1: CTAs walk over tiles of 2,048 consecutive particles: coalesced loads, (pT, px, py) of the visible
-// particles staged in shared memory; the events the tile touches are found by a warp-wide search of the offsets and
-// their offsets staged relative to the tile (a CTA walks over consecutive tiles, so a tile starts in the event the
-// previous one ended in and one window of 257 offsets, loaded with the particles, normally covers it); warps then
-// take (event, piece) work items, sum in 64-bit fixed point
-// (units of 2^-32 GeV: associative, so the result does not depend on tiles, pieces or the order of the atomics) and
-// add the three sums to the event's accumulators in the workspace.  Kernel 2: accumulators -> fp32 outputs.
+// A segmented reduction over the CSR particle arrays, reading px, py, pid (12 B per particle).
+// Kernel 1: a CTA walks over CONSECUTIVE tiles of 2,048 particles.  16-byte loads (four adjacent particles per
+// thread), issued one tile ahead; (pT, px, py) of the visible particles staged in shared memory.  A tile starts in
+// the event the previous one ended in, so one window of 257 offsets, loaded together with the particles, normally
+// covers the events it touches (otherwise: a warp-wide 33-ary search for its last event, offsets beyond the window
+// from global memory).  Three ways to sum, chosen per tile: fewer than 8 events -> every event's segment is cut into
+// 8 pieces, one per warp; 8..31 events -> a warp per event; 32 or more -> a thread per event.  Sums are 64-bit fixed
+// point (units of 2^-32 GeV: associative, so the result does not depend on tiles, pieces, batching or the order of
+// the atomics) and are added to the event's three accumulators in the workspace with 64-bit atomics.
+// Kernel 2: accumulators -> fp32 outputs.
 #include <cuda_runtime.h>
 
 #include <cstdint>
