@@ -1,11 +1,13 @@
 // pd_impact.cu -- track impact parameters d0, z0 and their errors (Table 2;
 // SURVEY.md 8f NEXT-3; readings I1..I3 of DESIGN.md section 14).  Product code; shares nothing with oracle/.
 //
-// One thread per output track of a pd_simulate call.  The event of a track (needed for the Philox counter and for
-// the particle's index within its event) is found by bisection of the track offsets; a CTA first narrows the range
-// to the events its 1,024 consecutive tracks touch and stages those offsets in shared memory when they fit, so the
-// per-thread search runs on chip.  The truth particle is gathered through trk.src (ascending inside an event, so
-// the gathers of a warp fall into a few cache lines).
+// A thread takes four adjacent output tracks of a pd_simulate call (16-byte loads of trk.src, 16-byte stores of the
+// four outputs).  The event of a track (needed for the Philox counter and for the particle's index within its
+// event) comes from the track offsets: two warps find the events of the first and the last track of a 1,024-track
+// tile by a 33-ary search, the offsets in between are staged in shared memory relative to the tile, and a thread
+// bisects them once for its first track and walks forward for the other three.  The truth particle is gathered
+// through trk.src (ascending inside an event, so the gathers of a warp fall into a few cache lines); all loads of a
+// thread are issued before anything is computed.
 //
 // Geometry in fp32, arranged so that nothing cancels (frame: p^ along the transverse momentum, n^ to its left):
 //   w = v . p^, u = v . n^ (both from error-free products), helix centre c = (w, u + s rho), r_c = |c|,
