@@ -74,7 +74,8 @@ def test_ragged_tile_boundaries_and_features_of_survivors():
             feat = pd.DeviceFeatures(dst.n_events, max(n, 1))
             pd.event_features(dst, feat)
             g = feat.to_numpy(int(got["offsets"][-1]))
-            r = pdo.event_features(got["offsets"], got["cls"], got["pt"], got["eta"], got["phi"])
+            # the oracle's inputs are the ORACLE's survivors (bit-identical to the device's, checked by _same above)
+            r = pdo.event_features(ref["offsets"], ref["cls"], ref["pt"], ref["eta"], ref["phi"])
             assert np.all(np.abs(g["ht"] - r["ht"]) <= np.maximum(1e-5 * r["ht"], 1e-6))
             ok = r["iso_amb"] == 0
             assert np.all(np.abs(g["r_iso"] - r["r_iso"])[ok] <= np.maximum(1e-5 * r["r_iso"], 1e-6)[ok])
