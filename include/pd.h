@@ -302,7 +302,11 @@ int pd_set_tile_events(int g);
 
 /* Same computation with HOST pointers everywhere (inputs and outputs in host memory, pinned or
  * pageable).  Copies inputs to the device, runs pd_simulate, copies the three collections back and
- * synchronises.  Output capacities as for pd_simulate; totals are offsets[n_events]. */
+ * synchronises.  Output capacities as for pd_simulate; totals are offsets[n_events].  Large batches (>= 4M particles)
+ * go through in chunks of consecutive events with the copies of one chunk overlapping the kernel of the next (same
+ * results, bit for bit).  Optional layout hint: if the 4-byte arrays of a collection (events: pid, px..vz; tracks: src,
+ * pid, pt..phi_out; towers: tower, eta..ET; eflow: src, pt..E; in this order) are equally spaced rows of ONE pinned
+ * host allocation, a chunk of all of them moves with one strided copy instead of one copy per array. */
 int pd_simulate_host(const pd_card *card, const pd_events *events, uint64_t seed, int64_t event_base,
                      pd_tracks *tracks, pd_towers *towers, pd_eflow *eflow, void *cuda_stream);
 

@@ -492,9 +492,11 @@ def last_status(out: DeviceOutputs, stream=None) -> int:
 
 
 class HostBuffers:
-    """Pinned host buffers for pd_simulate_host (the end-to-end path)."""
+    """Pinned host buffers for pd_simulate_host (the end-to-end path).  packed=True (default) lays the 4-byte arrays of
+    each collection out as the rows of one block; packed=False allocates every array on its own (the C ABI takes
+    either: equal spacing is detected, not required)."""
 
-    def __init__(self, ev, pin=True):
+    def __init__(self, ev, pin=True, packed=True):
         torch = _torch()
         self.n_events = int(ev.offsets.shape[0] - 1)
         self.n_particles = int(ev.offsets[-1])
@@ -505,11 +507,31 @@ class HostBuffers:
             t = torch.from_numpy(np.ascontiguousarray(a))
             return t.pin_memory() if pin else t
 
-        self.ev = {name: host(np.ascontiguousarray(getattr(ev, name), dtype=dt)) for name, dt in EVENT_FIELDS}
+        def rows(fields, m):
+            """The 4-byte arrays of a collection as the rows of ONE pinned block (equal spacing lets pd_simulate_host move
+            a chunk of all of them with one strided copy); the others on their own."""
+            four = [k for k, dt in fields if np.dtype(dt).itemsize == 4 and packed]
+            block = torch.empty((len(four), m), dtype=torch.int32, pin_memory=pin)
+            out = {}
+            for k, dt in fields:
+                if k in four:
+                    out[k] = block[four.index(k)].view(getattr(torch, dt))
+                else:
+                    out[k] = torch.empty(m, dtype=getattr(torch, dt), pin_memory=pin)
+            return out, block
+
+        ev_fields = [(k, np.dtype(dt).name) for k, dt in EVENT_FIELDS if k != "offsets"]
+        self.ev, self._ev_block = rows(ev_fields, n)
+        for k, dt in ev_fields:
+            self.ev[k][: self.n_particles].copy_(torch.from_numpy(np.ascontiguousarray(getattr(ev, k), dtype=dt)))
+        self.ev = {"offsets": host(np.ascontiguousarray(ev.offsets, dtype=np.int64)), **self.ev}
         mk = lambda m, dt: torch.empty(m, dtype=getattr(torch, dt), pin_memory=pin)  # noqa: E731
-        self.trk = {"offsets": mk(self.n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TRACK_FIELDS}}
-        self.tow = {"offsets": mk(self.n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TOWER_FIELDS}}
-        self.efl = {"offsets": mk(self.n_events + 1, "int64"), **{k: mk(2 * n, dt) for k, dt in EFLOW_FIELDS}}
+        trk, self._trk_block = rows(TRACK_FIELDS, n)
+        tow, self._tow_block = rows(TOWER_FIELDS, n)
+        efl, self._efl_block = rows(EFLOW_FIELDS, 2 * n)
+        self.trk = {"offsets": mk(self.n_events + 1, "int64"), **trk}
+        self.tow = {"offsets": mk(self.n_events + 1, "int64"), **tow}
+        self.efl = {"offsets": mk(self.n_events + 1, "int64"), **efl}
         self.c_ev = Events(self.n_events, self.n_particles, *[_tptr(self.ev[k]) for k, _ in EVENT_FIELDS])
         self.c_trk = Tracks(n, _tptr(self.trk["offsets"]), *[_tptr(self.trk[k]) for k, _ in TRACK_FIELDS])
         self.c_tow = Towers(n, _tptr(self.tow["offsets"]), *[_tptr(self.tow[k]) for k, _ in TOWER_FIELDS])

@@ -597,13 +597,15 @@ static int simulate_host_pipelined(const pd_card *card, const pd_events *ev, uin
     return ptr;
   };
   int64_t *d_off = (int64_t *)take(8 * (size_t)(ne + 1 + K));
-  int32_t *d_pid = (int32_t *)take(4 * np);
+  // within each collection the 4-byte arrays are allocated back to back (equal pitch): when the caller's host arrays
+  // are equally spaced too, a chunk's copies collapse into one 2-D copy per group (copy_rows below)
   int8_t *d_q = (int8_t *)take(np);
+  int32_t *d_pid = (int32_t *)take(4 * np);
   float *d_in[7];
   for (auto &ptr : d_in) ptr = (float *)take(4 * np);
   int64_t *t_off = (int64_t *)take(8 * (size_t)(ne + 1 + K));
-  int32_t *t_src = (int32_t *)take(4 * np), *t_pid = (int32_t *)take(4 * np);
   int8_t *t_q = (int8_t *)take(np);
+  int32_t *t_src = (int32_t *)take(4 * np), *t_pid = (int32_t *)take(4 * np);
   float *t_f[6];
   for (auto &ptr : t_f) ptr = (float *)take(4 * np);
   int64_t *w_off = (int64_t *)take(8 * (size_t)(ne + 1 + K));
@@ -641,12 +643,41 @@ static int simulate_host_pipelined(const pd_card *card, const pd_events *ev, uin
   auto cp = [&](void *dst, const void *src, size_t bytes, cudaMemcpyKind kind, cudaStream_t s) {
     if (ce == cudaSuccess && bytes > 0 && dst && src) ce = cudaMemcpyAsync(dst, src, bytes, kind, s);
   };
+  // `rows` copies of `bytes` each; one strided copy when source and destination rows are equally spaced
+  bool strided_ok = true;
+  auto copy_rows = [&](int rows, void *const *dst, const void *const *src, size_t bytes, cudaMemcpyKind kind, cudaStream_t s) {
+    if (bytes == 0 || ce != cudaSuccess) return;
+    bool strided = rows > 1;
+    ptrdiff_t dp = 0, sp = 0;
+    if (strided) {
+      dp = (const char *)dst[1] - (const char *)dst[0], sp = (const char *)src[1] - (const char *)src[0];
+      strided = dp >= (ptrdiff_t)bytes && sp >= (ptrdiff_t)bytes && dp < (ptrdiff_t)0x7fffffff && sp < (ptrdiff_t)0x7fffffff;
+      for (int k = 2; k < rows && strided; ++k)
+        strided = (const char *)dst[k] - (const char *)dst[k - 1] == dp && (const char *)src[k] - (const char *)src[k - 1] == sp;
+    }
+    if (strided) {
+      // equally spaced rows that belong to SEPARATE host allocations are refused at enqueue time (the strided copy
+      // must lie inside one allocation): nothing was queued, fall back to a copy per row from then on
+      const cudaError_t e2 = strided_ok ? cudaMemcpy2DAsync(dst[0], (size_t)dp, src[0], (size_t)sp, bytes, (size_t)rows, kind, s)
+                                        : cudaErrorInvalidValue;
+      if (e2 == cudaSuccess) return;
+      if (e2 != cudaErrorInvalidValue) {
+        ce = e2;
+        return;
+      }
+      if (strided_ok) cudaGetLastError();
+      strided_ok = false;
+    }
+    for (int k = 0; k < rows; ++k) cp(dst[k], src[k], bytes, kind, s);
+  };
   auto upload = [&](int c) {
     const int64_t e0 = eb[c], e1 = eb[c + 1], p0 = ev->offsets[e0], nc = ev->offsets[e1] - p0;
     cp(d_off + e0 + c, ev->offsets + e0, 8 * (size_t)(e1 - e0 + 1), cudaMemcpyHostToDevice, s_in);  // absolute offsets
-    cp(d_pid + p0, ev->pid + p0, 4 * (size_t)nc, cudaMemcpyHostToDevice, s_in);
     cp(d_q + p0, ev->charge + p0, (size_t)nc, cudaMemcpyHostToDevice, s_in);
-    for (int f = 0; f < 7; ++f) cp(d_in[f] + p0, h_in[f] + p0, 4 * (size_t)nc, cudaMemcpyHostToDevice, s_in);
+    void *dd[8] = {d_pid + p0};
+    const void *hh[8] = {ev->pid + p0};
+    for (int f = 0; f < 7; ++f) dd[1 + f] = d_in[f] + p0, hh[1 + f] = h_in[f] + p0;
+    copy_rows(8, dd, hh, 4 * (size_t)nc, cudaMemcpyHostToDevice, s_in);
     if (ce == cudaSuccess) ce = cudaEventRecord(e_in[c], s_in);
   };
   std::vector<int64_t> tot(3 * (size_t)K, 0), basec(3 * (size_t)(K + 1), 0);
@@ -687,13 +718,26 @@ static int simulate_host_pipelined(const pd_card *card, const pd_events *ev, uin
     cp(trk->offsets + e0 + 1, t_off + e0 + c + 1, 8 * (size_t)nec, cudaMemcpyDeviceToHost, s_out);
     cp(tow->offsets + e0 + 1, w_off + e0 + c + 1, 8 * (size_t)nec, cudaMemcpyDeviceToHost, s_out);
     cp(efl->offsets + e0 + 1, f_off + e0 + c + 1, 8 * (size_t)nec, cudaMemcpyDeviceToHost, s_out);
-    cp(trk->src + bt, t_src + p0, 4 * nt, cudaMemcpyDeviceToHost, s_out), cp(trk->pid + bt, t_pid + p0, 4 * nt, cudaMemcpyDeviceToHost, s_out);
-    cp(trk->charge + bt, t_q + p0, nt, cudaMemcpyDeviceToHost, s_out);
-    for (int f = 0; f < 6; ++f) cp(h_tf[f] + bt, t_f[f] + p0, 4 * nt, cudaMemcpyDeviceToHost, s_out);
-    cp(tow->tower + bw, w_id + p0, 4 * nw, cudaMemcpyDeviceToHost, s_out);
-    for (int f = 0; f < 6; ++f) cp(h_wf[f] + bw, w_f[f] + p0, 4 * nw, cudaMemcpyDeviceToHost, s_out);
-    cp(efl->cls + bf, f_cls + 2 * p0, nf, cudaMemcpyDeviceToHost, s_out), cp(efl->src + bf, f_src + 2 * p0, 4 * nf, cudaMemcpyDeviceToHost, s_out);
-    for (int f = 0; f < 4; ++f) cp(h_ff[f] + bf, f_f[f] + 2 * p0, 4 * nf, cudaMemcpyDeviceToHost, s_out);
+    {
+      void *hh[8] = {trk->src + bt, trk->pid + bt};
+      const void *dd[8] = {t_src + p0, t_pid + p0};
+      for (int f = 0; f < 6; ++f) hh[2 + f] = h_tf[f] + bt, dd[2 + f] = t_f[f] + p0;
+      copy_rows(8, hh, dd, 4 * nt, cudaMemcpyDeviceToHost, s_out);
+      cp(trk->charge + bt, t_q + p0, nt, cudaMemcpyDeviceToHost, s_out);
+    }
+    {
+      void *hh[7] = {tow->tower + bw};
+      const void *dd[7] = {w_id + p0};
+      for (int f = 0; f < 6; ++f) hh[1 + f] = h_wf[f] + bw, dd[1 + f] = w_f[f] + p0;
+      copy_rows(7, hh, dd, 4 * nw, cudaMemcpyDeviceToHost, s_out);
+    }
+    {
+      void *hh[5] = {efl->src + bf};
+      const void *dd[5] = {f_src + 2 * p0};
+      for (int f = 0; f < 4; ++f) hh[1 + f] = h_ff[f] + bf, dd[1 + f] = f_f[f] + 2 * p0;
+      copy_rows(5, hh, dd, 4 * nf, cudaMemcpyDeviceToHost, s_out);
+      cp(efl->cls + bf, f_cls + 2 * p0, nf, cudaMemcpyDeviceToHost, s_out);
+    }
   }
   int words[16] = {0};
   if (rc == PD_OK) {

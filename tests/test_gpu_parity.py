@@ -116,11 +116,14 @@ def test_host_pointer_entry_matches_device_entry(monkeypatch):
             monkeypatch.delenv("PD_HOST_CHUNKS", raising=False)
         else:
             monkeypatch.setenv("PD_HOST_CHUNKS", chunks)
-        hb = pd.HostBuffers(ev)
-        pd.simulate_host(card, hb, 9)
-        got = hb.to_numpy()
-        for k, v in got.items():
-            assert v.tobytes() == ref[k].tobytes(), (chunks, k)
+        # host arrays as equally spaced rows of one block (a chunk then moves with one strided copy per group) and
+        # allocated one by one (a copy per array)
+        for packed in (True, False):
+            hb = pd.HostBuffers(ev, packed=packed)
+            pd.simulate_host(card, hb, 9)
+            got = hb.to_numpy()
+            for k, v in got.items():
+                assert v.tobytes() == ref[k].tobytes(), (chunks, packed, k)
 
 
 def test_skewed_event_sizes_need_one_event_per_tile():
