@@ -84,3 +84,30 @@ def test_header_is_plain_c(tmp_path):
     src.write_text('#include "pd.h"\nint main(void) { pd_events e; pd_condition c; pd_pileup_config p; (void)e; (void)c; (void)p; return 0; }\n')
     subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
                            "-fsyntax-only", str(src)])
+
+
+def test_host_buffers_packed_layout():
+    """HostBuffers(packed=True): the 4-byte arrays of every collection are equally spaced rows of one block, in the
+    order include/pd.h names for the strided copies of pd_simulate_host; packed=False: separate arrays.  (Host logic
+    only: no CUDA call is made.)"""
+    import importlib
+
+    import numpy as np
+
+    from paper_2606_26089_b200 import binding as B
+
+    wl = importlib.import_module("workloads.generate")
+    ev = wl.generate(0, 20)
+    hb = B.HostBuffers(ev, pin=False, packed=True)
+    n = ev.n_particles
+    groups = ((hb.ev, ("pid", "px", "py", "pz", "E", "vx", "vy", "vz"), n), (hb.trk, ("src", "pid", "pt", "eta", "phi", "E", "eta_out", "phi_out"), n),
+              (hb.tow, ("tower", "eta", "phi", "E", "Eem", "Ehad", "ET"), n), (hb.efl, ("src", "pt", "eta", "phi", "E"), 2 * n))
+    for d, names, m in groups:
+        ptrs = [d[k].data_ptr() for k in names]
+        assert all(b - a == 4 * m for a, b in zip(ptrs, ptrs[1:])), names
+        assert all(d[k].numel() == m for k in names)
+    for k in ("pid", "charge", "px", "vz"):
+        assert np.array_equal(hb.ev[k].numpy()[:n], getattr(ev, k))
+    assert np.array_equal(hb.ev["offsets"].numpy(), ev.offsets)
+    loose = B.HostBuffers(ev, pin=False, packed=False)
+    assert np.array_equal(loose.ev["px"].numpy()[:n], ev.px) and loose.trk["pt"].numel() == n
