@@ -19,7 +19,7 @@ thread_local int t_launches = 0;
 thread_local char t_cuda_msg[256] = "";
 std::mutex g_card_mutex;
 
-constexpr size_t kWsHeader = 16;  // tile counter (u32), status word (i32), padding
+constexpr size_t kWsHeader = 16;  // tile counter of kernel T (u32), status word (i32), tile counter of kernel P (u32), padding
 
 int cuda_fail(cudaError_t e, const char *what) {
   std::snprintf(t_cuda_msg, sizeof(t_cuda_msg), "CUDA error in %s: %s", what, cudaGetErrorString(e));
@@ -34,11 +34,13 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 }  // namespace
 
-// header + look-back words, rounded up so that the ring behind them is 256-byte aligned
+// header + look-back words of the two kernels, rounded up so that the keys behind them are 256-byte aligned
 static size_t ws_chain_bytes(const PdLaunchPlan &plan) {
-  const size_t b = kWsHeader + 2 * sizeof(unsigned long long) * (size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1);
+  const size_t b = kWsHeader + sizeof(unsigned long long) * ((size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1) + (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1));
   return (b + 255) & ~size_t(255);
 }
+// the 16-bit key kernel P leaves per particle for kernel T
+static size_t ws_key_bytes(const PdLaunchPlan &plan) { return sizeof(unsigned short) * (size_t)PD_PTILE * (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1); }
 
 extern "C" {
 
@@ -90,7 +92,7 @@ int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_part
   if (!card || n_events < 0 || n_particles < 0) return PD_EINVAL;
   PdLaunchPlan plan;
   pd_plan(card, n_events, n_particles, &plan);
-  return (int64_t)(ws_chain_bytes(plan) + sizeof(float) * 6 * (size_t)plan.max_ctas * (size_t)plan.capacity);
+  return (int64_t)(ws_chain_bytes(plan) + ws_key_bytes(plan));
 }
 
 int pd_last_launch_count(void) { return t_launches; }
@@ -350,11 +352,11 @@ int pd_card_to_device(const pd_card *c) {
   return PD_OK;
 }
 
-extern "C" {
-
-int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
-                pd_towers *tow, pd_eflow *efl, pd_debug *dbg, void *workspace, int64_t workspace_bytes,
-                void *cuda_stream) {
+// particle_base = offsets[0] (device memory; the host must know it): 0 for the public entry, the first particle of the
+// chunk for the pipelined host entry, whose chunks keep absolute offsets into the whole-batch arrays
+static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                         pd_towers *tow, pd_eflow *efl, pd_debug *dbg, void *workspace, int64_t workspace_bytes,
+                         void *cuda_stream, int64_t particle_base) {
   t_launches = 0;
   if (!card || !ev || !trk || !tow || !efl) return PD_EINVAL;
   if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 30)) return PD_EINVAL;
@@ -373,7 +375,7 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
 
   PdLaunchPlan plan;
   pd_plan(card, ev->n_events, n, &plan);
-  PD_CUDA(cudaMemsetAsync(workspace, 0, ws_chain_bytes(plan), st));  // counters + look-back words; the ring needs no init
+  PD_CUDA(cudaMemsetAsync(workspace, 0, ws_chain_bytes(plan), st));  // counters + look-back words; the keys need no init
   if (ev->n_events == 0) {
     PD_CUDA(cudaMemsetAsync(trk->offsets, 0, sizeof(int64_t), st));
     PD_CUDA(cudaMemsetAsync(tow->offsets, 0, sizeof(int64_t), st));
@@ -420,13 +422,34 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
   unsigned char *ws = (unsigned char *)workspace;
   p.tile_counter = (unsigned int *)ws;
   p.status_word = (int *)(ws + 4);
+  p.ptile_counter = (unsigned int *)(ws + 8);
   p.chain = (unsigned long long *)(ws + kWsHeader);
-  p.ring = (float *)(ws + ws_chain_bytes(plan));
+  p.chain_p = p.chain + (plan.n_tiles > 0 ? plan.n_tiles : 1);
+  p.key = (unsigned short *)(ws + ws_chain_bytes(plan));
+  p.n_ptiles = plan.n_ptiles;
+  p.p_base = particle_base;
+  {
+    // bulk copies (cp.async.bulk) want 16-byte aligned global addresses: tiles start at multiples of PD_PTILE
+    // particles, so it is the base pointers that count
+    const uintptr_t all = reinterpret_cast<uintptr_t>(ev->pid) | reinterpret_cast<uintptr_t>(ev->charge) | reinterpret_cast<uintptr_t>(ev->px) |
+                          reinterpret_cast<uintptr_t>(ev->py) | reinterpret_cast<uintptr_t>(ev->pz) | reinterpret_cast<uintptr_t>(ev->vx) |
+                          reinterpret_cast<uintptr_t>(ev->vy) | reinterpret_cast<uintptr_t>(ev->vz) | reinterpret_cast<uintptr_t>(ev->E);
+    p.tma_ok = (all & 15u) == 0 ? 1 : 0;
+  }
+  if (n == 0) PD_CUDA(cudaMemsetAsync(trk->offsets, 0, sizeof(int64_t) * (size_t)(ev->n_events + 1), st));  // kernel P has no tile
 
   rc = pd_launch_chain(p, plan, dbg != nullptr, cuda_stream);
   if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "kernel launch");
-  t_launches = 1;
+  t_launches = n > 0 ? 2 : 1;
   return PD_OK;
+}
+
+extern "C" {
+
+int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                pd_towers *tow, pd_eflow *efl, pd_debug *dbg, void *workspace, int64_t workspace_bytes,
+                void *cuda_stream) {
+  return simulate_impl(card, ev, seed, event_base, trk, tow, efl, dbg, workspace, workspace_bytes, cuda_stream, 0);
 }
 
 int pd_last_status(const void *workspace, void *cuda_stream) {
@@ -697,7 +720,7 @@ static int simulate_host_pipelined(const pd_card *card, const pd_events *ev, uin
     pd_tracks ct = {nc, t_off + e0 + c, t_src + p0, t_pid + p0, t_q + p0, t_f[0] + p0, t_f[1] + p0, t_f[2] + p0, t_f[3] + p0, t_f[4] + p0, t_f[5] + p0};
     pd_towers cw = {nc, w_off + e0 + c, w_id + p0, w_f[0] + p0, w_f[1] + p0, w_f[2] + p0, w_f[3] + p0, w_f[4] + p0, w_f[5] + p0};
     pd_eflow cf = {2 * nc, f_off + e0 + c, f_cls + 2 * p0, f_src + 2 * p0, f_f[0] + 2 * p0, f_f[1] + 2 * p0, f_f[2] + 2 * p0, f_f[3] + 2 * p0};
-    rc = pd_simulate(card, &cev, seed, event_base + e0, &ct, &cw, &cf, nullptr, ws, ws_bytes, cuda_stream);
+    rc = simulate_impl(card, &cev, seed, event_base + e0, &ct, &cw, &cf, nullptr, ws, ws_bytes, cuda_stream, p0);
     if (rc != PD_OK) break;
     launches += t_launches;
     cp(&tot[3 * (size_t)c + 0], t_off + e0 + c + nec, 8, cudaMemcpyDeviceToHost, st);

@@ -238,6 +238,7 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
       s.T_edge[k] = k < s.n_T ? float(te[size_t(k)]) : std::numeric_limits<float>::infinity();
     }
     s.eff_per_species = 0;
+    for (int k = 0; k <= PD_MAX_EFF; ++k) s.row_eps[k] = 0.f;
     for (const Row &w : rows) s.eff_per_species |= w.species != 0 ? 1 : 0;
     // one grid per species (reading J1: a row applies to every charged particle or to one species only)
     for (int sp = 1; sp <= 3; ++sp)
@@ -260,6 +261,7 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
             }
           }
           s.cell_eps[sp - 1][ip * (s.n_T + 1) + it] = eps;
+          if (rowi >= 0) s.row_eps[rowi] = eps;
           s.cell_row[sp - 1][ip * (s.n_T + 1) + it] = (signed char)rowi;
         }
       }
@@ -297,6 +299,7 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     c->inv_cosh[i] = float(1.0 / std::cosh(eta));
   }
   c->offset[nb] = acc;
+  s.tb_first = c->tb[0], s.tb_last = c->tb[nb];
 
   // ---- eta-bin lookup: cells of |u| by float bits (2^(23 - PD_LUT_SHIFT) cells per octave, |u| < 2^MIN_EXP in
   // one cell), mirrored for u < 0.  lut[cell] = the bin holding the cell's LOWER bound (clamped to the grid);

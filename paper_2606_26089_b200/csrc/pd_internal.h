@@ -9,10 +9,11 @@
 #include "pd.h"
 
 constexpr int PD_MAX_BINS = 1024;      // eta/theta bins of a card's grid
-constexpr int PD_MAX_EFF = 32;         // rows of the efficiency table in a card
+constexpr int PD_MAX_EFF = 31;         // rows of the efficiency table in a card (kernel P keeps the row in 5 bits, 31 = none)
 constexpr int PD_MAX_EFF_EDGES = 8;    // distinct pT edges / distinct |eta| edges of the table
 constexpr int PD_MAX_EFF_CELLS = (PD_MAX_EFF_EDGES + 1) * (PD_MAX_EFF_EDGES + 1);
-constexpr int PD_MAX_TOWERS = 1 << 15;  // tower ids are packed into 15 bits on chip
+constexpr int PD_MAX_TOWERS = (1 << 15) - 1;  // tower ids are packed into 15 bits on chip, 0x7fff = none
+constexpr int PD_PTILE = 1280;         // particles per tile of kernel P (pd_particles.cu): a multiple of 32, <= 2048
 constexpr int PD_LUT_SHIFT = 19;       // eta-bin lookup: 16 cells per octave of |u|
 constexpr int PD_LUT_MIN_EXP = -8;     // |u| < 2^-8 shares one cell per side
 
@@ -27,6 +28,7 @@ struct PdCardScalars {
   int words_per_event;    // tower bitmap: ceil(n_towers / 128) * 4 words of 32 tower bits
   // eta-bin lookup table over the float bits of |u| (see pd_card.cpp): cells per side, bias
   int lut_side, lut_base;
+  float tb_first, tb_last;  // the grid's coverage in u: tb[0] <= u < tb[n_bins]
   // efficiency table resolved into a grid at load (reading A8: first matching row wins):
   // cell = (#pT edges with pT > e) * (n_T + 1) + (#T edges with |pz|/pT >= t)
   int n_pt, n_T;
@@ -35,6 +37,7 @@ struct PdCardScalars {
   // one grid per species (0 electron, 1 muon, 2 charged hadron; reading J1 of DESIGN.md section 13)
   float cell_eps[3][PD_MAX_EFF_CELLS];
   signed char cell_row[3][PD_MAX_EFF_CELLS];  // row of the card's table, -1 none
+  float row_eps[PD_MAX_EFF + 1];              // efficiency of a row of the card's table
   float trk_a2[3], trk_b[3];  // sigma_rel^2 = a^2 + (b pT)^2, per species (reading J2)
   int trk_per_species;        // 0: the three entries are equal (pass T then skips the pid lookup)
   int eff_per_species;        // 0: no efficiency row names a species (the three grids are equal)
@@ -116,29 +119,37 @@ struct PdParams {
   int n_tiles;
   int capacity;          // C: particles a tile may hold on chip
   int sparse;            // 1: two-level tower bitmap (large grids, small events), see make_layout
-  unsigned long long *chain;  // [2][n_tiles] look-back words: tracks; towers | neutrals
-  float *ring;                // [max_ctas][6][capacity] smeared track records parked between pass T and pass O
+  unsigned long long *chain;  // [n_tiles] look-back words of kernel T: towers | neutrals
   unsigned int *tile_counter;
   int *status_word;
+  // kernel P (pd_particles.cu): flat tiles of PD_PTILE particles
+  long long p_base;              // offsets[0]: first particle of the call in the arrays (0 for a public call)
+  int n_ptiles;
+  int tma_ok;                    // 1: every input array is 16-byte aligned (bulk copies), 0: plain loads
+  unsigned long long *chain_p;   // [n_ptiles] look-back words: accepted tracks
+  unsigned int *ptile_counter;
+  unsigned short *key;           // [n_ptiles * PD_PTILE] per particle: tower id | HCAL bit << 15, 0xffff = no deposit
 };
 
 // pd_card.cpp
 int pd_card_parse(const char *name_or_path, pd_card *c);
 // pd_api.cu
 int pd_card_to_device(const pd_card *c);
-// pd_kernels.cu
+// pd_towers.cu
 struct PdLaunchPlan {
   int threads;       // 512 (two CTAs per SM) or 1024 (one)
   int capacity;      // C
   int events_per_tile;
   int n_tiles;
-  int max_ctas;      // upper bound of the grid (sizes the workspace ring)
+  int n_ptiles;      // tiles of kernel P
   int sparse;        // two-level tower bitmap
   size_t smem_bytes;
 };
 int pd_plan_set_tile_events(int g);
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);
 int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, void *stream);
+// pd_particles.cu
+int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_smem_optin, void *stream);
 
 // pd_features.cu: event features + lepton isolation (pd_event_features)
 struct PdFeatParams {

@@ -263,6 +263,136 @@ static __device__ __noinline__ bool graze_double(const PdCardScalars &sc, float 
   return true;
 }
 
+// readings A4, A5: born on/outside the cylinder, or no transverse momentum -> dropped
+__device__ __forceinline__ bool vertex_dropped(const PdCardScalars &sc, float px, float py, float vx, float vy, float vz) {
+  const float pt2 = fmaf(px, px, py * py);
+  const float r02 = fmaf(vx, vx, vy * vy);
+  return r02 >= sc.R2 || fabsf(vz) >= sc.L || pt2 < 1e-9f;
+}
+
+// S2, first half: cell of the efficiency grid at the true vertex momentum (A7, A8).  pT edges are compared on pT^2
+// in double (px^2 + py^2 is then exact to ~1e-16, so a generator floor at exactly an edge, e.g. pT = 0.1 GeV, is
+// decided like the fp64 definition); |eta| edges as |pz| >= sinh(edge) pT; unused edges are +max / +inf.
+__device__ __forceinline__ int eff_cell(const PdCardScalars &sc, float px, float py, float pz) {
+  const double p2 = (double)px * (double)px + (double)py * (double)py;
+  const float pt2 = fmaf(px, px, py * py);
+  const float pt = pt2 * fast_rsqrt(pt2);
+  const float apz = fabsf(pz);
+  int ip = 0, it = 0;
+  // the first two edges of either kind without a branch, the rest (cards with finer tables) in uniform loops
+  ip += p2 > sc.pt_edge2_d[0] ? 1 : 0;
+  ip += p2 > sc.pt_edge2_d[1] ? 1 : 0;
+  for (int k = 2; k < sc.n_pt; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
+  it += apz >= sc.T_edge[0] * pt ? 1 : 0;
+  it += apz >= sc.T_edge[1] * pt ? 1 : 0;
+  for (int k = 2; k < sc.n_T; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
+  return ip * (sc.n_T + 1) + it;
+}
+
+// S1 for a neutral particle (or no field): straight line to r = R or |z| = L, whichever comes first.  The caller
+// has excluded dropped vertices.  Returns the face; (x, y, z) = the hit.
+__device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, float py, float pz, float vx, float vy, float vz,
+                                             float &x, float &y, float &z) {
+  const float pt2 = fmaf(px, px, py * py);
+  const float apz = fabsf(pz);
+  const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
+  const float zdist = sc.L - sgnz * vz;  // distance to the endcap the particle flies towards (> 0)
+  const float D = sc.R2 - fmaf(vx, vx, vy * vy);  // > 0
+  // t_R = num / den, t_Z = zdist / |pz|
+  const float b = fmaf(vx, px, vy * py);
+  const float sq = fast_sqrt(fmaf(b, b, pt2 * D));
+  const float num = b > 0.f ? D : sq - b;
+  const float den = b > 0.f ? b + sq : pt2;
+  const bool endcap = apz > 0.f && zdist * den < num * apz;
+  const float t = endcap ? zdist * fast_rcp(apz) : num * fast_rcp(den);
+  x = fmaf(t, px, vx), y = fmaf(t, py, vy);
+  z = endcap ? sgnz * sc.L : fmaf(t, pz, vz);
+  return endcap ? PD_ENDCAP : PD_BARREL;
+}
+
+// S1 for a charged particle in the field: helix of radius rho; momentum azimuth phi0 + s alpha (reading A3: q > 0
+// in +z field turns clockwise).  Returns PD_DROPPED | PD_LOOPER for a trapped looper (reading A6), else the face
+// (| PD_LOOPER when the helix never reaches r = R).
+__device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, float px, float py, float pz, float vx, float vy,
+                                              float vz, float &x, float &y, float &z) {
+  const float pt2 = fmaf(px, px, py * py);
+  const float ipt = fast_rsqrt(pt2);
+  const float pt = pt2 * ipt;
+  const float apz = fabsf(pz);
+  const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
+  const float D = sc.R2 - fmaf(vx, vx, vy * vy);  // > 0
+  uint32_t looper = 0;
+  const float aq = fabsf((float)q);
+  const float rho = aq == 1.f ? pt * sc.inv_kB : pt * sc.inv_kB * fast_rcp(aq);
+  const float s = ((q > 0) == (sc.sB > 0.f)) ? -1.f : 1.f;
+  const float c0 = px * ipt, s0 = py * ipt;
+  // vertex in the (u0, s n0) frame: a = v.u0, b = s v.n0
+  const float a_ = fmaf(vx, c0, vy * s0);
+  const float b_ = s * fmaf(vy, c0, -vx * s0);
+  // |v + 2 rho sin h u(phi0 + s h)|^2 = R^2 with t = tan h:  Q t^2 + 2 P t - D = 0   (h = alpha/2)
+  const float P = 2.f * rho * a_;
+  const float Q = fmaf(4.f * rho, rho + b_, -D);
+  const float disc = fmaf(P, P, Q * D);
+  const float scale = fmaf(P, P, 4.f * rho * rho * D);
+  bool reach;
+  float cc = 1.f, ss = 0.f;  // (cos, sin) of the barrel half-angle h_R, unnormalised, ss >= 0
+  if (disc >= 0.f ? disc < 0.08f * scale : -disc < 1e-3f * scale) {
+    reach = graze_double(sc, px, py, vx, vy, aq, s, cc, ss);
+  } else {
+    reach = disc >= 0.f;
+    const float S = fast_sqrt(fmaxf(disc, 0.f));
+    // first crossing: (cos h, sin h) proportional to (P + S, D) if P >= 0 else (Q, S - P)
+    cc = P >= 0.f ? P + S : Q;
+    ss = P >= 0.f ? D : S - P;
+  }
+  if (!reach) looper = PD_LOOPER;
+  if (!reach && apz == 0.f) return PD_DROPPED | looper;  // trapped (reading A6)
+  // endcap half-angle h_Z = zdist kappa |q| B / (2 |pz|), as f = h_Z / pi in double: the turning angle of a
+  // looper can be ~1e5 rad.  1/|pz| = MUFU seed + one Newton step in double.
+  float sh = 0.f, ch = 1.f;
+  bool endcap = false;
+  if (apz > 0.f) {
+    const double pzd = (double)apz;
+    const double r0 = (double)fast_rcp(apz);
+    const double r1 = fma(r0, fma(-pzd, r0, 1.0), r0);
+    const double zd = (double)sc.L - (double)(sgnz * vz);
+    const double fd = zd * (sc.kB_d * (0.5 * 0.31830988618379067154) * (double)aq) * r1;
+    const double nd = (fd + 6755399441055744.0) - 6755399441055744.0;  // rint
+    const float frac = (float)(fd - nd);                                // in [-0.5, 0.5]
+    const float ff = (float)fd;
+    sincospi_half(frac, sh, ch);  // (sin, cos)(h_Z) up to a common sign (-1)^n
+    // h_Z < h_R  <=>  h_Z < pi and sin(h_R - h_Z) > 0   (both half-angles lie in (0, pi))
+    const float cross = fmaf(ss, ch, -cc * sh);
+    endcap = !reach || (ff < 1.f && (frac < 0.f ? -cross : cross) > 0.f);
+  }
+  if (endcap) {
+    z = sgnz * sc.L;
+  } else {
+    const float inv = fast_rsqrt(fmaf(cc, cc, ss * ss));
+    ch = cc * inv, sh = ss * inv;
+    const float hR = fast_atan2(ss, cc);
+    z = fmaf(2.f * hR, pz * sc.inv_kB * (aq == 1.f ? 1.f : fast_rcp(aq)), vz);
+  }
+  // chord form (pi-periodic in h): position = v + 2 rho sin h u(phi0 + s h)
+  const float l2 = 2.f * rho * sh;
+  x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
+  y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
+  return (endcap ? PD_ENDCAP : PD_BARREL) | looper;
+}
+
+// hit (x, y, z) on the face `status` -> grid coordinate u = z/r (or -z/r for a theta grid) and azimuth
+__device__ __forceinline__ void hit_coords(const PdCardScalars &sc, uint32_t status, float x, float y, float z, float &u, float &phi_pos) {
+  const float ir = (status & PD_ENDCAP) ? fast_rsqrt(fmaf(x, x, y * y)) : sc.inv_R;
+  u = (sc.grid_theta ? -z : z) * ir;
+  phi_pos = fast_atan2(y, x);
+}
+
+// S4: tower of the hit, -1 outside the grid
+__device__ __forceinline__ int hit_tower(const PdCardScalars &sc, const SmCard &cd, float u, float phi_pos) {
+  const int i = grid_bin(cd, sc, u);
+  return i >= 0 ? cd.offset[i] + phi_bin(cd, i, phi_pos) : -1;
+}
+
 __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const SmCard &cd, int q, float px, float py,
                                                float pz, float vx, float vy, float vz, const PhiloxKeys &seed,
                                                long long event, uint32_t pidx, int species, ParticleOut &o) {
@@ -272,113 +402,15 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
   o.accepted = false;
   o.u = __int_as_float(0x7fc00000);
   o.phi_pos = o.u;
-
-  const float pt2 = fmaf(px, px, py * py);
-  const float r02 = fmaf(vx, vx, vy * vy);
-  // readings A4, A5: born on/outside the cylinder, or no transverse momentum -> dropped
-  if (r02 >= sc.R2 || fabsf(vz) >= sc.L || pt2 < 1e-9f) return;
-  const float ipt = fast_rsqrt(pt2);
-  const float pt = pt2 * ipt;
-  const float apz = fabsf(pz);
-  const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
-  const float zdist = sc.L - sgnz * vz;  // distance to the endcap the particle flies towards (> 0)
-  const float D = sc.R2 - r02;           // > 0
+  if (vertex_dropped(sc, px, py, vx, vy, vz)) return;
   float x, y, z;
-  bool endcap;
-  uint32_t looper = 0;
-
-  if (q == 0 || sc.sB == 0.f) {
-    // straight line to r = R or |z| = L, whichever comes first: t_R = num / den, t_Z = zdist / |pz|
-    const float b = fmaf(vx, px, vy * py);
-    const float sq = fast_sqrt(fmaf(b, b, pt2 * D));
-    const float num = b > 0.f ? D : sq - b;
-    const float den = b > 0.f ? b + sq : pt2;
-    endcap = apz > 0.f && zdist * den < num * apz;
-    const float t = endcap ? zdist * fast_rcp(apz) : num * fast_rcp(den);
-    x = fmaf(t, px, vx), y = fmaf(t, py, vy);
-    z = endcap ? sgnz * sc.L : fmaf(t, pz, vz);
-  } else {
-    // helix of radius rho; momentum azimuth phi0 + s alpha (reading A3: q > 0 in +z field turns clockwise)
-    const float aq = fabsf((float)q);
-    const float rho = aq == 1.f ? pt * sc.inv_kB : pt * sc.inv_kB * fast_rcp(aq);
-    const float s = ((q > 0) == (sc.sB > 0.f)) ? -1.f : 1.f;
-    const float c0 = px * ipt, s0 = py * ipt;
-    // vertex in the (u0, s n0) frame: a = v.u0, b = s v.n0
-    const float a_ = fmaf(vx, c0, vy * s0);
-    const float b_ = s * fmaf(vy, c0, -vx * s0);
-    // |v + 2 rho sin h u(phi0 + s h)|^2 = R^2 with t = tan h:  Q t^2 + 2 P t - D = 0   (h = alpha/2)
-    const float P = 2.f * rho * a_;
-    const float Q = fmaf(4.f * rho, rho + b_, -D);
-    const float disc = fmaf(P, P, Q * D);
-    const float scale = fmaf(P, P, 4.f * rho * rho * D);
-    bool reach;
-    float cc = 1.f, ss = 0.f;  // (cos, sin) of the barrel half-angle h_R, unnormalised, ss >= 0
-    if (disc >= 0.f ? disc < 0.08f * scale : -disc < 1e-3f * scale) {
-      reach = graze_double(sc, px, py, vx, vy, aq, s, cc, ss);
-    } else {
-      reach = disc >= 0.f;
-      const float S = fast_sqrt(fmaxf(disc, 0.f));
-      // first crossing: (cos h, sin h) proportional to (P + S, D) if P >= 0 else (Q, S - P)
-      cc = P >= 0.f ? P + S : Q;
-      ss = P >= 0.f ? D : S - P;
-    }
-    if (!reach) looper = PD_LOOPER;
-    if (!reach && apz == 0.f) {
-      o.status = PD_DROPPED | looper;  // trapped (reading A6)
-      return;
-    }
-    // endcap half-angle h_Z = zdist kappa |q| B / (2 |pz|), as f = h_Z / pi in double: the turning angle of a
-    // looper can be ~1e5 rad.  1/|pz| = MUFU seed + one Newton step in double.
-    float sh = 0.f, ch = 1.f;
-    endcap = false;
-    if (apz > 0.f) {
-      const double pzd = (double)apz;
-      const double r0 = (double)fast_rcp(apz);
-      const double r1 = fma(r0, fma(-pzd, r0, 1.0), r0);
-      const double zd = (double)sc.L - (double)(sgnz * vz);
-      const double fd = zd * (sc.kB_d * (0.5 * 0.31830988618379067154) * (double)aq) * r1;
-      const double nd = (fd + 6755399441055744.0) - 6755399441055744.0;  // rint
-      const float frac = (float)(fd - nd);                                // in [-0.5, 0.5]
-      const float ff = (float)fd;
-      sincospi_half(frac, sh, ch);  // (sin, cos)(h_Z) up to a common sign (-1)^n
-      // h_Z < h_R  <=>  h_Z < pi and sin(h_R - h_Z) > 0   (both half-angles lie in (0, pi))
-      const float cross = fmaf(ss, ch, -cc * sh);
-      endcap = !reach || (ff < 1.f && (frac < 0.f ? -cross : cross) > 0.f);
-    }
-    if (endcap) {
-      z = sgnz * sc.L;
-    } else {
-      const float inv = fast_rsqrt(fmaf(cc, cc, ss * ss));
-      ch = cc * inv, sh = ss * inv;
-      const float hR = fast_atan2(ss, cc);
-      z = fmaf(2.f * hR, pz * sc.inv_kB * (aq == 1.f ? 1.f : fast_rcp(aq)), vz);
-    }
-    // chord form (pi-periodic in h): position = v + 2 rho sin h u(phi0 + s h)
-    const float l2 = 2.f * rho * sh;
-    x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
-    y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
-  }
-  o.status = (endcap ? PD_ENDCAP : PD_BARREL) | looper;
-  const float ir = endcap ? fast_rsqrt(fmaf(x, x, y * y)) : sc.inv_R;
-  const float u = (sc.grid_theta ? -z : z) * ir;
-  const float phi_pos = fast_atan2(y, x);
-  o.u = u;
-  o.phi_pos = phi_pos;
-
+  if (q == 0 || sc.sB == 0.f) o.status = line_hit(sc, px, py, pz, vx, vy, vz, x, y, z);
+  else o.status = helix_hit(sc, q, px, py, pz, vx, vy, vz, x, y, z);
+  if ((o.status & PD_FACE_MASK) == PD_DROPPED) return;
+  hit_coords(sc, o.status, x, y, z, o.u, o.phi_pos);
   // S2 track: efficiency cell at the true vertex momentum (A7); accept iff u24 < eps (A11)
   if (q != 0) {
-    // pT edges are compared on pT^2 in double (px^2 + py^2 is then exact to ~1e-16, so a generator floor at
-    // exactly an edge, e.g. pT = 0.1 GeV, is decided like the fp64 definition); unused edges are +max
-    const double p2 = (double)px * (double)px + (double)py * (double)py;
-    int ip = 0, it = 0;
-    // the first two edges of either kind without a branch, the rest (cards with finer tables) in uniform loops
-    ip += p2 > sc.pt_edge2_d[0] ? 1 : 0;
-    ip += p2 > sc.pt_edge2_d[1] ? 1 : 0;
-    for (int k = 2; k < sc.n_pt; ++k) ip += p2 > sc.pt_edge2_d[k] ? 1 : 0;
-    it += apz >= sc.T_edge[0] * pt ? 1 : 0;
-    it += apz >= sc.T_edge[1] * pt ? 1 : 0;
-    for (int k = 2; k < sc.n_T; ++k) it += apz >= sc.T_edge[k] * pt ? 1 : 0;
-    const int cell = ip * (sc.n_T + 1) + it;
+    const int cell = eff_cell(sc, px, py, pz);
     const float eps = sc.cell_eps[species][cell];
     o.eps_row = sc.cell_row[species][cell];
     if (eps > 0.f) {
@@ -387,10 +419,7 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
       o.accepted = uniform24(rn[0]) < eps;
     }
   }
-
-  // S4 tower of the hit
-  const int i = grid_bin(cd, sc, u);
-  if (i >= 0) o.tower = cd.offset[i] + phi_bin(cd, i, phi_pos);
+  o.tower = hit_tower(sc, cd, o.u, o.phi_pos);
 }
 
 // S3 for one accepted track (A12/A13): log-normal with mean pT and std sigma_rel pT, driven by words
@@ -399,19 +428,25 @@ struct TrackOut {
   float pt_s, eta_mom, phi0, E_trk;
 };
 
-__device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, float py, float pz,
-                                            const PhiloxKeys &seed, long long event, uint32_t pidx, int species, TrackOut &t) {
+// r1, r2: words 1 and 2 of the particle's Philox block (stream 0)
+__device__ __forceinline__ void track_smear_words(const PdCardScalars &sc, float px, float py, float pz, uint32_t r1, uint32_t r2,
+                                                  int species, TrackOut &t) {
   const float pt2 = fmaf(px, px, py * py);
   const float ipt = fast_rsqrt(pt2);
   const float pt = pt2 * ipt;
-  uint32_t rn[4];
-  rng_block(seed, event, pidx, 0u, rn);
   const float bp = sc.trk_b[species] * pt;
   const float rel2 = fmaf(bp, bp, sc.trk_a2[species]);
-  t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(rn[1], rn[2])) : pt;
+  t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(r1, r2)) : pt;
   t.E_trk = t.pt_s * (fast_sqrt(fmaf(pz, pz, pt2)) * ipt);
   t.eta_mom = fast_asinh(pz * ipt);
   t.phi0 = fast_atan2(py, px);
+}
+
+__device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, float py, float pz,
+                                            const PhiloxKeys &seed, long long event, uint32_t pidx, int species, TrackOut &t) {
+  uint32_t rn[4];
+  rng_block(seed, event, pidx, 0u, rn);
+  track_smear_words(sc, px, py, pz, rn[1], rn[2], species, t);
 }
 
 // per-tower smear of both components (S6): the common case of a single non-zero component runs one

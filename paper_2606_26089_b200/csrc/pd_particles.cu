@@ -1,0 +1,413 @@
+// pd_particles.cu -- kernel P of the chain: the per-particle half (steps S0-S4 of SURVEY.md section 8a, and the
+// track half of S8), as a FLAT pass over the particle arrays: tiles of PT_TILE consecutive particles, whatever
+// events they belong to, so there is no limit on the size of an event.
+//
+// Why flat: the chain is bound by instruction issue, and with one thread per particle in particle order a warp
+// runs the helix, the straight line, the Philox block and the smear for whoever needs them (17.6 of 32 lanes
+// active in round 1).  Here a tile's inputs are staged in shared memory by bulk asynchronous copies
+// (cp.async.bulk, one elected thread, completion on an mbarrier), the particles are split by CLASS into index
+// lists -- A: charged inside the tracker acceptance (efficiency > 0: helix + Philox + accept + smear), B: other
+// charged (helix only), N: neutral (straight line) -- and the lists are processed by full warps gathering from
+// shared memory.  An accepted track is smeared on the spot (its Philox block is in registers) and its record
+// parked in the particle's own staging slots; after a scan over the accepted bits in particle order and a
+// decoupled look-back over the tiles the Track collection is written in its final place.
+//
+// What the tower pass (pd_towers.cu) needs is a 16-bit key per particle (tower id | HCAL bit, 0xffff = no deposit),
+// written to the workspace with one bulk store per tile, and the Track collection itself.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "pd_internal.h"
+#include "pd_math.cuh"
+#include "pd_scan.cuh"
+
+namespace pdk {
+
+constexpr int PT_THREADS = 256;
+constexpr int PT_WARPS = PT_THREADS / 32;
+constexpr int PT_TILE = PD_PTILE;  // particles per tile (pd_internal.h); a multiple of 32
+constexpr int PT_WORDS = PT_TILE / 32;
+constexpr uint32_t PT_NONE = 0xffffu;
+static_assert(PT_TILE % 32 == 0 && PT_TILE <= 2048, "list entries keep the particle in 11 bits");
+
+// Shared-memory carve-up of kernel P: the per-particle arrays sit at compile-time offsets (their addresses fold into
+// the instructions), the card tables behind them at offsets that depend on the card.
+constexpr int PT_PER_WARP = PT_TILE / PT_WARPS;  // particles a warp owns: a multiple of 32
+constexpr int PT_ITERS = PT_PER_WARP / 32;
+static_assert(PT_PER_WARP % 32 == 0 && PT_PER_WARP <= 255, "a warp owns whole 32-particle rows; ranks fit 8 bits");
+constexpr size_t PO_F = 0;                                  // px, py, pz, vx, vy, vz: 6 x 4 B x TILE
+constexpr size_t PO_PID = PO_F + 6 * 4 * (size_t)PT_TILE;   // 4 B x TILE
+constexpr size_t PO_Q = PO_PID + 4 * (size_t)PT_TILE;       // 1 B x TILE
+constexpr size_t PO_EVK = PO_Q + (size_t)PT_TILE;           // 2 B x TILE: event of the particle (relative), then its key
+constexpr size_t PO_EST = PO_EVK + 2 * (size_t)PT_TILE;     // 2 B x TILE: local index of the first particle of its event
+constexpr size_t PO_LIST = PO_EST + 2 * (size_t)PT_TILE;    // 2 B x TILE: class lists (per warp: A | B | N), then tracks in order
+constexpr size_t PO_MASK = PO_LIST + 2 * (size_t)PT_TILE;   // accepted bits
+constexpr size_t PO_PRE = PO_MASK + 4 * (size_t)PT_WORDS;   // their prefix per word (+ total)
+constexpr size_t PO_MISC = (PO_PRE + 4 * (size_t)(PT_WORDS + 1) + 15) & ~size_t(15);
+constexpr size_t PO_TABLES = PO_MISC + 8 * 16;
+static_assert(PO_PID % 16 == 0 && PO_Q % 16 == 0 && PO_EVK % 16 == 0 && PO_LIST % 16 == 0, "bulk copies need 16-byte aligned slots");
+
+struct PTables {
+  size_t tb, binrec, lut, total;
+};
+__host__ __device__ inline PTables make_ptables(int n_bins, int lut_cells) {
+  PTables l;
+  size_t o = PO_TABLES;
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o = (o + bytes + 15) & ~size_t(15);
+    return at;
+  };
+  l.tb = take(4 * (size_t)(n_bins + 1));
+  l.binrec = take(16 * (size_t)n_bins);  // per bin: inv_w, half, offset | nphi << 16, pad
+  l.lut = take(2 * (size_t)lut_cells);
+  l.total = o;
+  return l;
+}
+
+// S4 with the per-bin record in one 16-byte load: tower of the hit (u, phi), -1 outside the grid
+__device__ __forceinline__ int hit_tower_rec(const PdCardScalars &sc, const float *tb, const float4 *rec, const unsigned short *lut,
+                                             float u, float phi) {
+  if (!(u >= sc.tb_first) || !(u < sc.tb_last)) return -1;
+  int ca = (__float_as_int(fabsf(u)) >> PD_LUT_SHIFT) - sc.lut_base;
+  ca = min(max(ca, 0), sc.lut_side - 1);
+  const int cell = u < 0.f ? sc.lut_side - 1 - ca : sc.lut_side + ca;
+  int b = lut[cell];
+  while (u >= tb[b + 1]) ++b;  // terminates: u < tb[n_bins]
+  const float4 r = rec[b];
+  const int on = __float_as_int(r.z);
+  const int n = on >> 16;
+  int j = (int)floorf(fmaf(phi, r.x, r.y)) + (n >> 1);
+  j = j < 0 ? 0 : j;
+  j = j > n - 1 ? n - 1 : j;
+  return (on & 0xffff) + j;
+}
+
+template <bool DEBUG>
+__global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid_constant__ PdParams prm) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const PdCardScalars &sc = prm.sc;
+  const int nb = sc.n_bins;
+  float *s_px = (float *)(smem + PO_F), *s_py = s_px + PT_TILE, *s_pz = s_py + PT_TILE;
+  float *s_vx = s_pz + PT_TILE, *s_vy = s_vx + PT_TILE, *s_vz = s_vy + PT_TILE;
+  int *s_pid = (int *)(smem + PO_PID);
+  signed char *s_q = (signed char *)(smem + PO_Q);
+  unsigned short *s_evk = (unsigned short *)(smem + PO_EVK);
+  unsigned short *s_est = (unsigned short *)(smem + PO_EST);
+  unsigned short *s_list = (unsigned short *)(smem + PO_LIST);
+  uint32_t *s_accmask = (uint32_t *)(smem + PO_MASK);
+  uint32_t *s_accpre = (uint32_t *)(smem + PO_PRE);
+  unsigned long long *s_misc = (unsigned long long *)(smem + PO_MISC);
+  uint64_t *s_bar = (uint64_t *)(s_misc + 0);
+  int *s_cnt = (int *)(s_misc + 1);               // [0] accepted tracks so far, [1] warps done with their class A, [2] tile
+  long long *s_win = (long long *)(s_misc + 3);   // [0] e_lo, [1] offsets[e_lo], [2] first event with offset >= s, [3] first with offset >= s + T
+  long long *s_base = (long long *)(s_misc + 8);  // [0] track prefix of the tile
+  const PTables TL = make_ptables(nb, 2 * sc.lut_side);
+  float *s_tb = (float *)(smem + TL.tb);
+  float4 *s_rec = (float4 *)(smem + TL.binrec);
+  unsigned short *s_lut = (unsigned short *)(smem + TL.lut);
+
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+
+  for (int i = tid; i <= nb; i += PT_THREADS) s_tb[i] = prm.tab.tb[i];
+  for (int i = tid; i < nb; i += PT_THREADS)
+    s_rec[i] = make_float4(prm.tab.inv_w[i], prm.tab.half[i], __int_as_float(prm.tab.offset[i] | (prm.tab.nphi[i] << 16)), 0.f);
+  for (int i = tid; i < 2 * sc.lut_side; i += PT_THREADS) s_lut[i] = prm.tab.lut[i];
+  if (tid == 0) {
+    mbar_init(s_bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  uint32_t phase = 0;
+  // the particles of the call are [p_base, p_end) of the arrays (p_base = offsets[0]: 0 for a public call, the chunk's
+  // first particle for the pipelined host entry); tiles start at p_al = p_base rounded down to 16 particles, so that
+  // every tile start is 16-byte aligned in all arrays; the (< 16) particles in front of p_base are skipped
+  const long long p_base = prm.p_base, p_al = p_base & ~15ll, n_all = p_base + prm.n_particles;
+  const int wbase = wid * PT_PER_WARP;  // this warp owns particles [wbase, wbase + PT_PER_WARP) of every tile
+
+  for (;;) {
+    __syncthreads();  // previous tile fully done with shared memory (tables staged, mbarrier initialised)
+    if (tid == 0) {
+      s_cnt[2] = (int)atomicAdd(prm.ptile_counter, 1u);
+      s_cnt[0] = 0, s_cnt[1] = 0;
+    }
+    for (int k = tid; k < PT_WORDS; k += PT_THREADS) s_accmask[k] = 0u;
+    __syncthreads();
+    const int tile = s_cnt[2];
+    if (tile >= prm.n_ptiles) break;
+    const long long s0 = p_al + (long long)tile * PT_TILE;
+    const int n = (int)min((long long)PT_TILE, n_all - s0);
+    const int lo_skip = (int)max(p_base - s0, 0ll);  // > 0 only in tile 0
+    const long long s_eff = s0 + lo_skip;            // first particle of the call in the tile
+    const bool full = n == PT_TILE && prm.tma_ok;
+
+    // ---- stage the tile's inputs: eight bulk copies (one thread), or plain loads for the ragged last tile /
+    // unaligned arrays
+    if (full) {
+      if (tid == 0) {
+        fence_async_smem();  // the staging slots were last written through the generic proxy
+        mbar_expect_tx(s_bar, 29u * PT_TILE);
+        bulk_g2s(s_px, prm.px + s0, 4u * PT_TILE, s_bar);
+        bulk_g2s(s_py, prm.py + s0, 4u * PT_TILE, s_bar);
+        bulk_g2s(s_pz, prm.pz + s0, 4u * PT_TILE, s_bar);
+        bulk_g2s(s_vx, prm.vx + s0, 4u * PT_TILE, s_bar);
+        bulk_g2s(s_vy, prm.vy + s0, 4u * PT_TILE, s_bar);
+        bulk_g2s(s_vz, prm.vz + s0, 4u * PT_TILE, s_bar);
+        bulk_g2s(s_pid, prm.pid + s0, 4u * PT_TILE, s_bar);
+        bulk_g2s(s_q, prm.charge + s0, 1u * PT_TILE, s_bar);
+      }
+    } else {
+      for (int i = tid; i < n; i += PT_THREADS) {
+        s_px[i] = __ldg(prm.px + s0 + i), s_py[i] = __ldg(prm.py + s0 + i), s_pz[i] = __ldg(prm.pz + s0 + i);
+        s_vx[i] = __ldg(prm.vx + s0 + i), s_vy[i] = __ldg(prm.vy + s0 + i), s_vz[i] = __ldg(prm.vz + s0 + i);
+        s_pid[i] = __ldg(prm.pid + s0 + i), s_q[i] = __ldg(prm.charge + s0 + i);
+      }
+    }
+
+    // ---- the events of the tile (while the copies are in flight).  offsets[0..n_events] is non-decreasing:
+    // e_lo = the event of particle s_eff; [w2, w3) = the events whose first particle (or empty position) lies in the
+    // tile: this tile writes their track offsets.
+    if (wid == 0) {
+      const long long ne1 = prm.n_events + 1;
+      const long long ub = warp_lower_bound(prm.offsets, ne1, s_eff + 1);  // entries <= s_eff
+      const long long e_lo = ub - 1;
+      const long long o_lo = __ldg(prm.offsets + e_lo);
+      const long long w2 = o_lo == s_eff ? warp_lower_bound(prm.offsets, ne1, s_eff) : ub;
+      const long long w3 = s0 + PT_TILE >= n_all ? ne1 : warp_lower_bound(prm.offsets, ne1, s0 + PT_TILE);
+      if (lane == 0) s_win[0] = e_lo, s_win[1] = o_lo, s_win[2] = w2, s_win[3] = w3;
+    }
+    __syncthreads();
+    const long long e_lo = s_win[0];
+    const long long e_hi = min(s_win[3], prm.n_events) - 1;  // last event with a particle in the tile (or an empty one before the end)
+    const bool wide = e_hi - e_lo >= 0xffff;                  // only with > 65,000 empty events inside one tile
+    if (!wide) {
+      // warp per event, lanes over its particles
+      for (long long e = e_lo + wid; e <= e_hi; e += PT_WARPS) {
+        const long long a = __ldg(prm.offsets + e) - s0, b = __ldg(prm.offsets + e + 1) - s0;
+        const int j0 = (int)max(a, 0ll), j1 = (int)min(b, (long long)n);
+        const unsigned short st = a >= 0 ? (unsigned short)a : (unsigned short)PT_NONE;
+        for (int j = j0 + lane; j < j1; j += 32) s_evk[j] = (unsigned short)(e - e_lo), s_est[j] = st;
+      }
+    }
+    __syncthreads();  // events filled in (the partition overwrites the entry of a dropped particle); plain loads done
+    if (full) mbar_wait(s_bar, phase), phase ^= 1u;
+    const uint32_t head_shift = (uint32_t)(s0 - s_win[1]);  // index within its event of particle s0
+
+    // ---- partition of the warp's own particles by class (S0): A charged with efficiency > 0, B other charged,
+    // N neutral; dropped particles are finished here.  No other warp is involved: ballots and register counts.
+    int nA = 0, nB = 0, nN = 0;
+    uint32_t pk[PT_ITERS];  // per row: entry (i | row << 11) | class << 16 | rank within the class << 18
+#pragma unroll
+    for (int k = 0; k < PT_ITERS; ++k) {
+      const int i = wbase + 32 * k + lane;
+      int cls = 3;  // 0 A, 1 B, 2 N, 3 none
+      int row = 0;
+      if (i < n && i < lo_skip) s_evk[i] = (unsigned short)PT_NONE;
+      if (i < n && i >= lo_skip) {
+        const int q = (int)s_q[i];
+        const float px = s_px[i], py = s_py[i];
+        if (vertex_dropped(sc, px, py, s_vx[i], s_vy[i], s_vz[i])) {
+          s_evk[i] = (unsigned short)PT_NONE;
+          if (DEBUG) {
+            const long long g = s0 + i;
+            const float nanv = __int_as_float(0x7fc00000);
+            if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)PD_DROPPED;
+            if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = nanv;
+            if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = nanv;
+            if (prm.dbg_tower) prm.dbg_tower[g] = -1;
+            if (prm.dbg_accepted) prm.dbg_accepted[g] = 0;
+            if (prm.dbg_eps_row) prm.dbg_eps_row[g] = -1;
+            if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = 0.f;
+          }
+        } else if (q == 0) {
+          cls = 2;
+        } else {
+          const int sp = sc.eff_per_species ? species_of(s_pid[i]) : 2;
+          row = (int)sc.cell_row[sp][eff_cell(sc, px, py, s_pz[i])];
+          cls = (row >= 0 && sc.row_eps[row] > 0.f) ? 0 : 1;
+          row = row < 0 ? 31 : row;  // class B keeps the row for the debug output (31: none; PD_MAX_EFF = 31 rows)
+        }
+      }
+      const unsigned mA = __ballot_sync(0xffffffffu, cls == 0), mB = __ballot_sync(0xffffffffu, cls == 1),
+                     mN = __ballot_sync(0xffffffffu, cls == 2);
+      const unsigned mine = cls == 0 ? mA : (cls == 1 ? mB : mN);
+      const int before = cls == 0 ? nA : (cls == 1 ? nB : nN);
+      pk[k] = (uint32_t)(i | (row << 11)) | ((uint32_t)cls << 16) | ((uint32_t)(before + __popc(mine & lt_mask)) << 18);
+      nA += __popc(mA), nB += __popc(mB), nN += __popc(mN);
+    }
+#pragma unroll
+    for (int k = 0; k < PT_ITERS; ++k) {
+      const int cls = (int)((pk[k] >> 16) & 3u), rank = (int)(pk[k] >> 18);
+      if (cls != 3) s_list[wbase + (cls == 0 ? 0 : (cls == 1 ? nA : nA + nB)) + rank] = (unsigned short)pk[k];
+    }
+    __syncwarp();
+    const int n_work = nA + nB + nN;
+
+    // ---- S1-S4 on the warp's lists A | B | N: rows of one class (the rows at the two boundaries are mixed)
+    int n_acc = 0;
+    bool signalled = false;
+#pragma unroll 1
+    for (int k = 0; k < PT_ITERS; ++k) {
+      const int v = 32 * k + lane;
+      if (v < n_work) {
+        const int cls = v < nA ? 0 : (v < nA + nB ? 1 : 2);
+        const unsigned ent = s_list[wbase + v];
+        const int i = (int)(ent & 0x7ffu);
+        const float px = s_px[i], py = s_py[i], pz = s_pz[i], vx = s_vx[i], vy = s_vy[i], vz = s_vz[i];
+        const int pid = s_pid[i];
+        float x, y, z;
+        uint32_t status;
+        if (cls == 2 || sc.sB == 0.f) status = line_hit(sc, px, py, pz, vx, vy, vz, x, y, z);
+        else status = helix_hit(sc, (int)s_q[i], px, py, pz, vx, vy, vz, x, y, z);
+        const bool live = (status & PD_FACE_MASK) != PD_DROPPED;
+        float u = __int_as_float(0x7fc00000), phi_pos = u;
+        int tower = -1;
+        if (live) {
+          hit_coords(sc, status, x, y, z, u, phi_pos);
+          tower = hit_tower_rec(sc, s_tb, s_rec, s_lut, u, phi_pos);
+        }
+        const int apid = pid < 0 ? -pid : pid;
+        const bool to_ecal = apid == 11 || apid == 22;  // reading A18
+        const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
+        bool accepted = false;
+        float pt_s = 0.f;
+        if (cls == 0 && live) {
+          // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0
+          long long ev;
+          uint32_t pidx;
+          if (!wide) {
+            const unsigned er = s_evk[i], st = s_est[i];
+            ev = e_lo + er;
+            pidx = st == PT_NONE ? head_shift + (uint32_t)i : (uint32_t)i - st;
+          } else {
+            long long lo = e_lo, hi = e_hi;  // last event with offsets[e] <= s0 + i
+            const long long g = s0 + i;
+            while (lo < hi) {
+              const long long mid = (lo + hi + 1) >> 1;
+              if (__ldg(prm.offsets + mid) <= g) lo = mid;
+              else hi = mid - 1;
+            }
+            ev = lo, pidx = (uint32_t)(g - __ldg(prm.offsets + lo));
+          }
+          uint32_t rn[4];
+          rng_block(prm.rk, prm.event_base + ev, pidx, 0u, rn);
+          accepted = uniform24(rn[0]) < sc.row_eps[ent >> 11];
+          if (accepted) {
+            // S3 on the spot; the record is parked in the particle's own staging slots until its place is known
+            TrackOut t;
+            track_smear_words(sc, px, py, pz, rn[1], rn[2], sc.trk_per_species ? species_of(pid) : 2, t);
+            pt_s = t.pt_s;
+            s_px[i] = t.pt_s, s_py[i] = t.eta_mom, s_pz[i] = t.phi0, s_vx[i] = t.E_trk;
+            s_vy[i] = eta_from_u(sc, u), s_vz[i] = phi_pos;
+            atomicOr(&s_accmask[i >> 5], 1u << (i & 31));
+          }
+        }
+        // what the tower pass needs: tower | HCAL bit, or "no deposit"
+        s_evk[i] = (tower >= 0 && !to_none) ? (unsigned short)((unsigned)tower | (to_ecal ? 0u : 0x8000u)) : (unsigned short)PT_NONE;
+        n_acc += accepted ? 1 : 0;
+        if (DEBUG) {
+          const long long g = s0 + i;
+          const int row = (int)(ent >> 11);
+          if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)status;
+          if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = live ? eta_from_u(sc, u) : u;
+          if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = phi_pos;
+          if (prm.dbg_tower) prm.dbg_tower[g] = tower;
+          if (prm.dbg_accepted) prm.dbg_accepted[g] = accepted ? 1 : 0;
+          if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)((cls == 2 || !live || row == 31) ? -1 : row);
+          if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = pt_s;
+        }
+      }
+      // The tile's number of accepted tracks is known as soon as every warp is through its class A: the last warp to
+      // get there PUBLISHES it on the look-back chain, a good part of the tile before anyone needs the prefix.
+      if (!signalled && 32 * (k + 1) >= nA) {
+        signalled = true;
+        const int mine = (int)__reduce_add_sync(0xffffffffu, (unsigned)n_acc);
+        if (lane == 0) {
+          atomicAdd(&s_cnt[0], mine);
+          __threadfence_block();
+          if (atomicAdd(&s_cnt[1], 1) == PT_WARPS - 1) chain_publish(prm.chain_p, tile, (unsigned long long)atomicAdd(&s_cnt[0], 0));
+        }
+      }
+    }
+    fence_async_smem();  // the keys go out with a bulk store (async proxy)
+    __syncthreads();
+
+    // ---- accepted tracks in particle order: prefix over the mask words, the ordered list
+    if (wid == 0) {
+      // PT_WORDS <= 64 words: two per lane
+      const int k0 = 2 * lane, k1 = 2 * lane + 1;
+      const unsigned c0 = k0 < PT_WORDS ? (unsigned)__popc(s_accmask[k0]) : 0u, c1 = k1 < PT_WORDS ? (unsigned)__popc(s_accmask[k1]) : 0u;
+      const unsigned incl = warp_incl_scan(c0 + c1);
+      const unsigned excl = incl - (c0 + c1);
+      if (k0 < PT_WORDS) s_accpre[k0] = excl;
+      if (k1 < PT_WORDS) s_accpre[k1] = excl + c0;
+      const unsigned total = __shfl_sync(0xffffffffu, incl, 31);
+      if (lane == 0) {
+        s_accpre[PT_WORDS] = total;
+        // the keys of a full tile leave with one bulk store (the ragged last tile: plain stores below)
+        if (full) {
+          bulk_s2g(prm.key + (s0 - p_al), s_evk, 2u * PT_TILE);
+          bulk_commit();
+        }
+      }
+    }
+    __syncthreads();
+    const int n_trk = (int)s_accpre[PT_WORDS];
+    for (int i = tid; i < n; i += PT_THREADS) {
+      const uint32_t m = s_accmask[i >> 5];
+      if ((m >> (i & 31)) & 1u) s_list[s_accpre[i >> 5] + __popc(m & ((1u << (i & 31)) - 1u))] = (unsigned short)i;
+    }
+    if (!full)
+      for (int i = tid; i < n; i += PT_THREADS) prm.key[s0 - p_al + i] = s_evk[i];
+    if (wid == 0) {
+      const unsigned long long ex = chain_resolve<8>(prm.chain_p, tile, (unsigned long long)n_trk);
+      if (lane == 0) s_base[0] = (long long)ex;
+    }
+    __syncthreads();
+    const long long base = s_base[0];
+
+    // ---- S8 for tracks: the collection in its final place, and the track offsets of the events that start here
+    for (int r = tid; r < n_trk; r += PT_THREADS) {
+      const int i = s_list[r];
+      const unsigned g = (unsigned)base + (unsigned)r;  // all output indices fit 32 bits (n_particles < 2^30)
+      prm.trk_src[g] = (int)(s0 + i);
+      prm.trk_pid[g] = s_pid[i];
+      prm.trk_charge[g] = s_q[i];
+      prm.trk_pt[g] = s_px[i];
+      prm.trk_eta[g] = s_py[i];
+      prm.trk_phi[g] = s_pz[i];
+      prm.trk_E[g] = s_vx[i];
+      prm.trk_eta_out[g] = s_vy[i];
+      prm.trk_phi_out[g] = s_vz[i];
+    }
+    for (long long e = s_win[2] + tid; e < s_win[3]; e += PT_THREADS) {
+      const int j = (int)(__ldg(prm.offsets + e) - s0);  // 0..n
+      const int w = j >> 5;
+      const unsigned below = j >= n ? (unsigned)n_trk : s_accpre[w] + (unsigned)__popc(s_accmask[w] & ((1u << (j & 31)) - 1u));
+      prm.trk_offsets[e] = base + below;
+    }
+    if (full && tid == 0) bulk_wait_read0();  // the key store has read its shared-memory source
+    fence_async_smem();  // the parked records were generic-proxy writes to slots the next tile's bulk copies overwrite
+  }
+}
+
+}  // namespace pdk
+
+size_t pd_particle_smem_bytes(const pd_card *c) { return pdk::make_ptables(c->sc.n_bins, 2 * c->sc.lut_side).total; }
+
+int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_smem_optin, void *stream) {
+  const size_t smem = pdk::make_ptables(prm.sc.n_bins, 2 * prm.sc.lut_side).total;
+  if (smem > (size_t)max_smem_optin) return PD_ECUDA;
+  auto kern = debug ? pdk::pd_particle_kernel<true> : pdk::pd_particle_kernel<false>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin) != cudaSuccess) return PD_ECUDA;
+  // persistent CTAs wait on one another through the look-back chain: the grid must be co-resident
+  int per_sm = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, pdk::PT_THREADS, smem) != cudaSuccess) return PD_ECUDA;
+  if (per_sm < 1) return PD_ECUDA;
+  int grid = num_sms * per_sm;
+  if (grid > prm.n_ptiles) grid = prm.n_ptiles;
+  if (grid < 1) grid = 1;
+  kern<<<grid, pdk::PT_THREADS, smem, (cudaStream_t)stream>>>(prm);
+  return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
+}

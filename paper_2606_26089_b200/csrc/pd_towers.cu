@@ -1,0 +1,681 @@
+// pd_towers.cu -- kernel T of the chain: the per-event half (steps S5-S8 of SURVEY.md section 8a).
+//
+// Kernel P (pd_particles.cu) has left, per particle, a 16-bit key (tower id | HCAL bit, 0xffff = no deposit) and
+// the finished Track collection.  Here persistent CTAs (two 512-thread CTAs per SM, or one 1024-thread CTA for
+// large events) claim TILES (runs of G whole events, <= C particles) from an atomic counter and take each through
+//   pass A'  S5         keys and deposit energies of the tile (coalesced); marks the tower in the event's BITMAP
+//   scan 1              popcount prefix of the bitmaps = the rank ("slot") of every occupied tower in
+//                       (event, tower id) order -- this replaces a sort of the deposits; meanwhile the energies of
+//                       the tile's tracks are scattered to their particles
+//   pass B   S5         every deposit pushes itself on its slot's list (one integer atomicExch)
+//   pass W   S5-S7      one thread per occupied tower: exact fixed-point sum of its list (order-independent),
+//                       Philox tower stream, log-normal smear, thresholds, EFlow subtraction
+//   scan W              one scan over the per-warp counts; chain W published and resolved (decoupled look-back)
+//   pass O   S8         ordered compaction of towers / photons / neutral hadrons, the EFlow entries of the tracks
+//                       (copied from the Track collection), CSR offsets
+// Large grids with small events use a two-level bitmap (sparse mode, see make_layout): groups first, then the
+// tower bits of the non-empty groups only.
+// Sums are order-stable: each tower's deposits are added as 64-bit fixed-point integers (exact, hence independent
+// of the order in which the list was built), and the only atomics are integer (bitmap OR, list exchange, counters).
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+
+#include "pd_internal.h"
+#include "pd_math.cuh"
+#include "pd_scan.cuh"
+
+namespace pdk {
+
+constexpr int G_MAX = 256;         // events per tile (event index of a particle is kept in 8 bits)
+constexpr int C_MAX = 8191;        // particles per tile: list links are 13 bits, 0x1fff = end of list
+constexpr uint32_t LINK_END = 0x1fffu;
+// per-particle result word: tower id (15 bits, 0x7fff none) | flags | link to the next deposit of the tower
+constexpr uint32_t RES_TOWER = 0x7fffu, RES_DEP = 1u << 15, RES_HCAL = 1u << 16, RES_ACC = 1u << 17;
+constexpr int RES_LINK_SHIFT = 18;
+constexpr unsigned long long FIELD_MASK = (1ull << 31) - 1;  // chain W packs towers | neutrals << 31
+// per-slot word after pass W: head particle (13 bits) | tower id (15 bits) << 13 | what the slot emits
+constexpr uint32_t SLOT_TW = 1u << 28, SLOT_PH = 1u << 29, SLOT_NH = 1u << 30;
+
+__host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~size_t(15); }
+
+// Shared-memory carve-up, identical on host (size) and device (pointers).
+struct Layout {
+  size_t offset, w, eta_c, inv_cosh, binlut;     // card tables (what pass O needs)
+  size_t off32, ntrk, ntow, nph, nnh;            // per-event arrays [G+1]
+  size_t misc;                                   // scratch words
+  size_t cnt;                                    // pass W warp counts -> prefixes [2][256]
+  size_t bitmap, gprefix;                        // per event: tower bits, group prefix
+  size_t l2p, pool;                              // sparse mode (see make_layout)
+  size_t res, Ev, Et, head, stg, ev;             // per particle / per slot
+  size_t total;
+};
+
+// Dense mode: one bit per tower and event (bitmap), a prefix per 128-tower group (gprefix).
+// Sparse mode (large grids, small events: the bitmaps would be almost empty and take most of the shared memory):
+// `bitmap` holds one bit per 128-tower GROUP and event, `l2p` the rank of the first non-empty group of each of its
+// words, `pool` the tower bits of the non-empty groups only (at most one per deposit), `gprefix` their prefixes.
+__host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int words_per_event, int G, int C, int sparse) {
+  Layout l;
+  size_t o = 0;
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o = align16(o + bytes);
+    return at;
+  };
+  l.offset = take(4 * (n_bins + 1));
+  l.w = take(4 * n_bins);
+  l.eta_c = take(4 * n_bins);
+  l.inv_cosh = take(4 * n_bins);
+  l.binlut = take(2 * (size_t)((n_towers >> 5) + 2));
+  l.off32 = take(4 * (G + 1));
+  l.ntrk = take(4 * (G + 1));
+  l.ntow = take(4 * (G + 1));
+  l.nph = take(4 * (G + 1));
+  l.nnh = take(4 * (G + 1));
+  l.misc = take(8 * 64);
+  l.cnt = take(4 * 2 * 256);
+  const int gpe = words_per_event / 4, l2w = (gpe + 31) / 32;
+  l.l2p = 0, l.pool = 0;
+  if (!sparse) {
+    l.bitmap = take(4 * (size_t)G * words_per_event);
+    l.gprefix = take(2 * ((size_t)G * gpe + 1));
+  } else {
+    l.bitmap = take(4 * (size_t)G * l2w);
+    l.l2p = take(2 * ((size_t)G * l2w + 1));
+    l.pool = take(16 * (size_t)C);
+    l.gprefix = take(2 * ((size_t)C + 1));
+  }
+  l.res = take(4 * (size_t)C);
+  l.Ev = take(4 * ((size_t)C + 4));   // + 4: the bulk copy of the deposit energies starts at a 16-byte boundary
+  l.Et = take(4 * (size_t)C);
+  l.head = take(4 * (size_t)C);
+  l.stg = take(4 * ((size_t)C + 4));  // first the keys (2 B each, + 8 for the same reason), later one float per slot
+  l.ev = take(G > 1 ? (size_t)C : 0);
+  l.total = o;
+  return l;
+}
+constexpr int T_BYTES_PER_PARTICLE = 20;  // res, Ev, Et, head, stg
+
+// counts a[0..ne) -> exclusive prefix in place, a[ne] = total.  One warp; ne <= G_MAX = 256.
+__device__ __forceinline__ void event_scan(int *a, int ne) {
+  const int lane = threadIdx.x & 31;
+  int v[8], sum = 0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const int idx = lane * 8 + k;
+    v[k] = idx < ne ? a[idx] : 0;
+    sum += v[k];
+  }
+  int incl = sum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  const int total = __shfl_sync(0xffffffffu, incl, 31);
+  __syncwarp();
+  int run = incl - sum;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const int idx = lane * 8 + k;
+    if (idx < ne) a[idx] = run;
+    run += v[k];
+  }
+  if (lane == 0) a[ne] = total;
+}
+
+// Block-wide exclusive prefix of per-warp totals wtot[W] (REDUX adds): returns the exclusive prefix of this
+// thread's WARP and the block total.
+template <int W>
+__device__ __forceinline__ void warp_totals_scan(const unsigned *wtot, unsigned &excl_warp, unsigned &total) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const unsigned v = lane < W ? wtot[lane] : 0u;
+  total = __reduce_add_sync(0xffffffffu, v);
+  excl_warp = __reduce_add_sync(0xffffffffu, lane < wid ? v : 0u);
+}
+
+__device__ __forceinline__ int popc4(const uint4 &v) { return __popc(v.x) + __popc(v.y) + __popc(v.z) + __popc(v.w); }
+
+// number of set bits of the 128-bit group below bit position pos (0..127)
+__device__ __forceinline__ int popc_below(const uint4 &v, int pos) {
+  const int w = pos >> 5;
+  const uint32_t m = (1u << (pos & 31)) - 1u;
+  // branch-free: words below w count in full, word w below the bit, words above not at all
+  const uint32_t m0 = w > 0 ? 0xffffffffu : m, m1 = w > 1 ? 0xffffffffu : (w == 1 ? m : 0u),
+                 m2 = w > 2 ? 0xffffffffu : (w == 2 ? m : 0u), m3 = w == 3 ? m : 0u;
+  return __popc(v.x & m0) + __popc(v.y & m1) + __popc(v.z & m2) + __popc(v.w & m3);
+}
+
+template <int THREADS, int CTAS, bool DEBUG, bool SPARSE>
+__global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_constant__ PdParams prm) {
+  constexpr int W = THREADS / 32;
+  extern __shared__ __align__(16) unsigned char smem[];
+  const PdCardScalars &sc = prm.sc;
+  const int nb = sc.n_bins;
+  const int C = prm.capacity, G = prm.events_per_tile;
+  const int wpe = sc.words_per_event, gpe = wpe >> 2;
+  constexpr bool sparse = SPARSE;   // two-level tower bitmap, chosen by pd_plan (prm.sparse)
+  const int l2w = (gpe + 31) >> 5;  // words of the per-event group bitmap (sparse mode)
+  const Layout L = make_layout(nb, sc.n_towers, wpe, G, C, prm.sparse);
+  int *s_offset = (int *)(smem + L.offset);
+  float *s_w = (float *)(smem + L.w);
+  float *s_eta_c = (float *)(smem + L.eta_c);
+  float *s_inv_cosh = (float *)(smem + L.inv_cosh);
+  unsigned short *s_binlut = (unsigned short *)(smem + L.binlut);
+  int *s_off32 = (int *)(smem + L.off32);
+  int *s_ntrk = (int *)(smem + L.ntrk);  // tracks of the tile before event e (from the Track offsets kernel P wrote)
+  int *s_ntow = (int *)(smem + L.ntow);
+  int *s_nph = (int *)(smem + L.nph);
+  int *s_nnh = (int *)(smem + L.nnh);
+  unsigned long long *s_misc = (unsigned long long *)(smem + L.misc);
+  unsigned *s_wtot = (unsigned *)(s_misc + 8);    // [32] per-warp totals of scan 1
+  unsigned *s_preA = (unsigned *)(smem + L.cnt);  // per (iteration, warp) of pass W: towers | photons << 16 ...
+  unsigned *s_preB = s_preA + 256;                // ... and neutral hadrons (counts, then exclusive prefixes)
+  uint32_t *s_bitmap = (uint32_t *)(smem + L.bitmap);
+  unsigned short *s_gp = (unsigned short *)(smem + L.gprefix);
+  unsigned short *s_l2p = (unsigned short *)(smem + L.l2p);  // sparse mode: rank of the first non-empty group of a word
+  uint4 *s_pool = (uint4 *)(smem + L.pool);                  // sparse mode: tower bits of the non-empty groups
+  uint32_t *s_res = (uint32_t *)(smem + L.res);
+  float *s_Ev_raw = (float *)(smem + L.Ev);  // deposit energy; after pass W, at the head particle: Ehad''
+  float *s_Et = (float *)(smem + L.Et);     // track energy of accepted tracks; after pass W, at the head: photon energy
+  unsigned *s_head = (unsigned *)(smem + L.head);  // per slot: last pusher, then head | tower id << 13 | flags
+  float *s_stg = (float *)(smem + L.stg);   // per slot after pass W: Eem''  (neutral-hadron energy goes to s_res[head])
+  unsigned char *s_ev = smem + L.ev;
+  uint64_t *s_bar = (uint64_t *)(s_misc + 4);
+
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+
+  for (int i = tid; i <= nb; i += THREADS) s_offset[i] = prm.tab.offset[i];
+  for (int i = tid; i < nb; i += THREADS) {
+    s_w[i] = prm.tab.w[i];
+    s_eta_c[i] = prm.tab.eta_c[i];
+    s_inv_cosh[i] = prm.tab.inv_cosh[i];
+  }
+  __syncthreads();
+  // eta bin of tower ids 0, 32, 64, ...: start of the short forward search of pass O
+  for (int c = tid; c <= (sc.n_towers >> 5); c += THREADS) {
+    const int id = c << 5;
+    int lo = 0, hi = nb;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (s_offset[mid] <= id) lo = mid;
+      else hi = mid;
+    }
+    s_binlut[c] = (unsigned short)lo;
+  }
+  if (tid == 0) {
+    mbar_init(s_bar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  uint32_t phase = 0;
+  const long long p_al = prm.p_base & ~15ll;  // the key of particle p sits at key[p - p_al]
+
+  for (;;) {
+    __syncthreads();  // previous tile fully done with shared memory (and card tables staged)
+    if (tid == 0) s_misc[0] = atomicAdd(prm.tile_counter, 1u);
+    __syncthreads();
+    const int tile = (int)s_misc[0];
+    if (tile >= prm.n_tiles) break;
+    const long long e0 = (long long)tile * G;
+    const int ne = (int)min((long long)G, prm.n_events - e0);
+    const bool multi = G > 1;
+    const long long p0 = prm.offsets[e0];
+    const long long p1 = prm.offsets[e0 + ne];
+    int n = (int)min(p1 - p0, (long long)0x7fffffff);
+    const bool overflow = (p1 - p0) > (long long)C;
+    if (overflow) {
+      n = 0;
+      if (tid == 0) atomicExch(prm.status_word, (int)PD_EEVENTSIZE);
+    }
+    // the tile's deposit energies and keys arrive by bulk copies (one thread; completion on the mbarrier) while the
+    // CTA sets up the tile: 16-byte aligned start, whole 16-byte pieces; the few elements behind them by plain loads
+    const int shE = (int)(p0 & 3), shK = (int)((p0 - p_al) & 7);
+    const int nbE = prm.tma_ok ? ((shE + n) & ~3) : 0, nbK = prm.tma_ok ? ((shK + n) & ~7) : 0;
+    float *s_Ev = s_Ev_raw + shE;
+    const unsigned short *s_key = (const unsigned short *)s_stg + shK;
+    const bool bulk = nbE > 0 || nbK > 0;
+    if (tid == 0 && bulk) {
+      fence_async_smem();  // the slots were last written through the generic proxy
+      mbar_expect_tx(s_bar, 4u * nbE + 2u * nbK);
+      if (nbE > 0) bulk_g2s(s_Ev_raw, prm.E + (p0 - shE), 4u * nbE, s_bar);
+      if (nbK > 0) bulk_g2s(s_stg, prm.key + (p0 - p_al - shK), 2u * nbK, s_bar);
+    }
+    for (int i = nbE - shE + tid; i < n; i += THREADS) s_Ev[i] = __ldg(prm.E + p0 + i);
+    for (int i = nbK - shK + tid; i < n; i += THREADS) ((unsigned short *)s_stg)[shK + i] = __ldg(prm.key + (p0 - p_al) + i);
+    const long long t0 = prm.trk_offsets[e0];  // first track of the tile (kernel P wrote the Track collection)
+    const int n_trk = overflow ? 0 : (int)(prm.trk_offsets[e0 + ne] - t0);
+    for (int e = tid; e <= ne; e += THREADS) {
+      s_off32[e] = overflow ? 0 : (int)(prm.offsets[e0 + e] - p0);
+      s_ntrk[e] = overflow ? 0 : (int)(prm.trk_offsets[e0 + e] - t0);
+      s_ntow[e] = 0, s_nph[e] = 0, s_nnh[e] = 0;
+    }
+    const int NG = ne * gpe;  // 128-tower bitmap groups of the tile
+    const int NW = ne * l2w;  // sparse mode: words of the group bitmaps
+    if (!sparse) {
+      for (int k = tid; k < NG; k += THREADS) ((uint4 *)s_bitmap)[k] = make_uint4(0u, 0u, 0u, 0u);
+    } else {
+      for (int k = tid; k < NW; k += THREADS) s_bitmap[k] = 0u;
+    }
+    __syncthreads();
+    if (multi) {
+      // event index of every particle of the tile: warp per event, lanes over its particles
+      for (int e = wid; e < ne; e += W)
+        for (int i = s_off32[e] + lane; i < s_off32[e + 1]; i += 32) s_ev[i] = (unsigned char)e;
+      __syncthreads();
+    }
+
+    // ------------------------------------------------------------------ pass A': keys (deposit energies are in place)
+    if (bulk) mbar_wait(s_bar, phase), phase ^= 1u;
+    for (int i = tid; i < n; i += THREADS) {
+      const unsigned key = s_key[i];
+      uint32_t res = RES_TOWER | (LINK_END << RES_LINK_SHIFT);
+      if (key != 0xffffu) {
+        const int tower = (int)(key & 0x7fffu);
+        const int e = multi ? (int)s_ev[i] : 0;
+        res = (uint32_t)tower | (LINK_END << RES_LINK_SHIFT) | RES_DEP | ((key & 0x8000u) ? RES_HCAL : 0u);
+        if (!sparse) atomicOr(&s_bitmap[e * wpe + (tower >> 5)], 1u << (tower & 31));
+        else atomicOr(&s_bitmap[e * l2w + (tower >> 12)], 1u << ((tower >> 7) & 31));  // its 128-tower group
+      }
+      s_res[i] = res;
+      s_head[i] = 0xffffffffu;
+      if (DEBUG && prm.dbg_tw_first) prm.dbg_tw_first[p0 + i] = 0;
+    }
+    __syncthreads();
+
+    // ------------------------------------------------------------------ scan 1: tower slots; track energies
+    // Each thread owns a contiguous chunk of bitmap groups (odd chunk lengths keep the shared-memory accesses of a
+    // warp on distinct banks).
+    int n_slots;
+    {
+      // dense: the groups' tower bits; sparse: the words of the group bitmaps (their bits = non-empty groups)
+      const int NS = sparse ? NW : NG;
+      const int kg = ((NS + THREADS - 1) / THREADS) | 1;
+      const int g0 = min(NS, tid * kg), g1 = min(NS, g0 + kg);
+      unsigned cnt_g = 0;
+      if (!sparse) {
+        for (int g = g0; g < g1; ++g) cnt_g += (unsigned)popc4(((const uint4 *)s_bitmap)[g]);
+      } else {
+        for (int g = g0; g < g1; ++g) cnt_g += (unsigned)__popc(s_bitmap[g]);
+      }
+      const unsigned incl = warp_incl_scan(cnt_g);
+      if (lane == 31) s_wtot[wid] = incl;
+      // the tile's accepted tracks: their energy goes to their particle (pass W subtracts it from the tower)
+      for (int t = tid; t < n_trk; t += THREADS) {
+        const int i = (int)((long long)__ldg(prm.trk_src + t0 + t) - p0);
+        s_Et[i] = __ldg(prm.trk_E + t0 + t);
+        s_res[i] |= RES_ACC;
+      }
+      __syncthreads();
+      unsigned excl_w, tot;
+      warp_totals_scan<W>(s_wtot, excl_w, tot);
+      int rg = (int)(excl_w + incl - cnt_g);
+      if (!sparse) {
+        for (int g = g0; g < g1; ++g) {
+          s_gp[g] = (unsigned short)rg;
+          rg += popc4(((const uint4 *)s_bitmap)[g]);
+        }
+      } else {
+        for (int g = g0; g < g1; ++g) {
+          s_l2p[g] = (unsigned short)rg;
+          rg += __popc(s_bitmap[g]);
+        }
+      }
+      n_slots = (int)tot;
+    }
+    __syncthreads();
+    if (sparse) {
+      // ---- sparse mode: n_slots is so far the number of NON-EMPTY GROUPS (<= deposits <= C).  Their tower bits go
+      // into the pool, at the rank of the group in (event, group) order; a second scan turns them into slots.
+      const int n_groups = n_slots;
+      for (int k = tid; k < n_groups; k += THREADS) s_pool[k] = make_uint4(0u, 0u, 0u, 0u);
+      __syncthreads();
+      for (int i = tid; i < n; i += THREADS) {
+        const uint32_t r = s_res[i];
+        if (r & RES_DEP) {
+          const int id = (int)(r & RES_TOWER);
+          const int w = (multi ? (int)s_ev[i] * l2w : 0) + (id >> 12);
+          const int pg = (int)s_l2p[w] + __popc(s_bitmap[w] & ((1u << ((id >> 7) & 31)) - 1u));
+          atomicOr(&((uint32_t *)s_pool)[4 * pg + ((id >> 5) & 3)], 1u << (id & 31));
+        }
+      }
+      __syncthreads();
+      const int kp = ((n_groups + THREADS - 1) / THREADS) | 1;
+      const int q0 = min(n_groups, tid * kp), q1 = min(n_groups, q0 + kp);
+      unsigned cnt_p = 0;
+      for (int g = q0; g < q1; ++g) cnt_p += (unsigned)popc4(s_pool[g]);
+      const unsigned incl_p = warp_incl_scan(cnt_p);
+      if (lane == 31) s_wtot[wid] = incl_p;
+      __syncthreads();
+      unsigned excl_wp, tot_p;
+      warp_totals_scan<W>(s_wtot, excl_wp, tot_p);
+      int rp = (int)(excl_wp + incl_p - cnt_p);
+      for (int g = q0; g < q1; ++g) {
+        s_gp[g] = (unsigned short)rp;
+        rp += popc4(s_pool[g]);
+      }
+      n_slots = (int)tot_p;
+      __syncthreads();
+    }
+
+    // ------------------------------------------------------------------ pass B (S5): every deposit finds its
+    // tower's slot and pushes itself on the slot's list
+    for (int i = tid; i < n; i += THREADS) {
+      const uint32_t r = s_res[i];
+      if (r & RES_DEP) {
+        const int id = (int)(r & RES_TOWER);
+        int g;
+        uint4 bits;
+        if (!sparse) {
+          g = (multi ? (int)s_ev[i] * gpe : 0) + (id >> 7);
+          bits = ((const uint4 *)s_bitmap)[g];
+        } else {
+          const int w = (multi ? (int)s_ev[i] * l2w : 0) + (id >> 12);
+          g = (int)s_l2p[w] + __popc(s_bitmap[w] & ((1u << ((id >> 7) & 31)) - 1u));
+          bits = s_pool[g];
+        }
+        const int slot = (int)s_gp[g] + popc_below(bits, id & 127);
+        const unsigned prev = atomicExch(&s_head[slot], (unsigned)i);
+        s_res[i] = (r & ~(LINK_END << RES_LINK_SHIFT)) | ((prev & LINK_END) << RES_LINK_SHIFT);
+      }
+    }
+    __syncthreads();
+
+    // ------------------------------------------------------------------ pass W: S5-S7, one thread per tower
+    const int n_it = (n_slots + THREADS - 1) / THREADS;  // <= C_MAX / THREADS + 1, so n_it * W <= 256
+    for (int it = 0; it < n_it; ++it) {
+      const int d = it * THREADS + tid;
+      bool f_tw = false, f_ph = false, f_nh = false;
+      if (d < n_slots) {
+        const int h = (int)(s_head[d] & LINK_END);
+        const uint32_t rh = s_res[h];
+        const int tower = (int)(rh & RES_TOWER);
+        const int e = multi ? (int)s_ev[h] : 0;
+        // S5: exact fixed-point sums (units of 2^-32 GeV, 64-bit integers) over the slot's list.  Integer
+        // addition is associative, so the sums do not depend on the order in which the deposits arrived:
+        // bitwise reproducible, and closer to the fp64 definition than a sequential fp32 sum.
+        long long a_em = 0, a_had = 0, t_em = 0, t_had = 0;
+        int first = h;
+        for (int c = h;;) {
+          const uint32_t rc = c == h ? rh : s_res[c];
+          const long long Ev = __float2ll_rn(s_Ev[c] * 4294967296.f);
+          const long long Tv = (rc & RES_ACC) ? __float2ll_rn(s_Et[c] * 4294967296.f) : 0ll;
+          if (rc & RES_HCAL) a_had += Ev, t_had += Tv;
+          else a_em += Ev, t_em += Tv;
+          first = min(first, c);
+          c = (int)(rc >> RES_LINK_SHIFT);
+          if (c == (int)LINK_END) break;
+        }
+        const float Eem = (float)a_em * 2.3283064365386963e-10f, Ehad = (float)a_had * 2.3283064365386963e-10f;
+        const float Tem = (float)t_em * 2.3283064365386963e-10f, Thad = (float)t_had * 2.3283064365386963e-10f;
+        uint32_t rn[4];
+        rng_block(prm.rk, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
+        float em_s, had_s;
+        tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
+        // reading A22: the threshold is applied twice, strictly, per component
+        const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
+        const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
+        const float n_em = em_f - Tem, n_had = had_f - Thad;
+        f_ph = n_em > sc.thr_ecal, f_nh = n_had > sc.thr_hcal;
+        f_tw = em_f + had_f > 0.f;
+        if (multi) {
+          if (f_tw) atomicAdd(&s_ntow[e], 1);
+          if (f_ph) atomicAdd(&s_nph[e], 1);
+          if (f_nh) atomicAdd(&s_nnh[e], 1);
+        }
+        // stage the tower: per slot and at its head particle's index (only this thread ever touches that particle
+        // again); pass O takes the decisions from the flags, not from the staged values
+        s_stg[d] = em_f, s_Ev[h] = had_f, s_Et[h] = n_em;
+        s_res[h] = __float_as_uint(n_had);
+        s_head[d] = (unsigned)h | ((unsigned)tower << 13) | (f_tw ? SLOT_TW : 0u) | (f_ph ? SLOT_PH : 0u) | (f_nh ? SLOT_NH : 0u);
+        if (DEBUG) {
+          const long long g = p0 + first;
+          if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 1;
+          if (prm.dbg_tw[0]) prm.dbg_tw[0][g] = Eem;
+          if (prm.dbg_tw[1]) prm.dbg_tw[1][g] = Ehad;
+          if (prm.dbg_tw[2]) prm.dbg_tw[2][g] = Tem;
+          if (prm.dbg_tw[3]) prm.dbg_tw[3][g] = Thad;
+          if (prm.dbg_tw[4]) prm.dbg_tw[4][g] = em_s;
+          if (prm.dbg_tw[5]) prm.dbg_tw[5][g] = had_s;
+          if (prm.dbg_tw_dec)
+            prm.dbg_tw_dec[g] = (unsigned char)((k_em ? PD_DEC_EEM : 0) | (k_had ? PD_DEC_EHAD : 0) |
+                                                (f_ph ? PD_DEC_NEM : 0) | (f_nh ? PD_DEC_NHAD : 0));
+        }
+      }
+      // counts of this warp's 32 slots; scanned over all (iteration, warp) pairs below = slot order
+      const unsigned m_tw = __ballot_sync(0xffffffffu, f_tw), m_ph = __ballot_sync(0xffffffffu, f_ph),
+                     m_nh = __ballot_sync(0xffffffffu, f_nh);
+      if (lane == 0) {
+        s_preA[it * W + wid] = (unsigned)__popc(m_tw) | ((unsigned)__popc(m_ph) << 16);
+        s_preB[it * W + wid] = (unsigned)__popc(m_nh);
+      }
+    }
+    __syncthreads();
+
+    // ------------------------------------------------------------------ scan W + chain W (towers | neutrals)
+    if (wid == 0) {
+      // exclusive prefix over the <= 256 (iteration, warp) counts: eight consecutive entries per lane
+      const int n_ent = n_it * W;
+      unsigned va[8], vb[8], sa = 0, sb = 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int idx = lane * 8 + k;
+        va[k] = idx < n_ent ? s_preA[idx] : 0u;
+        vb[k] = idx < n_ent ? s_preB[idx] : 0u;
+        sa += va[k], sb += vb[k];
+      }
+      const unsigned ia = warp_incl_scan(sa), ib = warp_incl_scan(sb);
+      const unsigned ta = __shfl_sync(0xffffffffu, ia, 31), tb = __shfl_sync(0xffffffffu, ib, 31);
+      unsigned ra = ia - sa, rb = ib - sb;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int idx = lane * 8 + k;
+        if (idx < n_ent) s_preA[idx] = ra, s_preB[idx] = rb;
+        ra += va[k], rb += vb[k];
+      }
+      const int n_tow = (int)(ta & 0xffffu), n_ph = (int)(ta >> 16), n_nh = (int)tb;
+      if (!multi && lane == 0) s_ntow[0] = 0, s_ntow[1] = n_tow, s_nph[0] = 0, s_nph[1] = n_ph, s_nnh[0] = 0, s_nnh[1] = n_nh;
+      const unsigned long long agg = (unsigned long long)n_tow | ((unsigned long long)(n_ph + n_nh) << 31);
+      if (lane == 0) chain_publish(prm.chain, tile, agg);  // successors add it up without waiting for this tile's prefix
+      const unsigned long long ex = chain_resolve<8>(prm.chain, tile, agg);
+      if (lane == 0) s_misc[2] = ex;
+    } else if (multi) {
+      if (wid == 2) event_scan(s_ntow, ne);
+      else if (wid == 3) event_scan(s_nph, ne);
+      else if (wid == 4) event_scan(s_nnh, ne);
+    }
+    __syncthreads();
+    const long long base_tow = (long long)(s_misc[2] & FIELD_MASK);
+    const long long base_efl = t0 + (long long)((s_misc[2] >> 31) & FIELD_MASK);
+
+    // ------------------------------------------------------------------ pass O: ordered outputs
+    for (int e = tid; e < ne; e += THREADS) {
+      prm.tow_offsets[e0 + e + 1] = base_tow + s_ntow[e + 1];
+      prm.efl_offsets[e0 + e + 1] = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + s_nnh[e + 1];
+    }
+    if (tile == 0 && tid == 0) prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
+    // the EFlow entries of the tracks: copied from the Track collection (coalesced reads, L2 hits)
+    for (int s = tid; s < n_trk; s += THREADS) {
+      const long long g = t0 + s;
+      const int src = __ldg(prm.trk_src + g);
+      const int pid = __ldg(prm.trk_pid + g);
+      const float pt = __ldg(prm.trk_pt + g), eta = __ldg(prm.trk_eta + g), phi = __ldg(prm.trk_phi + g), Et = __ldg(prm.trk_E + g);
+      const int e = multi ? (int)s_ev[(int)((long long)src - p0)] : 0;
+      const unsigned at = (unsigned)base_efl + (unsigned)(s + s_nph[e] + s_nnh[e]);
+      const int apid = pid < 0 ? -pid : pid;
+      prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
+      prm.efl_src[at] = src;
+      prm.efl_pt[at] = pt;
+      prm.efl_eta[at] = eta;
+      prm.efl_phi[at] = phi;
+      prm.efl_E[at] = Et;
+    }
+    for (int it = 0; it < n_it; ++it) {
+      const int d = it * THREADS + tid;
+      const unsigned hv = d < n_slots ? s_head[d] : 0u;
+      const bool f_tw = hv & SLOT_TW, f_ph = hv & SLOT_PH, f_nh = hv & SLOT_NH;
+      const unsigned m_tw = __ballot_sync(0xffffffffu, f_tw), m_ph = __ballot_sync(0xffffffffu, f_ph),
+                     m_nh = __ballot_sync(0xffffffffu, f_nh);
+      if (hv & (SLOT_TW | SLOT_PH | SLOT_NH)) {
+        const int h = (int)(hv & LINK_END), tower = (int)((hv >> 13) & RES_TOWER);
+        const float em = s_stg[d], had = s_Ev[h], nem = s_Et[h], nhad = __uint_as_float(s_res[h]);
+        const unsigned pa = s_preA[it * W + wid], pb = s_preB[it * W + wid];
+        const int e = multi ? (int)s_ev[h] : 0;
+        int b = (int)s_binlut[tower >> 5];
+        while (tower >= s_offset[b + 1]) ++b;
+        const int j = tower - s_offset[b];
+        const float eta_c = s_eta_c[b];
+        const float phi_c = fmaf((float)j + 0.5f, s_w[b], -kPiF);
+        const float ic = s_inv_cosh[b];
+        if (f_tw) {
+          const unsigned at = (unsigned)base_tow + (pa & 0xffffu) + (unsigned)__popc(m_tw & lt_mask);
+          prm.tow_tower[at] = tower;
+          prm.tow_eta[at] = eta_c;
+          prm.tow_phi[at] = phi_c;
+          prm.tow_E[at] = em + had;
+          prm.tow_Eem[at] = em;
+          prm.tow_Ehad[at] = had;
+          prm.tow_ET[at] = (em + had) * ic;
+        }
+        if (f_ph) {
+          const int slot = (int)(pa >> 16) + __popc(m_ph & lt_mask);
+          const unsigned at = (unsigned)base_efl + (unsigned)(s_ntrk[e + 1] + s_nnh[e] + slot);
+          prm.efl_cls[at] = (signed char)PD_CLS_PHOTON;
+          prm.efl_src[at] = tower;
+          prm.efl_pt[at] = nem * ic;
+          prm.efl_eta[at] = eta_c;
+          prm.efl_phi[at] = phi_c;
+          prm.efl_E[at] = nem;
+        }
+        if (f_nh) {
+          const int slot = (int)pb + __popc(m_nh & lt_mask);
+          const unsigned at = (unsigned)base_efl + (unsigned)(s_ntrk[e + 1] + s_nph[e + 1] + slot);
+          prm.efl_cls[at] = (signed char)PD_CLS_NEUHAD;
+          prm.efl_src[at] = tower;
+          prm.efl_pt[at] = nhad * ic;
+          prm.efl_eta[at] = eta_c;
+          prm.efl_phi[at] = phi_c;
+          prm.efl_E[at] = nhad;
+        }
+      }
+    }
+    fence_async_smem();  // generic-proxy writes to slots the next tile's bulk copies overwrite
+  }
+}
+
+}  // namespace pdk
+
+// ---- host side: plan + launch ------------------------------------------------------------------
+
+static int g_num_sms = 0;
+static int g_max_smem_optin = 0;
+
+static int query_device() {
+  if (g_num_sms > 0) return PD_OK;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PD_ECUDA;
+  if (cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PD_ECUDA;
+  if (cudaDeviceGetAttribute(&g_max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) return PD_ECUDA;
+  return PD_OK;
+}
+
+// Tile plan of kernel T from sizes the host knows (n_events, n_particles).  B200: 228 KB of shared memory per SM,
+// 1 KB reserved per CTA, 227 KB per CTA at most.  Preferred shape: two 512-thread CTAs per SM (113 KB each), so one
+// CTA's barriers and look-back waits are covered by the other; events too large for that get one 1024-thread CTA
+// with the whole SM.  G = events per tile: as many as fit the on-chip capacity C with 6 sigma of head-room
+// for a Poisson-like sum, but no more than keeps every CTA slot of the GPU busy on small inputs.
+static thread_local int t_tile_events = 0;  // pd_set_tile_events: 0 = automatic
+int pd_plan_set_tile_events(int g) {
+  const int prev = t_tile_events;
+  t_tile_events = g < 0 ? 0 : (g > pdk::G_MAX ? pdk::G_MAX : g);
+  return prev;
+}
+
+int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan) {
+  const PdCardScalars &sc = c->sc;
+  const double avg = n_events > 0 ? double(n_particles) / double(n_events) : 0.0;
+  const size_t budget2 = (228 * 1024 - 2 * 1024) / 2, budget1 = 227 * 1024;
+  int sparse = 0;
+  auto cap_for = [&](int G, size_t budget) {
+    const size_t fixed = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, G, 0, sparse).total;
+    const size_t per = pdk::T_BYTES_PER_PARTICLE + (G > 1 ? 1 : 0) + (sparse ? 18 : 0);
+    long cap = budget > fixed + 7 * 16 ? long((budget - fixed - 7 * 16) / per) : 0;
+    cap &= ~3L;
+    return int(cap > pdk::C_MAX ? pdk::C_MAX : cap);
+  };
+  auto fits = [&](int G, size_t budget) {
+    const double C = cap_for(G, budget);
+    return double(G) * avg + 6.0 * std::sqrt(double(G) * avg + 1.0) + 16.0 <= C;
+  };
+  static const int force_threads = std::getenv("PD_THREADS") ? std::atoi(std::getenv("PD_THREADS")) : 0;
+  size_t budget = budget2;
+  plan->threads = 512;
+  // one event per tile on request (pd_set_tile_events(1), the fall-back for batches with outlier events): the
+  // large variant, so that the only limit left is the capacity of a whole SM
+  if (force_threads == 1024 || t_tile_events == 1 || (force_threads == 0 && !fits(1, budget2))) {
+    budget = budget1;
+    plan->threads = 1024;
+  }
+  int g = 1;
+  while (g < pdk::G_MAX && fits(g + 1, budget)) ++g;
+  if (plan->threads == 512) {
+    // sparse mode (two-level tower bitmap) when it packs clearly more events into a tile: large grids, small events
+    static const int force_sparse = std::getenv("PD_SPARSE") ? std::atoi(std::getenv("PD_SPARSE")) : -1;
+    const int g_dense = g;
+    sparse = 1;
+    int gs = 1;
+    while (gs < pdk::G_MAX && fits(gs + 1, budget)) ++gs;
+    const bool take = force_sparse >= 0 ? force_sparse != 0 : (g_dense > 1 && 2 * gs >= 3 * g_dense);
+    if (take && fits(1, budget)) g = gs;
+    else sparse = 0;
+  }
+  // keep all CTA slots busy: aim for >= 4 tiles per resident CTA when the input is small
+  const long slots = 148L * (plan->threads == 512 ? 2 : 1);
+  const long g_bal = long((n_events + 4 * slots - 1) / (4 * slots));
+  if (g > g_bal) g = int(g_bal < 1 ? 1 : g_bal);
+  if (t_tile_events > 0 && g > t_tile_events) g = t_tile_events;
+  plan->events_per_tile = g;
+  plan->capacity = cap_for(g, budget);
+  plan->n_tiles = int((n_events + g - 1) / g);
+  plan->n_ptiles = int((n_particles + 15 + PD_PTILE - 1) / PD_PTILE);  // + 15: tiles start at a multiple of 16 particles
+  plan->sparse = sparse;
+  plan->smem_bytes = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse).total;
+  return PD_OK;
+}
+
+template <int THREADS, bool DEBUG, bool SPARSE>
+static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
+  constexpr int CTAS = THREADS == 512 ? 2 : 1;
+  auto kern = pdk::pd_tower_kernel<THREADS, CTAS, DEBUG, SPARSE>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g_max_smem_optin) != cudaSuccess) return PD_ECUDA;
+  // persistent CTAs wait on one another through the look-back chain: the grid must be co-resident
+  int per_sm = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, THREADS, plan.smem_bytes) != cudaSuccess) return PD_ECUDA;
+  if (per_sm < 1) return PD_ECUDA;
+  if (per_sm > CTAS) per_sm = CTAS;
+  int grid = g_num_sms * per_sm;
+  if (grid > plan.n_tiles) grid = plan.n_tiles;
+  if (grid < 1) grid = 1;
+  kern<<<grid, THREADS, plan.smem_bytes, stream>>>(prm);
+  return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
+}
+
+// the two kernels of the chain, back to back on the stream: P (particles -> keys + tracks), then T (towers, EFlow)
+int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, void *stream) {
+  if (query_device() != PD_OK) return PD_ECUDA;
+  if (plan.smem_bytes > (size_t)g_max_smem_optin) return PD_ECUDA;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (prm.n_ptiles > 0) {
+    const int rc = pd_launch_particles(prm, debug, g_num_sms, g_max_smem_optin, stream);
+    if (rc != PD_OK) return rc;
+  }
+  if (plan.threads == 1024) {
+    if (plan.sparse) return PD_EINVAL;  // pd_plan never pairs the two
+    return debug ? launch_variant<1024, true, false>(prm, plan, st) : launch_variant<1024, false, false>(prm, plan, st);
+  }
+  if (plan.sparse) return debug ? launch_variant<512, true, true>(prm, plan, st) : launch_variant<512, false, true>(prm, plan, st);
+  return debug ? launch_variant<512, true, false>(prm, plan, st) : launch_variant<512, false, false>(prm, plan, st);
+}
