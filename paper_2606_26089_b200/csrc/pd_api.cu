@@ -34,13 +34,34 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 }  // namespace
 
-// header + look-back words of the two kernels, rounded up so that the keys behind them are 256-byte aligned
+// header + the two look-back chains of kernel T, rounded up so that what follows is 256-byte aligned
 static size_t ws_chain_bytes(const PdLaunchPlan &plan) {
-  const size_t b = kWsHeader + sizeof(unsigned long long) * ((size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1) + (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1));
+  const size_t b = kWsHeader + 2 * sizeof(unsigned long long) * (size_t)(plan.n_tiles > 0 ? plan.n_tiles : 1);
   return (b + 255) & ~size_t(255);
 }
-// the 16-bit key kernel P leaves per particle for kernel T
-static size_t ws_key_bytes(const PdLaunchPlan &plan) { return sizeof(unsigned short) * (size_t)PD_PTILE * (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1); }
+// What kernel P leaves for kernel T, per particle slot (n_ptiles * PD_PTILE slots): the 16-bit key, the accepted bit,
+// and the parked track records (segment index 1 B, charge 1 B, pid 4 B, six floats).  Each array 256-byte aligned.
+struct WsLayout {
+  size_t key, accmask, idx, q, pid, f[6], total;
+};
+static WsLayout ws_layout(const PdLaunchPlan &plan) {
+  const size_t slots = (size_t)PD_PTILE * (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1);
+  WsLayout l;
+  size_t o = ws_chain_bytes(plan);
+  auto take = [&](size_t bytes) {
+    size_t at = o;
+    o = (o + bytes + 255) & ~size_t(255);
+    return at;
+  };
+  l.key = take(2 * slots);
+  l.accmask = take(slots / 8);
+  l.idx = take(slots);
+  l.q = take(slots);
+  l.pid = take(4 * slots);
+  for (int k = 0; k < 6; ++k) l.f[k] = take(4 * slots);
+  l.total = o;
+  return l;
+}
 
 extern "C" {
 
@@ -92,7 +113,7 @@ int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_part
   if (!card || n_events < 0 || n_particles < 0) return PD_EINVAL;
   PdLaunchPlan plan;
   pd_plan(card, n_events, n_particles, &plan);
-  return (int64_t)(ws_chain_bytes(plan) + ws_key_bytes(plan));
+  return (int64_t)ws_layout(plan).total;
 }
 
 int pd_last_launch_count(void) { return t_launches; }
@@ -424,8 +445,16 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
   p.status_word = (int *)(ws + 4);
   p.ptile_counter = (unsigned int *)(ws + 8);
   p.chain = (unsigned long long *)(ws + kWsHeader);
-  p.chain_p = p.chain + (plan.n_tiles > 0 ? plan.n_tiles : 1);
-  p.key = (unsigned short *)(ws + ws_chain_bytes(plan));
+  p.chain_t = p.chain + (plan.n_tiles > 0 ? plan.n_tiles : 1);
+  {
+    const WsLayout wl = ws_layout(plan);
+    p.key = (unsigned short *)(ws + wl.key);
+    p.accmask = (unsigned int *)(ws + wl.accmask);
+    p.park_idx = ws + wl.idx;
+    p.park_q = (signed char *)(ws + wl.q);
+    p.park_pid = (int *)(ws + wl.pid);
+    for (int k = 0; k < 6; ++k) p.park_f[k] = (float *)(ws + wl.f[k]);
+  }
   p.n_ptiles = plan.n_ptiles;
   p.p_base = particle_base;
   {
@@ -436,7 +465,6 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
                           reinterpret_cast<uintptr_t>(ev->vy) | reinterpret_cast<uintptr_t>(ev->vz) | reinterpret_cast<uintptr_t>(ev->E);
     p.tma_ok = (all & 15u) == 0 ? 1 : 0;
   }
-  if (n == 0) PD_CUDA(cudaMemsetAsync(trk->offsets, 0, sizeof(int64_t) * (size_t)(ev->n_events + 1), st));  // kernel P has no tile
 
   rc = pd_launch_chain(p, plan, dbg != nullptr, cuda_stream);
   if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "kernel launch");

@@ -13,7 +13,8 @@ constexpr int PD_MAX_EFF = 31;         // rows of the efficiency table in a card
 constexpr int PD_MAX_EFF_EDGES = 8;    // distinct pT edges / distinct |eta| edges of the table
 constexpr int PD_MAX_EFF_CELLS = (PD_MAX_EFF_EDGES + 1) * (PD_MAX_EFF_EDGES + 1);
 constexpr int PD_MAX_TOWERS = (1 << 15) - 1;  // tower ids are packed into 15 bits on chip, 0x7fff = none
-constexpr int PD_PTILE = 1280;         // particles per tile of kernel P (pd_particles.cu): a multiple of 32, <= 2048
+constexpr int PD_PSEG = 160;           // particles per segment (one warp of kernel P): a multiple of 32, <= 255
+constexpr int PD_PTILE = 8 * PD_PSEG;         // particles per tile of kernel P (pd_particles.cu): a multiple of 32, <= 2048
 constexpr int PD_LUT_SHIFT = 19;       // eta-bin lookup: 16 cells per octave of |u|
 constexpr int PD_LUT_MIN_EXP = -8;     // |u| < 2^-8 shares one cell per side
 
@@ -126,7 +127,13 @@ struct PdParams {
   long long p_base;              // offsets[0]: first particle of the call in the arrays (0 for a public call)
   int n_ptiles;
   int tma_ok;                    // 1: every input array is 16-byte aligned (bulk copies), 0: plain loads
-  unsigned long long *chain_p;   // [n_ptiles] look-back words: accepted tracks
+  unsigned long long *chain_t;   // [n_tiles] look-back words of kernel T: tracks
+  // accepted tracks parked by kernel P, compacted within every segment of PD_PSEG consecutive particles
+  unsigned int *accmask;         // [n_ptiles * PD_PTILE / 32] accepted bits
+  unsigned char *park_idx;       // [n_ptiles * PD_PTILE] index of the track's particle within its segment
+  int *park_pid;
+  signed char *park_q;
+  float *park_f[6];              // pt, eta, phi, E, eta_out, phi_out
   unsigned int *ptile_counter;
   unsigned short *key;           // [n_ptiles * PD_PTILE] per particle: tower id | HCAL bit << 15, 0xffff = no deposit
 };

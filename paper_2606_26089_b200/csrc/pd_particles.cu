@@ -16,7 +16,9 @@
 // written to the workspace with one bulk store per tile, and the Track collection itself.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
+#include <cstdlib>
 
 #include "pd_internal.h"
 #include "pd_math.cuh"
@@ -36,17 +38,18 @@ static_assert(PT_TILE % 32 == 0 && PT_TILE <= 2048, "list entries keep the parti
 constexpr int PT_PER_WARP = PT_TILE / PT_WARPS;  // particles a warp owns: a multiple of 32
 constexpr int PT_ITERS = PT_PER_WARP / 32;
 static_assert(PT_PER_WARP % 32 == 0 && PT_PER_WARP <= 255, "a warp owns whole 32-particle rows; ranks fit 8 bits");
+constexpr int PT_WCAP = 1024;                               // event offsets of a tile kept on chip (more: looked up in global memory)
 constexpr size_t PO_F = 0;                                  // px, py, pz, vx, vy, vz: 6 x 4 B x TILE
 constexpr size_t PO_PID = PO_F + 6 * 4 * (size_t)PT_TILE;   // 4 B x TILE
 constexpr size_t PO_Q = PO_PID + 4 * (size_t)PT_TILE;       // 1 B x TILE
-constexpr size_t PO_EVK = PO_Q + (size_t)PT_TILE;           // 2 B x TILE: event of the particle (relative), then its key
-constexpr size_t PO_EST = PO_EVK + 2 * (size_t)PT_TILE;     // 2 B x TILE: local index of the first particle of its event
-constexpr size_t PO_LIST = PO_EST + 2 * (size_t)PT_TILE;    // 2 B x TILE: class lists (per warp: A | B | N), then tracks in order
+constexpr size_t PO_KEY = PO_Q + (size_t)PT_TILE;           // 2 B x TILE: the particle's key for the tower pass
+constexpr size_t PO_LIST = PO_KEY + 2 * (size_t)PT_TILE;    // 2 B x TILE: class lists (per warp: A | B | N), then its tracks in order
 constexpr size_t PO_MASK = PO_LIST + 2 * (size_t)PT_TILE;   // accepted bits
-constexpr size_t PO_PRE = PO_MASK + 4 * (size_t)PT_WORDS;   // their prefix per word (+ total)
-constexpr size_t PO_MISC = (PO_PRE + 4 * (size_t)(PT_WORDS + 1) + 15) & ~size_t(15);
-constexpr size_t PO_TABLES = PO_MISC + 8 * 16;
-static_assert(PO_PID % 16 == 0 && PO_Q % 16 == 0 && PO_EVK % 16 == 0 && PO_LIST % 16 == 0, "bulk copies need 16-byte aligned slots");
+constexpr size_t PO_PRE = PO_MASK + 4 * (size_t)PT_WORDS;   // their prefix per word, within the owning warp
+constexpr size_t PO_WOFF = (PO_PRE + 4 * (size_t)PT_WORDS + 15) & ~size_t(15);  // event offsets of the tile, relative to its start
+constexpr size_t PO_MISC = PO_WOFF + 4 * (size_t)PT_WCAP;
+constexpr size_t PO_TABLES = PO_MISC + 8 * 24;
+static_assert(PO_PID % 16 == 0 && PO_Q % 16 == 0 && PO_KEY % 16 == 0 && PO_LIST % 16 == 0, "bulk copies need 16-byte aligned slots");
 
 struct PTables {
   size_t tb, binrec, lut, total;
@@ -93,16 +96,14 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
   float *s_vx = s_pz + PT_TILE, *s_vy = s_vx + PT_TILE, *s_vz = s_vy + PT_TILE;
   int *s_pid = (int *)(smem + PO_PID);
   signed char *s_q = (signed char *)(smem + PO_Q);
-  unsigned short *s_evk = (unsigned short *)(smem + PO_EVK);
-  unsigned short *s_est = (unsigned short *)(smem + PO_EST);
+  unsigned short *s_key = (unsigned short *)(smem + PO_KEY);
   unsigned short *s_list = (unsigned short *)(smem + PO_LIST);
   uint32_t *s_accmask = (uint32_t *)(smem + PO_MASK);
-  uint32_t *s_accpre = (uint32_t *)(smem + PO_PRE);
+  int *s_woff = (int *)(smem + PO_WOFF);
   unsigned long long *s_misc = (unsigned long long *)(smem + PO_MISC);
   uint64_t *s_bar = (uint64_t *)(s_misc + 0);
-  int *s_cnt = (int *)(s_misc + 1);               // [0] accepted tracks so far, [1] warps done with their class A, [2] tile
-  long long *s_win = (long long *)(s_misc + 3);   // [0] e_lo, [1] offsets[e_lo], [2] first event with offset >= s, [3] first with offset >= s + T
-  long long *s_base = (long long *)(s_misc + 8);  // [0] track prefix of the tile
+  int *s_cnt = (int *)(s_misc + 1);               // [2] this tile
+  long long *s_win = (long long *)(s_misc + 3);   // [0] e_lo, [1] e_hi
   const PTables TL = make_ptables(nb, 2 * sc.lut_side);
   float *s_tb = (float *)(smem + TL.tb);
   float4 *s_rec = (float4 *)(smem + TL.binrec);
@@ -118,6 +119,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
   if (tid == 0) {
     mbar_init(s_bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    s_cnt[2] = (int)atomicAdd(prm.ptile_counter, 1u);
   }
   uint32_t phase = 0;
   // the particles of the call are [p_base, p_end) of the arrays (p_base = offsets[0]: 0 for a public call, the chunk's
@@ -125,15 +127,10 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
   // every tile start is 16-byte aligned in all arrays; the (< 16) particles in front of p_base are skipped
   const long long p_base = prm.p_base, p_al = p_base & ~15ll, n_all = p_base + prm.n_particles;
   const int wbase = wid * PT_PER_WARP;  // this warp owns particles [wbase, wbase + PT_PER_WARP) of every tile
+  const int wword = wid * PT_ITERS;     // ... and these words of the accepted mask
 
   for (;;) {
-    __syncthreads();  // previous tile fully done with shared memory (tables staged, mbarrier initialised)
-    if (tid == 0) {
-      s_cnt[2] = (int)atomicAdd(prm.ptile_counter, 1u);
-      s_cnt[0] = 0, s_cnt[1] = 0;
-    }
-    for (int k = tid; k < PT_WORDS; k += PT_THREADS) s_accmask[k] = 0u;
-    __syncthreads();
+    __syncthreads();  // (A) previous tile fully done with shared memory; this tile's index is in s_cnt[2]
     const int tile = s_cnt[2];
     if (tile >= prm.n_ptiles) break;
     const long long s0 = p_al + (long long)tile * PT_TILE;
@@ -166,33 +163,24 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     }
 
     // ---- the events of the tile (while the copies are in flight).  offsets[0..n_events] is non-decreasing:
-    // e_lo = the event of particle s_eff; [w2, w3) = the events whose first particle (or empty position) lies in the
-    // tile: this tile writes their track offsets.
+    // e_lo = the event of particle s_eff, e_hi = the last event with a particle in the tile.  The offsets of
+    // e_lo .. e_hi + 1, relative to the tile, go to shared memory: class A looks its event up there.
     if (wid == 0) {
       const long long ne1 = prm.n_events + 1;
-      const long long ub = warp_lower_bound(prm.offsets, ne1, s_eff + 1);  // entries <= s_eff
-      const long long e_lo = ub - 1;
-      const long long o_lo = __ldg(prm.offsets + e_lo);
-      const long long w2 = o_lo == s_eff ? warp_lower_bound(prm.offsets, ne1, s_eff) : ub;
+      const long long e_lo = warp_lower_bound(prm.offsets, ne1, s_eff + 1) - 1;  // entries <= s_eff, minus one
       const long long w3 = s0 + PT_TILE >= n_all ? ne1 : warp_lower_bound(prm.offsets, ne1, s0 + PT_TILE);
-      if (lane == 0) s_win[0] = e_lo, s_win[1] = o_lo, s_win[2] = w2, s_win[3] = w3;
+      const long long e_hi = min(w3, prm.n_events) - 1;
+      if (lane == 0) s_win[0] = e_lo, s_win[1] = e_hi;
+      if (e_hi - e_lo + 2 <= PT_WCAP)
+        for (int k = lane; k <= (int)(e_hi - e_lo) + 1; k += 32) s_woff[k] = (int)(__ldg(prm.offsets + e_lo + k) - s0);
     }
-    __syncthreads();
-    const long long e_lo = s_win[0];
-    const long long e_hi = min(s_win[3], prm.n_events) - 1;  // last event with a particle in the tile (or an empty one before the end)
-    const bool wide = e_hi - e_lo >= 0xffff;                  // only with > 65,000 empty events inside one tile
-    if (!wide) {
-      // warp per event, lanes over its particles
-      for (long long e = e_lo + wid; e <= e_hi; e += PT_WARPS) {
-        const long long a = __ldg(prm.offsets + e) - s0, b = __ldg(prm.offsets + e + 1) - s0;
-        const int j0 = (int)max(a, 0ll), j1 = (int)min(b, (long long)n);
-        const unsigned short st = a >= 0 ? (unsigned short)a : (unsigned short)PT_NONE;
-        for (int j = j0 + lane; j < j1; j += 32) s_evk[j] = (unsigned short)(e - e_lo), s_est[j] = st;
-      }
-    }
-    __syncthreads();  // events filled in (the partition overwrites the entry of a dropped particle); plain loads done
+    // this warp's words of the accepted mask
+    if (lane < PT_ITERS) s_accmask[wword + lane] = 0u;
+    __syncthreads();  // (B) events in place; plain loads done
     if (full) mbar_wait(s_bar, phase), phase ^= 1u;
-    const uint32_t head_shift = (uint32_t)(s0 - s_win[1]);  // index within its event of particle s0
+    const long long e_lo = s_win[0], e_hi = s_win[1];
+    const int n_win = (int)min(e_hi - e_lo + 1, (long long)PT_WCAP);  // events of the tile
+    const bool wide = e_hi - e_lo + 2 > PT_WCAP;                     // only with > 1,000 events in one tile (empty ones)
 
     // ---- partition of the warp's own particles by class (S0): A charged with efficiency > 0, B other charged,
     // N neutral; dropped particles are finished here.  No other warp is involved: ballots and register counts.
@@ -203,12 +191,12 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
       const int i = wbase + 32 * k + lane;
       int cls = 3;  // 0 A, 1 B, 2 N, 3 none
       int row = 0;
-      if (i < n && i < lo_skip) s_evk[i] = (unsigned short)PT_NONE;
+      if (i < n && i < lo_skip) s_key[i] = (unsigned short)PT_NONE;
       if (i < n && i >= lo_skip) {
         const int q = (int)s_q[i];
         const float px = s_px[i], py = s_py[i];
         if (vertex_dropped(sc, px, py, s_vx[i], s_vy[i], s_vz[i])) {
-          s_evk[i] = (unsigned short)PT_NONE;
+          s_key[i] = (unsigned short)PT_NONE;
           if (DEBUG) {
             const long long g = s0 + i;
             const float nanv = __int_as_float(0x7fc00000);
@@ -245,8 +233,6 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     const int n_work = nA + nB + nN;
 
     // ---- S1-S4 on the warp's lists A | B | N: rows of one class (the rows at the two boundaries are mixed)
-    int n_acc = 0;
-    bool signalled = false;
 #pragma unroll 1
     for (int k = 0; k < PT_ITERS; ++k) {
       const int v = 32 * k + lane;
@@ -273,15 +259,20 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
         bool accepted = false;
         float pt_s = 0.f;
         if (cls == 0 && live) {
-          // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0
+          // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0.
+          // The event: the last one whose offset is <= i (bisection of the tile's offsets; one step on big events)
           long long ev;
           uint32_t pidx;
           if (!wide) {
-            const unsigned er = s_evk[i], st = s_est[i];
-            ev = e_lo + er;
-            pidx = st == PT_NONE ? head_shift + (uint32_t)i : (uint32_t)i - st;
+            int lo = 0, hi = n_win - 1;
+            while (lo < hi) {
+              const int mid = (lo + hi + 1) >> 1;
+              if (s_woff[mid] <= i) lo = mid;
+              else hi = mid - 1;
+            }
+            ev = e_lo + lo, pidx = (uint32_t)(i - s_woff[lo]);
           } else {
-            long long lo = e_lo, hi = e_hi;  // last event with offsets[e] <= s0 + i
+            long long lo = e_lo, hi = e_hi;
             const long long g = s0 + i;
             while (lo < hi) {
               const long long mid = (lo + hi + 1) >> 1;
@@ -304,8 +295,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
           }
         }
         // what the tower pass needs: tower | HCAL bit, or "no deposit"
-        s_evk[i] = (tower >= 0 && !to_none) ? (unsigned short)((unsigned)tower | (to_ecal ? 0u : 0x8000u)) : (unsigned short)PT_NONE;
-        n_acc += accepted ? 1 : 0;
+        s_key[i] = (tower >= 0 && !to_none) ? (unsigned short)((unsigned)tower | (to_ecal ? 0u : 0x8000u)) : (unsigned short)PT_NONE;
         if (DEBUG) {
           const long long g = s0 + i;
           const int row = (int)(ent >> 11);
@@ -318,76 +308,39 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
           if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = pt_s;
         }
       }
-      // The tile's number of accepted tracks is known as soon as every warp is through its class A: the last warp to
-      // get there PUBLISHES it on the look-back chain, a good part of the tile before anyone needs the prefix.
-      if (!signalled && 32 * (k + 1) >= nA) {
-        signalled = true;
-        const int mine = (int)__reduce_add_sync(0xffffffffu, (unsigned)n_acc);
-        if (lane == 0) {
-          atomicAdd(&s_cnt[0], mine);
-          __threadfence_block();
-          if (atomicAdd(&s_cnt[1], 1) == PT_WARPS - 1) chain_publish(prm.chain_p, tile, (unsigned long long)atomicAdd(&s_cnt[0], 0));
-        }
+    }
+    // ---- the warp's accepted tracks in particle order (its own mask words: nobody else sets their bits), parked
+    // SEGMENT by segment in the workspace: the tracks of the PT_PER_WARP particles this warp owns, compacted, at the
+    // segment's start.  Kernel T, which knows where an event's tracks go, moves them into the Track collection.
+    __syncwarp();
+    {
+      const long long seg0 = (s0 - p_al) + wbase;  // first slot of the segment in the parking arrays
+      int run = 0;
+#pragma unroll
+      for (int k = 0; k < PT_ITERS; ++k) {
+        const uint32_t m = s_accmask[wword + k];
+        if ((m >> lane) & 1u) s_list[wbase + run + __popc(m & lt_mask)] = (unsigned short)(wbase + 32 * k + lane);
+        run += __popc(m);
+      }
+      if (lane < PT_ITERS) prm.accmask[(seg0 >> 5) + lane] = s_accmask[wword + lane];
+      __syncwarp();
+      for (int r = lane; r < run; r += 32) {
+        const int i = s_list[wbase + r];
+        const long long g = seg0 + r;
+        prm.park_idx[g] = (unsigned char)(i - wbase);
+        prm.park_pid[g] = s_pid[i];
+        prm.park_q[g] = s_q[i];
+        prm.park_f[0][g] = s_px[i], prm.park_f[1][g] = s_py[i], prm.park_f[2][g] = s_pz[i];
+        prm.park_f[3][g] = s_vx[i], prm.park_f[4][g] = s_vy[i], prm.park_f[5][g] = s_vz[i];
       }
     }
-    fence_async_smem();  // the keys go out with a bulk store (async proxy)
-    __syncthreads();
-
-    // ---- accepted tracks in particle order: prefix over the mask words, the ordered list
-    if (wid == 0) {
-      // PT_WORDS <= 64 words: two per lane
-      const int k0 = 2 * lane, k1 = 2 * lane + 1;
-      const unsigned c0 = k0 < PT_WORDS ? (unsigned)__popc(s_accmask[k0]) : 0u, c1 = k1 < PT_WORDS ? (unsigned)__popc(s_accmask[k1]) : 0u;
-      const unsigned incl = warp_incl_scan(c0 + c1);
-      const unsigned excl = incl - (c0 + c1);
-      if (k0 < PT_WORDS) s_accpre[k0] = excl;
-      if (k1 < PT_WORDS) s_accpre[k1] = excl + c0;
-      const unsigned total = __shfl_sync(0xffffffffu, incl, 31);
-      if (lane == 0) {
-        s_accpre[PT_WORDS] = total;
-        // the keys of a full tile leave with one bulk store (the ragged last tile: plain stores below)
-        if (full) {
-          bulk_s2g(prm.key + (s0 - p_al), s_evk, 2u * PT_TILE);
-          bulk_commit();
-        }
-      }
+    // the warp's keys (what the tower pass needs): PT_PER_WARP 16-bit words, stored as 32-bit ones
+    {
+      const uint32_t *src = (const uint32_t *)(s_key + wbase);
+      uint32_t *dst = (uint32_t *)(prm.key + (s0 - p_al) + wbase);
+      for (int j = lane; j < PT_PER_WARP / 2; j += 32) dst[j] = src[j];
     }
-    __syncthreads();
-    const int n_trk = (int)s_accpre[PT_WORDS];
-    for (int i = tid; i < n; i += PT_THREADS) {
-      const uint32_t m = s_accmask[i >> 5];
-      if ((m >> (i & 31)) & 1u) s_list[s_accpre[i >> 5] + __popc(m & ((1u << (i & 31)) - 1u))] = (unsigned short)i;
-    }
-    if (!full)
-      for (int i = tid; i < n; i += PT_THREADS) prm.key[s0 - p_al + i] = s_evk[i];
-    if (wid == 0) {
-      const unsigned long long ex = chain_resolve<8>(prm.chain_p, tile, (unsigned long long)n_trk);
-      if (lane == 0) s_base[0] = (long long)ex;
-    }
-    __syncthreads();
-    const long long base = s_base[0];
-
-    // ---- S8 for tracks: the collection in its final place, and the track offsets of the events that start here
-    for (int r = tid; r < n_trk; r += PT_THREADS) {
-      const int i = s_list[r];
-      const unsigned g = (unsigned)base + (unsigned)r;  // all output indices fit 32 bits (n_particles < 2^30)
-      prm.trk_src[g] = (int)(s0 + i);
-      prm.trk_pid[g] = s_pid[i];
-      prm.trk_charge[g] = s_q[i];
-      prm.trk_pt[g] = s_px[i];
-      prm.trk_eta[g] = s_py[i];
-      prm.trk_phi[g] = s_pz[i];
-      prm.trk_E[g] = s_vx[i];
-      prm.trk_eta_out[g] = s_vy[i];
-      prm.trk_phi_out[g] = s_vz[i];
-    }
-    for (long long e = s_win[2] + tid; e < s_win[3]; e += PT_THREADS) {
-      const int j = (int)(__ldg(prm.offsets + e) - s0);  // 0..n
-      const int w = j >> 5;
-      const unsigned below = j >= n ? (unsigned)n_trk : s_accpre[w] + (unsigned)__popc(s_accmask[w] & ((1u << (j & 31)) - 1u));
-      prm.trk_offsets[e] = base + below;
-    }
-    if (full && tid == 0) bulk_wait_read0();  // the key store has read its shared-memory source
+    if (tid == 0) s_cnt[2] = (int)atomicAdd(prm.ptile_counter, 1u);  // the CTA's next tile
     fence_async_smem();  // the parked records were generic-proxy writes to slots the next tile's bulk copies overwrite
   }
 }
@@ -405,6 +358,7 @@ int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_sm
   int per_sm = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, pdk::PT_THREADS, smem) != cudaSuccess) return PD_ECUDA;
   if (per_sm < 1) return PD_ECUDA;
+  if (const char *e = getenv("PD_P_PER_SM")) per_sm = std::min(per_sm, atoi(e));  // experiment
   int grid = num_sms * per_sm;
   if (grid > prm.n_ptiles) grid = prm.n_ptiles;
   if (grid < 1) grid = 1;

@@ -19,6 +19,7 @@
 // of the order in which the list was built), and the only atomics are integer (bitmap OR, list exchange, counters).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -46,6 +47,7 @@ struct Layout {
   size_t offset, w, eta_c, inv_cosh, binlut;     // card tables (what pass O needs)
   size_t off32, ntrk, ntow, nph, nnh;            // per-event arrays [G+1]
   size_t misc;                                   // scratch words
+  size_t seg;                                    // track segments of the tile [3][64]
   size_t cnt;                                    // pass W warp counts -> prefixes [2][256]
   size_t bitmap, gprefix;                        // per event: tower bits, group prefix
   size_t l2p, pool;                              // sparse mode (see make_layout)
@@ -76,6 +78,7 @@ __host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int word
   l.nph = take(4 * (G + 1));
   l.nnh = take(4 * (G + 1));
   l.misc = take(8 * 64);
+  l.seg = take(4 * 3 * 64);
   l.cnt = take(4 * 2 * 256);
   const int gpe = words_per_event / 4, l2w = (gpe + 31) / 32;
   l.l2p = 0, l.pool = 0;
@@ -166,7 +169,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
   float *s_inv_cosh = (float *)(smem + L.inv_cosh);
   unsigned short *s_binlut = (unsigned short *)(smem + L.binlut);
   int *s_off32 = (int *)(smem + L.off32);
-  int *s_ntrk = (int *)(smem + L.ntrk);  // tracks of the tile before event e (from the Track offsets kernel P wrote)
+  int *s_ntrk = (int *)(smem + L.ntrk);  // tracks of the tile before event e
   int *s_ntow = (int *)(smem + L.ntow);
   int *s_nph = (int *)(smem + L.nph);
   int *s_nnh = (int *)(smem + L.nnh);
@@ -185,6 +188,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
   float *s_stg = (float *)(smem + L.stg);   // per slot after pass W: Eem''  (neutral-hadron energy goes to s_res[head])
   unsigned char *s_ev = smem + L.ev;
   uint64_t *s_bar = (uint64_t *)(s_misc + 4);
+  // kernel P parked the accepted tracks compacted within SEGMENTS of PD_PSEG particles; per segment that overlaps the
+  // tile: rank of the tile's first track in the segment, number of the tile's tracks in it, their exclusive prefix
+  int *s_sega = (int *)(smem + L.seg), *s_segc = s_sega + 64, *s_segp = s_segc + 64;
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
@@ -246,12 +252,23 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
     }
     for (int i = nbE - shE + tid; i < n; i += THREADS) s_Ev[i] = __ldg(prm.E + p0 + i);
     for (int i = nbK - shK + tid; i < n; i += THREADS) ((unsigned short *)s_stg)[shK + i] = __ldg(prm.key + (p0 - p_al) + i);
-    const long long t0 = prm.trk_offsets[e0];  // first track of the tile (kernel P wrote the Track collection)
-    const int n_trk = overflow ? 0 : (int)(prm.trk_offsets[e0 + ne] - t0);
     for (int e = tid; e <= ne; e += THREADS) {
       s_off32[e] = overflow ? 0 : (int)(prm.offsets[e0 + e] - p0);
-      s_ntrk[e] = overflow ? 0 : (int)(prm.trk_offsets[e0 + e] - t0);
-      s_ntow[e] = 0, s_nph[e] = 0, s_nnh[e] = 0;
+      s_ntrk[e] = 0, s_ntow[e] = 0, s_nph[e] = 0, s_nnh[e] = 0;
+    }
+    // the tile's tracks, segment by segment (warp per segment): from the accepted bits kernel P left
+    const long long q0 = p0 - p_al;  // the tile's first particle in the parking arrays
+    const long long gseg_lo = q0 / PD_PSEG;
+    const int n_seg = n > 0 ? (int)((q0 + n - 1) / PD_PSEG - gseg_lo) + 1 : 0;
+    for (int k = wid; k < n_seg; k += W) {
+      const long long gs = gseg_lo + k;
+      const uint32_t w = lane < PD_PSEG / 32 ? __ldg(prm.accmask + gs * (PD_PSEG / 32) + lane) : 0u;
+      const int lo = (int)max(q0 - gs * PD_PSEG, 0ll), hi = (int)min(q0 + n - gs * PD_PSEG, (long long)PD_PSEG);
+      const int nlo = min(max(lo - 32 * lane, 0), 32), nhi = min(max(hi - 32 * lane, 0), 32);
+      const uint32_t mlo = nlo == 32 ? 0xffffffffu : (1u << nlo) - 1u, mhi = nhi == 32 ? 0xffffffffu : (1u << nhi) - 1u;
+      const int a = (int)__reduce_add_sync(0xffffffffu, (unsigned)__popc(w & mlo));
+      const int b = (int)__reduce_add_sync(0xffffffffu, (unsigned)__popc(w & mhi));
+      if (lane == 0) s_sega[k] = a, s_segc[k] = b - a;
     }
     const int NG = ne * gpe;  // 128-tower bitmap groups of the tile
     const int NW = ne * l2w;  // sparse mode: words of the group bitmaps
@@ -261,6 +278,20 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
       for (int k = tid; k < NW; k += THREADS) s_bitmap[k] = 0u;
     }
     __syncthreads();
+    if (wid == 0) {
+      // exclusive prefix of the segments' track counts (<= 64 segments: two per lane); the tile's total goes on chain T
+      // at once: nobody will ever wait for it
+      const int c0 = 2 * lane < n_seg ? s_segc[2 * lane] : 0, c1 = 2 * lane + 1 < n_seg ? s_segc[2 * lane + 1] : 0;
+      const int incl = (int)warp_incl_scan((unsigned)(c0 + c1));
+      if (2 * lane < n_seg) s_segp[2 * lane] = incl - c0 - c1;
+      if (2 * lane + 1 < n_seg) s_segp[2 * lane + 1] = incl - c1;
+      const int total = __shfl_sync(0xffffffffu, incl, 31);
+      if (lane == 0) {
+        s_misc[5] = (unsigned long long)total;
+        chain_publish(prm.chain_t, tile, (unsigned long long)total);
+        if (!multi) s_ntrk[1] = total;
+      }
+    }
     if (multi) {
       // event index of every particle of the tile: warp per event, lanes over its particles
       for (int e = wid; e < ne; e += W)
@@ -304,10 +335,16 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
       const unsigned incl = warp_incl_scan(cnt_g);
       if (lane == 31) s_wtot[wid] = incl;
       // the tile's accepted tracks: their energy goes to their particle (pass W subtracts it from the tower)
-      for (int t = tid; t < n_trk; t += THREADS) {
-        const int i = (int)((long long)__ldg(prm.trk_src + t0 + t) - p0);
-        s_Et[i] = __ldg(prm.trk_E + t0 + t);
-        s_res[i] |= RES_ACC;
+      for (int k = wid; k < n_seg; k += W) {
+        const long long gs = (gseg_lo + k) * PD_PSEG;
+        const int a = s_sega[k], c = s_segc[k];
+        for (int r = lane; r < c; r += 32) {
+          const long long g = gs + a + r;
+          const int i = (int)(gs + (long long)__ldg(prm.park_idx + g) - q0);
+          s_Et[i] = __ldg(prm.park_f[3] + g);
+          s_res[i] |= RES_ACC;
+          if (multi) atomicAdd(&s_ntrk[(int)s_ev[i]], 1);
+        }
       }
       __syncthreads();
       unsigned excl_w, tot;
@@ -479,13 +516,46 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
       const int n_tow = (int)(ta & 0xffffu), n_ph = (int)(ta >> 16), n_nh = (int)tb;
       if (!multi && lane == 0) s_ntow[0] = 0, s_ntow[1] = n_tow, s_nph[0] = 0, s_nph[1] = n_ph, s_nnh[0] = 0, s_nnh[1] = n_nh;
       const unsigned long long agg = (unsigned long long)n_tow | ((unsigned long long)(n_ph + n_nh) << 31);
-      if (lane == 0) chain_publish(prm.chain, tile, agg);  // successors add it up without waiting for this tile's prefix
-      const unsigned long long ex = chain_resolve<8>(prm.chain, tile, agg);
-      if (lane == 0) s_misc[2] = ex;
+      if (lane == 0) chain_publish(prm.chain, tile, agg), s_misc[3] = agg;  // successors add it up without waiting for this tile's prefix
+    } else if (wid == 1) {
+      // the track prefix: every predecessor published its count when it started its tile, so this never waits
+      if (multi) event_scan(s_ntrk, ne);
+      const unsigned long long ex = chain_resolve<8>(prm.chain_t, tile, s_misc[5]);
+      if (lane == 0) s_misc[1] = ex;
     } else if (multi) {
       if (wid == 2) event_scan(s_ntow, ne);
       else if (wid == 3) event_scan(s_nph, ne);
       else if (wid == 4) event_scan(s_nnh, ne);
+    }
+    __syncthreads();
+    const long long t0 = (long long)s_misc[1];  // first track of the tile
+    // Warp 0 resolves the tower / neutral prefix (the one place a CTA waits for its predecessors); meanwhile the other
+    // warps move the tile's tracks from where kernel P parked them into the Track collection, which needs the track
+    // prefix only.
+    if (wid == 0) {
+      const unsigned long long ex = chain_resolve<8>(prm.chain, tile, s_misc[3]);
+      if (lane == 0) s_misc[2] = ex;
+    } else {
+      for (int e = tid - 32; e < ne; e += THREADS - 32) prm.trk_offsets[e0 + e + 1] = t0 + s_ntrk[e + 1];
+      if (tile == 0 && tid == 32) prm.trk_offsets[0] = 0;
+      for (int k = wid - 1; k < n_seg; k += W - 1) {
+        const long long gs = (gseg_lo + k) * PD_PSEG;
+        const int a = s_sega[k], c = s_segc[k];
+        const unsigned ob = (unsigned)t0 + (unsigned)s_segp[k];
+        for (int r = lane; r < c; r += 32) {
+          const long long g = gs + a + r;
+          const unsigned o = ob + (unsigned)r;
+          prm.trk_src[o] = (int)(p_al + gs + (long long)__ldg(prm.park_idx + g));
+          prm.trk_pid[o] = __ldg(prm.park_pid + g);
+          prm.trk_charge[o] = __ldg(prm.park_q + g);
+          prm.trk_pt[o] = __ldg(prm.park_f[0] + g);
+          prm.trk_eta[o] = __ldg(prm.park_f[1] + g);
+          prm.trk_phi[o] = __ldg(prm.park_f[2] + g);
+          prm.trk_E[o] = __ldg(prm.park_f[3] + g);
+          prm.trk_eta_out[o] = __ldg(prm.park_f[4] + g);
+          prm.trk_phi_out[o] = __ldg(prm.park_f[5] + g);
+        }
+      }
     }
     __syncthreads();
     const long long base_tow = (long long)(s_misc[2] & FIELD_MASK);
@@ -497,21 +567,24 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
       prm.efl_offsets[e0 + e + 1] = base_efl + s_ntrk[e + 1] + s_nph[e + 1] + s_nnh[e + 1];
     }
     if (tile == 0 && tid == 0) prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
-    // the EFlow entries of the tracks: copied from the Track collection (coalesced reads, L2 hits)
-    for (int s = tid; s < n_trk; s += THREADS) {
-      const long long g = t0 + s;
-      const int src = __ldg(prm.trk_src + g);
-      const int pid = __ldg(prm.trk_pid + g);
-      const float pt = __ldg(prm.trk_pt + g), eta = __ldg(prm.trk_eta + g), phi = __ldg(prm.trk_phi + g), Et = __ldg(prm.trk_E + g);
-      const int e = multi ? (int)s_ev[(int)((long long)src - p0)] : 0;
-      const unsigned at = (unsigned)base_efl + (unsigned)(s + s_nph[e] + s_nnh[e]);
-      const int apid = pid < 0 ? -pid : pid;
-      prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
-      prm.efl_src[at] = src;
-      prm.efl_pt[at] = pt;
-      prm.efl_eta[at] = eta;
-      prm.efl_phi[at] = phi;
-      prm.efl_E[at] = Et;
+    // the EFlow entries of the tracks, from the parked records (L2 hits)
+    for (int k = wid; k < n_seg; k += W) {
+      const long long gs = (gseg_lo + k) * PD_PSEG;
+      const int a = s_sega[k], c = s_segc[k], sp = s_segp[k];
+      for (int r = lane; r < c; r += 32) {
+        const long long g = gs + a + r;
+        const int il = (int)(gs + (long long)__ldg(prm.park_idx + g) - q0);
+        const int pid = __ldg(prm.park_pid + g);
+        const int e = multi ? (int)s_ev[il] : 0;
+        const unsigned at = (unsigned)base_efl + (unsigned)(sp + r + s_nph[e] + s_nnh[e]);
+        const int apid = pid < 0 ? -pid : pid;
+        prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
+        prm.efl_src[at] = (int)(p0 + il);
+        prm.efl_pt[at] = __ldg(prm.park_f[0] + g);
+        prm.efl_eta[at] = __ldg(prm.park_f[1] + g);
+        prm.efl_phi[at] = __ldg(prm.park_f[2] + g);
+        prm.efl_E[at] = __ldg(prm.park_f[3] + g);
+      }
     }
     for (int it = 0; it < n_it; ++it) {
       const int d = it * THREADS + tid;
@@ -656,6 +729,7 @@ static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStr
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, THREADS, plan.smem_bytes) != cudaSuccess) return PD_ECUDA;
   if (per_sm < 1) return PD_ECUDA;
   if (per_sm > CTAS) per_sm = CTAS;
+  if (const char *e = getenv("PD_T_PER_SM")) per_sm = std::min(per_sm, atoi(e));  // experiment
   int grid = g_num_sms * per_sm;
   if (grid > plan.n_tiles) grid = plan.n_tiles;
   if (grid < 1) grid = 1;
