@@ -42,7 +42,7 @@ static size_t ws_chain_bytes(const PdLaunchPlan &plan) {
 // What kernel P leaves for kernel T, per particle slot (n_ptiles * PD_PTILE slots): the 16-bit key, the accepted bit,
 // and the parked track records (segment index 1 B, charge 1 B, pid 4 B, six floats).  Each array 256-byte aligned.
 struct WsLayout {
-  size_t key, accmask, idx, q, pid, f[6], total;
+  size_t tile_ev, key, accmask, idx, q, pid, f[6], total;
 };
 static WsLayout ws_layout(const PdLaunchPlan &plan) {
   const size_t slots = (size_t)PD_PTILE * (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1);
@@ -53,6 +53,7 @@ static WsLayout ws_layout(const PdLaunchPlan &plan) {
     o = (o + bytes + 255) & ~size_t(255);
     return at;
   };
+  l.tile_ev = take(8 * ((size_t)plan.n_ptiles + 1));
   l.key = take(2 * slots);
   l.accmask = take(slots / 8);
   l.idx = take(slots);
@@ -440,6 +441,7 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
   p.n_tiles = plan.n_tiles;
   p.capacity = plan.capacity;
   p.sparse = plan.sparse;
+  p.lay = plan.lay;
   unsigned char *ws = (unsigned char *)workspace;
   p.tile_counter = (unsigned int *)ws;
   p.status_word = (int *)(ws + 4);
@@ -448,6 +450,7 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
   p.chain_t = p.chain + (plan.n_tiles > 0 ? plan.n_tiles : 1);
   {
     const WsLayout wl = ws_layout(plan);
+    p.tile_ev = (int *)(ws + wl.tile_ev);
     p.key = (unsigned short *)(ws + wl.key);
     p.accmask = (unsigned int *)(ws + wl.accmask);
     p.park_idx = ws + wl.idx;
@@ -468,7 +471,7 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
 
   rc = pd_launch_chain(p, plan, dbg != nullptr, cuda_stream);
   if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "kernel launch");
-  t_launches = n > 0 ? 2 : 1;
+  t_launches = n > 0 ? 3 : 1;
   return PD_OK;
 }
 

@@ -13,7 +13,7 @@ constexpr int PD_MAX_EFF = 31;         // rows of the efficiency table in a card
 constexpr int PD_MAX_EFF_EDGES = 8;    // distinct pT edges / distinct |eta| edges of the table
 constexpr int PD_MAX_EFF_CELLS = (PD_MAX_EFF_EDGES + 1) * (PD_MAX_EFF_EDGES + 1);
 constexpr int PD_MAX_TOWERS = (1 << 15) - 1;  // tower ids are packed into 15 bits on chip, 0x7fff = none
-constexpr int PD_PSEG = 160;           // particles per segment (one warp of kernel P): a multiple of 32, <= 255
+constexpr int PD_PSEG = 192;           // particles per segment (one warp of kernel P): a multiple of 32, <= 255
 constexpr int PD_PTILE = 8 * PD_PSEG;         // particles per tile of kernel P (pd_particles.cu): a multiple of 32, <= 2048
 constexpr int PD_LUT_SHIFT = 19;       // eta-bin lookup: 16 cells per octave of |u|
 constexpr int PD_LUT_MIN_EXP = -8;     // |u| < 2^-8 shares one cell per side
@@ -80,6 +80,19 @@ struct PdPhiloxKeys {
   uint32_t k0[10], k1[10];
 };
 
+// Shared-memory carve-up of kernel T (byte offsets; pd_towers.cu make_layout)
+struct PdTLayout {
+  uint32_t offset, w, eta_c, inv_cosh, binlut;  // card tables (what pass O needs)
+  uint32_t off32, ntrk, ntow, nph, nnh;         // per-event arrays [G+1]
+  uint32_t misc;                                // scratch words
+  uint32_t seg;                                 // track segments of the tile [3][64]
+  uint32_t cnt;                                 // pass W warp counts -> prefixes [2][256]
+  uint32_t bitmap, gprefix;                     // per event: tower bits, group prefix
+  uint32_t l2p, pool;                           // sparse mode
+  uint32_t res, Ev, Et, head, stg, ev;          // per particle / per slot
+  uint32_t total;
+};
+
 // Kernel parameters (passed by value).
 struct PdParams {
   PdCardScalars sc;
@@ -120,6 +133,7 @@ struct PdParams {
   int n_tiles;
   int capacity;          // C: particles a tile may hold on chip
   int sparse;            // 1: two-level tower bitmap (large grids, small events), see make_layout
+  PdTLayout lay;         // shared-memory carve-up of kernel T
   unsigned long long *chain;  // [n_tiles] look-back words of kernel T: towers | neutrals
   unsigned int *tile_counter;
   int *status_word;
@@ -135,6 +149,7 @@ struct PdParams {
   signed char *park_q;
   float *park_f[6];              // pt, eta, phi, E, eta_out, phi_out
   unsigned int *ptile_counter;
+  int *tile_ev;                  // [n_ptiles + 1][2] per tile boundary: first event with offset >= it, last with offset <= it
   unsigned short *key;           // [n_ptiles * PD_PTILE] per particle: tower id | HCAL bit << 15, 0xffff = no deposit
 };
 
@@ -151,6 +166,7 @@ struct PdLaunchPlan {
   int n_ptiles;      // tiles of kernel P
   int sparse;        // two-level tower bitmap
   size_t smem_bytes;
+  PdTLayout lay;
 };
 int pd_plan_set_tile_events(int g);
 int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);

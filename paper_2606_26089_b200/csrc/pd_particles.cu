@@ -38,7 +38,7 @@ static_assert(PT_TILE % 32 == 0 && PT_TILE <= 2048, "list entries keep the parti
 constexpr int PT_PER_WARP = PT_TILE / PT_WARPS;  // particles a warp owns: a multiple of 32
 constexpr int PT_ITERS = PT_PER_WARP / 32;
 static_assert(PT_PER_WARP % 32 == 0 && PT_PER_WARP <= 255, "a warp owns whole 32-particle rows; ranks fit 8 bits");
-constexpr int PT_WCAP = 1024;                               // event offsets of a tile kept on chip (more: looked up in global memory)
+constexpr int PT_WCAP = 384;                                // event offsets of a tile kept on chip (more: looked up in global memory)
 constexpr size_t PO_F = 0;                                  // px, py, pz, vx, vy, vz: 6 x 4 B x TILE
 constexpr size_t PO_PID = PO_F + 6 * 4 * (size_t)PT_TILE;   // 4 B x TILE
 constexpr size_t PO_Q = PO_PID + 4 * (size_t)PT_TILE;       // 1 B x TILE
@@ -85,6 +85,28 @@ __device__ __forceinline__ int hit_tower_rec(const PdCardScalars &sc, const floa
   j = j < 0 ? 0 : j;
   j = j > n - 1 ? n - 1 : j;
   return (on & 0xffff) + j;
+}
+
+// For every tile boundary j (the first particle of tile j; the call's first particle for j = 0): the first event whose
+// offset is >= that particle, and the last one whose offset is <= it (= the event the particle belongs to).
+__global__ void pd_tile_events_kernel(const long long *offsets, long long n_events, long long p_base, int n_ptiles, int *out) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j > n_ptiles) return;
+  const long long s = j == 0 ? p_base : (p_base & ~15ll) + (long long)j * PT_TILE;
+  long long lo = 0, hi = n_events + 1;  // first entry >= s
+  while (lo < hi) {
+    const long long mid = (lo + hi) >> 1;
+    if (__ldg(offsets + mid) < s) lo = mid + 1;
+    else hi = mid;
+  }
+  out[2 * j] = (int)lo;
+  hi = n_events + 1;  // first entry > s (from lo on)
+  while (lo < hi) {
+    const long long mid = (lo + hi) >> 1;
+    if (__ldg(offsets + mid) <= s) lo = mid + 1;
+    else hi = mid;
+  }
+  out[2 * j + 1] = (int)lo - 1;
 }
 
 template <bool DEBUG>
@@ -166,13 +188,21 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     // e_lo = the event of particle s_eff, e_hi = the last event with a particle in the tile.  The offsets of
     // e_lo .. e_hi + 1, relative to the tile, go to shared memory: class A looks its event up there.
     if (wid == 0) {
-      const long long ne1 = prm.n_events + 1;
-      const long long e_lo = warp_lower_bound(prm.offsets, ne1, s_eff + 1) - 1;  // entries <= s_eff, minus one
-      const long long w3 = s0 + PT_TILE >= n_all ? ne1 : warp_lower_bound(prm.offsets, ne1, s0 + PT_TILE);
+      // found by pd_tile_events_kernel for every tile boundary: first event with offset >= s, last with offset <= s
+      const long long e_lo = (long long)__ldg(prm.tile_ev + 2 * tile + 1);
+      const long long w3 = s0 + PT_TILE >= n_all ? prm.n_events + 1 : (long long)__ldg(prm.tile_ev + 2 * (tile + 1));
       const long long e_hi = min(w3, prm.n_events) - 1;
       if (lane == 0) s_win[0] = e_lo, s_win[1] = e_hi;
       if (e_hi - e_lo + 2 <= PT_WCAP)
         for (int k = lane; k <= (int)(e_hi - e_lo) + 1; k += 32) s_woff[k] = (int)(__ldg(prm.offsets + e_lo + k) - s0);
+    } else if (tid == 32 && prm.tma_ok) {
+      // the tile this CTA will most likely take next: towards L2 now, so that its bulk copies find it there
+      const long long sn = s0 + (long long)gridDim.x * PT_TILE;
+      if (sn + PT_TILE <= n_all) {
+        l2_prefetch(prm.px + sn, 4u * PT_TILE), l2_prefetch(prm.py + sn, 4u * PT_TILE), l2_prefetch(prm.pz + sn, 4u * PT_TILE);
+        l2_prefetch(prm.vx + sn, 4u * PT_TILE), l2_prefetch(prm.vy + sn, 4u * PT_TILE), l2_prefetch(prm.vz + sn, 4u * PT_TILE);
+        l2_prefetch(prm.pid + sn, 4u * PT_TILE), l2_prefetch(prm.charge + sn, 1u * PT_TILE);
+      }
     }
     // this warp's words of the accepted mask
     if (lane < PT_ITERS) s_accmask[wword + lane] = 0u;
@@ -362,6 +392,7 @@ int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_sm
   int grid = num_sms * per_sm;
   if (grid > prm.n_ptiles) grid = prm.n_ptiles;
   if (grid < 1) grid = 1;
+  pdk::pd_tile_events_kernel<<<(prm.n_ptiles + 1 + 255) / 256, 256, 0, (cudaStream_t)stream>>>(prm.offsets, prm.n_events, prm.p_base, prm.n_ptiles, prm.tile_ev);
   kern<<<grid, pdk::PT_THREADS, smem, (cudaStream_t)stream>>>(prm);
   return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
 }

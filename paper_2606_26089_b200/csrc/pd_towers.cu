@@ -42,18 +42,9 @@ constexpr uint32_t SLOT_TW = 1u << 28, SLOT_PH = 1u << 29, SLOT_NH = 1u << 30;
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~size_t(15); }
 
-// Shared-memory carve-up, identical on host (size) and device (pointers).
-struct Layout {
-  size_t offset, w, eta_c, inv_cosh, binlut;     // card tables (what pass O needs)
-  size_t off32, ntrk, ntow, nph, nnh;            // per-event arrays [G+1]
-  size_t misc;                                   // scratch words
-  size_t seg;                                    // track segments of the tile [3][64]
-  size_t cnt;                                    // pass W warp counts -> prefixes [2][256]
-  size_t bitmap, gprefix;                        // per event: tower bits, group prefix
-  size_t l2p, pool;                              // sparse mode (see make_layout)
-  size_t res, Ev, Et, head, stg, ev;             // per particle / per slot
-  size_t total;
-};
+// Shared-memory carve-up of kernel T (PdTLayout, pd_internal.h): computed once on the host and handed to the kernel
+// in its parameters, so that an array's address is one constant-bank operand instead of arithmetic on G and C.
+using Layout = PdTLayout;
 
 // Dense mode: one bit per tower and event (bitmap), a prefix per 128-tower group (gprefix).
 // Sparse mode (large grids, small events: the bitmaps would be almost empty and take most of the shared memory):
@@ -65,7 +56,7 @@ __host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int word
   auto take = [&](size_t bytes) {
     size_t at = o;
     o = align16(o + bytes);
-    return at;
+    return (uint32_t)at;
   };
   l.offset = take(4 * (n_bins + 1));
   l.w = take(4 * n_bins);
@@ -97,7 +88,7 @@ __host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int word
   l.head = take(4 * (size_t)C);
   l.stg = take(4 * ((size_t)C + 4));  // first the keys (2 B each, + 8 for the same reason), later one float per slot
   l.ev = take(G > 1 ? (size_t)C : 0);
-  l.total = o;
+  l.total = (uint32_t)o;
   return l;
 }
 constexpr int T_BYTES_PER_PARTICLE = 20;  // res, Ev, Et, head, stg
@@ -162,7 +153,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
   const int wpe = sc.words_per_event, gpe = wpe >> 2;
   constexpr bool sparse = SPARSE;   // two-level tower bitmap, chosen by pd_plan (prm.sparse)
   const int l2w = (gpe + 31) >> 5;  // words of the per-event group bitmap (sparse mode)
-  const Layout L = make_layout(nb, sc.n_towers, wpe, G, C, prm.sparse);
+  const Layout &L = prm.lay;
   int *s_offset = (int *)(smem + L.offset);
   float *s_w = (float *)(smem + L.w);
   float *s_eta_c = (float *)(smem + L.eta_c);
@@ -715,7 +706,8 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   plan->n_tiles = int((n_events + g - 1) / g);
   plan->n_ptiles = int((n_particles + 15 + PD_PTILE - 1) / PD_PTILE);  // + 15: tiles start at a multiple of 16 particles
   plan->sparse = sparse;
-  plan->smem_bytes = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse).total;
+  plan->lay = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse);
+  plan->smem_bytes = plan->lay.total;
   return PD_OK;
 }
 
