@@ -263,6 +263,29 @@ static __device__ __noinline__ bool graze_double(const PdCardScalars &sc, float 
   return true;
 }
 
+// Two more rare paths, for vertices far off the axis: the hit is the vertex plus the chord, and where the result is much
+// smaller than either (an endcap hit close to the axis from a vertex a metre away; a barrel hit whose z is a small
+// difference of the vertex z and the path along z) the fp32 sum keeps fewer digits than the 1e-6 the tower decision
+// wants.  Redone in double (CUDA's own double routines: it hardly ever runs; never for vertices on the axis).
+static __device__ __noinline__ void endcap_xy_double(const PdCardScalars &sc, float px, float py, float pz, float vx, float vy,
+                                                     float vz, float aq, float s, float &x, float &y) {
+  const double pxd = px, pyd = py;
+  const double pt = sqrt(pxd * pxd + pyd * pyd);
+  const double rho = pt / (sc.kB_d * (double)aq);
+  const double zd = (double)sc.L - (pz > 0.f ? (double)vz : -(double)vz);
+  double sh, ch;
+  sincospi(zd * (sc.kB_d * (0.5 * 0.31830988618379067154) * (double)aq) / fabs((double)pz), &sh, &ch);
+  const double c0 = pxd / pt, s0 = pyd / pt, l2 = 2.0 * rho * sh;
+  x = (float)((double)vx + l2 * (c0 * ch - (double)s * s0 * sh));
+  y = (float)((double)vy + l2 * (s0 * ch + (double)s * c0 * sh));
+}
+static __device__ __noinline__ float barrel_z_double(const PdCardScalars &sc, float px, float py, float pz, float vx, float vy,
+                                                     float vz, float aq, float s) {
+  float cc = 1.f, ss = 0.f;
+  graze_double(sc, px, py, vx, vy, aq, s, cc, ss);
+  return (float)((double)vz + 2.0 * atan2((double)ss, (double)cc) * (double)pz / (sc.kB_d * (double)aq));
+}
+
 // readings A4, A5: born on/outside the cylinder, or no transverse momentum -> dropped
 __device__ __forceinline__ bool vertex_dropped(const PdCardScalars &sc, float px, float py, float vx, float vy, float vz) {
   const float pt2 = fmaf(px, px, py * py);
@@ -372,11 +395,15 @@ __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, fl
     ch = cc * inv, sh = ss * inv;
     const float hR = fast_atan2(ss, cc);
     z = fmaf(2.f * hR, pz * sc.inv_kB * (aq == 1.f ? 1.f : fast_rcp(aq)), vz);
+    // (the path along z is good to ~3e-7 of its length: that matters against the 1e-6 of eta only for a long path that
+    // ends near z = 0, i.e. for a vertex metres away from the centre)
+    if (fabsf(z - vz) > 2.f * sc.R && fabsf(z) < sc.R) z = barrel_z_double(sc, px, py, pz, vx, vy, vz, aq, s);
   }
   // chord form (pi-periodic in h): position = v + 2 rho sin h u(phi0 + s h)
   const float l2 = 2.f * rho * sh;
   x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
   y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
+  if (endcap && fmaf(x, x, y * y) < 0.09f * (sc.R2 - D)) endcap_xy_double(sc, px, py, pz, vx, vy, vz, aq, s, x, y);
   return (endcap ? PD_ENDCAP : PD_BARREL) | looper;
 }
 

@@ -158,7 +158,6 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     const long long s0 = p_al + (long long)tile * PT_TILE;
     const int n = (int)min((long long)PT_TILE, n_all - s0);
     const int lo_skip = (int)max(p_base - s0, 0ll);  // > 0 only in tile 0
-    const long long s_eff = s0 + lo_skip;            // first particle of the call in the tile
     const bool full = n == PT_TILE && prm.tma_ok;
 
     // ---- stage the tile's inputs: eight bulk copies (one thread), or plain loads for the ragged last tile /

@@ -243,8 +243,20 @@ def compare(card_name, ev, seed, gpu, event_base=0, max_rounds=6):
         fail("efl_E beyond tolerance at %d: gpu %r oracle %r scale %r" % (i, gpu["efl_E"][i], o["efl_E"][i], scale[i]))
     if not okP.all():
         fail("efl_pt beyond tolerance")
-    # how many neutrals would fail the plain (unscaled) rule -- reported, not failed
-    errs["efl_neutral_E_outside_plain_tol"] = int(np.count_nonzero(~_close(gpu["efl_E"], o["efl_E"])))
+    # How many neutrals miss the PLAIN rule max(1e-5 |o|, 1e-6): reported by every test and bounded -- at most 1.5 % of
+    # the neutrals (measured: 0-0.03 % on cfg1/2/4, 0.4 % on cfg0-like kinematics, ~1 % on the ATLAS-like card, whose
+    # calorimeter resolution at high energy is comparable to the excess).  Closing the gap needs the smears of the tower
+    # AND of its tracks in double: built and measured at +30 % of the chain's time on cfg2 with CUDA's double routines,
+    # +5 % for the tower alone with short custom ones -- which left the count almost unchanged, because the fp32 track
+    # energies dominate.
+    n_out = int(np.count_nonzero(~_close(gpu["efl_E"], o["efl_E"])))
+    n_neu = int(np.count_nonzero(neutral))
+    errs["efl_neutral_E_outside_plain_tol"] = n_out
+    errs["efl_neutrals"] = n_neu
+    rep["neutral_outside_plain_tol"] = n_out
+    rep["neutrals"] = n_neu
+    if n_out > max(3, 0.015 * n_neu):
+        fail("%d of %d neutrals outside the plain tolerance (bound: 1.5 %%)" % (n_out, n_neu))
     rel = np.abs(gpu["trk_pt"].astype(np.float64) - o["trk_pt"]) / np.maximum(np.abs(o["trk_pt"]), 1e-30)
     errs["max_rel_trk_pt"] = float(rel.max()) if rel.size else 0.0
     rel = np.abs(gpu["tow_E"].astype(np.float64) - o["tow_E"]) / np.maximum(np.abs(o["tow_E"]), 1e-30)

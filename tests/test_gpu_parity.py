@@ -14,9 +14,11 @@ pytestmark = pytest.mark.gpu
 SMALL = {0: 1000, 1: 400, 2: 24, 3: 3000, 4: 3000}
 
 
-def _check(rep, max_override_frac=2e-3):
+def _check(rep, max_override_frac=5e-4):
+    """unexcused mismatches: none; near-edge overrides: at most 5e-4 of the particles (SURVEY 8c.6 predicts ~1e-4; a
+    floor of 3 for tiny inputs); neutrals outside the plain tolerance: bounded inside compare()."""
     assert rep["unexcused"] == 0, rep["problems"][:10]
-    assert rep["overridden_particles"] <= max(2, max_override_frac * rep["n_particles"]), rep
+    assert rep["overridden_particles"] <= max(3, max_override_frac * rep["n_particles"]), rep
     return rep
 
 
@@ -33,6 +35,51 @@ def test_config_parity(cfg):
     assert gpu["launches"] >= 1
     rep = _check(compare(card, ev, seed, gpu))
     print("cfg%d parity: %s" % (cfg, {k: v for k, v in rep.items() if k != "problems"}))
+
+
+@pytest.mark.parametrize("card,bz", [("cms_like", None), ("atlas_like", None), ("aleph_like", None), ("cms_like", -3.8)])
+def test_displaced_vertices_randomised(card, bz, tmp_path):
+    """SURVEY 8c.2 O2, general-vertex helix: every particle has its own vertex anywhere in the tracker volume
+    (r0 < 0.95 R, |vz| < 0.95 L), pT from 0.15 GeV (circles that do and do not enclose the axis, loopers, helices that
+    graze the barrel), |q| in {1, 2}; the three cards and a reversed field: >= 2e5 particles in all, none unexcused."""
+    import cards
+    from gpu_util import run_gpu
+    from oracle import pdo
+    from parity import compare
+
+    base = pdo.Card(card)
+    info = {"cms_like": (1.29, 3.0), "atlas_like": (1.15, 3.5), "aleph_like": (1.8, 2.5)}[card]
+    ev = wl.displaced(1200, 45.0, info[0], info[1], seed=101 + len(card))
+    assert ev.n_particles >= 50000
+    path = card if bz is None else cards.variant(tmp_path / "rev.card", base.edges, base.nphi, bz=bz)
+    gpu = run_gpu(path, ev, 41)
+    assert gpu["status_word"] == 0
+    rep = _check(compare(path, ev, 41, gpu))
+    assert int(gpu["trk_offsets"][-1]) > 1000
+    st = gpu["dbg_status"]
+    # the sample really exercises the branches: barrel, endcap, loopers, dropped
+    assert (st == 1).sum() > 1000 and (st == 2).sum() > 1000 and ((st & 4) != 0).sum() > 500
+    print(card, bz, {k: rep[k] for k in ("n_particles", "flagged_particles", "overridden_particles", "neutral_outside_plain_tol", "neutrals")})
+
+
+def test_many_tiny_and_empty_events_in_one_particle_tile():
+    """Events of 0-2 particles: a tile of kernel P (1,536 particles) then spans > 1,000 events, more than the window of
+    event offsets it keeps on chip, and looks its events up in global memory instead; kernel T packs 256 events a tile."""
+    from gpu_util import run_gpu
+    from parity import compare
+
+    rng = np.random.default_rng(3)
+    base = wl.generate(0, 400)
+    P = wl.particle
+    lists = []
+    for k in range(6000):
+        m = int(rng.integers(0, 3))
+        lists.append([P(211 if (k + j) % 2 else -211, 1 if (k + j) % 2 else -1, 0.3 + 3.0 * rng.random(), 2.0 * rng.random() - 1.0,
+                        6.0 * rng.random() - 3.0, 0.13957039) for j in range(m)])
+    ev = wl.concat_events([wl.slice_events(base, 0, 100), wl.from_lists(lists), wl.slice_events(base, 100, 400), wl.from_lists([[] for _ in range(3000)])])
+    gpu = run_gpu("cms_like", ev, 13)
+    assert gpu["status_word"] == 0
+    _check(compare("cms_like", ev, 13, gpu))
 
 
 def test_edge_cases_empty_and_ragged():
@@ -74,7 +121,7 @@ def test_degenerate_particles():
     for card in ("cms_like", "atlas_like", "aleph_like"):
         gpu = run_gpu(card, ev, 5)
         assert gpu["status_word"] == 0
-        _check(compare(card, ev, 5, gpu), max_override_frac=1.0)
+        _check(compare(card, ev, 5, gpu), max_override_frac=1.0)  # hand-made particles sit ON edges
 
 
 def test_bitwise_reproducible_and_event_base():
@@ -225,9 +272,36 @@ def test_card_file_variants_and_multiply_charged_particles(tmp_path):
     for name, path in variants.items():
         gpu = run_gpu(path, ev, 17, event_base=1000)
         assert gpu["status_word"] == 0, name
-        rep = _check(compare(path, ev, 17, gpu, event_base=1000), max_override_frac=5e-3)
+        rep = _check(compare(path, ev, 17, gpu, event_base=1000))
         assert int(gpu["efl_offsets"][-1]) > 0, name
         print(name, {k: rep[k] for k in ("flagged_particles", "overridden_particles", "flagged_towers", "overridden_towers")})
+
+
+def test_forced_kernel_variants_in_a_subprocess(tmp_path):
+    """PD_SPARSE=1 (two-level tower bitmap) and PD_THREADS=1024 (one CTA per SM) are read once per process: each forced
+    variant runs in a fresh interpreter on the three cards and must match the oracle like the automatic plan does."""
+    import os
+    import subprocess
+    import sys
+
+    code = (
+        "import sys, importlib; sys.path.insert(0, %r); sys.path.insert(0, %r)\n"
+        "wl = importlib.import_module('workloads.generate')\n"
+        "from gpu_util import run_gpu; from parity import compare\n"
+        "for cfg, ne in ((0, 300), (3, 600), (4, 600), (1, 60)):\n"
+        "    ev = wl.generate(cfg, ne); card = wl.config_card(cfg)\n"
+        "    g = run_gpu(card, ev, 7)\n"
+        "    assert g['status_word'] == 0, (cfg, g['status_word'])\n"
+        "    rep = compare(card, ev, 7, g)\n"
+        "    assert rep['unexcused'] == 0, rep['problems'][:5]\n"
+        "    assert rep['overridden_particles'] <= max(3, 5e-4 * rep['n_particles'])\n"
+        "print('variant ok')\n"
+    ) % (os.path.dirname(os.path.dirname(os.path.abspath(__file__))), os.path.dirname(os.path.abspath(__file__)))
+    for env_add in ({"PD_SPARSE": "1"}, {"PD_THREADS": "1024"}, {"PD_SPARSE": "0"}):
+        env = dict(os.environ)
+        env.update(env_add)
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
+        assert out.returncode == 0 and "variant ok" in out.stdout, (env_add, out.stdout[-2000:], out.stderr[-2000:])
 
 
 def test_per_species_card(tmp_path):
@@ -243,7 +317,7 @@ def test_per_species_card(tmp_path):
     ev = _sample(400)
     gpu = run_gpu(path, ev, 23)
     assert gpu["status_word"] == 0
-    rep = _check(compare(path, ev, 23, gpu), max_override_frac=5e-3)
+    rep = _check(compare(path, ev, 23, gpu))
     # the species tables really are in use: the same events through the species-less card give other tracks
     plain = run_gpu("cms_like", ev, 23, debug=False)
     assert int(plain["trk_offsets"][-1]) != int(gpu["trk_offsets"][-1])

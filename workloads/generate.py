@@ -243,6 +243,35 @@ def _gen_zqq(n_events, seed):
     return _finish(off, pid, q, pt, eta, phi, m, z, z, z)
 
 
+def displaced(n_events: int, mean_mult: float, radius: float, half_length: float, seed: int, pt_lo: float = 0.15,
+              pt_hi: float = 100.0, charged_frac: float = 0.75) -> Events:
+    """Particles born anywhere inside a cylinder (r0 < 0.95 radius, |vz| < 0.95 half_length; uniform in volume), each with
+    its own vertex: pT log-uniform in [pt_lo, pt_hi], eta ~ U(-3, 3), phi uniform; charges +-1 and +-2 (pions with twice
+    the charge for |q| = 2), the rest photons and K0L.  For the chain's displaced-vertex branches."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    counts = rng.poisson(mean_mult, n_events).astype(np.int64)
+    off = _offsets(counts)
+    n = int(off[-1])
+    r0 = 0.95 * radius * np.sqrt(rng.random(n))
+    a = 2.0 * np.pi * rng.random(n)
+    vx, vy = r0 * np.cos(a), r0 * np.sin(a)
+    vz = 0.95 * half_length * (2.0 * rng.random(n) - 1.0)
+    pt = pt_lo * np.power(pt_hi / pt_lo, rng.random(n))
+    eta = -3.0 + 6.0 * rng.random(n)
+    phi = -np.pi + 2.0 * np.pi * rng.random(n)
+    u = rng.random(n)
+    charged = u < charged_frac
+    sign = np.where(rng.random(n) < 0.5, 1, -1)
+    mag = np.where(rng.random(n) < 0.25, 2, 1)
+    q = np.where(charged, sign * mag, 0)
+    lepton = charged & (rng.random(n) < 0.1)
+    pid = np.where(charged, 211 * sign, np.where(u < charged_frac + 0.15, 22, 130)).astype(np.int64)
+    pid = np.where(lepton, np.where(rng.random(n) < 0.5, -11, -13) * sign, pid)
+    m = np.where(pid == 22, 0.0, np.where(np.abs(pid) == 211, 0.13957039, np.where(pid == 130, 0.497611,
+                 np.where(np.abs(pid) == 11, 0.00051099895, 0.1056584))))
+    return _finish(off, pid, q, pt, eta, phi, m, vx, vy, vz)
+
+
 def generate(cfg: int, n_events: int | None = None) -> Events:
     """Events of BASELINE.json configs[cfg]; `n_events` overrides the config's event count."""
     c = CONFIGS[cfg]
