@@ -38,7 +38,7 @@ typedef enum {
   PD_ECAPACITY = -3,  /* an output capacity is below the sufficient bound (see pd_simulate)    */
   PD_EWORKSPACE = -4, /* workspace null or smaller than pd_workspace_bytes()                  */
   PD_ECUDA = -5,      /* a CUDA runtime call failed (no device, launch error, ...)            */
-  PD_EEVENTSIZE = -6  /* device-side: a tile of events exceeded the on-chip capacity           */
+  PD_EEVENTSIZE = -6  /* (not raised any more: events of any size are handled; kept for ABI stability) */
 } pd_status;
 
 /* status byte of a propagated particle ("PropagatedParticle"): low two bits = face */
@@ -128,8 +128,10 @@ int pd_load_card(const char *name_or_path, pd_card **out);
 void pd_free_card(pd_card *card);
 int pd_card_info(const pd_card *card, pd_card_info_t *out);
 
-/* Bytes of DEVICE workspace pd_simulate needs for a call of this size (look-back chains, tile
- * counter, status word, the ring in which smeared track records wait for their output offsets).  Negative pd_status on invalid arguments. */
+/* Bytes of DEVICE workspace pd_simulate needs for a call of this size: look-back chains, tile counters, status word,
+ * and what kernel P leaves for kernel T -- per particle a 16-bit tower key, an accepted bit and room for a parked track
+ * record (~32 B per particle in all) -- plus the accumulators of the big-tile path (40 B x towers x resident CTAs).
+ * Negative pd_status on invalid arguments. */
 int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles);
 
 /* One pass of the whole chain S0..S8 over a batch of events.
@@ -142,14 +144,17 @@ int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_part
  *   cuda_stream: a cudaStream_t (NULL = default stream).  Asynchronous: results are valid after the
  *     caller synchronises the stream; pd_last_status() then reports device-side conditions.
  * Errors are detected synchronously (PD_EINVAL, PD_ECAPACITY, PD_EWORKSPACE, PD_ECUDA); there is no
- * device-side overflow path for the outputs because the capacities above are sufficient bounds. */
+ * device-side overflow path for the outputs because the capacities above are sufficient bounds, and no limit on the
+ * number of particles of an event.  Three kernel launches (event windows of the particle tiles; kernel P: particles ->
+ * tower keys + parked tracks; kernel T: towers, EFlow, ordered collections) and one memset. */
 int pd_simulate(const pd_card *card, const pd_events *events, uint64_t seed, int64_t event_base,
                 pd_tracks *tracks, pd_towers *towers, pd_eflow *eflow, pd_debug *debug,
                 void *workspace, int64_t workspace_bytes, void *cuda_stream);
 
-/* Reads back (synchronising the stream) the device-side status word a pd_simulate call left in its
- * workspace: PD_OK, or PD_EEVENTSIZE if some tile of events did not fit on chip (its events then
- * produced no objects; see pd_set_tile_events). */
+/* Reads back (synchronising the stream) the device-side status word a call left in its workspace: PD_OK for
+ * pd_simulate (there is no event-size limit: a tile of events that does not fit on chip is processed event by event
+ * through exact accumulators in the workspace -- "no fixed model limit"), PD_ECAPACITY for a
+ * pd_pileup_merge whose output did not fit. */
 int pd_last_status(const void *workspace, void *cuda_stream);
 
 /* ---- Event features and lepton isolation (section 2.4 Eq. 1; L141 Table 2) ----
@@ -290,14 +295,11 @@ int pd_truth_features(const pd_events *events, int32_t skip_neutrinos, pd_featur
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 
-/* Events per on-chip tile for the calls this thread makes from now on: 0 (default) = chosen from the
- * average event size with head-room for Poisson-like fluctuations; g >= 1 = at most g (<= 256).  A batch
- * whose event sizes are far from Poisson (a few huge events among many small ones) can make a tile of the
- * automatic plan exceed the on-chip capacity: pd_last_status() then reports PD_EEVENTSIZE and the caller
- * re-runs the call after pd_set_tile_events(1) (pd_simulate_host does that itself): one event per tile in
- * the one-CTA-per-SM variant of the kernel, whose only limit is 8,191 particles per event.  Results do not depend on
- * the tiling.  pd_workspace_bytes() depends on it: call it after changing the setting.  Returns the
- * previous value. */
+/* Tuning / testing only: events per on-chip tile of kernel T for the calls this thread makes from now on: 0 (default) =
+ * chosen from the average event size with head-room for Poisson-like fluctuations; g >= 1 = at most g (<= 256; 1 also
+ * selects the one-CTA-per-SM variant).  Results never depend on it, and no setting is ever needed for correctness:
+ * tiles that exceed the on-chip capacity take the (slower) path through the workspace by themselves.
+ * pd_workspace_bytes() depends on it: call it after changing the setting.  Returns the previous value. */
 int pd_set_tile_events(int g);
 
 /* Same computation with HOST pointers everywhere (inputs and outputs in host memory, pinned or

@@ -42,9 +42,9 @@ static size_t ws_chain_bytes(const PdLaunchPlan &plan) {
 // What kernel P leaves for kernel T, per particle slot (n_ptiles * PD_PTILE slots): the 16-bit key, the accepted bit,
 // and the parked track records (segment index 1 B, charge 1 B, pid 4 B, six floats).  Each array 256-byte aligned.
 struct WsLayout {
-  size_t tile_ev, key, accmask, idx, q, pid, f[6], total;
+  size_t tile_ev, key, accmask, idx, q, pid, f[6], big_acc, total;
 };
-static WsLayout ws_layout(const PdLaunchPlan &plan) {
+static WsLayout ws_layout(const PdLaunchPlan &plan, int n_towers) {
   const size_t slots = (size_t)PD_PTILE * (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1);
   WsLayout l;
   size_t o = ws_chain_bytes(plan);
@@ -60,6 +60,7 @@ static WsLayout ws_layout(const PdLaunchPlan &plan) {
   l.q = take(slots);
   l.pid = take(4 * slots);
   for (int k = 0; k < 6; ++k) l.f[k] = take(4 * slots);
+  l.big_acc = take(8 * 5 * (size_t)n_towers * (size_t)plan.max_ctas);  // tiles that do not fit on chip (any event size)
   l.total = o;
   return l;
 }
@@ -114,7 +115,7 @@ int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_part
   if (!card || n_events < 0 || n_particles < 0) return PD_EINVAL;
   PdLaunchPlan plan;
   pd_plan(card, n_events, n_particles, &plan);
-  return (int64_t)ws_layout(plan).total;
+  return (int64_t)ws_layout(plan, card->sc.n_towers).total;
 }
 
 int pd_last_launch_count(void) { return t_launches; }
@@ -449,13 +450,14 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
   p.chain = (unsigned long long *)(ws + kWsHeader);
   p.chain_t = p.chain + (plan.n_tiles > 0 ? plan.n_tiles : 1);
   {
-    const WsLayout wl = ws_layout(plan);
+    const WsLayout wl = ws_layout(plan, card->sc.n_towers);
     p.tile_ev = (int *)(ws + wl.tile_ev);
     p.key = (unsigned short *)(ws + wl.key);
     p.accmask = (unsigned int *)(ws + wl.accmask);
     p.park_idx = ws + wl.idx;
     p.park_q = (signed char *)(ws + wl.q);
     p.park_pid = (int *)(ws + wl.pid);
+    p.big_acc = (long long *)(ws + wl.big_acc);
     for (int k = 0; k < 6; ++k) p.park_f[k] = (float *)(ws + wl.f[k]);
   }
   p.n_ptiles = plan.n_ptiles;

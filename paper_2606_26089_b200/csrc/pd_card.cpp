@@ -170,6 +170,27 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
   }
 
   if (total > long(PD_MAX_TOWERS)) return PD_ECARD;
+  // every number finite and in its range: thresholds and resolutions >= 0 (a negative threshold would let pass W count
+  // a neutral that pass O never writes), efficiencies in [0, 1], |cos theta| cut in (0, 1], edges and rows ordered
+  {
+    auto fin = [](double x) { return std::isfinite(x); };
+    auto nonneg = [&](double x) { return fin(x) && x >= 0.0; };
+    if (!fin(r.bz) || !fin(r.radius) || !fin(r.half_length) || !fin(r.kappa)) return PD_ECARD;
+    if (!nonneg(r.thr_ecal) || !nonneg(r.thr_hcal) || !nonneg(r.trk_a) || !nonneg(r.trk_b)) return PD_ECARD;
+    for (int k = 0; k < 3; ++k)
+      if (!nonneg(r.ecal[k]) || !nonneg(r.hcal[k])) return PD_ECARD;
+    for (int sp = 1; sp <= 3; ++sp)
+      if (r.has_trk_sp[sp] && (!nonneg(r.trk_a_sp[sp]) || !nonneg(r.trk_b_sp[sp]))) return PD_ECARD;
+    if (r.has_cos && !(fin(r.cos_max) && r.cos_max > 0.0 && r.cos_max <= 1.0)) return PD_ECARD;
+    for (double e : r.edges)
+      if (!fin(e)) return PD_ECARD;
+    if (r.theta && !(r.edges.front() >= 0.0 && r.edges.back() <= kPi)) return PD_ECARD;
+    for (const auto &row : r.eff) {
+      // pt_lo < pt_hi, |eta|_lo < |eta|_hi (the upper ends may be +inf), 0 <= eps <= 1
+      if (!(nonneg(row[0]) && row[1] > row[0] && nonneg(row[2]) && row[3] > row[2])) return PD_ECARD;
+      if (!(fin(row[4]) && row[4] >= 0.0 && row[4] <= 1.0)) return PD_ECARD;
+    }
+  }
 
   c->name = r.name;
   c->bz = float(r.bz);

@@ -137,6 +137,7 @@ struct PdParams {
   unsigned long long *chain;  // [n_tiles] look-back words of kernel T: towers | neutrals
   unsigned int *tile_counter;
   int *status_word;
+  long long *big_acc;    // [max_ctas][n_towers][5] exact accumulators of the tiles that do not fit on chip (pd_towers.cu big_event)
   // kernel P (pd_particles.cu): flat tiles of PD_PTILE particles
   long long p_base;              // offsets[0]: first particle of the call in the arrays (0 for a public call)
   int n_ptiles;
@@ -164,6 +165,7 @@ struct PdLaunchPlan {
   int events_per_tile;
   int n_tiles;
   int n_ptiles;      // tiles of kernel P
+  int max_ctas;      // upper bound of kernel T's grid (sizes big_acc)
   int sparse;        // two-level tower bitmap
   size_t smem_bytes;
   PdTLayout lay;

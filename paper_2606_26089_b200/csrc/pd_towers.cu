@@ -143,6 +143,261 @@ __device__ __forceinline__ int popc_below(const uint4 &v, int pos) {
   return __popc(v.x & m0) + __popc(v.y & m1) + __popc(v.z & m2) + __popc(v.w & m3);
 }
 
+// ---- tiles that do not fit on chip ---------------------------------------------------------------------------
+// A tile of the plan (G whole events) whose particles exceed the on-chip capacity C -- one huge event, or a few large
+// ones among the small ones the plan was made for -- takes this path: its events one by one, of ANY size ("no fixed
+// model limit"), with the per-tower sums in a dense array of exact 64-bit fixed-point accumulators in
+// the workspace (global atomics: integer, hence still order-independent and bitwise reproducible) instead of lists in
+// shared memory.  Two sweeps over the tile: the first counts what every event emits, so that the tile can take its
+// place in the look-back chains like any other; the second writes.  Slow (everything is computed twice, through L2)
+// but exact, and it only runs for the tiles that need it.
+struct BigCounts {
+  int trk, tow, ph, nh;
+};
+
+// one event [pa, pb) of a big tile.  write == false: count only.  Shared memory: bmap[wpe] tower bits, wcnt[2 * wpe]
+// per-word counts / prefixes, scal[8] scalars.  acc: this CTA's [n_towers][5] accumulators, all zero on entry and exit.
+template <int THREADS, bool DEBUG>
+__device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_index, long long pa, long long pb, bool write,
+                                            long long base_trk, long long base_tow, long long base_efl, const int *s_offset,
+                                            const unsigned short *s_binlut, const float *s_w, const float *s_eta_c,
+                                            const float *s_inv_cosh, uint32_t *bmap, unsigned *wcnt, int *scal, long long *acc) {
+  constexpr int W = THREADS / 32;
+  const PdCardScalars &sc = prm.sc;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const int wpe = sc.words_per_event;
+  const long long p_al = prm.p_base & ~15ll;
+  unsigned long long *uacc = (unsigned long long *)acc;
+  for (int k = tid; k < wpe; k += THREADS) bmap[k] = 0u;
+  if (tid < 8) scal[tid] = 0;
+  __syncthreads();
+  // deposits: tower bit + exact sum, by component
+  for (long long i = pa + tid; i < pb; i += THREADS) {
+    const unsigned key = (unsigned)__ldg(prm.key + (i - p_al));
+    if (key != 0xffffu) {
+      const int tower = (int)(key & 0x7fffu), hc = (int)(key >> 15);
+      atomicOr(&bmap[tower >> 5], 1u << (tower & 31));
+      atomicAdd(uacc + 5 * (size_t)tower + hc, (unsigned long long)__float2ll_rn(__ldg(prm.E + i) * 4294967296.f));
+      if (DEBUG) atomicMin(acc + 5 * (size_t)tower + 4, i - pa - (1ll << 40));  // first depositing particle (biased: the slot starts at 0)
+    }
+  }
+  // the event's tracks, segment by segment (warp per segment): energy into the tower's track sums; in the writing sweep
+  // also into the Track collection and the EFlow collection (the event's tracks come first in both)
+  {
+    const long long qa = pa - p_al, qb = pb - p_al;
+    const long long gs_lo = qa / PD_PSEG, gs_hi = pb > pa ? (qb - 1) / PD_PSEG : gs_lo - 1;
+    int done = 0;  // tracks of earlier segments (all warps walk the segments in the same order, so each keeps the count)
+    for (long long gsi = gs_lo; gsi <= gs_hi; ++gsi) {
+      const uint32_t w = lane < PD_PSEG / 32 ? __ldg(prm.accmask + gsi * (PD_PSEG / 32) + lane) : 0u;
+      const int lo = (int)max(qa - gsi * PD_PSEG, 0ll), hi = (int)min(qb - gsi * PD_PSEG, (long long)PD_PSEG);
+      const int nlo = min(max(lo - 32 * lane, 0), 32), nhi = min(max(hi - 32 * lane, 0), 32);
+      const uint32_t mlo = nlo == 32 ? 0xffffffffu : (1u << nlo) - 1u, mhi = nhi == 32 ? 0xffffffffu : (1u << nhi) - 1u;
+      const int a = (int)__reduce_add_sync(0xffffffffu, (unsigned)__popc(w & mlo));
+      const int c = (int)__reduce_add_sync(0xffffffffu, (unsigned)__popc(w & mhi)) - a;
+      if ((int)((gsi - gs_lo) % W) == wid) {
+        for (int r = lane; r < c; r += 32) {
+          const long long g = gsi * PD_PSEG + a + r;
+          const long long q = gsi * PD_PSEG + (long long)__ldg(prm.park_idx + g);  // the particle, relative to p_al
+          const unsigned key = (unsigned)__ldg(prm.key + q);
+          const float Et = __ldg(prm.park_f[3] + g);
+          if (key != 0xffffu)
+            atomicAdd(uacc + 5 * (size_t)(key & 0x7fffu) + 2 + (key >> 15), (unsigned long long)__float2ll_rn(Et * 4294967296.f));
+          if (write) {
+            const int pid = __ldg(prm.park_pid + g);
+            const float pt = __ldg(prm.park_f[0] + g), eta = __ldg(prm.park_f[1] + g), phi = __ldg(prm.park_f[2] + g);
+            const unsigned o = (unsigned)base_trk + (unsigned)(done + r);
+            prm.trk_src[o] = (int)(p_al + q);
+            prm.trk_pid[o] = pid;
+            prm.trk_charge[o] = __ldg(prm.park_q + g);
+            prm.trk_pt[o] = pt, prm.trk_eta[o] = eta, prm.trk_phi[o] = phi, prm.trk_E[o] = Et;
+            prm.trk_eta_out[o] = __ldg(prm.park_f[4] + g), prm.trk_phi_out[o] = __ldg(prm.park_f[5] + g);
+            const unsigned at = (unsigned)base_efl + (unsigned)(done + r);
+            const int apid = pid < 0 ? -pid : pid;
+            prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
+            prm.efl_src[at] = (int)(p_al + q);
+            prm.efl_pt[at] = pt, prm.efl_eta[at] = eta, prm.efl_phi[at] = phi, prm.efl_E[at] = Et;
+          }
+        }
+      }
+      done += c;
+    }
+    if (tid == 0) scal[0] = done;
+  }
+  __threadfence();
+  __syncthreads();
+  const int n_trk = scal[0];
+  // sweep A over the occupied towers (a thread takes whole bitmap words, ascending ids inside): sums -> smear ->
+  // thresholds -> EFlow subtraction, exactly as pass W; the results are stashed in the tower's accumulators
+  for (int w = tid; w < wpe; w += THREADS) {
+    uint32_t m = bmap[w];
+    unsigned c_tw = 0, c_ph = 0, c_nh = 0;
+    while (m) {
+      const int b = __ffs(m) - 1;
+      m &= m - 1;
+      const int tower = 32 * w + b;
+      long long *a5 = acc + 5 * (size_t)tower;
+      const long long a_em = __ldcg(a5), a_had = __ldcg(a5 + 1), t_em = __ldcg(a5 + 2), t_had = __ldcg(a5 + 3);
+      const float Eem = (float)a_em * 2.3283064365386963e-10f, Ehad = (float)a_had * 2.3283064365386963e-10f;
+      const float Tem = (float)t_em * 2.3283064365386963e-10f, Thad = (float)t_had * 2.3283064365386963e-10f;
+      uint32_t rn[4];
+      rng_block(prm.rk, ev_index, (uint32_t)tower, 1u, rn);
+      float em_s, had_s;
+      tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
+      const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
+      const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
+      const float n_em = em_f - Tem, n_had = had_f - Thad;
+      const bool f_ph = n_em > sc.thr_ecal, f_nh = n_had > sc.thr_hcal, f_tw = em_f + had_f > 0.f;
+      c_tw += f_tw, c_ph += f_ph, c_nh += f_nh;
+      if (DEBUG && write) {
+        const long long g = pa + (__ldcg(a5 + 4) + (1ll << 40));
+        if (prm.dbg_tw_first) prm.dbg_tw_first[g] = 1;
+        if (prm.dbg_tw[0]) prm.dbg_tw[0][g] = Eem;
+        if (prm.dbg_tw[1]) prm.dbg_tw[1][g] = Ehad;
+        if (prm.dbg_tw[2]) prm.dbg_tw[2][g] = Tem;
+        if (prm.dbg_tw[3]) prm.dbg_tw[3][g] = Thad;
+        if (prm.dbg_tw[4]) prm.dbg_tw[4][g] = em_s;
+        if (prm.dbg_tw[5]) prm.dbg_tw[5][g] = had_s;
+        if (prm.dbg_tw_dec)
+          prm.dbg_tw_dec[g] = (unsigned char)((k_em ? PD_DEC_EEM : 0) | (k_had ? PD_DEC_EHAD : 0) | (f_ph ? PD_DEC_NEM : 0) | (f_nh ? PD_DEC_NHAD : 0));
+      }
+      if (write) {
+        __stcg(a5, (long long)(((unsigned long long)__float_as_uint(had_f) << 32) | __float_as_uint(em_f)));
+        __stcg(a5 + 1, (long long)(((unsigned long long)__float_as_uint(n_had) << 32) | __float_as_uint(n_em)));
+        __stcg(a5 + 2, (long long)((f_tw ? 1 : 0) | (f_ph ? 2 : 0) | (f_nh ? 4 : 0)));
+      } else {
+        __stcg(a5, 0ll), __stcg(a5 + 1, 0ll), __stcg(a5 + 2, 0ll), __stcg(a5 + 3, 0ll), __stcg(a5 + 4, 0ll);
+      }
+    }
+    wcnt[w] = c_tw | (c_ph << 16), wcnt[wpe + w] = c_nh;
+    if (c_tw) atomicAdd(&scal[1], (int)c_tw);
+    if (c_ph) atomicAdd(&scal[2], (int)c_ph);
+    if (c_nh) atomicAdd(&scal[3], (int)c_nh);
+  }
+  __syncthreads();
+  BigCounts out;
+  out.trk = n_trk, out.tow = scal[1], out.ph = scal[2], out.nh = scal[3];
+  if (!write) return out;
+  // exclusive prefix of the per-word counts (one warp, a run of words per lane)
+  if (wid == 0) {
+    const int chunk = (wpe + 31) / 32, lo = min(wpe, lane * chunk), hi = min(wpe, lo + chunk);
+    unsigned sa = 0, sb = 0;
+    for (int k = lo; k < hi; ++k) sa += wcnt[k], sb += wcnt[wpe + k];
+    unsigned ra = warp_incl_scan(sa) - sa, rb = warp_incl_scan(sb) - sb;
+    for (int k = lo; k < hi; ++k) {
+      const unsigned ta = wcnt[k], tb = wcnt[wpe + k];
+      wcnt[k] = ra, wcnt[wpe + k] = rb;
+      ra += ta, rb += tb;
+    }
+  }
+  __syncthreads();
+  // sweep B: the ordered outputs of the event
+  const unsigned b_ph = (unsigned)base_efl + (unsigned)n_trk, b_nh = b_ph + (unsigned)out.ph;
+  for (int w = tid; w < wpe; w += THREADS) {
+    uint32_t m = bmap[w];
+    unsigned k_tw = (unsigned)base_tow + (wcnt[w] & 0xffffu), k_ph = b_ph + (wcnt[w] >> 16), k_nh = b_nh + wcnt[wpe + w];
+    while (m) {
+      const int b = __ffs(m) - 1;
+      m &= m - 1;
+      const int tower = 32 * w + b;
+      long long *a5 = acc + 5 * (size_t)tower;
+      const unsigned long long v0 = (unsigned long long)__ldcg(a5), v1 = (unsigned long long)__ldcg(a5 + 1);
+      const int flags = (int)__ldcg(a5 + 2);
+      __stcg(a5, 0ll), __stcg(a5 + 1, 0ll), __stcg(a5 + 2, 0ll), __stcg(a5 + 3, 0ll), __stcg(a5 + 4, 0ll);
+      if (!flags) continue;
+      const float em = __uint_as_float((unsigned)v0), had = __uint_as_float((unsigned)(v0 >> 32));
+      const float nem = __uint_as_float((unsigned)v1), nhad = __uint_as_float((unsigned)(v1 >> 32));
+      int bin = (int)s_binlut[tower >> 5];
+      while (tower >= s_offset[bin + 1]) ++bin;
+      const float eta_c = s_eta_c[bin], phi_c = fmaf((float)(tower - s_offset[bin]) + 0.5f, s_w[bin], -kPiF), ic = s_inv_cosh[bin];
+      if (flags & 1) {
+        const unsigned at = k_tw++;
+        prm.tow_tower[at] = tower, prm.tow_eta[at] = eta_c, prm.tow_phi[at] = phi_c;
+        prm.tow_E[at] = em + had, prm.tow_Eem[at] = em, prm.tow_Ehad[at] = had, prm.tow_ET[at] = (em + had) * ic;
+      }
+      if (flags & 2) {
+        const unsigned at = k_ph++;
+        prm.efl_cls[at] = (signed char)PD_CLS_PHOTON, prm.efl_src[at] = tower;
+        prm.efl_pt[at] = nem * ic, prm.efl_eta[at] = eta_c, prm.efl_phi[at] = phi_c, prm.efl_E[at] = nem;
+      }
+      if (flags & 4) {
+        const unsigned at = k_nh++;
+        prm.efl_cls[at] = (signed char)PD_CLS_NEUHAD, prm.efl_src[at] = tower;
+        prm.efl_pt[at] = nhad * ic, prm.efl_eta[at] = eta_c, prm.efl_phi[at] = phi_c, prm.efl_E[at] = nhad;
+      }
+    }
+  }
+  __threadfence();
+  __syncthreads();
+  (void)lt_mask;
+  return out;
+}
+
+// a whole tile through big_event: count sweep, the tile's place in both look-back chains, write sweep
+template <int THREADS, bool DEBUG>
+__device__ __noinline__ void big_tile(const PdParams &prm, unsigned char *smem, int tile, long long e0, int ne, long long p0, long long p1,
+                                      bool acc_ready) {
+  const PdCardScalars &sc = prm.sc;
+  const PdTLayout &L = prm.lay;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int *s_offset = (const int *)(smem + L.offset);
+  const float *s_w = (const float *)(smem + L.w), *s_eta_c = (const float *)(smem + L.eta_c), *s_inv_cosh = (const float *)(smem + L.inv_cosh);
+  const unsigned short *s_binlut = (const unsigned short *)(smem + L.binlut);
+  int *s_ntrk = (int *)(smem + L.ntrk), *s_ntow = (int *)(smem + L.ntow), *s_nph = (int *)(smem + L.nph), *s_nnh = (int *)(smem + L.nnh);
+  unsigned long long *s_misc = (unsigned long long *)(smem + L.misc);
+  unsigned *s_wtot = (unsigned *)(s_misc + 8);
+  uint32_t *s_res = (uint32_t *)(smem + L.res);
+  unsigned *s_head = (unsigned *)(smem + L.head);
+  {
+      uint32_t *bmap = s_res;
+      unsigned *wcnt = s_head;
+      int *scal = (int *)s_wtot;
+      long long *acc = prm.big_acc + (size_t)blockIdx.x * 5 * (size_t)sc.n_towers;
+      if (!acc_ready) {
+        for (size_t k = tid; k < 5 * (size_t)sc.n_towers; k += THREADS) __stcg(acc + k, 0ll);
+        __threadfence();
+        __syncthreads();
+      }
+      for (int e = 0; e < ne; ++e) {
+        const BigCounts c = big_event<THREADS, DEBUG>(prm, prm.event_base + e0 + e, prm.offsets[e0 + e], prm.offsets[e0 + e + 1], false, 0, 0, 0,
+                                                      s_offset, s_binlut, s_w, s_eta_c, s_inv_cosh, bmap, wcnt, scal, acc);
+        if (tid == 0) s_ntrk[e] = c.trk, s_ntow[e] = c.tow, s_nph[e] = c.ph, s_nnh[e] = c.nh;
+        __syncthreads();
+      }
+      if (wid == 1) event_scan(s_ntrk, ne);
+      else if (wid == 2) event_scan(s_ntow, ne);
+      else if (wid == 3) event_scan(s_nph, ne);
+      else if (wid == 4) event_scan(s_nnh, ne);
+      __syncthreads();
+      if (wid == 0) {
+        const unsigned long long n_t = (unsigned long long)s_ntrk[ne];
+        const unsigned long long agg = (unsigned long long)s_ntow[ne] | ((unsigned long long)(s_nph[ne] + s_nnh[ne]) << 31);
+        if (lane == 0) chain_publish(prm.chain_t, tile, n_t), chain_publish(prm.chain, tile, agg);
+        const unsigned long long ext = chain_resolve<8>(prm.chain_t, tile, n_t);
+        const unsigned long long exw = chain_resolve<8>(prm.chain, tile, agg);
+        if (lane == 0) s_misc[1] = ext, s_misc[2] = exw;
+      }
+      __syncthreads();
+      const long long bt = (long long)s_misc[1], bw = (long long)(s_misc[2] & FIELD_MASK);
+      const long long bf = bt + (long long)((s_misc[2] >> 31) & FIELD_MASK);
+      for (int e = tid; e < ne; e += THREADS) {
+        prm.trk_offsets[e0 + e + 1] = bt + s_ntrk[e + 1];
+        prm.tow_offsets[e0 + e + 1] = bw + s_ntow[e + 1];
+        prm.efl_offsets[e0 + e + 1] = bf + s_ntrk[e + 1] + s_nph[e + 1] + s_nnh[e + 1];
+      }
+      if (tile == 0 && tid == 0) prm.trk_offsets[0] = 0, prm.tow_offsets[0] = 0, prm.efl_offsets[0] = 0;
+      if (DEBUG && prm.dbg_tw_first)
+        for (long long i = p0 + tid; i < p1; i += THREADS) prm.dbg_tw_first[i] = 0;
+      __syncthreads();
+      for (int e = 0; e < ne; ++e) {
+        const int kt = s_ntrk[e], kw = s_ntow[e], kp = s_nph[e], kn = s_nnh[e];
+        __syncthreads();  // the scalars above are read before big_event reuses shared memory next to them
+        big_event<THREADS, DEBUG>(prm, prm.event_base + e0 + e, prm.offsets[e0 + e], prm.offsets[e0 + e + 1], true, bt + kt, bw + kw,
+                                  bf + kt + kp + kn, s_offset, s_binlut, s_w, s_eta_c, s_inv_cosh, bmap, wcnt, scal, acc);
+      }
+  }
+}
+
 template <int THREADS, int CTAS, bool DEBUG, bool SPARSE>
 __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_constant__ PdParams prm) {
   constexpr int W = THREADS / 32;
@@ -209,6 +464,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   uint32_t phase = 0;
+  bool acc_ready = false;  // the accumulators of the big-tile path are cleared when a CTA first needs them
   const long long p_al = prm.p_base & ~15ll;  // the key of particle p sits at key[p - p_al]
 
   for (;;) {
@@ -222,12 +478,13 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
     const bool multi = G > 1;
     const long long p0 = prm.offsets[e0];
     const long long p1 = prm.offsets[e0 + ne];
-    int n = (int)min(p1 - p0, (long long)0x7fffffff);
-    const bool overflow = (p1 - p0) > (long long)C;
-    if (overflow) {
-      n = 0;
-      if (tid == 0) atomicExch(prm.status_word, (int)PD_EEVENTSIZE);
+    if ((p1 - p0) > (long long)C) {
+      // the tile does not fit on chip: its events one by one through the accumulators in the workspace
+      big_tile<THREADS, DEBUG>(prm, smem, tile, e0, ne, p0, p1, acc_ready);
+      acc_ready = true;
+      continue;
     }
+    const int n = (int)(p1 - p0);
     // the tile's deposit energies and keys arrive by bulk copies (one thread; completion on the mbarrier) while the
     // CTA sets up the tile: 16-byte aligned start, whole 16-byte pieces; the few elements behind them by plain loads
     const int shE = (int)(p0 & 3), shK = (int)((p0 - p_al) & 7);
@@ -244,7 +501,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
     for (int i = nbE - shE + tid; i < n; i += THREADS) s_Ev[i] = __ldg(prm.E + p0 + i);
     for (int i = nbK - shK + tid; i < n; i += THREADS) ((unsigned short *)s_stg)[shK + i] = __ldg(prm.key + (p0 - p_al) + i);
     for (int e = tid; e <= ne; e += THREADS) {
-      s_off32[e] = overflow ? 0 : (int)(prm.offsets[e0 + e] - p0);
+      s_off32[e] = (int)(prm.offsets[e0 + e] - p0);
       s_ntrk[e] = 0, s_ntow[e] = 0, s_nph[e] = 0, s_nnh[e] = 0;
     }
     // the tile's tracks, segment by segment (warp per segment): from the accepted bits kernel P left
@@ -706,6 +963,11 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   plan->n_tiles = int((n_events + g - 1) / g);
   plan->n_ptiles = int((n_particles + 15 + PD_PTILE - 1) / PD_PTILE);  // + 15: tiles start at a multiple of 16 particles
   plan->sparse = sparse;
+  {
+    // grid <= resident CTAs of the device (256 SMs assumed when no device can be queried yet)
+    const long sms = query_device() == PD_OK ? g_num_sms : 256;
+    plan->max_ctas = int(sms * (plan->threads == 1024 ? 1 : 2));
+  }
   plan->lay = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse);
   plan->smem_bytes = plan->lay.total;
   return PD_OK;

@@ -46,6 +46,14 @@ def test_card_file_and_errors(tmp_path):
     bad.write_text("bz = 1\nradius = 1\nhalf_length = 1\nedges = 0 1 0.5\nnphi = 4 4\n")
     with pytest.raises(B.PdError):
         B.Card(str(bad))
+    # numbers out of range are refused at load (a negative threshold would make the kernel count neutrals it never
+    # writes): thresholds / resolutions < 0 or NaN, efficiencies outside [0, 1], a |cos theta| cut outside (0, 1]
+    for k, kw in enumerate((dict(ecal_thr=-0.1), dict(hcal_thr=float("nan")), dict(hcal=(0.05, -1.5, 0.0)), dict(track_res=(-0.01, 0.0)),
+                            dict(eff=[(1.0, "inf", 0.0, 1.5, 1.2)]), dict(eff=[(1.0, 0.5, 0.0, 1.5, 0.9)]), dict(abs_costheta_max=1.5),
+                            dict(bz=float("inf")), dict(eff=[(0.1, 1.0, 2.0, 1.0, 0.5)]))):
+        with pytest.raises(B.PdError) as e:
+            B.Card(cards.variant(tmp_path / ("r%d.card" % k), o.edges, o.nphi, **kw))
+        assert e.value.code == B.PD_ECARD, kw
 
 
 def test_argument_checking_without_gpu():

@@ -173,10 +173,10 @@ def test_host_pointer_entry_matches_device_entry(monkeypatch):
                 assert v.tobytes() == ref[k].tobytes(), (chunks, packed, k)
 
 
-def test_skewed_event_sizes_need_one_event_per_tile():
-    """A few huge events among many tiny ones: a tile of the automatic plan overflows the on-chip capacity
-    (PD_EEVENTSIZE); with pd_set_tile_events(1) the same batch runs and matches the oracle, and
-    pd_simulate_host falls back by itself."""
+def test_skewed_event_sizes_take_the_big_tile_path():
+    """A few huge events among many tiny ones: a tile of the automatic plan (made from the average event size) exceeds the
+    on-chip capacity and goes, events one by one, through the accumulators in the workspace; the result is the oracle's,
+    and identical to the one-event-per-tile plan and to the host entry."""
     import paper_2606_26089_b200 as pd
     from gpu_util import run_gpu
     from parity import compare
@@ -185,59 +185,65 @@ def test_skewed_event_sizes_need_one_event_per_tile():
     small = wl.generate(0, 40000)                # ~60 particles each: the automatic plan packs ~30 per tile
     ev = wl.concat_events([wl.slice_events(small, 0, 7000), wl.slice_events(big, 0, 1), wl.slice_events(small, 7000, 39000),
                            wl.slice_events(big, 1, 3), wl.slice_events(small, 39000, 40000)])
-    auto = run_gpu("cms_like", ev, 21, debug=False)
-    assert auto["status_word"] == pd.binding.PD_EEVENTSIZE
+    auto = run_gpu("cms_like", ev, 21)
+    assert auto["status_word"] == 0
+    _check(compare("cms_like", ev, 21, auto))
     prev = pd.set_tile_events(1)
     try:
         one = run_gpu("cms_like", ev, 21)
         assert one["status_word"] == 0
-        _check(compare("cms_like", ev, 21, one))
     finally:
         pd.set_tile_events(prev)
+    for k, v in one.items():
+        if isinstance(v, np.ndarray):
+            assert v.tobytes() == auto[k].tobytes(), k
     card = pd.Card("cms_like")
     hb = pd.HostBuffers(ev)
-    pd.simulate_host(card, hb, 21)               # retries with one event per tile internally
+    pd.simulate_host(card, hb, 21)
     got = hb.to_numpy()
     for k, v in got.items():
-        assert v.tobytes() == one[k].tobytes(), k
+        assert v.tobytes() == auto[k].tobytes(), k
 
 
-def test_huge_events_take_the_1024_thread_kernel_and_the_limit_is_reported():
-    """Events too large for half an SM's shared memory (> ~4,900 particles) run in the one-CTA-per-SM variant of the
-    kernel (1,024 threads, up to 8,191 particles on chip); beyond that the call reports PD_EEVENTSIZE."""
+def _glued_event(n_particles):
+    """One event of n_particles particles: cfg2-like events glued together."""
+    ev = wl.generate(2, max(1, (n_particles + 3999) // 4000 + 1))
+    assert ev.n_particles >= n_particles
+    return wl.Events(offsets=np.array([0, n_particles], dtype=np.int64),
+                     **{k: np.ascontiguousarray(getattr(ev, k)[:n_particles]) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
+
+
+def test_events_of_any_size():
+    """"No fixed model limit": events up to ~4,900 particles share an SM between two CTAs, up to 8,191
+    one CTA takes the SM, beyond that the event goes through the accumulators in the workspace -- 8,192, 20,000 and
+    60,000 particles here, alone, among small events, and on all three cards -- always with the oracle's result."""
     import paper_2606_26089_b200 as pd
     from gpu_util import run_gpu
     from parity import compare
 
-    def big_event(n_particles, seed):
-        ev = wl.generate(2, 3)                       # ~4,060 particles each: glue them into one event
-        one = wl.Events(offsets=np.array([0, ev.n_particles], dtype=np.int64),
-                        **{k: getattr(ev, k) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
-        keep = n_particles
-        return wl.Events(offsets=np.array([0, keep], dtype=np.int64),
-                         **{k: np.ascontiguousarray(getattr(one, k)[:keep]) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
-
-    # a batch of uniformly huge events: the plan picks the large variant by itself
-    ev = wl.concat_events([big_event(7000, 1), big_event(8191, 2), big_event(5200, 3)])
+    ev = wl.concat_events([_glued_event(7000), _glued_event(8191), _glued_event(5200)])
     gpu = run_gpu("cms_like", ev, 31)
     assert gpu["status_word"] == 0
     _check(compare("cms_like", ev, 31, gpu))
-    # outliers among small events: the automatic plan (made from the average) overflows; one event per tile works
-    mixed = wl.concat_events([big_event(7000, 1), wl.generate(0, 50), big_event(8191, 2), big_event(5200, 3)])
-    assert run_gpu("cms_like", mixed, 31, debug=False)["status_word"] == pd.binding.PD_EEVENTSIZE
-    too_big = wl.concat_events([wl.generate(0, 3), big_event(8192, 4)])
-    prev = pd.set_tile_events(1)
-    try:
-        for card in ("cms_like", "atlas_like", "aleph_like"):
-            g = run_gpu(card, mixed, 31)
-            assert g["status_word"] == 0
-            _check(compare(card, mixed, 31, g))
-        assert run_gpu("cms_like", too_big, 31, debug=False)["status_word"] == pd.binding.PD_EEVENTSIZE
-    finally:
-        pd.set_tile_events(prev)
-    hb = pd.HostBuffers(mixed)                       # the host entry falls back by itself
+    mixed = wl.concat_events([_glued_event(7000), wl.generate(0, 50), _glued_event(8192), _glued_event(20000), wl.from_lists([[], []]),
+                              _glued_event(5200), wl.generate(1, 5)])
+    for card in ("cms_like", "atlas_like", "aleph_like"):
+        g = run_gpu(card, mixed, 31)
+        assert g["status_word"] == 0
+        _check(compare(card, mixed, 31, g))
+    huge = wl.concat_events([wl.generate(0, 3), _glued_event(60000), wl.generate(0, 2)])
+    g = run_gpu("cms_like", huge, 33)
+    assert g["status_word"] == 0
+    _check(compare("cms_like", huge, 33, g))
+    h = run_gpu("cms_like", huge, 33)   # accumulators are left clean: the second run is bitwise the first
+    for k, v in g.items():
+        if isinstance(v, np.ndarray):
+            assert v.tobytes() == h[k].tobytes(), k
+    hb = pd.HostBuffers(mixed)
     pd.simulate_host(pd.Card("cms_like"), hb, 31)
-    assert int(hb.to_numpy()["trk_offsets"][-1]) > 0
+    ref = run_gpu("cms_like", mixed, 31, debug=False)
+    for k, v in hb.to_numpy().items():
+        assert v.tobytes() == ref[k].tobytes(), k
 
 
 def test_card_file_variants_and_multiply_charged_particles(tmp_path):

@@ -80,28 +80,47 @@ def test_edge_cases_capacity_and_batching():
         assert np.concatenate([a[k], b[k]]).tobytes() == full[k].tobytes(), k
 
 
-def test_merged_batch_through_the_chain():
-    """Pile-up merging feeding pd_simulate on the device, against the oracle chain on the oracle's merged batch."""
+@pytest.mark.parametrize("mu,n_hs", [(30.0, 60), (200.0, 24), (500.0, 10)])
+def test_merged_batch_through_the_chain(mu, n_hs):
+    """Pile-up merging feeding pd_simulate on the device, against the oracle chain on the oracle's merged batch.  At a
+    mean pile-up of 200 ("PU200") and 500 the merged events hold ~8,000 and ~20,000 particles: beyond what an SM holds
+    on chip, they take the chain's big-tile path (the paper's own benchmark runs with pile-up merging on)."""
     import paper_2606_26089_b200 as pd
     from oracle import pdo
     from parity import compare
 
-    hs = wl.generate(0, 60)
+    hs = wl.generate(0, n_hs)
     pool = wl.generate(3, 500)
-    out, status = _gpu(hs, pool, 30.0, seed=13)
+    out, status = _gpu(hs, pool, mu, seed=13)
     assert status == 0
     g = out.to_numpy()
-    ref = pdo.pileup_merge(hs, pool, 30.0, seed=13)
+    ref = pdo.pileup_merge(hs, pool, mu, seed=13)
     _compare(g, ref)
+    if mu >= 200.0:
+        assert np.diff(ref["offsets"]).max() > 6000
     card = pd.Card("cms_like")
     dev = out.as_events()
     res = pd.DeviceOutputs(card, dev.n_events, dev.n_particles, debug=True)
     pd.simulate(card, dev, res, 13)
     got = res.to_numpy()
     assert pd.last_status(res) == 0
-    # the comparator runs the oracle chain on the ORACLE's merged batch (no oracle input comes from the CUDA path);
-    # the GPU chain saw vz values that differ from it by at most an ulp or so (checked above)
+    # the comparator runs the oracle chain on the ORACLE's merged batch (no oracle input comes from the CUDA path)
     merged = wl.Events(offsets=ref["offsets"], **{k: ref[k] for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
-    rep = compare("cms_like", merged, 13, got)
-    assert rep["unexcused"] == 0, rep["problems"][:5]
+    if mu < 100.0:
+        # the GPU chain saw vz values that differ from the oracle's by at most an ulp or so (checked above)
+        rep = compare("cms_like", merged, 13, got)
+        assert rep["unexcused"] == 0, rep["problems"][:5]
+    else:
+        # With ~1e5 particles some looper turns thousands of radians before the endcap, and an ulp of vz moves its hit by
+        # more than the tolerance: the strict comparison is made on the oracle's merged batch, uploaded as it is; the
+        # device-resident GPU-merged batch must give the same collections up to those few particles.
+        from gpu_util import run_gpu
+
+        strict = run_gpu("cms_like", merged, 13)
+        assert strict["status_word"] == 0
+        rep = compare("cms_like", merged, 13, strict)
+        assert rep["unexcused"] == 0, rep["problems"][:5]
+        assert rep["overridden_particles"] <= max(3, 5e-4 * rep["n_particles"])
+        for k in ("trk_offsets", "tow_offsets", "efl_offsets"):
+            assert np.abs(got[k].astype(np.int64) - strict[k]).max() <= 5, k
     assert int(got["trk_offsets"][-1]) > 0 and int(got["efl_offsets"][-1]) > int(got["trk_offsets"][-1])
