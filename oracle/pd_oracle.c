@@ -17,6 +17,7 @@
 #define PDO_MAX_EFF_ROWS 32
 #define PDO_PI 3.14159265358979323846
 #define PDO_TWO_PI 6.28318530717958647692
+#define PDO_MAX_RES_ROWS 8
 #define PDO_REL_TOL 1e-6 /* near-edge band of BASELINE.json north_star / SURVEY 8c.4 */
 
 struct pdo_card {
@@ -38,6 +39,11 @@ struct pdo_card {
   double trk_a_species[4], trk_b_species[4];
   double ecal[3], hcal[3]; /* (C, S, N): sigma = sqrt(C^2 E^2 + S^2 E + N^2)  (reading A20)   */
   double thr_ecal, thr_hcal;
+  /* higher card fidelity (readings K1-K3 of DESIGN.md section 17) */
+  int n_ecal_eta, n_hcal_eta;            /* K1: rows (aeta_lo, aeta_hi, C, S, N) by the tower centre's |eta|  */
+  double ecal_eta[PDO_MAX_RES_ROWS][5], hcal_eta[PDO_MAX_RES_ROWS][5];
+  double nsig_ecal, nsig_hcal;           /* K2: component kept iff also E' > n_sigma sigma(E')                  */
+  int smear_center;                      /* K3: reported tower (eta, phi) uniform inside the cell               */
 };
 
 /* reading A28: every card number is rounded to fp32 at load; the oracle uses the promoted value */
@@ -90,6 +96,16 @@ static void card_finish(pdo_card *c) {
   }
   c->thr_ecal = f32(c->thr_ecal);
   c->thr_hcal = f32(c->thr_hcal);
+  for (i = 0; i < c->n_ecal_eta; ++i) {
+    int k;
+    for (k = 0; k < 5; ++k) c->ecal_eta[i][k] = f32(c->ecal_eta[i][k]);
+  }
+  for (i = 0; i < c->n_hcal_eta; ++i) {
+    int k;
+    for (k = 0; k < 5; ++k) c->hcal_eta[i][k] = f32(c->hcal_eta[i][k]);
+  }
+  c->nsig_ecal = f32(c->nsig_ecal);
+  c->nsig_hcal = f32(c->nsig_hcal);
 }
 
 /* the three efficiency rows of BASELINE.json configs[0] in reading A8 */
@@ -231,6 +247,11 @@ static int card_from_file(pdo_card *c, const char *path) {
       c->has_trk_species[(int)v[2]] = 1, c->trk_a_species[(int)v[2]] = v[0], c->trk_b_species[(int)v[2]] = v[1];
     else if (!strcmp(key, "ecal_res") && nv == 3) memcpy(c->ecal, v, 3 * sizeof(double));
     else if (!strcmp(key, "hcal_res") && nv == 3) memcpy(c->hcal, v, 3 * sizeof(double));
+    else if (!strcmp(key, "ecal_res_eta") && nv == 5 && c->n_ecal_eta < PDO_MAX_RES_ROWS) memcpy(c->ecal_eta[c->n_ecal_eta++], v, 5 * sizeof(double));
+    else if (!strcmp(key, "hcal_res_eta") && nv == 5 && c->n_hcal_eta < PDO_MAX_RES_ROWS) memcpy(c->hcal_eta[c->n_hcal_eta++], v, 5 * sizeof(double));
+    else if (!strcmp(key, "ecal_nsigma") && nv == 1) c->nsig_ecal = v[0];
+    else if (!strcmp(key, "hcal_nsigma") && nv == 1) c->nsig_hcal = v[0];
+    else if (!strcmp(key, "smear_tower_center") && nv == 1) c->smear_center = v[0] != 0.0;
     else if (!strcmp(key, "ecal_thr") && nv == 1) c->thr_ecal = v[0];
     else if (!strcmp(key, "hcal_thr") && nv == 1) c->thr_hcal = v[0];
     else if (!strcmp(key, "eff") && (nv == 5 || (nv == 6 && (v[5] == 0.0 || v[5] == 1.0 || v[5] == 2.0 || v[5] == 3.0))) &&
@@ -362,6 +383,15 @@ double pdo_lognormal(double m, double s, double z) {
 
 static double resolution(const double csn[3], double E) {
   return sqrt(csn[0] * csn[0] * E * E + csn[1] * csn[1] * E + csn[2] * csn[2]);
+}
+
+/* reading K1: (C, S, N) of a tower = the first row whose [aeta_lo, aeta_hi) holds the |eta| of the tower CENTRE, else the
+ * card's common line */
+static const double *resolution_row(const double dflt[3], const double rows[][5], int n_rows, double aeta_c) {
+  int r;
+  for (r = 0; r < n_rows; ++r)
+    if (aeta_c >= rows[r][0] && aeta_c < rows[r][1]) return rows[r] + 2;
+  return dflt;
 }
 
 /* ------------------------------------------------------------------ grid ------------------- */
@@ -672,6 +702,34 @@ static int above_thr(double value, double thr, double scale, int forced, int *ne
   return res;
 }
 
+/* reading K2 on top of A22: the smeared component is kept iff E' > thr AND E' > n_sigma sigma(E'), sigma taken at the
+ * smeared energy; near if either comparison is (n_sigma = 0 leaves A22 as it was) */
+static int component_kept(double Es, double thr, const double csn[3], double nsig, int forced, int *near) {
+  const double cut = nsig > 0.0 ? nsig * resolution(csn, Es) : 0.0;
+  int res = Es > thr && (nsig <= 0.0 || Es > cut);
+  *near = fabs(Es - thr) <= 1e-5 * fmax(thr, Es) || (nsig > 0.0 && Es > 0.0 && fabs(Es - cut) <= 1e-5 * fmax(cut, Es));
+  if (forced >= 0 && *near) res = forced;
+  return res;
+}
+
+/* reading K3: the reported position of a tower, uniform inside its cell (Philox stream 4, object = tower id: word 0 ->
+ * eta or theta, word 1 -> phi); smear_center = 0: the cell centre */
+int pdo_tower_position(const pdo_card *c, uint64_t seed, int64_t event, int32_t tower, double *eta, double *phi) {
+  int i, j;
+  uint32_t r[4];
+  double x;
+  if (!c || tower < 0 || tower >= c->n_towers) return PDO_EINVAL;
+  if (!c->smear_center) return pdo_tower_centre(c, tower, eta, phi);
+  for (i = c->n_bins - 1; i > 0; --i)
+    if (c->offset[i] <= tower) break;
+  j = tower - c->offset[i];
+  pdo_rng_block(seed, event, (uint32_t)tower, 4u, r);
+  x = c->edges[i] + pdo_uniform(r[0]) * (c->edges[i + 1] - c->edges[i]);
+  if (eta) *eta = c->grid_coord ? -log(tan(0.5 * x)) : x;
+  if (phi) *phi = -PDO_PI + ((double)j + pdo_uniform(r[1])) * (PDO_TWO_PI / (double)c->nphi[i]);
+  return PDO_OK;
+}
+
 int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t event_base,
                  pdo_tracks *trk, pdo_towers *tow, pdo_eflow *efl, pdo_debug *dbg,
                  const pdo_overrides *ov) {
@@ -834,11 +892,16 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
         }
       }
       pdo_rng_block(seed, event, (uint32_t)id, 1u, r);
-      em_s = pdo_lognormal(Eem[id], resolution(c->ecal, Eem[id]), pdo_normal(r[0], r[1]));
-      had_s = pdo_lognormal(Ehad[id], resolution(c->hcal, Ehad[id]), pdo_normal(r[2], r[3]));
-      /* reading A22: the threshold is applied twice, strictly, per component */
-      em_f = above_thr(em_s, c->thr_ecal, fmax(c->thr_ecal, em_s), forced[0], &nr[0]) ? em_s : 0.0;
-      had_f = above_thr(had_s, c->thr_hcal, fmax(c->thr_hcal, had_s), forced[1], &nr[1]) ? had_s : 0.0;
+      pdo_tower_centre(c, id, &eta_c, &phi_c);
+      {
+        const double *ecal = resolution_row(c->ecal, c->ecal_eta, c->n_ecal_eta, fabs(eta_c));
+        const double *hcal = resolution_row(c->hcal, c->hcal_eta, c->n_hcal_eta, fabs(eta_c));
+        em_s = pdo_lognormal(Eem[id], resolution(ecal, Eem[id]), pdo_normal(r[0], r[1]));
+        had_s = pdo_lognormal(Ehad[id], resolution(hcal, Ehad[id]), pdo_normal(r[2], r[3]));
+        /* reading A22 (+ K2): the threshold is applied twice, strictly, per component */
+        em_f = component_kept(em_s, c->thr_ecal, ecal, c->nsig_ecal, forced[0], &nr[0]) ? em_s : 0.0;
+        had_f = component_kept(had_s, c->thr_hcal, hcal, c->nsig_hcal, forced[1], &nr[1]) ? had_s : 0.0;
+      }
       n_em = em_f - Tem[id];
       n_had = had_f - Thad[id];
       is_ph = above_thr(n_em, c->thr_ecal, fmax(c->thr_ecal, fmax(em_f, Tem[id])), forced[2], &nr[2]);
@@ -862,7 +925,7 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
         if (dbg->tw_near) dbg->tw_near[n_dbg_tw] = tw_near;
         ++n_dbg_tw;
       }
-      pdo_tower_centre(c, id, &eta_c, &phi_c);
+      pdo_tower_position(c, seed, event, id, &eta_c, &phi_c);
       if (em_f + had_f > 0.0) {
         if (n_tow >= tow->capacity) {
           rc = PDO_ECAPACITY;
@@ -895,7 +958,7 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
       int is_photon = t < n_ph;
       int32_t id = is_photon ? ph_id[t] : nh_id[t - n_ph];
       double En = is_photon ? ph_E[t] : nh_E[t - n_ph], eta_c, phi_c;
-      pdo_tower_centre(c, id, &eta_c, &phi_c);
+      pdo_tower_position(c, seed, event, id, &eta_c, &phi_c);
       efl->cls[n_efl] = (int8_t)(is_photon ? PDO_CLS_PHOTON : PDO_CLS_NEUHAD);
       efl->src[n_efl] = id;
       efl->pt[n_efl] = En / cosh(eta_c);

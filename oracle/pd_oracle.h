@@ -134,6 +134,9 @@ int pdo_card_info(const pdo_card *card, pdo_card_info_t *out);
 int pdo_card_grid(const pdo_card *card, double *edges, int32_t *nphi, int32_t *offset);
 /* tower centre (eta_c, phi_c) of a tower id; returns PDO_EINVAL if out of range */
 int pdo_tower_centre(const pdo_card *card, int32_t tower, double *eta_c, double *phi_c);
+/* reading K3: the reported position of a tower -- uniform inside the cell if the card says
+ * smear_tower_center = 1 (Philox stream 4, object = tower id), else the centre */
+int pdo_tower_position(const pdo_card *card, uint64_t seed, int64_t event, int32_t tower, double *eta, double *phi);
 
 int pdo_simulate(const pdo_card *card, const pdo_events *ev, uint64_t seed, int64_t event_base,
                  pdo_tracks *tracks, pdo_towers *towers, pdo_eflow *eflow, pdo_debug *debug,

@@ -84,6 +84,7 @@ def lib():
         L.pdo_card_info.argtypes = [_p, C.POINTER(_CardInfo)]
         L.pdo_card_grid.argtypes = [_p, _p, _p, _p]
         L.pdo_tower_centre.argtypes = [_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.pdo_tower_position.argtypes = [_p, C.c_uint64, C.c_int64, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.pdo_simulate.argtypes = [_p, C.POINTER(_Events), C.c_uint64, C.c_int64, C.POINTER(_Tracks),
                                    C.POINTER(_Towers), C.POINTER(_EFlow), C.POINTER(_Debug),
                                    C.POINTER(_Overrides)]
@@ -216,6 +217,14 @@ def normal(xa, xb):
 
 def lognormal(m, s, z):
     return lib().pdo_lognormal(float(m), float(s), float(z))
+
+
+def tower_position(card: Card, seed: int, event: int, tower: int):
+    """Reported (eta, phi) of a tower: uniform inside the cell if the card smears tower centres (reading K3)."""
+    e, p = C.c_double(), C.c_double()
+    if lib().pdo_tower_position(card._h, int(seed), int(event), int(tower), C.byref(e), C.byref(p)) != PDO_OK:
+        raise OracleError(PDO_EINVAL)
+    return e.value, p.value
 
 
 def simulate(card: Card, ev, seed: int, event_base: int = 0, overrides: dict | None = None,

@@ -1,0 +1,143 @@
+"""Pins of the oracle's higher-card-fidelity steps (readings K1-K3 of DESIGN.md section 17):
+eta-dependent calorimeter resolutions, the significance cut, tower positions smeared inside the cell.
+Closed forms, limiting cases that reduce to the plain card, and statistics -- no formula of the oracle is retyped."""
+import importlib
+import math
+
+import numpy as np
+import pytest
+import scipy.stats
+
+import cards
+from oracle import pdo
+
+wl = importlib.import_module("workloads.generate")
+P = wl.particle
+
+
+def _photons(etas, E=40.0, n_events=1):
+    """n_events identical events of photons from the origin, one per eta, all at phi = 0.3: each alone in its tower."""
+    ev = [[P(22, 0, E / math.cosh(eta), eta, 0.3, 0.0) for eta in etas] for _ in range(n_events)]
+    return wl.from_lists(ev)
+
+
+def test_eta_rows_pick_the_row_of_the_tower_centre(tmp_path):
+    b = pdo.Card("cms_like")
+    # K1: rows that repeat the common line change nothing, bit for bit
+    same = cards.variant(tmp_path / "same.card", b.edges, b.nphi, ecal_res_eta=[(0.0, 1.5, 0.007, 0.07, 0.35), (1.5, 9.0, 0.007, 0.07, 0.35)],
+                         hcal_res_eta=[(0.0, 9.0, 0.05, 1.5, 0.0)])
+    ev = wl.generate(0, 60)
+    ref, got = pdo.simulate(b, ev, 3), pdo.simulate(pdo.Card(same), ev, 3)
+    for k in ref:
+        assert got[k].tobytes() == ref[k].tobytes(), k
+    # a row with zero resolution for |eta_c| in [0.5, 1.5): towers there come out UNSMEARED (E' = E exactly: reading A21,
+    # s <= 0), towers elsewhere are smeared; the interval is half open and is tested on the tower CENTRE, not on the hit
+    path = cards.variant(tmp_path / "rows.card", b.edges, b.nphi, ecal_res_eta=[(0.5, 1.5, 0.0, 0.0, 0.0)], ecal_thr=0.0)
+    # 0.087-wide bins: 0.51 lies in [0.435, 0.522), centre 0.4785 (outside the row although the hit is inside); 1.49 lies in
+    # [1.479, 1.566), centre 1.5225 (outside although the hit is inside)
+    etas = [0.02, 0.51, 0.53, 0.9, 1.45, 1.49, -0.7, -1.6, 2.5]
+    ev = _photons(etas)
+    o = pdo.simulate(pdo.Card(path), ev, 5)
+    assert len(o["tow_tower"]) == len(etas)
+    n_in = 0
+    for k, eta in enumerate(etas):
+        i = int(np.searchsorted(b.edges, np.float32(eta), side="right") - 1)
+        centre = 0.5 * (float(b.edges[i]) + float(b.edges[i + 1]))
+        sel = np.nonzero(np.abs(o["tow_eta"] - centre) < 1e-9)[0]
+        assert sel.size == 1
+        inside = 0.5 <= abs(centre) < 1.5
+        n_in += inside
+        assert (float(o["tow_E"][sel[0]]) == float(ev.E[k])) == inside, (eta, centre)
+    assert n_in == 4
+
+
+def test_eta_rows_give_the_rows_resolution(tmp_path):
+    """Sample standard deviation of E'/E over many events = sigma_row(E)/E, row by row (4 sigma of the estimator)."""
+    b = pdo.Card("cms_like")
+    rows = [(0.0, 1.0, 0.10, 0.0, 0.0), (1.0, 2.0, 0.0, 0.632455532, 0.0), (2.0, 9.0, 0.0, 0.0, 4.0)]  # 10 %, 0.632/sqrt(E), 4 GeV
+    path = cards.variant(tmp_path / "res.card", b.edges, b.nphi, hcal_res_eta=rows, hcal=(0.5, 0.0, 0.0), hcal_thr=0.0)
+    n_ev, E = 4000, 40.0
+    ev = wl.from_lists([[P(130, 0, E / math.cosh(eta), eta, 0.3, 0.0) for eta in (0.3, 1.5, 2.4)] for _ in range(n_ev)])
+    o = pdo.simulate(pdo.Card(path), ev, 11)
+    for k, eta in enumerate((0.3, 1.5, 2.4)):
+        i = int(np.searchsorted(b.edges, np.float32(eta), side="right") - 1)
+        centre = 0.5 * (float(b.edges[i]) + float(b.edges[i + 1]))
+        sel = np.abs(o["tow_eta"] - centre) < 1e-9
+        Ein = float(ev.E[k])
+        ratio = o["tow_Ehad"][sel] / Ein
+        assert ratio.shape[0] == n_ev
+        rel = (0.10, 0.632455532 / math.sqrt(Ein), 4.0 / Ein)[k]  # C; S / sqrt(E); N / E
+        assert abs(ratio.mean() - 1.0) < 4.0 * rel / math.sqrt(n_ev)
+        assert abs(ratio.std() - rel) < 4.0 * rel / math.sqrt(2.0 * n_ev), (k, ratio.std(), rel)
+
+
+def test_significance_cut_closed_forms(tmp_path):
+    b = pdo.Card("cms_like")
+    ev = wl.generate(0, 80)
+    # sigma = 0.5 E': E' > n 0.5 E' <=> n < 2 -- just below keeps every HCAL component the plain card keeps, just above none
+    for nsig, keeps in ((1.9, True), (2.1, False)):
+        path = cards.variant(tmp_path / ("s%g.card" % nsig), b.edges, b.nphi, hcal=(0.5, 0.0, 0.0), hcal_nsigma=nsig)
+        plain = cards.variant(tmp_path / ("p%g.card" % nsig), b.edges, b.nphi, hcal=(0.5, 0.0, 0.0))
+        o, ref = pdo.simulate(pdo.Card(path), ev, 7), pdo.simulate(pdo.Card(plain), ev, 7)
+        if keeps:
+            for k in ref:
+                assert o[k].tobytes() == ref[k].tobytes(), k
+        else:
+            assert (o["tow_Ehad"] == 0).all() and not (o["efl_cls"] == 3).any()
+            assert np.array_equal(o["tow_Eem"], ref["tow_Eem"][ref["tow_Eem"] > 0])  # the ECAL side is untouched
+    # sigma = S sqrt(E'): E' > n S sqrt(E') <=> E' > n^2 S^2 = 2.25 GeV for n = 3, S = 0.5 -- an energy threshold
+    path = cards.variant(tmp_path / "sq.card", b.edges, b.nphi, hcal=(0.0, 0.5, 0.0), hcal_nsigma=3.0, hcal_thr=1.0)
+    as_thr = cards.variant(tmp_path / "thr.card", b.edges, b.nphi, hcal=(0.0, 0.5, 0.0), hcal_thr=2.25)
+    o, ref = pdo.simulate(pdo.Card(path), ev, 9), pdo.simulate(pdo.Card(as_thr), ev, 9)
+    assert np.array_equal(o["tow_tower"], ref["tow_tower"]) and o["tow_Ehad"].tobytes() == ref["tow_Ehad"].tobytes()
+    had = o["tow_Ehad"]
+    assert (had[had > 0] > 2.25).all() and (o["tow_Ehad"] > 0).sum() < (pdo.simulate(pdo.Card(
+        cards.variant(tmp_path / "no.card", b.edges, b.nphi, hcal=(0.0, 0.5, 0.0))), ev, 9)["tow_Ehad"] > 0).sum()
+    # the neutral-hadron threshold itself stays hcal_thr = 1.0 (the cut acts on the tower component, reading K2)
+    nh = o["efl_E"][o["efl_cls"] == 3]
+    assert nh.size > 0 and nh.min() > 1.0
+
+
+@pytest.mark.parametrize("name", ["cms_like", "aleph_like"])
+def test_tower_positions_uniform_inside_the_cell(name, tmp_path):
+    b = pdo.Card(name)
+    path = cards.variant(tmp_path / "c.card", b.edges, b.nphi, base=name, smear_tower_center=1)
+    card = pdo.Card(path)
+    cfg = 0 if name == "cms_like" else 4
+    ev = wl.generate(cfg, 400)
+    o, ref = pdo.simulate(card, ev, 21), pdo.simulate(b, ev, 21)
+    # K3 moves the reported position only: same towers, same energies, same neutrals
+    for k in ("tow_tower", "tow_E", "tow_Eem", "tow_Ehad", "efl_cls", "efl_src", "efl_E", "trk_pt"):
+        assert o[k].tobytes() == ref[k].tobytes(), k
+    edges = np.asarray(b.edges, dtype=np.float64)
+    nphi = np.asarray(b.nphi)
+    off = np.concatenate([[0], np.cumsum(nphi)])
+    i = np.searchsorted(off, o["tow_tower"], side="right") - 1
+    j = o["tow_tower"] - off[i]
+    coord = o["tow_eta"] if name == "cms_like" else 2.0 * np.arctan(np.exp(-o["tow_eta"]))
+    u1 = (coord - edges[i]) / (edges[i + 1] - edges[i])
+    u2 = (o["tow_phi"] + math.pi) / (2.0 * math.pi / nphi[i]) - j
+    assert (u1 >= -1e-9).all() and (u1 < 1 + 1e-9).all() and (u2 >= -1e-9).all() and (u2 < 1 + 1e-9).all()
+    assert scipy.stats.kstest(np.clip(u1, 0, 1), "uniform").pvalue > 1e-4
+    assert scipy.stats.kstest(np.clip(u2, 0, 1), "uniform").pvalue > 1e-4
+    assert abs(np.corrcoef(u1, u2)[0, 1]) < 4.0 / math.sqrt(u1.size)
+    # ET and the neutrals' pT follow the reported position: pT = E / cosh(eta)
+    assert np.allclose(o["tow_ET"], o["tow_E"] / np.cosh(o["tow_eta"]), rtol=1e-12)
+    neu = o["efl_cls"] >= 3
+    assert np.allclose(o["efl_pt"][neu], o["efl_E"][neu] / np.cosh(o["efl_eta"][neu]), rtol=1e-12)
+    # one draw per (seed, event, tower): the Tower and its neutrals sit at the same point; another seed moves it
+    tow_ev = np.repeat(np.arange(400), np.diff(o["tow_offsets"]))
+    efl_ev = np.repeat(np.arange(400), np.diff(o["efl_offsets"]))
+    pos = {(int(e), int(t)): (float(a), float(p)) for e, t, a, p in zip(tow_ev, o["tow_tower"], o["tow_eta"], o["tow_phi"])}
+    n_checked = 0
+    for e, t, a, p, c in zip(efl_ev, o["efl_src"], o["efl_eta"], o["efl_phi"], o["efl_cls"]):
+        if c >= 3 and (int(e), int(t)) in pos:
+            assert pos[(int(e), int(t))] == (float(a), float(p))
+            n_checked += 1
+    assert n_checked > 100
+    other = pdo.simulate(card, ev, 22)
+    assert not np.array_equal(other["tow_eta"][:50], o["tow_eta"][:50])
+    # the library entry point gives the same position, and the centre when the card does not smear
+    e0, t0 = int(tow_ev[5]), int(o["tow_tower"][5])
+    assert pdo.tower_position(card, 21, e0, t0) == (float(o["tow_eta"][5]), float(o["tow_phi"][5]))
+    assert pdo.tower_position(b, 21, e0, t0) == b.tower_centre(t0)
