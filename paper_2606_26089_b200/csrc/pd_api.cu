@@ -338,7 +338,7 @@ int pd_card_to_device(const pd_card *c) {
   }
   const size_t nb = (size_t)c->sc.n_bins;
   const size_t lut_words = (c->lut.size() + 1) / 2;
-  const size_t words = (nb + 1) + nb + (nb + 1) + 5 * nb + lut_words;
+  const size_t words = (nb + 1) + nb + (nb + 1) + 5 * nb + lut_words + (nb + 1) + 6 * nb;
   std::vector<uint32_t> blob(words);
   size_t o = 0;
   auto put = [&](const void *src, size_t n) {
@@ -353,6 +353,7 @@ int pd_card_to_device(const pd_card *c) {
   const size_t o_lut = o;
   std::memcpy(blob.data() + o, c->lut.data(), 2 * c->lut.size());
   o += lut_words;
+  const size_t o_edge = put(c->edges.data(), nb + 1), o_res2 = put(c->res2.data(), 6 * nb);
   void *d = nullptr;
   PD_CUDA(cudaMalloc(&d, 4 * words));
   cudaError_t e = cudaMemcpy(d, blob.data(), 4 * words, cudaMemcpyHostToDevice);
@@ -370,6 +371,8 @@ int pd_card_to_device(const pd_card *c) {
   c->dev_tab.eta_c = (const float *)(base + o_eta);
   c->dev_tab.inv_cosh = (const float *)(base + o_ic);
   c->dev_tab.lut = (const unsigned short *)(base + o_lut);
+  c->dev_tab.edge = (const float *)(base + o_edge);
+  c->dev_tab.res2 = (const float *)(base + o_res2);
   c->dev_blob = d;
   c->dev_id = dev;
   return PD_OK;

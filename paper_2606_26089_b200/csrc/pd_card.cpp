@@ -34,6 +34,9 @@ struct RawCard {
   double trk_a_sp[4] = {0, 0, 0, 0}, trk_b_sp[4] = {0, 0, 0, 0};
   double ecal[3] = {0, 0, 0}, hcal[3] = {0, 0, 0};
   double thr_ecal = 0.5, thr_hcal = 1.0;
+  std::vector<std::array<double, 5>> ecal_eta, hcal_eta;  // reading K1: aeta_lo, aeta_hi, C, S, N
+  double nsig_ecal = 0, nsig_hcal = 0;                    // reading K2
+  bool smear_center = false;                              // reading K3
 };
 
 constexpr double kPi = 3.14159265358979323846;
@@ -134,6 +137,11 @@ bool from_file(RawCard &r, const char *path) {
       r.has_trk_sp[int(v[2])] = true, r.trk_a_sp[int(v[2])] = v[0], r.trk_b_sp[int(v[2])] = v[1];
     else if (key == "ecal_res" && v.size() == 3) std::copy(v.begin(), v.end(), r.ecal);
     else if (key == "hcal_res" && v.size() == 3) std::copy(v.begin(), v.end(), r.hcal);
+    else if (key == "ecal_res_eta" && v.size() == 5 && r.ecal_eta.size() < 8) r.ecal_eta.push_back({{v[0], v[1], v[2], v[3], v[4]}});
+    else if (key == "hcal_res_eta" && v.size() == 5 && r.hcal_eta.size() < 8) r.hcal_eta.push_back({{v[0], v[1], v[2], v[3], v[4]}});
+    else if (key == "ecal_nsigma" && v.size() == 1) r.nsig_ecal = v[0];
+    else if (key == "hcal_nsigma" && v.size() == 1) r.nsig_hcal = v[0];
+    else if (key == "smear_tower_center" && v.size() == 1) r.smear_center = v[0] != 0.0;
     else if (key == "ecal_thr" && v.size() == 1) r.thr_ecal = v[0];
     else if (key == "hcal_thr" && v.size() == 1) r.thr_hcal = v[0];
     else if (key == "eff" && (v.size() == 5 || (v.size() == 6 && (v[5] == 0.0 || v[5] == 1.0 || v[5] == 2.0 || v[5] == 3.0))) &&
@@ -185,6 +193,10 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     for (double e : r.edges)
       if (!fin(e)) return PD_ECARD;
     if (r.theta && !(r.edges.front() >= 0.0 && r.edges.back() <= kPi)) return PD_ECARD;
+    if (!nonneg(r.nsig_ecal) || !nonneg(r.nsig_hcal)) return PD_ECARD;
+    for (const auto *rows : {&r.ecal_eta, &r.hcal_eta})
+      for (const auto &row : *rows)
+        if (!(nonneg(row[0]) && row[1] > row[0] && nonneg(row[2]) && nonneg(row[3]) && nonneg(row[4]))) return PD_ECARD;
     for (const auto &row : r.eff) {
       // pt_lo < pt_hi, |eta|_lo < |eta|_hi (the upper ends may be +inf), 0 <= eps <= 1
       if (!(nonneg(row[0]) && row[1] > row[0] && nonneg(row[2]) && row[3] > row[2])) return PD_ECARD;
@@ -320,6 +332,28 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     c->inv_cosh[i] = float(1.0 / std::cosh(eta));
   }
   c->offset[nb] = acc;
+  // readings K1-K3: per-bin resolutions (the first row whose [aeta_lo, aeta_hi) holds |eta| of the bin's tower centres,
+  // else the card's common line), significance cut, smeared tower positions
+  s.res_per_bin = (!r.ecal_eta.empty() || !r.hcal_eta.empty()) ? 1 : 0;
+  c->res2.assign(6 * nb, 0.f);
+  for (size_t i = 0; i < nb; ++i) {
+    const double mid = 0.5 * (double(c->edges[i]) + double(c->edges[i + 1]));
+    const double aeta = std::fabs(r.theta ? -std::log(std::tan(0.5 * mid)) : mid);
+    auto pick = [&](const std::vector<std::array<double, 5>> &rows, const double *dflt, float *out) {
+      const double *csn = dflt;
+      for (const auto &row : rows)
+        if (aeta >= f32(row[0]) && aeta < f32(row[1])) {
+          csn = row.data() + 2;
+          break;
+        }
+      for (int k = 0; k < 3; ++k) out[k] = float(f32(csn[k]) * f32(csn[k]));
+    };
+    pick(r.ecal_eta, r.ecal, &c->res2[6 * i]);
+    pick(r.hcal_eta, r.hcal, &c->res2[6 * i + 3]);
+  }
+  s.nsig2_ecal = float(f32(r.nsig_ecal) * f32(r.nsig_ecal));
+  s.nsig2_hcal = float(f32(r.nsig_hcal) * f32(r.nsig_hcal));
+  s.smear_center = r.smear_center ? 1 : 0;
   s.tb_first = c->tb[0], s.tb_last = c->tb[nb];
 
   // ---- eta-bin lookup: cells of |u| by float bits (2^(23 - PD_LUT_SHIFT) cells per octave, |u| < 2^MIN_EXP in

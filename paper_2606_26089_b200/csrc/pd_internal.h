@@ -44,6 +44,10 @@ struct PdCardScalars {
   int eff_per_species;        // 0: no efficiency row names a species (the three grids are equal)
   float ecal2[3], hcal2[3];  // C^2, S^2, N^2 of sigma^2 = C^2 E^2 + S^2 E + N^2
   float thr_ecal, thr_hcal;
+  // higher card fidelity (readings K1-K3)
+  int res_per_bin;                // K1: the card has eta-dependent resolution rows: C^2, S^2, N^2 per eta bin (PdCardTables::res2)
+  float nsig2_ecal, nsig2_hcal;   // K2: n_sigma^2 of the significance cut (0: none)
+  int smear_center;               // K3: reported tower position uniform inside the cell (Philox stream 4)
 };
 
 // Per-bin tables, contiguous in one device allocation.
@@ -57,6 +61,8 @@ struct PdCardTables {
   const float *eta_c;     // [n_bins] tower-centre pseudorapidity
   const float *inv_cosh;  // [n_bins] 1 / cosh(eta_c)
   const unsigned short *lut;  // [2 * lut_side] first candidate bin of a cell
+  const float *edge;      // [n_bins+1] the card's edges (eta or theta), fp32
+  const float *res2;      // [n_bins][6] ECAL C^2, S^2, N^2, HCAL C^2, S^2, N^2 of the bin's towers (reading K1)
 };
 
 struct pd_card {
@@ -67,6 +73,7 @@ struct pd_card {
   std::vector<float> tb, inv_w, half, w, eta_c, inv_cosh;
   std::vector<int> nphi, offset;
   std::vector<unsigned short> lut;
+  std::vector<float> res2;   // [n_bins][6]
   float bz = 0.f;
   int n_eff_rows = 0;
   // device copy, created lazily by the first simulate call
@@ -83,6 +90,7 @@ struct PdPhiloxKeys {
 // Shared-memory carve-up of kernel T (byte offsets; pd_towers.cu make_layout)
 struct PdTLayout {
   uint32_t offset, w, eta_c, inv_cosh, binlut;  // card tables (what pass O needs)
+  uint32_t res2, edge;                          // K1 / K3 tables (size 0 when the card does not use them)
   uint32_t off32, ntrk, ntow, nph, nnh;         // per-event arrays [G+1]
   uint32_t misc;                                // scratch words
   uint32_t seg;                                 // track segments of the tile [3][64]

@@ -478,12 +478,11 @@ __device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, f
 
 // per-tower smear of both components (S6): the common case of a single non-zero component runs one
 // branch-free log-normal; only towers holding both ECAL and HCAL energy take the second
-__device__ __forceinline__ void tower_smear(const PdCardScalars &sc, float Eem, float Ehad, const uint32_t (&rn)[4],
-                                            float &em_s, float &had_s) {
+__device__ __forceinline__ void tower_smear_csn(const float (&ecal2)[3], const float (&hcal2)[3], float Eem, float Ehad,
+                                                const uint32_t (&rn)[4], float &em_s, float &had_s) {
   const bool prim_em = Eem > 0.f;
   const float Ep = prim_em ? Eem : Ehad;
-  const float c2 = prim_em ? sc.ecal2[0] : sc.hcal2[0], s2c = prim_em ? sc.ecal2[1] : sc.hcal2[1],
-              n2 = prim_em ? sc.ecal2[2] : sc.hcal2[2];
+  const float c2 = prim_em ? ecal2[0] : hcal2[0], s2c = prim_em ? ecal2[1] : hcal2[1], n2 = prim_em ? ecal2[2] : hcal2[2];
   const uint32_t xa = prim_em ? rn[0] : rn[2], xb = prim_em ? rn[1] : rn[3];
   float sp = 0.f;
   if (Ep > 0.f) {
@@ -493,7 +492,7 @@ __device__ __forceinline__ void tower_smear(const PdCardScalars &sc, float Eem, 
   }
   em_s = prim_em ? sp : 0.f;
   had_s = prim_em ? 0.f : sp;
-  if (prim_em && Ehad > 0.f) had_s = smear_component(Ehad, sc.hcal2, rn[2], rn[3]);
+  if (prim_em && Ehad > 0.f) had_s = smear_component(Ehad, hcal2, rn[2], rn[3]);
 }
 
 }  // namespace pdk

@@ -50,7 +50,8 @@ using Layout = PdTLayout;
 // Sparse mode (large grids, small events: the bitmaps would be almost empty and take most of the shared memory):
 // `bitmap` holds one bit per 128-tower GROUP and event, `l2p` the rank of the first non-empty group of each of its
 // words, `pool` the tower bits of the non-empty groups only (at most one per deposit), `gprefix` their prefixes.
-__host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int words_per_event, int G, int C, int sparse) {
+__host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int words_per_event, int G, int C, int sparse, int res_per_bin = 0,
+                                              int smear_center = 0) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) {
@@ -63,6 +64,8 @@ __host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int word
   l.eta_c = take(4 * n_bins);
   l.inv_cosh = take(4 * n_bins);
   l.binlut = take(2 * (size_t)((n_towers >> 5) + 2));
+  l.res2 = take(res_per_bin ? 4 * 6 * (size_t)n_bins : 0);
+  l.edge = take(smear_center ? 4 * (size_t)(n_bins + 1) : 0);
   l.off32 = take(4 * (G + 1));
   l.ntrk = take(4 * (G + 1));
   l.ntow = take(4 * (G + 1));
@@ -143,6 +146,54 @@ __device__ __forceinline__ int popc_below(const uint4 &v, int pos) {
   return __popc(v.x & m0) + __popc(v.y & m1) + __popc(v.z & m2) + __popc(v.w & m3);
 }
 
+// ---- higher card fidelity ----------------------------------------------------------------
+// what S6 / S8 need of the card, by value or in shared memory (never a pointer into the kernel parameters)
+struct TCard {
+  const int *offset;             // [n_bins+1]
+  const unsigned short *binlut;  // eta bin of tower ids 0, 32, 64, ...
+  const float *w, *eta_c, *inv_cosh;
+  const float *res2;             // [n_bins][6] (reading K1), only if sc.res_per_bin
+  const float *edge;             // [n_bins+1] (reading K3), only if sc.smear_center
+};
+__device__ __forceinline__ int tower_bin(const TCard &tc, int tower) {
+  int b = (int)tc.binlut[tower >> 5];
+  while (tower >= tc.offset[b + 1]) ++b;
+  return b;
+}
+// S6 of one tower with the resolutions of its eta bin (K1) and the significance cut (K2): smeared components and
+// whether each is kept (reading A22: > threshold; K2: and > n_sigma sigma(E'), i.e. E'^2 > n_sigma^2 sigma^2(E'))
+template <bool FID>
+__device__ __forceinline__ void tower_components(const PdCardScalars &sc, const TCard &tc, int tower, float Eem, float Ehad, const uint32_t (&rn)[4],
+                                                 float &em_s, float &had_s, bool &k_em, bool &k_had) {
+  float e2[3] = {sc.ecal2[0], sc.ecal2[1], sc.ecal2[2]}, h2[3] = {sc.hcal2[0], sc.hcal2[1], sc.hcal2[2]};
+  if (FID && sc.res_per_bin) {
+    const float *r = tc.res2 + 6 * tower_bin(tc, tower);
+    e2[0] = r[0], e2[1] = r[1], e2[2] = r[2], h2[0] = r[3], h2[1] = r[4], h2[2] = r[5];
+  }
+  tower_smear_csn(e2, h2, Eem, Ehad, rn, em_s, had_s);
+  k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
+  if (FID && sc.nsig2_ecal > 0.f) k_em = k_em && em_s * em_s > sc.nsig2_ecal * fmaf(e2[0] * em_s, em_s, fmaf(e2[1], em_s, e2[2]));
+  if (FID && sc.nsig2_hcal > 0.f) k_had = k_had && had_s * had_s > sc.nsig2_hcal * fmaf(h2[0] * had_s, had_s, fmaf(h2[1], had_s, h2[2]));
+}
+// S8: where a tower (and its neutrals) is reported: the cell centre, or (K3) a point uniform inside the cell drawn from
+// Philox stream 4 of (seed, event, tower): word 0 -> eta or theta, word 1 -> phi
+template <bool FID>
+__device__ __forceinline__ void tower_position(const PdCardScalars &sc, const TCard &tc, const PhiloxKeys &rk, long long event, int tower,
+                                               float &eta, float &phi, float &inv_cosh) {
+  const int b = tower_bin(tc, tower);
+  const int j = tower - tc.offset[b];
+  if (!FID || !sc.smear_center) {
+    eta = tc.eta_c[b], phi = fmaf((float)j + 0.5f, tc.w[b], -kPiF), inv_cosh = tc.inv_cosh[b];
+    return;
+  }
+  uint32_t rn[4];
+  rng_block(rk, event, (uint32_t)tower, 4u, rn);
+  const float lo = tc.edge[b], x = fmaf(uniform24(rn[0]), tc.edge[b + 1] - lo, lo);
+  eta = sc.grid_theta ? -logf(tanf(0.5f * x)) : x;
+  phi = fmaf((float)j + uniform24(rn[1]), tc.w[b], -kPiF);
+  inv_cosh = 1.0f / coshf(eta);
+}
+
 // ---- tiles that do not fit on chip ---------------------------------------------------------------------------
 // A tile of the plan (G whole events) whose particles exceed the on-chip capacity C -- one huge event, or a few large
 // ones among the small ones the plan was made for -- takes this path: its events one by one, of ANY size ("no fixed
@@ -159,9 +210,8 @@ struct BigCounts {
 // per-word counts / prefixes, scal[8] scalars.  acc: this CTA's [n_towers][5] accumulators, all zero on entry and exit.
 template <int THREADS, bool DEBUG>
 __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_index, long long pa, long long pb, bool write,
-                                            long long base_trk, long long base_tow, long long base_efl, const int *s_offset,
-                                            const unsigned short *s_binlut, const float *s_w, const float *s_eta_c,
-                                            const float *s_inv_cosh, uint32_t *bmap, unsigned *wcnt, int *scal, long long *acc) {
+                                            long long base_trk, long long base_tow, long long base_efl, const TCard &tc, uint32_t *bmap,
+                                            unsigned *wcnt, int *scal, long long *acc) {
   constexpr int W = THREADS / 32;
   const PdCardScalars &sc = prm.sc;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -243,8 +293,8 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
       uint32_t rn[4];
       rng_block(prm.rk, ev_index, (uint32_t)tower, 1u, rn);
       float em_s, had_s;
-      tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
-      const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
+      bool k_em, k_had;
+      tower_components<true>(sc, tc, tower, Eem, Ehad, rn, em_s, had_s, k_em, k_had);
       const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
       const float n_em = em_f - Tem, n_had = had_f - Thad;
       const bool f_ph = n_em > sc.thr_ecal, f_nh = n_had > sc.thr_hcal, f_tw = em_f + had_f > 0.f;
@@ -307,9 +357,8 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
       if (!flags) continue;
       const float em = __uint_as_float((unsigned)v0), had = __uint_as_float((unsigned)(v0 >> 32));
       const float nem = __uint_as_float((unsigned)v1), nhad = __uint_as_float((unsigned)(v1 >> 32));
-      int bin = (int)s_binlut[tower >> 5];
-      while (tower >= s_offset[bin + 1]) ++bin;
-      const float eta_c = s_eta_c[bin], phi_c = fmaf((float)(tower - s_offset[bin]) + 0.5f, s_w[bin], -kPiF), ic = s_inv_cosh[bin];
+      float eta_c, phi_c, ic;
+      tower_position<true>(sc, tc, prm.rk, ev_index, tower, eta_c, phi_c, ic);
       if (flags & 1) {
         const unsigned at = k_tw++;
         prm.tow_tower[at] = tower, prm.tow_eta[at] = eta_c, prm.tow_phi[at] = phi_c;
@@ -340,9 +389,8 @@ __device__ __noinline__ void big_tile(const PdParams &prm, unsigned char *smem, 
   const PdCardScalars &sc = prm.sc;
   const PdTLayout &L = prm.lay;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int *s_offset = (const int *)(smem + L.offset);
-  const float *s_w = (const float *)(smem + L.w), *s_eta_c = (const float *)(smem + L.eta_c), *s_inv_cosh = (const float *)(smem + L.inv_cosh);
-  const unsigned short *s_binlut = (const unsigned short *)(smem + L.binlut);
+  const TCard tc{(const int *)(smem + L.offset), (const unsigned short *)(smem + L.binlut), (const float *)(smem + L.w),
+                 (const float *)(smem + L.eta_c), (const float *)(smem + L.inv_cosh), (const float *)(smem + L.res2), (const float *)(smem + L.edge)};
   int *s_ntrk = (int *)(smem + L.ntrk), *s_ntow = (int *)(smem + L.ntow), *s_nph = (int *)(smem + L.nph), *s_nnh = (int *)(smem + L.nnh);
   unsigned long long *s_misc = (unsigned long long *)(smem + L.misc);
   unsigned *s_wtot = (unsigned *)(s_misc + 8);
@@ -360,7 +408,7 @@ __device__ __noinline__ void big_tile(const PdParams &prm, unsigned char *smem, 
       }
       for (int e = 0; e < ne; ++e) {
         const BigCounts c = big_event<THREADS, DEBUG>(prm, prm.event_base + e0 + e, prm.offsets[e0 + e], prm.offsets[e0 + e + 1], false, 0, 0, 0,
-                                                      s_offset, s_binlut, s_w, s_eta_c, s_inv_cosh, bmap, wcnt, scal, acc);
+                                                      tc, bmap, wcnt, scal, acc);
         if (tid == 0) s_ntrk[e] = c.trk, s_ntow[e] = c.tow, s_nph[e] = c.ph, s_nnh[e] = c.nh;
         __syncthreads();
       }
@@ -393,12 +441,12 @@ __device__ __noinline__ void big_tile(const PdParams &prm, unsigned char *smem, 
         const int kt = s_ntrk[e], kw = s_ntow[e], kp = s_nph[e], kn = s_nnh[e];
         __syncthreads();  // the scalars above are read before big_event reuses shared memory next to them
         big_event<THREADS, DEBUG>(prm, prm.event_base + e0 + e, prm.offsets[e0 + e], prm.offsets[e0 + e + 1], true, bt + kt, bw + kw,
-                                  bf + kt + kp + kn, s_offset, s_binlut, s_w, s_eta_c, s_inv_cosh, bmap, wcnt, scal, acc);
+                                  bf + kt + kp + kn, tc, bmap, wcnt, scal, acc);
       }
   }
 }
 
-template <int THREADS, int CTAS, bool DEBUG, bool SPARSE>
+template <int THREADS, int CTAS, bool DEBUG, bool SPARSE, bool FID>
 __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_constant__ PdParams prm) {
   constexpr int W = THREADS / 32;
   extern __shared__ __align__(16) unsigned char smem[];
@@ -414,6 +462,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
   float *s_eta_c = (float *)(smem + L.eta_c);
   float *s_inv_cosh = (float *)(smem + L.inv_cosh);
   unsigned short *s_binlut = (unsigned short *)(smem + L.binlut);
+  float *s_res2 = (float *)(smem + L.res2), *s_edge = (float *)(smem + L.edge);
+  const TCard tc{s_offset, s_binlut, s_w, s_eta_c, s_inv_cosh, s_res2, s_edge};
   int *s_off32 = (int *)(smem + L.off32);
   int *s_ntrk = (int *)(smem + L.ntrk);  // tracks of the tile before event e
   int *s_ntow = (int *)(smem + L.ntow);
@@ -447,6 +497,10 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
     s_eta_c[i] = prm.tab.eta_c[i];
     s_inv_cosh[i] = prm.tab.inv_cosh[i];
   }
+  if (sc.res_per_bin)
+    for (int i = tid; i < 6 * nb; i += THREADS) s_res2[i] = prm.tab.res2[i];
+  if (sc.smear_center)
+    for (int i = tid; i <= nb; i += THREADS) s_edge[i] = prm.tab.edge[i];
   __syncthreads();
   // eta bin of tower ids 0, 32, 64, ...: start of the short forward search of pass O
   for (int c = tid; c <= (sc.n_towers >> 5); c += THREADS) {
@@ -699,9 +753,9 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
         uint32_t rn[4];
         rng_block(prm.rk, prm.event_base + e0 + e, (uint32_t)tower, 1u, rn);
         float em_s, had_s;
-        tower_smear(sc, Eem, Ehad, rn, em_s, had_s);
-        // reading A22: the threshold is applied twice, strictly, per component
-        const bool k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
+        bool k_em, k_had;
+        // reading A22: the threshold is applied twice, strictly, per component (K1 / K2: per-bin resolutions, significance)
+        tower_components<FID>(sc, tc, tower, Eem, Ehad, rn, em_s, had_s, k_em, k_had);
         const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
         const float n_em = em_f - Tem, n_had = had_f - Thad;
         f_ph = n_em > sc.thr_ecal, f_nh = n_had > sc.thr_hcal;
@@ -845,12 +899,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
         const float em = s_stg[d], had = s_Ev[h], nem = s_Et[h], nhad = __uint_as_float(s_res[h]);
         const unsigned pa = s_preA[it * W + wid], pb = s_preB[it * W + wid];
         const int e = multi ? (int)s_ev[h] : 0;
-        int b = (int)s_binlut[tower >> 5];
-        while (tower >= s_offset[b + 1]) ++b;
-        const int j = tower - s_offset[b];
-        const float eta_c = s_eta_c[b];
-        const float phi_c = fmaf((float)j + 0.5f, s_w[b], -kPiF);
-        const float ic = s_inv_cosh[b];
+        float eta_c, phi_c, ic;
+        tower_position<FID>(sc, tc, prm.rk, prm.event_base + e0 + e, tower, eta_c, phi_c, ic);
         if (f_tw) {
           const unsigned at = (unsigned)base_tow + (pa & 0xffffu) + (unsigned)__popc(m_tw & lt_mask);
           prm.tow_tower[at] = tower;
@@ -921,7 +971,7 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   const size_t budget2 = (228 * 1024 - 2 * 1024) / 2, budget1 = 227 * 1024;
   int sparse = 0;
   auto cap_for = [&](int G, size_t budget) {
-    const size_t fixed = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, G, 0, sparse).total;
+    const size_t fixed = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, G, 0, sparse, sc.res_per_bin, sc.smear_center).total;
     const size_t per = pdk::T_BYTES_PER_PARTICLE + (G > 1 ? 1 : 0) + (sparse ? 18 : 0);
     long cap = budget > fixed + 7 * 16 ? long((budget - fixed - 7 * 16) / per) : 0;
     cap &= ~3L;
@@ -968,15 +1018,15 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
     const long sms = query_device() == PD_OK ? g_num_sms : 256;
     plan->max_ctas = int(sms * (plan->threads == 1024 ? 1 : 2));
   }
-  plan->lay = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse);
+  plan->lay = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse, sc.res_per_bin, sc.smear_center);
   plan->smem_bytes = plan->lay.total;
   return PD_OK;
 }
 
-template <int THREADS, bool DEBUG, bool SPARSE>
-static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
+template <int THREADS, bool DEBUG, bool SPARSE, bool FID>
+static int launch_variant2(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
   constexpr int CTAS = THREADS == 512 ? 2 : 1;
-  auto kern = pdk::pd_tower_kernel<THREADS, CTAS, DEBUG, SPARSE>;
+  auto kern = pdk::pd_tower_kernel<THREADS, CTAS, DEBUG, SPARSE, FID>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, g_max_smem_optin) != cudaSuccess) return PD_ECUDA;
   // persistent CTAs wait on one another through the look-back chain: the grid must be co-resident
   int per_sm = 0;
@@ -989,6 +1039,13 @@ static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStr
   if (grid < 1) grid = 1;
   kern<<<grid, THREADS, plan.smem_bytes, stream>>>(prm);
   return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
+}
+
+// the variant with the higher-fidelity card options (K1-K3) compiled in only for the cards that use them
+template <int THREADS, bool DEBUG, bool SPARSE>
+static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
+  const bool fid = prm.sc.res_per_bin || prm.sc.smear_center || prm.sc.nsig2_ecal > 0.f || prm.sc.nsig2_hcal > 0.f;
+  return fid ? launch_variant2<THREADS, DEBUG, SPARSE, true>(prm, plan, stream) : launch_variant2<THREADS, DEBUG, SPARSE, false>(prm, plan, stream);
 }
 
 // the two kernels of the chain, back to back on the stream: P (particles -> keys + tracks), then T (towers, EFlow)

@@ -310,6 +310,42 @@ def test_forced_kernel_variants_in_a_subprocess(tmp_path):
         assert out.returncode == 0 and "variant ok" in out.stdout, (env_add, out.stdout[-2000:], out.stderr[-2000:])
 
 
+@pytest.mark.parametrize("base,cfg,ne", [("cms_like", 0, 600), ("cms_like", 1, 200), ("aleph_like", 4, 1500)])
+def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
+    """SURVEY 8f NEXT-3, readings K1-K3: eta-dependent ECAL / HCAL resolutions, the significance cut
+    and tower positions smeared inside the cell -- one at a time and all together, on an eta grid and on a theta grid;
+    and an event too large for the chip (the big-tile path has its own copy of the tower code)."""
+    import cards
+    from gpu_util import run_gpu
+    from oracle import pdo
+    from parity import compare
+
+    b = pdo.Card(base)
+    ecal_rows = [(0.0, 0.8, 0.005, 0.05, 0.2), (0.8, 1.6, 0.01, 0.1, 0.3), (2.0, 3.0, 0.03, 0.2, 0.0)]
+    hcal_rows = [(0.0, 1.3, 0.04, 1.0, 0.0), (1.3, 3.0, 0.06, 1.3, 0.5), (3.0, 9.0, 0.10, 2.0, 1.0)]
+    variants = {
+        "eta_rows": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows),
+        "significance": dict(ecal_nsigma=2.0, hcal_nsigma=1.5),
+        "smeared_centres": dict(smear_tower_center=1),
+        "all": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows, ecal_nsigma=1.0, hcal_nsigma=1.2, smear_tower_center=1),
+    }
+    ev = wl.generate(cfg, ne)
+    if cfg == 0:
+        big = wl.generate(2, 4)
+        big = wl.Events(offsets=np.array([0, big.n_particles], dtype=np.int64),
+                        **{k: getattr(big, k) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
+        ev = wl.concat_events([ev, big, wl.generate(0, 20)])
+    plain = run_gpu(base, ev, 29, debug=False)
+    for name, kw in variants.items():
+        path = cards.variant(tmp_path / (name + ".card"), b.edges, b.nphi, base=base, **kw)
+        gpu = run_gpu(path, ev, 29)
+        assert gpu["status_word"] == 0, name
+        rep = _check(compare(path, ev, 29, gpu))
+        changed = any(gpu[k].shape != plain[k].shape or gpu[k].tobytes() != plain[k].tobytes() for k in ("tow_E", "tow_eta", "efl_E"))
+        assert changed, name  # the card option really is in use
+        print(base, name, {k: rep[k] for k in ("flagged_particles", "overridden_particles", "flagged_towers", "overridden_towers", "neutral_outside_plain_tol")})
+
+
 def test_per_species_card(tmp_path):
     """Per-species efficiency rows and track resolutions on a lepton-rich sample."""
     import cards
