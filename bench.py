@@ -9,10 +9,10 @@ particles), the largest config, on which north_star states the bandwidth target.
 
   value      truth particles/s, whole job (all ranks), device-timed with CUDA events, max over ranks
   e2e        same metric through pd_simulate_host: pinned HOST buffers in and out, copies timed
-  roofline   algorithmic HBM bytes of one launch / its CUDA-event duration, against the measured
-             copy bandwidth in MEASURED_PEAKS.json
-  cpu_baseline  the fp64 oracle (oracle/, as it stands) on a bounded sample of the same workload,
-             one host core
+  roofline   algorithmic HBM bytes of one step (three launches) / its CUDA-event duration, against the
+             measured copy bandwidth in MEASURED_PEAKS.json
+  cpu_baseline  the fp64 oracle (oracle/, as it stands) on a bounded sample of the same workload:
+             one host core, and all host cores (events sharded over worker processes); CPU model stated
 
 N > 1 (torchrun): events are independent, so every rank runs the same-size batch with its own
 event_base (weak scaling, no data-path collective); rank 0 prints.
@@ -83,6 +83,62 @@ def _sample_events(ev, max_particles):
     k = int(np.searchsorted(ev.offsets, max_particles, side="right") - 1)
     k = max(1, min(k, ev.n_events))
     return wl.slice_events(ev, 0, k), k
+
+
+def _cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def _oracle_warm(cfg):
+    from oracle import pdo
+
+    pdo.Card(wl.config_card(cfg))
+    return 0
+
+
+def _oracle_worker(job):
+    """One shard of the all-cores oracle run: its own process, its own copy of the oracle library."""
+    cfg, seed, e0, arrays = job
+    from oracle import pdo
+
+    ev = wl.Events(**arrays)
+    card = pdo.Card(wl.config_card(cfg))
+    t0 = time.perf_counter()
+    pdo.simulate(card, ev, seed, event_base=e0, debug=False)
+    return time.perf_counter() - t0, int(ev.n_particles)
+
+
+def _oracle_rate_all_cores(cfg, ev, seed, per_worker=1_500_000):
+    """The same oracle, events sharded over os.cpu_count() worker processes (events are independent and the RNG is keyed by
+    the global event index, so the shards reproduce the single run).  Returns particles/s over the wall time of the pool."""
+    import multiprocessing as mp
+
+    cores = os.cpu_count() or 1
+    sample, k = _sample_events(ev, min(int(ev.n_particles), per_worker * cores))
+    bounds = np.linspace(0, k, cores + 1).astype(int)
+    jobs = []
+    for w in range(cores):
+        a, b = int(bounds[w]), int(bounds[w + 1])
+        if b <= a:
+            continue
+        sub = wl.slice_events(sample, a, b)
+        jobs.append((cfg, seed, a, {f: getattr(sub, f) for f in ("offsets", "pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")}))
+    ctx = mp.get_context("fork")
+    with ctx.Pool(len(jobs)) as pool:
+        pool.map(_oracle_warm, [cfg] * len(jobs))  # every worker has the library and the card loaded
+        t0 = time.perf_counter()
+        res = pool.map(_oracle_worker, jobs)
+        wall = time.perf_counter() - t0
+    n = sum(r[1] for r in res)
+    what = "first %d events (%d particles) of %s over %d worker processes" % (k, n, wl.CONFIGS[cfg]["name"], len(jobs))
+    return n / wall, len(jobs), what
 
 
 def _oracle_rate(cfg, ev, seed, steps=1, warmup=0):
@@ -323,7 +379,11 @@ def run_ours(args, rank, world, local_rank):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the (single) kernel: algorithmic bytes / launch
+    # ---- roofline of the chain.  A step is three launches on the stream -- pd_tile_events_kernel (~10 us), pd_particle_kernel
+    # (kernel P) and pd_tower_kernel (kernel T) -- that split the algorithmic bytes between them (P reads the particles and
+    # writes nothing that counts, T writes the three collections), so the roofline is taken over the step: algorithmic
+    # bytes of one pd_simulate / its CUDA-event duration.  The per-kernel times of the same command are in the committed
+    # ncu launch list (profiles/r02*_launches.*).
     alg_bytes = 33 * n + 8 * (ne + 1) + 33 * totals[0] + 28 * totals[1] + 21 * totals[2] + 3 * 8 * (ne + 1)
     kern_ms = float(np.mean(per_launch_ms))
     peak, peak_src = _peaks()
@@ -338,8 +398,12 @@ def run_ours(args, rank, world, local_rank):
         alu_view = {"warp_instructions_per_launch": inst, "warp_instructions_per_particle": inst / max(n, 1),
                     "achieved_warp_inst_per_s": inst / (kern_ms * 1e-3), "issue_peak_warp_inst_per_s": issue_peak,
                     "frac_of_issue_peak": inst / (kern_ms * 1e-3) / issue_peak,
-                    "note": "instruction count from profiles/ (ncu), time live; the path is issue- and barrier-bound, not HBM-bound"}
+                    "note": "instruction count of the two kernels from profiles/ (ncu), time live; the path is bound by instruction issue and on-chip synchronisation, not by HBM"}
     cpu_rate, cpu_dt, cpu_what = _oracle_rate(cfg, ev, seed)
+    try:
+        all_rate, all_cores, all_what = _oracle_rate_all_cores(cfg, ev, seed)
+    except Exception as exc:  # the baseline is context, never a reason to lose the line
+        all_rate, all_cores, all_what = None, 0, "failed: %r" % (exc,)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -350,9 +414,11 @@ def run_ours(args, rank, world, local_rank):
                    "input_sha256": ev.sha256()[:16], "numpy": np.__version__},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": _traffic(cfg), "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
-                     "bytes_per_particle": alg_bytes / max(n, 1), "kernel_ms": kern_ms, "kernel": "pd_chain_kernel",
+                     "bytes_per_particle": alg_bytes / max(n, 1), "kernel_ms": kern_ms,
+                     "kernel": "pd_simulate = pd_tile_events_kernel + pd_particle_kernel + pd_tower_kernel (one step)",
                      "frac_of_8TBs_nominal": achieved / 8000.0, "alu_view": alu_view},
-        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": cpu_what},
+        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": cpu_what, "cpu_model": _cpu_model(),
+                         "all_cores": {"value": all_rate, "unit": UNIT, "cores": all_cores, "host_cores": os.cpu_count(), "sample": all_what}},
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
         "gpu_launches": launches, "clocks": clk,
         "next": {"event_features": {"ms": feat_ms, "objects_per_s": totals[2] / (feat_ms * 1e-3), "kernel": "pd_features_kernel",
