@@ -218,14 +218,17 @@ int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *co
  *   vertex shift: normal of width sigma_z truncated to |z| <= max_z_spread, sampled by inversion of its
  *            distribution function (one uniform, no rejection).
  * Output event e = the hard-scatter particles (vz shifted) followed by the particles of the n picked pool
- * events in draw order (vz shifted); every other field is copied.  sigma_t / max_t_spread of Table C.9 have no
- * effect: the chain carries no time coordinate (reading A29).  The output is a pd_events-shaped CSR batch that
- * pd_simulate takes as it is. */
+ * events in draw order (vz shifted); every other field is copied.  sigma_t / max_t_spread of Table C.9: every
+ * interaction also gets a time, the same truncated normal from word 2 of its block (the hard scatter's from block 0 if
+ * smear_hs_vertex, else 0), written per particle to `vt` (reading H7); the detector chain itself carries no time
+ * coordinate (reading A29).  The output is a pd_events-shaped CSR batch that pd_simulate takes as it is. */
 typedef struct {
   float mean_pileup;  /* 0 <= mean <= 500 */
   float sigma_z;      /* metres, >= 0 (Table C.9 default 0.053) */
   float max_z_spread; /* metres, >= 0 (default 0.25) */
   int32_t smear_hs_vertex;
+  float sigma_t;      /* seconds, >= 0 (Table C.9 default 160e-12); 0: every interaction at t = 0 */
+  float max_t_spread; /* seconds, >= 0 (default 800e-12) */
 } pd_pileup_config;
 
 typedef struct {
@@ -236,6 +239,7 @@ typedef struct {
   float *px, *py, *pz, *E, *vx, *vy, *vz;
   uint8_t *is_pu;    /* 1 for pile-up particles */
   int32_t *n_pileup; /* [n_events] interactions merged into each event */
+  float *vt;         /* time of the particle's interaction, seconds (reading H7); may be NULL */
 } pd_merged_events;
 
 /* Bytes of DEVICE workspace pd_pileup_merge needs (status word, per-event counts, scan words). */

@@ -1128,36 +1128,42 @@ static double pdo_truncated_z(uint32_t r1, double sigma_z, double max_z) {
   return -sign * sigma_z * pdo_norm_quantile_lower(q);
 }
 
-int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_pileup, double sigma_z,
-                     double max_z_spread, int smear_hs_vertex, uint64_t seed, int64_t event_base, int64_t out_capacity,
-                     int64_t *out_offsets, int32_t *out_pid, int8_t *out_charge, float *out_px, float *out_py,
-                     float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz, uint8_t *is_pu,
-                     int32_t *n_pileup) {
+/* reading H7: with sigma_t > 0 every interaction also gets a time, the same truncated normal (width sigma_t, cut at
+ * max_t_spread; Table C.9) from word 2 of its block -- the hard scatter's from block 0 if smear_hs_vertex, else 0 --
+ * written per particle to out_vt (seconds; may be NULL) */
+int pdo_pileup_merge_t(const pdo_events *hs, const pdo_events *pool, double mean_pileup, double sigma_z,
+                       double max_z_spread, double sigma_t, double max_t_spread, int smear_hs_vertex, uint64_t seed,
+                       int64_t event_base, int64_t out_capacity, int64_t *out_offsets, int32_t *out_pid, int8_t *out_charge,
+                       float *out_px, float *out_py, float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz,
+                       uint8_t *is_pu, int32_t *n_pileup, float *out_vt) {
   int64_t e, n_out = 0;
   int rc = PDO_OK;
   if (!hs || !pool || !out_offsets || hs->n_events < 0 || pool->n_events < 1 || !hs->offsets || !pool->offsets) return PDO_EINVAL;
   if (!(mean_pileup >= 0.0) || mean_pileup > 500.0 || !(sigma_z >= 0.0) || !(max_z_spread >= 0.0)) return PDO_EINVAL;
+  if (!(sigma_t >= 0.0) || !(max_t_spread >= 0.0)) return PDO_EINVAL;
   out_offsets[0] = 0;
   for (e = 0; e < hs->n_events; ++e) {
     const int64_t event = event_base + e;
     uint32_t r[4];
     int n, k, s;
-    double dz_hs;
+    double dz_hs, dt_hs;
     pdo_rng_block(seed, event, 0u, 2u, r);
     n = pdo_poisson_inverse(mean_pileup, pdo_uniform(r[0]));
     dz_hs = smear_hs_vertex ? pdo_truncated_z(r[1], sigma_z, max_z_spread) : 0.0;
+    dt_hs = smear_hs_vertex ? pdo_truncated_z(r[2], sigma_t, max_t_spread) : 0.0;
     if (n_pileup) n_pileup[e] = n;
     /* sources: s = -1 the hard-scatter event, s = k the k-th pile-up interaction */
     for (s = -1; s < n; ++s) {
       const pdo_events *src = hs;
       int64_t a = hs->offsets[e], b = hs->offsets[e + 1], i;
-      double dz = dz_hs;
+      double dz = dz_hs, dt = dt_hs;
       k = s;
       if (s >= 0) {
         int64_t j;
         pdo_rng_block(seed, event, (uint32_t)(1 + k), 2u, r);
         j = (int64_t)(((uint64_t)(r[0] >> 8) * (uint64_t)pool->n_events) >> 24);
         dz = pdo_truncated_z(r[1], sigma_z, max_z_spread);
+        dt = pdo_truncated_z(r[2], sigma_t, max_t_spread);
         src = pool, a = pool->offsets[j], b = pool->offsets[j + 1];
       }
       for (i = a; i < b; ++i, ++n_out) {
@@ -1170,11 +1176,21 @@ int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_p
         out_vx[n_out] = src->vx[i], out_vy[n_out] = src->vy[i];
         out_vz[n_out] = (float)((double)src->vz[i] + dz);
         if (is_pu) is_pu[n_out] = (uint8_t)(s >= 0);
+        if (out_vt) out_vt[n_out] = (float)dt;
       }
     }
     out_offsets[e + 1] = n_out;
   }
   return rc;
+}
+
+int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_pileup, double sigma_z,
+                     double max_z_spread, int smear_hs_vertex, uint64_t seed, int64_t event_base, int64_t out_capacity,
+                     int64_t *out_offsets, int32_t *out_pid, int8_t *out_charge, float *out_px, float *out_py,
+                     float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz, uint8_t *is_pu,
+                     int32_t *n_pileup) {
+  return pdo_pileup_merge_t(hs, pool, mean_pileup, sigma_z, max_z_spread, 0.0, 0.0, smear_hs_vertex, seed, event_base, out_capacity,
+                            out_offsets, out_pid, out_charge, out_px, out_py, out_pz, out_E, out_vx, out_vy, out_vz, is_pu, n_pileup, NULL);
 }
 
 /* ---- track impact parameters (Table 2) ----

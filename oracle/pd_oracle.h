@@ -217,6 +217,15 @@ int pdo_pileup_merge(const pdo_events *hs, const pdo_events *pool, double mean_p
                      float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz, uint8_t *is_pu,
                      int32_t *n_pileup /* [n_events], may be NULL */);
 
+/* The same with the time coordinate of Table C.9 (sigma_t, max_t_spread; reading H7 of DESIGN.md section 12): the time
+ * of an interaction is the truncated normal of width sigma_t cut at max_t_spread from word 2 of its block (hard scatter:
+ * block 0, only if smear_hs_vertex); out_vt [capacity], seconds, may be NULL. */
+int pdo_pileup_merge_t(const pdo_events *hs, const pdo_events *pool, double mean_pileup, double sigma_z,
+                       double max_z_spread, double sigma_t, double max_t_spread, int smear_hs_vertex, uint64_t seed,
+                       int64_t event_base, int64_t out_capacity, int64_t *out_offsets, int32_t *out_pid, int8_t *out_charge,
+                       float *out_px, float *out_py, float *out_pz, float *out_E, float *out_vx, float *out_vy, float *out_vz,
+                       uint8_t *is_pu, int32_t *n_pileup, float *out_vt);
+
 /* ---- track impact parameters ("where supported, track impact parameters"; P:L138
  * Table 2 "d_0, z_0 and their errors for charged particles"; P:L424-426 PFlow.D0 / PFlow.Z0) ----
  * The paper names the outputs and gives no formula; readings I1..I3 of DESIGN.md section 14:

@@ -363,9 +363,14 @@ def _events_struct(ev):
     return _Events(int(ev.offsets.shape[0] - 1), int(ev.offsets[-1]), *[_ptr(a) for a in keep]), keep
 
 
+def _vp(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
 def pileup_merge(hs, pool, mean_pileup: float, sigma_z: float = 0.053, max_z_spread: float = 0.25,
-                 smear_hs_vertex: bool = True, seed: int = 0, event_base: int = 0) -> dict:
-    """pdo_pileup_merge (Listing 8, Table C.9): returns offsets, pid, charge, px..vz, is_pu, n_pileup."""
+                 smear_hs_vertex: bool = True, seed: int = 0, event_base: int = 0, sigma_t: float = 160e-12,
+                 max_t_spread: float = 800e-12) -> dict:
+    """pdo_pileup_merge_t (Listing 8, Table C.9): returns offsets, pid, charge, px..vz, is_pu, vt, n_pileup."""
     chs, k1 = _events_struct(hs)
     cpool, k2 = _events_struct(pool)
     ne = chs.n_events
@@ -373,18 +378,24 @@ def pileup_merge(hs, pool, mean_pileup: float, sigma_z: float = 0.053, max_z_spr
     npu = np.zeros(max(ne, 1), dtype=np.int32)
     dt = dict(pid=np.int32, charge=np.int8, px=np.float32, py=np.float32, pz=np.float32, E=np.float32, vx=np.float32,
               vy=np.float32, vz=np.float32, is_pu=np.uint8)
+    L = lib()
+    L.pdo_pileup_merge_t.restype = C.c_int
+    L.pdo_pileup_merge_t.argtypes = [C.POINTER(_Events), C.POINTER(_Events), C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                     C.c_int, C.c_uint64, C.c_int64, C.c_int64] + [C.c_void_p] * 13
     cap = 0
     for _ in range(2):  # first pass sizes the output (PDO_ECAPACITY with complete offsets), second fills it
         out = {k: np.zeros(max(cap, 1), dtype=d) for k, d in dt.items()}
-        rc = lib().pdo_pileup_merge(C.byref(chs), C.byref(cpool), float(mean_pileup), float(sigma_z), float(max_z_spread),
-                                    int(bool(smear_hs_vertex)), int(seed) & (2**64 - 1), int(event_base), cap, _ptr(off),
-                                    *[_ptr(out[k]) for k in dt], _ptr(npu))
+        vt = np.zeros(max(cap, 1), dtype=np.float32)
+        rc = L.pdo_pileup_merge_t(C.byref(chs), C.byref(cpool), float(mean_pileup), float(sigma_z), float(max_z_spread),
+                                  float(sigma_t), float(max_t_spread), int(bool(smear_hs_vertex)), int(seed) & (2**64 - 1),
+                                  int(event_base), cap, _vp(off), *[_vp(out[k]) for k in dt], _vp(npu), _vp(vt))
         if rc == 0:
             break
         if rc != -3:
             raise OracleError(rc)
         cap = int(off[-1])
     res = {k: v[: int(off[-1])] for k, v in out.items()}
+    res["vt"] = vt[: int(off[-1])]
     res["offsets"], res["n_pileup"] = off, npu[:ne]
     return res
 

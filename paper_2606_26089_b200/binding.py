@@ -51,12 +51,13 @@ class Impact(C.Structure):
 
 
 class PileupConfig(C.Structure):
-    _fields_ = [("mean_pileup", C.c_float), ("sigma_z", C.c_float), ("max_z_spread", C.c_float), ("smear_hs_vertex", C.c_int32)]
+    _fields_ = [("mean_pileup", C.c_float), ("sigma_z", C.c_float), ("max_z_spread", C.c_float), ("smear_hs_vertex", C.c_int32),
+                ("sigma_t", C.c_float), ("max_t_spread", C.c_float)]
 
 
 class MergedEvents(C.Structure):
     _fields_ = [("capacity", C.c_int64)] + [(k, _p) for k in ("offsets", "pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz",
-                                                        "is_pu", "n_pileup")]
+                                                        "is_pu", "n_pileup", "vt")]
 
 
 class Events(C.Structure):
@@ -441,11 +442,12 @@ class DeviceMerged:
             self.t[name] = torch.empty(cap, dtype=getattr(torch, dt), device=device)
         self.t["is_pu"] = torch.empty(cap, dtype=torch.uint8, device=device)
         self.t["n_pileup"] = torch.empty(max(self.n_events, 1), dtype=torch.int32, device=device)
+        self.t["vt"] = torch.empty(cap, dtype=torch.float32, device=device)
         nbytes = int(lib().pd_pileup_workspace_bytes(self.n_events))
         self.ws_bytes = nbytes
         self.ws = torch.empty(nbytes + 16, dtype=torch.uint8, device=device)
         self.c = MergedEvents(self.capacity, *[_tptr(self.t[k]) for k in ("offsets", "pid", "charge", "px", "py", "pz", "E", "vx", "vy",
-                                                                            "vz", "is_pu", "n_pileup")])
+                                                                            "vz", "is_pu", "n_pileup", "vt")])
 
     def total(self) -> int:
         _torch().cuda.synchronize()
@@ -462,19 +464,20 @@ class DeviceMerged:
     def to_numpy(self) -> dict:
         n = self.total()
         out = {"offsets": self.t["offsets"].cpu().numpy(), "n_pileup": self.t["n_pileup"][: self.n_events].cpu().numpy()}
-        for k in [name for name, _ in EVENT_FIELDS[1:]] + ["is_pu"]:
+        for k in [name for name, _ in EVENT_FIELDS[1:]] + ["is_pu", "vt"]:
             out[k] = self.t[k][:n].cpu().numpy()
         return out
 
 
 def pileup_merge(hs: "DeviceEvents", pool: "DeviceEvents", out: DeviceMerged, mean_pileup: float, sigma_z: float = 0.053,
-                 max_z_spread: float = 0.25, smear_hs_vertex: bool = True, seed: int = 0, event_base: int = 0, stream=None):
+                 max_z_spread: float = 0.25, smear_hs_vertex: bool = True, seed: int = 0, event_base: int = 0, stream=None,
+                 sigma_t: float = 160e-12, max_t_spread: float = 800e-12):
     """pd_pileup_merge (asynchronous).  pileup_status(out) afterwards reports PD_ECAPACITY if `out` was too small."""
     torch = _torch()
     if not torch.cuda.is_available():
         raise PdError(PD_ECUDA)
     st = torch.cuda.current_stream() if stream is None else stream
-    cfg = PileupConfig(float(mean_pileup), float(sigma_z), float(max_z_spread), int(bool(smear_hs_vertex)))
+    cfg = PileupConfig(float(mean_pileup), float(sigma_z), float(max_z_spread), int(bool(smear_hs_vertex)), float(sigma_t), float(max_t_spread))
     _check(lib().pd_pileup_merge(C.byref(hs.c), C.byref(pool.c), C.byref(cfg), int(seed) & (2**64 - 1), int(event_base),
                                  C.byref(out.c), _tptr(out.ws), out.ws_bytes, C.c_void_p(st.cuda_stream)))
 

@@ -140,6 +140,7 @@ int pd_pileup_merge(const pd_events *hs, const pd_events *pool, const pd_pileup_
   if (!hs || !pool || !cfg || !out || hs->n_events < 0 || pool->n_events < 1 || !hs->offsets || !pool->offsets) return PD_EINVAL;
   if (!(cfg->mean_pileup >= 0.f) || cfg->mean_pileup > 500.f || !(cfg->sigma_z >= 0.f) || !(cfg->max_z_spread >= 0.f)) return PD_EINVAL;
   if (!std::isfinite(cfg->sigma_z) || !std::isfinite(cfg->max_z_spread)) return PD_EINVAL;
+  if (!(cfg->sigma_t >= 0.f) || !(cfg->max_t_spread >= 0.f) || !std::isfinite(cfg->sigma_t) || !std::isfinite(cfg->max_t_spread)) return PD_EINVAL;
   if (!out->offsets || out->capacity < 0) return PD_EINVAL;
   if (hs->n_events > 0 && !out->n_pileup) return PD_EINVAL;
   if (out->capacity > 0 && (!out->pid || !out->charge || !out->px || !out->py || !out->pz || !out->E || !out->vx || !out->vy ||
@@ -172,6 +173,12 @@ int pd_pileup_merge(const pd_events *hs, const pd_events *pool, const pd_pileup_
   p.sigma_z = cfg->sigma_z;
   const double lo = sz > 0.0 ? 0.5 * std::erfc((zmax / sz) / std::sqrt(2.0)) : 0.0;
   p.phi_lo = (float)lo, p.half_minus_lo = (float)(0.5 - lo);
+  {
+    const double st = (double)cfg->sigma_t, tmax = (double)cfg->max_t_spread;
+    const double lo_t = st > 0.0 ? 0.5 * std::erfc((tmax / st) / std::sqrt(2.0)) : 0.0;
+    p.sigma_t = cfg->sigma_t, p.phi_lo_t = (float)lo_t, p.half_minus_lo_t = (float)(0.5 - lo_t);
+    p.out_vt = out->vt;
+  }
   for (int r = 0; r < 10; ++r) {
     p.rk.k0[r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
     p.rk.k1[r] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;

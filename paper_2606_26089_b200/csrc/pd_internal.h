@@ -230,6 +230,8 @@ struct PdPileupParams {
   double mu, p0;                     // mean, exp(-mean)
   int n_max, smear_hs;
   float sigma_z, phi_lo, half_minus_lo;  // Phi(-a), 1/2 - Phi(-a), a = max_z / sigma_z
+  float sigma_t, phi_lo_t, half_minus_lo_t;  // the same for the time of an interaction (reading H7)
+  float *out_vt;                         // nullable
   PdPhiloxKeys rk;
   long long event_base;
   long long capacity;

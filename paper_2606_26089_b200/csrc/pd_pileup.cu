@@ -57,15 +57,22 @@ __device__ __forceinline__ int poisson_inverse(const PdPileupParams &prm, uint32
 }
 
 // reading H4: truncated normal by inversion, through the lower tail
-__device__ __forceinline__ float truncated_z(const PdPileupParams &prm, uint32_t r1) {
-  if (!(prm.sigma_z > 0.f)) return 0.f;
+__device__ __forceinline__ float truncated_normal(float sigma, float phi_lo, float half_minus_lo, uint32_t r1) {
+  if (!(sigma > 0.f)) return 0.f;
   // u = (k + 1/2) 2^-24, v = |2u - 1|: 1 - v = (2^24 - |2k + 1 - 2^24|) 2^-24, formed in integers so that the far
   // tail (u next to 0 or 1) keeps its relative precision
   const int k2 = 2 * (int)(r1 >> 8) + 1 - (1 << 24);
   const float t = (float)((1 << 24) - (k2 < 0 ? -k2 : k2)) * 5.9604644775390625e-08f;  // exact
-  const float q = fmaf(t, prm.half_minus_lo, prm.phi_lo);
-  const float z = -prm.sigma_z * normcdfinvf(q);
+  const float q = fmaf(t, half_minus_lo, phi_lo);
+  const float z = -sigma * normcdfinvf(q);
   return k2 < 0 ? -z : z;
+}
+__device__ __forceinline__ float truncated_z(const PdPileupParams &prm, uint32_t r1) {
+  return truncated_normal(prm.sigma_z, prm.phi_lo, prm.half_minus_lo, r1);
+}
+// reading H7: the time of the interaction, the same way from word 2 (seconds)
+__device__ __forceinline__ float truncated_t(const PdPileupParams &prm, uint32_t r2) {
+  return truncated_normal(prm.sigma_t, prm.phi_lo_t, prm.half_minus_lo_t, r2);
 }
 
 __device__ __forceinline__ long long pool_pick(const PdPileupParams &prm, uint32_t r0) {
@@ -179,6 +186,7 @@ __global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_consta
   __shared__ long long s_a[MAX_SOURCES], s_o[MAX_SOURCES];
   __shared__ int s_len[MAX_SOURCES];
   __shared__ float s_dz[MAX_SOURCES];
+  __shared__ float s_dt[MAX_SOURCES];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   if (prm.out_off[prm.n_hs] > prm.capacity) return;  // reported by the scan kernel through the status word
   for (long long e = blockIdx.x; e < prm.n_hs; e += gridDim.x) {
@@ -191,17 +199,19 @@ __global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_consta
         const int s = s0 + lane;  // source s: block s of the event's stream (0 = the hard scatter)
         long long a = 0;
         int len = 0;
-        float dz = 0.f;
+        float dz = 0.f, dt = 0.f;
         if (s < n_src) {
           uint32_t r[4];
           rng_block2(prm.rk, event, (uint32_t)s, r);
           if (s == 0) {
             a = __ldg(prm.hs_off + e), len = (int)(__ldg(prm.hs_off + e + 1) - a);
             dz = prm.smear_hs ? truncated_z(prm, r[1]) : 0.f;
+            dt = prm.smear_hs ? truncated_t(prm, r[2]) : 0.f;
           } else {
             const long long j = pool_pick(prm, r[0]);
             a = __ldg(prm.pool_off + j), len = (int)(__ldg(prm.pool_off + j + 1) - a);
             dz = truncated_z(prm, r[1]);
+            dt = truncated_t(prm, r[2]);
           }
         }
         int incl = len;
@@ -210,7 +220,7 @@ __global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_consta
           const int t = __shfl_up_sync(0xffffffffu, incl, o);
           if (lane >= o) incl += t;
         }
-        if (s < n_src) s_a[s] = a, s_len[s] = len, s_dz[s] = dz, s_o[s] = run + (incl - len);
+        if (s < n_src) s_a[s] = a, s_len[s] = len, s_dz[s] = dz, s_dt[s] = dt, s_o[s] = run + (incl - len);
         run += __shfl_sync(0xffffffffu, incl, 31);
       }
     }
@@ -219,7 +229,7 @@ __global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_consta
       const bool pu = s > 0;
       const long long a = s_a[s], o = s_o[s];
       const int len = s_len[s];
-      const float dz = s_dz[s];
+      const float dz = s_dz[s], dt = s_dt[s];
       const int *src_pid = pu ? prm.pool_pid : prm.hs_pid;
       const signed char *src_q = pu ? prm.pool_charge : prm.hs_charge;
       for (int i = lane; i < len; i += 32) {
@@ -230,6 +240,7 @@ __global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_consta
         for (int f = 0; f < 6; ++f) prm.out_f[f][d] = __ldg((pu ? prm.pool_f[f] : prm.hs_f[f]) + a + i);
         prm.out_f[6][d] = __ldg((pu ? prm.pool_f[6] : prm.hs_f[6]) + a + i) + dz;
         prm.is_pu[d] = pu ? 1 : 0;
+        if (prm.out_vt) prm.out_vt[d] = dt;
       }
     }
   }

@@ -844,18 +844,26 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
         const long long gs = (gseg_lo + k) * PD_PSEG;
         const int a = s_sega[k], c = s_segc[k];
         const unsigned ob = (unsigned)t0 + (unsigned)s_segp[k];
-        for (int r = lane; r < c; r += 32) {
-          const long long g = gs + a + r;
+        // two rows of a segment at a time: twenty independent loads in flight per lane before the first store
+        for (int r = lane; r < c; r += 64) {
+          const bool two = r + 32 < c;
+          const long long g = gs + a + r, g2 = two ? g + 32 : g;
           const unsigned o = ob + (unsigned)r;
-          prm.trk_src[o] = (int)(p_al + gs + (long long)__ldg(prm.park_idx + g));
-          prm.trk_pid[o] = __ldg(prm.park_pid + g);
-          prm.trk_charge[o] = __ldg(prm.park_q + g);
-          prm.trk_pt[o] = __ldg(prm.park_f[0] + g);
-          prm.trk_eta[o] = __ldg(prm.park_f[1] + g);
-          prm.trk_phi[o] = __ldg(prm.park_f[2] + g);
-          prm.trk_E[o] = __ldg(prm.park_f[3] + g);
-          prm.trk_eta_out[o] = __ldg(prm.park_f[4] + g);
-          prm.trk_phi_out[o] = __ldg(prm.park_f[5] + g);
+          const int i0 = (int)__ldg(prm.park_idx + g), i1 = (int)__ldg(prm.park_idx + g2);
+          const int d0 = __ldg(prm.park_pid + g), d1 = __ldg(prm.park_pid + g2);
+          const signed char q0_ = __ldg(prm.park_q + g), q1_ = __ldg(prm.park_q + g2);
+          float f0[6], f1[6];
+#pragma unroll
+          for (int k6 = 0; k6 < 6; ++k6) f0[k6] = __ldg(prm.park_f[k6] + g), f1[k6] = __ldg(prm.park_f[k6] + g2);
+          prm.trk_src[o] = (int)(p_al + gs + i0), prm.trk_pid[o] = d0, prm.trk_charge[o] = q0_;
+          prm.trk_pt[o] = f0[0], prm.trk_eta[o] = f0[1], prm.trk_phi[o] = f0[2], prm.trk_E[o] = f0[3];
+          prm.trk_eta_out[o] = f0[4], prm.trk_phi_out[o] = f0[5];
+          if (two) {
+            const unsigned o2 = o + 32u;
+            prm.trk_src[o2] = (int)(p_al + gs + i1), prm.trk_pid[o2] = d1, prm.trk_charge[o2] = q1_;
+            prm.trk_pt[o2] = f1[0], prm.trk_eta[o2] = f1[1], prm.trk_phi[o2] = f1[2], prm.trk_E[o2] = f1[3];
+            prm.trk_eta_out[o2] = f1[4], prm.trk_phi_out[o2] = f1[5];
+          }
         }
       }
     }

@@ -1,7 +1,8 @@
 """-m gpu: pd_pileup_merge (Listing 8, Table C.9) through the C ABI against the fp64 oracle.
 Integers (the Poisson counts, the pool picks as seen through the copied particles, offsets, order, pid, charge,
 is_pu) and every copied float must be bit-exact; the shifted vz must agree within 1e-6 m (north-star absolute
-tolerance; the shift is a fp32 normal quantile on the GPU, a fp64 bisection in the oracle).  Then the merged batch
+tolerance; the shift is a fp32 normal quantile on the GPU, a fp64 bisection in the oracle), the interaction time vt
+(reading H7) within 1e-5 relative with a floor of 1e-15 s.  Then the merged batch
 goes through pd_simulate and is compared with the oracle chain run on the ORACLE's merged batch."""
 import importlib
 
@@ -31,6 +32,9 @@ def _compare(g, o):
         assert g[k].tobytes() == o[k].tobytes(), k
     d = np.abs(g["vz"].astype(np.float64) - o["vz"])
     assert d.max(initial=0.0) <= 1e-6, d.max()
+    # time coordinate (reading H7): seconds, |t| <= 0.8 ns -- the absolute floor scales with the unit (1e-6 of the cut)
+    dt = np.abs(g["vt"].astype(np.float64) - o["vt"])
+    assert np.all(dt <= np.maximum(1e-5 * np.abs(o["vt"]), 1e-15)), dt.max()
     return d.max(initial=0.0)
 
 

@@ -137,3 +137,48 @@ def test_truncated_normal_is_the_quantile_formula():
             assert abs(float(r["vz"][pos]) - z) < 1e-7
             pos += 1
     assert pos == len(r["vz"])
+
+
+def test_time_coordinate_of_an_interaction():
+    """Reading H7 (Table C.9 P:L601-603 sigma_t / max_t_spread; Listing 8): one time per interaction, the
+    truncated normal of reading H4 with (sigma_t, max_t_spread) from word 2 of the interaction's block; against scipy's
+    quantile per draw, the closed-form moments, the bound, the hard-scatter rules and independence from the z shift."""
+    one = wl.from_lists([[wl.particle(22, 0, 1.0, 0.0, 0.0, 0.0), wl.particle(211, 1, 0.0, 1.0, 0.0, 0.13957039)]])
+    hs = wl.from_lists([[wl.particle(22, 0, 2.0, 0.0, 0.0, 0.0)] * 3 for _ in range(3000)])
+    st, tmax = 160e-12, 800e-12
+    r = pdo.pileup_merge(hs, one, 4.0, seed=8, sigma_t=st, max_t_spread=tmax)
+    vt = r["vt"].astype(np.float64)
+    pu = r["is_pu"] == 1
+    assert np.abs(vt).max() <= tmax * (1 + 1e-6)
+    # every particle of a source carries the source's time; per draw it is the quantile formula on word 2
+    pos = 0
+    for e in range(200):
+        assert vt[pos] == vt[pos + 1] == vt[pos + 2]
+        w = [pdo.rng_block(8, e, 0, 2)[2]] + [pdo.rng_block(8, e, 1 + k, 2)[2] for k in range(int(r["n_pileup"][e]))]
+        for i, r2 in enumerate(w):
+            u = ((r2 >> 8) + 0.5) / 2**24
+            lo = stats.norm.cdf(-tmax / st)
+            t = -np.sign(u - 0.5) * st * stats.norm.ppf(lo + (1 - abs(2 * u - 1)) * (0.5 - lo))
+            a = pos if i == 0 else pos + 3 + 2 * (i - 1)
+            assert abs(vt[a] - t) <= 1e-6 * abs(t) + 1e-18, (e, i)
+            assert i == 0 or vt[a] == vt[a + 1]
+        pos = int(r["offsets"][e + 1])
+    # distribution: truncated normal, cut at 5 sigma
+    t = stats.truncnorm(-tmax / st, tmax / st, scale=st)
+    d = vt[pu][::2]
+    assert len(d) > 10000 and abs(d.mean()) < 4 * t.std() / np.sqrt(len(d)) and abs(d.std() - t.std()) < 0.02 * t.std()
+    assert stats.kstest(d, t.cdf).pvalue > 1e-3
+    # a tight cut: |t| <= max_t_spread, the width shrinks accordingly
+    r2_ = pdo.pileup_merge(hs, one, 4.0, seed=8, sigma_t=st, max_t_spread=100e-12)
+    d2 = r2_["vt"][r2_["is_pu"] == 1].astype(np.float64)
+    t2 = stats.truncnorm(-100 / 160, 100 / 160, scale=st)
+    assert np.abs(d2).max() <= 100e-12 * (1 + 1e-6) and abs(d2.std() - t2.std()) < 0.02 * t2.std()
+    # time and z come from different words: uncorrelated, and the z shifts do not change when sigma_t does
+    dz = r["vz"][pu].astype(np.float64)[::2]
+    assert abs(np.corrcoef(dz, d)[0, 1]) < 4 / np.sqrt(len(d))
+    assert r2_["vz"].tobytes() == r["vz"].tobytes() and np.array_equal(r2_["n_pileup"], r["n_pileup"])
+    # hard scatter: time 0 when its vertex is not smeared; sigma_t = 0: no times at all
+    r3 = pdo.pileup_merge(hs, one, 4.0, smear_hs_vertex=False, seed=8, sigma_t=st, max_t_spread=tmax)
+    assert np.all(r3["vt"][r3["is_pu"] == 0] == 0) and r3["vt"][r3["is_pu"] == 1].tobytes() == r["vt"][pu].tobytes()
+    r4 = pdo.pileup_merge(hs, one, 4.0, seed=8, sigma_t=0.0, max_t_spread=tmax)
+    assert not r4["vt"].any() and r4["vz"].tobytes() == r["vz"].tobytes()
