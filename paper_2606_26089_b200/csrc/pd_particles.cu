@@ -9,11 +9,13 @@
 // lists -- A: charged inside the tracker acceptance (efficiency > 0: helix + Philox + accept + smear), B: other
 // charged (helix only), N: neutral (straight line) -- and the lists are processed by full warps gathering from
 // shared memory.  An accepted track is smeared on the spot (its Philox block is in registers) and its record
-// parked in the particle's own staging slots; after a scan over the accepted bits in particle order and a
-// decoupled look-back over the tiles the Track collection is written in its final place.
+// parked in the particle's own staging slots; at the end of the tile every warp compacts the tracks of the
+// PD_PSEG particles it owns, in particle order, and PARKS them in the workspace at the start of its segment, with
+// the segment's accepted bits beside them.  Nothing here depends on another tile: no chain, no waiting.  Kernel T,
+// which works event by event and knows where an event's tracks go, moves them into the Track collection.
 //
-// What the tower pass (pd_towers.cu) needs is a 16-bit key per particle (tower id | HCAL bit, 0xffff = no deposit),
-// written to the workspace with one bulk store per tile, and the Track collection itself.
+// What the tower pass (pd_towers.cu) needs besides: a 16-bit key per particle (tower id | HCAL bit, 0xffff = no
+// deposit), written to the workspace by the warp that owns the particle.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -383,7 +385,7 @@ int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_sm
   if (smem > (size_t)max_smem_optin) return PD_ECUDA;
   auto kern = debug ? pdk::pd_particle_kernel<true> : pdk::pd_particle_kernel<false>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin) != cudaSuccess) return PD_ECUDA;
-  // persistent CTAs wait on one another through the look-back chain: the grid must be co-resident
+  // persistent CTAs that claim their tiles from a counter: as many as fit on the device
   int per_sm = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, pdk::PT_THREADS, smem) != cudaSuccess) return PD_ECUDA;
   if (per_sm < 1) return PD_ECUDA;
