@@ -11,7 +11,8 @@
 //   step 1b a run that is one big event: counting sort of its object indices by (eta strip, phi cell), both at
 //           least dr_max wide, so that a lepton only meets the objects of the 3 x 3 cells around it
 //   step 2  H_T and E_T^miss: a warp per event (all warps for one big event), exact 64-bit fixed-point sums
-//   step 3  isolation: a warp per lepton, lanes over the candidate objects, three exact fixed-point sums
+//   step 3  isolation: sixteen lanes per lepton over its candidate objects in the cache (a warp per lepton, lanes over the
+//           objects, for an event streamed from global memory), three exact fixed-point sums
 // Fixed-point sums (units of 2^-32 GeV) are associative: results do not depend on the order of the objects,
 // the chunking or the launch shape.
 #include <cuda_runtime.h>
@@ -144,16 +145,98 @@ __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, P
     }
   };
   if (s_lep != nullptr) {
-    // cached run: the leptons were listed by step 1; its event is found by bisection of the run's offsets
-    for (int k = wid; k < n_lep; k += W) {
-      const int i = (int)s_lep[k];
-      int lo = 0, hi = ne;  // s_off[lo] <= i < s_off[hi]
-      while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (s_off[mid] <= i) lo = mid;
-        else hi = mid;
+    // cached run: the leptons were listed by step 1.  SIXTEEN LANES per lepton (two leptons per warp pass) walk over the
+    // candidates of a big event in shared memory -- the objects of the 3 x 3 cells around it (a hundred or so), as ONE
+    // index space over the (up to four) contiguous pieces of the cell list, so that the lanes stay full and the two
+    // halves of a warp run the same loop; the three sums are folded with four shuffle steps.  The event of a lepton is
+    // found by bisection of the run's offsets.
+    // (eight lanes per lepton, four leptons per pass, when the candidates are the few objects of a small event)
+    const bool listed = s_idx != nullptr;
+    const int GL = listed ? 16 : 8, per_warp = 32 / GL;
+    const int grp = lane / GL, gl = lane & (GL - 1);
+    for (int k0 = 0; k0 < n_lep; k0 += per_warp * W) {
+      const int k = k0 + per_warp * wid + grp;
+      const bool active = k < n_lep;
+      const int i = active ? (int)s_lep[k] : 0;
+      const float eta_i = o_eta[i], phi_i = o_phi[i];
+      // pieces [b0, b0 + n0), [b1, ...), ...: positions in s_idx (listed) or object indices (one event of a multi-event run)
+      int b0 = 0, n0 = 0, b1 = 0, n1 = 0, b2 = 0, n2 = 0, b3 = 0, n3 = 0;
+      if (active) {
+        if (listed) {
+          const int st = eta_strip(eta_i, prm.inv_strip), pc = phi_cell(phi_i, prm), np = prm.n_phi;
+          const bool wrap = np > 3 && (pc == 0 || pc == np - 1);
+          // per strip: cells [lo, hi) around pc, clipped; a lepton in the first / last phi cell also takes the cell at the
+          // other end: since the strips follow one another in the list, that cell of strip s and the first cells of strip s + 1
+          // are not adjacent, so it gets a piece of its own only in the lepton's strip... keep it simple: three pieces for the
+          // clipped windows, and the wrap-around cells of all three strips scanned as extra pieces one after the other below
+          const int s_lo = max(st - 1, 0), s_hi = min(st + 1, N_STRIPS - 1);
+          const int c_lo = np <= 3 ? 0 : max(pc - 1, 0), c_hi = np <= 3 ? np : min(pc + 2, np);
+          const unsigned short *r0 = s_cstart + s_lo * N_PHI_MAX;
+          b0 = r0[c_lo], n0 = r0[c_hi] - b0;
+          if (s_lo + 1 <= s_hi) {
+            const unsigned short *r1 = r0 + N_PHI_MAX;
+            b1 = r1[c_lo], n1 = r1[c_hi] - b1;
+          }
+          if (s_lo + 2 <= s_hi) {
+            const unsigned short *r2 = r0 + 2 * N_PHI_MAX;
+            b2 = r2[c_lo], n2 = r2[c_hi] - b2;
+          }
+          if (wrap) {
+            // the cell at the other end of the phi range, strip by strip, through the fourth piece
+            const int wc = pc == 0 ? np - 1 : 0;
+            b3 = -1 - wc;  // marker: handled by the loop below
+          }
+        } else {
+          int lo = 0, hi = ne;  // s_off[lo] <= i < s_off[hi]
+          while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (s_off[mid] <= i) lo = mid;
+            else hi = mid;
+          }
+          b0 = s_off[lo], n0 = s_off[lo + 1] - b0;
+        }
       }
-      isolate(i, s_off[lo], s_off[lo + 1]);
+      long long s_ch = 0, s_nh = 0, s_ph = 0;
+      auto test = [&](int j) {
+        const float deta = o_eta[j] - eta_i;
+        float dphi = o_phi[j] - phi_i;
+        dphi = dphi > kPi ? dphi - kTwoPi : (dphi <= -kPi ? dphi + kTwoPi : dphi);
+        const float dr2 = fmaf(deta, deta, dphi * dphi);
+        if (dr2 < prm.dr_max2 && j != i) {
+          const int cj = (int)o_cls[j];
+          const long long fx = to_fix(o_pt[j]);
+          if (cj <= PD_CLS_MUON) s_ch += fx;
+          else if (cj == PD_CLS_NEUHAD) s_nh += fx;
+          else if (!(dr2 < prm.fsr2)) s_ph += fx;
+        }
+      };
+      const int n01 = n0 + n1, n012 = n01 + n2;
+      for (int v = gl; v < n012; v += GL) {
+        const int pos = v < n0 ? b0 + v : (v < n01 ? b1 + (v - n0) : b2 + (v - n01));
+        test(listed ? (int)s_idx[pos] : pos);
+      }
+      if (b3 < 0) {
+        const int wc = -1 - b3;
+        const int st = eta_strip(eta_i, prm.inv_strip);
+        for (int s2 = max(st - 1, 0); s2 <= min(st + 1, N_STRIPS - 1); ++s2) {
+          const unsigned short *row = s_cstart + s2 * N_PHI_MAX;
+          for (int pos = row[wc] + gl; pos < row[wc + 1]; pos += 16) test((int)s_idx[pos]);
+        }
+      }
+      __syncwarp();
+      if (listed) s_ch += __shfl_xor_sync(0xffffffffu, s_ch, 8), s_nh += __shfl_xor_sync(0xffffffffu, s_nh, 8), s_ph += __shfl_xor_sync(0xffffffffu, s_ph, 8);
+#pragma unroll
+      for (int o = 4; o > 0; o >>= 1) {
+        s_ch += __shfl_xor_sync(0xffffffffu, s_ch, o);
+        s_nh += __shfl_xor_sync(0xffffffffu, s_nh, o);
+        s_ph += __shfl_xor_sync(0xffffffffu, s_ph, o);
+      }
+      if (active && gl == 0) {
+        prm.iso_charged[a0 + i] = (float)((double)s_ch * kInvFix);
+        prm.iso_neutral[a0 + i] = (float)((double)s_nh * kInvFix);
+        prm.iso_photon[a0 + i] = (float)((double)s_ph * kInvFix);
+        prm.r_iso[a0 + i] = (float)((double)(s_ch + s_nh + s_ph) * kInvFix / (double)o_pt[i]);
+      }
     }
   } else {
     // an event larger than the cache: every warp looks for the leptons among its share of the objects
