@@ -78,6 +78,34 @@ __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, P
       atomicAdd(&s_acc[1], (unsigned long long)s_x);
       atomicAdd(&s_acc[2], (unsigned long long)s_y);
     }
+  } else if (ne >= 8 && n < 48 * ne) {
+    // small events: eight lanes per event, four events per warp pass (the lanes stay busy, and the fold and the
+    // epilogue in double are shared by four events)
+    const int grp = lane >> 3, gl = lane & 7;
+    for (int e4 = 4 * wid; e4 < ne; e4 += 4 * W) {
+      const int e = e4 + grp;
+      long long s_ht = 0, s_x = 0, s_y = 0;
+      if (e < ne)
+        for (int i = s_off[e] + gl; i < s_off[e + 1]; i += 8) {
+          const float pt = o_pt[i];
+          float sn, cs;
+          sincosf(o_phi[i], &sn, &cs);
+          s_ht += to_fix(pt), s_x += to_fix(pt * cs), s_y += to_fix(pt * sn);
+        }
+      __syncwarp();
+#pragma unroll
+      for (int o = 4; o > 0; o >>= 1) {
+        s_ht += __shfl_xor_sync(0xffffffffu, s_ht, o);
+        s_x += __shfl_xor_sync(0xffffffffu, s_x, o);
+        s_y += __shfl_xor_sync(0xffffffffu, s_y, o);
+      }
+      if (e < ne && gl == 0) {
+        const double mx = -(double)s_x * kInvFix, my = -(double)s_y * kInvFix;
+        prm.ht[e0 + e] = (float)((double)s_ht * kInvFix);
+        prm.met_x[e0 + e] = (float)mx, prm.met_y[e0 + e] = (float)my;
+        prm.met[e0 + e] = (float)sqrt(mx * mx + my * my);
+      }
+    }
   } else
   for (int e = wid; e < ne; e += W) {
     long long s_ht = 0, s_x = 0, s_y = 0;
@@ -261,6 +289,9 @@ __global__ void __launch_bounds__(THREADS, 4) pd_features_kernel(const __grid_co
   __shared__ unsigned long long s_acc[3];  // H_T, sum pT cos, sum pT sin of a run that is one big event
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
 
+  const long long n_total = __ldg(prm.offsets + prm.n_events);
+  // bulk prefetches want 16-byte aligned addresses: true for every array of the collection or not used at all
+  const bool pf_ok = ((((uintptr_t)prm.pt | (uintptr_t)prm.eta | (uintptr_t)prm.phi | (uintptr_t)prm.cls) & 15) == 0);
   for (long long chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
     const long long c0 = chunk * events_per_chunk;
     const long long c1 = min(c0 + (long long)events_per_chunk, prm.n_events);
@@ -280,18 +311,46 @@ __global__ void __launch_bounds__(THREADS, 4) pd_features_kernel(const __grid_co
       __syncthreads();
       const int n = s_off[ne];
 
-      // ---- step 1: cache the run; zero the isolation of everything that is not a lepton
-      for (int i = tid; i < n; i += THREADS) {
-        const signed char c = __ldg(prm.cls + a0 + i);
-        if (cached) {
-          s_cls[i] = c;
-          s_pt[i] = __ldg(prm.pt + a0 + i), s_eta[i] = __ldg(prm.eta + a0 + i), s_phi[i] = __ldg(prm.phi + a0 + i);
+      // ---- step 1: cache the run; zero the isolation of everything that is not a lepton.  Four objects per thread at a
+      // time, all their loads issued before the first store (the stores would otherwise fence the loads of the next
+      // iteration: the phase is bound by memory latency)
+      if (tid == 0) {
+        // the objects that follow (the next run of this chunk, most of the time) towards L2 meanwhile
+        const long long nb = a0 + n, ne_ = min(nb + (long long)n, n_total);
+        const long long lo4 = (nb + 3) & ~3ll, hi4 = ne_ & ~3ll, lo16 = (nb + 15) & ~15ll, hi16 = ne_ & ~15ll;
+        if (pf_ok && hi4 > lo4) {
+          const unsigned bytes = (unsigned)(4 * (hi4 - lo4));
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(prm.pt + lo4), "r"(bytes) : "memory");
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(prm.eta + lo4), "r"(bytes) : "memory");
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(prm.phi + lo4), "r"(bytes) : "memory");
         }
-        if (c == PD_CLS_ELECTRON || c == PD_CLS_MUON) {
-          if (cached) s_lep[atomicAdd(&s_nlep, 1u)] = (unsigned short)i;
-        } else {
-          prm.iso_charged[a0 + i] = 0.f, prm.iso_neutral[a0 + i] = 0.f, prm.iso_photon[a0 + i] = 0.f;
-          prm.r_iso[a0 + i] = 0.f;
+        if (pf_ok && hi16 > lo16)
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(prm.cls + lo16), "r"((unsigned)(hi16 - lo16)) : "memory");
+      }
+      for (int i0 = tid; i0 < n; i0 += 4 * THREADS) {
+        signed char c[4];
+        float vp[4], ve[4], vf[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int i = i0 + u * THREADS;
+          c[u] = 0, vp[u] = ve[u] = vf[u] = 0.f;
+          if (i < n) {
+            c[u] = __ldg(prm.cls + a0 + i);
+            if (cached) vp[u] = __ldg(prm.pt + a0 + i), ve[u] = __ldg(prm.eta + a0 + i), vf[u] = __ldg(prm.phi + a0 + i);
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int i = i0 + u * THREADS;
+          if (i < n) {
+            if (cached) s_cls[i] = c[u], s_pt[i] = vp[u], s_eta[i] = ve[u], s_phi[i] = vf[u];
+            if (c[u] == PD_CLS_ELECTRON || c[u] == PD_CLS_MUON) {
+              if (cached) s_lep[atomicAdd(&s_nlep, 1u)] = (unsigned short)i;
+            } else {
+              prm.iso_charged[a0 + i] = 0.f, prm.iso_neutral[a0 + i] = 0.f, prm.iso_photon[a0 + i] = 0.f;
+              prm.r_iso[a0 + i] = 0.f;
+            }
+          }
         }
       }
       __syncthreads();
