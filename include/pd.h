@@ -296,6 +296,23 @@ int64_t pd_truth_workspace_bytes(int64_t n_events);
 int pd_truth_features(const pd_events *events, int32_t skip_neutrinos, pd_features *out, void *workspace,
                       int64_t workspace_bytes, void *cuda_stream);
 
+/* ---- The same, for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): NO workspace argument.  The scratch (the [n_events][3] 64-bit accumulators of
+ * pd_truth_features) lives in a fixed array inside the library, 24 * PD_TRUTH_STATIC_MAX_EVENTS bytes = 6 MiB of device
+ * memory that every GPU which loads the library holds until the process exits.  Inputs, outputs, results and launches
+ * are those of pd_truth_features (bitwise: the sums are exact).  The call makes no cudaMalloc / cudaFree and calls no
+ * allocating library routine; the first call on a device looks the array's device address up (cudaGetSymbolAddress, once
+ * per device, with that device current) -- a call with events->n_events == 0 does just that and returns PD_OK, which is
+ * the way to do the set-up ahead of a capture.
+ * Limit: events->n_events <= PD_TRUTH_STATIC_MAX_EVENTS, else PD_EWORKSPACE ("workspace missing or too small": the
+ * built-in scratch is; use pd_truth_features with a workspace of your own, or split the batch).
+ * The array is SHARED by every call on the device and keeps the last call's contents: each call clears the part it uses
+ * on its stream before summing, so calls ordered on one stream are independent, but calls that overlap on the GPU
+ * (different streams, different host threads) race on it -- serialise them, or use pd_truth_features.
+ * Does not update pd_last_launch_count().  Errors: PD_EINVAL, PD_EWORKSPACE, PD_ECUDA. */
+#define PD_TRUTH_STATIC_MAX_EVENTS 262144
+int pd_truth_features_static(const pd_events *events, int32_t skip_neutrinos, pd_features *out, void *cuda_stream);
+
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 

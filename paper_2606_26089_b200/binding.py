@@ -18,7 +18,7 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_track_impact", "pd_truth_workspace_bytes", "pd_truth_features", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_track_impact", "pd_truth_workspace_bytes", "pd_truth_features", "pd_truth_features_static", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
@@ -131,6 +131,8 @@ def lib():
         L.pd_truth_workspace_bytes.argtypes = [C.c_int64]
         L.pd_truth_workspace_bytes.restype = C.c_int64
         L.pd_truth_features.argtypes = [C.POINTER(Events), C.c_int32, C.POINTER(Features), _p, C.c_int64, _p]
+        L.pd_truth_features_static.argtypes = [C.POINTER(Events), C.c_int32, C.POINTER(Features), _p]
+        L.pd_truth_features_static.restype = C.c_int
         L.pd_track_impact.argtypes = [_p, C.POINTER(Events), C.POINTER(Tracks), C.POINTER(ImpactConfig), C.c_uint64, C.c_int64,
                                       C.POINTER(Impact), _p]
         L.pd_simulate_host.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks),
@@ -375,6 +377,19 @@ def truth_features(dev_events: "DeviceEvents", feat: "DeviceFeatures", skip_neut
     _check(lib().pd_truth_features(C.byref(dev_events.c), int(bool(skip_neutrinos)), C.byref(feat.c), _tptr(workspace),
                                    workspace.numel() * workspace.element_size(), C.c_void_p(st.cuda_stream)))
     return workspace
+
+
+TRUTH_STATIC_MAX_EVENTS = 262144  # PD_TRUTH_STATIC_MAX_EVENTS of pd.h
+
+
+def truth_features_static(dev_events: "DeviceEvents", feat: "DeviceFeatures", skip_neutrinos: bool = True, stream=None):
+    """pd_truth_features_static: as truth_features, with the scratch in a fixed array inside the library (no workspace,
+    no allocation; at most TRUTH_STATIC_MAX_EVENTS events; calls that overlap on the GPU race on it).  Asynchronous."""
+    torch = _torch()
+    if not torch.cuda.is_available():
+        raise PdError(PD_ECUDA)
+    st = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().pd_truth_features_static(C.byref(dev_events.c), int(bool(skip_neutrinos)), C.byref(feat.c), C.c_void_p(st.cuda_stream)))
 
 
 class DeviceTrackRefs:

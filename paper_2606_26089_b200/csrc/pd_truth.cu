@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <mutex>
 
 #include "pd_internal.h"
 
@@ -228,4 +229,52 @@ int pd_launch_truth(const PdTruthParams &prm, void *stream) {
   if (blocks > 4LL * sms) blocks = 4LL * sms;
   pdt::pd_truth_finish_kernel<<<(unsigned)blocks, 256, 0, st>>>(prm);
   return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
+}
+
+// ---- pd_truth_features_static (pd.h): the entry point that allocates nothing ----------------------------------------
+// The accumulators live in a file-scope device array instead of a caller's workspace.  In HOST code the array's name is a
+// host-side stand-in, not a device address: the address the kernels get is looked up with cudaGetSymbolAddress, once per
+// device, with that device current (every device that loads the library has its own copy of the array).
+namespace pdt {
+static __device__ __align__(256) unsigned long long g_static_acc[3 * (size_t)PD_TRUTH_STATIC_MAX_EVENTS];
+}
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned long long *g_static_ptr[kMaxDevices] = {};  // device address of pdt::g_static_acc on device d, once known
+
+// device address of the scratch on the current device; no allocation (the array is part of the loaded module)
+int static_scratch(unsigned long long **out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PD_ECUDA;
+  if (dev < 0 || dev >= kMaxDevices) return PD_ECUDA;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    unsigned long long *ptr = nullptr;
+    if (cudaGetSymbolAddress((void **)&ptr, pdt::g_static_acc) != cudaSuccess || !ptr) return PD_ECUDA;
+    g_static_ptr[dev] = ptr;
+  }
+  *out = g_static_ptr[dev];
+  return PD_OK;
+}
+}  // namespace
+
+extern "C" int pd_truth_features_static(const pd_events *ev, int32_t skip_neutrinos, pd_features *out, void *cuda_stream) {
+  if (!ev || !out || ev->n_events < 0 || ev->n_particles < 0) return PD_EINVAL;
+  if (ev->n_events > (int64_t)PD_TRUTH_STATIC_MAX_EVENTS) return PD_EWORKSPACE;  // the built-in scratch is too small
+  unsigned long long *acc = nullptr;
+  const int rs = static_scratch(&acc);  // also for an empty batch: the set-up call
+  if (rs != PD_OK) return rs;
+  if (ev->n_events == 0) return PD_OK;
+  if (!ev->offsets || !out->ht || !out->met_x || !out->met_y || !out->met) return PD_EINVAL;
+  if (ev->n_particles > 0 && (!ev->pid || !ev->px || !ev->py)) return PD_EINVAL;
+  PdTruthParams p;
+  p.n_events = ev->n_events, p.n_particles = ev->n_particles;
+  p.ev_off = (const long long *)ev->offsets, p.pid = ev->pid, p.px = ev->px, p.py = ev->py;
+  p.skip_neutrinos = skip_neutrinos != 0;
+  p.acc = acc;
+  p.ht = out->ht, p.met_x = out->met_x, p.met_y = out->met_y, p.met = out->met;
+  // clears acc[0 .. 3 n_events) on the stream (the array keeps the last call's contents), then the two kernels
+  return pd_launch_truth(p, cuda_stream);
 }
