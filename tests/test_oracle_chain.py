@@ -19,9 +19,13 @@ def _perfect_card(tmp_path, base="cms_like", **kw):
     return pdo.Card(cards.variant(tmp_path / ("perfect_%s.card" % base), b.edges, b.nphi, base=base, **args))
 
 
-def test_tiny_event_T1(tmp_path):
-    card = _perfect_card(tmp_path)
-    rows = read_table("tiny_event_T1.txt")
+@pytest.mark.parametrize("fixture,base", [("tiny_event_T1.txt", "cms_like"), ("tiny_event_T2_atlas_like.txt", "atlas_like"),
+                                          ("tiny_event_T3_aleph_like.txt", "aleph_like")])
+def test_tiny_worked_events(tmp_path, fixture, base):
+    """Hand-computed tiny events on each built-in card's geometry and grid (an eta grid with two regions, a uniform eta grid,
+    a theta grid): a wrong constant or grid rule of a card shows here, where tower counts and closed forms alone would not."""
+    card = _perfect_card(tmp_path, base)
+    rows = read_table(fixture)
     parts = [r for r in rows if r[0] == "P"]
     ev = from_lists([[particle(int(r[2]), int(r[3]), float(r[4]), float(r[5]), float(r[6]), float(r[8]), 0.0, 0.0, float(r[7]))
                       for r in parts]])
@@ -36,15 +40,17 @@ def test_tiny_event_T1(tmp_path):
     assert list(r["tow_tower"]) == [int(d[1]) for d in dep if d[6] == "1"]
     neu = [x for x in rows if x[0] == "N"]
     nt = len(trk)
-    assert r["efl_offsets"][-1] == nt + len(neu) == 7
-    assert list(r["efl_cls"]) == [0, 2, 0, 0] + [int(x[1]) for x in neu]
+    assert r["efl_offsets"][-1] == nt + len(neu)
+    # class of a track's EFlow entry: hadron 0, electron 1, muon 2
+    trk_cls = [{11: 1, 13: 2}.get(abs(int(parts[int(t[1])][2])), 0) for t in trk]
+    assert list(r["efl_cls"]) == trk_cls + [int(x[1]) for x in neu]
     assert list(r["efl_src"][nt:]) == [int(x[2]) for x in neu]
     assert np.allclose(r["efl_E"][nt:], [float(x[3]) for x in neu], rtol=0, atol=3e-6)
     assert np.allclose(r["efl_eta"][nt:], [float(x[4]) for x in neu], rtol=0, atol=1e-6)
     assert np.allclose(r["efl_phi"][nt:], [float(x[5]) for x in neu], rtol=0, atol=1e-6)
-    # pT of a neutral = E / cosh(eta_c); muon deposits nothing
+    # pT of a neutral = E / cosh(eta_c); a muon deposits nothing
     assert np.allclose(r["efl_pt"][nt:], r["efl_E"][nt:] / np.cosh(r["efl_eta"][nt:]))
-    assert r["dbg_tower"][3] >= 0  # the muon has a geometric tower but no deposit
+    assert r["dbg_tower"][3] >= 0  # the muon (particle 3 of every fixture) has a geometric tower but no deposit
     assert int(r["dbg_tower"][3]) not in set(r["dtw_id"])
 
 
