@@ -316,12 +316,29 @@ int pd_truth_features_static(const pd_events *events, int32_t skip_neutrinos, pd
 /* Number of kernels the last pd_simulate / pd_simulate_host call on this thread launched. */
 int pd_last_launch_count(void);
 
-/* Tuning / testing only: events per on-chip tile of kernel T for the calls this thread makes from now on: 0 (default) =
- * chosen from the average event size with head-room for Poisson-like fluctuations; g >= 1 = at most g (<= 256; 1 also
- * selects the one-CTA-per-SM variant).  Results never depend on it, and no setting is ever needed for correctness:
- * tiles that exceed the on-chip capacity take the (slower) path through the workspace by themselves.
- * pd_workspace_bytes() depends on it: call it after changing the setting.  Returns the previous value. */
-int pd_set_tile_events(int g);
+/* ---- Options, and the set-up that can be done ahead of the first call ----
+ * The library keeps no state between calls: what used to be a per-thread setting (the events per tile) is an argument.
+ * pd_options: plain data, all zero = the defaults; a NULL pointer means the same.
+ *   tile_events: tuning / testing only.  Events per on-chip tile of kernel T: 0 = chosen from the average event size with
+ *     head-room for Poisson-like fluctuations; g >= 1 = at most g (<= 256; 1 also selects the one-CTA-per-SM variant).
+ *     Results never depend on it, and no setting is ever needed for correctness: tiles that exceed the on-chip capacity
+ *     take the (slower) path through the workspace by themselves.  The workspace size depends on it: size the workspace
+ *     with pd_workspace_bytes_ex and the same options.
+ * pd_workspace_bytes_ex / pd_simulate_ex: pd_workspace_bytes / pd_simulate with options (those two = options NULL). */
+typedef struct pd_options {
+  int32_t tile_events;
+  int32_t reserved[7]; /* must be 0 */
+} pd_options;
+int64_t pd_workspace_bytes_ex(const pd_card *card, int64_t n_events, int64_t n_particles, const pd_options *options);
+int pd_simulate_ex(const pd_card *card, const pd_events *events, uint64_t seed, int64_t event_base,
+                   pd_tracks *tracks, pd_towers *towers, pd_eflow *eflow, pd_debug *debug,
+                   void *workspace, int64_t workspace_bytes, const pd_options *options, void *cuda_stream);
+
+/* Copies the card's per-bin tables (a few KB) to the CURRENT device, if they are not there yet: one cudaMalloc and one
+ * synchronous copy per (card, device), kept until pd_free_card.  pd_simulate does this by itself on its first call with a
+ * card on a device; after pd_card_upload, pd_simulate / pd_simulate_ex allocate nothing and can run where allocation is
+ * not allowed.  A card can be resident on up to 16 devices at once.  Errors: PD_EINVAL, PD_ECUDA. */
+int pd_card_upload(const pd_card *card);
 
 /* Same computation with HOST pointers everywhere (inputs and outputs in host memory, pinned or
  * pageable).  Copies inputs to the device, runs pd_simulate, copies the three collections back and

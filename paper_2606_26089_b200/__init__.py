@@ -4,4 +4,4 @@
 There is no CPU fallback."""
 from . import binding  # noqa: F401
 from .binding import (Card, DeviceEFlow, DeviceImpact, DeviceTrackRefs, DeviceEvents, DeviceFeatures, DeviceMerged, DeviceObjects, DeviceOutputs, HostBuffers, PdError, last_launch_count, last_status,  # noqa: F401
-                      event_features, filter_eflow, pileup_merge, pileup_status, set_tile_events, simulate, simulate_host, track_impact, truth_features, truth_features_static, workspace_bytes)
+                      event_features, filter_eflow, pileup_merge, pileup_status, card_upload, simulate, simulate_host, track_impact, truth_features, truth_features_static, workspace_bytes)

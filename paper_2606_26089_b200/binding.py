@@ -18,10 +18,15 @@ PD_DEC_EEM, PD_DEC_EHAD, PD_DEC_NEM, PD_DEC_NHAD = 1, 2, 4, 8
 
 # every symbol include/pd.h declares
 SYMBOLS = ("pd_load_card", "pd_free_card", "pd_card_info", "pd_workspace_bytes", "pd_simulate", "pd_last_status",
-           "pd_last_launch_count", "pd_set_tile_events", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_track_impact", "pd_truth_workspace_bytes", "pd_truth_features", "pd_truth_features_static", "pd_simulate_host", "pd_strerror")
+           "pd_last_launch_count", "pd_workspace_bytes_ex", "pd_simulate_ex", "pd_card_upload", "pd_event_features", "pd_filter_workspace_bytes", "pd_filter_eflow", "pd_pileup_workspace_bytes", "pd_pileup_merge", "pd_track_impact", "pd_truth_workspace_bytes", "pd_truth_features", "pd_truth_features_static", "pd_simulate_host", "pd_strerror")
 
 _p = C.c_void_p
 _lib = None
+
+
+class Options(C.Structure):
+    """pd_options"""
+    _fields_ = [("tile_events", C.c_int32), ("reserved", C.c_int32 * 7)]
 
 
 class CardInfo(C.Structure):
@@ -118,7 +123,11 @@ def lib():
                                   C.POINTER(EFlow), C.POINTER(Debug), _p, C.c_int64, _p]
         L.pd_last_status.argtypes = [_p, _p]
         L.pd_last_launch_count.argtypes = []
-        L.pd_set_tile_events.argtypes = [C.c_int]
+        L.pd_workspace_bytes_ex.argtypes = [_p, C.c_int64, C.c_int64, C.POINTER(Options)]
+        L.pd_workspace_bytes_ex.restype = C.c_int64
+        L.pd_simulate_ex.argtypes = [_p, C.POINTER(Events), C.c_uint64, C.c_int64, C.POINTER(Tracks), C.POINTER(Towers),
+                                     C.POINTER(EFlow), C.POINTER(Debug), _p, C.c_int64, C.POINTER(Options), _p]
+        L.pd_card_upload.argtypes = [_p]
         L.pd_pileup_workspace_bytes.argtypes = [C.c_int64]
         L.pd_pileup_workspace_bytes.restype = C.c_int64
         L.pd_pileup_merge.argtypes = [C.POINTER(Events), C.POINTER(Events), C.POINTER(PileupConfig), C.c_uint64, C.c_int64,
@@ -174,21 +183,22 @@ class Card:
             self._h = None
 
 
-def workspace_bytes(card: Card, n_events: int, n_particles: int) -> int:
-    n = lib().pd_workspace_bytes(card._h, int(n_events), int(n_particles))
+def workspace_bytes(card: Card, n_events: int, n_particles: int, tile_events: int = 0) -> int:
+    """pd_workspace_bytes_ex; tile_events: pd_options.tile_events (0 = automatic; a tuning knob)."""
+    opt = Options(int(tile_events))
+    n = lib().pd_workspace_bytes_ex(card._h, int(n_events), int(n_particles), C.byref(opt))
     if n < 0:
         raise PdError(n)
     return int(n)
 
 
+def card_upload(card: Card):
+    """pd_card_upload: the card's tables to the current device now, so that simulate() allocates nothing later."""
+    _check(lib().pd_card_upload(card._h))
+
+
 def last_launch_count() -> int:
     return int(lib().pd_last_launch_count())
-
-
-def set_tile_events(g: int) -> int:
-    """pd_set_tile_events: events per on-chip tile (0 = automatic); returns the previous setting.  Buffers
-    made by DeviceOutputs before the call keep the workspace size of the old setting."""
-    return int(lib().pd_set_tile_events(int(g)))
 
 
 def _torch():
@@ -221,8 +231,9 @@ class DeviceEvents:
 class DeviceOutputs:
     """Output buffers (torch tensors) sized to the sufficient bounds of pd.h, plus the workspace."""
 
-    def __init__(self, card: Card, n_events: int, n_particles: int, debug: bool = False, device="cuda"):
+    def __init__(self, card: Card, n_events: int, n_particles: int, debug: bool = False, device="cuda", tile_events: int = 0):
         torch = _torch()
+        self.tile_events = int(tile_events)  # pd_options.tile_events for the calls that use these buffers (sizes the workspace)
         n = max(int(n_particles), 1)
         self.n_events, self.n_particles = int(n_events), int(n_particles)
         mk = lambda m, dt: torch.empty(m, dtype=getattr(torch, dt), device=device)  # noqa: E731
@@ -230,7 +241,7 @@ class DeviceOutputs:
         self.tow = {"offsets": mk(n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TOWER_FIELDS}}
         self.efl = {"offsets": mk(n_events + 1, "int64"), **{k: mk(2 * n, dt) for k, dt in EFLOW_FIELDS}}
         self.dbg = {k: mk(n, dt) for k, dt in DEBUG_FIELDS} if debug else None
-        self.ws_bytes = workspace_bytes(card, n_events, n_particles)
+        self.ws_bytes = workspace_bytes(card, n_events, n_particles, self.tile_events)
         self.ws = torch.empty(self.ws_bytes + 16, dtype=torch.uint8, device=device)
         self.c_trk = Tracks(n, _tptr(self.trk["offsets"]), *[_tptr(self.trk[k]) for k, _ in TRACK_FIELDS])
         self.c_tow = Towers(n, _tptr(self.tow["offsets"]), *[_tptr(self.tow[k]) for k, _ in TOWER_FIELDS])
@@ -434,14 +445,15 @@ def track_impact(card: Card, dev_events: DeviceEvents, tracks, out: DeviceImpact
 
 
 def simulate(card: Card, dev_events: DeviceEvents, out: DeviceOutputs, seed: int, event_base: int = 0, stream=None):
-    """pd_simulate on torch's current stream (or `stream`).  Asynchronous."""
+    """pd_simulate_ex on torch's current stream (or `stream`), with the options `out` was made for.  Asynchronous."""
     torch = _torch()
     if not torch.cuda.is_available():
         raise PdError(PD_ECUDA)
     st = torch.cuda.current_stream() if stream is None else stream
-    rc = lib().pd_simulate(card._h, C.byref(dev_events.c), int(seed) & (2**64 - 1), int(event_base), C.byref(out.c_trk),
-                           C.byref(out.c_tow), C.byref(out.c_efl), C.byref(out.c_dbg) if out.c_dbg is not None else None,
-                           _tptr(out.ws), out.ws_bytes, C.c_void_p(st.cuda_stream))
+    opt = Options(int(getattr(out, "tile_events", 0)))
+    rc = lib().pd_simulate_ex(card._h, C.byref(dev_events.c), int(seed) & (2**64 - 1), int(event_base), C.byref(out.c_trk),
+                              C.byref(out.c_tow), C.byref(out.c_efl), C.byref(out.c_dbg) if out.c_dbg is not None else None,
+                              _tptr(out.ws), out.ws_bytes, C.byref(opt), C.c_void_p(st.cuda_stream))
     _check(rc)
 
 

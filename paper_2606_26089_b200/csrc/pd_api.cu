@@ -95,7 +95,8 @@ int pd_load_card(const char *name_or_path, pd_card **out) {
 
 void pd_free_card(pd_card *card) {
   if (!card) return;
-  if (card->dev_blob) cudaFree(card->dev_blob);
+  for (int k = 0; k < card->n_dev; ++k)
+    if (card->dev_blob[k]) cudaFree(card->dev_blob[k]);
   delete card;
 }
 
@@ -111,16 +112,32 @@ int pd_card_info(const pd_card *card, pd_card_info_t *out) {
   return PD_OK;
 }
 
-int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles) {
-  if (!card || n_events < 0 || n_particles < 0) return PD_EINVAL;
+static int tile_events_of(const pd_options *opt) { return opt ? opt->tile_events : 0; }
+static bool options_ok(const pd_options *opt) {
+  if (!opt) return true;
+  if (opt->tile_events < 0) return false;
+  for (int k = 0; k < 7; ++k)
+    if (opt->reserved[k] != 0) return false;
+  return true;
+}
+
+int64_t pd_workspace_bytes_ex(const pd_card *card, int64_t n_events, int64_t n_particles, const pd_options *opt) {
+  if (!card || n_events < 0 || n_particles < 0 || !options_ok(opt)) return PD_EINVAL;
   PdLaunchPlan plan;
-  pd_plan(card, n_events, n_particles, &plan);
+  pd_plan(card, n_events, n_particles, tile_events_of(opt), &plan);
   return (int64_t)ws_layout(plan, card->sc.n_towers).total;
+}
+int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles) {
+  return pd_workspace_bytes_ex(card, n_events, n_particles, nullptr);
+}
+
+int pd_card_upload(const pd_card *card) {
+  if (!card) return PD_EINVAL;
+  const PdCardTables *tab = nullptr;
+  return pd_card_to_device(card, &tab);
 }
 
 int pd_last_launch_count(void) { return t_launches; }
-
-int pd_set_tile_events(int g) { return pd_plan_set_tile_events(g); }
 
 // pile-up workspace: [tile counter, status word, pad] 16 B | scan words, one per 1,024 events | sizes, 8 B per event
 static size_t pileup_chain_bytes(int64_t n_events) {
@@ -333,16 +350,21 @@ int pd_track_impact(const pd_card *card, const pd_events *ev, const pd_tracks *t
 
 }  // extern "C"
 
-// Upload the per-bin tables of a card to the current device (once).
-int pd_card_to_device(const pd_card *c) {
+// The per-bin tables of a card on the current device: uploaded on first use, kept per device until pd_free_card.
+int pd_card_to_device(const pd_card *c, const PdCardTables **tab) {
   std::lock_guard<std::mutex> lock(g_card_mutex);
   int dev = 0;
   PD_CUDA(cudaGetDevice(&dev));
-  if (c->dev_blob && c->dev_id == dev) return PD_OK;
-  if (c->dev_blob) {
-    cudaFree(c->dev_blob);
-    c->dev_blob = nullptr;
+  for (int k = 0; k < c->n_dev; ++k)
+    if (c->dev_id[k] == dev) {
+      *tab = &c->dev_tab[k];
+      return PD_OK;
+    }
+  if (c->n_dev >= PD_MAX_CARD_DEVICES) {
+    std::snprintf(t_cuda_msg, sizeof(t_cuda_msg), "card already resident on %d devices", PD_MAX_CARD_DEVICES);
+    return PD_ECUDA;
   }
+  const int slot = c->n_dev;
   const size_t nb = (size_t)c->sc.n_bins;
   const size_t lut_words = (c->lut.size() + 1) / 2;
   const size_t words = (nb + 1) + nb + (nb + 1) + 5 * nb + lut_words + (nb + 1) + 6 * nb;
@@ -369,19 +391,21 @@ int pd_card_to_device(const pd_card *c) {
     return cuda_fail(e, "cudaMemcpy(card)");
   }
   const uint32_t *base = (const uint32_t *)d;
-  c->dev_tab.tb = (const float *)(base + o_tb);
-  c->dev_tab.nphi = (const int *)(base + o_nphi);
-  c->dev_tab.offset = (const int *)(base + o_off);
-  c->dev_tab.inv_w = (const float *)(base + o_iw);
-  c->dev_tab.half = (const float *)(base + o_half);
-  c->dev_tab.w = (const float *)(base + o_w);
-  c->dev_tab.eta_c = (const float *)(base + o_eta);
-  c->dev_tab.inv_cosh = (const float *)(base + o_ic);
-  c->dev_tab.lut = (const unsigned short *)(base + o_lut);
-  c->dev_tab.edge = (const float *)(base + o_edge);
-  c->dev_tab.res2 = (const float *)(base + o_res2);
-  c->dev_blob = d;
-  c->dev_id = dev;
+  c->dev_tab[slot].tb = (const float *)(base + o_tb);
+  c->dev_tab[slot].nphi = (const int *)(base + o_nphi);
+  c->dev_tab[slot].offset = (const int *)(base + o_off);
+  c->dev_tab[slot].inv_w = (const float *)(base + o_iw);
+  c->dev_tab[slot].half = (const float *)(base + o_half);
+  c->dev_tab[slot].w = (const float *)(base + o_w);
+  c->dev_tab[slot].eta_c = (const float *)(base + o_eta);
+  c->dev_tab[slot].inv_cosh = (const float *)(base + o_ic);
+  c->dev_tab[slot].lut = (const unsigned short *)(base + o_lut);
+  c->dev_tab[slot].edge = (const float *)(base + o_edge);
+  c->dev_tab[slot].res2 = (const float *)(base + o_res2);
+  c->dev_blob[slot] = d;
+  c->dev_id[slot] = dev;
+  c->n_dev = slot + 1;
+  *tab = &c->dev_tab[slot];
   return PD_OK;
 }
 
@@ -389,9 +413,9 @@ int pd_card_to_device(const pd_card *c) {
 // chunk for the pipelined host entry, whose chunks keep absolute offsets into the whole-batch arrays
 static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
                          pd_towers *tow, pd_eflow *efl, pd_debug *dbg, void *workspace, int64_t workspace_bytes,
-                         void *cuda_stream, int64_t particle_base) {
+                         void *cuda_stream, int64_t particle_base, const pd_options *opt = nullptr) {
   t_launches = 0;
-  if (!card || !ev || !trk || !tow || !efl) return PD_EINVAL;
+  if (!card || !ev || !trk || !tow || !efl || !options_ok(opt)) return PD_EINVAL;
   if (ev->n_events < 0 || ev->n_particles < 0 || ev->n_particles >= (int64_t(1) << 30)) return PD_EINVAL;
   if (!ev->offsets || !trk->offsets || !tow->offsets || !efl->offsets) return PD_EINVAL;
   const int64_t n = ev->n_particles;
@@ -402,12 +426,12 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
     if (!efl->cls || !efl->src || !efl->pt || !efl->eta || !efl->phi || !efl->E) return PD_EINVAL;
   }
   if (trk->capacity < n || tow->capacity < n || efl->capacity < 2 * n) return PD_ECAPACITY;
-  const int64_t need = pd_workspace_bytes(card, ev->n_events, n);
+  const int64_t need = pd_workspace_bytes_ex(card, ev->n_events, n, opt);
   if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15u)) return PD_EWORKSPACE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
 
   PdLaunchPlan plan;
-  pd_plan(card, ev->n_events, n, &plan);
+  pd_plan(card, ev->n_events, n, tile_events_of(opt), &plan);
   PD_CUDA(cudaMemsetAsync(workspace, 0, ws_chain_bytes(plan), st));  // counters + look-back words; the keys need no init
   if (ev->n_events == 0) {
     PD_CUDA(cudaMemsetAsync(trk->offsets, 0, sizeof(int64_t), st));
@@ -415,13 +439,14 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
     PD_CUDA(cudaMemsetAsync(efl->offsets, 0, sizeof(int64_t), st));
     return PD_OK;
   }
-  int rc = pd_card_to_device(card);
+  const PdCardTables *tab = nullptr;
+  int rc = pd_card_to_device(card, &tab);
   if (rc != PD_OK) return rc;
 
   PdParams p;
   std::memset(&p, 0, sizeof(p));
   p.sc = card->sc;
-  p.tab = card->dev_tab;
+  p.tab = *tab;
   p.n_events = ev->n_events, p.n_particles = n;
   p.offsets = (const long long *)ev->offsets;
   p.pid = ev->pid, p.charge = ev->charge;
@@ -493,6 +518,12 @@ int pd_simulate(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t
                 pd_towers *tow, pd_eflow *efl, pd_debug *dbg, void *workspace, int64_t workspace_bytes,
                 void *cuda_stream) {
   return simulate_impl(card, ev, seed, event_base, trk, tow, efl, dbg, workspace, workspace_bytes, cuda_stream, 0);
+}
+
+int pd_simulate_ex(const pd_card *card, const pd_events *ev, uint64_t seed, int64_t event_base, pd_tracks *trk,
+                   pd_towers *tow, pd_eflow *efl, pd_debug *dbg, void *workspace, int64_t workspace_bytes,
+                   const pd_options *opt, void *cuda_stream) {
+  return simulate_impl(card, ev, seed, event_base, trk, tow, efl, dbg, workspace, workspace_bytes, cuda_stream, 0, opt);
 }
 
 int pd_last_status(const void *workspace, void *cuda_stream) {
@@ -849,14 +880,6 @@ int pd_simulate_host(const pd_card *card, const pd_events *ev, uint64_t seed, in
   }
   int rc = K > 1 ? simulate_host_pipelined(card, ev, seed, event_base, trk, tow, efl, cuda_stream, K)
                  : simulate_host_once(card, ev, seed, event_base, trk, tow, efl, cuda_stream);
-  if (rc == PD_EEVENTSIZE) {
-    // a tile of the automatic plan did not fit on chip (event sizes far from Poisson): one event per tile
-    const int launches = t_launches;
-    const int prev = pd_plan_set_tile_events(1);
-    if (prev != 1) rc = simulate_host_once(card, ev, seed, event_base, trk, tow, efl, cuda_stream);
-    pd_plan_set_tile_events(prev);
-    t_launches += launches;
-  }
   return rc;
 }
 

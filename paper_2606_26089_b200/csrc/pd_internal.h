@@ -65,6 +65,7 @@ struct PdCardTables {
   const float *res2;      // [n_bins][6] ECAL C^2, S^2, N^2, HCAL C^2, S^2, N^2 of the bin's towers (reading K1)
 };
 
+constexpr int PD_MAX_CARD_DEVICES = 16;
 struct pd_card {
   std::string name;
   // host copy (rounded to fp32 where the kernels use fp32)
@@ -77,9 +78,11 @@ struct pd_card {
   float bz = 0.f;
   int n_eff_rows = 0;
   // device copy, created lazily by the first simulate call
-  mutable void *dev_blob = nullptr;
-  mutable int dev_id = -1;
-  mutable PdCardTables dev_tab{};
+  // the tables on the devices that have used the card (pd_card_to_device): slot k holds device dev_id[k]
+  mutable void *dev_blob[PD_MAX_CARD_DEVICES] = {};
+  mutable int dev_id[PD_MAX_CARD_DEVICES] = {};
+  mutable PdCardTables dev_tab[PD_MAX_CARD_DEVICES] = {};
+  mutable int n_dev = 0;
 };
 
 // Philox4x32-10 round keys of the call's seed: (seed lo + r W0, seed hi + r W1), r = 0..9
@@ -165,7 +168,7 @@ struct PdParams {
 // pd_card.cpp
 int pd_card_parse(const char *name_or_path, pd_card *c);
 // pd_api.cu
-int pd_card_to_device(const pd_card *c);
+int pd_card_to_device(const pd_card *c, const PdCardTables **tab);  // tables on the current device (uploaded once)
 // pd_towers.cu
 struct PdLaunchPlan {
   int threads;       // 512 (two CTAs per SM) or 1024 (one)
@@ -178,8 +181,7 @@ struct PdLaunchPlan {
   size_t smem_bytes;
   PdTLayout lay;
 };
-int pd_plan_set_tile_events(int g);
-int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan);
+int pd_plan(const pd_card *c, long long n_events, long long n_particles, int tile_events, PdLaunchPlan *plan);  // tile_events: 0 = automatic
 int pd_launch_chain(const PdParams &prm, const PdLaunchPlan &plan, bool debug, void *stream);
 // pd_particles.cu
 int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_smem_optin, void *stream);

@@ -966,14 +966,9 @@ static int query_device() {
 // CTA's barriers and look-back waits are covered by the other; events too large for that get one 1024-thread CTA
 // with the whole SM.  G = events per tile: as many as fit the on-chip capacity C with 6 sigma of head-room
 // for a Poisson-like sum, but no more than keeps every CTA slot of the GPU busy on small inputs.
-static thread_local int t_tile_events = 0;  // pd_set_tile_events: 0 = automatic
-int pd_plan_set_tile_events(int g) {
-  const int prev = t_tile_events;
-  t_tile_events = g < 0 ? 0 : (g > pdk::G_MAX ? pdk::G_MAX : g);
-  return prev;
-}
-
-int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunchPlan *plan) {
+// tile_events: the caller's cap on the events per tile (pd_options.tile_events), 0 = automatic
+int pd_plan(const pd_card *c, long long n_events, long long n_particles, int tile_events, PdLaunchPlan *plan) {
+  const int t_tile_events = tile_events < 0 ? 0 : (tile_events > pdk::G_MAX ? pdk::G_MAX : tile_events);
   const PdCardScalars &sc = c->sc;
   const double avg = n_events > 0 ? double(n_particles) / double(n_events) : 0.0;
   const size_t budget2 = (228 * 1024 - 2 * 1024) / 2, budget1 = 227 * 1024;
@@ -992,7 +987,7 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, PdLaunc
   static const int force_threads = std::getenv("PD_THREADS") ? std::atoi(std::getenv("PD_THREADS")) : 0;
   size_t budget = budget2;
   plan->threads = 512;
-  // one event per tile on request (pd_set_tile_events(1), the fall-back for batches with outlier events): the
+  // one event per tile on request (pd_options.tile_events = 1): the
   // large variant, so that the only limit left is the capacity of a whole SM
   if (force_threads == 1024 || t_tile_events == 1 || (force_threads == 0 && !fits(1, budget2))) {
     budget = budget1;

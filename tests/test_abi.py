@@ -66,6 +66,19 @@ def test_argument_checking_without_gpu():
     assert L.pd_simulate(c._h, C.byref(ev), 1, 0, C.byref(trk), C.byref(tow), C.byref(efl), None, None, 0, None) == B.PD_EINVAL
     assert L.pd_simulate(None, C.byref(ev), 1, 0, C.byref(trk), C.byref(tow), C.byref(efl), None, None, 0, None) == B.PD_EINVAL
     assert L.pd_strerror(B.PD_ECAPACITY).decode().startswith("output capacity")
+    # options (pd_options): NULL and all-zero are the defaults; the workspace size depends on the events per tile;
+    # negative values and non-zero reserved fields are refused; the library keeps no per-thread setting
+    dflt = B.workspace_bytes(c, 1000, 60000)
+    assert L.pd_workspace_bytes_ex(c._h, 1000, 60000, None) == dflt == L.pd_workspace_bytes(c._h, 1000, 60000)
+    assert 0 < B.workspace_bytes(c, 1000, 60000, tile_events=1) != dflt
+    assert B.workspace_bytes(c, 1000, 60000) == dflt  # ... and the call before left nothing behind
+    bad = B.Options(-1)
+    assert L.pd_workspace_bytes_ex(c._h, 1000, 60000, C.byref(bad)) == B.PD_EINVAL
+    bad = B.Options(0)
+    bad.reserved[3] = 1
+    assert L.pd_workspace_bytes_ex(c._h, 1000, 60000, C.byref(bad)) == B.PD_EINVAL
+    assert L.pd_simulate_ex(c._h, C.byref(ev), 1, 0, C.byref(trk), C.byref(tow), C.byref(efl), None, None, 0, C.byref(bad), None) == B.PD_EINVAL
+    assert L.pd_card_upload(None) == B.PD_EINVAL
 
 
 def test_no_cpu_fallback():

@@ -91,3 +91,28 @@ def test_results_do_not_depend_on_the_number_of_resident_ctas(case, monkeypatch)
             continue
         for k, v in got.items():
             assert v.tobytes() == ref[k].tobytes(), (case, p_per_sm, t_per_sm, k)
+
+
+def test_after_card_upload_a_step_allocates_no_device_memory():
+    """pd_card_upload (pd.h): the one allocation of the chain -- the card's tables on a device -- done ahead of time; the step
+    itself (pd_simulate_ex with caller-owned buffers and workspace) then leaves the free device memory as it found it."""
+    import torch
+
+    import paper_2606_26089_b200 as pd
+
+    card = pd.Card("atlas_like")  # a card object no earlier test has used on the device
+    ev = wl.generate(3, 2000)
+    dev = pd.DeviceEvents(ev)
+    out = pd.DeviceOutputs(card, dev.n_events, dev.n_particles, debug=False)
+    warm = pd.Card("cms_like")    # module load, kernel attributes and first launches, on another card
+    pd.simulate(warm, pd.DeviceEvents(wl.generate(0, 50)), pd.DeviceOutputs(warm, 50, wl.generate(0, 50).n_particles), 1)
+    torch.cuda.synchronize()
+    pd.card_upload(card)
+    pd.card_upload(card)  # idempotent
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    pd.simulate(card, dev, out, 7)
+    torch.cuda.synchronize()
+    free1, _ = torch.cuda.mem_get_info()
+    assert pd.last_status(out) == 0 and int(out.trk["offsets"][-1]) > 0
+    assert free1 == free0, (free0, free1)

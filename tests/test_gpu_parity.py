@@ -188,12 +188,8 @@ def test_skewed_event_sizes_take_the_big_tile_path():
     auto = run_gpu("cms_like", ev, 21)
     assert auto["status_word"] == 0
     _check(compare("cms_like", ev, 21, auto))
-    prev = pd.set_tile_events(1)
-    try:
-        one = run_gpu("cms_like", ev, 21)
-        assert one["status_word"] == 0
-    finally:
-        pd.set_tile_events(prev)
+    one = run_gpu("cms_like", ev, 21, tile_events=1)  # pd_options.tile_events = 1: one event per tile, 1,024-thread variant
+    assert one["status_word"] == 0
     for k, v in one.items():
         if isinstance(v, np.ndarray):
             assert v.tobytes() == auto[k].tobytes(), k
