@@ -42,6 +42,9 @@ struct pdo_card {
   /* higher card fidelity (readings K1-K3 of DESIGN.md section 17) */
   int n_ecal_eta, n_hcal_eta;            /* K1: rows (aeta_lo, aeta_hi, C, S, N) by the tower centre's |eta|  */
   double ecal_eta[PDO_MAX_RES_ROWS][5], hcal_eta[PDO_MAX_RES_ROWS][5];
+  /* K4: track resolution rows (aeta_lo, aeta_hi, a, b, species 0..3) by the |eta| of the true momentum; sinh of the edges */
+  int n_trk_eta;
+  double trk_eta[PDO_MAX_RES_ROWS][5], trk_eta_sinh[PDO_MAX_RES_ROWS][2];
   double nsig_ecal, nsig_hcal;           /* K2: component kept iff also E' > n_sigma sigma(E')                  */
   int smear_center;                      /* K3: reported tower (eta, phi) uniform inside the cell               */
 };
@@ -103,6 +106,11 @@ static void card_finish(pdo_card *c) {
   for (i = 0; i < c->n_hcal_eta; ++i) {
     int k;
     for (k = 0; k < 5; ++k) c->hcal_eta[i][k] = f32(c->hcal_eta[i][k]);
+  }
+  for (i = 0; i < c->n_trk_eta; ++i) {
+    int k;
+    for (k = 0; k < 4; ++k) c->trk_eta[i][k] = f32(c->trk_eta[i][k]);
+    c->trk_eta_sinh[i][0] = sinh(c->trk_eta[i][0]), c->trk_eta_sinh[i][1] = sinh(c->trk_eta[i][1]); /* sinh(inf) = inf */
   }
   c->nsig_ecal = f32(c->nsig_ecal);
   c->nsig_hcal = f32(c->nsig_hcal);
@@ -249,6 +257,11 @@ static int card_from_file(pdo_card *c, const char *path) {
     else if (!strcmp(key, "hcal_res") && nv == 3) memcpy(c->hcal, v, 3 * sizeof(double));
     else if (!strcmp(key, "ecal_res_eta") && nv == 5 && c->n_ecal_eta < PDO_MAX_RES_ROWS) memcpy(c->ecal_eta[c->n_ecal_eta++], v, 5 * sizeof(double));
     else if (!strcmp(key, "hcal_res_eta") && nv == 5 && c->n_hcal_eta < PDO_MAX_RES_ROWS) memcpy(c->hcal_eta[c->n_hcal_eta++], v, 5 * sizeof(double));
+    else if (!strcmp(key, "track_res_eta") && (nv == 4 || (nv == 5 && (v[4] == 0.0 || v[4] == 1.0 || v[4] == 2.0 || v[4] == 3.0))) &&
+             c->n_trk_eta < PDO_MAX_RES_ROWS) {
+      if (nv == 4) v[4] = 0.0;
+      memcpy(c->trk_eta[c->n_trk_eta++], v, 5 * sizeof(double));
+    }
     else if (!strcmp(key, "ecal_nsigma") && nv == 1) c->nsig_ecal = v[0];
     else if (!strcmp(key, "hcal_nsigma") && nv == 1) c->nsig_hcal = v[0];
     else if (!strcmp(key, "smear_tower_center") && nv == 1) c->smear_center = v[0] != 0.0;
@@ -383,6 +396,27 @@ double pdo_lognormal(double m, double s, double z) {
 
 static double resolution(const double csn[3], double E) {
   return sqrt(csn[0] * csn[0] * E * E + csn[1] * csn[1] * E + csn[2] * csn[2]);
+}
+
+/* reading K4: (a, b) of step S3 for a track of the given species with true vertex momentum
+ * (px, py, pz): the first track_res_eta row, in file order, that names no species or this one and whose
+ * [aeta_lo, aeta_hi) holds |eta_mom| -- decided as sinh(aeta_lo) pT <= |pz| < sinh(aeta_hi) pT in fp64 (pT = sqrt(px^2 +
+ * py^2), products and sum rounded one by one), the form in which the CUDA path can take the same decision bit for bit;
+ * else reading J2: the species' own track_res line, else the card's common one.  Returns the row or -1. */
+int pdo_track_resolution(const pdo_card *c, int species, double px, double py, double pz, double *a, double *b) {
+  const double pt = sqrt(px * px + py * py), apz = fabs(pz);
+  int r;
+  if (species < 1 || species > 3) species = PDO_SPECIES_CHHAD;
+  for (r = 0; r < c->n_trk_eta; ++r) {
+    const int sp = (int)c->trk_eta[r][4];
+    if ((sp == 0 || sp == species) && apz >= c->trk_eta_sinh[r][0] * pt && apz < c->trk_eta_sinh[r][1] * pt) {
+      *a = c->trk_eta[r][2], *b = c->trk_eta[r][3];
+      return r;
+    }
+  }
+  *a = c->has_trk_species[species] ? c->trk_a_species[species] : c->trk_a;
+  *b = c->has_trk_species[species] ? c->trk_b_species[species] : c->trk_b;
+  return -1;
 }
 
 /* reading K1: (C, S, N) of a tower = the first row whose [aeta_lo, aeta_hi) holds the |eta| of the tower CENTRE, else the
@@ -808,9 +842,10 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
           if (accepted) {
             /* track smearing (A12, A13): log-normal, mean pT, std sigma_rel pT; eta, phi unchanged */
             /* reading J2: the resolution given for the particle's species, else the card's common one */
-            const double ta = c->has_trk_species[species] ? c->trk_a_species[species] : c->trk_a;
-            const double tb = c->has_trk_species[species] ? c->trk_b_species[species] : c->trk_b;
-            double srel = sqrt(ta * ta + (tb * pt) * (tb * pt));
+            /* reading K4: an eta-dependent row of the card first */
+            double ta, tb, srel;
+            pdo_track_resolution(c, species, px, py, pz, &ta, &tb);
+            srel = sqrt(ta * ta + (tb * pt) * (tb * pt));
             pt_smeared = pdo_lognormal(pt, srel * pt, pdo_normal(r[1], r[2]));
             Etrk = pt_smeared * cosh(eta_mom);
             if (n_trk >= trk->capacity || n_efl >= efl->capacity) {

@@ -285,6 +285,10 @@ double pdo_efficiency(const pdo_card *card, double pt, double eta_mom, double ab
  * charged-hadron case (identical for cards whose rows name no species) */
 enum { PDO_SPECIES_ALL = 0, PDO_SPECIES_ELECTRON = 1, PDO_SPECIES_MUON = 2, PDO_SPECIES_CHHAD = 3 };
 double pdo_efficiency_species(const pdo_card *c, double pt, double eta_mom, double abs_costheta, int species, int *row);
+/* reading K4 (eta-dependent track resolution rows, card key track_res_eta = aeta_lo aeta_hi a b [species]): the (a, b) of
+ * sigma_rel = sqrt(a^2 + (b pT)^2) for a track of the species with true momentum (px, py, pz); returns the row, -1 = the
+ * species' / the card's track_res line (reading J2) */
+int pdo_track_resolution(const pdo_card *c, int species, double px, double py, double pz, double *a, double *b);
 
 #ifdef __cplusplus
 }

@@ -108,6 +108,8 @@ def lib():
         L.pdo_efficiency.restype = C.c_double
         L.pdo_efficiency_species.argtypes = [_p, C.c_double, C.c_double, C.c_double, C.c_int, C.POINTER(C.c_int)]
         L.pdo_efficiency_species.restype = C.c_double
+        L.pdo_track_resolution.argtypes = [_p, C.c_int, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.pdo_track_resolution.restype = C.c_int
         L.pdo_pileup_merge.argtypes = [C.POINTER(_Events), C.POINTER(_Events), C.c_double, C.c_double, C.c_double, C.c_int,
                                        C.c_uint64, C.c_int64, C.c_int64] + [_p] * 12
         L.pdo_filter_eflow.argtypes = [C.c_int64] + [_p] * 7 + [C.POINTER(_Condition), C.c_int32, C.c_int32] + [_p] * 8
@@ -171,6 +173,12 @@ class Card:
         else:
             eps = lib().pdo_efficiency_species(self._h, float(pt), float(eta_mom), float(abs_costheta), int(species), C.byref(row))
         return eps, row.value
+
+    def track_resolution(self, species, px, py, pz):
+        """(row, a, b) of reading K4 / J2 for a track of the species (1 electron, 2 muon, 3 charged hadron)"""
+        a, b = C.c_double(), C.c_double()
+        row = lib().pdo_track_resolution(self._h, int(species), float(px), float(py), float(pz), C.byref(a), C.byref(b))
+        return int(row), a.value, b.value
 
     def propagate(self, q, px, py, pz, vx=0.0, vy=0.0, vz=0.0):
         out = [C.c_double() for _ in range(6)]

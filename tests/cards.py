@@ -3,7 +3,8 @@
 Format ("key = values", '#' comments): name, bz, radius, half_length, kappa, grid (eta|theta),
 edges (may repeat), nphi (may repeat), eff (pt_lo pt_hi aeta_lo aeta_hi eps; one line per row),
 abs_costheta_max, track_res (a b), ecal_res (C S N), hcal_res (C S N), ecal_thr, hcal_thr;
-ecal_res_eta / hcal_res_eta (aeta_lo aeta_hi C S N; one line per row), ecal_nsigma, hcal_nsigma, smear_tower_center.
+ecal_res_eta / hcal_res_eta (aeta_lo aeta_hi C S N; one line per row), ecal_nsigma, hcal_nsigma, smear_tower_center,
+track_res_eta (aeta_lo aeta_hi a b [species]; one line per row: DESIGN.md section 17, reading K4).
 Per-species cards: an eff row may carry a sixth number and a track_res line a third one,
 the species it applies to (1 electrons, 2 muons, 3 charged hadrons; 0 or absent: every charged particle).
 """
@@ -21,7 +22,7 @@ DEFAULT_EFF = [(1.0, "inf", 0.0, 1.5, 0.97), (1.0, "inf", 1.5, 2.5, 0.85), (0.1,
 def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kappa=0.299792458,
               eff=DEFAULT_EFF, abs_costheta_max=None, track_res=(0.01, 1.5e-4), ecal=(0.007, 0.07, 0.35),
               hcal=(0.05, 1.5, 0.0), ecal_thr=0.5, hcal_thr=1.0, name="custom", track_res_species=None,
-              ecal_res_eta=(), hcal_res_eta=(), ecal_nsigma=None, hcal_nsigma=None, smear_tower_center=None):
+              ecal_res_eta=(), hcal_res_eta=(), ecal_nsigma=None, hcal_nsigma=None, smear_tower_center=None, track_res_eta=()):
     lines = ["name = %s" % name, "bz = %r" % bz, "radius = %r" % radius, "half_length = %r" % half_length,
              "kappa = %r" % kappa, "grid = %s" % grid]
     edges = [float(x) for x in edges]
@@ -37,6 +38,8 @@ def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kap
     lines.append("track_res = %r %r" % tuple(track_res))
     for sp, ab in sorted((track_res_species or {}).items()):
         lines.append("track_res = %r %r %d" % (ab[0], ab[1], sp))
+    for row in track_res_eta:  # (aeta_lo, aeta_hi, a, b[, species]): reading K4
+        lines.append("track_res_eta = " + " ".join(repr(float(x)) for x in row[:4]) + (" %d" % row[4] if len(row) > 4 else ""))
     lines.append("ecal_res = %r %r %r" % tuple(ecal))
     lines.append("hcal_res = %r %r %r" % tuple(hcal))
     for row in ecal_res_eta:  # (aeta_lo, aeta_hi, C, S, N): DESIGN.md section 17, reading K1

@@ -141,3 +141,61 @@ def test_tower_positions_uniform_inside_the_cell(name, tmp_path):
     e0, t0 = int(tow_ev[5]), int(o["tow_tower"][5])
     assert pdo.tower_position(card, 21, e0, t0) == (float(o["tow_eta"][5]), float(o["tow_phi"][5]))
     assert pdo.tower_position(b, 21, e0, t0) == b.tower_centre(t0)
+
+
+def _tracks(pid, q, etas, pt=20.0, n_events=1, mass=0.13957039):
+    """n_events identical events of charged particles from the origin, one per eta, spread in phi"""
+    return wl.from_lists([[P(pid, q, pt, eta, 0.1 + 0.3 * k, mass) for k, eta in enumerate(etas)] for _ in range(n_events)])
+
+
+def test_track_resolution_rows_by_eta_and_species(tmp_path):
+    """Reading K4: eta-dependent track resolution rows (first match in file order, optional species, half-open |eta| range of the
+    TRUE momentum), falling back to the species' / the card's track_res line (J2)."""
+    b = pdo.Card("cms_like")
+    eff = [(0.1, "inf", 0.0, 2.5, 1.0)]
+    # rows that repeat the common line change nothing, bit for bit
+    same = cards.variant(tmp_path / "same.card", b.edges, b.nphi, track_res_eta=[(0.0, 1.0, 0.01, 1.5e-4), (1.0, 9.0, 0.01, 1.5e-4, 3)])
+    ev = wl.generate(0, 60)
+    ref, got = pdo.simulate(b, ev, 3), pdo.simulate(pdo.Card(same), ev, 3)
+    for k in ref:
+        assert got[k].tobytes() == ref[k].tobytes(), k
+    # the selection function: first match wins, species rows apply to their species only, the range is [lo, hi)
+    rows = [(0.5, 1.5, 0.0, 0.0), (1.0, 2.0, 0.07, 0.0, 2), (0.0, 9.0, 0.03, 2e-4, 1)]
+    path = cards.variant(tmp_path / "rows.card", b.edges, b.nphi, eff=eff, track_res=(0.02, 1e-4), track_res_eta=rows)
+    c = pdo.Card(path)
+    f32 = lambda x: float(np.float32(x))  # noqa: E731
+    mom = lambda eta, pt=10.0: (pt, 0.0, pt * math.sinh(eta))  # noqa: E731
+    assert c.track_resolution(3, *mom(0.7)) == (0, 0.0, 0.0)                     # hadron inside row 0
+    assert c.track_resolution(3, *mom(-1.2)) == (0, 0.0, 0.0)                    # |eta|: both signs
+    assert c.track_resolution(2, *mom(1.2)) == (0, 0.0, 0.0)                     # row 0 precedes the muon row
+    assert c.track_resolution(2, *mom(1.7)) == (1, f32(0.07), 0.0)               # muon row
+    assert c.track_resolution(3, *mom(1.7)) == (-1, f32(0.02), f32(1e-4))        # no row for a hadron there: the common line
+    assert c.track_resolution(1, *mom(1.7)) == (2, f32(0.03), f32(2e-4))         # electron row (any eta)
+    assert c.track_resolution(1, *mom(0.7))[0] == 0                              # ... but row 0 comes first
+    lo, hi = f32(0.5), f32(1.5)
+    assert c.track_resolution(3, *mom(lo * (1 + 1e-9)))[0] == 0 and c.track_resolution(3, *mom(lo * (1 - 1e-9)))[0] == -1
+    assert c.track_resolution(3, *mom(hi * (1 - 1e-9)))[0] == 0 and c.track_resolution(3, *mom(hi * (1 + 1e-9)))[0] == -1
+    # through the chain: tracks in the zero-resolution row come out with pT' = pT exactly, the others are smeared
+    etas = [0.2, 0.45, 0.55, 1.0, 1.45, 1.55, -0.8, -2.0]
+    ev = _tracks(211, 1, etas)
+    o = pdo.simulate(c, ev, 5)
+    assert list(o["trk_src"]) == list(range(len(etas)))
+    pt_true = np.hypot(ev.px.astype(np.float64), ev.py.astype(np.float64))
+    for k, eta in enumerate(etas):
+        assert (float(o["trk_pt"][k]) == pt_true[k]) == (0.5 <= abs(eta) < 1.5), eta
+
+
+def test_track_resolution_rows_give_the_rows_width(tmp_path):
+    """Sample std of pT'/pT over many events = the row's sigma_rel (a for b = 0; b pT for a = 0), row by row and by species."""
+    b = pdo.Card("cms_like")
+    rows = [(0.0, 1.0, 0.05, 0.0), (1.0, 2.0, 0.0, 1e-3), (2.0, 9.0, 0.12, 0.0, 2)]
+    path = cards.variant(tmp_path / "w.card", b.edges, b.nphi, eff=[(0.1, "inf", 0.0, 2.5, 1.0)], track_res=(0.01, 0.0), track_res_eta=rows)
+    n_ev, pt = 4000, 30.0
+    for pid, mass, want in ((211, 0.13957039, (0.05, 1e-3 * pt, 0.01)), (13, 0.1056584, (0.05, 1e-3 * pt, 0.12))):
+        ev = _tracks(pid, 1, (0.4, 1.5, 2.3), pt=pt, n_events=n_ev, mass=mass)
+        o = pdo.simulate(pdo.Card(path), ev, 17)
+        assert o["trk_src"].shape[0] == 3 * n_ev
+        ratio = (o["trk_pt"] / np.hypot(ev.px.astype(np.float64), ev.py.astype(np.float64))[o["trk_src"]]).reshape(n_ev, 3)
+        for k in range(3):
+            assert abs(ratio[:, k].mean() - 1.0) < 4.0 * want[k] / math.sqrt(n_ev)
+            assert abs(ratio[:, k].std() - want[k]) < 4.0 * want[k] / math.sqrt(2.0 * n_ev), (pid, k, ratio[:, k].std(), want[k])
