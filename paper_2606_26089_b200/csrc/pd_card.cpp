@@ -37,6 +37,7 @@ struct RawCard {
   std::vector<std::array<double, 5>> ecal_eta, hcal_eta;  // reading K1: aeta_lo, aeta_hi, C, S, N
   double nsig_ecal = 0, nsig_hcal = 0;                    // reading K2
   bool smear_center = false;                              // reading K3
+  std::vector<std::array<double, 5>> trk_eta;             // reading K4: aeta_lo, aeta_hi, a, b, species
 };
 
 constexpr double kPi = 3.14159265358979323846;
@@ -139,6 +140,9 @@ bool from_file(RawCard &r, const char *path) {
     else if (key == "hcal_res" && v.size() == 3) std::copy(v.begin(), v.end(), r.hcal);
     else if (key == "ecal_res_eta" && v.size() == 5 && r.ecal_eta.size() < 8) r.ecal_eta.push_back({{v[0], v[1], v[2], v[3], v[4]}});
     else if (key == "hcal_res_eta" && v.size() == 5 && r.hcal_eta.size() < 8) r.hcal_eta.push_back({{v[0], v[1], v[2], v[3], v[4]}});
+    else if (key == "track_res_eta" && (v.size() == 4 || (v.size() == 5 && (v[4] == 0.0 || v[4] == 1.0 || v[4] == 2.0 || v[4] == 3.0))) &&
+             r.trk_eta.size() < size_t(PD_MAX_TRK_ROWS))
+      r.trk_eta.push_back({{v[0], v[1], v[2], v[3], v.size() == 5 ? v[4] : 0.0}});
     else if (key == "ecal_nsigma" && v.size() == 1) r.nsig_ecal = v[0];
     else if (key == "hcal_nsigma" && v.size() == 1) r.nsig_hcal = v[0];
     else if (key == "smear_tower_center" && v.size() == 1) r.smear_center = v[0] != 0.0;
@@ -194,6 +198,8 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
       if (!fin(e)) return PD_ECARD;
     if (r.theta && !(r.edges.front() >= 0.0 && r.edges.back() <= kPi)) return PD_ECARD;
     if (!nonneg(r.nsig_ecal) || !nonneg(r.nsig_hcal)) return PD_ECARD;
+    for (const auto &row : r.trk_eta)  // aeta_hi may be "inf"
+      if (!(nonneg(row[0]) && row[1] > row[0] && nonneg(row[2]) && nonneg(row[3]))) return PD_ECARD;
     for (const auto *rows : {&r.ecal_eta, &r.hcal_eta})
       for (const auto &row : *rows)
         if (!(nonneg(row[0]) && row[1] > row[0] && nonneg(row[2]) && nonneg(row[3]) && nonneg(row[4]))) return PD_ECARD;
@@ -354,6 +360,17 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
   s.nsig2_ecal = float(f32(r.nsig_ecal) * f32(r.nsig_ecal));
   s.nsig2_hcal = float(f32(r.nsig_hcal) * f32(r.nsig_hcal));
   s.smear_center = r.smear_center ? 1 : 0;
+  // reading K4: the rows' edges as sinh of the fp32-rounded |eta| (fp64, the form the kernel compares |pz| / pT with)
+  s.n_trk_rows = int(r.trk_eta.size());
+  for (int k = 0; k < PD_MAX_TRK_ROWS; ++k) {
+    const bool on = k < s.n_trk_rows;
+    s.trk_row_sp[k] = on ? int(r.trk_eta[k][4]) : 0;
+    s.trk_row_lo_d[k] = on ? std::sinh(f32(r.trk_eta[k][0])) : 0.0;
+    s.trk_row_hi_d[k] = on ? std::sinh(f32(r.trk_eta[k][1])) : 0.0;
+    const double a = on ? f32(r.trk_eta[k][2]) : 0.0;
+    s.trk_row_a2[k] = float(a * a);
+    s.trk_row_b[k] = on ? float(r.trk_eta[k][3]) : 0.f;
+  }
   s.tb_first = c->tb[0], s.tb_last = c->tb[nb];
 
   // ---- eta-bin lookup: cells of |u| by float bits (2^(23 - PD_LUT_SHIFT) cells per octave, |u| < 2^MIN_EXP in

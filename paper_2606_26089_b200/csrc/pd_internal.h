@@ -19,6 +19,7 @@ constexpr int PD_LUT_SHIFT = 19;       // eta-bin lookup: 16 cells per octave of
 constexpr int PD_LUT_MIN_EXP = -8;     // |u| < 2^-8 shares one cell per side
 
 // Scalars of a card as the kernels want them (all derived in double at load, stored as fp32).
+constexpr int PD_MAX_TRK_ROWS = 8;
 struct PdCardScalars {
   float R, L, R2, inv_R;  // calorimeter radius, half length, R^2, 1/R
   float kB, inv_kB;       // kappa * |B|  [GeV / m] and its inverse
@@ -48,6 +49,12 @@ struct PdCardScalars {
   int res_per_bin;                // K1: the card has eta-dependent resolution rows: C^2, S^2, N^2 per eta bin (PdCardTables::res2)
   float nsig2_ecal, nsig2_hcal;   // K2: n_sigma^2 of the significance cut (0: none)
   int smear_center;               // K3: reported tower position uniform inside the cell (Philox stream 4)
+  // K4: eta-dependent track resolution rows (first match in file order; species 0 = any, 1 e, 2 mu, 3 charged hadron);
+  // a row holds sinh(aeta_lo) pT <= |pz| < sinh(aeta_hi) pT, decided in fp64 exactly as the definition does
+  int n_trk_rows;
+  int trk_row_sp[PD_MAX_TRK_ROWS];
+  double trk_row_lo_d[PD_MAX_TRK_ROWS], trk_row_hi_d[PD_MAX_TRK_ROWS];
+  float trk_row_a2[PD_MAX_TRK_ROWS], trk_row_b[PD_MAX_TRK_ROWS];
 };
 
 // Per-bin tables, contiguous in one device allocation.

@@ -455,14 +455,33 @@ struct TrackOut {
   float pt_s, eta_mom, phi0, E_trk;
 };
 
+// reading K4: the first track-resolution row (species 0 = any, else 1 + the species index used here) that holds the true
+// momentum: sinh(lo) pT <= |pz| < sinh(hi) pT, in fp64 with every operation rounded once, as the fp64 definition takes it,
+// so that the row -- an integer decision -- is the same on both sides bit for bit.  Off the fast path: cards without rows
+// never get here.
+static __device__ __noinline__ void track_res_row(const PdCardScalars &sc, float px, float py, float pz, int species, float &a2, float &b) {
+  const double pxd = px, pyd = py;
+  const double pt = __dsqrt_rn(__dadd_rn(__dmul_rn(pxd, pxd), __dmul_rn(pyd, pyd)));
+  const double apz = fabs((double)pz);
+  for (int r = 0; r < sc.n_trk_rows; ++r) {
+    const int sp = sc.trk_row_sp[r];
+    if ((sp == 0 || sp == species + 1) && apz >= __dmul_rn(sc.trk_row_lo_d[r], pt) && apz < __dmul_rn(sc.trk_row_hi_d[r], pt)) {
+      a2 = sc.trk_row_a2[r], b = sc.trk_row_b[r];
+      return;
+    }
+  }
+}
+
 // r1, r2: words 1 and 2 of the particle's Philox block (stream 0)
 __device__ __forceinline__ void track_smear_words(const PdCardScalars &sc, float px, float py, float pz, uint32_t r1, uint32_t r2,
                                                   int species, TrackOut &t) {
   const float pt2 = fmaf(px, px, py * py);
   const float ipt = fast_rsqrt(pt2);
   const float pt = pt2 * ipt;
-  const float bp = sc.trk_b[species] * pt;
-  const float rel2 = fmaf(bp, bp, sc.trk_a2[species]);
+  float a2 = sc.trk_a2[species], b = sc.trk_b[species];
+  if (sc.n_trk_rows > 0) track_res_row(sc, px, py, pz, species, a2, b);  // reading K4 (cards with eta-dependent rows only)
+  const float bp = b * pt;
+  const float rel2 = fmaf(bp, bp, a2);
   t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(r1, r2)) : pt;
   t.E_trk = t.pt_s * (fast_sqrt(fmaf(pz, pz, pt2)) * ipt);
   t.eta_mom = fast_asinh(pz * ipt);

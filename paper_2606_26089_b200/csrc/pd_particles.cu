@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
           if (accepted) {
             // S3 on the spot; the record is parked in the particle's own staging slots until its place is known
             TrackOut t;
-            track_smear_words(sc, px, py, pz, rn[1], rn[2], sc.trk_per_species ? species_of(pid) : 2, t);
+            track_smear_words(sc, px, py, pz, rn[1], rn[2], (sc.trk_per_species || sc.n_trk_rows > 0) ? species_of(pid) : 2, t);
             pt_s = t.pt_s;
             s_px[i] = t.pt_s, s_py[i] = t.eta_mom, s_pz[i] = t.phi0, s_vx[i] = t.E_trk;
             s_vy[i] = eta_from_u(sc, u), s_vz[i] = phi_pos;

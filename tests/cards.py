@@ -39,7 +39,7 @@ def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kap
     for sp, ab in sorted((track_res_species or {}).items()):
         lines.append("track_res = %r %r %d" % (ab[0], ab[1], sp))
     for row in track_res_eta:  # (aeta_lo, aeta_hi, a, b[, species]): reading K4
-        lines.append("track_res_eta = " + " ".join(repr(float(x)) for x in row[:4]) + (" %d" % row[4] if len(row) > 4 else ""))
+        lines.append("track_res_eta = " + " ".join("inf" if x == "inf" else repr(float(x)) for x in row[:4]) + (" %d" % row[4] if len(row) > 4 else ""))
     lines.append("ecal_res = %r %r %r" % tuple(ecal))
     lines.append("hcal_res = %r %r %r" % tuple(hcal))
     for row in ecal_res_eta:  # (aeta_lo, aeta_hi, C, S, N): DESIGN.md section 17, reading K1

@@ -308,7 +308,7 @@ def test_forced_kernel_variants_in_a_subprocess(tmp_path):
 
 @pytest.mark.parametrize("base,cfg,ne", [("cms_like", 0, 600), ("cms_like", 1, 200), ("aleph_like", 4, 1500)])
 def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
-    """SURVEY 8f NEXT-3, readings K1-K3: eta-dependent ECAL / HCAL resolutions, the significance cut
+    """SURVEY 8f NEXT-3, readings K1-K4: eta-dependent ECAL / HCAL / track resolutions, the significance cut
     and tower positions smeared inside the cell -- one at a time and all together, on an eta grid and on a theta grid;
     and an event too large for the chip (the big-tile path has its own copy of the tower code)."""
     import cards
@@ -319,11 +319,15 @@ def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
     b = pdo.Card(base)
     ecal_rows = [(0.0, 0.8, 0.005, 0.05, 0.2), (0.8, 1.6, 0.01, 0.1, 0.3), (2.0, 3.0, 0.03, 0.2, 0.0)]
     hcal_rows = [(0.0, 1.3, 0.04, 1.0, 0.0), (1.3, 3.0, 0.06, 1.3, 0.5), (3.0, 9.0, 0.10, 2.0, 1.0)]
+    # K4: track resolution rows by |eta| of the momentum, the second for muons only, a gap between 1.4 and 1.7, an open end
+    trk_rows = [(0.0, 0.9, 0.015, 2e-4), (0.9, 1.4, 0.05, 0.0, 2), (0.9, 1.4, 0.02, 3e-4), (1.7, "inf", 0.04, 1e-3)]
     variants = {
         "eta_rows": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows),
         "significance": dict(ecal_nsigma=2.0, hcal_nsigma=1.5),
         "smeared_centres": dict(smear_tower_center=1),
-        "all": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows, ecal_nsigma=1.0, hcal_nsigma=1.2, smear_tower_center=1),
+        "track_rows": dict(track_res_eta=trk_rows),
+        "all": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows, ecal_nsigma=1.0, hcal_nsigma=1.2, smear_tower_center=1,
+                    track_res_eta=trk_rows),
     }
     ev = wl.generate(cfg, ne)
     if cfg == 0:
@@ -337,7 +341,7 @@ def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
         gpu = run_gpu(path, ev, 29)
         assert gpu["status_word"] == 0, name
         rep = _check(compare(path, ev, 29, gpu))
-        changed = any(gpu[k].shape != plain[k].shape or gpu[k].tobytes() != plain[k].tobytes() for k in ("tow_E", "tow_eta", "efl_E"))
+        changed = any(gpu[k].shape != plain[k].shape or gpu[k].tobytes() != plain[k].tobytes() for k in ("tow_E", "tow_eta", "efl_E", "trk_pt"))
         assert changed, name  # the card option really is in use
         print(base, name, {k: rep[k] for k in ("flagged_particles", "overridden_particles", "flagged_towers", "overridden_towers", "neutral_outside_plain_tol")})
 
