@@ -8,10 +8,10 @@
 // (cp.async.bulk, one elected thread, completion on an mbarrier), the particles are split by CLASS into index
 // lists -- A: charged inside the tracker acceptance (efficiency > 0: helix + Philox + accept + smear), B: other
 // charged (helix only), N: neutral (straight line) -- and the lists are processed by full warps gathering from
-// shared memory.  An accepted track is smeared on the spot (its Philox block is in registers) and its record
-// parked in the particle's own staging slots; at the end of the tile every warp compacts the tracks of the
-// PD_PSEG particles it owns, in particle order, and PARKS them in the workspace at the start of its segment, with
-// the segment's accepted bits beside them.  Nothing here depends on another tile: no chain, no waiting.  Kernel T,
+// shared memory.  An accepted track is smeared on the spot (its Philox block is in registers) and its record PARKED at
+// once in the workspace, compacted at the start of the warp's segment of PD_PSEG particles in particle order (the rank
+// of a track among its segment's tracks is a running count over the rows of list A), with the segment's accepted bits
+// beside them.  Nothing here depends on another tile: no chain, no waiting.  Kernel T,
 // which works event by event and knows where an event's tracks go, moves them into the Track collection.
 //
 // What the tower pass (pd_towers.cu) needs besides: a 16-bit key per particle (tower id | HCAL bit, 0xffff = no
@@ -263,22 +263,33 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     __syncwarp();
     const int n_work = nA + nB + nN;
 
-    // ---- S1-S4 on the warp's lists A | B | N: rows of one class (the rows at the two boundaries are mixed)
+    // ---- S1-S4 on the warp's lists A | B | N: rows of one class (the rows at the two boundaries are mixed).
+    // Accepted tracks are smeared on the spot and PARKED at once in the workspace: list A is in particle order and only
+    // its entries can be accepted, so the rank of a track among the tracks of the segment -- its place in the parking
+    // arrays -- is the number of tracks accepted so far (a ballot per row and a running count).  Kernel T, which knows
+    // where an event's tracks go, moves them into the Track collection.
+    const long long seg0 = (s0 - p_al) + wbase;  // first slot of the warp's segment in the parking arrays
+    int run = 0;                                 // tracks of the segment so far
 #pragma unroll 1
     for (int k = 0; k < PT_ITERS; ++k) {
       const int v = 32 * k + lane;
+      bool accepted = false;
+      int i = 0, pid = 0;
+      float px = 0.f, py = 0.f, pz = 0.f, u = 0.f, phi_pos = 0.f;
+      uint32_t r1 = 0u, r2 = 0u;
       if (v < n_work) {
         const int cls = v < nA ? 0 : (v < nA + nB ? 1 : 2);
         const unsigned ent = s_list[wbase + v];
-        const int i = (int)(ent & 0x7ffu);
-        const float px = s_px[i], py = s_py[i], pz = s_pz[i], vx = s_vx[i], vy = s_vy[i], vz = s_vz[i];
-        const int pid = s_pid[i];
+        i = (int)(ent & 0x7ffu);
+        px = s_px[i], py = s_py[i], pz = s_pz[i];
+        const float vx = s_vx[i], vy = s_vy[i], vz = s_vz[i];
+        pid = s_pid[i];
         float x, y, z;
         uint32_t status;
         if (cls == 2 || sc.sB == 0.f) status = line_hit(sc, px, py, pz, vx, vy, vz, x, y, z);
         else status = helix_hit(sc, (int)s_q[i], px, py, pz, vx, vy, vz, x, y, z);
         const bool live = (status & PD_FACE_MASK) != PD_DROPPED;
-        float u = __int_as_float(0x7fc00000), phi_pos = u;
+        u = __int_as_float(0x7fc00000), phi_pos = u;
         int tower = -1;
         if (live) {
           hit_coords(sc, status, x, y, z, u, phi_pos);
@@ -287,8 +298,6 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
         const int apid = pid < 0 ? -pid : pid;
         const bool to_ecal = apid == 11 || apid == 22;  // reading A18
         const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
-        bool accepted = false;
-        float pt_s = 0.f;
         if (cls == 0 && live) {
           // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0.
           // The event: the last one whose offset is <= i (bisection of the tile's offsets; one step on big events)
@@ -315,15 +324,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
           uint32_t rn[4];
           rng_block(prm.rk, prm.event_base + ev, pidx, 0u, rn);
           accepted = uniform24(rn[0]) < sc.row_eps[ent >> 11];
-          if (accepted) {
-            // S3 on the spot; the record is parked in the particle's own staging slots until its place is known
-            TrackOut t;
-            track_smear_words(sc, px, py, pz, rn[1], rn[2], (sc.trk_per_species || sc.n_trk_rows > 0) ? species_of(pid) : 2, t);
-            pt_s = t.pt_s;
-            s_px[i] = t.pt_s, s_py[i] = t.eta_mom, s_pz[i] = t.phi0, s_vx[i] = t.E_trk;
-            s_vy[i] = eta_from_u(sc, u), s_vz[i] = phi_pos;
-            atomicOr(&s_accmask[i >> 5], 1u << (i & 31));
-          }
+          r1 = rn[1], r2 = rn[2];
         }
         // what the tower pass needs: tower | HCAL bit, or "no deposit"
         s_key[i] = (tower >= 0 && !to_none) ? (unsigned short)((unsigned)tower | (to_ecal ? 0u : 0x8000u)) : (unsigned short)PT_NONE;
@@ -336,35 +337,28 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
           if (prm.dbg_tower) prm.dbg_tower[g] = tower;
           if (prm.dbg_accepted) prm.dbg_accepted[g] = accepted ? 1 : 0;
           if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)((cls == 2 || !live || row == 31) ? -1 : row);
-          if (prm.dbg_pt_smeared) prm.dbg_pt_smeared[g] = pt_s;
+          if (prm.dbg_pt_smeared && !accepted) prm.dbg_pt_smeared[g] = 0.f;
         }
       }
-    }
-    // ---- the warp's accepted tracks in particle order (its own mask words: nobody else sets their bits), parked
-    // SEGMENT by segment in the workspace: the tracks of the PT_PER_WARP particles this warp owns, compacted, at the
-    // segment's start.  Kernel T, which knows where an event's tracks go, moves them into the Track collection.
-    __syncwarp();
-    {
-      const long long seg0 = (s0 - p_al) + wbase;  // first slot of the segment in the parking arrays
-      int run = 0;
-#pragma unroll
-      for (int k = 0; k < PT_ITERS; ++k) {
-        const uint32_t m = s_accmask[wword + k];
-        if ((m >> lane) & 1u) s_list[wbase + run + __popc(m & lt_mask)] = (unsigned short)(wbase + 32 * k + lane);
-        run += __popc(m);
-      }
-      if (lane < PT_ITERS) prm.accmask[(seg0 >> 5) + lane] = s_accmask[wword + lane];
-      __syncwarp();
-      for (int r = lane; r < run; r += 32) {
-        const int i = s_list[wbase + r];
-        const long long g = seg0 + r;
+      const unsigned m_acc = __ballot_sync(0xffffffffu, accepted);
+      if (accepted) {
+        // S3 on the spot (the Philox words are in registers); the record goes straight to its parking slot
+        TrackOut t;
+        track_smear_words(sc, px, py, pz, r1, r2, (sc.trk_per_species || sc.n_trk_rows > 0) ? species_of(pid) : 2, t);
+        const long long g = seg0 + run + __popc(m_acc & lt_mask);
         prm.park_idx[g] = (unsigned char)(i - wbase);
-        prm.park_pid[g] = s_pid[i];
+        prm.park_pid[g] = pid;
         prm.park_q[g] = s_q[i];
-        prm.park_f[0][g] = s_px[i], prm.park_f[1][g] = s_py[i], prm.park_f[2][g] = s_pz[i];
-        prm.park_f[3][g] = s_vx[i], prm.park_f[4][g] = s_vy[i], prm.park_f[5][g] = s_vz[i];
+        prm.park_f[0][g] = t.pt_s, prm.park_f[1][g] = t.eta_mom, prm.park_f[2][g] = t.phi0;
+        prm.park_f[3][g] = t.E_trk, prm.park_f[4][g] = eta_from_u(sc, u), prm.park_f[5][g] = phi_pos;
+        atomicOr(&s_accmask[i >> 5], 1u << (i & 31));
+        if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[s0 + i] = t.pt_s;
       }
+      run += __popc(m_acc);
     }
+    // the segment's accepted bits (the warp's own mask words: nobody else sets their bits) go beside the parked tracks
+    __syncwarp();
+    if (lane < PT_ITERS) prm.accmask[(seg0 >> 5) + lane] = s_accmask[wword + lane];
     // the warp's keys (what the tower pass needs): PT_PER_WARP 16-bit words, stored as 32-bit ones
     {
       const uint32_t *src = (const uint32_t *)(s_key + wbase);
@@ -372,7 +366,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
       for (int j = lane; j < PT_PER_WARP / 2; j += 32) dst[j] = src[j];
     }
     if (tid == 0) s_cnt[2] = (int)atomicAdd(prm.ptile_counter, 1u);  // the CTA's next tile
-    fence_async_smem();  // the parked records were generic-proxy writes to slots the next tile's bulk copies overwrite
+    fence_async_smem();  // the keys and lists were generic-proxy writes; the next tile's bulk copies overwrite the staging slots
   }
 }
 
