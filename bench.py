@@ -338,6 +338,19 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     imp_ms = f0.elapsed_time(f1) / f_steps
     del imp
+    # the same values from the chain itself (pd_options.impact: kernel P computes them while the particle is on chip): what the
+    # step costs with the option on; its difference to ms_per_step replaces the stand-alone kernel's time
+    out_f = pd.DeviceOutputs(card, ne, n, debug=False, impact=ip_res)
+    for _ in range(3):
+        pd.simulate(card, dev, out_f, seed, event_base)
+    barrier()
+    f0.record(stream)
+    for _ in range(f_steps):
+        pd.simulate(card, dev, out_f, seed, event_base)
+    f1.record(stream)
+    barrier()
+    step_imp_ms = f0.elapsed_time(f1) / f_steps
+    del out_f
     # ---- H_T and E_T^miss of the truth collection (the step's input)
     tfeat = pd.DeviceFeatures(ne, 1)
     tws = pd.truth_features(dev, tfeat)
@@ -436,7 +449,8 @@ def run_ours(args, rank, world, local_rank):
                  "track_impact": {"ms": imp_ms, "tracks_per_s": totals[0] / (imp_ms * 1e-3), "kernel": "pd_impact_kernel",
                                   "algorithmic_bytes": 45 * totals[0] + 16 * (ne + 1),
                                   "hbm_frac": (45 * totals[0] + 16 * (ne + 1)) / (imp_ms * 1e-3) / 1e9 / peak,
-                                  "note": "d0, z0 and errors (a (+) b/pT) for the step's tracks; truth particles gathered through trk.src; 1 launch; rank 0, not in value"},
+                                  "step_ms_with_impact_option": step_imp_ms, "extra_ms_in_chain": step_imp_ms - total_ms / args.steps,
+                                  "note": "d0, z0 and errors (a (+) b/pT) for the step's tracks; stand-alone kernel: truth particles gathered through trk.src, 1 launch; or from the chain itself (pd_options.impact): the whole step then takes step_ms_with_impact_option; rank 0, not in value"},
                  "particle_filter": {"ms": filt_ms, "objects_per_s": totals[2] / (filt_ms * 1e-3), "kept": kept, "kernel": "pd_filter_kernel",
                                      "algorithmic_bytes": 21 * totals[2] + 21 * kept + 16 * (ne + 1),
                                      "hbm_frac": (21 * totals[2] + 21 * kept + 16 * (ne + 1)) / (filt_ms * 1e-3) / 1e9 / peak,

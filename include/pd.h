@@ -267,12 +267,12 @@ int pd_pileup_merge(const pd_events *hs, const pd_events *pool, const pd_pileup_
  *     (same key and event numbering as pd_simulate, so splitting a batch does not change a value).
  * One value per track of `tracks` (the collection a pd_simulate call wrote for `events` on the same stream or
  * after synchronisation): only tracks->offsets and tracks->src are read.  a = b = 0 gives the true values. */
-typedef struct {
+typedef struct pd_impact_config_s {
   float d0_a, d0_b; /* metres, metres GeV; >= 0 */
   float z0_a, z0_b;
 } pd_impact_config;
 
-typedef struct {
+typedef struct pd_impact_s {
   float *d0, *z0, *d0_err, *z0_err; /* DEVICE arrays of at least tracks->capacity (>= n_particles) elements */
 } pd_impact;
 
@@ -328,6 +328,14 @@ int pd_last_launch_count(void);
 typedef struct pd_options {
   int32_t tile_events;
   int32_t reserved[7]; /* must be 0 */
+  /* impact parameters of the tracks from the chain itself (see pd_track_impact below for the definition): both NULL = off;
+   * both set = kernel P computes d0, z0 and their errors for every track it accepts (the particle is on chip there) and
+   * kernel T writes them beside the Track collection, element k for track k: the same values as a pd_track_impact call
+   * with this config, seed and event_base after the step, bit for bit, without its gather over the particle arrays.
+   * impact->d0, z0, d0_err, z0_err: DEVICE arrays of at least tracks->capacity elements.  The workspace grows by 16 bytes
+   * per particle slot (pd_workspace_bytes_ex with the same options). */
+  const struct pd_impact_config_s *impact_config;
+  struct pd_impact_s *impact;
 } pd_options;
 int64_t pd_workspace_bytes_ex(const pd_card *card, int64_t n_events, int64_t n_particles, const pd_options *options);
 int pd_simulate_ex(const pd_card *card, const pd_events *events, uint64_t seed, int64_t event_base,

@@ -24,11 +24,6 @@ _p = C.c_void_p
 _lib = None
 
 
-class Options(C.Structure):
-    """pd_options"""
-    _fields_ = [("tile_events", C.c_int32), ("reserved", C.c_int32 * 7)]
-
-
 class CardInfo(C.Structure):
     _fields_ = [("n_towers", C.c_int32), ("n_eta_bins", C.c_int32), ("grid_coord", C.c_int32), ("bz", C.c_float),
                 ("radius", C.c_float), ("half_length", C.c_float), ("n_eff_rows", C.c_int32)]
@@ -53,6 +48,12 @@ class ImpactConfig(C.Structure):
 
 class Impact(C.Structure):
     _fields_ = [(k, _p) for k in ("d0", "z0", "d0_err", "z0_err")]
+
+
+class Options(C.Structure):
+    """pd_options"""
+    _fields_ = [("tile_events", C.c_int32), ("reserved", C.c_int32 * 7), ("impact_config", C.POINTER(ImpactConfig)),
+                ("impact", C.POINTER(Impact))]
 
 
 class PileupConfig(C.Structure):
@@ -183,9 +184,13 @@ class Card:
             self._h = None
 
 
-def workspace_bytes(card: Card, n_events: int, n_particles: int, tile_events: int = 0) -> int:
-    """pd_workspace_bytes_ex; tile_events: pd_options.tile_events (0 = automatic; a tuning knob)."""
+def workspace_bytes(card: Card, n_events: int, n_particles: int, tile_events: int = 0, impact: bool = False) -> int:
+    """pd_workspace_bytes_ex; tile_events: pd_options.tile_events (0 = automatic; a tuning knob); impact: with room for the
+    impact parameters computed by the chain (pd_options.impact)."""
     opt = Options(int(tile_events))
+    if impact:
+        cfg, dummy = ImpactConfig(0.0, 0.0, 0.0, 0.0), Impact(*[C.c_void_p(16)] * 4)  # only their presence matters for the size
+        opt.impact_config, opt.impact = C.pointer(cfg), C.pointer(dummy)
     n = lib().pd_workspace_bytes_ex(card._h, int(n_events), int(n_particles), C.byref(opt))
     if n < 0:
         raise PdError(n)
@@ -231,9 +236,13 @@ class DeviceEvents:
 class DeviceOutputs:
     """Output buffers (torch tensors) sized to the sufficient bounds of pd.h, plus the workspace."""
 
-    def __init__(self, card: Card, n_events: int, n_particles: int, debug: bool = False, device="cuda", tile_events: int = 0):
+    def __init__(self, card: Card, n_events: int, n_particles: int, debug: bool = False, device="cuda", tile_events: int = 0, impact=None):
+        """impact: None, or (d0_res, z0_res) = ((a, b), (a, b)): the chain itself writes d0, z0 and their errors of every track
+        to self.impact (a DeviceImpact), pd_options.impact"""
         torch = _torch()
         self.tile_events = int(tile_events)  # pd_options.tile_events for the calls that use these buffers (sizes the workspace)
+        self.impact_res = impact
+        self.impact = None
         n = max(int(n_particles), 1)
         self.n_events, self.n_particles = int(n_events), int(n_particles)
         mk = lambda m, dt: torch.empty(m, dtype=getattr(torch, dt), device=device)  # noqa: E731
@@ -241,7 +250,9 @@ class DeviceOutputs:
         self.tow = {"offsets": mk(n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TOWER_FIELDS}}
         self.efl = {"offsets": mk(n_events + 1, "int64"), **{k: mk(2 * n, dt) for k, dt in EFLOW_FIELDS}}
         self.dbg = {k: mk(n, dt) for k, dt in DEBUG_FIELDS} if debug else None
-        self.ws_bytes = workspace_bytes(card, n_events, n_particles, self.tile_events)
+        self.ws_bytes = workspace_bytes(card, n_events, n_particles, self.tile_events, impact is not None)
+        if impact is not None:
+            self.impact = DeviceImpact(n, device=device)
         self.ws = torch.empty(self.ws_bytes + 16, dtype=torch.uint8, device=device)
         self.c_trk = Tracks(n, _tptr(self.trk["offsets"]), *[_tptr(self.trk[k]) for k, _ in TRACK_FIELDS])
         self.c_tow = Towers(n, _tptr(self.tow["offsets"]), *[_tptr(self.tow[k]) for k, _ in TOWER_FIELDS])
@@ -451,6 +462,10 @@ def simulate(card: Card, dev_events: DeviceEvents, out: DeviceOutputs, seed: int
         raise PdError(PD_ECUDA)
     st = torch.cuda.current_stream() if stream is None else stream
     opt = Options(int(getattr(out, "tile_events", 0)))
+    if getattr(out, "impact", None) is not None:
+        (d0a, d0b), (z0a, z0b) = out.impact_res
+        icfg = ImpactConfig(float(d0a), float(d0b), float(z0a), float(z0b))
+        opt.impact_config, opt.impact = C.pointer(icfg), C.pointer(out.impact.c)
     rc = lib().pd_simulate_ex(card._h, C.byref(dev_events.c), int(seed) & (2**64 - 1), int(event_base), C.byref(out.c_trk),
                               C.byref(out.c_tow), C.byref(out.c_efl), C.byref(out.c_dbg) if out.c_dbg is not None else None,
                               _tptr(out.ws), out.ws_bytes, C.byref(opt), C.c_void_p(st.cuda_stream))

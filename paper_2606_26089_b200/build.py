@@ -12,7 +12,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpd.so")
 SOURCES = ["pd_card.cpp", "pd_api.cu", "pd_particles.cu", "pd_towers.cu", "pd_features.cu", "pd_filter.cu", "pd_pileup.cu", "pd_impact.cu", "pd_truth.cu"]
-HEADERS = [os.path.join(CSRC, "pd_internal.h"), os.path.join(CSRC, "pd_math.cuh"), os.path.join(CSRC, "pd_scan.cuh"), os.path.join(ROOT, "include", "pd.h")]
+HEADERS = [os.path.join(CSRC, "pd_internal.h"), os.path.join(CSRC, "pd_math.cuh"), os.path.join(CSRC, "pd_scan.cuh"), os.path.join(CSRC, "pd_impact_math.cuh"), os.path.join(ROOT, "include", "pd.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -42,9 +42,9 @@ static size_t ws_chain_bytes(const PdLaunchPlan &plan) {
 // What kernel P leaves for kernel T, per particle slot (n_ptiles * PD_PTILE slots): the 16-bit key, the accepted bit,
 // and the parked track records (segment index 1 B, charge 1 B, pid 4 B, six floats).  Each array 256-byte aligned.
 struct WsLayout {
-  size_t tile_ev, key, accmask, idx, q, pid, f[6], big_acc, total;
+  size_t tile_ev, key, accmask, idx, q, pid, f[6], imp[4], big_acc, total;
 };
-static WsLayout ws_layout(const PdLaunchPlan &plan, int n_towers) {
+static WsLayout ws_layout(const PdLaunchPlan &plan, int n_towers, bool impact = false) {
   const size_t slots = (size_t)PD_PTILE * (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1);
   WsLayout l;
   size_t o = ws_chain_bytes(plan);
@@ -60,6 +60,7 @@ static WsLayout ws_layout(const PdLaunchPlan &plan, int n_towers) {
   l.q = take(slots);
   l.pid = take(4 * slots);
   for (int k = 0; k < 6; ++k) l.f[k] = take(4 * slots);
+  for (int k = 0; k < 4; ++k) l.imp[k] = take(impact ? 4 * slots : 0);  // pd_options.impact
   l.big_acc = take(8 * 5 * (size_t)n_towers * (size_t)plan.max_ctas);  // tiles that do not fit on chip (any event size)
   l.total = o;
   return l;
@@ -113,11 +114,20 @@ int pd_card_info(const pd_card *card, pd_card_info_t *out) {
 }
 
 static int tile_events_of(const pd_options *opt) { return opt ? opt->tile_events : 0; }
+static bool impact_of(const pd_options *opt) { return opt && opt->impact_config && opt->impact; }
 static bool options_ok(const pd_options *opt) {
   if (!opt) return true;
   if (opt->tile_events < 0) return false;
   for (int k = 0; k < 7; ++k)
     if (opt->reserved[k] != 0) return false;
+  if ((opt->impact_config != nullptr) != (opt->impact != nullptr)) return false;  // both or neither
+  if (opt->impact_config) {
+    const pd_impact_config *c = opt->impact_config;
+    for (float v : {c->d0_a, c->d0_b, c->z0_a, c->z0_b})
+      if (!(v >= 0.f) || !std::isfinite(v)) return false;
+    const pd_impact *o = opt->impact;
+    if (!o->d0 || !o->z0 || !o->d0_err || !o->z0_err) return false;
+  }
   return true;
 }
 
@@ -125,7 +135,7 @@ int64_t pd_workspace_bytes_ex(const pd_card *card, int64_t n_events, int64_t n_p
   if (!card || n_events < 0 || n_particles < 0 || !options_ok(opt)) return PD_EINVAL;
   PdLaunchPlan plan;
   pd_plan(card, n_events, n_particles, tile_events_of(opt), &plan);
-  return (int64_t)ws_layout(plan, card->sc.n_towers).total;
+  return (int64_t)ws_layout(plan, card->sc.n_towers, impact_of(opt)).total;
 }
 int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles) {
   return pd_workspace_bytes_ex(card, n_events, n_particles, nullptr);
@@ -485,7 +495,7 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
   p.chain = (unsigned long long *)(ws + kWsHeader);
   p.chain_t = p.chain + (plan.n_tiles > 0 ? plan.n_tiles : 1);
   {
-    const WsLayout wl = ws_layout(plan, card->sc.n_towers);
+    const WsLayout wl = ws_layout(plan, card->sc.n_towers, impact_of(opt));
     p.tile_ev = (int *)(ws + wl.tile_ev);
     p.key = (unsigned short *)(ws + wl.key);
     p.accmask = (unsigned int *)(ws + wl.accmask);
@@ -494,6 +504,13 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
     p.park_pid = (int *)(ws + wl.pid);
     p.big_acc = (long long *)(ws + wl.big_acc);
     for (int k = 0; k < 6; ++k) p.park_f[k] = (float *)(ws + wl.f[k]);
+    if (impact_of(opt)) {
+      p.imp_on = 1;
+      p.imp_d0_a = opt->impact_config->d0_a, p.imp_d0_b = opt->impact_config->d0_b;
+      p.imp_z0_a = opt->impact_config->z0_a, p.imp_z0_b = opt->impact_config->z0_b;
+      for (int k = 0; k < 4; ++k) p.park_imp[k] = (float *)(ws + wl.imp[k]);
+      p.imp_out[0] = opt->impact->d0, p.imp_out[1] = opt->impact->z0, p.imp_out[2] = opt->impact->d0_err, p.imp_out[3] = opt->impact->z0_err;
+    }
   }
   p.n_ptiles = plan.n_ptiles;
   p.p_base = particle_base;

@@ -18,20 +18,12 @@
 #include <cstdint>
 
 #include "pd_internal.h"
-#include "pd_math.cuh"
+#include "pd_impact_math.cuh"
 
 namespace pdi {
 
 constexpr int THREADS = 256, ITEMS = 4, TILE = THREADS * ITEMS;  // ITEMS = 4: the 16-byte vectors below
 constexpr int OFF_CACHE = 2048;  // staged track offsets per CTA (events touched by a tile, + 1)
-
-// a b - c d with one rounding of the result's leading part (Kahan): exact products via fma
-__device__ __forceinline__ float diff_of_products(float a, float b, float c, float d) {
-  const float cd = c * d;
-  const float err = fmaf(-c, d, cd);
-  const float dop = fmaf(a, b, -cd);
-  return dop + err;
-}
 
 // largest e in [lo, hi) with off[e] <= t (off non-decreasing, off[lo] <= t < off[hi])
 template <typename P>
@@ -120,37 +112,11 @@ __global__ void __launch_bounds__(THREADS, 4) pd_impact_kernel(const __grid_cons
       ob_[k] = i - (int)__ldg(prm.ev_off + e_[k]);
     }
     float o_d0[ITEMS], o_z0[ITEMS], o_sd[ITEMS], o_sz[ITEMS];
+    const pdk::ImpactCfg cfg{prm.inv_kB, prm.sB, prm.d0_a, prm.d0_b, prm.z0_a, prm.z0_b};
 #pragma unroll
-    for (int k = 0; k < ITEMS; ++k) {
-      const float px = px_[k], py = py_[k], pz = pz_[k], vx = vx_[k], vy = vy_[k], vz = vz_[k];
-      const int q = q_[k];
-      const float pt2 = fmaf(px, px, py * py);
-      const float ipt = pdk::fast_rsqrt(pt2), pt = pt2 * ipt;
-      const float u = -diff_of_products(vx, py, vy, px) * ipt;  // v . n^
-      const float w = diff_of_products(vx, px, -vy, py) * ipt;  // v . p^
-      const float tl = pz * ipt;
-      float d0, z0;
-      if (q == 0 || prm.sB == 0.f) {
-        d0 = -u, z0 = fmaf(-w, tl, vz);
-      } else {
-        const float rho = pt * prm.inv_kB * pdk::fast_rcp(fabsf((float)q));
-        const float s = (q > 0) == (prm.sB > 0.f) ? -1.f : 1.f;
-        const float cy = fmaf(s, rho, u);  // centre in the (p^, n^) frame: (w, u + s rho)
-        const float rc = pdk::fast_sqrt(fmaf(w, w, cy * cy));
-        const float r02 = fmaf(u, u, w * w);
-        d0 = -fmaf(2.f * rho, u, s * r02) * pdk::fast_rcp(rho + rc);
-        const float alpha = pdk::fast_atan2(-w, fmaf(s, u, rho));
-        z0 = fmaf(rho * alpha, tl, vz);
-      }
-      // resolution a (+) b / pT and the two normals of stream 3 (readings I2, I3)
-      const float bd = prm.d0_b * ipt, bz = prm.z0_b * ipt;
-      const float sd = pdk::fast_sqrt(fmaf(prm.d0_a, prm.d0_a, bd * bd)), sz = pdk::fast_sqrt(fmaf(prm.z0_a, prm.z0_a, bz * bz));
-      uint32_t r[4];
-      pdk::rng_block(prm.rk, prm.event_base + e_[k], (uint32_t)ob_[k], 3u, r);
-      o_d0[k] = fmaf(sd, pdk::normal_bm(r[0], r[1]), d0);
-      o_z0[k] = fmaf(sz, pdk::normal_bm(r[2], r[3]), z0);
-      o_sd[k] = sd, o_sz[k] = sz;
-    }
+    for (int k = 0; k < ITEMS; ++k)
+      pdk::track_impact(cfg, prm.rk, prm.event_base + e_[k], (uint32_t)ob_[k], q_[k], px_[k], py_[k], pz_[k], vx_[k], vy_[k], vz_[k], o_d0[k],
+                        o_z0[k], o_sd[k], o_sz[k]);
     if (full) {
       *reinterpret_cast<float4 *>(prm.d0 + tb) = make_float4(o_d0[0], o_d0[1], o_d0[2], o_d0[3]);
       *reinterpret_cast<float4 *>(prm.z0 + tb) = make_float4(o_z0[0], o_z0[1], o_z0[2], o_z0[3]);

@@ -167,6 +167,12 @@ struct PdParams {
   int *park_pid;
   signed char *park_q;
   float *park_f[6];              // pt, eta, phi, E, eta_out, phi_out
+  // impact parameters from the chain itself (pd_options.impact): kernel P parks d0, z0, d0_err, z0_err of an accepted track
+  // beside its record, kernel T moves them to imp_out[.][track]; imp_on = 0: none of this is touched
+  int imp_on;
+  float imp_d0_a, imp_d0_b, imp_z0_a, imp_z0_b;
+  float *park_imp[4];
+  float *imp_out[4];
   unsigned int *ptile_counter;
   int *tile_ev;                  // [n_ptiles + 1][2] per tile boundary: first event with offset >= it, last with offset <= it
   unsigned short *key;           // [n_ptiles * PD_PTILE] per particle: tower id | HCAL bit << 15, 0xffff = no deposit

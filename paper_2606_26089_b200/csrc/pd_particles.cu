@@ -23,6 +23,7 @@
 #include <cstdlib>
 
 #include "pd_internal.h"
+#include "pd_impact_math.cuh"
 #include "pd_math.cuh"
 #include "pd_scan.cuh"
 
@@ -111,7 +112,7 @@ __global__ void pd_tile_events_kernel(const long long *offsets, long long n_even
   out[2 * j + 1] = (int)lo - 1;
 }
 
-template <bool DEBUG>
+template <bool DEBUG, bool IMPACT>
 __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid_constant__ PdParams prm) {
   extern __shared__ __align__(128) unsigned char smem[];
   const PdCardScalars &sc = prm.sc;
@@ -276,7 +277,8 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
       bool accepted = false;
       int i = 0, pid = 0;
       float px = 0.f, py = 0.f, pz = 0.f, u = 0.f, phi_pos = 0.f;
-      uint32_t r1 = 0u, r2 = 0u;
+      uint32_t r1 = 0u, r2 = 0u, pidx_t = 0u;
+      long long ev_t = 0;  // (IMPACT: the track's event and index in it, for Philox stream 3)
       if (v < n_work) {
         const int cls = v < nA ? 0 : (v < nA + nB ? 1 : 2);
         const unsigned ent = s_list[wbase + v];
@@ -325,6 +327,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
           rng_block(prm.rk, prm.event_base + ev, pidx, 0u, rn);
           accepted = uniform24(rn[0]) < sc.row_eps[ent >> 11];
           r1 = rn[1], r2 = rn[2];
+          if (IMPACT) ev_t = prm.event_base + ev, pidx_t = pidx;
         }
         // what the tower pass needs: tower | HCAL bit, or "no deposit"
         s_key[i] = (tower >= 0 && !to_none) ? (unsigned short)((unsigned)tower | (to_ecal ? 0u : 0x8000u)) : (unsigned short)PT_NONE;
@@ -351,6 +354,13 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
         prm.park_q[g] = s_q[i];
         prm.park_f[0][g] = t.pt_s, prm.park_f[1][g] = t.eta_mom, prm.park_f[2][g] = t.phi0;
         prm.park_f[3][g] = t.E_trk, prm.park_f[4][g] = eta_from_u(sc, u), prm.park_f[5][g] = phi_pos;
+        if (IMPACT) {
+          // pd_options.impact: d0, z0 and their errors while the particle is on chip (the stand-alone kernel has to gather it)
+          const ImpactCfg ic{sc.inv_kB, sc.sB, prm.imp_d0_a, prm.imp_d0_b, prm.imp_z0_a, prm.imp_z0_b};
+          float d0m, z0m, sd, sz;
+          track_impact(ic, prm.rk, ev_t, pidx_t, (int)s_q[i], px, py, pz, s_vx[i], s_vy[i], s_vz[i], d0m, z0m, sd, sz);
+          prm.park_imp[0][g] = d0m, prm.park_imp[1][g] = z0m, prm.park_imp[2][g] = sd, prm.park_imp[3][g] = sz;
+        }
         atomicOr(&s_accmask[i >> 5], 1u << (i & 31));
         if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[s0 + i] = t.pt_s;
       }
@@ -377,7 +387,8 @@ size_t pd_particle_smem_bytes(const pd_card *c) { return pdk::make_ptables(c->sc
 int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_smem_optin, void *stream) {
   const size_t smem = pdk::make_ptables(prm.sc.n_bins, 2 * prm.sc.lut_side).total;
   if (smem > (size_t)max_smem_optin) return PD_ECUDA;
-  auto kern = debug ? pdk::pd_particle_kernel<true> : pdk::pd_particle_kernel<false>;
+  auto kern = prm.imp_on ? (debug ? pdk::pd_particle_kernel<true, true> : pdk::pd_particle_kernel<false, true>)
+                         : (debug ? pdk::pd_particle_kernel<true, false> : pdk::pd_particle_kernel<false, false>);
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin) != cudaSuccess) return PD_ECUDA;
   // persistent CTAs that claim their tiles from a counter: as many as fit on the device
   int per_sm = 0;

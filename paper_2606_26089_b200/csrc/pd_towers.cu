@@ -262,6 +262,10 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
             prm.trk_charge[o] = __ldg(prm.park_q + g);
             prm.trk_pt[o] = pt, prm.trk_eta[o] = eta, prm.trk_phi[o] = phi, prm.trk_E[o] = Et;
             prm.trk_eta_out[o] = __ldg(prm.park_f[4] + g), prm.trk_phi_out[o] = __ldg(prm.park_f[5] + g);
+            if (prm.imp_on) {
+#pragma unroll
+              for (int k4 = 0; k4 < 4; ++k4) prm.imp_out[k4][o] = __ldg(prm.park_imp[k4] + g);
+            }
             const unsigned at = (unsigned)base_efl + (unsigned)(done + r);
             const int apid = pid < 0 ? -pid : pid;
             prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
@@ -863,6 +867,20 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
             prm.trk_src[o2] = (int)(p_al + gs + i1), prm.trk_pid[o2] = d1, prm.trk_charge[o2] = q1_;
             prm.trk_pt[o2] = f1[0], prm.trk_eta[o2] = f1[1], prm.trk_phi[o2] = f1[2], prm.trk_E[o2] = f1[3];
             prm.trk_eta_out[o2] = f1[4], prm.trk_phi_out[o2] = f1[5];
+          }
+        }
+      }
+      if (prm.imp_on) {
+        // pd_options.impact: the four values kernel P parked beside each record, in a loop of their own (the common path
+        // above stays as it is)
+        for (int k = wid - 1; k < n_seg; k += W - 1) {
+          const long long gs = (gseg_lo + k) * PD_PSEG;
+          const int a = s_sega[k], c = s_segc[k];
+          const unsigned ob = (unsigned)t0 + (unsigned)s_segp[k];
+          for (int r = lane; r < c; r += 32) {
+            const long long g = gs + a + r;
+#pragma unroll
+            for (int k4 = 0; k4 < 4; ++k4) prm.imp_out[k4][ob + (unsigned)r] = __ldg(prm.park_imp[k4] + g);
           }
         }
       }

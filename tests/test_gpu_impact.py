@@ -201,3 +201,43 @@ def test_unaligned_arrays_take_the_scalar_path():
     torch.cuda.synchronize()
     for k in a:
         assert views[k][:n].cpu().numpy().tobytes() == a[k].tobytes(), k
+
+
+@pytest.mark.parametrize("card_name,cfg,n_events", [("cms_like", 0, 3000), ("cms_like", 2, 12), ("aleph_like", 4, 4000)])
+def test_impact_from_the_chain_itself(card_name, cfg, n_events):
+    """pd_options.impact: kernel P computes d0, z0 and their errors for the tracks it accepts (the particle is on chip there) and
+    kernel T writes them beside the Track collection -- bit for bit what pd_track_impact gives after the step (the same
+    device function), hence the oracle's values too (checked above); the collections themselves do not change.  With an event
+    that goes through the big-tile path."""
+    import paper_2606_26089_b200 as pd
+
+    ev = wl.generate(cfg, n_events)
+    if cfg == 0:
+        big = wl.generate(2, 3)
+        big = wl.Events(offsets=np.array([0, big.n_particles], dtype=np.int64),
+                        **{k: getattr(big, k) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
+        ev = wl.concat_events([wl.slice_events(ev, 0, 1500), big, wl.slice_events(ev, 1500, n_events)])
+    card = pd.Card(card_name)
+    dev = pd.DeviceEvents(ev)
+    res = ((2e-5, 1e-4), (3e-5, 2e-4))
+    plain = pd.DeviceOutputs(card, dev.n_events, dev.n_particles)
+    pd.simulate(card, dev, plain, 9, event_base=17)
+    n_trk = int(plain.trk["offsets"][-1])
+    assert n_trk > 1000
+    want = pd.DeviceImpact(dev.n_particles)
+    pd.track_impact(card, dev, plain, want, d0_res=res[0], z0_res=res[1], seed=9, event_base=17)
+    w = want.to_numpy(n_trk)
+    fused = pd.DeviceOutputs(card, dev.n_events, dev.n_particles, impact=res)
+    assert fused.ws_bytes > plain.ws_bytes
+    for t in fused.impact.t.values():
+        t.fill_(float("nan"))
+    pd.simulate(card, dev, fused, 9, event_base=17)
+    assert pd.last_status(fused) == 0
+    g = fused.impact.to_numpy(n_trk)
+    for k in ("d0", "z0", "d0_err", "z0_err"):
+        assert g[k].tobytes() == w[k].tobytes(), k
+    a, b = plain.to_numpy(), fused.to_numpy()
+    for k in a:
+        assert a[k].tobytes() == b[k].tobytes(), k
+    # nothing written beyond the tracks
+    assert bool(fused.impact.t["d0"][n_trk:].isnan().all())
