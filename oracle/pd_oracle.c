@@ -47,6 +47,7 @@ struct pdo_card {
   double trk_eta[PDO_MAX_RES_ROWS][5], trk_eta_sinh[PDO_MAX_RES_ROWS][2];
   double nsig_ecal, nsig_hcal;           /* K2: component kept iff also E' > n_sigma sigma(E')                  */
   int smear_center;                      /* K3: reported tower (eta, phi) uniform inside the cell               */
+  int eflow_weighted;                    /* K5: tracks of a component without a neutral are rescaled to the weighted mean */
 };
 
 /* reading A28: every card number is rounded to fp32 at load; the oracle uses the promoted value */
@@ -265,6 +266,7 @@ static int card_from_file(pdo_card *c, const char *path) {
     else if (!strcmp(key, "ecal_nsigma") && nv == 1) c->nsig_ecal = v[0];
     else if (!strcmp(key, "hcal_nsigma") && nv == 1) c->nsig_hcal = v[0];
     else if (!strcmp(key, "smear_tower_center") && nv == 1) c->smear_center = v[0] != 0.0;
+    else if (!strcmp(key, "eflow_weighted") && nv == 1) c->eflow_weighted = v[0] != 0.0;
     else if (!strcmp(key, "ecal_thr") && nv == 1) c->thr_ecal = v[0];
     else if (!strcmp(key, "hcal_thr") && nv == 1) c->thr_hcal = v[0];
     else if (!strcmp(key, "eff") && (nv == 5 || (nv == 6 && (v[5] == 0.0 || v[5] == 1.0 || v[5] == 2.0 || v[5] == 3.0))) &&
@@ -396,6 +398,16 @@ double pdo_lognormal(double m, double s, double z) {
 
 static double resolution(const double csn[3], double E) {
   return sqrt(csn[0] * csn[0] * E * E + csn[1] * csn[1] * E + csn[2] * csn[2]);
+}
+
+/* reading K5: the factor on the EFlow entries of the tracks of a tower component whose neutral excess
+ * is not emitted: tracks measure T with variance V = sum (sigma_rel,i E_trk,i)^2, the calorimeter E' with variance s2 =
+ * sigma(E')^2; the weighted mean (T / V + E' / s2) / (1 / V + 1 / s2) = (T s2 + E' V) / (s2 + V), over T.  No calorimeter
+ * information (E' = 0: nothing deposited or the component was cut) or no tracks: 1.  V = s2 = 0: 1. */
+double pdo_eflow_weight(double T, double V, double Ec, double sigma_c) {
+  const double s2 = sigma_c * sigma_c;
+  if (!(T > 0.0) || !(Ec > 0.0) || !(s2 + V > 0.0)) return 1.0;
+  return (T * s2 + Ec * V) / ((s2 + V) * T);
 }
 
 /* reading K4: (a, b) of step S3 for a track of the given species with true vertex momentum
@@ -767,7 +779,8 @@ int pdo_tower_position(const pdo_card *c, uint64_t seed, int64_t event, int32_t 
 int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t event_base,
                  pdo_tracks *trk, pdo_towers *tow, pdo_eflow *efl, pdo_debug *dbg,
                  const pdo_overrides *ov) {
-  double *Eem, *Ehad, *Tem, *Thad, *ph_E, *nh_E;
+  double *Eem, *Ehad, *Tem, *Thad, *Vem, *Vhad, *Fem, *Fhad, *ph_E, *nh_E;
+  int32_t *wt_tower = NULL; /* K5: per EFlow track entry of the call: tower * 2 + component (1 = HCAL), -1 none */
   uint8_t *touched;
   int32_t *list, *ph_id, *nh_id;
   int64_t e, n_trk = 0, n_tow = 0, n_efl = 0, n_dbg_tw = 0, rejected = 0;
@@ -775,7 +788,7 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
   int rc = PDO_OK;
   if (!c || !ev || !trk || !tow || !efl || ev->n_events < 0 || ev->n_particles < 0) return PDO_EINVAL;
   if (ev->n_events > 0 && !ev->offsets) return PDO_EINVAL;
-  Eem = (double *)calloc((size_t)c->n_towers * 4, sizeof(double));
+  Eem = (double *)calloc((size_t)c->n_towers * 8, sizeof(double));
   touched = (uint8_t *)calloc((size_t)c->n_towers, 1);
   list = (int32_t *)malloc((size_t)c->n_towers * 3 * sizeof(int32_t));
   ph_E = (double *)malloc((size_t)c->n_towers * 2 * sizeof(double));
@@ -795,13 +808,21 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
     qsort(ov_order, (size_t)ov->n_tower_ov, sizeof(int64_t), cmp_ov);
   }
   Ehad = Eem + c->n_towers, Tem = Ehad + c->n_towers, Thad = Tem + c->n_towers;
+  Vem = Thad + c->n_towers, Vhad = Vem + c->n_towers, Fem = Vhad + c->n_towers, Fhad = Fem + c->n_towers;
+  if (c->eflow_weighted) {
+    wt_tower = (int32_t *)malloc((size_t)(efl->capacity > 0 ? efl->capacity : 1) * sizeof(int32_t));
+    if (!wt_tower) {
+      free(Eem), free(touched), free(list), free(ph_E), free(ov_order);
+      return PDO_EINVAL;
+    }
+  }
   ph_id = list + c->n_towers, nh_id = ph_id + c->n_towers;
   nh_E = ph_E + c->n_towers;
   trk->offsets[0] = tow->offsets[0] = efl->offsets[0] = 0;
   if (dbg && dbg->tw_offsets) dbg->tw_offsets[0] = 0;
 
   for (e = 0; e < ev->n_events && rc == PDO_OK; ++e) {
-    int64_t i0 = ev->offsets[e], i1 = ev->offsets[e + 1], i, trk_begin = n_trk;
+    int64_t i0 = ev->offsets[e], i1 = ev->offsets[e + 1], i, trk_begin = n_trk, efl_begin = n_efl;
     int n_list = 0, n_ph = 0, n_nh = 0, t;
     int64_t event = event_base + e; /* reading A27 */
     for (i = i0; i < i1; ++i) {
@@ -811,7 +832,8 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
       double fe = (apid == 11 || apid == 22) ? 1.0 : 0.0;
       double fh = (apid == 11 || apid == 22 || apid == 13 || apid == 12 || apid == 14 || apid == 16) ? 0.0 : 1.0;
       double px = ev->px[i], py = ev->py[i], pz = ev->pz[i], E = ev->E[i];
-      double pt = hypot(px, py), pt_smeared = 0.0, Etrk = 0.0;
+      double pt = hypot(px, py), pt_smeared = 0.0, Etrk = 0.0, sigE = 0.0;
+      int64_t my_efl = -1;
       int accepted = 0, row = -1;
       int32_t tower;
       uint32_t near;
@@ -848,6 +870,7 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
             srel = sqrt(ta * ta + (tb * pt) * (tb * pt));
             pt_smeared = pdo_lognormal(pt, srel * pt, pdo_normal(r[1], r[2]));
             Etrk = pt_smeared * cosh(eta_mom);
+            sigE = srel * Etrk; /* K5: the track's energy resolution */
             if (n_trk >= trk->capacity || n_efl >= efl->capacity) {
               rc = PDO_ECAPACITY;
               break;
@@ -868,6 +891,8 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
             efl->eta[n_efl] = eta_mom;
             efl->phi[n_efl] = trk->phi[n_trk];
             efl->E[n_efl] = Etrk;
+            my_efl = n_efl;
+            if (wt_tower) wt_tower[n_efl] = -1;
             ++n_trk, ++n_efl;
           }
         }
@@ -883,6 +908,8 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
           Eem[tower] += fe * E;
           Ehad[tower] += fh * E;
           if (accepted) Tem[tower] += fe * Etrk, Thad[tower] += fh * Etrk;
+          if (accepted) Vem[tower] += fe * sigE * sigE, Vhad[tower] += fh * sigE * sigE;
+          if (accepted && wt_tower) wt_tower[my_efl] = tower * 2 + (fh != 0.0 ? 1 : 0);
         }
       }
       if (dbg) {
@@ -977,13 +1004,29 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
       }
       if (is_ph) ph_id[n_ph] = id, ph_E[n_ph] = n_em, ++n_ph;
       if (is_nh) nh_id[n_nh] = id, nh_E[n_nh] = n_had, ++n_nh;
+      /* reading K5: a component with tracks whose neutral excess is not emitted hands its calorimeter measurement to the
+       * tracks: their EFlow entries are rescaled to the weighted mean of the two */
+      Fem[id] = Fhad[id] = 1.0;
+      if (c->eflow_weighted) {
+        pdo_tower_centre(c, id, &eta_c, &phi_c);
+        if (!is_ph) Fem[id] = pdo_eflow_weight(Tem[id], Vem[id], em_f, resolution(resolution_row(c->ecal, c->ecal_eta, c->n_ecal_eta, fabs(eta_c)), em_f));
+        if (!is_nh) Fhad[id] = pdo_eflow_weight(Thad[id], Vhad[id], had_f, resolution(resolution_row(c->hcal, c->hcal_eta, c->n_hcal_eta, fabs(eta_c)), had_f));
+      }
       /* reset the dense accumulators for the next event */
-      Eem[id] = Ehad[id] = Tem[id] = Thad[id] = 0.0;
+      Eem[id] = Ehad[id] = Tem[id] = Thad[id] = Vem[id] = Vhad[id] = 0.0;
       touched[id] = 0;
     }
     if (rc != PDO_OK) break;
     tow->offsets[e + 1] = n_tow;
     if (dbg && dbg->tw_offsets) dbg->tw_offsets[e + 1] = n_dbg_tw;
+    if (wt_tower) {
+      int64_t k;
+      for (k = efl_begin; k < n_efl; ++k)
+        if (wt_tower[k] >= 0) {
+          const double f = (wt_tower[k] & 1) ? Fhad[wt_tower[k] >> 1] : Fem[wt_tower[k] >> 1];
+          efl->pt[k] *= f, efl->E[k] *= f;
+        }
+    }
     /* O7: EFlow = tracks (already written) ++ photons ascending id ++ neutral hadrons ascending id */
     if (n_efl + n_ph + n_nh > efl->capacity) {
       rc = PDO_ECAPACITY;
@@ -1005,7 +1048,7 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
     efl->offsets[e + 1] = n_efl;
   }
   if (rc == PDO_OK && ov_order) rejected += ov->n_tower_ov - ov_pos; /* overrides never reached */
-  free(Eem), free(touched), free(list), free(ph_E), free(ov_order);
+  free(Eem), free(touched), free(list), free(ph_E), free(ov_order), free(wt_tower);
   if (ov && ov->n_rejected) *ov->n_rejected = rejected;
   if (rc == PDO_OK && rejected > 0) rc = PDO_EOVERRIDE;
   return rc;

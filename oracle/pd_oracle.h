@@ -289,6 +289,10 @@ double pdo_efficiency_species(const pdo_card *c, double pt, double eta_mom, doub
  * sigma_rel = sqrt(a^2 + (b pT)^2) for a track of the species with true momentum (px, py, pz); returns the row, -1 = the
  * species' / the card's track_res line (reading J2) */
 int pdo_track_resolution(const pdo_card *c, int species, double px, double py, double pz, double *a, double *b);
+/* reading K5 (weighted EFlow, card key eflow_weighted = 1): factor on the EFlow entries (pT, E) of the tracks of a tower
+ * component whose neutral is not emitted; T, V: sum and variance of the tracks' energies, Ec, sigma_c: the component's kept
+ * smeared energy and its resolution there */
+double pdo_eflow_weight(double T, double V, double Ec, double sigma_c);
 
 #ifdef __cplusplus
 }

@@ -110,6 +110,8 @@ def lib():
         L.pdo_efficiency_species.restype = C.c_double
         L.pdo_track_resolution.argtypes = [_p, C.c_int, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.pdo_track_resolution.restype = C.c_int
+        L.pdo_eflow_weight.argtypes = [C.c_double] * 4
+        L.pdo_eflow_weight.restype = C.c_double
         L.pdo_pileup_merge.argtypes = [C.POINTER(_Events), C.POINTER(_Events), C.c_double, C.c_double, C.c_double, C.c_int,
                                        C.c_uint64, C.c_int64, C.c_int64] + [_p] * 12
         L.pdo_filter_eflow.argtypes = [C.c_int64] + [_p] * 7 + [C.POINTER(_Condition), C.c_int32, C.c_int32] + [_p] * 8
@@ -373,6 +375,11 @@ def _events_struct(ev):
 
 def _vp(a):
     return a.ctypes.data_as(C.c_void_p)
+
+
+def eflow_weight(T, V, Ec, sigma_c):
+    """pdo_eflow_weight (reading K5)"""
+    return float(lib().pdo_eflow_weight(float(T), float(V), float(Ec), float(sigma_c)))
 
 
 def pileup_merge(hs, pool, mean_pileup: float, sigma_z: float = 0.053, max_z_spread: float = 0.25,

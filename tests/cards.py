@@ -22,7 +22,7 @@ DEFAULT_EFF = [(1.0, "inf", 0.0, 1.5, 0.97), (1.0, "inf", 1.5, 2.5, 0.85), (0.1,
 def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kappa=0.299792458,
               eff=DEFAULT_EFF, abs_costheta_max=None, track_res=(0.01, 1.5e-4), ecal=(0.007, 0.07, 0.35),
               hcal=(0.05, 1.5, 0.0), ecal_thr=0.5, hcal_thr=1.0, name="custom", track_res_species=None,
-              ecal_res_eta=(), hcal_res_eta=(), ecal_nsigma=None, hcal_nsigma=None, smear_tower_center=None, track_res_eta=()):
+              ecal_res_eta=(), hcal_res_eta=(), ecal_nsigma=None, hcal_nsigma=None, smear_tower_center=None, track_res_eta=(), eflow_weighted=None):
     lines = ["name = %s" % name, "bz = %r" % bz, "radius = %r" % radius, "half_length = %r" % half_length,
              "kappa = %r" % kappa, "grid = %s" % grid]
     edges = [float(x) for x in edges]
@@ -52,6 +52,8 @@ def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kap
         lines.append("hcal_nsigma = %r" % hcal_nsigma)
     if smear_tower_center is not None:
         lines.append("smear_tower_center = %d" % int(smear_tower_center))
+    if eflow_weighted is not None:
+        lines.append("eflow_weighted = %d" % int(eflow_weighted))  # reading K5
     lines.append("ecal_thr = %r" % ecal_thr)
     lines.append("hcal_thr = %r" % hcal_thr)
     return "\n".join(lines) + "\n"

@@ -199,3 +199,82 @@ def test_track_resolution_rows_give_the_rows_width(tmp_path):
         for k in range(3):
             assert abs(ratio[:, k].mean() - 1.0) < 4.0 * want[k] / math.sqrt(n_ev)
             assert abs(ratio[:, k].std() - want[k]) < 4.0 * want[k] / math.sqrt(2.0 * n_ev), (pid, k, ratio[:, k].std(), want[k])
+
+
+def test_weighted_eflow_limits_and_closed_forms(tmp_path):
+    """Reading K5 (card key eflow_weighted): the EFlow entries of the tracks of a tower component whose neutral is not emitted are
+    rescaled to the inverse-variance weighted mean of the track and the calorimeter measurement.  Pinned on the textbook
+    properties of that mean and on limits in which the result has a closed form -- not on the formula."""
+    # the weight function: equal variances -> arithmetic mean; a perfect side wins; nothing to combine -> 1
+    assert pdo.eflow_weight(10.0, 4.0, 14.0, 2.0) == pytest.approx(1.2, rel=1e-15)     # (10 + 14) / 2 over 10
+    assert pdo.eflow_weight(10.0, 1.0, 14.0, 3.0) == pytest.approx((10 * 9 + 14 * 1) / 10.0 / 10.0, rel=1e-15)  # weights 9 : 1
+    assert pdo.eflow_weight(10.0, 0.0, 12.0, 1.0) == 1.0 and pdo.eflow_weight(10.0, 4.0, 12.0, 0.0) == pytest.approx(1.2, rel=1e-15)
+    assert pdo.eflow_weight(10.0, 4.0, 0.0, 1.0) == 1.0 and pdo.eflow_weight(0.0, 0.0, 5.0, 1.0) == 1.0 and pdo.eflow_weight(10.0, 0.0, 12.0, 0.0) == 1.0
+    for T, V, E, s in ((10.0, 4.0, 14.0, 1.0), (50.0, 0.3, 20.0, 7.0), (3.0, 9.0, 3.5, 0.1)):
+        m = T * pdo.eflow_weight(T, V, E, s)
+        assert min(T, E) <= m <= max(T, E)                                   # a mean lies between its arguments
+        assert abs(m - (T if V < s * s else E)) <= abs(m - (E if V < s * s else T))  # ... nearer the better measurement
+
+    b = pdo.Card("cms_like")
+    eff = [(0.1, "inf", 0.0, 2.5, 1.0)]
+    etas = [-1.9, -1.2, -0.6, 0.1, 0.7, 1.3, 2.0]   # distinct towers, all inside the tracker acceptance
+    n_ev = 3000
+    # pions of 40 GeV each; HCAL threshold 20 GeV: the component (E' ~ 40 +- 4) is always kept, its neutral excess (E' - T ~ 0 +- 5.7)
+    # practically never emitted
+    ev = wl.from_lists([[P(211, 1, 40.0 / math.cosh(eta), eta, 0.2 + 0.4 * k, 0.13957039) for k, eta in enumerate(etas)] for _ in range(n_ev)])
+    E_true = ev.E.astype(np.float64)
+
+    def run(**kw):
+        """oracle outputs with the EFlow arrays cut down to the entries of the tracks (classes 0-2: same order as the Track collection)"""
+        args = dict(eff=eff, track_res=(0.1, 0.0), hcal=(0.1, 0.0, 0.0), hcal_thr=20.0, eflow_weighted=1)
+        args.update(kw)
+        o = pdo.simulate(pdo.Card(cards.variant(tmp_path / ("w%d.card" % len(list(tmp_path.iterdir()))), b.edges, b.nphi, **args)), ev, 31)
+        rows = o["efl_cls"] < 3
+        assert rows.sum() == len(o["trk_E"]) == len(E_true) and (~rows).sum() < 30   # (a neutral is emitted in a handful of cases)
+        return dict(o, **{k: o[k][rows] for k in ("efl_E", "efl_pt", "efl_eta", "efl_phi")})
+
+    off = run(eflow_weighted=0)
+    assert off["efl_E"].tobytes() == off["trk_E"].tobytes()                  # without the key: EFlow tracks = the tracks
+    # 10 % + 10 %: the combination resolves E to 10 % / sqrt(2) (textbook), better than either alone; tracks and towers unchanged
+    o = run()
+    assert o["trk_E"].tobytes() == off["trk_E"].tobytes() and o["tow_E"].tobytes() == off["tow_E"].tobytes()
+    assert len(o["tow_Ehad"]) == len(E_true)
+    r_trk, r_cal, r_w = o["trk_E"] / E_true, o["tow_Ehad"] / E_true, o["efl_E"] / E_true
+    assert abs(r_trk.std() - 0.1) < 0.004 and abs(r_cal.std() - 0.1) < 0.004
+    assert abs(r_w.std() - 0.1 / math.sqrt(2.0)) < 0.004, r_w.std()
+    assert np.all(r_w >= np.minimum(r_trk, r_cal) - 1e-6) and np.all(r_w <= np.maximum(r_trk, r_cal) + 1e-6)
+    assert np.allclose(o["efl_pt"] / o["trk_pt"], o["efl_E"] / o["trk_E"], rtol=1e-6)   # pT and E by the same factor; eta, phi untouched
+    assert o["efl_eta"].tobytes() == o["trk_eta"].tobytes() and o["efl_phi"].tobytes() == o["trk_phi"].tobytes()
+    # a perfect tracker ignores the calorimeter; a perfect calorimeter overrules the tracker: EFlow E = the deposited energy
+    o = run(track_res=(0.0, 0.0))
+    assert o["efl_E"].tobytes() == o["trk_E"].tobytes()
+    o = run(hcal=(0.0, 0.0, 0.0))
+    assert np.allclose(o["efl_E"], E_true, rtol=2e-7) and not np.allclose(o["trk_E"], E_true, rtol=1e-3)
+    # the component cut away (here: by an impossible significance cut): no calorimeter information, the tracks stay
+    o = run(hcal_nsigma=1e6)
+    assert not o["tow_Ehad"].any() and o["efl_E"].tobytes() == o["trk_E"].tobytes()
+    # where the neutral IS emitted the tracks stay as they are: a K0L of 200 GeV joins every pion's tower
+    ev2 = wl.from_lists([[p for k, eta in enumerate(etas) for p in (P(211, 1, 20.0, eta, 0.2 + 0.4 * k, 0.13957039), P(130, 0, 200.0 / math.cosh(eta), eta, 0.2 + 0.4 * k, 0.497611))]
+                         for _ in range(50)])
+    c2 = pdo.Card(cards.variant(tmp_path / "emit.card", b.edges, b.nphi, eff=eff, track_res=(0.1, 0.0), hcal=(0.1, 0.0, 0.0), eflow_weighted=1))
+    o = pdo.simulate(c2, ev2, 31)
+    nt = len(o["trk_E"])
+    assert (o["efl_cls"] == 3).sum() > 300 and nt == 50 * len(etas)
+    emitted = set(zip(np.repeat(np.arange(50), np.diff(o["efl_offsets"]))[o["efl_cls"] == 3].tolist(), o["efl_src"][o["efl_cls"] == 3].tolist()))
+    trk_ev = np.repeat(np.arange(50), np.diff(o["trk_offsets"]))
+    dbg_tower = o["dbg_tower"][o["trk_src"]]
+    trk_rows = np.nonzero(o["efl_cls"] < 3)[0]
+    for k in range(nt):
+        same = o["efl_E"][trk_rows[k]] == o["trk_E"][k]
+        assert same == ((int(trk_ev[k]), int(dbg_tower[k])) in emitted), k
+    # several tracks in one component share the factor; a muon (no deposit) is never touched
+    ev3 = wl.from_lists([[P(211, 1, 20.0, 0.30, 0.50, 0.13957039), P(-211, -1, 35.0, 0.30, 0.50, 0.13957039), P(13, -1, 30.0, 0.30, 0.50, 0.1056584),
+                          P(211, 1, 40.0, -1.0, 2.0, 0.13957039)] for _ in range(40)])
+    o = pdo.simulate(pdo.Card(cards.variant(tmp_path / "multi.card", b.edges, b.nphi, eff=eff, track_res=(0.1, 0.0), hcal=(0.1, 0.0, 0.0), hcal_thr=30.0,
+                                            eflow_weighted=1)), ev3, 31)
+    assert (o["efl_cls"] < 3).sum() == 160 == len(o["trk_E"])
+    f = (o["efl_E"][o["efl_cls"] < 3] / o["trk_E"]).reshape(40, 4)
+    t = o["dbg_tower"].reshape(40, 4)
+    assert (t[:, 0] == t[:, 1]).all() and (t[:, 0] != t[:, 3]).all()      # the two pions of 20 and 35 GeV hit one tower
+    assert np.allclose(f[:, 0], f[:, 1], rtol=1e-12) and not np.allclose(f[:, 0], f[:, 3], rtol=1e-3)
+    assert np.all(f[:, 2] == 1.0) and np.all(np.abs(f[:, 0] - 1.0) > 1e-6) and np.all(np.abs(f[:, 3] - 1.0) > 1e-6)
