@@ -249,7 +249,8 @@ class DeviceOutputs:
         self.trk = {"offsets": mk(n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TRACK_FIELDS}}
         self.tow = {"offsets": mk(n_events + 1, "int64"), **{k: mk(n, dt) for k, dt in TOWER_FIELDS}}
         self.efl = {"offsets": mk(n_events + 1, "int64"), **{k: mk(2 * n, dt) for k, dt in EFLOW_FIELDS}}
-        self.dbg = {k: mk(n, dt) for k, dt in DEBUG_FIELDS} if debug else None
+        # (zero-filled: the per-tower debug arrays are written only at the first depositing particle of each tower)
+        self.dbg = {k: torch.zeros(n, dtype=getattr(torch, dt), device=device) for k, dt in DEBUG_FIELDS} if debug else None
         self.ws_bytes = workspace_bytes(card, n_events, n_particles, self.tile_events, impact is not None)
         if impact is not None:
             self.impact = DeviceImpact(n, device=device)

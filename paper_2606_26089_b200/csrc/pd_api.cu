@@ -42,9 +42,9 @@ static size_t ws_chain_bytes(const PdLaunchPlan &plan) {
 // What kernel P leaves for kernel T, per particle slot (n_ptiles * PD_PTILE slots): the 16-bit key, the accepted bit,
 // and the parked track records (segment index 1 B, charge 1 B, pid 4 B, six floats).  Each array 256-byte aligned.
 struct WsLayout {
-  size_t tile_ev, key, accmask, idx, q, pid, f[6], imp[4], big_acc, total;
+  size_t tile_ev, key, accmask, idx, q, pid, f[6], imp[4], sig, big_acc, total;
 };
-static WsLayout ws_layout(const PdLaunchPlan &plan, int n_towers, bool impact = false) {
+static WsLayout ws_layout(const PdLaunchPlan &plan, int n_towers, bool impact = false, bool weighted = false) {
   const size_t slots = (size_t)PD_PTILE * (size_t)(plan.n_ptiles > 0 ? plan.n_ptiles : 1);
   WsLayout l;
   size_t o = ws_chain_bytes(plan);
@@ -61,7 +61,8 @@ static WsLayout ws_layout(const PdLaunchPlan &plan, int n_towers, bool impact = 
   l.pid = take(4 * slots);
   for (int k = 0; k < 6; ++k) l.f[k] = take(4 * slots);
   for (int k = 0; k < 4; ++k) l.imp[k] = take(impact ? 4 * slots : 0);  // pd_options.impact
-  l.big_acc = take(8 * 5 * (size_t)n_towers * (size_t)plan.max_ctas);  // tiles that do not fit on chip (any event size)
+  l.sig = take(weighted ? 4 * slots : 0);                                // reading K5: sigma_E of the parked tracks
+  l.big_acc = take(8 * (weighted ? 7 : 5) * (size_t)n_towers * (size_t)plan.max_ctas);  // tiles that do not fit on chip (any event size)
   l.total = o;
   return l;
 }
@@ -135,7 +136,7 @@ int64_t pd_workspace_bytes_ex(const pd_card *card, int64_t n_events, int64_t n_p
   if (!card || n_events < 0 || n_particles < 0 || !options_ok(opt)) return PD_EINVAL;
   PdLaunchPlan plan;
   pd_plan(card, n_events, n_particles, tile_events_of(opt), &plan);
-  return (int64_t)ws_layout(plan, card->sc.n_towers, impact_of(opt)).total;
+  return (int64_t)ws_layout(plan, card->sc.n_towers, impact_of(opt), card->sc.eflow_weighted != 0).total;
 }
 int64_t pd_workspace_bytes(const pd_card *card, int64_t n_events, int64_t n_particles) {
   return pd_workspace_bytes_ex(card, n_events, n_particles, nullptr);
@@ -495,7 +496,7 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
   p.chain = (unsigned long long *)(ws + kWsHeader);
   p.chain_t = p.chain + (plan.n_tiles > 0 ? plan.n_tiles : 1);
   {
-    const WsLayout wl = ws_layout(plan, card->sc.n_towers, impact_of(opt));
+    const WsLayout wl = ws_layout(plan, card->sc.n_towers, impact_of(opt), card->sc.eflow_weighted != 0);
     p.tile_ev = (int *)(ws + wl.tile_ev);
     p.key = (unsigned short *)(ws + wl.key);
     p.accmask = (unsigned int *)(ws + wl.accmask);
@@ -504,6 +505,8 @@ static int simulate_impl(const pd_card *card, const pd_events *ev, uint64_t seed
     p.park_pid = (int *)(ws + wl.pid);
     p.big_acc = (long long *)(ws + wl.big_acc);
     for (int k = 0; k < 6; ++k) p.park_f[k] = (float *)(ws + wl.f[k]);
+    p.acc_stride = card->sc.eflow_weighted ? 7 : 5;
+    if (card->sc.eflow_weighted) p.park_sig = (float *)(ws + wl.sig);
     if (impact_of(opt)) {
       p.imp_on = 1;
       p.imp_d0_a = opt->impact_config->d0_a, p.imp_d0_b = opt->impact_config->d0_b;

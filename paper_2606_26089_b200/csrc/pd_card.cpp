@@ -38,6 +38,7 @@ struct RawCard {
   double nsig_ecal = 0, nsig_hcal = 0;                    // reading K2
   bool smear_center = false;                              // reading K3
   std::vector<std::array<double, 5>> trk_eta;             // reading K4: aeta_lo, aeta_hi, a, b, species
+  bool eflow_weighted = false;                            // reading K5
 };
 
 constexpr double kPi = 3.14159265358979323846;
@@ -146,6 +147,7 @@ bool from_file(RawCard &r, const char *path) {
     else if (key == "ecal_nsigma" && v.size() == 1) r.nsig_ecal = v[0];
     else if (key == "hcal_nsigma" && v.size() == 1) r.nsig_hcal = v[0];
     else if (key == "smear_tower_center" && v.size() == 1) r.smear_center = v[0] != 0.0;
+    else if (key == "eflow_weighted" && v.size() == 1) r.eflow_weighted = v[0] != 0.0;
     else if (key == "ecal_thr" && v.size() == 1) r.thr_ecal = v[0];
     else if (key == "hcal_thr" && v.size() == 1) r.thr_hcal = v[0];
     else if (key == "eff" && (v.size() == 5 || (v.size() == 6 && (v[5] == 0.0 || v[5] == 1.0 || v[5] == 2.0 || v[5] == 3.0))) &&
@@ -360,6 +362,7 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
   s.nsig2_ecal = float(f32(r.nsig_ecal) * f32(r.nsig_ecal));
   s.nsig2_hcal = float(f32(r.nsig_hcal) * f32(r.nsig_hcal));
   s.smear_center = r.smear_center ? 1 : 0;
+  s.eflow_weighted = r.eflow_weighted ? 1 : 0;
   // reading K4: the rows' edges as sinh of the fp32-rounded |eta| (fp64, the form the kernel compares |pz| / pT with)
   s.n_trk_rows = int(r.trk_eta.size());
   for (int k = 0; k < PD_MAX_TRK_ROWS; ++k) {

@@ -49,6 +49,7 @@ struct PdCardScalars {
   int res_per_bin;                // K1: the card has eta-dependent resolution rows: C^2, S^2, N^2 per eta bin (PdCardTables::res2)
   float nsig2_ecal, nsig2_hcal;   // K2: n_sigma^2 of the significance cut (0: none)
   int smear_center;               // K3: reported tower position uniform inside the cell (Philox stream 4)
+  int eflow_weighted;             // K5: tracks of a component without a neutral rescaled to the weighted mean of track and calorimeter
   // K4: eta-dependent track resolution rows (first match in file order; species 0 = any, 1 e, 2 mu, 3 charged hadron);
   // a row holds sinh(aeta_lo) pT <= |pz| < sinh(aeta_hi) pT, decided in fp64 exactly as the definition does
   int n_trk_rows;
@@ -108,6 +109,7 @@ struct PdTLayout {
   uint32_t bitmap, gprefix;                     // per event: tower bits, group prefix
   uint32_t l2p, pool;                           // sparse mode
   uint32_t res, Ev, Et, head, stg, ev;          // per particle / per slot
+  uint32_t Es;                                  // K5: per particle, sigma_E of an accepted track (size 0 otherwise)
   uint32_t total;
 };
 
@@ -169,6 +171,10 @@ struct PdParams {
   float *park_f[6];              // pt, eta, phi, E, eta_out, phi_out
   // impact parameters from the chain itself (pd_options.impact): kernel P parks d0, z0, d0_err, z0_err of an accepted track
   // beside its record, kernel T moves them to imp_out[.][track]; imp_on = 0: none of this is touched
+  // weighted EFlow (reading K5): kernel P parks sigma_E = sigma_rel E_trk of an accepted track; accumulators of the big-tile
+  // path: acc_stride 64-bit words per tower (5, or 7 with the two variance sums)
+  float *park_sig;
+  int acc_stride;
   int imp_on;
   float imp_d0_a, imp_d0_b, imp_z0_a, imp_z0_b;
   float *park_imp[4];

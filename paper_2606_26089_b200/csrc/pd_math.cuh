@@ -453,6 +453,7 @@ __device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const Sm
 // 1 and 2 of the particle's Philox block; eta, phi unchanged; E = pT' cosh(eta) = pT' |p| / pT.
 struct TrackOut {
   float pt_s, eta_mom, phi0, E_trk;
+  float rel2;  // sigma_rel^2 of the smear (K5: sigma_E = sqrt(rel2) E_trk)
 };
 
 // reading K4: the first track-resolution row (species 0 = any, else 1 + the species index used here) that holds the true
@@ -482,6 +483,7 @@ __device__ __forceinline__ void track_smear_words(const PdCardScalars &sc, float
   if (sc.n_trk_rows > 0) track_res_row(sc, px, py, pz, species, a2, b);  // reading K4 (cards with eta-dependent rows only)
   const float bp = b * pt;
   const float rel2 = fmaf(bp, bp, a2);
+  t.rel2 = rel2;
   t.pt_s = rel2 > 0.f ? lognormal_rel(pt, rel2, normal_bm(r1, r2)) : pt;
   t.E_trk = t.pt_s * (fast_sqrt(fmaf(pz, pz, pt2)) * ipt);
   t.eta_mom = fast_asinh(pz * ipt);

@@ -112,7 +112,7 @@ __global__ void pd_tile_events_kernel(const long long *offsets, long long n_even
   out[2 * j + 1] = (int)lo - 1;
 }
 
-template <bool DEBUG, bool IMPACT>
+template <bool DEBUG, bool IMPACT, bool WEIGHTED>
 __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid_constant__ PdParams prm) {
   extern __shared__ __align__(128) unsigned char smem[];
   const PdCardScalars &sc = prm.sc;
@@ -361,6 +361,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
           track_impact(ic, prm.rk, ev_t, pidx_t, (int)s_q[i], px, py, pz, s_vx[i], s_vy[i], s_vz[i], d0m, z0m, sd, sz);
           prm.park_imp[0][g] = d0m, prm.park_imp[1][g] = z0m, prm.park_imp[2][g] = sd, prm.park_imp[3][g] = sz;
         }
+        if (WEIGHTED) prm.park_sig[g] = fast_sqrt(t.rel2) * t.E_trk;  // reading K5 (cards with eflow_weighted only)
         atomicOr(&s_accmask[i >> 5], 1u << (i & 31));
         if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[s0 + i] = t.pt_s;
       }
@@ -387,8 +388,13 @@ size_t pd_particle_smem_bytes(const pd_card *c) { return pdk::make_ptables(c->sc
 int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_smem_optin, void *stream) {
   const size_t smem = pdk::make_ptables(prm.sc.n_bins, 2 * prm.sc.lut_side).total;
   if (smem > (size_t)max_smem_optin) return PD_ECUDA;
-  auto kern = prm.imp_on ? (debug ? pdk::pd_particle_kernel<true, true> : pdk::pd_particle_kernel<false, true>)
-                         : (debug ? pdk::pd_particle_kernel<true, false> : pdk::pd_particle_kernel<false, false>);
+  // variants: debug outputs; impact parameters from the chain (pd_options.impact); weighted EFlow (card key, reading K5)
+  using Kern = void (*)(const PdParams);
+  static const Kern kerns[8] = {pdk::pd_particle_kernel<false, false, false>, pdk::pd_particle_kernel<true, false, false>,
+                                pdk::pd_particle_kernel<false, true, false>,  pdk::pd_particle_kernel<true, true, false>,
+                                pdk::pd_particle_kernel<false, false, true>,  pdk::pd_particle_kernel<true, false, true>,
+                                pdk::pd_particle_kernel<false, true, true>,   pdk::pd_particle_kernel<true, true, true>};
+  const Kern kern = kerns[(debug ? 1 : 0) | (prm.imp_on ? 2 : 0) | (prm.park_sig ? 4 : 0)];
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin) != cudaSuccess) return PD_ECUDA;
   // persistent CTAs that claim their tiles from a counter: as many as fit on the device
   int per_sm = 0;

@@ -51,7 +51,7 @@ using Layout = PdTLayout;
 // `bitmap` holds one bit per 128-tower GROUP and event, `l2p` the rank of the first non-empty group of each of its
 // words, `pool` the tower bits of the non-empty groups only (at most one per deposit), `gprefix` their prefixes.
 __host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int words_per_event, int G, int C, int sparse, int res_per_bin = 0,
-                                              int smear_center = 0) {
+                                              int smear_center = 0, int weighted = 0) {
   Layout l;
   size_t o = 0;
   auto take = [&](size_t bytes) {
@@ -91,6 +91,7 @@ __host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int word
   l.head = take(4 * (size_t)C);
   l.stg = take(4 * ((size_t)C + 4));  // first the keys (2 B each, + 8 for the same reason), later one float per slot
   l.ev = take(G > 1 ? (size_t)C : 0);
+  l.Es = take(weighted ? 4 * (size_t)C : 0);  // reading K5
   l.total = (uint32_t)o;
   return l;
 }
@@ -162,9 +163,10 @@ __device__ __forceinline__ int tower_bin(const TCard &tc, int tower) {
 }
 // S6 of one tower with the resolutions of its eta bin (K1) and the significance cut (K2): smeared components and
 // whether each is kept (reading A22: > threshold; K2: and > n_sigma sigma(E'), i.e. E'^2 > n_sigma^2 sigma^2(E'))
+// var_em / var_had (K5): sigma^2 of the component's resolution at its smeared energy, with the tower's row
 template <bool FID>
 __device__ __forceinline__ void tower_components(const PdCardScalars &sc, const TCard &tc, int tower, float Eem, float Ehad, const uint32_t (&rn)[4],
-                                                 float &em_s, float &had_s, bool &k_em, bool &k_had) {
+                                                 float &em_s, float &had_s, bool &k_em, bool &k_had, float *var_em = nullptr, float *var_had = nullptr) {
   float e2[3] = {sc.ecal2[0], sc.ecal2[1], sc.ecal2[2]}, h2[3] = {sc.hcal2[0], sc.hcal2[1], sc.hcal2[2]};
   if (FID && sc.res_per_bin) {
     const float *r = tc.res2 + 6 * tower_bin(tc, tower);
@@ -173,8 +175,19 @@ __device__ __forceinline__ void tower_components(const PdCardScalars &sc, const 
   tower_smear_csn(e2, h2, Eem, Ehad, rn, em_s, had_s);
   k_em = em_s > sc.thr_ecal, k_had = had_s > sc.thr_hcal;
   if (FID && sc.nsig2_ecal > 0.f) k_em = k_em && em_s * em_s > sc.nsig2_ecal * fmaf(e2[0] * em_s, em_s, fmaf(e2[1], em_s, e2[2]));
-  if (FID && sc.nsig2_hcal > 0.f) k_had = k_had && had_s * had_s > sc.nsig2_hcal * fmaf(h2[0] * had_s, had_s, fmaf(h2[1], had_s, h2[2]));
+  if (FID && sc.nsig2_hcal > 0.f) k_had = k_had && had_s * had_s > sc.nsig2_hcal * fmaf(h2[0] * had_s, had_s, fmaf(h2[1], had_s, h2[2]));  if (FID && var_em) *var_em = fmaf(e2[0] * em_s, em_s, fmaf(e2[1], em_s, e2[2])), *var_had = fmaf(h2[0] * had_s, had_s, fmaf(h2[1], had_s, h2[2]));
 }
+// reading K5: the factor on the EFlow entries of the tracks of a component whose neutral is not emitted: tracks measure T with
+// variance V, the calorimeter Ec (kept smeared energy; 0 = no information) with variance s2: weighted mean over T
+__device__ __forceinline__ float eflow_weight(float T, float V, float Ec, float s2) {
+  const float d = s2 + V;
+  if (!(T > 0.f) || !(Ec > 0.f) || !(d > 0.f)) return 1.f;
+  return fmaf(T, s2, Ec * V) / (d * T);
+}
+// exact sums of sigma_E^2: units of 2^-44 GeV^2, terms capped at 2^19 GeV^2
+__device__ __forceinline__ long long var_fix(float sig) { return __float2ll_rn(fminf(sig * sig, 524288.f) * 17592186044416.f); }
+constexpr float kVarUnit = 5.6843418860808015e-14f;  // 2^-44
+
 // S8: where a tower (and its neutrals) is reported: the cell centre, or (K3) a point uniform inside the cell drawn from
 // Philox stream 4 of (seed, event, tower): word 0 -> eta or theta, word 1 -> phi
 template <bool FID>
@@ -219,6 +232,8 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
   const int wpe = sc.words_per_event;
   const long long p_al = prm.p_base & ~15ll;
   unsigned long long *uacc = (unsigned long long *)acc;
+  const size_t AS = (size_t)prm.acc_stride;  // 5, or 7 with the two variance sums of reading K5
+  const bool weighted = sc.eflow_weighted != 0;
   for (int k = tid; k < wpe; k += THREADS) bmap[k] = 0u;
   if (tid < 8) scal[tid] = 0;
   __syncthreads();
@@ -228,8 +243,8 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
     if (key != 0xffffu) {
       const int tower = (int)(key & 0x7fffu), hc = (int)(key >> 15);
       atomicOr(&bmap[tower >> 5], 1u << (tower & 31));
-      atomicAdd(uacc + 5 * (size_t)tower + hc, (unsigned long long)__float2ll_rn(__ldg(prm.E + i) * 4294967296.f));
-      if (DEBUG) atomicMin(acc + 5 * (size_t)tower + 4, i - pa - (1ll << 40));  // first depositing particle (biased: the slot starts at 0)
+      atomicAdd(uacc + AS * (size_t)tower + hc, (unsigned long long)__float2ll_rn(__ldg(prm.E + i) * 4294967296.f));
+      if (DEBUG) atomicMin(acc + AS * (size_t)tower + 4, i - pa - (1ll << 40));  // first depositing particle (biased: the slot starts at 0)
     }
   }
   // the event's tracks, segment by segment (warp per segment): energy into the tower's track sums; in the writing sweep
@@ -252,7 +267,9 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
           const unsigned key = (unsigned)__ldg(prm.key + q);
           const float Et = __ldg(prm.park_f[3] + g);
           if (key != 0xffffu)
-            atomicAdd(uacc + 5 * (size_t)(key & 0x7fffu) + 2 + (key >> 15), (unsigned long long)__float2ll_rn(Et * 4294967296.f));
+            atomicAdd(uacc + AS * (size_t)(key & 0x7fffu) + 2 + (key >> 15), (unsigned long long)__float2ll_rn(Et * 4294967296.f));
+          if (weighted && key != 0xffffu)
+            atomicAdd(uacc + AS * (size_t)(key & 0x7fffu) + 5 + (key >> 15), (unsigned long long)var_fix(__ldg(prm.park_sig + g)));
           if (write) {
             const int pid = __ldg(prm.park_pid + g);
             const float pt = __ldg(prm.park_f[0] + g), eta = __ldg(prm.park_f[1] + g), phi = __ldg(prm.park_f[2] + g);
@@ -290,7 +307,7 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
       const int b = __ffs(m) - 1;
       m &= m - 1;
       const int tower = 32 * w + b;
-      long long *a5 = acc + 5 * (size_t)tower;
+      long long *a5 = acc + AS * (size_t)tower;
       const long long a_em = __ldcg(a5), a_had = __ldcg(a5 + 1), t_em = __ldcg(a5 + 2), t_had = __ldcg(a5 + 3);
       const float Eem = (float)a_em * 2.3283064365386963e-10f, Ehad = (float)a_had * 2.3283064365386963e-10f;
       const float Tem = (float)t_em * 2.3283064365386963e-10f, Thad = (float)t_had * 2.3283064365386963e-10f;
@@ -298,10 +315,17 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
       rng_block(prm.rk, ev_index, (uint32_t)tower, 1u, rn);
       float em_s, had_s;
       bool k_em, k_had;
-      tower_components<true>(sc, tc, tower, Eem, Ehad, rn, em_s, had_s, k_em, k_had);
+      float var_em = 0.f, var_had = 0.f;
+      tower_components<true>(sc, tc, tower, Eem, Ehad, rn, em_s, had_s, k_em, k_had, weighted ? &var_em : nullptr, &var_had);
       const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
-      const float n_em = em_f - Tem, n_had = had_f - Thad;
+      float n_em = em_f - Tem, n_had = had_f - Thad;
       const bool f_ph = n_em > sc.thr_ecal, f_nh = n_had > sc.thr_hcal, f_tw = em_f + had_f > 0.f;
+      if (weighted) {
+        // reading K5: where the neutral is not emitted the stashed value is the factor for the component's tracks
+        if (!f_ph) n_em = eflow_weight(Tem, (float)__ldcg(a5 + 5) * kVarUnit, em_f, var_em);
+        if (!f_nh) n_had = eflow_weight(Thad, (float)__ldcg(a5 + 6) * kVarUnit, had_f, var_had);
+        __stcg(a5 + 5, 0ll), __stcg(a5 + 6, 0ll);
+      }
       c_tw += f_tw, c_ph += f_ph, c_nh += f_nh;
       if (DEBUG && write) {
         const long long g = pa + (__ldcg(a5 + 4) + (1ll << 40));
@@ -332,6 +356,39 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
   BigCounts out;
   out.trk = n_trk, out.tow = scal[1], out.ph = scal[2], out.nh = scal[3];
   if (!write) return out;
+  if (weighted) {
+    // reading K5: the EFlow entries of the event's tracks (written above, in track order from base_efl) take the factor of
+    // their tower component, stashed by sweep A where the component's neutral is not emitted
+    __threadfence();
+    const long long qa = pa - p_al, qb = pb - p_al;
+    const long long gs_lo = qa / PD_PSEG, gs_hi = pb > pa ? (qb - 1) / PD_PSEG : gs_lo - 1;
+    int done = 0;
+    for (long long gsi = gs_lo; gsi <= gs_hi; ++gsi) {
+      const uint32_t w = lane < PD_PSEG / 32 ? __ldg(prm.accmask + gsi * (PD_PSEG / 32) + lane) : 0u;
+      const int lo = (int)max(qa - gsi * PD_PSEG, 0ll), hi = (int)min(qb - gsi * PD_PSEG, (long long)PD_PSEG);
+      const int nlo = min(max(lo - 32 * lane, 0), 32), nhi = min(max(hi - 32 * lane, 0), 32);
+      const uint32_t mlo = nlo == 32 ? 0xffffffffu : (1u << nlo) - 1u, mhi = nhi == 32 ? 0xffffffffu : (1u << nhi) - 1u;
+      const int a = (int)__reduce_add_sync(0xffffffffu, (unsigned)__popc(w & mlo));
+      const int c = (int)__reduce_add_sync(0xffffffffu, (unsigned)__popc(w & mhi)) - a;
+      if ((int)((gsi - gs_lo) % W) == wid) {
+        for (int r = lane; r < c; r += 32) {
+          const long long g = gsi * PD_PSEG + a + r;
+          const long long q = gsi * PD_PSEG + (long long)__ldg(prm.park_idx + g);
+          const unsigned key = (unsigned)__ldg(prm.key + q);
+          if (key == 0xffffu) continue;
+          const long long *a5 = acc + AS * (size_t)(key & 0x7fffu);
+          const unsigned long long v1 = (unsigned long long)__ldcg(a5 + 1);
+          const int flags = (int)__ldcg(a5 + 2);
+          const float fw = (key & 0x8000u) ? ((flags & 4) ? 1.f : __uint_as_float((unsigned)(v1 >> 32))) : ((flags & 2) ? 1.f : __uint_as_float((unsigned)v1));
+          const unsigned at = (unsigned)base_efl + (unsigned)(done + r);
+          prm.efl_pt[at] *= fw, prm.efl_E[at] *= fw;
+        }
+      }
+      done += c;
+    }
+    __threadfence();
+    __syncthreads();
+  }
   // exclusive prefix of the per-word counts (one warp, a run of words per lane)
   if (wid == 0) {
     const int chunk = (wpe + 31) / 32, lo = min(wpe, lane * chunk), hi = min(wpe, lo + chunk);
@@ -354,7 +411,7 @@ __device__ __noinline__ BigCounts big_event(const PdParams &prm, long long ev_in
       const int b = __ffs(m) - 1;
       m &= m - 1;
       const int tower = 32 * w + b;
-      long long *a5 = acc + 5 * (size_t)tower;
+      long long *a5 = acc + AS * (size_t)tower;
       const unsigned long long v0 = (unsigned long long)__ldcg(a5), v1 = (unsigned long long)__ldcg(a5 + 1);
       const int flags = (int)__ldcg(a5 + 2);
       __stcg(a5, 0ll), __stcg(a5 + 1, 0ll), __stcg(a5 + 2, 0ll), __stcg(a5 + 3, 0ll), __stcg(a5 + 4, 0ll);
@@ -404,9 +461,9 @@ __device__ __noinline__ void big_tile(const PdParams &prm, unsigned char *smem, 
       uint32_t *bmap = s_res;
       unsigned *wcnt = s_head;
       int *scal = (int *)s_wtot;
-      long long *acc = prm.big_acc + (size_t)blockIdx.x * 5 * (size_t)sc.n_towers;
+      long long *acc = prm.big_acc + (size_t)blockIdx.x * (size_t)prm.acc_stride * (size_t)sc.n_towers;
       if (!acc_ready) {
-        for (size_t k = tid; k < 5 * (size_t)sc.n_towers; k += THREADS) __stcg(acc + k, 0ll);
+        for (size_t k = tid; k < (size_t)prm.acc_stride * (size_t)sc.n_towers; k += THREADS) __stcg(acc + k, 0ll);
         __threadfence();
         __syncthreads();
       }
@@ -487,6 +544,8 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
   unsigned *s_head = (unsigned *)(smem + L.head);  // per slot: last pusher, then head | tower id << 13 | flags
   float *s_stg = (float *)(smem + L.stg);   // per slot after pass W: Eem''  (neutral-hadron energy goes to s_res[head])
   unsigned char *s_ev = smem + L.ev;
+  float *s_Es = (float *)(smem + L.Es);     // K5: sigma_E of an accepted track, at its particle
+  const bool weighted = FID && sc.eflow_weighted;
   uint64_t *s_bar = (uint64_t *)(s_misc + 4);
   // kernel P parked the accepted tracks compacted within SEGMENTS of PD_PSEG particles; per segment that overlaps the
   // tile: rank of the tile's first track in the segment, number of the tile's tracks in it, their exclusive prefix
@@ -648,6 +707,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
           const long long g = gs + a + r;
           const int i = (int)(gs + (long long)__ldg(prm.park_idx + g) - q0);
           s_Et[i] = __ldg(prm.park_f[3] + g);
+          if (weighted) s_Es[i] = __ldg(prm.park_sig + g);
           s_res[i] |= RES_ACC;
           if (multi) atomicAdd(&s_ntrk[(int)s_ev[i]], 1);
         }
@@ -740,7 +800,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
         // S5: exact fixed-point sums (units of 2^-32 GeV, 64-bit integers) over the slot's list.  Integer
         // addition is associative, so the sums do not depend on the order in which the deposits arrived:
         // bitwise reproducible, and closer to the fp64 definition than a sequential fp32 sum.
-        long long a_em = 0, a_had = 0, t_em = 0, t_had = 0;
+        long long a_em = 0, a_had = 0, t_em = 0, t_had = 0, v_em = 0, v_had = 0;
         int first = h;
         for (int c = h;;) {
           const uint32_t rc = c == h ? rh : s_res[c];
@@ -748,6 +808,10 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
           const long long Tv = (rc & RES_ACC) ? __float2ll_rn(s_Et[c] * 4294967296.f) : 0ll;
           if (rc & RES_HCAL) a_had += Ev, t_had += Tv;
           else a_em += Ev, t_em += Tv;
+          if (weighted && (rc & RES_ACC)) {  // K5: the variance of the component's track sum (exact, like the sums)
+            if (rc & RES_HCAL) v_had += var_fix(s_Es[c]);
+            else v_em += var_fix(s_Es[c]);
+          }
           first = min(first, c);
           c = (int)(rc >> RES_LINK_SHIFT);
           if (c == (int)LINK_END) break;
@@ -759,10 +823,16 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
         float em_s, had_s;
         bool k_em, k_had;
         // reading A22: the threshold is applied twice, strictly, per component (K1 / K2: per-bin resolutions, significance)
-        tower_components<FID>(sc, tc, tower, Eem, Ehad, rn, em_s, had_s, k_em, k_had);
+        float var_em = 0.f, var_had = 0.f;
+        tower_components<FID>(sc, tc, tower, Eem, Ehad, rn, em_s, had_s, k_em, k_had, weighted ? &var_em : nullptr, &var_had);
         const float em_f = k_em ? em_s : 0.f, had_f = k_had ? had_s : 0.f;
-        const float n_em = em_f - Tem, n_had = had_f - Thad;
+        float n_em = em_f - Tem, n_had = had_f - Thad;
         f_ph = n_em > sc.thr_ecal, f_nh = n_had > sc.thr_hcal;
+        if (weighted) {
+          // reading K5: where the neutral is not emitted the staged value is the factor for the component's tracks instead
+          if (!f_ph) n_em = eflow_weight(Tem, (float)v_em * kVarUnit, em_f, var_em);
+          if (!f_nh) n_had = eflow_weight(Thad, (float)v_had * kVarUnit, had_f, var_had);
+        }
         f_tw = em_f + had_f > 0.f;
         if (multi) {
           if (f_tw) atomicAdd(&s_ntow[e], 1);
@@ -906,12 +976,36 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
         const int e = multi ? (int)s_ev[il] : 0;
         const unsigned at = (unsigned)base_efl + (unsigned)(sp + r + s_nph[e] + s_nnh[e]);
         const int apid = pid < 0 ? -pid : pid;
+        float fw = 1.f;
+        if (weighted) {
+          // reading K5: the factor of the track's tower component (staged by pass W where its neutral is not emitted); the
+          // slot of the tower through the bitmap ranks, as in pass B
+          const unsigned key = (unsigned)__ldg(prm.key + (q0 + il));
+          if (key != 0xffffu) {
+            const int id = (int)(key & 0x7fffu);
+            int gi;
+            uint4 bits;
+            if (!sparse) {
+              gi = e * gpe + (id >> 7);
+              bits = ((const uint4 *)s_bitmap)[gi];
+            } else {
+              const int wq = e * l2w + (id >> 12);
+              gi = (int)s_l2p[wq] + __popc(s_bitmap[wq] & ((1u << ((id >> 7) & 31)) - 1u));
+              bits = s_pool[gi];
+            }
+            const int slot = (int)s_gp[gi] + popc_below(bits, id & 127);
+            const unsigned hv = s_head[slot];
+            const int hh = (int)(hv & LINK_END);
+            if (key & 0x8000u) fw = (hv & SLOT_NH) ? 1.f : __uint_as_float(s_res[hh]);
+            else fw = (hv & SLOT_PH) ? 1.f : s_Et[hh];
+          }
+        }
         prm.efl_cls[at] = (signed char)(apid == 11 ? PD_CLS_ELECTRON : (apid == 13 ? PD_CLS_MUON : PD_CLS_CHHAD));
         prm.efl_src[at] = (int)(p0 + il);
-        prm.efl_pt[at] = __ldg(prm.park_f[0] + g);
+        prm.efl_pt[at] = __ldg(prm.park_f[0] + g) * fw;
         prm.efl_eta[at] = __ldg(prm.park_f[1] + g);
         prm.efl_phi[at] = __ldg(prm.park_f[2] + g);
-        prm.efl_E[at] = __ldg(prm.park_f[3] + g);
+        prm.efl_E[at] = __ldg(prm.park_f[3] + g) * fw;
       }
     }
     for (int it = 0; it < n_it; ++it) {
@@ -992,8 +1086,8 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, int til
   const size_t budget2 = (228 * 1024 - 2 * 1024) / 2, budget1 = 227 * 1024;
   int sparse = 0;
   auto cap_for = [&](int G, size_t budget) {
-    const size_t fixed = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, G, 0, sparse, sc.res_per_bin, sc.smear_center).total;
-    const size_t per = pdk::T_BYTES_PER_PARTICLE + (G > 1 ? 1 : 0) + (sparse ? 18 : 0);
+    const size_t fixed = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, G, 0, sparse, sc.res_per_bin, sc.smear_center, sc.eflow_weighted).total;
+    const size_t per = pdk::T_BYTES_PER_PARTICLE + (G > 1 ? 1 : 0) + (sparse ? 18 : 0) + (sc.eflow_weighted ? 4 : 0);
     long cap = budget > fixed + 7 * 16 ? long((budget - fixed - 7 * 16) / per) : 0;
     cap &= ~3L;
     return int(cap > pdk::C_MAX ? pdk::C_MAX : cap);
@@ -1039,7 +1133,7 @@ int pd_plan(const pd_card *c, long long n_events, long long n_particles, int til
     const long sms = query_device() == PD_OK ? g_num_sms : 256;
     plan->max_ctas = int(sms * (plan->threads == 1024 ? 1 : 2));
   }
-  plan->lay = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse, sc.res_per_bin, sc.smear_center);
+  plan->lay = pdk::make_layout(sc.n_bins, sc.n_towers, sc.words_per_event, g, plan->capacity, sparse, sc.res_per_bin, sc.smear_center, sc.eflow_weighted);
   plan->smem_bytes = plan->lay.total;
   return PD_OK;
 }
@@ -1065,7 +1159,7 @@ static int launch_variant2(const PdParams &prm, const PdLaunchPlan &plan, cudaSt
 // the variant with the higher-fidelity card options (K1-K3) compiled in only for the cards that use them
 template <int THREADS, bool DEBUG, bool SPARSE>
 static int launch_variant(const PdParams &prm, const PdLaunchPlan &plan, cudaStream_t stream) {
-  const bool fid = prm.sc.res_per_bin || prm.sc.smear_center || prm.sc.nsig2_ecal > 0.f || prm.sc.nsig2_hcal > 0.f;
+  const bool fid = prm.sc.res_per_bin || prm.sc.smear_center || prm.sc.nsig2_ecal > 0.f || prm.sc.nsig2_hcal > 0.f || prm.sc.eflow_weighted;
   return fid ? launch_variant2<THREADS, DEBUG, SPARSE, true>(prm, plan, stream) : launch_variant2<THREADS, DEBUG, SPARSE, false>(prm, plan, stream);
 }
 

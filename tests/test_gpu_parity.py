@@ -308,8 +308,8 @@ def test_forced_kernel_variants_in_a_subprocess(tmp_path):
 
 @pytest.mark.parametrize("base,cfg,ne", [("cms_like", 0, 600), ("cms_like", 1, 200), ("aleph_like", 4, 1500)])
 def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
-    """SURVEY 8f NEXT-3, readings K1-K4: eta-dependent ECAL / HCAL / track resolutions, the significance cut
-    and tower positions smeared inside the cell -- one at a time and all together, on an eta grid and on a theta grid;
+    """SURVEY 8f NEXT-3, readings K1-K5: eta-dependent ECAL / HCAL / track resolutions, the significance cut,
+    tower positions smeared inside the cell and the weighted EFlow -- one at a time and all together, on an eta grid and on a theta grid;
     and an event too large for the chip (the big-tile path has its own copy of the tower code)."""
     import cards
     from gpu_util import run_gpu
@@ -326,8 +326,9 @@ def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
         "significance": dict(ecal_nsigma=2.0, hcal_nsigma=1.5),
         "smeared_centres": dict(smear_tower_center=1),
         "track_rows": dict(track_res_eta=trk_rows),
+        "weighted_eflow": dict(eflow_weighted=1, track_res=(0.03, 5e-4)),
         "all": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows, ecal_nsigma=1.0, hcal_nsigma=1.2, smear_tower_center=1,
-                    track_res_eta=trk_rows),
+                    track_res_eta=trk_rows, eflow_weighted=1),
     }
     ev = wl.generate(cfg, ne)
     if cfg == 0:
@@ -341,7 +342,7 @@ def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
         gpu = run_gpu(path, ev, 29)
         assert gpu["status_word"] == 0, name
         rep = _check(compare(path, ev, 29, gpu))
-        changed = any(gpu[k].shape != plain[k].shape or gpu[k].tobytes() != plain[k].tobytes() for k in ("tow_E", "tow_eta", "efl_E", "trk_pt"))
+        changed = any(gpu[k].shape != plain[k].shape or gpu[k].tobytes() != plain[k].tobytes() for k in ("tow_E", "tow_eta", "efl_E", "trk_pt", "efl_pt"))
         assert changed, name  # the card option really is in use
         print(base, name, {k: rep[k] for k in ("flagged_particles", "overridden_particles", "flagged_towers", "overridden_towers", "neutral_outside_plain_tol")})
 
