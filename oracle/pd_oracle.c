@@ -28,7 +28,16 @@ struct pdo_card {
   double *edges;   /* [n_bins+1], ascending */
   int32_t *nphi;   /* [n_bins]              */
   int32_t *offset; /* [n_bins] exclusive prefix sum of nphi */
-  int n_towers;
+  int n_towers;    /* of this grid (for a dual card: of the ECAL grid + of the HCAL grid, see below) */
+  /* reading K6: a second grid for the HCAL (hcal_edges / hcal_nphi).  Tower ids: the ECAL grid's towers first, then the HCAL
+   * grid's; a particle's tower is looked up in the grid of the section it deposits in.  The two grids are kept as cards of
+   * their own (shallow copies that share everything but the grid), so that every grid function below works on either. */
+  int dual;
+  struct pdo_card *view[2]; /* [0] ECAL grid, [1] HCAL grid (dual cards only) */
+  int32_t hcal_base;        /* id of the HCAL grid's first tower */
+  int h_n_bins;
+  double *h_edges;
+  int32_t *h_nphi, *h_offset;
   int n_eff;
   double eff[PDO_MAX_EFF_ROWS][5]; /* pt_lo, pt_hi, aeta_lo, aeta_hi, eps   (reading A8)      */
   int eff_species[PDO_MAX_EFF_ROWS]; /* 0: every charged particle, 1 electrons, 2 muons, 3 charged hadrons (reading J1) */
@@ -82,6 +91,12 @@ static void card_finish(pdo_card *c) {
     acc += c->nphi[i];
   }
   c->n_towers = acc;
+  if (c->h_edges) {
+    int hacc = 0;
+    for (i = 0; i <= c->h_n_bins; ++i) c->h_edges[i] = f32(c->h_edges[i]);
+    for (i = 0; i < c->h_n_bins; ++i) c->h_offset[i] = hacc, hacc += c->h_nphi[i];
+    c->dual = 1, c->hcal_base = acc, c->n_towers = acc + hacc;
+  }
   c->bz = f32(c->bz);
   c->radius = f32(c->radius);
   c->half_length = f32(c->half_length);
@@ -115,6 +130,18 @@ static void card_finish(pdo_card *c) {
   }
   c->nsig_ecal = f32(c->nsig_ecal);
   c->nsig_hcal = f32(c->nsig_hcal);
+  if (c->dual) {
+    /* the two grids as cards of their own: everything shared, only the grid (and its tower count) differs */
+    int g;
+    for (g = 0; g < 2; ++g) {
+      pdo_card *v = (pdo_card *)malloc(sizeof(pdo_card));
+      memcpy(v, c, sizeof(pdo_card));
+      v->dual = 0, v->view[0] = v->view[1] = NULL;
+      if (g == 1) v->n_bins = c->h_n_bins, v->edges = c->h_edges, v->nphi = c->h_nphi, v->offset = c->h_offset;
+      v->n_towers = g == 0 ? c->hcal_base : c->n_towers - c->hcal_base;
+      c->view[g] = v;
+    }
+  }
 }
 
 /* the three efficiency rows of BASELINE.json configs[0] in reading A8 */
@@ -194,8 +221,8 @@ static int card_from_file(pdo_card *c, const char *path) {
   FILE *f = fopen(path, "r");
   char *line = NULL;
   size_t cap = 1 << 16;
-  double *edges = NULL, *nphi = NULL;
-  int n_edges = 0, n_nphi = 0, cap_e = 0, cap_n = 0, ok = 1, i;
+  double *edges = NULL, *nphi = NULL, *hedges = NULL, *hnphi = NULL;
+  int n_edges = 0, n_nphi = 0, cap_e = 0, cap_n = 0, n_he = 0, n_hn = 0, cap_he = 0, cap_hn = 0, ok = 1, i;
   if (!f) return -1;
   line = (char *)malloc(cap);
   card_default_eff(c);
@@ -225,10 +252,11 @@ static int card_from_file(pdo_card *c, const char *path) {
       c->grid_coord = !strncmp(val, "theta", 5) ? 1 : 0;
       continue;
     }
-    if (!strcmp(key, "edges") || !strcmp(key, "nphi")) {
-      double **arr = !strcmp(key, "edges") ? &edges : &nphi;
-      int *n = !strcmp(key, "edges") ? &n_edges : &n_nphi;
-      int *cp = !strcmp(key, "edges") ? &cap_e : &cap_n;
+    if (!strcmp(key, "edges") || !strcmp(key, "nphi") || !strcmp(key, "hcal_edges") || !strcmp(key, "hcal_nphi")) {
+      const int h = !strncmp(key, "hcal_", 5), e = !strcmp(key + (h ? 5 : 0), "edges");
+      double **arr = h ? (e ? &hedges : &hnphi) : (e ? &edges : &nphi);
+      int *n = h ? (e ? &n_he : &n_hn) : (e ? &n_edges : &n_nphi);
+      int *cp = h ? (e ? &cap_he : &cap_hn) : (e ? &cap_e : &cap_n);
       for (;;) {
         double x = strtod(val, &end);
         if (end == val) break;
@@ -290,8 +318,27 @@ static int card_from_file(pdo_card *c, const char *path) {
     for (i = 1; i < n_edges; ++i)
       if (!((float)edges[i] > (float)edges[i - 1])) ok = 0;
   }
+  if (ok && (n_he || n_hn)) {
+    /* reading K6: the HCAL's own grid */
+    if (n_he < 2 || n_hn != n_he - 1) ok = 0;
+    if (ok) {
+      c->h_n_bins = n_he - 1;
+      c->h_edges = (double *)calloc((size_t)n_he, sizeof(double));
+      c->h_nphi = (int32_t *)calloc((size_t)n_hn, sizeof(int32_t));
+      c->h_offset = (int32_t *)calloc((size_t)n_hn, sizeof(int32_t));
+      for (i = 0; i < n_he; ++i) c->h_edges[i] = hedges[i];
+      for (i = 0; i < n_hn; ++i) {
+        c->h_nphi[i] = (int32_t)hnphi[i];
+        if (c->h_nphi[i] < 1) ok = 0;
+      }
+      for (i = 1; i < n_he; ++i)
+        if (!((float)hedges[i] > (float)hedges[i - 1])) ok = 0;
+    }
+  }
   free(edges);
   free(nphi);
+  free(hedges);
+  free(hnphi);
   return ok ? 0 : -1;
 }
 
@@ -320,6 +367,8 @@ void pdo_free_card(pdo_card *c) {
   free(c->edges);
   free(c->nphi);
   free(c->offset);
+  free(c->h_edges), free(c->h_nphi), free(c->h_offset);
+  free(c->view[0]), free(c->view[1]);
   free(c);
 }
 
@@ -344,6 +393,16 @@ int pdo_card_grid(const pdo_card *c, double *edges, int32_t *nphi, int32_t *offs
     if (offset) offset[i] = c->offset[i];
   }
   return PDO_OK;
+}
+
+int pdo_card_hcal_grid(const pdo_card *c, double *edges, int32_t *nphi, int32_t *base) {
+  int i;
+  if (!c) return PDO_EINVAL;
+  if (!c->dual) return 0;
+  for (i = 0; i <= c->h_n_bins && edges; ++i) edges[i] = c->h_edges[i];
+  for (i = 0; i < c->h_n_bins && nphi; ++i) nphi[i] = c->h_nphi[i];
+  if (base) *base = c->hcal_base;
+  return c->h_n_bins;
 }
 
 /* ------------------------------------------------------------------ O0: RNG ---------------- */
@@ -466,6 +525,27 @@ int32_t pdo_tower_index(const pdo_card *c, double coord, double phi_pos) {
   return c->offset[i] + phi_bin(c->nphi[i], phi_pos);
 }
 
+/* reading K6: the grid a deposit of section det (0 ECAL, 1 HCAL) is looked up in, and the id of its first tower */
+static const pdo_card *grid_of(const pdo_card *c, int det, int32_t *base) {
+  *base = (c->dual && det) ? c->hcal_base : 0;
+  return c->dual ? c->view[det ? 1 : 0] : c;
+}
+int32_t pdo_tower_index_det(const pdo_card *c, int det, double coord, double phi_pos) {
+  int32_t base, t;
+  const pdo_card *g = grid_of(c, det, &base);
+  t = pdo_tower_index(g, coord, phi_pos);
+  return t < 0 ? t : base + t;
+}
+/* the grid that holds tower id `tower` of the card, and the id inside it */
+static const pdo_card *grid_of_tower(const pdo_card *c, int32_t *tower) {
+  if (!c->dual) return c;
+  if (*tower >= c->hcal_base) {
+    *tower -= c->hcal_base;
+    return c->view[1];
+  }
+  return c->view[0];
+}
+
 /* is `tower` an outcome the position (coord, phi) may legitimately take within the tolerance? */
 static int tower_allowed(const pdo_card *c, double coord, double phi_pos, int32_t tower) {
   int i, j, n;
@@ -525,6 +605,7 @@ int pdo_tower_centre(const pdo_card *c, int32_t tower, double *eta_c, double *ph
   int i, j;
   double mid;
   if (!c || tower < 0 || tower >= c->n_towers) return PDO_EINVAL;
+  if (c->dual) c = grid_of_tower(c, &tower);
   for (i = c->n_bins - 1; i > 0; --i)
     if (c->offset[i] <= tower) break;
   j = tower - c->offset[i];
@@ -766,10 +847,11 @@ int pdo_tower_position(const pdo_card *c, uint64_t seed, int64_t event, int32_t 
   double x;
   if (!c || tower < 0 || tower >= c->n_towers) return PDO_EINVAL;
   if (!c->smear_center) return pdo_tower_centre(c, tower, eta, phi);
+  pdo_rng_block(seed, event, (uint32_t)tower, 4u, r); /* object = the card's tower id */
+  if (c->dual) c = grid_of_tower(c, &tower);           /* reading K6: the cell in the tower's own grid */
   for (i = c->n_bins - 1; i > 0; --i)
     if (c->offset[i] <= tower) break;
   j = tower - c->offset[i];
-  pdo_rng_block(seed, event, (uint32_t)tower, 4u, r);
   x = c->edges[i] + pdo_uniform(r[0]) * (c->edges[i + 1] - c->edges[i]);
   if (eta) *eta = c->grid_coord ? -log(tan(0.5 * x)) : x;
   if (phi) *phi = -PDO_PI + ((double)j + pdo_uniform(r[1])) * (PDO_TWO_PI / (double)c->nphi[i]);
@@ -897,11 +979,20 @@ int pdo_simulate(const pdo_card *c, const pdo_events *ev, uint64_t seed, int64_t
           }
         }
         /* O4 deposit: tower of the hit position; sums in particle order (A17, A19) */
-        tower = pdo_tower_index(c, h.coord, h.phi_pos);
-        near |= tower_near(c, h.coord, h.phi_pos);
-        if (ov && ov->tower && ov->tower[i] != -2 && ov->tower[i] != tower) {
-          if (tower_allowed(c, h.coord, h.phi_pos, ov->tower[i])) tower = ov->tower[i];
-          else ++rejected;
+        {
+          /* reading K6: a card with a grid of its own for the HCAL: the tower is looked up in the grid of the section the
+           * particle deposits in (electrons and photons: ECAL; everything else, also what deposits nothing: HCAL) */
+          int32_t base;
+          const pdo_card *g = grid_of(c, fe != 0.0 ? 0 : 1, &base);
+          tower = pdo_tower_index(g, h.coord, h.phi_pos);
+          if (tower >= 0) tower += base;
+          near |= tower_near(g, h.coord, h.phi_pos);
+          if (ov && ov->tower && ov->tower[i] != -2 && ov->tower[i] != tower) {
+            const int32_t want = ov->tower[i];
+            const int in_grid = want < 0 || (want >= base && want - base < g->n_towers);
+            if (in_grid && tower_allowed(g, h.coord, h.phi_pos, want < 0 ? want : want - base)) tower = want;
+            else ++rejected;
+          }
         }
         if (tower >= 0 && (fe != 0.0 || fh != 0.0)) {
           if (!touched[tower]) touched[tower] = 1, list[n_list++] = tower;

@@ -278,6 +278,12 @@ int pdo_propagate(const pdo_card *card, int charge, double px, double py, double
                   double *eta_pos, double *phi_pos);
 /* tower id (or -1) of a position given as (eta_pos or theta_pos per the card's grid, phi_pos) */
 int32_t pdo_tower_index(const pdo_card *card, double coord, double phi_pos);
+/* reading K6 (card keys hcal_edges / hcal_nphi: a grid of its own for the HCAL; tower ids: the ECAL grid's towers, then the
+ * HCAL grid's): the tower of a hit for a deposit in section det (0 ECAL, 1 HCAL); pdo_tower_index is det = 0.  On a card with
+ * one grid det does not matter.  pdo_card_hcal_grid: bins of the HCAL grid (0: the card has one grid) and, if the pointers
+ * are not NULL, its edges [n+1] and nphi [n]; *base receives the id of its first tower. */
+int32_t pdo_tower_index_det(const pdo_card *card, int det, double coord, double phi_pos);
+int pdo_card_hcal_grid(const pdo_card *card, double *edges, int32_t *nphi, int32_t *base);
 /* efficiency of O3 for true (pt, eta_mom, |cos theta|); *row receives the row index or -1 */
 double pdo_efficiency(const pdo_card *card, double pt, double eta_mom, double abs_costheta,
                       int *row);

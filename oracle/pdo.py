@@ -164,8 +164,23 @@ class Card:
             raise OracleError(PDO_EINVAL)
         return e.value, p.value
 
-    def tower_index(self, coord: float, phi: float) -> int:
-        return int(lib().pdo_tower_index(self._h, float(coord), float(phi)))
+    def tower_index(self, coord: float, phi: float, det: int = 0) -> int:
+        """tower of a hit; det: section of the deposit (0 ECAL, 1 HCAL), which matters on a card with two grids (reading K6)"""
+        L = lib()
+        L.pdo_tower_index_det.argtypes = [_p, C.c_int, C.c_double, C.c_double]
+        L.pdo_tower_index_det.restype = C.c_int32
+        return int(L.pdo_tower_index_det(self._h, int(det), float(coord), float(phi)))
+
+    def hcal_grid(self):
+        """(edges, nphi, base) of the HCAL's own grid, or None for a card with one grid (reading K6)"""
+        L = lib()
+        L.pdo_card_hcal_grid.argtypes = [_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        n = int(L.pdo_card_hcal_grid(self._h, None, None, None))
+        if n <= 0:
+            return None
+        e, p, b = np.zeros(n + 1), np.zeros(n, dtype=np.int32), C.c_int32(0)
+        L.pdo_card_hcal_grid(self._h, e.ctypes.data_as(C.c_void_p), p.ctypes.data_as(C.c_void_p), C.cast(C.byref(b), C.c_void_p))
+        return e, p, int(b.value)
 
     def efficiency(self, pt, eta_mom, abs_costheta=0.0, species=None):
         """(eps, row) of the card's table; species: None (a charged hadron), 1 electron, 2 muon, 3 charged hadron."""

@@ -22,7 +22,7 @@ DEFAULT_EFF = [(1.0, "inf", 0.0, 1.5, 0.97), (1.0, "inf", 1.5, 2.5, 0.85), (0.1,
 def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kappa=0.299792458,
               eff=DEFAULT_EFF, abs_costheta_max=None, track_res=(0.01, 1.5e-4), ecal=(0.007, 0.07, 0.35),
               hcal=(0.05, 1.5, 0.0), ecal_thr=0.5, hcal_thr=1.0, name="custom", track_res_species=None,
-              ecal_res_eta=(), hcal_res_eta=(), ecal_nsigma=None, hcal_nsigma=None, smear_tower_center=None, track_res_eta=(), eflow_weighted=None):
+              ecal_res_eta=(), hcal_res_eta=(), ecal_nsigma=None, hcal_nsigma=None, smear_tower_center=None, track_res_eta=(), eflow_weighted=None, hcal_edges=None, hcal_nphi=None):
     lines = ["name = %s" % name, "bz = %r" % bz, "radius = %r" % radius, "half_length = %r" % half_length,
              "kappa = %r" % kappa, "grid = %s" % grid]
     edges = [float(x) for x in edges]
@@ -31,6 +31,13 @@ def card_text(edges, nphi, grid="eta", bz=3.8, radius=1.29, half_length=3.0, kap
     nphi = [int(x) for x in nphi]
     for i in range(0, len(nphi), 16):
         lines.append("nphi = " + " ".join(str(x) for x in nphi[i:i + 16]))
+    if hcal_edges is not None:  # reading K6: the HCAL's own grid
+        he = [float(x) for x in hcal_edges]
+        for i in range(0, len(he), 8):
+            lines.append("hcal_edges = " + " ".join(repr(x) for x in he[i:i + 8]))
+        hn = [int(x) for x in hcal_nphi]
+        for i in range(0, len(hn), 16):
+            lines.append("hcal_nphi = " + " ".join(str(x) for x in hn[i:i + 16]))
     for row in eff:
         lines.append("eff = " + " ".join(str(x) for x in row))
     if abs_costheta_max is not None:

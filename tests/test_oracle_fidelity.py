@@ -278,3 +278,73 @@ def test_weighted_eflow_limits_and_closed_forms(tmp_path):
     assert (t[:, 0] == t[:, 1]).all() and (t[:, 0] != t[:, 3]).all()      # the two pions of 20 and 35 GeV hit one tower
     assert np.allclose(f[:, 0], f[:, 1], rtol=1e-12) and not np.allclose(f[:, 0], f[:, 3], rtol=1e-3)
     assert np.all(f[:, 2] == 1.0) and np.all(np.abs(f[:, 0] - 1.0) > 1e-6) and np.all(np.abs(f[:, 3] - 1.0) > 1e-6)
+
+
+def test_separate_ecal_and_hcal_grids(tmp_path):
+    """Reading K6: a grid of its own for the HCAL (card keys hcal_edges / hcal_nphi).  Tower ids: the ECAL grid's towers first,
+    then the HCAL grid's; a deposit is looked up in the grid of its section.  Pinned on closed-form tower ids of uniform grids
+    and on the one-grid oracle run with a perfect detector."""
+    a = pdo.Card("atlas_like")           # ECAL: 64 eta bins of 0.1 over |eta| < 3.2, 64 phi bins: 4,096 towers
+    he = [np.float32(-3.2 + 0.2 * k) if k < 32 else np.float32(3.2) for k in range(33)]
+    he = [-float(np.float32(0.2 * k)) for k in range(16, 0, -1)] + [float(np.float32(0.2 * k)) for k in range(17)]   # 32 bins of 0.2
+    hn = [32] * 32
+    perfect = dict(eff=[(0.1, "inf", 0.0, 2.5, 1.0)], track_res=(0.0, 0.0), ecal=(0.0, 0.0, 0.0), hcal=(0.0, 0.0, 0.0))
+    dual = pdo.Card(cards.variant(tmp_path / "dual.card", a.edges, a.nphi, base="atlas_like", hcal_edges=he, hcal_nphi=hn, **perfect))
+    one = pdo.Card(cards.variant(tmp_path / "one.card", a.edges, a.nphi, base="atlas_like", **perfect))
+    assert (dual.n_towers, one.n_towers) == (4096 + 1024, 4096)
+    e, n, base = dual.hcal_grid()
+    assert base == 4096 and len(n) == 32 and np.allclose(e, he) and one.hcal_grid() is None
+    # closed-form ids of the two uniform grids (hits of neutral particles from the origin are at their own eta, phi)
+    id_e = lambda eta, phi: 64 * int(math.floor((eta + 3.2) / 0.1)) + int(math.floor((phi + math.pi) / (2 * math.pi / 64)))   # noqa: E731
+    id_h = lambda eta, phi: 4096 + 32 * int(math.floor((eta + 3.2) / 0.2)) + int(math.floor((phi + math.pi) / (2 * math.pi / 32)))  # noqa: E731
+    pts = [(0.05, 0.3), (-1.234, -2.5), (2.17, 1.0), (-3.15, 3.0), (1.05, -0.02), (0.31, 2.2)]
+    for eta, phi in pts:
+        assert dual.tower_index(eta, phi, det=0) == id_e(eta, phi) == one.tower_index(eta, phi, det=1)   # one grid: det does not matter
+        assert dual.tower_index(eta, phi, det=1) == id_h(eta, phi)
+        ec, pc = dual.tower_centre(id_h(eta, phi))
+        assert abs(ec - (-3.2 + 0.2 * (math.floor((eta + 3.2) / 0.2) + 0.5))) < 1e-6
+        assert abs(pc - (-math.pi + (math.floor((phi + math.pi) / (2 * math.pi / 32)) + 0.5) * 2 * math.pi / 32)) < 1e-12
+    assert dual.tower_index(3.3, 0.0, det=1) == -1 and dual.tower_index(-3.21, 0.0, det=0) == -1
+    # through the chain: a photon, a K0L and a muon in each of the directions above
+    ev = wl.from_lists([[p for eta, phi in pts for p in (P(22, 0, 10.0, eta, phi, 0.0), P(130, 0, 12.0, eta, phi, 0.497611), P(13, 1, 500.0, eta, phi, 0.1056584))]])
+    o = pdo.simulate(dual, ev, 3)
+    want_e, want_h = sorted(id_e(*p) for p in pts), sorted(id_h(*p) for p in pts)
+    assert list(o["tow_tower"]) == want_e + want_h                       # ascending ids: the ECAL grid's towers first
+    k = len(pts)
+    assert np.all(o["tow_Ehad"][:k] == 0) and np.all(o["tow_Eem"][:k] > 0) and np.all(o["tow_Eem"][k:] == 0) and np.all(o["tow_Ehad"][k:] > 0)
+    assert list(o["dbg_tower"][0::3]) == [id_e(*p) for p in pts] and list(o["dbg_tower"][1::3]) == [id_h(*p) for p in pts]
+    mu = o["dbg_tower"][2::3]                                            # 500 GeV muons barely bend: the K0L's HCAL tower or a neighbour; no deposit
+    assert np.all(mu >= 4096) and len(o["tow_tower"]) == 2 * k
+    assert list(o["efl_src"][o["efl_cls"] == 4]) == want_e and list(o["efl_src"][o["efl_cls"] == 3]) == want_h
+    # a perfect detector on realistic events: per event the same energy in each section as with one grid, the HCAL deposits
+    # re-binned: summing the one-grid card's HCAL energies over the coarse cells gives the dual card's HCAL towers
+    evs = wl.generate(3, 40)
+    od, oo = pdo.simulate(dual, evs, 9), pdo.simulate(one, evs, 9)
+    assert od["trk_pt"].tobytes() == oo["trk_pt"].tobytes()
+    for ev_i in range(40):
+        d = slice(int(od["tow_offsets"][ev_i]), int(od["tow_offsets"][ev_i + 1]))
+        s = slice(int(oo["tow_offsets"][ev_i]), int(oo["tow_offsets"][ev_i + 1]))
+        td, ts = od["tow_tower"][d], oo["tow_tower"][s]
+        em_d = {int(t): float(x) for t, x in zip(td, od["tow_Eem"][d]) if t < 4096}
+        em_s = {int(t): float(x) for t, x in zip(ts, oo["tow_Eem"][s]) if x > 0}
+        assert em_d == em_s
+        coarse = {}
+        for t, x in zip(ts, oo["tow_Ehad"][s]):
+            if x > 0:
+                ie, ip = divmod(int(t), 64)
+                key = 4096 + 32 * (ie // 2) + ip // 2
+                coarse[key] = coarse.get(key, 0.0) + float(x)
+        had_d = {int(t): float(x) for t, x in zip(td, od["tow_Ehad"][d]) if t >= 4096}
+        # (the one-grid card applies the 1 GeV threshold per fine tower, the dual card per coarse tower: compare what passes both)
+        for key, x in had_d.items():
+            assert key in coarse and coarse[key] <= x * (1 + 1e-12) + 1e-9
+        assert set(coarse) <= set(had_d)
+    # K3 on a dual card: the reported position of an HCAL tower lies in its own (coarse) cell
+    sm = pdo.Card(cards.variant(tmp_path / "dual_sm.card", a.edges, a.nphi, base="atlas_like", hcal_edges=he, hcal_nphi=hn, smear_tower_center=1, **perfect))
+    os_ = pdo.simulate(sm, evs, 9)
+    hsel = os_["tow_tower"] >= 4096
+    loc = os_["tow_tower"][hsel] - 4096
+    u1 = (os_["tow_eta"][hsel] + 3.2) / 0.2 - loc // 32
+    u2 = (os_["tow_phi"][hsel] + math.pi) / (2 * math.pi / 32) - loc % 32
+    assert hsel.sum() > 300 and (u1 >= -1e-6).all() and (u1 < 1 + 1e-6).all() and (u2 >= -1e-9).all() and (u2 < 1 + 1e-9).all()
+    assert scipy.stats.kstest(np.clip(u1, 0, 1), "uniform").pvalue > 1e-4
