@@ -105,7 +105,7 @@ void pd_free_card(pd_card *card) {
 int pd_card_info(const pd_card *card, pd_card_info_t *out) {
   if (!card || !out) return PD_EINVAL;
   out->n_towers = card->sc.n_towers;
-  out->n_eta_bins = card->sc.n_bins;
+  out->n_eta_bins = card->sc.g_nb[0];  // of the (ECAL) grid; a card with a second grid for the HCAL has more bins in all
   out->grid_coord = card->sc.grid_theta;
   out->bz = card->bz;
   out->radius = card->sc.R;
@@ -378,7 +378,7 @@ int pd_card_to_device(const pd_card *c, const PdCardTables **tab) {
   const int slot = c->n_dev;
   const size_t nb = (size_t)c->sc.n_bins;
   const size_t lut_words = (c->lut.size() + 1) / 2;
-  const size_t words = (nb + 1) + nb + (nb + 1) + 5 * nb + lut_words + (nb + 1) + 6 * nb;
+  const size_t words = c->tb.size() + nb + (nb + 1) + 5 * nb + lut_words + 2 * nb + 6 * nb;
   std::vector<uint32_t> blob(words);
   size_t o = 0;
   auto put = [&](const void *src, size_t n) {
@@ -387,13 +387,13 @@ int pd_card_to_device(const pd_card *c, const PdCardTables **tab) {
     o += n;
     return at;
   };
-  const size_t o_tb = put(c->tb.data(), nb + 1), o_nphi = put(c->nphi.data(), nb), o_off = put(c->offset.data(), nb + 1);
+  const size_t o_tb = put(c->tb.data(), c->tb.size()), o_nphi = put(c->nphi.data(), nb), o_off = put(c->offset.data(), nb + 1);
   const size_t o_iw = put(c->inv_w.data(), nb), o_half = put(c->half.data(), nb), o_w = put(c->w.data(), nb);
   const size_t o_eta = put(c->eta_c.data(), nb), o_ic = put(c->inv_cosh.data(), nb);
   const size_t o_lut = o;
   std::memcpy(blob.data() + o, c->lut.data(), 2 * c->lut.size());
   o += lut_words;
-  const size_t o_edge = put(c->edges.data(), nb + 1), o_res2 = put(c->res2.data(), 6 * nb);
+  const size_t o_edge = put(c->edges.data(), 2 * nb), o_res2 = put(c->res2.data(), 6 * nb);
   void *d = nullptr;
   PD_CUDA(cudaMalloc(&d, 4 * words));
   cudaError_t e = cudaMemcpy(d, blob.data(), 4 * words, cudaMemcpyHostToDevice);

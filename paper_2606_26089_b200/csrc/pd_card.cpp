@@ -39,6 +39,8 @@ struct RawCard {
   bool smear_center = false;                              // reading K3
   std::vector<std::array<double, 5>> trk_eta;             // reading K4: aeta_lo, aeta_hi, a, b, species
   bool eflow_weighted = false;                            // reading K5
+  std::vector<double> hcal_edges;                         // reading K6: the HCAL's own grid
+  std::vector<long> hcal_nphi;
 };
 
 constexpr double kPi = 3.14159265358979323846;
@@ -128,6 +130,8 @@ bool from_file(RawCard &r, const char *path) {
     std::vector<double> v;
     if (!parse_numbers(val, v)) return false;
     if (key == "edges") r.edges.insert(r.edges.end(), v.begin(), v.end());
+    else if (key == "hcal_edges") r.hcal_edges.insert(r.hcal_edges.end(), v.begin(), v.end());
+    else if (key == "hcal_nphi") for (double x : v) r.hcal_nphi.push_back(long(x));
     else if (key == "nphi") for (double x : v) r.nphi.push_back(long(x));
     else if (key == "bz" && v.size() == 1) r.bz = v[0];
     else if (key == "radius" && v.size() == 1) r.radius = v[0];
@@ -182,6 +186,18 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     if (n < 1) return PD_ECARD;
     total += n;
   }
+  // reading K6: a grid of its own for the HCAL
+  const bool dual = !r.hcal_edges.empty() || !r.hcal_nphi.empty();
+  const size_t nbh = dual && r.hcal_edges.size() >= 2 ? r.hcal_edges.size() - 1 : 0;
+  if (dual) {
+    if (nbh < 1 || nb + nbh > size_t(PD_MAX_BINS) || r.hcal_nphi.size() != nbh) return PD_ECARD;
+    for (size_t i = 1; i <= nbh; ++i)
+      if (!(float(r.hcal_edges[i]) > float(r.hcal_edges[i - 1]))) return PD_ECARD;
+    for (long n : r.hcal_nphi) {
+      if (n < 1) return PD_ECARD;
+      total += n;
+    }
+  }
 
   if (total > long(PD_MAX_TOWERS)) return PD_ECARD;
   // every number finite and in its range: thresholds and resolutions >= 0 (a negative threshold would let pass W count
@@ -198,7 +214,10 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     if (r.has_cos && !(fin(r.cos_max) && r.cos_max > 0.0 && r.cos_max <= 1.0)) return PD_ECARD;
     for (double e : r.edges)
       if (!fin(e)) return PD_ECARD;
+    for (double e : r.hcal_edges)
+      if (!fin(e)) return PD_ECARD;
     if (r.theta && !(r.edges.front() >= 0.0 && r.edges.back() <= kPi)) return PD_ECARD;
+    if (r.theta && dual && !(r.hcal_edges.front() >= 0.0 && r.hcal_edges.back() <= kPi)) return PD_ECARD;
     if (!nonneg(r.nsig_ecal) || !nonneg(r.nsig_hcal)) return PD_ECARD;
     for (const auto &row : r.trk_eta)  // aeta_hi may be "inf"
       if (!(nonneg(row[0]) && row[1] > row[0] && nonneg(row[2]) && nonneg(row[3]))) return PD_ECARD;
@@ -223,7 +242,7 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
   s.inv_kB = s.kB_d > 0 ? float(1.0 / s.kB_d) : 0.f;
   s.sB = B > 0 ? 1.f : (B < 0 ? -1.f : 0.f);
   s.grid_theta = r.theta ? 1 : 0;
-  s.n_bins = int(nb);
+  s.n_bins = int(nb + nbh);  // all bins of the card: the ECAL grid's, then (reading K6) the HCAL grid's
   s.n_towers = int(total);
   s.words_per_event = int((total + 127) / 128) * 4;
   for (int sp = 1; sp <= 3; ++sp) {  // reading J2: the species' own resolution, else the card's common one
@@ -308,44 +327,98 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
       }
   }
 
-  c->edges.resize(nb + 1);
-  c->tb.resize(nb + 1);
-  c->nphi.resize(nb);
-  c->offset.resize(nb + 1);
-  c->inv_w.resize(nb), c->half.resize(nb), c->w.resize(nb), c->eta_c.resize(nb), c->inv_cosh.resize(nb);
+  // ---- per-bin tables, grid by grid (one grid, or the ECAL's followed by the HCAL's: reading K6); tower offsets run on
+  const size_t nball = nb + nbh;
+  c->edges.assign(2 * nball, 0.f);
+  c->tb.clear();
+  c->nphi.resize(nball);
+  c->offset.resize(nball + 1);
+  c->inv_w.resize(nball), c->half.resize(nball), c->w.resize(nball), c->eta_c.resize(nball), c->inv_cosh.resize(nball);
+  c->lut.clear();
   int acc = 0;
-  for (size_t i = 0; i <= nb; ++i) {
-    const double e = f32(r.edges[i]);
-    c->edges[i] = float(e);
-    // bin test "edge_i <= coord < edge_{i+1}" mapped to u = z/r (eta: u = sinh eta, ascending) or
-    // u = -z/r (theta: u = -cot theta, ascending in theta)
-    double t;
-    if (!r.theta) t = std::sinh(e);
-    else if (e <= 0.0) t = -kInf;
-    else if (e >= kPi) t = kInf;
-    else t = -std::cos(e) / std::sin(e);
-    c->tb[i] = float(t);
+  s.n_grids = dual ? 2 : 1;
+  for (int g = 0; g < s.n_grids; ++g) {
+    const std::vector<double> &ge = g == 0 ? r.edges : r.hcal_edges;
+    const std::vector<long> &gn = g == 0 ? r.nphi : r.hcal_nphi;
+    const size_t gnb = ge.size() - 1, b0 = g == 0 ? 0 : nb, t0 = c->tb.size();
+    s.g_nb[g] = int(gnb), s.g_bin_off[g] = int(b0), s.g_tb_off[g] = int(t0);
+    for (size_t i = 0; i <= gnb; ++i) {
+      const double e = f32(ge[i]);
+      if (i < gnb) c->edges[2 * (b0 + i)] = float(e);
+      if (i > 0) c->edges[2 * (b0 + i - 1) + 1] = float(e);
+      // bin test "edge_i <= coord < edge_{i+1}" mapped to u = z/r (eta: u = sinh eta, ascending) or
+      // u = -z/r (theta: u = -cot theta, ascending in theta)
+      double t;
+      if (!r.theta) t = std::sinh(e);
+      else if (e <= 0.0) t = -kInf;
+      else if (e >= kPi) t = kInf;
+      else t = -std::cos(e) / std::sin(e);
+      c->tb.push_back(float(t));
+    }
+    for (size_t i = 0; i < gnb; ++i) {
+      const size_t bi = b0 + i;
+      const int n = int(gn[i]);
+      c->nphi[bi] = n;
+      c->offset[bi] = acc;
+      acc += n;
+      c->inv_w[bi] = float(double(n) / (2.0 * kPi));
+      c->w[bi] = float(2.0 * kPi / double(n));
+      c->half[bi] = (n & 1) ? 0.5f : 0.f;
+      const double mid = 0.5 * (double(c->edges[2 * bi]) + double(c->edges[2 * bi + 1]));
+      const double eta = r.theta ? -std::log(std::tan(0.5 * mid)) : mid;
+      c->eta_c[bi] = float(eta);
+      c->inv_cosh[bi] = float(1.0 / std::cosh(eta));
+    }
+    s.g_tb_first[g] = c->tb[t0], s.g_tb_last[g] = c->tb[t0 + gnb];
+    // ---- eta-bin lookup of the grid: cells of |u| by float bits (2^(23 - PD_LUT_SHIFT) cells per octave, |u| < 2^MIN_EXP
+    // in one cell), mirrored for u < 0.  lut[cell] = the bin (relative to the grid) holding the cell's LOWER bound
+    // (clamped to the grid); the kernel then steps forward while u >= tb[bin + 1], so any monotone edge list is handled exactly.
+    const float *tbg = c->tb.data() + t0;
+    float umax = 1.f;
+    for (size_t i = 0; i <= gnb; ++i)
+      if (std::isfinite(tbg[i])) umax = std::max(umax, std::fabs(tbg[i]));
+    auto bits = [](float x) {
+      uint32_t b;
+      std::memcpy(&b, &x, 4);
+      return int(b >> PD_LUT_SHIFT);
+    };
+    const int lbase = bits(std::ldexp(1.f, PD_LUT_MIN_EXP));
+    const int side = bits(umax) - lbase + 2;
+    s.g_lut_base[g] = lbase, s.g_lut_side[g] = side, s.g_lut_off[g] = int(c->lut.size());
+    const size_t l0 = c->lut.size();
+    c->lut.resize(l0 + size_t(2 * side), 0);
+    auto cell_lo_abs = [&](int ca) {  // smallest |u| of cell ca on one side
+      if (ca <= 0) return 0.f;
+      const uint32_t b = uint32_t(ca + lbase) << PD_LUT_SHIFT;
+      float x;
+      std::memcpy(&x, &b, 4);
+      return x;
+    };
+    auto bin_of = [&](double u) {  // largest b with tb[b] <= u, clamped to [0, gnb-1]
+      int b = 0;
+      while (b + 1 < int(gnb) && double(tbg[size_t(b + 1)]) <= u) ++b;
+      return b;
+    };
+    for (int ca = 0; ca < side; ++ca) {
+      // positive side: u in [lo(ca), lo(ca+1)); cell index side + ca
+      c->lut[l0 + size_t(side + ca)] = (unsigned short)bin_of(double(cell_lo_abs(ca)));
+      // negative side: u in (-lo(ca+1), -lo(ca)]; lower bound -lo(ca+1) (-inf for the last cell)
+      const double lo = ca + 1 < side ? -double(cell_lo_abs(ca + 1)) : -kInf;
+      c->lut[l0 + size_t(side - 1 - ca)] = (unsigned short)bin_of(lo);
+    }
   }
-  for (size_t i = 0; i < nb; ++i) {
-    const int n = int(r.nphi[i]);
-    c->nphi[i] = n;
-    c->offset[i] = acc;
-    acc += n;
-    c->inv_w[i] = float(double(n) / (2.0 * kPi));
-    c->w[i] = float(2.0 * kPi / double(n));
-    c->half[i] = (n & 1) ? 0.5f : 0.f;
-    const double mid = 0.5 * (double(c->edges[i]) + double(c->edges[i + 1]));
-    const double eta = r.theta ? -std::log(std::tan(0.5 * mid)) : mid;
-    c->eta_c[i] = float(eta);
-    c->inv_cosh[i] = float(1.0 / std::cosh(eta));
+  c->offset[nball] = acc;
+  if (!dual) {  // one grid: both entries describe it, so that the kernels index by section without a branch
+    s.g_nb[1] = s.g_nb[0], s.g_bin_off[1] = s.g_bin_off[0], s.g_tb_off[1] = s.g_tb_off[0], s.g_lut_off[1] = s.g_lut_off[0];
+    s.g_lut_side[1] = s.g_lut_side[0], s.g_lut_base[1] = s.g_lut_base[0], s.g_tb_first[1] = s.g_tb_first[0], s.g_tb_last[1] = s.g_tb_last[0];
   }
-  c->offset[nb] = acc;
+  s.n_tb = int(c->tb.size()), s.lut_cells = int(c->lut.size());
   // readings K1-K3: per-bin resolutions (the first row whose [aeta_lo, aeta_hi) holds |eta| of the bin's tower centres,
   // else the card's common line), significance cut, smeared tower positions
   s.res_per_bin = (!r.ecal_eta.empty() || !r.hcal_eta.empty()) ? 1 : 0;
-  c->res2.assign(6 * nb, 0.f);
-  for (size_t i = 0; i < nb; ++i) {
-    const double mid = 0.5 * (double(c->edges[i]) + double(c->edges[i + 1]));
+  c->res2.assign(6 * nball, 0.f);
+  for (size_t i = 0; i < nball; ++i) {
+    const double mid = 0.5 * (double(c->edges[2 * i]) + double(c->edges[2 * i + 1]));
     const double aeta = std::fabs(r.theta ? -std::log(std::tan(0.5 * mid)) : mid);
     auto pick = [&](const std::vector<std::array<double, 5>> &rows, const double *dflt, float *out) {
       const double *csn = dflt;
@@ -373,44 +446,6 @@ int pd_card_parse(const char *name_or_path, pd_card *c) {
     const double a = on ? f32(r.trk_eta[k][2]) : 0.0;
     s.trk_row_a2[k] = float(a * a);
     s.trk_row_b[k] = on ? float(r.trk_eta[k][3]) : 0.f;
-  }
-  s.tb_first = c->tb[0], s.tb_last = c->tb[nb];
-
-  // ---- eta-bin lookup: cells of |u| by float bits (2^(23 - PD_LUT_SHIFT) cells per octave, |u| < 2^MIN_EXP in
-  // one cell), mirrored for u < 0.  lut[cell] = the bin holding the cell's LOWER bound (clamped to the grid);
-  // the kernel then steps forward while u >= tb[bin + 1], so any monotone edge list is handled exactly.
-  {
-    float umax = 1.f;
-    for (float t : c->tb)
-      if (std::isfinite(t)) umax = std::max(umax, std::fabs(t));
-    auto bits = [](float x) {
-      uint32_t b;
-      std::memcpy(&b, &x, 4);
-      return int(b >> PD_LUT_SHIFT);
-    };
-    s.lut_base = bits(std::ldexp(1.f, PD_LUT_MIN_EXP));
-    s.lut_side = bits(umax) - s.lut_base + 2;
-    const int side = s.lut_side;
-    c->lut.assign(size_t(2 * side), 0);
-    auto cell_lo_abs = [&](int ca) {  // smallest |u| of cell ca on one side
-      if (ca <= 0) return 0.f;
-      const uint32_t b = uint32_t(ca + s.lut_base) << PD_LUT_SHIFT;
-      float x;
-      std::memcpy(&x, &b, 4);
-      return x;
-    };
-    auto bin_of = [&](double u) {  // largest b with tb[b] <= u, clamped to [0, nb-1]
-      int b = 0;
-      while (b + 1 < int(nb) && double(c->tb[size_t(b + 1)]) <= u) ++b;
-      return b;
-    };
-    for (int ca = 0; ca < side; ++ca) {
-      // positive side: u in [lo(ca), lo(ca+1)); cell index side + ca
-      c->lut[size_t(side + ca)] = (unsigned short)bin_of(double(cell_lo_abs(ca)));
-      // negative side: u in (-lo(ca+1), -lo(ca)]; lower bound -lo(ca+1) (-inf for the last cell)
-      const double lo = ca + 1 < side ? -double(cell_lo_abs(ca + 1)) : -kInf;
-      c->lut[size_t(side - 1 - ca)] = (unsigned short)bin_of(lo);
-    }
   }
   return PD_OK;
 }

@@ -29,8 +29,12 @@ struct PdCardScalars {
   int n_bins, n_towers;
   int words_per_event;    // tower bitmap: ceil(n_towers / 128) * 4 words of 32 tower bits
   // eta-bin lookup table over the float bits of |u| (see pd_card.cpp): cells per side, bias
-  int lut_side, lut_base;
-  float tb_first, tb_last;  // the grid's coverage in u: tb[0] <= u < tb[n_bins]
+  // One grid, or (reading K6) two: [0] the ECAL's, [1] the HCAL's (one grid: both entries describe it).  Per grid g: its
+  // bins are g_bin_off[g] .. + g_nb[g] of the per-bin tables (tower offsets run on through both grids), its u thresholds
+  // tb[g_tb_off[g] .. + g_nb[g]], its lookup cells lut[g_lut_off[g] .. + 2 g_lut_side[g]) holding bins relative to the grid.
+  int n_grids, n_tb, lut_cells;
+  int g_nb[2], g_bin_off[2], g_tb_off[2], g_lut_off[2], g_lut_side[2], g_lut_base[2];
+  float g_tb_first[2], g_tb_last[2];  // the grid's coverage in u: tb[first] <= u < tb[last]
   // efficiency table resolved into a grid at load (reading A8: first matching row wins):
   // cell = (#pT edges with pT > e) * (n_T + 1) + (#T edges with |pz|/pT >= t)
   int n_pt, n_T;
@@ -60,7 +64,7 @@ struct PdCardScalars {
 
 // Per-bin tables, contiguous in one device allocation.
 struct PdCardTables {
-  const float *tb;        // [n_bins+1] bin thresholds in u = z/r (eta grid) or -z/r (theta grid)
+  const float *tb;        // [n_tb] bin thresholds in u = z/r (eta grid) or -z/r (theta grid): n_bins + 1 per grid
   const int *nphi;        // [n_bins]
   const int *offset;      // [n_bins+1] exclusive prefix sum of nphi
   const float *inv_w;     // [n_bins] nphi / (2 pi)
@@ -68,8 +72,8 @@ struct PdCardTables {
   const float *w;         // [n_bins] 2 pi / nphi
   const float *eta_c;     // [n_bins] tower-centre pseudorapidity
   const float *inv_cosh;  // [n_bins] 1 / cosh(eta_c)
-  const unsigned short *lut;  // [2 * lut_side] first candidate bin of a cell
-  const float *edge;      // [n_bins+1] the card's edges (eta or theta), fp32
+  const unsigned short *lut;  // [lut_cells] first candidate bin of a cell (per grid: 2 * g_lut_side cells)
+  const float *edge;      // [n_bins][2] the bins' lower and upper edges (eta or theta), fp32
   const float *res2;      // [n_bins][6] ECAL C^2, S^2, N^2, HCAL C^2, S^2, N^2 of the bin's towers (reading K1)
 };
 
@@ -78,7 +82,7 @@ struct pd_card {
   std::string name;
   // host copy (rounded to fp32 where the kernels use fp32)
   PdCardScalars sc{};
-  std::vector<float> edges;  // [n_bins+1] the card's edges (eta or theta), fp32
+  std::vector<float> edges;  // [n_bins][2] lower and upper edge of every bin (eta or theta), fp32
   std::vector<float> tb, inv_w, half, w, eta_c, inv_cosh;
   std::vector<int> nphi, offset;
   std::vector<unsigned short> lut;

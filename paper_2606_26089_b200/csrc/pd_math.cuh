@@ -20,12 +20,6 @@ constexpr float kTwoM24 = 5.9604644775390625e-08f;  // 2^-24
 constexpr float kInfF = __builtin_huge_valf();
 
 // Card tables staged in shared memory (pointers into the CTA's dynamic shared memory).
-struct SmCard {
-  const float *tb;
-  const int *nphi, *offset;
-  const float *inv_w, *half, *w, *eta_c, *inv_cosh;
-  const unsigned short *lut;
-};
 
 // ---- S-RNG: Philox4x32-10 (Salmon et al., SC'11), reading A26: key = (seed lo, seed hi),
 // counter = (object, event lo, event hi, stream << 16) -----------------------------------------
@@ -190,27 +184,6 @@ __device__ __forceinline__ float smear_component(float E, const float (&csn2)[3]
   return lognormal_rel(E, s2 * iE * iE, normal_bm(xa, xb));
 }
 
-// bin i with tb[i] <= u < tb[i+1], -1 if outside or NaN.  The lookup table gives the bin that holds
-// the lower bound of u's cell; the forward steps make the result exact for any monotone edge list.
-__device__ __forceinline__ int grid_bin(const SmCard &cd, const PdCardScalars &sc, float u) {
-  const int nb = sc.n_bins;
-  if (!(u >= cd.tb[0]) || !(u < cd.tb[nb])) return -1;
-  int ca = (__float_as_int(fabsf(u)) >> PD_LUT_SHIFT) - sc.lut_base;
-  ca = min(max(ca, 0), sc.lut_side - 1);
-  const int cell = u < 0.f ? sc.lut_side - 1 - ca : sc.lut_side + ca;
-  int b = cd.lut[cell];
-  while (u >= cd.tb[b + 1]) ++b;  // terminates: u < tb[nb]
-  return b;
-}
-
-__device__ __forceinline__ int phi_bin(const SmCard &cd, int i, float phi) {
-  const int n = cd.nphi[i];
-  int j = (int)floorf(fmaf(phi, cd.inv_w[i], cd.half[i])) + (n >> 1);
-  j = j < 0 ? 0 : j;
-  return j > n - 1 ? n - 1 : j;
-}
-
-// eta of a hit from u (only tracks and debug need it as a number)
 __device__ __forceinline__ float eta_from_u(const PdCardScalars &sc, float u) { return fast_asinh(sc.grid_theta ? -u : u); }
 
 // species of a charged particle for the per-species card tables: 0 electron, 1 muon, 2 charged hadron
@@ -218,15 +191,6 @@ __device__ __forceinline__ int species_of(int pid) {
   const int a = pid < 0 ? -pid : pid;
   return a == 11 ? 0 : (a == 13 ? 1 : 2);
 }
-
-// ---- S1..S4 for one particle -------------------------------------------------------------------
-struct ParticleOut {
-  uint32_t status;   // PD_DROPPED / PD_BARREL / PD_ENDCAP | PD_LOOPER
-  int tower;         // tower id of the hit, -1: outside the grid or dropped
-  int eps_row;       // row of the card's efficiency table, -1 none
-  bool accepted;
-  float u, phi_pos;  // hit: u = z/r (or -z/r for a theta grid), azimuth
-};
 
 // Rare path: a helix grazing the barrel (within a few % of the looper threshold).  The crossing angle
 // amplifies the rounding of rho by 1/sqrt(distance to tangency), so the quadratic is redone in double.
@@ -414,41 +378,6 @@ __device__ __forceinline__ void hit_coords(const PdCardScalars &sc, uint32_t sta
   phi_pos = fast_atan2(y, x);
 }
 
-// S4: tower of the hit, -1 outside the grid
-__device__ __forceinline__ int hit_tower(const PdCardScalars &sc, const SmCard &cd, float u, float phi_pos) {
-  const int i = grid_bin(cd, sc, u);
-  return i >= 0 ? cd.offset[i] + phi_bin(cd, i, phi_pos) : -1;
-}
-
-__device__ __forceinline__ void particle_chain(const PdCardScalars &sc, const SmCard &cd, int q, float px, float py,
-                                               float pz, float vx, float vy, float vz, const PhiloxKeys &seed,
-                                               long long event, uint32_t pidx, int species, ParticleOut &o) {
-  o.status = PD_DROPPED;
-  o.tower = -1;
-  o.eps_row = -1;
-  o.accepted = false;
-  o.u = __int_as_float(0x7fc00000);
-  o.phi_pos = o.u;
-  if (vertex_dropped(sc, px, py, vx, vy, vz)) return;
-  float x, y, z;
-  if (q == 0 || sc.sB == 0.f) o.status = line_hit(sc, px, py, pz, vx, vy, vz, x, y, z);
-  else o.status = helix_hit(sc, q, px, py, pz, vx, vy, vz, x, y, z);
-  if ((o.status & PD_FACE_MASK) == PD_DROPPED) return;
-  hit_coords(sc, o.status, x, y, z, o.u, o.phi_pos);
-  // S2 track: efficiency cell at the true vertex momentum (A7); accept iff u24 < eps (A11)
-  if (q != 0) {
-    const int cell = eff_cell(sc, px, py, pz);
-    const float eps = sc.cell_eps[species][cell];
-    o.eps_row = sc.cell_row[species][cell];
-    if (eps > 0.f) {
-      uint32_t rn[4];
-      rng_block(seed, event, pidx, 0u, rn);
-      o.accepted = uniform24(rn[0]) < eps;
-    }
-  }
-  o.tower = hit_tower(sc, cd, o.u, o.phi_pos);
-}
-
 // S3 for one accepted track (A12/A13): log-normal with mean pT and std sigma_rel pT, driven by words
 // 1 and 2 of the particle's Philox block; eta, phi unchanged; E = pT' cosh(eta) = pT' |p| / pT.
 struct TrackOut {
@@ -488,13 +417,6 @@ __device__ __forceinline__ void track_smear_words(const PdCardScalars &sc, float
   t.E_trk = t.pt_s * (fast_sqrt(fmaf(pz, pz, pt2)) * ipt);
   t.eta_mom = fast_asinh(pz * ipt);
   t.phi0 = fast_atan2(py, px);
-}
-
-__device__ __forceinline__ void track_smear(const PdCardScalars &sc, float px, float py, float pz,
-                                            const PhiloxKeys &seed, long long event, uint32_t pidx, int species, TrackOut &t) {
-  uint32_t rn[4];
-  rng_block(seed, event, pidx, 0u, rn);
-  track_smear_words(sc, px, py, pz, rn[1], rn[2], species, t);
 }
 
 // per-tower smear of both components (S6): the common case of a single non-zero component runs one

@@ -57,7 +57,7 @@ static_assert(PO_PID % 16 == 0 && PO_Q % 16 == 0 && PO_KEY % 16 == 0 && PO_LIST 
 struct PTables {
   size_t tb, binrec, lut, total;
 };
-__host__ __device__ inline PTables make_ptables(int n_bins, int lut_cells) {
+__host__ __device__ inline PTables make_ptables(int n_bins, int n_tb, int lut_cells) {
   PTables l;
   size_t o = PO_TABLES;
   auto take = [&](size_t bytes) {
@@ -65,23 +65,26 @@ __host__ __device__ inline PTables make_ptables(int n_bins, int lut_cells) {
     o = (o + bytes + 15) & ~size_t(15);
     return at;
   };
-  l.tb = take(4 * (size_t)(n_bins + 1));
+  l.tb = take(4 * (size_t)n_tb);
   l.binrec = take(16 * (size_t)n_bins);  // per bin: inv_w, half, offset | nphi << 16, pad
   l.lut = take(2 * (size_t)lut_cells);
   l.total = o;
   return l;
 }
 
-// S4 with the per-bin record in one 16-byte load: tower of the hit (u, phi), -1 outside the grid
-__device__ __forceinline__ int hit_tower_rec(const PdCardScalars &sc, const float *tb, const float4 *rec, const unsigned short *lut,
-                                             float u, float phi) {
-  if (!(u >= sc.tb_first) || !(u < sc.tb_last)) return -1;
-  int ca = (__float_as_int(fabsf(u)) >> PD_LUT_SHIFT) - sc.lut_base;
-  ca = min(max(ca, 0), sc.lut_side - 1);
-  const int cell = u < 0.f ? sc.lut_side - 1 - ca : sc.lut_side + ca;
-  int b = lut[cell];
-  while (u >= tb[b + 1]) ++b;  // terminates: u < tb[n_bins]
-  const float4 r = rec[b];
+// S4 with the per-bin record in one 16-byte load: tower of the hit (u, phi), -1 outside the grid.  g: the grid the deposit is
+// looked up in (0 ECAL, 1 HCAL: reading K6; on a card with one grid both describe it)
+__device__ __forceinline__ int hit_tower_rec(const PdCardScalars &sc, int g, const float *tb_all, const float4 *rec_all,
+                                             const unsigned short *lut_all, float u, float phi) {
+  if (!(u >= sc.g_tb_first[g]) || !(u < sc.g_tb_last[g])) return -1;
+  const float *tb = tb_all + sc.g_tb_off[g];
+  const int side = sc.g_lut_side[g];
+  int ca = (__float_as_int(fabsf(u)) >> PD_LUT_SHIFT) - sc.g_lut_base[g];
+  ca = min(max(ca, 0), side - 1);
+  const int cell = u < 0.f ? side - 1 - ca : side + ca;
+  int b = lut_all[sc.g_lut_off[g] + cell];
+  while (u >= tb[b + 1]) ++b;  // terminates: u < tb[last]
+  const float4 r = rec_all[sc.g_bin_off[g] + b];
   const int on = __float_as_int(r.z);
   const int n = on >> 16;
   int j = (int)floorf(fmaf(phi, r.x, r.y)) + (n >> 1);
@@ -129,7 +132,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
   uint64_t *s_bar = (uint64_t *)(s_misc + 0);
   int *s_cnt = (int *)(s_misc + 1);               // [2] this tile
   long long *s_win = (long long *)(s_misc + 3);   // [0] e_lo, [1] e_hi
-  const PTables TL = make_ptables(nb, 2 * sc.lut_side);
+  const PTables TL = make_ptables(nb, sc.n_tb, sc.lut_cells);
   float *s_tb = (float *)(smem + TL.tb);
   float4 *s_rec = (float4 *)(smem + TL.binrec);
   unsigned short *s_lut = (unsigned short *)(smem + TL.lut);
@@ -137,10 +140,10 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
 
-  for (int i = tid; i <= nb; i += PT_THREADS) s_tb[i] = prm.tab.tb[i];
+  for (int i = tid; i < sc.n_tb; i += PT_THREADS) s_tb[i] = prm.tab.tb[i];
   for (int i = tid; i < nb; i += PT_THREADS)
     s_rec[i] = make_float4(prm.tab.inv_w[i], prm.tab.half[i], __int_as_float(prm.tab.offset[i] | (prm.tab.nphi[i] << 16)), 0.f);
-  for (int i = tid; i < 2 * sc.lut_side; i += PT_THREADS) s_lut[i] = prm.tab.lut[i];
+  for (int i = tid; i < sc.lut_cells; i += PT_THREADS) s_lut[i] = prm.tab.lut[i];
   if (tid == 0) {
     mbar_init(s_bar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -293,13 +296,13 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
         const bool live = (status & PD_FACE_MASK) != PD_DROPPED;
         u = __int_as_float(0x7fc00000), phi_pos = u;
         int tower = -1;
-        if (live) {
-          hit_coords(sc, status, x, y, z, u, phi_pos);
-          tower = hit_tower_rec(sc, s_tb, s_rec, s_lut, u, phi_pos);
-        }
         const int apid = pid < 0 ? -pid : pid;
         const bool to_ecal = apid == 11 || apid == 22;  // reading A18
         const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
+        if (live) {
+          hit_coords(sc, status, x, y, z, u, phi_pos);
+          tower = hit_tower_rec(sc, to_ecal ? 0 : 1, s_tb, s_rec, s_lut, u, phi_pos);  // in the grid of its section (K6)
+        }
         if (cls == 0 && live) {
           // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0.
           // The event: the last one whose offset is <= i (bisection of the tile's offsets; one step on big events)
@@ -383,10 +386,10 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
 
 }  // namespace pdk
 
-size_t pd_particle_smem_bytes(const pd_card *c) { return pdk::make_ptables(c->sc.n_bins, 2 * c->sc.lut_side).total; }
+size_t pd_particle_smem_bytes(const pd_card *c) { return pdk::make_ptables(c->sc.n_bins, c->sc.n_tb, c->sc.lut_cells).total; }
 
 int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_smem_optin, void *stream) {
-  const size_t smem = pdk::make_ptables(prm.sc.n_bins, 2 * prm.sc.lut_side).total;
+  const size_t smem = pdk::make_ptables(prm.sc.n_bins, prm.sc.n_tb, prm.sc.lut_cells).total;
   if (smem > (size_t)max_smem_optin) return PD_ECUDA;
   // variants: debug outputs; impact parameters from the chain (pd_options.impact); weighted EFlow (card key, reading K5)
   using Kern = void (*)(const PdParams);

@@ -65,7 +65,7 @@ __host__ __device__ inline Layout make_layout(int n_bins, int n_towers, int word
   l.inv_cosh = take(4 * n_bins);
   l.binlut = take(2 * (size_t)((n_towers >> 5) + 2));
   l.res2 = take(res_per_bin ? 4 * 6 * (size_t)n_bins : 0);
-  l.edge = take(smear_center ? 4 * (size_t)(n_bins + 1) : 0);
+  l.edge = take(smear_center ? 4 * 2 * (size_t)n_bins : 0);
   l.off32 = take(4 * (G + 1));
   l.ntrk = take(4 * (G + 1));
   l.ntow = take(4 * (G + 1));
@@ -154,7 +154,7 @@ struct TCard {
   const unsigned short *binlut;  // eta bin of tower ids 0, 32, 64, ...
   const float *w, *eta_c, *inv_cosh;
   const float *res2;             // [n_bins][6] (reading K1), only if sc.res_per_bin
-  const float *edge;             // [n_bins+1] (reading K3), only if sc.smear_center
+  const float *edge;             // [n_bins][2] (reading K3), only if sc.smear_center
 };
 __device__ __forceinline__ int tower_bin(const TCard &tc, int tower) {
   int b = (int)tc.binlut[tower >> 5];
@@ -201,7 +201,7 @@ __device__ __forceinline__ void tower_position(const PdCardScalars &sc, const TC
   }
   uint32_t rn[4];
   rng_block(rk, event, (uint32_t)tower, 4u, rn);
-  const float lo = tc.edge[b], x = fmaf(uniform24(rn[0]), tc.edge[b + 1] - lo, lo);
+  const float lo = tc.edge[2 * b], x = fmaf(uniform24(rn[0]), tc.edge[2 * b + 1] - lo, lo);
   eta = sc.grid_theta ? -logf(tanf(0.5f * x)) : x;
   phi = fmaf((float)j + uniform24(rn[1]), tc.w[b], -kPiF);
   inv_cosh = 1.0f / coshf(eta);
@@ -563,7 +563,7 @@ __global__ void __launch_bounds__(THREADS, CTAS) pd_tower_kernel(const __grid_co
   if (sc.res_per_bin)
     for (int i = tid; i < 6 * nb; i += THREADS) s_res2[i] = prm.tab.res2[i];
   if (sc.smear_center)
-    for (int i = tid; i <= nb; i += THREADS) s_edge[i] = prm.tab.edge[i];
+    for (int i = tid; i < 2 * nb; i += THREADS) s_edge[i] = prm.tab.edge[i];
   __syncthreads();
   // eta bin of tower ids 0, 32, 64, ...: start of the short forward search of pass O
   for (int c = tid; c <= (sc.n_towers >> 5); c += THREADS) {

@@ -308,8 +308,8 @@ def test_forced_kernel_variants_in_a_subprocess(tmp_path):
 
 @pytest.mark.parametrize("base,cfg,ne", [("cms_like", 0, 600), ("cms_like", 1, 200), ("aleph_like", 4, 1500)])
 def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
-    """SURVEY 8f NEXT-3, readings K1-K5: eta-dependent ECAL / HCAL / track resolutions, the significance cut,
-    tower positions smeared inside the cell and the weighted EFlow -- one at a time and all together, on an eta grid and on a theta grid;
+    """SURVEY 8f NEXT-3, readings K1-K6: eta-dependent ECAL / HCAL / track resolutions, the significance cut,
+    tower positions smeared inside the cell, the weighted EFlow and a grid of its own for the HCAL -- one at a time and all together, on an eta grid and on a theta grid;
     and an event too large for the chip (the big-tile path has its own copy of the tower code)."""
     import cards
     from gpu_util import run_gpu
@@ -321,14 +321,18 @@ def test_higher_fidelity_cards(base, cfg, ne, tmp_path):
     hcal_rows = [(0.0, 1.3, 0.04, 1.0, 0.0), (1.3, 3.0, 0.06, 1.3, 0.5), (3.0, 9.0, 0.10, 2.0, 1.0)]
     # K4: track resolution rows by |eta| of the momentum, the second for muons only, a gap between 1.4 and 1.7, an open end
     trk_rows = [(0.0, 0.9, 0.015, 2e-4), (0.9, 1.4, 0.05, 0.0, 2), (0.9, 1.4, 0.02, 3e-4), (1.7, "inf", 0.04, 1e-3)]
+    # K6: a grid of its own for the HCAL, twice as coarse in both directions as the card's (ECAL) grid
+    he = [float(x) for x in np.asarray(b.edges)[::2]]
+    hn = [max(1, int(n) // 2) for n in np.asarray(b.nphi)[::2]][: len(he) - 1]
     variants = {
         "eta_rows": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows),
         "significance": dict(ecal_nsigma=2.0, hcal_nsigma=1.5),
         "smeared_centres": dict(smear_tower_center=1),
         "track_rows": dict(track_res_eta=trk_rows),
         "weighted_eflow": dict(eflow_weighted=1, track_res=(0.03, 5e-4)),
+        "dual_grid": dict(hcal_edges=he, hcal_nphi=hn),
         "all": dict(ecal_res_eta=ecal_rows, hcal_res_eta=hcal_rows, ecal_nsigma=1.0, hcal_nsigma=1.2, smear_tower_center=1,
-                    track_res_eta=trk_rows, eflow_weighted=1),
+                    track_res_eta=trk_rows, eflow_weighted=1, hcal_edges=he, hcal_nphi=hn),
     }
     ev = wl.generate(cfg, ne)
     if cfg == 0:
