@@ -115,7 +115,7 @@ __global__ void pd_tile_events_kernel(const long long *offsets, long long n_even
   out[2 * j + 1] = (int)lo - 1;
 }
 
-template <bool DEBUG, bool IMPACT, bool WEIGHTED>
+template <bool DEBUG, bool IMPACT, bool WEIGHTED, bool DUAL>
 __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid_constant__ PdParams prm) {
   extern __shared__ __align__(128) unsigned char smem[];
   const PdCardScalars &sc = prm.sc;
@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
         const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
         if (live) {
           hit_coords(sc, status, x, y, z, u, phi_pos);
-          tower = hit_tower_rec(sc, to_ecal ? 0 : 1, s_tb, s_rec, s_lut, u, phi_pos);  // in the grid of its section (K6)
+          tower = hit_tower_rec(sc, DUAL ? (to_ecal ? 0 : 1) : 0, s_tb, s_rec, s_lut, u, phi_pos);  // in the grid of its section (K6)
         }
         if (cls == 0 && live) {
           // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0.
@@ -391,13 +391,14 @@ size_t pd_particle_smem_bytes(const pd_card *c) { return pdk::make_ptables(c->sc
 int pd_launch_particles(const PdParams &prm, bool debug, int num_sms, int max_smem_optin, void *stream) {
   const size_t smem = pdk::make_ptables(prm.sc.n_bins, prm.sc.n_tb, prm.sc.lut_cells).total;
   if (smem > (size_t)max_smem_optin) return PD_ECUDA;
-  // variants: debug outputs; impact parameters from the chain (pd_options.impact); weighted EFlow (card key, reading K5)
+  // variants: debug outputs; impact parameters from the chain (pd_options.impact); weighted EFlow (reading K5); a second grid
+  // for the HCAL (reading K6) -- each compiled in only for the calls and cards that use it
   using Kern = void (*)(const PdParams);
-  static const Kern kerns[8] = {pdk::pd_particle_kernel<false, false, false>, pdk::pd_particle_kernel<true, false, false>,
-                                pdk::pd_particle_kernel<false, true, false>,  pdk::pd_particle_kernel<true, true, false>,
-                                pdk::pd_particle_kernel<false, false, true>,  pdk::pd_particle_kernel<true, false, true>,
-                                pdk::pd_particle_kernel<false, true, true>,   pdk::pd_particle_kernel<true, true, true>};
-  const Kern kern = kerns[(debug ? 1 : 0) | (prm.imp_on ? 2 : 0) | (prm.park_sig ? 4 : 0)];
+#define PD_P4(I, W, D) pdk::pd_particle_kernel<false, I, W, D>, pdk::pd_particle_kernel<true, I, W, D>
+  static const Kern kerns[16] = {PD_P4(false, false, false), PD_P4(true, false, false), PD_P4(false, true, false), PD_P4(true, true, false),
+                                 PD_P4(false, false, true),  PD_P4(true, false, true),  PD_P4(false, true, true),  PD_P4(true, true, true)};
+#undef PD_P4
+  const Kern kern = kerns[(debug ? 1 : 0) | (prm.imp_on ? 2 : 0) | (prm.park_sig ? 4 : 0) | (prm.sc.n_grids > 1 ? 8 : 0)];
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin) != cudaSuccess) return PD_ECUDA;
   // persistent CTAs that claim their tiles from a counter: as many as fit on the device
   int per_sm = 0;
