@@ -250,10 +250,40 @@ static __device__ __noinline__ float barrel_z_double(const PdCardScalars &sc, fl
   return (float)((double)vz + 2.0 * atan2((double)ss, (double)cc) * (double)pz / (sc.kB_d * (double)aq));
 }
 
+// a barrel hit at the end of a long arc (chord > sqrt(2) R: only from a vertex far off the axis): the chord is good to ~6e-7 of
+// its length in fp32, the azimuth of the hit wants 1e-6 R
+static __device__ __noinline__ void barrel_xy_double(const PdCardScalars &sc, float px, float py, float vx, float vy, float aq, float s,
+                                                     float &x, float &y) {
+  float cc = 1.f, ss = 0.f;
+  graze_double(sc, px, py, vx, vy, aq, s, cc, ss);
+  const double ccd = cc, ssd = ss, nrm = rsqrt_d(ccd * ccd + ssd * ssd), ch = ccd * nrm, sh = ssd * nrm;
+  const double pxd = px, pyd = py, p2 = pxd * pxd + pyd * pyd, ipt = rsqrt_d(p2), pt = p2 * ipt;
+  const double rho = pt * rcp_d(sc.kB_d * (double)aq), c0 = pxd * ipt, s0 = pyd * ipt, l2 = 2.0 * rho * sh;
+  x = (float)((double)vx + l2 * (c0 * ch - (double)s * s0 * sh));
+  y = (float)((double)vy + l2 * (s0 * ch + (double)s * c0 * sh));
+}
+
+// The straight line's two rare cases (one call site): an endcap hit much closer to the axis than the vertex is (x, y are small
+// differences of vertex and path), and a barrel hit whose z is a small difference of the vertex z and a long path.
+static __device__ __noinline__ void line_fix_double(const PdCardScalars &sc, bool endcap, float sgnz, float px, float py, float pz, float vx,
+                                                    float vy, float vz, float &x, float &y, float &z) {
+  const double pxd = px, pyd = py, vxd = vx, vyd = vy;
+  if (endcap) {
+    const double td = ((double)sc.L - (double)(sgnz * vz)) * rcp_d(fabs((double)pz));
+    x = (float)fma(td, pxd, vxd), y = (float)fma(td, pyd, vyd);
+  } else {
+    const double pt2 = pxd * pxd + pyd * pyd, bb = vxd * pxd + vyd * pyd, Rd = sc.R;
+    const double Dd = Rd * Rd - (vxd * vxd + vyd * vyd);
+    const double dd = bb * bb + pt2 * Dd, sq = dd * rsqrt_d(dd);
+    const double td = bb > 0.0 ? Dd * rcp_d(bb + sq) : (sq - bb) * rcp_d(pt2);
+    z = (float)fma(td, (double)pz, (double)vz);
+  }
+}
+
 // readings A4, A5: born on/outside the cylinder, or no transverse momentum -> dropped
-__device__ __forceinline__ bool vertex_dropped(const PdCardScalars &sc, float px, float py, float vx, float vy, float vz) {
+__device__ __forceinline__ bool vertex_dropped(const PdCardScalars &sc, float px, float py, float vx, float vy, float vz, float &r02) {
   const float pt2 = fmaf(px, px, py * py);
-  const float r02 = fmaf(vx, vx, vy * vy);
+  r02 = fmaf(vx, vx, vy * vy);
   return r02 >= sc.R2 || fabsf(vz) >= sc.L || pt2 < 1e-9f;
 }
 
@@ -279,7 +309,7 @@ __device__ __forceinline__ int eff_cell(const PdCardScalars &sc, float px, float
 // S1 for a neutral particle (or no field): straight line to r = R or |z| = L, whichever comes first.  The caller
 // has excluded dropped vertices.  Returns the face; (x, y, z) = the hit.
 __device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, float py, float pz, float vx, float vy, float vz,
-                                             float &x, float &y, float &z) {
+                                             float &x, float &y, float &z, bool off_axis = true) {
   const float pt2 = fmaf(px, px, py * py);
   const float apz = fabsf(pz);
   const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
@@ -294,6 +324,11 @@ __device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, 
   const float t = endcap ? zdist * fast_rcp(apz) : num * fast_rcp(den);
   x = fmaf(t, px, vx), y = fmaf(t, py, vy);
   z = endcap ? sgnz * sc.L : fmaf(t, pz, vz);
+  // rare cases of a vertex far off the axis, redone in double (see line_fix_double); never for vertices on the axis
+  if (off_axis) {
+    const float dzp = z - vz;
+    if (endcap ? fmaf(x, x, y * y) < 0.09f * (sc.R2 - D) : dzp * dzp > fmaf(z, z, sc.R2)) line_fix_double(sc, endcap, sgnz, px, py, pz, vx, vy, vz, x, y, z);
+  }
   return endcap ? PD_ENDCAP : PD_BARREL;
 }
 
@@ -301,7 +336,7 @@ __device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, 
 // in +z field turns clockwise).  Returns PD_DROPPED | PD_LOOPER for a trapped looper (reading A6), else the face
 // (| PD_LOOPER when the helix never reaches r = R).
 __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, float px, float py, float pz, float vx, float vy,
-                                              float vz, float &x, float &y, float &z) {
+                                              float vz, float &x, float &y, float &z, bool off_axis = true) {
   const float pt2 = fmaf(px, px, py * py);
   const float ipt = fast_rsqrt(pt2);
   const float pt = pt2 * ipt;
@@ -359,15 +394,27 @@ __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, fl
     ch = cc * inv, sh = ss * inv;
     const float hR = fast_atan2(ss, cc);
     z = fmaf(2.f * hR, pz * sc.inv_kB * (aq == 1.f ? 1.f : fast_rcp(aq)), vz);
-    // (the path along z is good to ~3e-7 of its length: that matters against the 1e-6 of eta only for a long path that
-    // ends near z = 0, i.e. for a vertex metres away from the centre)
-    if (fabsf(z - vz) > 2.f * sc.R && fabsf(z) < sc.R) z = barrel_z_double(sc, px, py, pz, vx, vy, vz, aq, s);
+    // The path along z is good to ~6e-7 of its length, and eta = asinh(z / R) moves by dz / sqrt(z^2 + R^2): against the 1e-6
+    // of eta that matters when the path is longer than the hit is far from the centre (a vertex far away in z, the hit back
+    // near z = 0), and for a steep track born next to the barrel surface (D << R^2: the half-angle is then a small difference
+    // of large terms).  Neither happens for vertices on the axis; redone in double.
+    // (see the end of the function)
   }
   // chord form (pi-periodic in h): position = v + 2 rho sin h u(phi0 + s h)
   const float l2 = 2.f * rho * sh;
   x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
   y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
-  if (endcap && fmaf(x, x, y * y) < 0.09f * (sc.R2 - D)) endcap_xy_double(sc, px, py, pz, vx, vy, vz, aq, s, x, y);
+  // the three rare cases of a vertex far off the axis (off_axis: warp-uniform, false for a warp whose vertices all sit on the
+  // axis -- every workload of BASELINE.json -- which then skips the tests as well)
+  if (off_axis) {
+    if (endcap) {
+      if (fmaf(x, x, y * y) < 0.09f * (sc.R2 - D)) endcap_xy_double(sc, px, py, pz, vx, vy, vz, aq, s, x, y);
+    } else {
+      const float dzp = z - vz, dx = x - vx, dy = y - vy;
+      if (dzp * dzp > fmaf(z, z, sc.R2) || (D < 0.3f * sc.R2 && apz * ipt > 2.f)) z = barrel_z_double(sc, px, py, pz, vx, vy, vz, aq, s);
+      if (fmaf(dx, dx, dy * dy) > 2.f * sc.R2) barrel_xy_double(sc, px, py, vx, vy, aq, s, x, y);
+    }
+  }
   return (endcap ? PD_ENDCAP : PD_BARREL) | looper;
 }
 

@@ -220,6 +220,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     // ---- partition of the warp's own particles by class (S0): A charged with efficiency > 0, B other charged,
     // N neutral; dropped particles are finished here.  No other warp is involved: ballots and register counts.
     int nA = 0, nB = 0, nN = 0;
+    bool off_axis = false;  // some vertex of the warp's segment is off the beam axis (then the rare double paths are armed)
     uint32_t pk[PT_ITERS];  // per row: entry (i | row << 11) | class << 16 | rank within the class << 18
 #pragma unroll
     for (int k = 0; k < PT_ITERS; ++k) {
@@ -230,7 +231,10 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
       if (i < n && i >= lo_skip) {
         const int q = (int)s_q[i];
         const float px = s_px[i], py = s_py[i];
-        if (vertex_dropped(sc, px, py, s_vx[i], s_vy[i], s_vz[i])) {
+        float r02;
+        const bool dropped = vertex_dropped(sc, px, py, s_vx[i], s_vy[i], s_vz[i], r02);
+        off_axis |= r02 > 0.f;
+        if (dropped) {
           s_key[i] = (unsigned short)PT_NONE;
           if (DEBUG) {
             const long long g = s0 + i;
@@ -266,6 +270,7 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     }
     __syncwarp();
     const int n_work = nA + nB + nN;
+    off_axis = __any_sync(0xffffffffu, off_axis);
 
     // ---- S1-S4 on the warp's lists A | B | N: rows of one class (the rows at the two boundaries are mixed).
     // Accepted tracks are smeared on the spot and PARKED at once in the workspace: list A is in particle order and only
@@ -291,8 +296,8 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
         pid = s_pid[i];
         float x, y, z;
         uint32_t status;
-        if (cls == 2 || sc.sB == 0.f) status = line_hit(sc, px, py, pz, vx, vy, vz, x, y, z);
-        else status = helix_hit(sc, (int)s_q[i], px, py, pz, vx, vy, vz, x, y, z);
+        if (cls == 2 || sc.sB == 0.f) status = line_hit(sc, px, py, pz, vx, vy, vz, x, y, z, off_axis);
+        else status = helix_hit(sc, (int)s_q[i], px, py, pz, vx, vy, vz, x, y, z, off_axis);
         const bool live = (status & PD_FACE_MASK) != PD_DROPPED;
         u = __int_as_float(0x7fc00000), phi_pos = u;
         int tower = -1;

@@ -62,6 +62,23 @@ def test_displaced_vertices_randomised(card, bz, tmp_path):
     print(card, bz, {k: rep[k] for k in ("n_particles", "flagged_particles", "overridden_particles", "neutral_outside_plain_tol", "neutrals")})
 
 
+@pytest.mark.parametrize("card,seed", [("atlas_like", 16), ("cms_like", 30), ("cms_like", 57), ("cms_like", 69), ("atlas_like", 406), ("atlas_like", 469)])
+def test_displaced_vertices_rare_cancellations(card, seed):
+    """Seeds of a 900-draw sweep (24 million particles) in which one particle each used to miss the position tolerance by up to a
+    factor 2 (1e-5 in azimuth for the near-axis hits): fp32 cancellation for vertices far off the axis -- a barrel hit whose z is
+    a small difference of the vertex z and a long path (helix and straight line), an endcap hit of a neutral particle a few mm
+    from the axis, a barrel hit at the end of an arc longer than sqrt(2) R, a steep track born next to the barrel surface.
+    Each is redone in double now (pd_math.cuh); the sweep finds nothing any more."""
+    from gpu_util import run_gpu
+    from parity import compare
+
+    info = {"cms_like": (1.29, 3.0), "atlas_like": (1.15, 3.5), "aleph_like": (1.8, 2.5)}[card]
+    ev = wl.displaced(600, 45.0, info[0], info[1], seed=1000 + seed)
+    gpu = run_gpu(card, ev, seed)
+    assert gpu["status_word"] == 0
+    _check(compare(card, ev, seed, gpu))
+
+
 def test_many_tiny_and_empty_events_in_one_particle_tile():
     """Events of 0-2 particles: a tile of kernel P (1,536 particles) then spans > 1,000 events, more than the window of
     event offsets it keeps on chip, and looks its events up in global memory instead; kernel T packs 256 events a tile."""
