@@ -308,8 +308,9 @@ __device__ __forceinline__ int eff_cell(const PdCardScalars &sc, float px, float
 
 // S1 for a neutral particle (or no field): straight line to r = R or |z| = L, whichever comes first.  The caller
 // has excluded dropped vertices.  Returns the face; (x, y, z) = the hit.
+template <bool OFF_AXIS = true>
 __device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, float py, float pz, float vx, float vy, float vz,
-                                             float &x, float &y, float &z, bool off_axis = true) {
+                                             float &x, float &y, float &z) {
   const float pt2 = fmaf(px, px, py * py);
   const float apz = fabsf(pz);
   const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
@@ -325,7 +326,7 @@ __device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, 
   x = fmaf(t, px, vx), y = fmaf(t, py, vy);
   z = endcap ? sgnz * sc.L : fmaf(t, pz, vz);
   // rare cases of a vertex far off the axis, redone in double (see line_fix_double); never for vertices on the axis
-  if (off_axis) {
+  if (OFF_AXIS) {
     const float dzp = z - vz;
     if (endcap ? fmaf(x, x, y * y) < 0.09f * (sc.R2 - D) : dzp * dzp > fmaf(z, z, sc.R2)) line_fix_double(sc, endcap, sgnz, px, py, pz, vx, vy, vz, x, y, z);
   }
@@ -335,8 +336,9 @@ __device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, 
 // S1 for a charged particle in the field: helix of radius rho; momentum azimuth phi0 + s alpha (reading A3: q > 0
 // in +z field turns clockwise).  Returns PD_DROPPED | PD_LOOPER for a trapped looper (reading A6), else the face
 // (| PD_LOOPER when the helix never reaches r = R).
+template <bool OFF_AXIS = true>
 __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, float px, float py, float pz, float vx, float vy,
-                                              float vz, float &x, float &y, float &z, bool off_axis = true) {
+                                              float vz, float &x, float &y, float &z) {
   const float pt2 = fmaf(px, px, py * py);
   const float ipt = fast_rsqrt(pt2);
   const float pt = pt2 * ipt;
@@ -404,9 +406,9 @@ __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, fl
   const float l2 = 2.f * rho * sh;
   x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
   y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
-  // the three rare cases of a vertex far off the axis (off_axis: warp-uniform, false for a warp whose vertices all sit on the
+  // the three rare cases of a vertex far off the axis (OFF_AXIS: false in the copy of the row loop that a warp whose vertices all sit on the
   // axis -- every workload of BASELINE.json -- which then skips the tests as well)
-  if (off_axis) {
+  if (OFF_AXIS) {
     if (endcap) {
       if (fmaf(x, x, y * y) < 0.09f * (sc.R2 - D)) endcap_xy_double(sc, px, py, pz, vx, vy, vz, aq, s, x, y);
     } else {

@@ -21,6 +21,7 @@
 #include <algorithm>
 #include <cstdint>
 #include <cstdlib>
+#include <type_traits>
 
 #include "pd_internal.h"
 #include "pd_impact_math.cuh"
@@ -279,102 +280,109 @@ __global__ void __launch_bounds__(PT_THREADS, 4) pd_particle_kernel(const __grid
     // where an event's tracks go, moves them into the Track collection.
     const long long seg0 = (s0 - p_al) + wbase;  // first slot of the warp's segment in the parking arrays
     int run = 0;                                 // tracks of the segment so far
-#pragma unroll 1
-    for (int k = 0; k < PT_ITERS; ++k) {
-      const int v = 32 * k + lane;
-      bool accepted = false;
-      int i = 0, pid = 0;
-      float px = 0.f, py = 0.f, pz = 0.f, u = 0.f, phi_pos = 0.f;
-      uint32_t r1 = 0u, r2 = 0u, pidx_t = 0u;
-      long long ev_t = 0;  // (IMPACT: the track's event and index in it, for Philox stream 3)
-      if (v < n_work) {
-        const int cls = v < nA ? 0 : (v < nA + nB ? 1 : 2);
-        const unsigned ent = s_list[wbase + v];
-        i = (int)(ent & 0x7ffu);
-        px = s_px[i], py = s_py[i], pz = s_pz[i];
-        const float vx = s_vx[i], vy = s_vy[i], vz = s_vz[i];
-        pid = s_pid[i];
-        float x, y, z;
-        uint32_t status;
-        if (cls == 2 || sc.sB == 0.f) status = line_hit(sc, px, py, pz, vx, vy, vz, x, y, z, off_axis);
-        else status = helix_hit(sc, (int)s_q[i], px, py, pz, vx, vy, vz, x, y, z, off_axis);
-        const bool live = (status & PD_FACE_MASK) != PD_DROPPED;
-        u = __int_as_float(0x7fc00000), phi_pos = u;
-        int tower = -1;
-        const int apid = pid < 0 ? -pid : pid;
-        const bool to_ecal = apid == 11 || apid == 22;  // reading A18
-        const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
-        if (live) {
-          hit_coords(sc, status, x, y, z, u, phi_pos);
-          tower = hit_tower_rec(sc, DUAL ? (to_ecal ? 0 : 1) : 0, s_tb, s_rec, s_lut, u, phi_pos);  // in the grid of its section (K6)
-        }
-        if (cls == 0 && live) {
-          // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0.
-          // The event: the last one whose offset is <= i (bisection of the tile's offsets; one step on big events)
-          long long ev;
-          uint32_t pidx;
-          if (!wide) {
-            int lo = 0, hi = n_win - 1;
-            while (lo < hi) {
-              const int mid = (lo + hi + 1) >> 1;
-              if (s_woff[mid] <= i) lo = mid;
-              else hi = mid - 1;
-            }
-            ev = e_lo + lo, pidx = (uint32_t)(i - s_woff[lo]);
-          } else {
-            long long lo = e_lo, hi = e_hi;
-            const long long g = s0 + i;
-            while (lo < hi) {
-              const long long mid = (lo + hi + 1) >> 1;
-              if (__ldg(prm.offsets + mid) <= g) lo = mid;
-              else hi = mid - 1;
-            }
-            ev = lo, pidx = (uint32_t)(g - __ldg(prm.offsets + lo));
+    // Two copies of the row loop: the one a warp whose vertices all sit on the beam axis takes (every workload of BASELINE.json)
+    // has none of the double-precision redos of far-off vertices compiled in (pd_math.cuh), not even their tests
+    auto rows = [&](auto off_tag) {
+      constexpr bool OFF = decltype(off_tag)::value;
+  #pragma unroll 1
+      for (int k = 0; k < PT_ITERS; ++k) {
+        const int v = 32 * k + lane;
+        bool accepted = false;
+        int i = 0, pid = 0;
+        float px = 0.f, py = 0.f, pz = 0.f, u = 0.f, phi_pos = 0.f;
+        uint32_t r1 = 0u, r2 = 0u, pidx_t = 0u;
+        long long ev_t = 0;  // (IMPACT: the track's event and index in it, for Philox stream 3)
+        if (v < n_work) {
+          const int cls = v < nA ? 0 : (v < nA + nB ? 1 : 2);
+          const unsigned ent = s_list[wbase + v];
+          i = (int)(ent & 0x7ffu);
+          px = s_px[i], py = s_py[i], pz = s_pz[i];
+          const float vx = s_vx[i], vy = s_vy[i], vz = s_vz[i];
+          pid = s_pid[i];
+          float x, y, z;
+          uint32_t status;
+          if (cls == 2 || sc.sB == 0.f) status = line_hit<OFF>(sc, px, py, pz, vx, vy, vz, x, y, z);
+          else status = helix_hit<OFF>(sc, (int)s_q[i], px, py, pz, vx, vy, vz, x, y, z);
+          const bool live = (status & PD_FACE_MASK) != PD_DROPPED;
+          u = __int_as_float(0x7fc00000), phi_pos = u;
+          int tower = -1;
+          const int apid = pid < 0 ? -pid : pid;
+          const bool to_ecal = apid == 11 || apid == 22;  // reading A18
+          const bool to_none = apid == 13 || apid == 12 || apid == 14 || apid == 16;
+          if (live) {
+            hit_coords(sc, status, x, y, z, u, phi_pos);
+            tower = hit_tower_rec(sc, DUAL ? (to_ecal ? 0 : 1) : 0, s_tb, s_rec, s_lut, u, phi_pos);  // in the grid of its section (K6)
           }
-          uint32_t rn[4];
-          rng_block(prm.rk, prm.event_base + ev, pidx, 0u, rn);
-          accepted = uniform24(rn[0]) < sc.row_eps[ent >> 11];
-          r1 = rn[1], r2 = rn[2];
-          if (IMPACT) ev_t = prm.event_base + ev, pidx_t = pidx;
+          if (cls == 0 && live) {
+            // S2: accept iff u24 < eps (A11); Philox(seed, event, particle index within the event), stream 0.
+            // The event: the last one whose offset is <= i (bisection of the tile's offsets; one step on big events)
+            long long ev;
+            uint32_t pidx;
+            if (!wide) {
+              int lo = 0, hi = n_win - 1;
+              while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (s_woff[mid] <= i) lo = mid;
+                else hi = mid - 1;
+              }
+              ev = e_lo + lo, pidx = (uint32_t)(i - s_woff[lo]);
+            } else {
+              long long lo = e_lo, hi = e_hi;
+              const long long g = s0 + i;
+              while (lo < hi) {
+                const long long mid = (lo + hi + 1) >> 1;
+                if (__ldg(prm.offsets + mid) <= g) lo = mid;
+                else hi = mid - 1;
+              }
+              ev = lo, pidx = (uint32_t)(g - __ldg(prm.offsets + lo));
+            }
+            uint32_t rn[4];
+            rng_block(prm.rk, prm.event_base + ev, pidx, 0u, rn);
+            accepted = uniform24(rn[0]) < sc.row_eps[ent >> 11];
+            r1 = rn[1], r2 = rn[2];
+            if (IMPACT) ev_t = prm.event_base + ev, pidx_t = pidx;
+          }
+          // what the tower pass needs: tower | HCAL bit, or "no deposit"
+          s_key[i] = (tower >= 0 && !to_none) ? (unsigned short)((unsigned)tower | (to_ecal ? 0u : 0x8000u)) : (unsigned short)PT_NONE;
+          if (DEBUG) {
+            const long long g = s0 + i;
+            const int row = (int)(ent >> 11);
+            if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)status;
+            if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = live ? eta_from_u(sc, u) : u;
+            if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = phi_pos;
+            if (prm.dbg_tower) prm.dbg_tower[g] = tower;
+            if (prm.dbg_accepted) prm.dbg_accepted[g] = accepted ? 1 : 0;
+            if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)((cls == 2 || !live || row == 31) ? -1 : row);
+            if (prm.dbg_pt_smeared && !accepted) prm.dbg_pt_smeared[g] = 0.f;
+          }
         }
-        // what the tower pass needs: tower | HCAL bit, or "no deposit"
-        s_key[i] = (tower >= 0 && !to_none) ? (unsigned short)((unsigned)tower | (to_ecal ? 0u : 0x8000u)) : (unsigned short)PT_NONE;
-        if (DEBUG) {
-          const long long g = s0 + i;
-          const int row = (int)(ent >> 11);
-          if (prm.dbg_status) prm.dbg_status[g] = (unsigned char)status;
-          if (prm.dbg_eta_pos) prm.dbg_eta_pos[g] = live ? eta_from_u(sc, u) : u;
-          if (prm.dbg_phi_pos) prm.dbg_phi_pos[g] = phi_pos;
-          if (prm.dbg_tower) prm.dbg_tower[g] = tower;
-          if (prm.dbg_accepted) prm.dbg_accepted[g] = accepted ? 1 : 0;
-          if (prm.dbg_eps_row) prm.dbg_eps_row[g] = (signed char)((cls == 2 || !live || row == 31) ? -1 : row);
-          if (prm.dbg_pt_smeared && !accepted) prm.dbg_pt_smeared[g] = 0.f;
+        const unsigned m_acc = __ballot_sync(0xffffffffu, accepted);
+        if (accepted) {
+          // S3 on the spot (the Philox words are in registers); the record goes straight to its parking slot
+          TrackOut t;
+          track_smear_words(sc, px, py, pz, r1, r2, (sc.trk_per_species || sc.n_trk_rows > 0) ? species_of(pid) : 2, t);
+          const long long g = seg0 + run + __popc(m_acc & lt_mask);
+          prm.park_idx[g] = (unsigned char)(i - wbase);
+          prm.park_pid[g] = pid;
+          prm.park_q[g] = s_q[i];
+          prm.park_f[0][g] = t.pt_s, prm.park_f[1][g] = t.eta_mom, prm.park_f[2][g] = t.phi0;
+          prm.park_f[3][g] = t.E_trk, prm.park_f[4][g] = eta_from_u(sc, u), prm.park_f[5][g] = phi_pos;
+          if (IMPACT) {
+            // pd_options.impact: d0, z0 and their errors while the particle is on chip (the stand-alone kernel has to gather it)
+            const ImpactCfg ic{sc.inv_kB, sc.sB, prm.imp_d0_a, prm.imp_d0_b, prm.imp_z0_a, prm.imp_z0_b};
+            float d0m, z0m, sd, sz;
+            track_impact(ic, prm.rk, ev_t, pidx_t, (int)s_q[i], px, py, pz, s_vx[i], s_vy[i], s_vz[i], d0m, z0m, sd, sz);
+            prm.park_imp[0][g] = d0m, prm.park_imp[1][g] = z0m, prm.park_imp[2][g] = sd, prm.park_imp[3][g] = sz;
+          }
+          if (WEIGHTED) prm.park_sig[g] = fast_sqrt(t.rel2) * t.E_trk;  // reading K5 (cards with eflow_weighted only)
+          atomicOr(&s_accmask[i >> 5], 1u << (i & 31));
+          if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[s0 + i] = t.pt_s;
         }
+        run += __popc(m_acc);
       }
-      const unsigned m_acc = __ballot_sync(0xffffffffu, accepted);
-      if (accepted) {
-        // S3 on the spot (the Philox words are in registers); the record goes straight to its parking slot
-        TrackOut t;
-        track_smear_words(sc, px, py, pz, r1, r2, (sc.trk_per_species || sc.n_trk_rows > 0) ? species_of(pid) : 2, t);
-        const long long g = seg0 + run + __popc(m_acc & lt_mask);
-        prm.park_idx[g] = (unsigned char)(i - wbase);
-        prm.park_pid[g] = pid;
-        prm.park_q[g] = s_q[i];
-        prm.park_f[0][g] = t.pt_s, prm.park_f[1][g] = t.eta_mom, prm.park_f[2][g] = t.phi0;
-        prm.park_f[3][g] = t.E_trk, prm.park_f[4][g] = eta_from_u(sc, u), prm.park_f[5][g] = phi_pos;
-        if (IMPACT) {
-          // pd_options.impact: d0, z0 and their errors while the particle is on chip (the stand-alone kernel has to gather it)
-          const ImpactCfg ic{sc.inv_kB, sc.sB, prm.imp_d0_a, prm.imp_d0_b, prm.imp_z0_a, prm.imp_z0_b};
-          float d0m, z0m, sd, sz;
-          track_impact(ic, prm.rk, ev_t, pidx_t, (int)s_q[i], px, py, pz, s_vx[i], s_vy[i], s_vz[i], d0m, z0m, sd, sz);
-          prm.park_imp[0][g] = d0m, prm.park_imp[1][g] = z0m, prm.park_imp[2][g] = sd, prm.park_imp[3][g] = sz;
-        }
-        if (WEIGHTED) prm.park_sig[g] = fast_sqrt(t.rel2) * t.E_trk;  // reading K5 (cards with eflow_weighted only)
-        atomicOr(&s_accmask[i >> 5], 1u << (i & 31));
-        if (DEBUG && prm.dbg_pt_smeared) prm.dbg_pt_smeared[s0 + i] = t.pt_s;
-      }
-      run += __popc(m_acc);
-    }
+    };
+    if (off_axis) rows(std::true_type{});
+    else rows(std::false_type{});
     // the segment's accepted bits (the warp's own mask words: nobody else sets their bits) go beside the parked tracks
     __syncwarp();
     if (lane < PT_ITERS) prm.accmask[(seg0 >> 5) + lane] = s_accmask[wword + lane];
