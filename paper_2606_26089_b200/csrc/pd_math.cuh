@@ -315,15 +315,18 @@ __device__ __forceinline__ uint32_t line_hit(const PdCardScalars &sc, float px, 
   const float apz = fabsf(pz);
   const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
   const float zdist = sc.L - sgnz * vz;  // distance to the endcap the particle flies towards (> 0)
-  const float D = sc.R2 - fmaf(vx, vx, vy * vy);  // > 0
+  // (OFF_AXIS false: vx = vy = 0 for certain -- the terms that vanish are left out; the results are bit for bit those of the
+  // general form)
+  const float D = OFF_AXIS ? sc.R2 - fmaf(vx, vx, vy * vy) : sc.R2;  // > 0
   // t_R = num / den, t_Z = zdist / |pz|
-  const float b = fmaf(vx, px, vy * py);
-  const float sq = fast_sqrt(fmaf(b, b, pt2 * D));
-  const float num = b > 0.f ? D : sq - b;
-  const float den = b > 0.f ? b + sq : pt2;
+  const float b = OFF_AXIS ? fmaf(vx, px, vy * py) : 0.f;
+  const float sq = fast_sqrt(OFF_AXIS ? fmaf(b, b, pt2 * D) : pt2 * D);
+  const float num = (OFF_AXIS && b > 0.f) ? D : (OFF_AXIS ? sq - b : sq);
+  const float den = (OFF_AXIS && b > 0.f) ? b + sq : pt2;
   const bool endcap = apz > 0.f && zdist * den < num * apz;
   const float t = endcap ? zdist * fast_rcp(apz) : num * fast_rcp(den);
-  x = fmaf(t, px, vx), y = fmaf(t, py, vy);
+  if (OFF_AXIS) x = fmaf(t, px, vx), y = fmaf(t, py, vy);
+  else x = t * px, y = t * py;
   z = endcap ? sgnz * sc.L : fmaf(t, pz, vz);
   // rare cases of a vertex far off the axis, redone in double (see line_fix_double); never for vertices on the axis
   if (OFF_AXIS) {
@@ -344,30 +347,30 @@ __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, fl
   const float pt = pt2 * ipt;
   const float apz = fabsf(pz);
   const float sgnz = pz > 0.f ? 1.f : (pz < 0.f ? -1.f : 0.f);
-  const float D = sc.R2 - fmaf(vx, vx, vy * vy);  // > 0
+  const float D = OFF_AXIS ? sc.R2 - fmaf(vx, vx, vy * vy) : sc.R2;  // > 0  (OFF_AXIS false: vx = vy = 0 for certain, see line_hit)
   uint32_t looper = 0;
   const float aq = fabsf((float)q);
   const float rho = aq == 1.f ? pt * sc.inv_kB : pt * sc.inv_kB * fast_rcp(aq);
   const float s = ((q > 0) == (sc.sB > 0.f)) ? -1.f : 1.f;
   const float c0 = px * ipt, s0 = py * ipt;
   // vertex in the (u0, s n0) frame: a = v.u0, b = s v.n0
-  const float a_ = fmaf(vx, c0, vy * s0);
-  const float b_ = s * fmaf(vy, c0, -vx * s0);
+  const float a_ = OFF_AXIS ? fmaf(vx, c0, vy * s0) : 0.f;
+  const float b_ = OFF_AXIS ? s * fmaf(vy, c0, -vx * s0) : 0.f;
   // |v + 2 rho sin h u(phi0 + s h)|^2 = R^2 with t = tan h:  Q t^2 + 2 P t - D = 0   (h = alpha/2)
-  const float P = 2.f * rho * a_;
-  const float Q = fmaf(4.f * rho, rho + b_, -D);
-  const float disc = fmaf(P, P, Q * D);
-  const float scale = fmaf(P, P, 4.f * rho * rho * D);
+  const float P = OFF_AXIS ? 2.f * rho * a_ : 0.f;
+  const float Q = fmaf(4.f * rho, OFF_AXIS ? rho + b_ : rho, -D);
+  const float disc = OFF_AXIS ? fmaf(P, P, Q * D) : Q * D;
+  const float scale = OFF_AXIS ? fmaf(P, P, 4.f * rho * rho * D) : 4.f * rho * rho * D;
   bool reach;
   float cc = 1.f, ss = 0.f;  // (cos, sin) of the barrel half-angle h_R, unnormalised, ss >= 0
   if (disc >= 0.f ? disc < 0.08f * scale : -disc < 1e-3f * scale) {
-    reach = graze_double(sc, px, py, vx, vy, aq, s, cc, ss);
+    reach = graze_double(sc, px, py, OFF_AXIS ? vx : 0.f, OFF_AXIS ? vy : 0.f, aq, s, cc, ss);
   } else {
     reach = disc >= 0.f;
     const float S = fast_sqrt(fmaxf(disc, 0.f));
     // first crossing: (cos h, sin h) proportional to (P + S, D) if P >= 0 else (Q, S - P)
-    cc = P >= 0.f ? P + S : Q;
-    ss = P >= 0.f ? D : S - P;
+    cc = (!OFF_AXIS || P >= 0.f) ? (OFF_AXIS ? P + S : S) : Q;
+    ss = (!OFF_AXIS || P >= 0.f) ? D : S - P;
   }
   if (!reach) looper = PD_LOOPER;
   if (!reach && apz == 0.f) return PD_DROPPED | looper;  // trapped (reading A6)
@@ -404,8 +407,13 @@ __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, fl
   }
   // chord form (pi-periodic in h): position = v + 2 rho sin h u(phi0 + s h)
   const float l2 = 2.f * rho * sh;
-  x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
-  y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
+  if (OFF_AXIS) {
+    x = fmaf(l2, fmaf(c0, ch, -s * s0 * sh), vx);
+    y = fmaf(l2, fmaf(s0, ch, s * c0 * sh), vy);
+  } else {
+    x = l2 * fmaf(c0, ch, -s * s0 * sh);
+    y = l2 * fmaf(s0, ch, s * c0 * sh);
+  }
   // the three rare cases of a vertex far off the axis (OFF_AXIS: false in the copy of the row loop that a warp whose vertices all sit on the
   // axis -- every workload of BASELINE.json -- which then skips the tests as well)
   if (OFF_AXIS) {

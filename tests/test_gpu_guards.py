@@ -116,3 +116,29 @@ def test_after_card_upload_a_step_allocates_no_device_memory():
     free1, _ = torch.cuda.mem_get_info()
     assert pd.last_status(out) == 0 and int(out.trk["offsets"][-1]) > 0
     assert free1 == free0, (free0, free1)
+
+
+def test_the_on_axis_copy_of_the_row_loop_is_bitwise_the_general_one():
+    """Kernel P keeps two copies of its row loop: warps whose vertices all sit on the beam axis take one in which the terms that
+    vanish for vx = vy = 0 are left out.  A vertex 1e-20 m off the axis on every 50th particle sends (nearly) every warp through
+    the general copy instead: the positions, towers and decisions of all the OTHER particles must not change by a bit."""
+    import paper_2606_26089_b200 as pd
+
+    for card_name, cfg, ne in (("cms_like", 0, 600), ("cms_like", 2, 6), ("aleph_like", 4, 900)):
+        ev = wl.generate(cfg, ne)
+        assert not ev.vx.any() and not ev.vy.any()
+        nudged = np.zeros(ev.n_particles, dtype=bool)
+        nudged[::50] = True
+        vx = ev.vx.copy()
+        vx[nudged] = np.float32(1e-20)
+        ev2 = wl.Events(offsets=ev.offsets, **{k: (vx if k == "vx" else getattr(ev, k)) for k in ("pid", "charge", "px", "py", "pz", "E", "vx", "vy", "vz")})
+        res = []
+        for e in (ev, ev2):
+            card = pd.Card(card_name)
+            dev = pd.DeviceEvents(e)
+            out = pd.DeviceOutputs(card, dev.n_events, dev.n_particles, debug=True)
+            pd.simulate(card, dev, out, 23)
+            res.append(out.to_numpy())
+        for k in ("dbg_status", "dbg_eta_pos", "dbg_phi_pos", "dbg_tower", "dbg_accepted", "dbg_pt_smeared"):
+            a, b = res[0][k][~nudged], res[1][k][~nudged]
+            assert a.tobytes() == b.tobytes(), (card_name, cfg, k)
