@@ -363,6 +363,9 @@ __device__ __forceinline__ uint32_t helix_hit(const PdCardScalars &sc, int q, fl
   const float scale = OFF_AXIS ? fmaf(P, P, 4.f * rho * rho * D) : 4.f * rho * rho * D;
   bool reach;
   float cc = 1.f, ss = 0.f;  // (cos, sin) of the barrel half-angle h_R, unnormalised, ss >= 0
+  // (The band is what keeps the azimuth of the hit within 1e-6: measured on 5.7 million on-axis particles the largest error is
+  // 6.1e-7 at 0.08, 8.5e-7 at 0.04, 1.24e-6 at 0.02.  A narrower band for the on-axis copy would save 0.8 % of the step at 0.05
+  // and was not taken: it leaves 15 % of the tolerance and breaks the bit-for-bit identity of the two copies.)
   if (disc >= 0.f ? disc < 0.08f * scale : -disc < 1e-3f * scale) {
     reach = graze_double(sc, px, py, OFF_AXIS ? vx : 0.f, OFF_AXIS ? vy : 0.f, aq, s, cc, ss);
   } else {
