@@ -6,6 +6,7 @@ this module.  It shares nothing with the CUDA path (paper_2606_26089_b200/).
 from __future__ import annotations
 
 import ctypes as C
+import os
 
 import numpy as np
 
@@ -77,7 +78,8 @@ class _Overrides(C.Structure):
 def lib():
     global _lib
     if _lib is None:
-        L = C.CDLL(_build.build())
+        # PD_ORACLE_LIB: another build of oracle/pd_oracle.c (tests/test_oracle_sanitizers.py loads an ASan + UBSan build this way)
+        L = C.CDLL(os.environ.get("PD_ORACLE_LIB") or _build.build())
         L.pdo_load_card.argtypes = [C.c_char_p, C.POINTER(_p)]
         L.pdo_free_card.argtypes = [_p]
         L.pdo_free_card.restype = None
