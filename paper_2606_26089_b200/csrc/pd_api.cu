@@ -224,7 +224,7 @@ int pd_pileup_merge(const pd_events *hs, const pd_events *pool, const pd_pileup_
   return PD_OK;
 }
 
-// filter workspace: [tile counter, pad] 16 B | look-back words, one per tile | exclusive ranks of positions 0..capacity
+// filter workspace: [tile counter, pad] 16 B | look-back words, one per tile | one 64-bit word per 32 positions 0..capacity
 static size_t filter_chain_bytes(int64_t capacity) {
   const size_t tiles = (size_t)((capacity + 1 + PD_FILTER_TILE - 1) / PD_FILTER_TILE);
   return (16 + 8 * tiles + 255) & ~size_t(255);
@@ -232,7 +232,7 @@ static size_t filter_chain_bytes(int64_t capacity) {
 
 int64_t pd_filter_workspace_bytes(int64_t capacity) {
   if (capacity < 0) return PD_EINVAL;
-  return (int64_t)(filter_chain_bytes(capacity) + 4 * (size_t)(capacity + 1));
+  return (int64_t)(filter_chain_bytes(capacity) + 8 * (size_t)((capacity + 1 + 31) / 32));
 }
 
 int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *conds, int32_t n_conds, int32_t combine_any,
@@ -268,7 +268,11 @@ int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *co
   unsigned char *ws = (unsigned char *)workspace;
   p.tile_counter = (unsigned int *)ws;
   p.chain = (unsigned long long *)(ws + 16);
-  p.rank = (int *)(ws + chain_bytes);
+  p.wordrank = (unsigned long long *)(ws + chain_bytes);
+  uintptr_t bits = 0;
+  for (const void *a : {(const void *)in->cls, (const void *)in->src, (const void *)in->pt, (const void *)in->eta, (const void *)in->phi, (const void *)in->E})
+    bits |= reinterpret_cast<uintptr_t>(a);
+  p.aligned16 = (bits & 15u) == 0;
   const int rc = pd_launch_filter(p, cuda_stream);
   if (rc != PD_OK) return cuda_fail(cudaGetLastError(), "filter kernel launch");
   t_launches = 2;

@@ -240,7 +240,8 @@ struct PdFilterParams {
   int n_conds, combine_any;
   unsigned int *tile_counter;     // workspace: next tile
   unsigned long long *chain;      // workspace: look-back word per tile
-  int *rank;                      // workspace: exclusive rank of every input position 0..n
+  unsigned long long *wordrank;   // workspace, per 32 input positions (0..n): survivor bits | rank of the first << 32
+  int aligned16;                  // all six input arrays start at a multiple of 16 bytes (bulk copies)
 };
 int pd_launch_filter(const PdFilterParams &prm, void *stream);
 

@@ -81,6 +81,54 @@ def test_ragged_tile_boundaries_and_features_of_survivors():
             assert np.all(np.abs(g["r_iso"] - r["r_iso"])[ok] <= np.maximum(1e-5 * r["r_iso"], 1e-6)[ok])
 
 
+def test_unaligned_arrays_nan_fields_and_many_tiles():
+    """arrays that do not start at a multiple of 16 bytes (every tile then comes by plain loads instead of bulk copies) give the same
+    survivors as aligned ones; NaN in a field fails every ordered comparison and == / "in", passes != / "not in" (the C operators
+    the oracle applies); 40 tiles and a ragged tail"""
+    import paper_2606_26089_b200 as pd
+    from oracle import pdo
+    from paper_2606_26089_b200 import binding as B
+
+    torch = B._torch()
+    rng = np.random.default_rng(11)
+    sizes = rng.integers(0, 90, 1900)
+    off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    n = int(off[-1])
+    assert n > 40 * 2048 and n % 2048 not in (0, 1)
+    arrays = {"offsets": off, "cls": rng.integers(0, 5, n).astype(np.int8), "src": rng.integers(0, 1 << 20, n).astype(np.int32),
+              "pt": (0.1 * 1000 ** rng.random(n)).astype(np.float32), "eta": rng.uniform(-4, 4, n).astype(np.float32),
+              "phi": rng.uniform(-np.pi, np.pi, n).astype(np.float32), "E": rng.random(n).astype(np.float32) * 100}
+    for k in ("pt", "eta", "phi", "E"):
+        arrays[k][rng.integers(0, n, 500)] = np.nan
+    arrays["E"][rng.integers(0, n, 500)] = 30.0  # equality cases of <=, ==, "in"
+    sets = SETS + [
+        ([{"field": "E", "op": "!=", "value": 30.0}], "all"),
+        ([{"field": "E", "op": "==", "value": 30.0}, {"field": "eta", "op": ">", "value": 3.9}], "any"),
+        ([{"field": "E", "op": "in", "value": [30.0, 12.0]}], "all"),
+        ([{"field": "E", "op": "not in", "value": [30.0]}, {"field": "phi", "op": "<=", "value": -1.0, "abs": False}], "all"),
+        ([{"field": "eta", "op": ">=", "value": 1.0, "abs": True}, {"field": "cls", "op": "==", "value": 2}], "all"),
+    ]
+    ne = len(off) - 1
+    for conds, comb in sets:
+        ref = pdo.filter_eflow(off, arrays["cls"], arrays["src"], arrays["pt"], arrays["eta"], arrays["phi"], arrays["E"], conds, comb)
+        got, _ = _gpu(arrays, conds, comb)
+        _same(got, ref)
+        # the same input one element into larger buffers: 4 bytes (1 for cls) past a 16-byte boundary
+        src = pd.DeviceEFlow(ne, n, arrays)
+        keep = []
+        for k, _dt in B.EFLOW_FIELDS:
+            big = torch.empty(n + 1, dtype=src.t[k].dtype, device="cuda")
+            big[1:].copy_(src.t[k][:n])
+            keep.append(big)
+            src.t[k] = big[1:]
+            assert src.t[k].data_ptr() % 16 != 0
+        src.c_efl = B.EFlow(src.capacity, B._tptr(src.t["offsets"]), *[B._tptr(src.t[k]) for k, _dt in B.EFLOW_FIELDS])
+        dst = pd.DeviceEFlow(ne, n)
+        ws = pd.filter_eflow(src, dst, conds, comb)
+        _same(dst.to_numpy(), ref)
+        del ws, keep
+
+
 def test_argument_checks():
     import ctypes as C
 
