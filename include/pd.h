@@ -203,6 +203,8 @@ int64_t pd_filter_workspace_bytes(int64_t capacity);
 /* in, out: structs in HOST memory whose pointer members are DEVICE pointers (in->offsets [n_events+1]; the number
  * of objects is read on the device).  out->capacity >= in->capacity; out->offsets [n_events+1]; in and out must
  * not overlap.  conds: HOST array.  Asynchronous on cuda_stream, two kernel launches, allocates nothing.
+ * The input arrays may start anywhere; when all six start at a multiple of 16 bytes the tiles are staged by bulk copies
+ * (the fast path).  A NaN field fails >, >=, <, <=, ==, "in" and passes !=, "not in".
  * Errors: PD_EINVAL (null pointers, bad field / op / counts), PD_ECAPACITY, PD_EWORKSPACE, PD_ECUDA. */
 int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *conds, int32_t n_conds, int32_t combine_any,
                     pd_eflow *out, void *workspace, int64_t workspace_bytes, void *cuda_stream);
