@@ -188,7 +188,7 @@ __device__ __forceinline__ void run_features(const PdFeatParams &prm, PF o_pt, P
       const int i = active ? (int)s_lep[k] : 0;
       const float eta_i = o_eta[i], phi_i = o_phi[i];
       // pieces [b0, b0 + n0), [b1, ...), ...: positions in s_idx (listed) or object indices (one event of a multi-event run)
-      int b0 = 0, n0 = 0, b1 = 0, n1 = 0, b2 = 0, n2 = 0, b3 = 0, n3 = 0;
+      int b0 = 0, n0 = 0, b1 = 0, n1 = 0, b2 = 0, n2 = 0, b3 = 0;
       if (active) {
         if (listed) {
           const int st = eta_strip(eta_i, prm.inv_strip), pc = phi_cell(phi_i, prm), np = prm.n_phi;
