@@ -180,69 +180,117 @@ __global__ void __launch_bounds__(256) pd_pileup_scan_kernel(const __grid_consta
 
 // A 256-thread CTA per merged event.  Warp 0 lists the event's sources (the hard scatter, then the n picked pool
 // events): start and length in their input batch, vertex shift, and -- by a warp scan -- where each lands in the
-// output; then the eight warps copy the sources side by side.
+// output; the warps copy the sources side by side.  The list of a CTA's NEXT event is made (a chain of dependent
+// loads: pick -> offsets -> scan, no traffic to speak of) while the other seven warps copy the current one, in a second set
+// of list arrays; warp 0 joins the copy when its list is done (sources are handed out by a counter).
+constexpr int UNR = 2;            // positions per lane in flight
 constexpr int MAX_SOURCES = 768;  // n_max + 1 <= ceil(500 + 10 sqrt(500) + 20) + 1 = 745
+struct SourceList {
+  long long a[MAX_SOURCES];  // first particle in its input batch
+  int ro[MAX_SOURCES];       // first position in the merged event
+  float dz[MAX_SOURCES], dt[MAX_SOURCES];
+  int total;                 // particles of the merged event
+};
 __global__ void __launch_bounds__(256) pd_pileup_fill_kernel(const __grid_constant__ PdPileupParams prm) {
-  __shared__ long long s_a[MAX_SOURCES], s_o[MAX_SOURCES];
-  __shared__ int s_len[MAX_SOURCES];
-  __shared__ float s_dz[MAX_SOURCES];
-  __shared__ float s_dt[MAX_SOURCES];
+  __shared__ SourceList s_list[2];
+  __shared__ int s_next[2];  // next source of the list to hand out
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   if (prm.out_off[prm.n_hs] > prm.capacity) return;  // reported by the scan kernel through the status word
-  for (long long e = blockIdx.x; e < prm.n_hs; e += gridDim.x) {
+  auto list_sources = [&](long long e, SourceList &L) {  // warp 0
     const long long event = prm.event_base + e;
     const int n_src = prm.n_pileup[e] + 1;
-    __syncthreads();  // the previous event's lists are no longer read
+    int run = 0;
+    for (int s0 = 0; s0 < n_src; s0 += 32) {
+      const int s = s0 + lane;  // source s: block s of the event's stream (0 = the hard scatter)
+      long long a = 0;
+      int len = 0;
+      float dz = 0.f, dt = 0.f;
+      if (s < n_src) {
+        uint32_t r[4];
+        rng_block2(prm.rk, event, (uint32_t)s, r);
+        if (s == 0) {
+          a = __ldg(prm.hs_off + e), len = (int)(__ldg(prm.hs_off + e + 1) - a);
+          dz = prm.smear_hs ? truncated_z(prm, r[1]) : 0.f;
+          dt = prm.smear_hs ? truncated_t(prm, r[2]) : 0.f;
+        } else {
+          const long long j = pool_pick(prm, r[0]);
+          a = __ldg(prm.pool_off + j), len = (int)(__ldg(prm.pool_off + j + 1) - a);
+          dz = truncated_z(prm, r[1]);
+          dt = truncated_t(prm, r[2]);
+        }
+      }
+      int incl = len;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+      }
+      if (s < n_src) L.a[s] = a, L.dz[s] = dz, L.dt[s] = dt, L.ro[s] = run + (incl - len);
+      run += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    if (lane == 0) L.total = run;
+  };
+  long long e = blockIdx.x;
+  if (e >= prm.n_hs) return;
+  if (wid == 0) list_sources(e, s_list[0]);
+  if (tid == 0) s_next[0] = 0;
+  __syncthreads();
+  for (int buf = 0; e < prm.n_hs; e += gridDim.x, buf ^= 1) {
+    const int n_src = prm.n_pileup[e] + 1;
+    const SourceList &L = s_list[buf];
     if (wid == 0) {
-      long long run = prm.out_off[e];
-      for (int s0 = 0; s0 < n_src; s0 += 32) {
-        const int s = s0 + lane;  // source s: block s of the event's stream (0 = the hard scatter)
-        long long a = 0;
-        int len = 0;
-        float dz = 0.f, dt = 0.f;
-        if (s < n_src) {
-          uint32_t r[4];
-          rng_block2(prm.rk, event, (uint32_t)s, r);
-          if (s == 0) {
-            a = __ldg(prm.hs_off + e), len = (int)(__ldg(prm.hs_off + e + 1) - a);
-            dz = prm.smear_hs ? truncated_z(prm, r[1]) : 0.f;
-            dt = prm.smear_hs ? truncated_t(prm, r[2]) : 0.f;
-          } else {
-            const long long j = pool_pick(prm, r[0]);
-            a = __ldg(prm.pool_off + j), len = (int)(__ldg(prm.pool_off + j + 1) - a);
-            dz = truncated_z(prm, r[1]);
-            dt = truncated_t(prm, r[2]);
-          }
-        }
-        int incl = len;
+      if (e + gridDim.x < prm.n_hs) list_sources(e + gridDim.x, s_list[buf ^ 1]);
+      if (lane == 0) s_next[buf ^ 1] = 0;
+    }
+    // the merged event position by position (every lane busy, stores coalesced), in chunks of 32 * UNR positions handed out by
+    // a counter; a position's source is the last one that starts at or before it
+    const long long o0 = prm.out_off[e];
+    const int total = L.total;
+    for (;;) {
+      int c = 0;
+      if (lane == 0) c = atomicAdd(&s_next[buf], 1);
+      c = __shfl_sync(0xffffffffu, c, 0);
+      if (c * (32 * UNR) >= total) break;
+      int k[UNR], src[UNR];
+      long long from[UNR];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const int t = __shfl_up_sync(0xffffffffu, incl, o);
-          if (lane >= o) incl += t;
+      for (int u = 0; u < UNR; ++u) {
+        k[u] = c * (32 * UNR) + u * 32 + lane;
+        int lo = 0, hi = n_src;
+        const int kk = min(k[u], total - 1);
+        while (hi - lo > 1) {
+          const int mid = (lo + hi) >> 1;
+          if (L.ro[mid] <= kk) lo = mid;
+          else hi = mid;
         }
-        if (s < n_src) s_a[s] = a, s_len[s] = len, s_dz[s] = dz, s_dt[s] = dt, s_o[s] = run + (incl - len);
-        run += __shfl_sync(0xffffffffu, incl, 31);
+        src[u] = lo, from[u] = L.a[lo] + (kk - L.ro[lo]);
+      }
+      int v_pid[UNR];
+      signed char v_q[UNR];
+      float v_f[UNR][7];
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) {
+        const bool pu = src[u] > 0;
+        v_pid[u] = __ldg((pu ? prm.pool_pid : prm.hs_pid) + from[u]);
+        v_q[u] = __ldg((pu ? prm.pool_charge : prm.hs_charge) + from[u]);
+#pragma unroll
+        for (int f = 0; f < 7; ++f) v_f[u][f] = __ldg((pu ? prm.pool_f[f] : prm.hs_f[f]) + from[u]);
+      }
+#pragma unroll
+      for (int u = 0; u < UNR; ++u) {
+        if (k[u] < total) {
+          const long long d = o0 + k[u];
+          prm.out_pid[d] = v_pid[u];
+          prm.out_charge[d] = v_q[u];
+#pragma unroll
+          for (int f = 0; f < 6; ++f) prm.out_f[f][d] = v_f[u][f];
+          prm.out_f[6][d] = v_f[u][6] + L.dz[src[u]];
+          prm.is_pu[d] = src[u] > 0 ? 1 : 0;
+          if (prm.out_vt) prm.out_vt[d] = L.dt[src[u]];
+        }
       }
     }
-    __syncthreads();
-    for (int s = wid; s < n_src; s += 8) {
-      const bool pu = s > 0;
-      const long long a = s_a[s], o = s_o[s];
-      const int len = s_len[s];
-      const float dz = s_dz[s], dt = s_dt[s];
-      const int *src_pid = pu ? prm.pool_pid : prm.hs_pid;
-      const signed char *src_q = pu ? prm.pool_charge : prm.hs_charge;
-      for (int i = lane; i < len; i += 32) {
-        const long long d = o + i;
-        prm.out_pid[d] = __ldg(src_pid + a + i);
-        prm.out_charge[d] = __ldg(src_q + a + i);
-#pragma unroll
-        for (int f = 0; f < 6; ++f) prm.out_f[f][d] = __ldg((pu ? prm.pool_f[f] : prm.hs_f[f]) + a + i);
-        prm.out_f[6][d] = __ldg((pu ? prm.pool_f[6] : prm.hs_f[6]) + a + i) + dz;
-        prm.is_pu[d] = pu ? 1 : 0;
-        if (prm.out_vt) prm.out_vt[d] = dt;
-      }
-    }
+    __syncthreads();  // the next list is complete, this one no longer read
   }
 }
 
@@ -260,8 +308,10 @@ int pd_launch_pileup(const PdPileupParams &prm, void *stream) {
   if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
   pdm::pd_pileup_scan_kernel<<<4 * sms, 256, 0, st>>>(prm);
   if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
-  long long fb = prm.n_hs;  // a CTA per event
-  if (fb > 8LL * sms) fb = 8LL * sms;
+  int per_sm = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pdm::pd_pileup_fill_kernel, 256, 0) != cudaSuccess || per_sm < 1) return PD_ECUDA;
+  long long fb = prm.n_hs;  // a CTA per event at a time
+  if (fb > (long long)per_sm * sms) fb = (long long)per_sm * sms;
   if (fb < 1) fb = 1;
   pdm::pd_pileup_fill_kernel<<<(unsigned)fb, 256, 0, st>>>(prm);
   return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
