@@ -79,20 +79,32 @@ __device__ __forceinline__ long long pool_pick(const PdPileupParams &prm, uint32
   return (long long)(((unsigned long long)(r0 >> 8) * (unsigned long long)prm.n_pool) >> 24);
 }
 
+// eight lanes per event: the picks of an event are independent draws, each a chain of dependent loads (pick -> two offsets)
 __global__ void __launch_bounds__(256) pd_pileup_count_kernel(const __grid_constant__ PdPileupParams prm) {
-  for (long long e = blockIdx.x * 256LL + threadIdx.x; e < prm.n_hs; e += 256LL * gridDim.x) {
-    const long long event = prm.event_base + e;
-    uint32_t r[4];
-    rng_block2(prm.rk, event, 0u, r);
-    const int n = poisson_inverse(prm, r[0]);
-    long long cnt = __ldg(prm.hs_off + e + 1) - __ldg(prm.hs_off + e);
-    for (int k = 0; k < n; ++k) {
-      rng_block2(prm.rk, event, (uint32_t)(1 + k), r);
-      const long long j = pool_pick(prm, r[0]);
-      cnt += __ldg(prm.pool_off + j + 1) - __ldg(prm.pool_off + j);
+  const int sub = threadIdx.x & 7;
+  const long long groups = 32LL * gridDim.x;  // groups of eight lanes in the grid
+  const long long rounds = (prm.n_hs + groups - 1) / groups;  // the same for every lane: the shuffles below need whole warps
+  long long e = blockIdx.x * 32LL + (threadIdx.x >> 3);
+  for (long long it = 0; it < rounds; ++it, e += groups) {
+    const bool valid = e < prm.n_hs;
+    int n = 0;
+    long long cnt = 0;
+    if (valid) {
+      const long long event = prm.event_base + e;
+      uint32_t r[4];
+      rng_block2(prm.rk, event, 0u, r);
+      n = poisson_inverse(prm, r[0]);
+      if (sub == 0) cnt = __ldg(prm.hs_off + e + 1) - __ldg(prm.hs_off + e);
+      for (int k = sub; k < n; k += 8) {
+        rng_block2(prm.rk, event, (uint32_t)(1 + k), r);
+        const long long j = pool_pick(prm, r[0]);
+        cnt += __ldg(prm.pool_off + j + 1) - __ldg(prm.pool_off + j);
+      }
     }
-    prm.n_pileup[e] = n;
-    prm.cnt[e] = cnt;
+    cnt += __shfl_xor_sync(0xffffffffu, cnt, 1);
+    cnt += __shfl_xor_sync(0xffffffffu, cnt, 2);
+    cnt += __shfl_xor_sync(0xffffffffu, cnt, 4);
+    if (valid && sub == 0) prm.n_pileup[e] = n, prm.cnt[e] = cnt;
   }
 }
 
@@ -301,7 +313,7 @@ int pd_launch_pileup(const PdPileupParams &prm, void *stream) {
   if (cudaGetDevice(&dev) != cudaSuccess) return PD_ECUDA;
   if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PD_ECUDA;
   cudaStream_t st = (cudaStream_t)stream;
-  long long blocks = (prm.n_hs + 255) / 256;
+  long long blocks = (prm.n_hs + 31) / 32;  // eight lanes per event
   if (blocks > 8LL * sms) blocks = 8LL * sms;
   if (blocks < 1) blocks = 1;
   pdm::pd_pileup_count_kernel<<<(unsigned)blocks, 256, 0, st>>>(prm);
