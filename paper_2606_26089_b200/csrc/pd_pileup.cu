@@ -1,12 +1,13 @@
 // pd_pileup.cu -- pile-up merging, the step right before the detector-response chain (Listing 8
 // L541-567, Table C.9; readings H1-H6 of DESIGN.md section 12).  Product code;
 // shares nothing with oracle/.
-//   kernel 1 (count)  a thread per hard-scatter event: Poisson draw, pool picks, size of the merged event
+//   kernel 1 (count)  eight lanes per hard-scatter event: Poisson draw, pool picks, size of the merged event
 //   kernel 2 (scan)   exclusive prefix of the sizes = CSR offsets of the output (decoupled look-back over
 //                     tiles of 1,024 events claimed from an atomic counter)
-//   kernel 3 (fill)   a CTA per event: warp 0 lists the sources (hard scatter, then every picked pool event) and
-//                     scans their sizes, the eight warps copy them side by side with coalesced loads and stores;
-//                     vz shifted by the source's truncated-normal draw
+//   kernel 3 (fill)   a CTA per event at a time: warp 0 lists the sources (hard scatter, then every picked pool event) and
+//                     scans their sizes; the merged event is then written position by position (a position's source by
+//                     binary search in the list; coalesced stores), vz shifted by the source's truncated-normal draw,
+//                     while warp 0 lists the CTA's next event
 // The random numbers are recomputed from their counters where they are needed (Philox4x32-10, stream 2).
 #include <cuda_runtime.h>
 
