@@ -10,7 +10,8 @@
 // from global memory).  Three ways to sum, chosen per tile: fewer than 8 events -> every event's segment is cut into
 // 8 pieces, one per warp; 8..31 events -> a warp per event; 32 or more -> a thread per event.  Sums are 64-bit fixed
 // point (units of 2^-32 GeV: associative, so the result does not depend on tiles, pieces, batching or the order of
-// the atomics) and are added to the event's three accumulators in the workspace with 64-bit atomics.
+// the atomics) and are added to the event's three accumulators in the workspace with 64-bit atomics.  A tile that lies in
+// one or two events (events of thousands of particles) skips the staging: sums in registers, a warp sum, atomics.
 // Kernel 2: accumulators -> fp32 outputs.
 #include <cuda_runtime.h>
 
@@ -56,6 +57,9 @@ __device__ __forceinline__ long long find_event_warp(const long long *off, long 
   return lo;
 }
 
+// FAST: with the register path for tiles that lie in one or two events (chosen by the host for batches of events of thousands
+// of particles; compiled out otherwise: batches of small events lose 30 % to its registers and its two extra loads per tile)
+template <bool FAST>
 __global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_constant__ PdTruthParams prm) {
   __shared__ __align__(16) float s_pt[TILE], s_px[TILE], s_py[TILE];
   __shared__ int s_off[THREADS + 1];  // offsets of the events e_cur .. e_cur + THREADS, relative to the tile, clamped
@@ -79,7 +83,7 @@ __global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_c
   constexpr int GROUPS = ITEMS / 4;
   float4 r_px[GROUPS], r_py[GROUPS];
   int4 r_pid[GROUPS];
-  long long w0, w1;
+  long long w0, w1, wb = 0, wc = 0;  // wb, wc: where the tile's second and third event start (the same for every thread)
   const bool vec_ok = ((reinterpret_cast<uintptr_t>(prm.px) | reinterpret_cast<uintptr_t>(prm.py) | reinterpret_cast<uintptr_t>(prm.pid)) & 15) == 0;
   auto load_tile = [&](long long tile, long long e_first) {
     const long long t0 = tile * TILE;
@@ -106,6 +110,7 @@ __global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_c
     }
     const long long ke = min(e_first + tid, ne);
     w0 = __ldg(prm.ev_off + ke), w1 = __ldg(prm.ev_off + min(ke + 1, ne));
+    if (FAST) wb = __ldg(prm.ev_off + min(e_first + 1, ne)), wc = __ldg(prm.ev_off + min(e_first + 2, ne));
   };
   auto visible = [&](int pid) {
     const int a = abs(pid);
@@ -115,6 +120,42 @@ __global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_c
   for (long long tile = tile_b; tile < tile_e; ++tile) {
     const long long t0 = tile * TILE, t1 = min(t0 + (long long)TILE, n) - 1;
     const int len = (int)(t1 - t0 + 1);
+    if (FAST && wc > t1) {
+      // ---- the tile lies in one or two events (events of thousands of particles): no staging, no barrier -- every thread sums
+      // its eight particles in registers, on the side of the boundary they fall on; a warp sum; three atomics per warp and event
+      const int bpos = (int)max(min(wb - t0, (long long)len), 0LL);  // first position of the second event
+      long long hA = 0, xA = 0, yA = 0, hB = 0, xB = 0, yB = 0;
+#pragma unroll
+      for (int g = 0; g < GROUPS; ++g) {
+        const int j = (g * THREADS + tid) * 4;  // positions >= len hold zeros
+        const float px4[4] = {r_px[g].x, r_px[g].y, r_px[g].z, r_px[g].w}, py4[4] = {r_py[g].x, r_py[g].y, r_py[g].z, r_py[g].w};
+        const int pid4[4] = {r_pid[g].x, r_pid[g].y, r_pid[g].z, r_pid[g].w};
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const bool vis = visible(pid4[c]);
+          const float x = vis ? px4[c] : 0.f, y = vis ? py4[c] : 0.f;
+          const long long fh = to_fix(sqrt_approx(fmaf(x, x, y * y))), fx = to_fix(x), fy = to_fix(y);
+          if (j + c < bpos) hA += fh, xA += fx, yA += fy;
+          else hB += fh, xB += fx, yB += fy;
+        }
+      }
+      const long long e_last = wb <= t1 ? e_cur + 1 : e_cur;
+      if (tile + 1 < tile_e) load_tile(tile + 1, e_last);  // in flight during the reductions and the next iteration's start
+      hA = warp_sum_ll(hA), xA = warp_sum_ll(xA), yA = warp_sum_ll(yA);
+      if (lane < 3) {
+        const long long v = lane == 0 ? hA : (lane == 1 ? xA : yA);
+        if (v != 0) atomicAdd(prm.acc + 3 * e_cur + lane, (unsigned long long)v);
+      }
+      if (e_last != e_cur) {
+        hB = warp_sum_ll(hB), xB = warp_sum_ll(xB), yB = warp_sum_ll(yB);
+        if (lane < 3) {
+          const long long v = lane == 0 ? hB : (lane == 1 ? xB : yB);
+          if (v != 0) atomicAdd(prm.acc + 3 * e_last + lane, (unsigned long long)v);
+        }
+      }
+      e_cur = e_last;
+      continue;
+    }
     __syncthreads();  // the previous tile's sums are done with the staging arrays
     if (tid == 0) s_found = 0;
 #pragma unroll
@@ -222,7 +263,8 @@ int pd_launch_truth(const PdTruthParams &prm, void *stream) {
   if (prm.n_particles > 0) {
     long long blocks = (prm.n_particles + pdt::TILE - 1) / pdt::TILE;
     if (blocks > 4LL * sms) blocks = 4LL * sms;
-    pdt::pd_truth_sum_kernel<<<(unsigned)blocks, pdt::THREADS, 0, st>>>(prm);
+    if (prm.n_particles >= 2048 * prm.n_events) pdt::pd_truth_sum_kernel<true><<<(unsigned)blocks, pdt::THREADS, 0, st>>>(prm);
+    else pdt::pd_truth_sum_kernel<false><<<(unsigned)blocks, pdt::THREADS, 0, st>>>(prm);
     if (cudaGetLastError() != cudaSuccess) return PD_ECUDA;
   }
   long long blocks = (prm.n_events + 255) / 256;

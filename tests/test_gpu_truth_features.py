@@ -77,6 +77,31 @@ def test_ragged_events_tile_boundaries_and_edge_cases():
     assert _run_gpu(_random_events(7, []))["ht"].shape == (0,)
 
 
+def test_batches_of_huge_events_take_the_register_path():
+    """batches whose events average 2,048 particles or more run the kernel variant with the register path (tiles that lie in one or
+    two events); its sums are the same exact fixed-point sums: against the oracle, and bit for bit against the other variant, which
+    the same events get when enough empty events are appended to bring the average down"""
+    from oracle import pdo
+
+    # boundaries exactly on, one before and one after a tile edge; runs of tiny and empty events between huge ones (those tiles take
+    # the staged path inside the same kernel); a last event that ends mid-tile
+    sizes = [5000, 0, 0, 3, 7000, 1, 2, 2, 6000, 4096, 2048, 2047, 2049, 10000, 0, 12288, 4095, 1, 20000, 6001] + [3000] * 7 + [9000, 0, 0]
+    assert sum(sizes) >= 2048 * len(sizes)
+    ev = _random_events(21, sizes)
+    for skip in (True, False):
+        g = _run_gpu(ev, skip)
+        _check(g, pdo.truth_features(ev, skip))
+        padded = _random_events(21, sizes + [0] * 100)  # the same particles (same seed and sizes first), average below 2,048
+        assert padded.px[: ev.n_particles].tobytes() == ev.px.tobytes()
+        h = _run_gpu(padded, skip)
+        for k in g:
+            assert h[k][: len(sizes)].tobytes() == g[k].tobytes(), k
+    # one event only; two events split inside a tile; a batch that ends exactly on a tile edge
+    for sz in ([30000], [3000, 3100], [2048, 2048, 4096]):
+        ev = _random_events(22, sz)
+        _check(_run_gpu(ev), pdo.truth_features(ev))
+
+
 def test_bitwise_reproducible_and_independent_of_batching():
     ev = _random_events(9, np.random.default_rng(2).poisson(300, 4000))
     a, b = _run_gpu(ev), _run_gpu(ev)
