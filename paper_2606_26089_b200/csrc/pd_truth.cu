@@ -112,9 +112,11 @@ __global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_c
     w0 = __ldg(prm.ev_off + ke), w1 = __ldg(prm.ev_off + min(ke + 1, ne));
     if (FAST) wb = __ldg(prm.ev_off + min(e_first + 1, ne)), wc = __ldg(prm.ev_off + min(e_first + 2, ne));
   };
+  // |pid| in {12, 14, 16} as a bit test (bits 12, 14, 16 of the mask; no bits when neutrinos count)
+  const unsigned nu_mask = prm.skip_neutrinos ? 0x15000u : 0u;
   auto visible = [&](int pid) {
-    const int a = abs(pid);
-    return !(prm.skip_neutrinos && (a == 12 || a == 14 || a == 16));
+    const unsigned a = (unsigned)abs(pid);
+    return !(a < 32u && ((nu_mask >> a) & 1u));
   };
   load_tile(tile_b, e_cur);
   for (long long tile = tile_b; tile < tile_e; ++tile) {
@@ -135,7 +137,7 @@ __global__ void __launch_bounds__(THREADS, 4) pd_truth_sum_kernel(const __grid_c
           const bool vis = visible(pid4[c]);
           const float x = vis ? px4[c] : 0.f, y = vis ? py4[c] : 0.f;
           const long long fh = to_fix(sqrt_approx(fmaf(x, x, y * y))), fx = to_fix(x), fy = to_fix(y);
-          if (j + c < bpos) hA += fh, xA += fx, yA += fy;
+          if (j + c < bpos) hA += fh, xA += fx, yA += fy;  // (sums per group of four first, one branch per group: slower, spills)
           else hB += fh, xB += fx, yB += fy;
         }
       }
