@@ -263,7 +263,7 @@ int pd_filter_eflow(const pd_eflow *in, int64_t n_events, const pd_condition *co
   p.cls = in->cls, p.src = in->src, p.pt = in->pt, p.eta = in->eta, p.phi = in->phi, p.E = in->E;
   p.out_offsets = (long long *)out->offsets;
   p.out_cls = out->cls, p.out_src = out->src, p.out_pt = out->pt, p.out_eta = out->eta, p.out_phi = out->phi, p.out_E = out->E;
-  for (int k = 0; k < n_conds; ++k) p.conds[k] = conds[k];
+  for (int k = 0; k < n_conds; ++k) p.conds[k] = conds[k], p.cond_fields |= 1u << conds[k].field;
   p.n_conds = n_conds, p.combine_any = combine_any ? 1 : 0;
   unsigned char *ws = (unsigned char *)workspace;
   p.tile_counter = (unsigned int *)ws;

@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(THREADS, 4) pd_filter_kernel(const __grid_cons
   __shared__ unsigned s_w[ITEMS * W];  // survivors per (row, warp), then their exclusive prefix
   __shared__ unsigned long long s_bcast;
   __shared__ long long s_tile[NS];
-  __shared__ __align__(8) uint64_t s_bar[NS];
+  __shared__ __align__(8) uint64_t s_bar[NS][2];  // [0]: the fields the conditions test (copied first), [1]: the other fields
   __shared__ Cond s_cond[PD_MAX_CONDITIONS];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
@@ -89,18 +89,30 @@ __global__ void __launch_bounds__(THREADS, 4) pd_filter_kernel(const __grid_cons
       const long long base = tile * PD_FILTER_TILE;
       Stage &st = stages[s];
       pdk::fence_async_smem();  // the stage was last read through the generic proxy
-      pdk::mbar_expect_tx(&s_bar[s], STAGE_BYTES);
-      pdk::bulk_g2s(st.pt, prm.pt + base, 4u * PD_FILTER_TILE, &s_bar[s]);
-      pdk::bulk_g2s(st.eta, prm.eta + base, 4u * PD_FILTER_TILE, &s_bar[s]);
-      pdk::bulk_g2s(st.phi, prm.phi + base, 4u * PD_FILTER_TILE, &s_bar[s]);
-      pdk::bulk_g2s(st.E, prm.E + base, 4u * PD_FILTER_TILE, &s_bar[s]);
-      pdk::bulk_g2s(st.src, prm.src + base, 4u * PD_FILTER_TILE, &s_bar[s]);
-      pdk::bulk_g2s(st.cls, prm.cls + base, 1u * PD_FILTER_TILE, &s_bar[s]);
+      // the fields the conditions test first, on a barrier of their own: the tile is counted (and its count published, which is
+      // what every later tile waits for) while the other fields are still on their way
+      const void *srcs[6] = {prm.pt + base, prm.eta + base, prm.phi + base, prm.E + base, prm.cls + base, prm.src + base};
+      void *dsts[6] = {st.pt, st.eta, st.phi, st.E, st.cls, st.src};
+      unsigned bytes0 = 0, bytes1 = 0;
+#pragma unroll
+      for (int f = 0; f < 6; ++f) {
+        const unsigned b = f == 4 ? 1u * PD_FILTER_TILE : 4u * PD_FILTER_TILE;
+        if ((prm.cond_fields >> f) & 1u) bytes0 += b;
+        else bytes1 += b;
+      }
+      pdk::mbar_expect_tx(&s_bar[s][0], bytes0);
+      pdk::mbar_expect_tx(&s_bar[s][1], bytes1);
+#pragma unroll
+      for (int f = 0; f < 6; ++f)
+        if ((prm.cond_fields >> f) & 1u) pdk::bulk_g2s(dsts[f], srcs[f], f == 4 ? 1u * PD_FILTER_TILE : 4u * PD_FILTER_TILE, &s_bar[s][0]);
+#pragma unroll
+      for (int f = 0; f < 6; ++f)
+        if (!((prm.cond_fields >> f) & 1u)) pdk::bulk_g2s(dsts[f], srcs[f], f == 4 ? 1u * PD_FILTER_TILE : 4u * PD_FILTER_TILE, &s_bar[s][1]);
     }
   };
   if (tid >= 32 && tid < 32 + prm.n_conds) make_cond(prm.conds[tid - 32], s_cond[tid - 32]);
   if (tid == 0) {
-    for (int s = 0; s < NS; ++s) pdk::mbar_init(&s_bar[s], 1);
+    for (int s = 0; s < NS; ++s) pdk::mbar_init(&s_bar[s][0], 1), pdk::mbar_init(&s_bar[s][1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     request(0);
   }
@@ -113,8 +125,7 @@ __global__ void __launch_bounds__(THREADS, 4) pd_filter_kernel(const __grid_cons
     const long long base = tile * PD_FILTER_TILE;
     Stage &st = stages[s];
     if (bulk(tile)) {
-      pdk::mbar_wait(&s_bar[s], (phase >> s) & 1u);
-      phase ^= 1u << s;
+      pdk::mbar_wait(&s_bar[s][0], (phase >> s) & 1u);
     } else {
       for (int i = tid; i < PD_FILTER_TILE; i += THREADS) {
         const long long p = base + i;
@@ -218,6 +229,10 @@ __global__ void __launch_bounds__(THREADS, 4) pd_filter_kernel(const __grid_cons
     }
     __syncthreads();
     const long long tile_excl = (long long)s_bcast;
+    if (bulk(tile)) {  // the other fields
+      pdk::mbar_wait(&s_bar[s][1], (phase >> s) & 1u);
+      phase ^= 1u << s;
+    }
     // ---- survivors to their final place; per 32 positions: the survivor bits and the rank of the first
 #pragma unroll
     for (int k = 0; k < ITEMS; ++k) {

@@ -242,6 +242,7 @@ struct PdFilterParams {
   unsigned long long *chain;      // workspace: look-back word per tile
   unsigned long long *wordrank;   // workspace, per 32 input positions (0..n): survivor bits | rank of the first << 32
   int aligned16;                  // all six input arrays start at a multiple of 16 bytes (bulk copies)
+  unsigned cond_fields;           // bit f: field f (PD_FIELD_*: pt, eta, phi, E, cls) is tested by a condition; bit 5 (src) never
 };
 int pd_launch_filter(const PdFilterParams &prm, void *stream);
 
