@@ -416,11 +416,8 @@ int pd_launch_features(const PdFeatParams &prm, void *stream) {
   if (epc > pdf::RUN_EVENTS) epc = pdf::RUN_EVENTS;
   const long long n_chunks = (prm.n_events + epc - 1) / epc;
   const long long grid = n_chunks < ctas ? n_chunks : ctas;
-  static bool configured = false;
-  if (!configured) {
-    if (cudaFuncSetAttribute(pdf::pd_features_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pdf::SMEM_BYTES) != cudaSuccess) return PD_ECUDA;
-    configured = true;
-  }
+  // per launch, not once per process: the attribute belongs to the current device's copy of the kernel
+  if (cudaFuncSetAttribute(pdf::pd_features_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pdf::SMEM_BYTES) != cudaSuccess) return PD_ECUDA;
   pdf::pd_features_kernel<<<(unsigned)grid, pdf::THREADS, pdf::SMEM_BYTES, (cudaStream_t)stream>>>(prm, (int)epc, n_chunks);
   return cudaGetLastError() == cudaSuccess ? PD_OK : PD_ECUDA;
 }
